@@ -1,0 +1,124 @@
+/*
+ * bfsc.h — C ABI of the B200 (sm_100a) BFS-frontier codec. The boundary of the product.
+ *
+ * Operation (arxiv 1704.00513 = /root/reference/PAPER.md): compress / decompress the BFS
+ * frontier traffic — sorted vertex-ID queues (§4.1.4) — before / after each of
+ * the two exchanges of a BFS level (Algorithm 4 lines 5-7 and 9-11, L1344-1379; call shape
+ * compress(buffer)->bytes, decompress(bytes)->buffer of Algorithm 5), with
+ * delta coding (L979-986) + frame-of-reference binary packing in blocks of 128 IDs with a
+ * per-block width b (eq. 6) + patched exceptions (L1000-1011),
+ * and a compression threshold below which a buffer is sent raw (§5.4.3).
+ * The byte layout is FORMAT.md (version 1). The batch calls take the (buffer, counts/displs)
+ * shape of the MPI ...V collectives the streams are sent with (L750-754); the size metadata
+ * (out_offsets) is handed back to the caller, who exchanges it first (L1790).
+ *
+ * Conventions
+ *  - Pointers named d_* are DEVICE pointers owned by the caller; h_* are HOST pointers.
+ *    The library allocates nothing, frees nothing and never synchronises (except the *_host
+ *    convenience calls, which synchronise `cuda_stream` before returning).
+ *  - Every call enqueues its kernels on `cuda_stream` (a cudaStream_t passed as void*;
+ *    NULL = the legacy default stream) and returns immediately.
+ *  - d_ids / d_out / d_in must be 16-byte aligned; element offsets inside a batch may be
+ *    arbitrary (unaligned buffers take a scalar load/store path).
+ *  - IDs are little-endian unsigned integers of W = 32 or 64 bits (bfsc_dtype).
+ *  - Return value: host-detectable errors only (null / misaligned pointer, bad dtype,
+ *    workspace too small, launch failure -> BFSC_ERR_CUDA).
+ *  - Data-dependent errors are written to *d_status (a device uint32, 0 = OK, first error
+ *    wins; the caller zero-initialises it or passes the same word through a sequence of
+ *    calls): BFSC_ERR_DST_TOO_SMALL (output / ids capacity exceeded: nothing is written
+ *    beyond capacity), BFSC_ERR_CORRUPT (decoder: anything FORMAT.md §4 rejects),
+ *    BFSC_ERR_INVALID_ARG (workspace too small for the block count found on the device,
+ *    non-monotone offsets). On error the output content is unspecified, but no out-of-bounds
+ *    access occurs. d_status may be NULL (errors are then dropped).
+ *  - raw_threshold_bytes: a buffer is sent RAW iff n*W/8 < raw_threshold_bytes
+ *    (FORMAT.md §1); 0 = always compress.
+ *  - Workspace: bfsc_workspace_bytes(n_ids_total, n_buf, t) bytes, 16-byte aligned, any
+ *    content on entry, clobbered by the call; one workspace per in-flight call.
+ *  - Compressed output is canonical: byte-identical to the scalar oracle (oracle/), pads
+ *    included. The decoder accepts any well-formed stream.
+ */
+#ifndef BFSC_H
+#define BFSC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BFSC_OK = 0,
+    BFSC_ERR_INVALID_ARG = 1,
+    BFSC_ERR_DST_TOO_SMALL = 2,
+    BFSC_ERR_CORRUPT = 3,
+    BFSC_ERR_CUDA = 4,
+    BFSC_ERR_UNSUPPORTED = 5
+} bfsc_status;
+
+typedef enum { BFSC_U32 = 32, BFSC_U64 = 64 } bfsc_dtype;
+
+/* library / format version: (format_version << 16) | abi_revision */
+uint32_t bfsc_version(void);
+
+/* Worst-case bytes of ONE stream of n_ids IDs, RAW or compressed (FORMAT.md §3). Host. */
+size_t bfsc_compress_bound(size_t n_ids, bfsc_dtype t);
+
+/* Sum of bfsc_compress_bound over a batch; h_counts = n_buf HOST element counts. */
+size_t bfsc_batch_compress_bound(const uint64_t* h_counts, size_t n_buf, bfsc_dtype t);
+
+/* Workspace bytes sufficient for any of the four device calls on a batch of n_buf buffers
+ * holding n_ids_total IDs in total (single-buffer calls: n_buf = 1). Host. */
+size_t bfsc_workspace_bytes(size_t n_ids_total, size_t n_buf, bfsc_dtype t);
+
+/* ONE buffer: d_ids[0..n_ids) -> one stream at d_out; *d_out_bytes (device) = its
+ * total_bytes. Steps E0-E5 of SURVEY.md §8(a). */
+bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
+                          void* d_out, size_t out_capacity, uint64_t* d_out_bytes,
+                          void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                          void* cuda_stream);
+
+/* ONE stream at d_in (in_bytes available, >= its total_bytes) -> d_ids[0..n); *d_n_ids
+ * (device) = n. Steps D0-D5. */
+bfsc_status bfsc_decompress(const void* d_in, size_t in_bytes, bfsc_dtype t,
+                            void* d_ids, size_t ids_capacity, uint64_t* d_n_ids,
+                            void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                            void* cuda_stream);
+
+/* n_buf buffers in one launch sequence. d_in_offsets: n_buf+1 non-decreasing ELEMENT
+ * offsets into d_ids (device). Streams are written back to back at d_out;
+ * d_out_offsets[0..n_buf] (device, written) are their BYTE offsets, [n_buf] = total. */
+bfsc_status bfsc_compress_batch(const void* d_ids, const uint64_t* d_in_offsets, size_t n_buf,
+                                bfsc_dtype t, size_t raw_threshold_bytes,
+                                void* d_out, size_t out_capacity, uint64_t* d_out_offsets,
+                                void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                void* cuda_stream);
+
+/* d_in_offsets: n_buf+1 BYTE offsets of the streams inside d_in (each a multiple of 16).
+ * IDs are written back to back at d_ids; d_id_offsets[0..n_buf] (device, written) are
+ * their ELEMENT offsets. */
+bfsc_status bfsc_decompress_batch(const void* d_in, const uint64_t* d_in_offsets, size_t n_buf,
+                                  bfsc_dtype t,
+                                  void* d_ids, size_t ids_capacity, uint64_t* d_id_offsets,
+                                  void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                  void* cuda_stream);
+
+/* End-to-end convenience calls with HOST buffers (pinned memory recommended): copy in,
+ * run the device call above, copy the result out, synchronise the stream. d_scratch is a
+ * caller-owned device buffer of at least bfsc_host_scratch_bytes(n_ids, t) bytes.
+ * *h_out_bytes / *h_n_ids and the returned status include data-dependent errors. */
+size_t bfsc_host_scratch_bytes(size_t n_ids, bfsc_dtype t);
+bfsc_status bfsc_compress_host(const void* h_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
+                               void* h_out, size_t out_capacity, uint64_t* h_out_bytes,
+                               void* d_scratch, size_t scratch_bytes, void* cuda_stream);
+bfsc_status bfsc_decompress_host(const void* h_in, size_t in_bytes, bfsc_dtype t,
+                                 void* h_ids, size_t ids_capacity, uint64_t* h_n_ids,
+                                 void* d_scratch, size_t scratch_bytes, void* cuda_stream);
+
+/* Number of kernels the library has launched in this process so far (bench bookkeeping). */
+uint64_t bfsc_kernel_launches(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

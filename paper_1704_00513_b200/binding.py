@@ -1,0 +1,174 @@
+"""Thin ctypes binding of libbfsc.so (include/bfsc.h). Argument marshalling only: every step
+of the path runs in the CUDA kernels. PyTorch supplies device memory and streams.
+
+There is NO CPU fallback: if libbfsc.so is missing or fails to load, `lib()` raises.
+Tensors carry the ID bit pattern: torch.int32/uint32 for W=32, torch.int64/uint64 for W=64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "libbfsc.so")
+_lib = None
+
+OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED = range(6)
+U32, U64 = 32, 64
+
+EXPORTS = [
+    "bfsc_version", "bfsc_compress_bound", "bfsc_batch_compress_bound", "bfsc_workspace_bytes",
+    "bfsc_compress", "bfsc_decompress", "bfsc_compress_batch", "bfsc_decompress_batch",
+    "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
+]
+
+
+class BfscError(RuntimeError):
+    def __init__(self, code, where=""):
+        super().__init__(f"bfsc error {code} {where}")
+        self.code = code
+
+
+def lib():
+    """Loads libbfsc.so (built by paper_1704_00513_b200.build / __graft_entry__.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(SO_PATH):
+            raise RuntimeError(f"{SO_PATH} not found: run `python -m paper_1704_00513_b200.build` "
+                               "(the CUDA extension is the only implementation; there is no fallback)")
+        L = ctypes.CDLL(SO_PATH)
+        c = ctypes
+        vp, sz, i32 = c.c_void_p, c.c_size_t, c.c_int
+        L.bfsc_version.restype = c.c_uint32
+        L.bfsc_kernel_launches.restype = c.c_uint64
+        L.bfsc_compress_bound.restype = sz
+        L.bfsc_compress_bound.argtypes = [sz, i32]
+        L.bfsc_batch_compress_bound.restype = sz
+        L.bfsc_batch_compress_bound.argtypes = [vp, sz, i32]
+        L.bfsc_workspace_bytes.restype = sz
+        L.bfsc_workspace_bytes.argtypes = [sz, sz, i32]
+        L.bfsc_host_scratch_bytes.restype = sz
+        L.bfsc_host_scratch_bytes.argtypes = [sz, i32]
+        L.bfsc_compress.restype = i32
+        L.bfsc_compress.argtypes = [vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_decompress.restype = i32
+        L.bfsc_decompress.argtypes = [vp, sz, i32, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_compress_batch.restype = i32
+        L.bfsc_compress_batch.argtypes = [vp, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_decompress_batch.restype = i32
+        L.bfsc_decompress_batch.argtypes = [vp, vp, sz, i32, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_compress_host.restype = i32
+        L.bfsc_compress_host.argtypes = [vp, sz, i32, sz, vp, sz, vp, vp, sz, vp]
+        L.bfsc_decompress_host.restype = i32
+        L.bfsc_decompress_host.argtypes = [vp, sz, i32, vp, sz, vp, vp, sz, vp]
+        _lib = L
+    return _lib
+
+
+def dtype_of(t: torch.Tensor) -> int:
+    if t.dtype in (torch.int32, torch.uint32):
+        return U32
+    if t.dtype in (torch.int64, torch.uint64):
+        return U64
+    raise TypeError(f"IDs must be 32- or 64-bit integers, got {t.dtype}")
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def compress_bound(n_ids: int, W: int) -> int:
+    return lib().bfsc_compress_bound(n_ids, W)
+
+
+def batch_compress_bound(counts, W: int) -> int:
+    arr = (ctypes.c_uint64 * len(counts))(*[int(c) for c in counts])
+    return lib().bfsc_batch_compress_bound(arr, len(counts), W)
+
+
+def workspace_bytes(n_ids_total: int, n_buf: int, W: int) -> int:
+    return lib().bfsc_workspace_bytes(n_ids_total, n_buf, W)
+
+
+def host_scratch_bytes(n_ids: int, W: int) -> int:
+    return lib().bfsc_host_scratch_bytes(n_ids, W)
+
+
+def kernel_launches() -> int:
+    return lib().bfsc_kernel_launches()
+
+
+def _check(rc, where):
+    if rc != OK:
+        raise BfscError(rc, where)
+
+
+def compress(d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_bytes, d_workspace, d_status):
+    """bfsc_compress: device tensors in, enqueue only (no sync). d_out: uint8; d_out_bytes:
+    int64[1]; d_status: int32[1] (zeroed by the caller)."""
+    _check(lib().bfsc_compress(_ptr(d_ids), n_ids, W, raw_threshold_bytes, _ptr(d_out), d_out.numel(),
+                               _ptr(d_out_bytes), _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
+                               ctypes.c_void_p(_stream())), "bfsc_compress")
+
+
+def decompress(d_in, in_bytes, W, d_ids, d_n_ids, d_workspace, d_status):
+    _check(lib().bfsc_decompress(_ptr(d_in), in_bytes, W, _ptr(d_ids), d_ids.numel(), _ptr(d_n_ids),
+                                 _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
+                                 ctypes.c_void_p(_stream())), "bfsc_decompress")
+
+
+def compress_batch(d_ids, d_in_offsets, n_buf, W, raw_threshold_bytes, d_out, d_out_offsets, d_workspace, d_status):
+    _check(lib().bfsc_compress_batch(_ptr(d_ids), _ptr(d_in_offsets), n_buf, W, raw_threshold_bytes, _ptr(d_out),
+                                     d_out.numel(), _ptr(d_out_offsets), _ptr(d_workspace), d_workspace.numel(),
+                                     _ptr(d_status), ctypes.c_void_p(_stream())), "bfsc_compress_batch")
+
+
+def decompress_batch(d_in, d_in_offsets, n_buf, W, d_ids, d_id_offsets, d_workspace, d_status):
+    _check(lib().bfsc_decompress_batch(_ptr(d_in), _ptr(d_in_offsets), n_buf, W, _ptr(d_ids), d_ids.numel(),
+                                       _ptr(d_id_offsets), _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
+                                       ctypes.c_void_p(_stream())), "bfsc_decompress_batch")
+
+
+def compress_host(h_ids, W, raw_threshold_bytes, h_out, d_scratch) -> int:
+    """bfsc_compress_host: (pinned) host tensors in/out; synchronises; returns stream bytes."""
+    nbytes = ctypes.c_uint64(0)
+    _check(lib().bfsc_compress_host(_ptr(h_ids), h_ids.numel(), W, raw_threshold_bytes, _ptr(h_out), h_out.numel(),
+                                    ctypes.byref(nbytes), _ptr(d_scratch), d_scratch.numel(),
+                                    ctypes.c_void_p(_stream())), "bfsc_compress_host")
+    return nbytes.value
+
+
+def decompress_host(h_in, in_bytes, W, h_ids, d_scratch) -> int:
+    n = ctypes.c_uint64(0)
+    _check(lib().bfsc_decompress_host(_ptr(h_in), in_bytes, W, _ptr(h_ids), h_ids.numel(), ctypes.byref(n),
+                                      _ptr(d_scratch), d_scratch.numel(), ctypes.c_void_p(_stream())),
+           "bfsc_decompress_host")
+    return n.value
+
+
+class Codec:
+    """Convenience holder of the device buffers one (batched) call needs. Still marshalling
+    only: sizes the buffers with the library's own bound functions and forwards."""
+
+    def __init__(self, max_ids: int, max_buf: int, W: int, device="cuda"):
+        self.W, self.max_ids, self.max_buf = W, max_ids, max_buf
+        dev = torch.device(device)
+        bound = max_buf * compress_bound(0, W) + compress_bound(max_ids, W) + 48 * max_buf
+        self.out = torch.empty(bound + 256, dtype=torch.uint8, device=dev)
+        self.ws = torch.empty(workspace_bytes(max_ids, max_buf, W), dtype=torch.uint8, device=dev)
+        self.out_off = torch.zeros(max_buf + 1, dtype=torch.int64, device=dev)
+        self.id_off = torch.zeros(max_buf + 1, dtype=torch.int64, device=dev)
+        self.status = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.ids = torch.empty(max_ids + 4, dtype=torch.int32 if W == 32 else torch.int64, device=dev)
+
+    def encode(self, d_ids, d_in_off, n_buf, thr):
+        compress_batch(d_ids, d_in_off, n_buf, self.W, thr, self.out, self.out_off, self.ws, self.status)
+
+    def decode(self, n_buf):
+        decompress_batch(self.out, self.out_off, n_buf, self.W, self.ids, self.id_off, self.ws, self.status)

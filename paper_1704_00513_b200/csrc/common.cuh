@@ -1,0 +1,160 @@
+// common.cuh — shared device/host helpers of the bfsc CUDA library (sm_100a only).
+// Product code: shares nothing with oracle/. Layout per FORMAT.md v1.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/bfsc.h"
+
+namespace bfsc {
+
+constexpr int kBlk = 128;               // IDs per block
+constexpr int kWarp = 32;
+constexpr uint32_t kFull = 0xffffffffu;
+constexpr int kNumSM = 148;             // B200
+
+// ---- workspace layout (device) -------------------------------------------------------
+// [WsHeader 256 B][blk_first u64 (n_buf+1)][fixed_prefix u64 (n_buf+1)][stream_start u64 (n_buf+1)]
+// [meta u32 (blk_cap+1)][bb16 u32 (blk_cap+1)][tile_state u64 (tile_cap)]
+struct WsHeader {
+    unsigned long long total_blocks;    // blocks of all PFOR streams of the batch
+    unsigned long long fixed_total;     // sum of per-stream fixed bytes (header+directory | header+raw)
+    unsigned long long total_out;       // encode: total output bytes; decode: total ids
+    unsigned int ok;                    // 1 = plan valid and capacity sufficient
+    unsigned int ticket;                // tile ticket counter (fused encode)
+    unsigned long long pad[28];
+};
+static_assert(sizeof(WsHeader) == 256, "WsHeader");
+
+struct WsView {
+    WsHeader* hdr;
+    unsigned long long* blk_first;      // n_buf+1 : first global block of each buffer
+    unsigned long long* fixed_prefix;   // n_buf+1 : exclusive prefix of fixed bytes
+    unsigned long long* stream_start;   // n_buf+1 : encode: 1 + byte offset of the stream (0 = not yet known)
+    uint32_t* meta;                     // blk_cap+1 : size16 | b<<8 | n_exc<<16
+    uint32_t* bb16;                     // blk_cap+1 : exclusive prefix of block sizes in 16-B units
+    unsigned long long* tile_state;     // tile_cap
+    size_t blk_cap;
+    size_t tile_cap;
+};
+
+constexpr int kTileBlocks = 32;         // blocks per look-back tile (fused encode)
+
+__host__ __device__ inline size_t align_up(size_t x, size_t k) { return (x + k - 1) / k * k; }
+
+__host__ inline size_t ws_blk_cap_for(size_t n_ids_total, size_t n_buf) { return n_ids_total / kBlk + n_buf + 1; }
+
+__host__ inline size_t ws_bytes_for(size_t n_ids_total, size_t n_buf) {
+    size_t blk_cap = ws_blk_cap_for(n_ids_total, n_buf);
+    size_t tile_cap = blk_cap / kTileBlocks + n_buf + 2;
+    return sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + 2 * align_up(4 * (blk_cap + 1), 16)
+           + align_up(8 * tile_cap, 16) + 4096;
+}
+
+// Carves the workspace; blk_cap is derived from the bytes actually provided.
+__host__ inline bool ws_carve(void* ws, size_t bytes, size_t n_buf, WsView* v) {
+    size_t fixed = sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + 64;
+    if (bytes < fixed + 64) return false;
+    size_t rest = bytes - fixed;
+    // per block: 8 B (meta + bb16) + 8/kTileBlocks B of tile state
+    if (rest < 128 + 8 * (n_buf + 2) + 1024) return false;
+    size_t blk_cap = (rest - 128 - 8 * (n_buf + 2)) * kTileBlocks / (8 * kTileBlocks + 8);
+    if (blk_cap < 2) return false;
+    blk_cap -= 1;
+    size_t tile_cap = blk_cap / kTileBlocks + n_buf + 2;
+    char* p = (char*)ws;
+    v->hdr = (WsHeader*)p; p += sizeof(WsHeader);
+    v->blk_first = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
+    v->fixed_prefix = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
+    v->stream_start = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
+    v->meta = (uint32_t*)p; p += align_up(4 * (blk_cap + 1), 16);
+    v->bb16 = (uint32_t*)p; p += align_up(4 * (blk_cap + 1), 16);
+    v->tile_state = (unsigned long long*)p; p += align_up(8 * tile_cap, 16);
+    v->blk_cap = blk_cap; v->tile_cap = tile_cap;
+    return (size_t)(p - (char*)ws) <= bytes;
+}
+
+// ---- device helpers ------------------------------------------------------------------
+__device__ __forceinline__ void set_status(uint32_t* st, uint32_t code) {
+    if (st) atomicCAS(st, 0u, code);
+}
+
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+// PTX shl/shr clamp shift amounts >= 32 (result 0); C++ << would be undefined there.
+__device__ __forceinline__ uint32_t shl32(uint32_t x, uint32_t s) {
+    uint32_t r; asm("shl.b32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(s)); return r;
+}
+__device__ __forceinline__ uint32_t shr32(uint32_t x, uint32_t s) {
+    uint32_t r; asm("shr.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(s)); return r;
+}
+__device__ __forceinline__ uint64_t shl64(uint64_t x, uint32_t s) {
+    uint64_t r; asm("shl.b64 %0, %1, %2;" : "=l"(r) : "l"(x), "r"(s)); return r;
+}
+__device__ __forceinline__ uint64_t shr64(uint64_t x, uint32_t s) {
+    uint64_t r; asm("shr.u64 %0, %1, %2;" : "=l"(r) : "l"(x), "r"(s)); return r;
+}
+__device__ __forceinline__ int width32(uint32_t v) { return 32 - __clz(v); }
+__device__ __forceinline__ int width64(uint64_t v) { return 64 - __clzll(v); }
+
+// bytes of the exception area: n ? align16(align_{W/8}(n) + n*W/8) : 0      (FORMAT.md §2)
+template <int W>
+__device__ __forceinline__ uint32_t exc_bytes(uint32_t n) {
+    constexpr uint32_t E = W / 8;
+    uint32_t a = ((n + E - 1) & ~(E - 1)) + n * E;
+    return n ? ((a + 15u) & ~15u) : 0u;
+}
+
+// first index i in [0, n_buf] with a[i] > g, minus 1  (buffers without blocks are skipped)
+__device__ __forceinline__ uint32_t find_buf(const unsigned long long* __restrict__ a, uint32_t n_buf,
+                                             unsigned long long g) {
+    uint32_t lo = 0, hi = n_buf;        // invariant: a[lo] <= g < a[hi]  (a[0] = 0, a[n_buf] = total > g)
+    while (hi - lo > 1) {
+        uint32_t mid = (lo + hi) >> 1;
+        if (a[mid] <= g) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// 1024-thread exclusive scan of two u64 values with running carry (plan kernels).
+struct Scan2 {
+    unsigned long long a, b;
+};
+__device__ inline Scan2 block_scan_excl2(Scan2 v, Scan2* total, Scan2* sm /* 33 entries */) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    Scan2 inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long ta = __shfl_up_sync(kFull, inc.a, o), tb = __shfl_up_sync(kFull, inc.b, o);
+        if (lane >= o) { inc.a += ta; inc.b += tb; }
+    }
+    if (lane == 31) sm[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        Scan2 w = lane < nw ? sm[lane] : Scan2{0, 0};
+        Scan2 wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long ta = __shfl_up_sync(kFull, wi.a, o), tb = __shfl_up_sync(kFull, wi.b, o);
+            if (lane >= o) { wi.a += ta; wi.b += tb; }
+        }
+        if (lane < nw) sm[lane] = Scan2{wi.a - w.a, wi.b - w.b};
+        if (lane == 31) sm[32] = wi;
+    }
+    __syncthreads();
+    Scan2 r{inc.a - v.a + sm[wid].a, inc.b - v.b + sm[wid].b};
+    *total = sm[32];
+    __syncthreads();
+    return r;
+}
+
+extern unsigned long long g_launches;   // host-side launch counter (api.cu)
+
+}  // namespace bfsc
+
+#define BFSC_LAUNCH_CHECK()                                        \
+    do {                                                           \
+        ::bfsc::g_launches++;                                      \
+        if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; } \
+    } while (0)

@@ -1,0 +1,226 @@
+"""GPU parity: CUDA path (through the C ABI) vs the oracle, on the same seeded inputs.
+Bar: compressed bytes memcmp-equal (headers, directory, pads), offsets equal, decoded IDs
+equal to the input (integer work: bit-exact)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1704_00513_b200.workloads import rmat, streams
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1704_00513_b200 import build, binding
+    build.build()
+    assert torch.cuda.is_available()
+    binding.lib()
+    return binding
+
+
+def _np(t, W):
+    a = t.cpu().numpy()
+    return a.view(np.uint32) if W == 32 else a.view(np.uint64)
+
+
+def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True):
+    """ids_t: CPU tensor (int32/int64 bit pattern), off_t: int64 offsets. Returns GPU bytes."""
+    dev = torch.device("cuda")
+    n, n_buf = ids_t.numel(), off_t.numel() - 1
+    counts = (off_t[1:] - off_t[:-1]).tolist()
+    cap = B.batch_compress_bound(counts, W)
+    d_ids = torch.empty(n + 4, dtype=ids_t.dtype, device=dev)
+    d_ids[:n] = ids_t.to(dev)
+    d_off = off_t.to(dev)
+    out = torch.full((cap + 64,), 0xAB, dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress_batch(d_ids, d_off, n_buf, W, thr, out, out_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    total = int(out_off[-1].item())
+    assert total <= cap
+    assert bool((out[cap:] == 0xAB).all()), "wrote beyond capacity"
+    gpu_bytes = out[:total].cpu().numpy()
+    gpu_off = out_off.cpu().numpy().astype(np.uint64)
+    if check_oracle:
+        ref, ref_off = oracle_mod.compress_batch(_np(ids_t, W), off_t.numpy().astype(np.uint64), thr, threads=8)
+        assert np.array_equal(gpu_off, ref_off)
+        if not np.array_equal(gpu_bytes, ref):
+            bad = int(np.nonzero(gpu_bytes != ref)[0][0])
+            raise AssertionError(f"compressed bytes differ at {bad} of {len(ref)}")
+    # decode on the GPU
+    back = torch.full((n + 4,), -1, dtype=ids_t.dtype, device=dev)
+    id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    status.zero_()
+    B.decompress_batch(out, out_off, n_buf, W, back, id_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    assert torch.equal(id_off.cpu(), off_t)
+    assert torch.equal(back[:n].cpu(), ids_t)
+    assert bool((back[n:] == -1).all())
+    return gpu_bytes, gpu_off
+
+
+def run_single(B, oracle_mod, ids_t, W, thr):
+    dev = torch.device("cuda")
+    n = ids_t.numel()
+    cap = B.compress_bound(n, W)
+    d_ids = ids_t.to(dev) if n else torch.empty(4, dtype=ids_t.dtype, device=dev)
+    out = torch.empty(cap, dtype=torch.uint8, device=dev)
+    nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress(d_ids, n, W, thr, out, nbytes, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    total = int(nbytes.item())
+    ref = oracle_mod.compress(_np(ids_t, W), thr)
+    assert total == len(ref)
+    assert np.array_equal(out[:total].cpu().numpy(), ref)
+    back = torch.empty(max(n, 4), dtype=ids_t.dtype, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+    B.decompress(out, total, W, back, n_out, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and int(n_out.item()) == n
+    assert torch.equal(back[:n].cpu(), ids_t)
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_single_edge_sizes(B, oracle_mod, W):
+    for n in (0, 1, 2, 127, 128, 129, 255, 256, 257, 1000, 4097, 128 * 300 + 5):
+        for mean in (1.0, 2.0, 256.0):
+            t = streams.gap_stream(n, mean, seed=11, W=W)
+            run_single(B, oracle_mod, t, W, 0)
+    run_single(B, oracle_mod, streams.gap_stream(100, 2.0, seed=1, W=W), W, 1024)   # RAW
+    run_single(B, oracle_mod, streams.gap_stream(300, 2.0, seed=1, W=W), W, 1024)
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_adversarial_values(B, oracle_mod, W):
+    rng = np.random.default_rng(W)
+    n = 128 * 40 + 77
+    dt = np.uint32 if W == 32 else np.uint64
+    tdt = torch.int32 if W == 32 else torch.int64
+    cases = {
+        "random_full_width": rng.integers(0, 1 << W, size=n, dtype=np.uint64, endpoint=False).astype(dt),
+        "alt_extremes": np.where(np.arange(n) % 2 == 0, 0, (1 << W) - 1).astype(dt),
+        "all_equal": np.full(n, 12345, dtype=dt),
+        "max": np.full(n, (1 << W) - 1, dtype=dt),
+        "wrap": ((np.uint64((1 << W) - 50) + np.arange(n, dtype=np.uint64)) & np.uint64((1 << W) - 1)).astype(dt),
+    }
+    for bits in (1, 3, 5, 7, 8, 9, 13, 16, 17, 24, 31, 32, 33, 40, 47, 63, 64):
+        if bits > W:
+            continue
+        g = rng.integers(0, 1 << min(bits, 63), size=n, dtype=np.uint64)
+        if bits == 64:
+            g = g * np.uint64(2) + rng.integers(0, 2, size=n, dtype=np.uint64)
+        cases[f"gaps_{bits}b"] = (np.cumsum(g) & np.uint64((1 << W) - 1)).astype(dt)
+        # heavy tail: mostly small gaps plus a few of `bits` bits
+        h = rng.integers(0, 4, size=n, dtype=np.uint64)
+        idx = rng.integers(0, n, size=n // 50)
+        h[idx] = g[idx]
+        cases[f"tail_{bits}b"] = (np.cumsum(h) & np.uint64((1 << W) - 1)).astype(dt)
+    for name, arr in cases.items():
+        t = torch.from_numpy(arr.view(np.int32 if W == 32 else np.int64).copy()).to(tdt)
+        off = torch.tensor([0, n], dtype=torch.int64)
+        try:
+            run_batch(B, oracle_mod, t, off, W, 0)
+        except AssertionError as e:
+            raise AssertionError(f"{name}: {e}")
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_batch_ragged(B, oracle_mod, W):
+    counts = streams.log_uniform_counts(300, 6, 14, W, seed=5)
+    counts[0] = 0
+    counts[5] = 0
+    counts[6] = 1
+    counts[7] = 128
+    counts[8] = 129
+    counts[299] = 0
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=W)
+    for thr in (0, 1024):
+        run_batch(B, oracle_mod, ids, off, W, thr)
+    # unaligned buffer starts (odd element offsets) exercise the scalar load/store path
+    ids2, off2 = streams.batch_of_streams(torch.tensor([3, 130, 257, 1, 1000]), 2.0, seed=6, W=W)
+    run_batch(B, oracle_mod, ids2, off2, W, 0)
+
+
+def test_tiny_rmat_config1(B, oracle_mod):
+    """BASELINE config 1: scale 12, 8 roots, 4 buffers by v mod 4, threshold 0, single + batch API."""
+    G = rmat.Graph(12, 16, seed=1)
+    for root in G.roots(8, seed=1):
+        for f in G.bfs_frontiers(root):
+            vals, off = streams.split_mod(f, 4)
+            ids = streams.as_ids(vals, 32)
+            run_batch(B, oracle_mod, ids, off, 32, 0)
+            for q in range(4):
+                run_single(B, oracle_mod, ids[int(off[q]):int(off[q + 1])].clone(), 32, 0)
+
+
+def test_streams_config2_reduced(B, oracle_mod):
+    """config 2 recipes at 2^18 IDs (several thousand blocks, oracle in seconds)."""
+    n = (1 << 18) + 37
+    for mean, outl in ((2.0, 0.0), (256.0, 0.0), (256.0, 0.01)):
+        for W in (32, 64):
+            t = streams.gap_stream(n, mean, seed=2, W=W, outlier_frac=outl)
+            run_batch(B, oracle_mod, t, torch.tensor([0, n], dtype=torch.int64), W, 0)
+
+
+def test_errors_reported_on_device(B):
+    dev = torch.device("cuda")
+    t = streams.gap_stream(5000, 16.0, seed=3, W=32).to(dev)
+    ws = torch.empty(B.workspace_bytes(5000, 1, 32), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
+    small = torch.full((256 + 64,), 0xCD, dtype=torch.uint8, device=dev)
+    B.lib().bfsc_compress(t.data_ptr(), 5000, 32, 0, small.data_ptr(), 256, nbytes.data_ptr(), ws.data_ptr(),
+                          ws.numel(), status.data_ptr(), None)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_DST_TOO_SMALL
+    assert bool((small[256:] == 0xCD).all())
+    # corrupt stream -> BFSC_ERR_CORRUPT, no crash
+    out = torch.empty(B.compress_bound(5000, 32), dtype=torch.uint8, device=dev)
+    status.zero_()
+    B.compress(t, 5000, 32, 0, out, nbytes, ws, status)
+    torch.cuda.synchronize()
+    total = int(nbytes.item())
+    back = torch.empty(5000, dtype=torch.int32, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+    for pos, val in ((0, 0x41), (5, 64), (36, 0)):
+        bad = out.clone()
+        bad[pos] = val
+        status.zero_()
+        B.decompress(bad, total, 32, back, n_out, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == B.ERR_CORRUPT, pos
+    first_blk = 16 * int(out[32:36].cpu().numpy().view(np.uint32)[0])
+    bad = out.clone()
+    bad[first_blk + 8] = 33
+    status.zero_()
+    B.decompress(bad, total, 32, back, n_out, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_CORRUPT
+    # ids capacity too small
+    status.zero_()
+    B.decompress(out, total, 32, back[:100], n_out, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_DST_TOO_SMALL
+
+
+def test_host_api_roundtrip(B, oracle_mod):
+    dev = torch.device("cuda")
+    for W in (32, 64):
+        n = 50_000
+        t = streams.gap_stream(n, 16.0, seed=4, W=W).pin_memory()
+        scratch = torch.empty(B.host_scratch_bytes(n, W) + 256, dtype=torch.uint8, device=dev)
+        h_out = torch.empty(B.compress_bound(n, W), dtype=torch.uint8).pin_memory()
+        nbytes = B.compress_host(t, W, 0, h_out, scratch)
+        ref = oracle_mod.compress(_np(t, W), 0)
+        assert nbytes == len(ref) and np.array_equal(h_out[:nbytes].numpy(), ref)
+        h_back = torch.empty(n, dtype=t.dtype).pin_memory()
+        assert B.decompress_host(h_out, nbytes, W, h_back, scratch) == n
+        assert torch.equal(h_back, t)
