@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the bfsc hot path (BASELINE.json metric:
+"encode/decode GB/s and % of HBM peak on 1 B200; compression ratio").
+
+Workload (config.workload): BASELINE.json configs[1] — three synthetic sorted u32 streams of
+2^24 IDs, seed 2: (a) geometric gaps mean 2, (b) mean 256, (c) mean 256 with 1 % of the gaps
+replaced by U[2^16, 2^24). One STEP = one pass of the whole hot path over that batch:
+bfsc_compress of a, b, c then bfsc_decompress of a, b, c (E0-E5, D0-D5 of SURVEY.md §8(a)).
+value = (raw bytes encoded + raw bytes decoded) / time, inputs resident in HBM.
+e2e   = the same through bfsc_compress_host / bfsc_decompress_host with pinned HOST buffers.
+roofline = algorithmic bytes (raw + compressed) of the dominant call / its CUDA-event duration
+           measured inside the timed region, against MEASURED_PEAKS.json hbm_gbs.
+cpu_baseline = the oracle (oracle/, as it stands) on the host cores on the same workload.
+`--impl reference` times the oracle alone (this tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+
+from paper_1704_00513_b200.workloads import streams  # noqa: E402
+
+LOG2_N = 24
+STREAMS = [("a_mean2", 2.0, 0.0), ("b_mean256", 256.0, 0.0), ("c_mean256_out1pct", 256.0, 0.01)]
+SEED = 2
+W = 32
+METRIC = "codec_throughput_encode_plus_decode"
+UNIT = "GB/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].startswith("Active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def make_streams(device, n):
+    return [streams.gap_stream(n, mean, seed=SEED, W=W, outlier_frac=outl, sub=i, device=device)
+            for i, (_, mean, outl) in enumerate(STREAMS)]
+
+
+def np_view(t):
+    return t.cpu().numpy().view(np.uint32 if W == 32 else np.uint64)
+
+
+# --------------------------------------------------------------------------- oracle arm
+def time_oracle(host_ids, threads, reps=1):
+    """oracle encode+decode of every stream; returns (seconds, raw_bytes_processed, ratio)."""
+    import oracle
+    oracle.build()
+    best = None
+    raw = comp = 0
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        raw = comp = 0
+        for a in host_ids:
+            off = np.array([0, len(a)], dtype=np.uint64)
+            s, so = oracle.compress_batch(a, off, 0, threads=threads)
+            y, _ = oracle.decompress_batch(s, so, W, len(a), threads=threads)
+            raw += 2 * a.nbytes
+            comp += len(s)
+            assert y[0] == a[0] and y[-1] == a[-1]
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return best, raw, (raw / 2) / comp
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    cores = len(os.sched_getaffinity(0))
+    n = 1 << 22                                            # bounded sample: first 2^22 IDs of each stream
+    host = [np_view(t) for t in make_streams("cpu", n)]
+    for _ in range(max(args.warmup, 0) and 1):
+        time_oracle([h[:1 << 16] for h in host], cores)
+    times = []
+    raw = ratio = 0
+    for _ in range(args.steps):
+        dt, raw, ratio = time_oracle(host, cores)
+        times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    val = raw / (ms * 1e-3) / 1e9
+    sample = f"first 2^22 of the 2^24 IDs of each of the 3 streams, encode+decode, {cores} threads"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic", "ratio": ratio,
+        "config": {"workload": "configs[1]: 3 sorted u32 streams (a,b,c), seed 2; oracle on a bounded sample", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# --------------------------------------------------------------------------- CUDA arm
+def run_ours(args, rank, local_rank, world):
+    from paper_1704_00513_b200 import binding as B
+    from paper_1704_00513_b200 import build as cuda_build
+    if rank == 0:
+        cuda_build.build()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    B.lib()
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    n = 1 << args.log2n
+    ids = make_streams(dev, n)
+    S = len(ids)
+    cap = B.compress_bound(n, W)
+    outs = [torch.empty(cap, dtype=torch.uint8, device=dev) for _ in range(S)]
+    nbytes = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(S)]
+    backs = [torch.empty(n, dtype=ids[0].dtype, device=dev) for _ in range(S)]
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    raw_bytes = n * (W // 8)
+
+    def step(ev=None):
+        for s in range(S):
+            if ev is not None:
+                ev[0][s][0].record()
+            B.compress(ids[s], n, W, 0, outs[s], nbytes[s], ws, status)
+            if ev is not None:
+                ev[0][s][1].record()
+        for s in range(S):
+            if ev is not None:
+                ev[1][s][0].record()
+            B.decompress(outs[s], cap, W, backs[s], n_out, ws, status)
+            if ev is not None:
+                ev[1][s][1].record()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0, f"device status {int(status.item())}"
+    comp = [int(x.item()) for x in nbytes]
+    for s in range(S):                                       # untimed sanity: decode == input
+        assert torch.equal(backs[s], ids[s]), "decode != input"
+
+    mk = lambda: torch.cuda.Event(enable_timing=True)       # noqa: E731
+    evs = [[[[mk(), mk()] for _ in range(S)] for _ in range(2)] for _ in range(args.steps)]
+    t0, t1 = mk(), mk()
+    launches0 = B.kernel_launches()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0.record()
+    for k in range(args.steps):
+        step(evs[k])
+    t1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    launches = B.kernel_launches() - launches0
+    ms_total = t0.elapsed_time(t1)
+    if world > 1:
+        tt = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    enc_ms = [float(np.mean([evs[k][0][s][0].elapsed_time(evs[k][0][s][1]) for k in range(args.steps)])) for s in range(S)]
+    dec_ms = [float(np.mean([evs[k][1][s][0].elapsed_time(evs[k][1][s][1]) for k in range(args.steps)])) for s in range(S)]
+    value = world * (2 * S * raw_bytes) / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end through the host-buffer C-ABI calls (pinned host memory) ----
+    e2e = None
+    if not args.no_e2e:
+        h_ids = [t.cpu().pin_memory() for t in ids]
+        h_out = [torch.empty(cap, dtype=torch.uint8).pin_memory() for _ in range(S)]
+        h_back = torch.empty(n, dtype=ids[0].dtype).pin_memory()
+        scratch = torch.empty(B.host_scratch_bytes(n, W) + 256, dtype=torch.uint8, device=dev)
+        e_steps = max(1, min(args.steps, 5))
+
+        def e2e_step():
+            hb = 0
+            for s in range(S):
+                hb = B.compress_host(h_ids[s], W, 0, h_out[s], scratch)
+            for s in range(S):
+                B.decompress_host(h_out[s], comp[s], W, h_back, scratch)
+            return hb
+
+        e2e_step()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        w0 = time.perf_counter()
+        for _ in range(e_steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        e_ms = 1e3 * (time.perf_counter() - w0) / e_steps
+        if world > 1:
+            tt = torch.tensor([e_ms], device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e_ms = float(tt.item())
+        assert torch.equal(h_back, h_ids[S - 1])
+        e2e = {"value": world * (2 * S * raw_bytes) / (e_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": e_ms,
+               "h2d_bytes_per_step": S * raw_bytes + sum(comp), "d2h_bytes_per_step": sum(comp) + S * raw_bytes + 32 * S,
+               "api": "bfsc_compress_host + bfsc_decompress_host, pinned host buffers"}
+
+    if rank != 0:
+        return
+    peak, peak_src = peaks()
+    per = {}
+    for s, (name, _, _) in enumerate(STREAMS):
+        alg = raw_bytes + comp[s] + 8
+        per[name] = {"ratio": raw_bytes / comp[s], "bits_per_id": 8 * comp[s] / n,
+                     "encode_ms": enc_ms[s], "decode_ms": dec_ms[s],
+                     "encode_GBps_in": raw_bytes / enc_ms[s] / 1e6, "decode_GBps_out": raw_bytes / dec_ms[s] / 1e6,
+                     "encode_alg_GBps": alg / enc_ms[s] / 1e6, "decode_alg_GBps": alg / dec_ms[s] / 1e6,
+                     "encode_frac_of_peak": alg / enc_ms[s] / 1e6 / peak, "decode_frac_of_peak": alg / dec_ms[s] / 1e6 / peak,
+                     "encode_frac_of_8TBps": alg / enc_ms[s] / 1e6 / 8000.0, "decode_frac_of_8TBps": alg / dec_ms[s] / 1e6 / 8000.0}
+    # dominant call = encode of stream (a): most raw bytes per compressed byte, the headline dense frontier
+    dom = STREAMS[0][0]
+    alg_a = raw_bytes + comp[0] + 8
+    roof = {"bound": "hbm", "kernel": "bfsc_compress call on stream a (all its launches)", "achieved": per[dom]["encode_alg_GBps"],
+            "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": per[dom]["encode_alg_GBps"] / peak,
+            "algorithmic_bytes_per_launch": alg_a, "traffic": None,
+            "decode": {"achieved": per[dom]["decode_alg_GBps"], "frac": per[dom]["decode_alg_GBps"] / peak}}
+    cpu = None
+    if not args.no_cpu:
+        cores = len(os.sched_getaffinity(0))
+        m = 1 << min(args.log2n, 22)
+        host = [np_view(t[:m]) for t in ids]
+        dt, raw, _ = time_oracle(host, cores)
+        cpu = {"value": raw / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first 2^{min(args.log2n, 22)} IDs of each of the 3 streams, encode+decode, {cores} threads, 1 pass"}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
+        "data": "synthetic",
+        "config": {"workload": f"configs[1]: 3 sorted u32 streams of 2^{args.log2n} IDs (a: geometric gaps mean 2, b: mean 256, "
+                               "c: mean 256 + 1% outliers in [2^16,2^24)), seed 2; step = compress a,b,c then decompress a,b,c",
+                   "raw_threshold_bytes": 0, "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2_policy": "inputs larger than L2: >=170 MB of other streams' traffic between any write and its re-read"},
+        "ratio": {k: v["ratio"] for k, v in per.items()},
+        "encode_GBps_in": S * raw_bytes / sum(enc_ms) / 1e6, "decode_GBps_out": S * raw_bytes / sum(dec_ms) / 1e6,
+        "per_stream": per, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--log2n", type=int, default=LOG2_N, help="IDs per stream = 2^log2n (default: the BASELINE size)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    run_ours(args, rank, local_rank, world)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -124,28 +124,29 @@ struct EncStage {
 
 // Assemble block (base, b, n_exc, deltas d[4] per lane) into st.out; returns its byte count.
 template <int W>
-__device__ __forceinline__ uint32_t pack_block(EncStage<W>& st, const typename IdT<W>::T d[4],
-                                               typename IdT<W>::T base, uint32_t b, uint32_t n_exc) {
+__device__ __forceinline__ uint32_t pack_block_to(typename IdT<W>::T* __restrict__ vals, unsigned char* __restrict__ out,
+                                                  const typename IdT<W>::T d[4], typename IdT<W>::T base,
+                                                  uint32_t b, uint32_t n_exc) {
     using T = typename IdT<W>::T;
     const int lane = lane_id();
-    uint32_t* out32 = reinterpret_cast<uint32_t*>(st.out);
+    uint32_t* out32 = reinterpret_cast<uint32_t*>(out);
     if (lane == 0) {
-        reinterpret_cast<unsigned long long*>(st.out)[0] = (unsigned long long)base;
-        reinterpret_cast<unsigned long long*>(st.out)[1] = (unsigned long long)(b | (n_exc << 8));
+        reinterpret_cast<unsigned long long*>(out)[0] = (unsigned long long)base;
+        reinterpret_cast<unsigned long long*>(out)[1] = (unsigned long long)(b | (n_exc << 8));
     }
     const uint32_t eb = exc_bytes<W>(n_exc);
     const uint32_t total = 16u + 16u * b + eb;
     if (b > 0) {
         T mask = (b >= (uint32_t)W) ? ~(T)0 : (((T)1 << b) - 1);
         if constexpr (W == 32) {
-            reinterpret_cast<uint4*>(st.vals)[lane] = make_uint4(d[0] & mask, d[1] & mask, d[2] & mask, d[3] & mask);
+            reinterpret_cast<uint4*>(vals)[lane] = make_uint4(d[0] & mask, d[1] & mask, d[2] & mask, d[3] & mask);
         } else {
-            reinterpret_cast<ulonglong2*>(st.vals)[2 * lane] = make_ulonglong2(d[0] & mask, d[1] & mask);
-            reinterpret_cast<ulonglong2*>(st.vals)[2 * lane + 1] = make_ulonglong2(d[2] & mask, d[3] & mask);
+            reinterpret_cast<ulonglong2*>(vals)[2 * lane] = make_ulonglong2(d[0] & mask, d[1] & mask);
+            reinterpret_cast<ulonglong2*>(vals)[2 * lane + 1] = make_ulonglong2(d[2] & mask, d[3] & mask);
         }
     }
     if (n_exc > 0) {                                // zero the exception area (pads must be 0)
-        uint4* z = reinterpret_cast<uint4*>(st.out + 16 + 16 * b);
+        uint4* z = reinterpret_cast<uint4*>(out + 16 + 16 * b);
         for (uint32_t i = lane; i < eb / 16; i += 32) z[i] = make_uint4(0, 0, 0, 0);
     }
     __syncwarp();
@@ -157,7 +158,7 @@ __device__ __forceinline__ uint32_t pack_block(EncStage<W>& st, const typename I
         const uint32_t r_hi = min(31u, div_small(32u * k + 31u, b));
         uint32_t word = 0;
         for (uint32_t r = r_lo; r <= r_hi; r++) {
-            const T val = st.vals[4 * r + c];
+            const T val = vals[4 * r + c];
             const int pos = (int)(r * b) - (int)(32u * k);
             if constexpr (W == 32) word |= (pos >= 0) ? (val << pos) : (val >> (-pos));
             else word |= (pos >= 0) ? (uint32_t)(val << pos) : (uint32_t)shr64(val, (uint32_t)(-pos));
@@ -165,7 +166,7 @@ __device__ __forceinline__ uint32_t pack_block(EncStage<W>& st, const typename I
         out32[4 + o] = word;
     }
     if (n_exc > 0) {                                // exceptions: ascending position = (row, column) order
-        unsigned char* e = st.out + 16 + 16 * b;
+        unsigned char* e = out + 16 + 16 * b;
         constexpr uint32_t E = W / 8;
         T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
         bool f[4];
@@ -187,6 +188,12 @@ __device__ __forceinline__ uint32_t pack_block(EncStage<W>& st, const typename I
     }
     __syncwarp();
     return total;
+}
+
+template <int W>
+__device__ __forceinline__ uint32_t pack_block(EncStage<W>& st, const typename IdT<W>::T d[4],
+                                               typename IdT<W>::T base, uint32_t b, uint32_t n_exc) {
+    return pack_block_to<W>(st.vals, st.out, d, base, b, n_exc);
 }
 
 // Copy an assembled block to global memory (dst 16-byte aligned) with 128-bit stores.

@@ -23,7 +23,8 @@ struct WsHeader {
     unsigned long long total_out;       // encode: total output bytes; decode: total ids
     unsigned int ok;                    // 1 = plan valid and capacity sufficient
     unsigned int ticket;                // tile ticket counter (fused encode)
-    unsigned long long pad[28];
+    unsigned long long grand16;         // encode: sum of all block sizes in 16-B units (written by the last tile)
+    unsigned long long pad[27];
 };
 static_assert(sizeof(WsHeader) == 256, "WsHeader");
 
@@ -39,7 +40,7 @@ struct WsView {
     size_t tile_cap;
 };
 
-constexpr int kTileBlocks = 32;         // blocks per look-back tile (fused encode)
+constexpr int kTileBlocks = 16;         // smallest look-back tile (u64: 16 blocks, u32: 32) — sizes tile_state
 
 __host__ __device__ inline size_t align_up(size_t x, size_t k) { return (x + k - 1) / k * k; }
 
