@@ -60,7 +60,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -180,6 +180,8 @@ def run_ours(args, rank, local_rank, world):
             if ev is not None:
                 ev[1][s][1].record()
 
+    sampler = ClockSampler(local_rank)
+    sampler.start()
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
@@ -192,8 +194,10 @@ def run_ours(args, rank, local_rank, world):
     evs = [[[[mk(), mk()] for _ in range(S)] for _ in range(2)] for _ in range(args.steps)]
     t0, t1 = mk(), mk()
     launches0 = B.kernel_launches()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
+    t_wait = time.time()
+    while not sampler.rows and time.time() - t_wait < 3.0:   # nvidia-smi needs a moment to start streaming
+        time.sleep(0.05)
+    sampler.rows.clear()
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
@@ -297,7 +301,7 @@ def run_ours(args, rank, local_rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--log2n", type=int, default=LOG2_N, help="IDs per stream = 2^log2n (default: the BASELINE size)")

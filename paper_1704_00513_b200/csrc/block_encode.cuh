@@ -47,6 +47,29 @@ __device__ __forceinline__ void load_rows(const typename IdT<W>::T* __restrict__
     }
 }
 
+// Same as load_rows, but with the default (evict-normal) cache policy: used by the first pass over a
+// tile, whose second pass re-reads the data from L2.
+template <int W>
+__device__ __forceinline__ void load_rows_keep(const typename IdT<W>::T* __restrict__ x, int m,
+                                               typename IdT<W>::T v[4]) {
+    using T = typename IdT<W>::T;
+    const int lane = lane_id();
+    const bool vec_ok = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
+    if (vec_ok) {
+        if constexpr (W == 32) {
+            uint4 q = __ldg(reinterpret_cast<const uint4*>(x) + lane);
+            v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+        } else {
+            const ulonglong2* p = reinterpret_cast<const ulonglong2*>(x) + 2 * lane;
+            ulonglong2 a = __ldg(p), b = __ldg(p + 1);
+            v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < 4; c++) v[c] = (4 * lane + c < m) ? x[4 * lane + c] : (T)0;
+    }
+}
+
 // d[c] = delta of ID 4*lane+c (d_0 = 0, zero beyond m). Returns base = first ID (all lanes).
 template <int W>
 __device__ __forceinline__ typename IdT<W>::T deltas(const typename IdT<W>::T v[4], int m,

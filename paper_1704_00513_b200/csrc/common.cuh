@@ -40,7 +40,7 @@ struct WsView {
     size_t tile_cap;
 };
 
-constexpr int kTileBlocks = 16;         // smallest look-back tile (u64: 16 blocks, u32: 32) — sizes tile_state
+constexpr int kTileBlocks = 2;          // smallest look-back tile (one warp: u64 2 blocks, u32 4) — sizes tile_state
 
 __host__ __device__ inline size_t align_up(size_t x, size_t k) { return (x + k - 1) / k * k; }
 

@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     __shared__ Scan2 sm[33];
     __shared__ int bad;
     constexpr unsigned long long E = W / 8;
-    constexpr unsigned long long kTile = (W == 32) ? 32 : 16;   // = 8 * FusedCfg<W>::kBpw
+    constexpr unsigned long long kTile = 256;                   // = kTileR of the fused kernel
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
     Scan2 carry{0, 0};
@@ -75,20 +75,20 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     }
 }
 
-// ---- E1-E4 fused: one pass over the input ------------------------------------------------
-// Persistent CTAs pull tiles of kBpw*8 consecutive blocks by ticket. 8 worker warps each own
-// kBpw blocks (warp = block); a 9th warp owns the bookkeeping: block -> buffer mapping, the
-// intra-tile scan of block sizes and the decoupled look-back that turns it into the device-wide
-// exclusive scan (E3) while the workers already pack into shared memory.
+// ---- E1-E4 fused: one pass over HBM -----------------------------------------------------
+// A CTA pulls tiles of kTileR consecutive blocks (128 KB of u32 IDs) by ticket.
+//   pass A  (E1+E2): every warp takes blocks of the tile (warp = block), computes deltas, widths
+//           and the canonical b; the block's size goes to shared memory.
+//   scan    (E3): intra-tile exclusive scan of the sizes, tile aggregate published, decoupled
+//           look-back over the (few hundred) tiles in flight -> device-wide exclusive scan.
+//   pass B  (E1+E4): the same blocks are read again — they are still in the 126 MB L2, so HBM is
+//           read once — deltas recomputed, packed in shared memory and stored with 128-bit
+//           coalesced stores at their final offsets, with their directory entries.
+// Large tiles keep the look-back shallow (tiles in flight = resident CTAs) and need no
+// on-chip copy of the tile between the passes.
 template <int W> struct FusedCfg { static constexpr int kBpw = (W == 32) ? 4 : 2; };
-
-struct BlkMeta {
-    unsigned long long xoff;     // element offset of the block's first ID in ids
-    unsigned long long first;    // first global block of its buffer
-    unsigned long long f0, f1;   // fixed_prefix[i], fixed_prefix[i+1]
-    uint32_t i;                  // buffer
-    int m;                       // valid IDs (0 = no such block)
-};
+constexpr int kEncWarps = 8;             // warps per CTA
+constexpr int kTileR = 256;              // blocks per tile (= threads per CTA)
 
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPre = 2ull << 62, kValMask = (1ull << 62) - 1;
 
@@ -102,155 +102,282 @@ __device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned 
 }
 
 template <int W>
-__global__ void __launch_bounds__(288) k_enc_fused(EncArgs a) {
+struct WarpStage {
+    static constexpr int kBpw = FusedCfg<W>::kBpw;
+    alignas(16) typename IdT<W>::T vals[kBpw][kBlk];                       // masked low parts, row-major
+    alignas(16) unsigned char out[kBpw][16 + 16 * W];                     // assembled blocks (canonical size <= 16+16W)
+};
+
+// header + masked values + exception list of one block into shared memory (no payload yet)
+template <int W>
+__device__ __forceinline__ void stage_block(typename IdT<W>::T* __restrict__ vals, unsigned char* __restrict__ out,
+                                            const typename IdT<W>::T d[4], typename IdT<W>::T base,
+                                            uint32_t b, uint32_t n_exc) {
     using T = typename IdT<W>::T;
-    constexpr int kBpw = FusedCfg<W>::kBpw, kTile = 8 * kBpw;
-    struct Stage {
-        alignas(16) T vals[kBlk];
-        alignas(16) unsigned char out[kBpw][EncStage<W>::kOutBytes];
-    };
-    __shared__ Stage stage[8];
-    __shared__ BlkMeta meta[2][kTile];
-    __shared__ uint32_t sm_size16[kTile];
-    __shared__ uint32_t sm_excl[kTile + 1];
-    __shared__ unsigned long long sm_tile_excl;
-    __shared__ unsigned long long sm_tile[2];
+    const int lane = lane_id();
+    if (lane == 0) {
+        reinterpret_cast<unsigned long long*>(out)[0] = (unsigned long long)base;
+        reinterpret_cast<unsigned long long*>(out)[1] = (unsigned long long)(b | (n_exc << 8));
+    }
+    if (b > 0) {
+        const T mask = (b >= (uint32_t)W) ? ~(T)0 : (((T)1 << b) - 1);
+        if constexpr (W == 32) {
+            reinterpret_cast<uint4*>(vals)[lane] = make_uint4(d[0] & mask, d[1] & mask, d[2] & mask, d[3] & mask);
+        } else {
+            reinterpret_cast<ulonglong2*>(vals)[2 * lane] = make_ulonglong2(d[0] & mask, d[1] & mask);
+            reinterpret_cast<ulonglong2*>(vals)[2 * lane + 1] = make_ulonglong2(d[2] & mask, d[3] & mask);
+        }
+    }
+    if (n_exc > 0) {                                 // warp-uniform
+        constexpr uint32_t E = W / 8;
+        unsigned char* e = out + 16 + 16 * b;
+        const uint32_t eb = exc_bytes<W>(n_exc);
+        uint4* z = reinterpret_cast<uint4*>(e);
+        for (uint32_t i = lane; i < eb / 16; i += 32) z[i] = make_uint4(0, 0, 0, 0);
+        __syncwarp();
+        T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
+        bool f[4];
+        uint32_t before = 0;
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+            f[c] = (d[c] >> b) != 0;                 // n_exc > 0 implies b < W
+            before += __popc(__ballot_sync(kFull, f[c]) & ((1u << lane) - 1u));
+        }
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+            if (f[c]) {
+                e[before] = (unsigned char)(4 * lane + c);
+                high[before] = d[c] >> b;
+                before++;
+            }
+        }
+    }
+}
+
+// E4 payloads of the warp's kBpw blocks, all lanes busy: work item = one 128-bit payload vector
+// (block q, vector k) = bits [32k, 32k+32) of the four column streams; it pulls rows
+// r_lo..r_hi from the staged values (row r sits at stream bits [r*b, r*b+b)).
+template <int W>
+__device__ __forceinline__ void pack_payloads(WarpStage<W>& st, const uint32_t (&bq)[FusedCfg<W>::kBpw]) {
+    using T = typename IdT<W>::T;
+    constexpr int kBpw = FusedCfg<W>::kBpw;
+    uint32_t cum[kBpw + 1];
+    cum[0] = 0;
+#pragma unroll
+    for (int q = 0; q < kBpw; q++) cum[q + 1] = cum[q] + bq[q];
+    for (uint32_t it = lane_id(); it < cum[kBpw]; it += 32) {
+        uint32_t q = 0, b = bq[0], k = it;
+#pragma unroll
+        for (int j = 1; j < kBpw; j++)
+            if (it >= cum[j]) { q = j; b = bq[j]; k = it - cum[j]; }
+        const uint32_t lo_bit = 32u * k;
+        const uint32_t r_lo = div_small(lo_bit, b);
+        const uint32_t r_hi = min(31u, div_small(lo_bit + 31u, b));
+        const uint32_t sh0 = lo_bit - r_lo * b;                     // 0 <= sh0 < b: first row is shifted right
+        uint32_t w0, w1, w2, w3;
+        if constexpr (W == 32) {
+            const uint4* rows = reinterpret_cast<const uint4*>(st.vals[q]);
+            uint4 v = rows[r_lo];
+            w0 = v.x >> sh0; w1 = v.y >> sh0; w2 = v.z >> sh0; w3 = v.w >> sh0;
+            uint32_t pos = b - sh0;
+            for (uint32_t r = r_lo + 1; r <= r_hi; r++, pos += b) {
+                v = rows[r];
+                w0 |= v.x << pos; w1 |= v.y << pos; w2 |= v.z << pos; w3 |= v.w << pos;
+            }
+        } else {
+            const ulonglong2* rows = reinterpret_cast<const ulonglong2*>(st.vals[q]);
+            ulonglong2 a = rows[2 * r_lo], c = rows[2 * r_lo + 1];
+            w0 = (uint32_t)(a.x >> sh0); w1 = (uint32_t)(a.y >> sh0);
+            w2 = (uint32_t)(c.x >> sh0); w3 = (uint32_t)(c.y >> sh0);
+            uint32_t pos = b - sh0;
+            for (uint32_t r = r_lo + 1; r <= r_hi; r++, pos += b) {  // pos < 32 here
+                a = rows[2 * r]; c = rows[2 * r + 1];
+                w0 |= (uint32_t)a.x << pos; w1 |= (uint32_t)a.y << pos;
+                w2 |= (uint32_t)c.x << pos; w3 |= (uint32_t)c.y << pos;
+            }
+        }
+        reinterpret_cast<uint4*>(st.out[q])[1 + k] = make_uint4(w0, w1, w2, w3);
+    }
+}
+
+
+template <int W>
+__global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
+    using T = typename IdT<W>::T;
+    constexpr int kBpw = FusedCfg<W>::kBpw;
+    static_assert(kTileR == kEncWarps * 32, "one thread per block of the tile in the bookkeeping step");
+    __shared__ WarpStage<W> stage_all[kEncWarps];
+    __shared__ uint32_t s_key[kTileR];               // pass A result per block: cost<<14 | (64-b)<<7 | n_exc
+    __shared__ uint32_t s_excl[kTileR + 1];          // exclusive scan of sizes (16-B units) inside the tile
+    __shared__ uint32_t s_buf[kTileR];               // buffer of each block
+    __shared__ int s_m[kTileR];                      // valid IDs of each block (0 = no block)
+    __shared__ unsigned long long s_xoff[kTileR];    // element offset of the block's first ID
+    __shared__ unsigned long long s_tile, s_tile_excl;
+    __shared__ unsigned long long s_lb_sum[kEncWarps];
+    __shared__ int s_lb_hit[kEncWarps];
 
     if (!a.ws.hdr->ok) return;
     const unsigned long long total = a.ws.hdr->total_blocks;
-    const unsigned long long n_tiles = (total + kTile - 1) / kTile;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const bool is_scan = (warp == 8);
+    const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
+    WarpStage<W>& st = stage_all[warp];
+    const T* ids = reinterpret_cast<const T*>(a.ids);
 
-    for (int it = 0;; it++) {
-        const int par = it & 1;
-        if (is_scan) {                                   // ticket + block metadata of the tile
-            unsigned long long t = 0;
-            if (lane == 0) t = atomicAdd(&a.ws.hdr->ticket, 1u);
-            t = __shfl_sync(kFull, t, 0);
-            if (lane == 0) sm_tile[par] = t;
-            const unsigned long long g = t * kTile + lane;
-            if (lane < kTile) {
-                BlkMeta mt;
-                mt.m = 0; mt.i = 0; mt.xoff = 0; mt.first = 0; mt.f0 = 0; mt.f1 = 0;
-                if (t < n_tiles && g < total) {
-                    const uint32_t i = find_buf(a.ws.blk_first, a.n_buf, g);
-                    mt.i = i;
-                    mt.first = a.ws.blk_first[i];
-                    const unsigned long long k = g - mt.first, n = buf_count(a, i);
-                    mt.m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-                    mt.xoff = buf_start(a, i) + kBlk * k;
-                    mt.f0 = a.ws.fixed_prefix[i];
-                    mt.f1 = a.ws.fixed_prefix[i + 1];
-                }
-                meta[par][lane] = mt;
-            }
-        }
-        __syncthreads();                                 // S1
-        const unsigned long long t = sm_tile[par];
+    while (true) {
+        if (tid == 0) s_tile = atomicAdd(&a.ws.hdr->ticket, 1u);
+        __syncthreads();
+        const unsigned long long t = s_tile;
         if (t >= n_tiles) break;
-        const unsigned long long g0 = t * kTile;
+        const unsigned long long g0 = t * kTileR;
 
-        T d[kBpw][4];
-        T base[kBpw];
-        uint32_t key[kBpw];
-        if (!is_scan) {                                  // E1 + E2
-            T v[kBpw][4];
-#pragma unroll
-            for (int q = 0; q < kBpw; q++) {
-                const BlkMeta& mt = meta[par][warp * kBpw + q];
-                if (mt.m > 0) load_rows<W>(reinterpret_cast<const T*>(a.ids) + mt.xoff, mt.m, v[q]);
-                else v[q][0] = v[q][1] = v[q][2] = v[q][3] = 0;
+        {   // bookkeeping: thread j describes block g0 + j
+            const unsigned long long g = g0 + tid;
+            int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
+            if (g < total) {
+                i = find_buf(a.ws.blk_first, a.n_buf, g);
+                const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
+                m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+                xoff = buf_start(a, i) + kBlk * k;
             }
+            s_m[tid] = m; s_buf[tid] = i; s_xoff[tid] = xoff;
+        }
+        __syncthreads();
+
+        // ---- pass A: sizes. warp w takes blocks w, w+8, ...; next block's load is issued before the math
+        {
+            T v[4], vn[4];
+            int j = warp;
+            if (s_m[j] > 0) load_rows_keep<W>(ids + s_xoff[j], s_m[j], vn);
+            for (; j < kTileR; j += kEncWarps) {
+                const int m = s_m[j];
 #pragma unroll
-            for (int q = 0; q < kBpw; q++) {
-                const int m = meta[par][warp * kBpw + q].m;
-                base[q] = deltas<W>(v[q], m > 0 ? m : 1, d[q]);
-                int w[4];
-                widths_of<W>(d[q], w);
-                key[q] = choose_b<W>(w);
-                if (lane == 0) sm_size16[warp * kBpw + q] = m > 0 ? (key[q] >> 18) : 0u;   // (cost >> 4)
+                for (int c = 0; c < 4; c++) v[c] = vn[c];
+                const int jn = j + kEncWarps;
+                if (jn < kTileR && s_m[jn] > 0) load_rows_keep<W>(ids + s_xoff[jn], s_m[jn], vn);
+                uint32_t key = 0;
+                if (m > 0) {
+                    T d[4];
+                    int w[4];
+                    deltas<W>(v, m, d);
+                    widths_of<W>(d, w);
+                    key = choose_b<W>(w);
+                }
+                if (lane == 0) s_key[j] = key;
             }
         }
-        __syncthreads();                                 // S2
-        if (is_scan) {                                   // E3: intra-tile scan, then look-back
-            uint32_t sz = lane < kTile ? sm_size16[lane] : 0u, inc = sz;
+        __syncthreads();
+
+        // ---- E3: intra-tile scan (warp 0), then CTA-wide decoupled look-back
+        if (warp == 0) {
+            uint32_t loc[kTileR / 32], sum = 0;
+#pragma unroll
+            for (int q = 0; q < kTileR / 32; q++) { loc[q] = sum; sum += s_key[lane * (kTileR / 32) + q] >> 18; }
+            uint32_t inc = sum;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 uint32_t x = __shfl_up_sync(kFull, inc, o);
                 if (lane >= o) inc += x;
             }
-            if (lane < kTile) sm_excl[lane] = inc - sz;
-            const unsigned long long agg = __shfl_sync(kFull, inc, 31);
-            if (lane == 0) {
-                sm_excl[kTile] = (uint32_t)agg;
-                if (t > 0) st_volatile_u64(&a.ws.tile_state[t], kFlagAgg | agg);
-            }
-            unsigned long long excl = 0;
-            if (t > 0) {
-                long long idx = (long long)t - 1;
-                while (true) {
-                    const long long mine = idx - lane;
-                    unsigned long long s = kFlagPre;     // tiles before 0: prefix 0
-                    if (mine >= 0) {
-                        do { s = ld_volatile_u64(&a.ws.tile_state[mine]); } while ((s >> 62) == 0);
-                    }
-                    const uint32_t pre = __ballot_sync(kFull, (s >> 62) == 2);
-                    const int stop = __ffs(pre) - 1;     // nearest tile with a full prefix (always exists: idx<0 lanes)
-                    unsigned long long val = (stop < 0 || lane <= stop) ? (s & kValMask) : 0ull;
+            const uint32_t base = inc - sum;
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(kFull, val, o);
-                    excl += val;
-                    if (stop >= 0) break;
-                    idx -= 32;
-                }
-            }
-            if (lane == 0) {
-                st_volatile_u64(&a.ws.tile_state[t], kFlagPre | (excl + agg));
-                sm_tile_excl = excl;
-                if (t == n_tiles - 1) {
-                    a.ws.hdr->grand16 = excl + agg;
-                    a.ws.hdr->total_out = a.ws.hdr->fixed_total + 16ull * (excl + agg);
-                }
-            }
-        } else {                                         // E4: pack into shared memory meanwhile
-#pragma unroll
-            for (int q = 0; q < kBpw; q++) {
-                if (meta[par][warp * kBpw + q].m > 0) {
-                    const uint32_t b = 64u - ((key[q] >> 7) & 127u), n_exc = key[q] & 127u;
-                    pack_block_to<W>(stage[warp].vals, stage[warp].out[q], d[q], base[q], b, n_exc);
-                }
+            for (int q = 0; q < kTileR / 32; q++) s_excl[lane * (kTileR / 32) + q] = base + loc[q];
+            if (lane == 31) {
+                s_excl[kTileR] = inc;
+                if (t > 0) st_volatile_u64(&a.ws.tile_state[t], kFlagAgg | (unsigned long long)inc);
             }
         }
-        __syncthreads();                                 // S3
-        if (!is_scan) {                                  // emit: 128-bit coalesced stores + directory entries
-            const unsigned long long tile_excl = sm_tile_excl;
+        unsigned long long excl = 0;
+        if (t > 0) {
+            long long idx = (long long)t - 1;
+            while (true) {                                       // 256 predecessors per round
+                const long long mine = idx - tid;
+                unsigned long long s = kFlagPre;                 // before tile 0: prefix 0
+                if (mine >= 0) {
+                    do { s = ld_volatile_u64(&a.ws.tile_state[mine]); } while ((s >> 62) == 0);
+                }
+                const uint32_t pre = __ballot_sync(kFull, (s >> 62) == 2);
+                const int stop = __ffs(pre) - 1;
+                unsigned long long val = (stop < 0 || lane <= stop) ? (s & kValMask) : 0ull;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(kFull, val, o);
+                if (lane == 0) { s_lb_sum[warp] = val; s_lb_hit[warp] = stop >= 0; }
+                __syncthreads();
+                bool hit = false;
+#pragma unroll
+                for (int w2 = 0; w2 < kEncWarps; w2++) {
+                    if (!hit) { excl += s_lb_sum[w2]; hit = s_lb_hit[w2] != 0; }
+                }
+                __syncthreads();
+                if (hit) break;
+                idx -= kTileR;
+            }
+        } else {
+            __syncthreads();
+        }
+        if (tid == 0) {
+            const unsigned long long agg = s_excl[kTileR];
+            st_volatile_u64(&a.ws.tile_state[t], kFlagPre | (excl + agg));
+            if (t == n_tiles - 1) {
+                a.ws.hdr->grand16 = excl + agg;
+                a.ws.hdr->total_out = a.ws.hdr->fixed_total + 16ull * (excl + agg);
+            }
+        }
+
+        // ---- pass B: pack + emit. warp w takes groups of kBpw consecutive blocks
+        for (int j0 = warp * kBpw; j0 < kTileR; j0 += kEncWarps * kBpw) {
+            if (s_m[j0] <= 0) break;                             // blocks of a tile are dense from 0
+            T v[kBpw][4];
 #pragma unroll
             for (int q = 0; q < kBpw; q++) {
-                const int blk = warp * kBpw + q;
-                const BlkMeta& mt = meta[par][blk];
-                if (mt.m <= 0) continue;
-                const unsigned long long g = g0 + blk;
-                const unsigned long long at = mt.f1 + 16ull * (tile_excl + sm_excl[blk]);
-                const uint32_t bytes = (key[q] >> 14);
+                if (s_m[j0 + q] > 0) load_rows<W>(ids + s_xoff[j0 + q], s_m[j0 + q], v[q]);
+                else v[q][0] = v[q][1] = v[q][2] = v[q][3] = 0;
+            }
+            uint32_t bq[kBpw];
+#pragma unroll
+            for (int q = 0; q < kBpw; q++) {
+                const int m = s_m[j0 + q];
+                const uint32_t key = s_key[j0 + q];
+                bq[q] = m > 0 ? 64u - ((key >> 7) & 127u) : 0u;
+                if (m > 0) {
+                    T d[4];
+                    const T base = deltas<W>(v[q], m, d);
+                    stage_block<W>(st.vals[q], st.out[q], d, base, bq[q], key & 127u);
+                }
+            }
+            __syncwarp();
+            pack_payloads<W>(st, bq);
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < kBpw; q++) {
+                const int j = j0 + q;
+                if (s_m[j] <= 0) continue;
+                const uint32_t i = s_buf[j];
+                const unsigned long long g = g0 + j;
+                const unsigned long long first = a.ws.blk_first[i];
+                const unsigned long long f0 = a.ws.fixed_prefix[i], f1 = a.ws.fixed_prefix[i + 1];
+                const unsigned long long at = f1 + 16ull * (excl + s_excl[j]);
+                const uint32_t bytes = s_key[j] >> 14;
                 unsigned long long S;
-                if (mt.first >= g0) {
-                    S = mt.f0 + 16ull * (tile_excl + sm_excl[mt.first - g0]);
+                if (first >= g0) {
+                    S = f0 + 16ull * (excl + s_excl[first - g0]);
+                } else if (i == 0) {
+                    S = 0;
                 } else {
                     unsigned long long s1 = 0;
-                    if (lane == 0) { do { s1 = ld_volatile_u64(&a.ws.stream_start[mt.i]); } while (s1 == 0); }
+                    if (lane == 0) { do { s1 = ld_volatile_u64(&a.ws.stream_start[i]); } while (s1 == 0); }
                     S = __shfl_sync(kFull, s1, 0) - 1;
                 }
                 if (at + bytes <= a.out_cap) {
-                    const uint4* src = reinterpret_cast<const uint4*>(stage[warp].out[q]);
+                    const uint4* src = reinterpret_cast<const uint4*>(st.out[q]);
                     uint4* dst = reinterpret_cast<uint4*>(a.out + at);
                     for (uint32_t x = lane; x < bytes / 16; x += 32) __stcs(dst + x, src[x]);
-                    if (lane == 0) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - mt.first] = (uint32_t)((at - S) >> 4);
+                    if (lane == 0) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
                 } else if (lane == 0) {
                     set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
                 }
-                if (lane == 0 && g == mt.first) st_volatile_u64(&a.ws.stream_start[mt.i], S + 1);
+                if (lane == 0 && g == first) st_volatile_u64(&a.ws.stream_start[i], S + 1);
             }
+            __syncwarp();
         }
     }
 }
@@ -319,7 +446,8 @@ template <int W>
 static bfsc_status launch_encode(const EncArgs& a, cudaStream_t s) {
     static int per_sm = 0;                        // persistent grid: every CTA resident (look-back needs it)
     if (per_sm == 0) {
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_fused<W>, 288, 0) != cudaSuccess || per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_fused<W>, kEncWarps * 32, 0) != cudaSuccess ||
+            per_sm < 1)
             per_sm = 1;
     }
     int dev = 0, sms = kNumSM;
@@ -328,7 +456,7 @@ static bfsc_status launch_encode(const EncArgs& a, cudaStream_t s) {
     const int grid = sms * per_sm;
     k_enc_plan<W><<<1, 1024, 0, s>>>(a);
     BFSC_LAUNCH_CHECK();
-    k_enc_fused<W><<<grid, 288, 0, s>>>(a);
+    k_enc_fused<W><<<grid, kEncWarps * 32, 0, s>>>(a);
     BFSC_LAUNCH_CHECK();
     const uint32_t sgrid = a.n_buf < (uint32_t)(kNumSM * 8) ? a.n_buf : (uint32_t)(kNumSM * 8);
     k_enc_streams<W><<<sgrid ? sgrid : 1, 256, 0, s>>>(a);
