@@ -1,5 +1,5 @@
 // encode.cu — bfsc_compress / bfsc_compress_batch (steps E0-E5).
-#include "block_encode.cuh"
+#include "quad_encode.cuh"
 
 namespace bfsc {
 
@@ -77,18 +77,15 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
 
 // ---- E1-E4 fused: one pass over HBM -----------------------------------------------------
 // A CTA pulls tiles of kTileR consecutive blocks (128 KB of u32 IDs) by ticket.
-//   pass A  (E1+E2): every warp takes blocks of the tile (warp = block), computes deltas, widths
-//           and the canonical b; the block's size goes to shared memory.
+//   pass A  (E1+E2): deltas, widths and the canonical b of every block; sizes to shared memory.
 //   scan    (E3): intra-tile exclusive scan of the sizes, tile aggregate published, decoupled
 //           look-back over the (few hundred) tiles in flight -> device-wide exclusive scan.
-//   pass B  (E1+E4): the same blocks are read again — they are still in the 126 MB L2, so HBM is
-//           read once — deltas recomputed, packed in shared memory and stored with 128-bit
-//           coalesced stores at their final offsets, with their directory entries.
-// Large tiles keep the look-back shallow (tiles in flight = resident CTAs) and need no
-// on-chip copy of the tile between the passes.
-template <int W> struct FusedCfg { static constexpr int kBpw = (W == 32) ? 4 : 2; };
-constexpr int kEncWarps = 8;             // warps per CTA
-constexpr int kTileR = 256;              // blocks per tile (= threads per CTA)
+//   pass B  (E1+E4): the blocks are read again — still in the 126 MB L2, so HBM is read once —
+//           packed in shared memory and stored with 128-bit stores at their final offsets, with
+//           their directory entries.
+// Both passes use four lanes per block (quad_encode.cuh): a warp works on 8 blocks at a time.
+template <int W> struct EncCfg { static constexpr int kWarps = (W == 32) ? 8 : 4; };
+constexpr int kTileR = 256;              // blocks per tile
 
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPre = 2ull << 62, kValMask = (1ull << 62) - 1;
 
@@ -102,125 +99,26 @@ __device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned 
 }
 
 template <int W>
-struct WarpStage {
-    static constexpr int kBpw = FusedCfg<W>::kBpw;
-    alignas(16) typename IdT<W>::T vals[kBpw][kBlk];                       // masked low parts, row-major
-    alignas(16) unsigned char out[kBpw][16 + 16 * W];                     // assembled blocks (canonical size <= 16+16W)
-};
-
-// header + masked values + exception list of one block into shared memory (no payload yet)
-template <int W>
-__device__ __forceinline__ void stage_block(typename IdT<W>::T* __restrict__ vals, unsigned char* __restrict__ out,
-                                            const typename IdT<W>::T d[4], typename IdT<W>::T base,
-                                            uint32_t b, uint32_t n_exc) {
+__global__ void __launch_bounds__(EncCfg<W>::kWarps * 32) k_enc_fused(EncArgs a) {
     using T = typename IdT<W>::T;
-    const int lane = lane_id();
-    if (lane == 0) {
-        reinterpret_cast<unsigned long long*>(out)[0] = (unsigned long long)base;
-        reinterpret_cast<unsigned long long*>(out)[1] = (unsigned long long)(b | (n_exc << 8));
-    }
-    if (b > 0) {
-        const T mask = (b >= (uint32_t)W) ? ~(T)0 : (((T)1 << b) - 1);
-        if constexpr (W == 32) {
-            reinterpret_cast<uint4*>(vals)[lane] = make_uint4(d[0] & mask, d[1] & mask, d[2] & mask, d[3] & mask);
-        } else {
-            reinterpret_cast<ulonglong2*>(vals)[2 * lane] = make_ulonglong2(d[0] & mask, d[1] & mask);
-            reinterpret_cast<ulonglong2*>(vals)[2 * lane + 1] = make_ulonglong2(d[2] & mask, d[3] & mask);
-        }
-    }
-    if (n_exc > 0) {                                 // warp-uniform
-        constexpr uint32_t E = W / 8;
-        unsigned char* e = out + 16 + 16 * b;
-        const uint32_t eb = exc_bytes<W>(n_exc);
-        uint4* z = reinterpret_cast<uint4*>(e);
-        for (uint32_t i = lane; i < eb / 16; i += 32) z[i] = make_uint4(0, 0, 0, 0);
-        __syncwarp();
-        T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
-        bool f[4];
-        uint32_t before = 0;
-#pragma unroll
-        for (int c = 0; c < 4; c++) {
-            f[c] = (d[c] >> b) != 0;                 // n_exc > 0 implies b < W
-            before += __popc(__ballot_sync(kFull, f[c]) & ((1u << lane) - 1u));
-        }
-#pragma unroll
-        for (int c = 0; c < 4; c++) {
-            if (f[c]) {
-                e[before] = (unsigned char)(4 * lane + c);
-                high[before] = d[c] >> b;
-                before++;
-            }
-        }
-    }
-}
-
-// E4 payloads of the warp's kBpw blocks, all lanes busy: work item = one 128-bit payload vector
-// (block q, vector k) = bits [32k, 32k+32) of the four column streams; it pulls rows
-// r_lo..r_hi from the staged values (row r sits at stream bits [r*b, r*b+b)).
-template <int W>
-__device__ __forceinline__ void pack_payloads(WarpStage<W>& st, const uint32_t (&bq)[FusedCfg<W>::kBpw]) {
-    using T = typename IdT<W>::T;
-    constexpr int kBpw = FusedCfg<W>::kBpw;
-    uint32_t cum[kBpw + 1];
-    cum[0] = 0;
-#pragma unroll
-    for (int q = 0; q < kBpw; q++) cum[q + 1] = cum[q] + bq[q];
-    for (uint32_t it = lane_id(); it < cum[kBpw]; it += 32) {
-        uint32_t q = 0, b = bq[0], k = it;
-#pragma unroll
-        for (int j = 1; j < kBpw; j++)
-            if (it >= cum[j]) { q = j; b = bq[j]; k = it - cum[j]; }
-        const uint32_t lo_bit = 32u * k;
-        const uint32_t r_lo = div_small(lo_bit, b);
-        const uint32_t r_hi = min(31u, div_small(lo_bit + 31u, b));
-        const uint32_t sh0 = lo_bit - r_lo * b;                     // 0 <= sh0 < b: first row is shifted right
-        uint32_t w0, w1, w2, w3;
-        if constexpr (W == 32) {
-            const uint4* rows = reinterpret_cast<const uint4*>(st.vals[q]);
-            uint4 v = rows[r_lo];
-            w0 = v.x >> sh0; w1 = v.y >> sh0; w2 = v.z >> sh0; w3 = v.w >> sh0;
-            uint32_t pos = b - sh0;
-            for (uint32_t r = r_lo + 1; r <= r_hi; r++, pos += b) {
-                v = rows[r];
-                w0 |= v.x << pos; w1 |= v.y << pos; w2 |= v.z << pos; w3 |= v.w << pos;
-            }
-        } else {
-            const ulonglong2* rows = reinterpret_cast<const ulonglong2*>(st.vals[q]);
-            ulonglong2 a = rows[2 * r_lo], c = rows[2 * r_lo + 1];
-            w0 = (uint32_t)(a.x >> sh0); w1 = (uint32_t)(a.y >> sh0);
-            w2 = (uint32_t)(c.x >> sh0); w3 = (uint32_t)(c.y >> sh0);
-            uint32_t pos = b - sh0;
-            for (uint32_t r = r_lo + 1; r <= r_hi; r++, pos += b) {  // pos < 32 here
-                a = rows[2 * r]; c = rows[2 * r + 1];
-                w0 |= (uint32_t)a.x << pos; w1 |= (uint32_t)a.y << pos;
-                w2 |= (uint32_t)c.x << pos; w3 |= (uint32_t)c.y << pos;
-            }
-        }
-        reinterpret_cast<uint4*>(st.out[q])[1 + k] = make_uint4(w0, w1, w2, w3);
-    }
-}
-
-
-template <int W>
-__global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
-    using T = typename IdT<W>::T;
-    constexpr int kBpw = FusedCfg<W>::kBpw;
-    static_assert(kTileR == kEncWarps * 32, "one thread per block of the tile in the bookkeeping step");
-    __shared__ WarpStage<W> stage_all[kEncWarps];
-    __shared__ uint32_t s_key[kTileR];               // pass A result per block: cost<<14 | (64-b)<<7 | n_exc
+    constexpr int kWarps = EncCfg<W>::kWarps, kThreads = kWarps * 32;
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    QuadStage<W>* stage_all = reinterpret_cast<QuadStage<W>*>(dyn_smem);
+    __shared__ uint32_t s_key[kTileR];               // pass A result per block: size<<14 | (64-b)<<7 | n_exc
     __shared__ uint32_t s_excl[kTileR + 1];          // exclusive scan of sizes (16-B units) inside the tile
     __shared__ uint32_t s_buf[kTileR];               // buffer of each block
     __shared__ int s_m[kTileR];                      // valid IDs of each block (0 = no block)
     __shared__ unsigned long long s_xoff[kTileR];    // element offset of the block's first ID
-    __shared__ unsigned long long s_tile, s_tile_excl;
-    __shared__ unsigned long long s_lb_sum[kEncWarps];
-    __shared__ int s_lb_hit[kEncWarps];
+    __shared__ unsigned long long s_tile;
+    __shared__ unsigned long long s_lb_sum[kWarps];
+    __shared__ int s_lb_hit[kWarps];
 
     if (!a.ws.hdr->ok) return;
     const unsigned long long total = a.ws.hdr->total_blocks;
     const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
-    WarpStage<W>& st = stage_all[warp];
+    const int q = lane >> 2, l = lane & 3;
+    QuadStage<W>& st = stage_all[warp];
     const T* ids = reinterpret_cast<const T*>(a.ids);
 
     while (true) {
@@ -230,8 +128,8 @@ __global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
         if (t >= n_tiles) break;
         const unsigned long long g0 = t * kTileR;
 
-        {   // bookkeeping: thread j describes block g0 + j
-            const unsigned long long g = g0 + tid;
+        for (int j = tid; j < kTileR; j += kThreads) {           // bookkeeping: block g0 + j
+            const unsigned long long g = g0 + j;
             int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
             if (g < total) {
                 i = find_buf(a.ws.blk_first, a.n_buf, g);
@@ -239,31 +137,36 @@ __global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
                 m = (int)min((unsigned long long)kBlk, n - kBlk * k);
                 xoff = buf_start(a, i) + kBlk * k;
             }
-            s_m[tid] = m; s_buf[tid] = i; s_xoff[tid] = xoff;
+            s_m[j] = m; s_buf[j] = i; s_xoff[j] = xoff; s_key[j] = 0;
         }
         __syncthreads();
 
-        // ---- pass A: sizes. warp w takes blocks w, w+8, ...; next block's load is issued before the math
-        {
-            T v[4], vn[4];
-            int j = warp;
-            if (s_m[j] > 0) load_rows_keep<W>(ids + s_xoff[j], s_m[j], vn);
-            for (; j < kTileR; j += kEncWarps) {
-                const int m = s_m[j];
+        // ---- pass A: sizes
+        for (int j0 = warp * kQuadBlocks; j0 < kTileR; j0 += kWarps * kQuadBlocks) {
+            if (s_m[j0] <= 0) break;                             // blocks of a tile are dense from 0
+            const int j = j0 + q, m = s_m[j];
+            T v[8][4], d[8][4];
+            quad_load<W>(ids + s_xoff[j], m, true, v);
+            quad_deltas<W>(v, m, d);
+            uint32_t key;
+            if constexpr (W == 32) {
+                key = quad_choose_b<32, uint32_t>(d);
+            } else {
+                uint64_t o = 0;
 #pragma unroll
-                for (int c = 0; c < 4; c++) v[c] = vn[c];
-                const int jn = j + kEncWarps;
-                if (jn < kTileR && s_m[jn] > 0) load_rows_keep<W>(ids + s_xoff[jn], s_m[jn], vn);
-                uint32_t key = 0;
-                if (m > 0) {
-                    T d[4];
-                    int w[4];
-                    deltas<W>(v, m, d);
-                    widths_of<W>(d, w);
-                    key = choose_b<W>(w);
+                for (int i = 0; i < 8; i++) o |= d[i][0] | d[i][1] | d[i][2] | d[i][3];
+                if (__all_sync(kFull, (o >> 32) == 0)) {
+                    uint32_t d32[8][4];
+#pragma unroll
+                    for (int i = 0; i < 8; i++)
+#pragma unroll
+                        for (int c = 0; c < 4; c++) d32[i][c] = (uint32_t)d[i][c];
+                    key = quad_choose_b<64, uint32_t>(d32);
+                } else {
+                    key = quad_choose_b<64, uint64_t>(d);
                 }
-                if (lane == 0) s_key[j] = key;
             }
+            if (l == 0) s_key[j] = m > 0 ? key : 0u;
         }
         __syncthreads();
 
@@ -271,16 +174,16 @@ __global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
         if (warp == 0) {
             uint32_t loc[kTileR / 32], sum = 0;
 #pragma unroll
-            for (int q = 0; q < kTileR / 32; q++) { loc[q] = sum; sum += s_key[lane * (kTileR / 32) + q] >> 18; }
+            for (int x = 0; x < kTileR / 32; x++) { loc[x] = sum; sum += s_key[lane * (kTileR / 32) + x] >> 18; }
             uint32_t inc = sum;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                uint32_t x = __shfl_up_sync(kFull, inc, o);
-                if (lane >= o) inc += x;
+                uint32_t y = __shfl_up_sync(kFull, inc, o);
+                if (lane >= o) inc += y;
             }
             const uint32_t base = inc - sum;
 #pragma unroll
-            for (int q = 0; q < kTileR / 32; q++) s_excl[lane * (kTileR / 32) + q] = base + loc[q];
+            for (int x = 0; x < kTileR / 32; x++) s_excl[lane * (kTileR / 32) + x] = base + loc[x];
             if (lane == 31) {
                 s_excl[kTileR] = inc;
                 if (t > 0) st_volatile_u64(&a.ws.tile_state[t], kFlagAgg | (unsigned long long)inc);
@@ -289,7 +192,7 @@ __global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
         unsigned long long excl = 0;
         if (t > 0) {
             long long idx = (long long)t - 1;
-            while (true) {                                       // 256 predecessors per round
+            while (true) {                                       // kThreads predecessors per round
                 const long long mine = idx - tid;
                 unsigned long long s = kFlagPre;                 // before tile 0: prefix 0
                 if (mine >= 0) {
@@ -304,12 +207,12 @@ __global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
                 __syncthreads();
                 bool hit = false;
 #pragma unroll
-                for (int w2 = 0; w2 < kEncWarps; w2++) {
+                for (int w2 = 0; w2 < kWarps; w2++) {
                     if (!hit) { excl += s_lb_sum[w2]; hit = s_lb_hit[w2] != 0; }
                 }
                 __syncthreads();
                 if (hit) break;
-                idx -= kTileR;
+                idx -= kThreads;
             }
         } else {
             __syncthreads();
@@ -323,59 +226,73 @@ __global__ void __launch_bounds__(kEncWarps * 32) k_enc_fused(EncArgs a) {
             }
         }
 
-        // ---- pass B: pack + emit. warp w takes groups of kBpw consecutive blocks
-        for (int j0 = warp * kBpw; j0 < kTileR; j0 += kEncWarps * kBpw) {
-            if (s_m[j0] <= 0) break;                             // blocks of a tile are dense from 0
-            T v[kBpw][4];
+        // ---- pass B: pack + emit
+        for (int j0 = warp * kQuadBlocks; j0 < kTileR; j0 += kWarps * kQuadBlocks) {
+            if (s_m[j0] <= 0) break;
+            const int j = j0 + q, m = s_m[j];
+            const uint32_t key = s_key[j];
+            const uint32_t b = m > 0 ? 64u - ((key >> 7) & 127u) : 0u, n_exc = key & 127u;
+            uint32_t* vq = st.vals + q * QuadStage<W>::kValWords;
+            unsigned char* oq = st.out + q * QuadStage<W>::kOutStride;
+            {
+                T v[8][4], d[8][4];
+                quad_load<W>(ids + s_xoff[j], m, false, v);
+                quad_deltas<W>(v, m, d);
+                if (l == 0) {                                    // block header (FORMAT.md §2)
+                    reinterpret_cast<unsigned long long*>(oq)[0] = (unsigned long long)v[0][0];
+                    reinterpret_cast<unsigned long long*>(oq)[1] = (unsigned long long)(b | (n_exc << 8));
+                }
+                if (__any_sync(kFull, n_exc > 0)) quad_exceptions<W, T>(vq, oq, d, b, n_exc);
+                if constexpr (W == 32) {
+                    quad_stage_vals<uint32_t>(vq, d, b);
+                } else {
+                    if (__any_sync(kFull, b > 32)) {             // wide payload somewhere in the batch
+                        quad_stage_vals<uint64_t>(vq, d, b);
+                        __syncwarp();
+                        quad_pack_column64(reinterpret_cast<const uint64_t*>(vq) + l,
+                                           reinterpret_cast<uint32_t*>(oq) + 4 + l, b);
+                    } else {
+                        uint32_t d32[8][4];
 #pragma unroll
-            for (int q = 0; q < kBpw; q++) {
-                if (s_m[j0 + q] > 0) load_rows<W>(ids + s_xoff[j0 + q], s_m[j0 + q], v[q]);
-                else v[q][0] = v[q][1] = v[q][2] = v[q][3] = 0;
-            }
-            uint32_t bq[kBpw];
+                        for (int i = 0; i < 8; i++)
 #pragma unroll
-            for (int q = 0; q < kBpw; q++) {
-                const int m = s_m[j0 + q];
-                const uint32_t key = s_key[j0 + q];
-                bq[q] = m > 0 ? 64u - ((key >> 7) & 127u) : 0u;
-                if (m > 0) {
-                    T d[4];
-                    const T base = deltas<W>(v[q], m, d);
-                    stage_block<W>(st.vals[q], st.out[q], d, base, bq[q], key & 127u);
+                            for (int c = 0; c < 4; c++) d32[i][c] = (uint32_t)d[i][c];
+                        quad_stage_vals<uint32_t>(vq, d32, b);
+                        __syncwarp();
+                        quad_pack_column32(vq + l, reinterpret_cast<uint32_t*>(oq) + 4 + l, b);
+                    }
                 }
             }
+            if constexpr (W == 32) {
+                __syncwarp();
+                quad_pack_column32(vq + l, reinterpret_cast<uint32_t*>(oq) + 4 + l, b);
+            }
             __syncwarp();
-            pack_payloads<W>(st, bq);
-            __syncwarp();
-#pragma unroll
-            for (int q = 0; q < kBpw; q++) {
-                const int j = j0 + q;
-                if (s_m[j] <= 0) continue;
+
+            // emit: final offsets, 128-bit stores, directory entry, stream start
+            if (m > 0) {
                 const uint32_t i = s_buf[j];
                 const unsigned long long g = g0 + j;
                 const unsigned long long first = a.ws.blk_first[i];
                 const unsigned long long f0 = a.ws.fixed_prefix[i], f1 = a.ws.fixed_prefix[i + 1];
                 const unsigned long long at = f1 + 16ull * (excl + s_excl[j]);
-                const uint32_t bytes = s_key[j] >> 14;
+                const uint32_t bytes = key >> 14;
                 unsigned long long S;
-                if (first >= g0) {
-                    S = f0 + 16ull * (excl + s_excl[first - g0]);
-                } else if (i == 0) {
-                    S = 0;
-                } else {
-                    unsigned long long s1 = 0;
-                    if (lane == 0) { do { s1 = ld_volatile_u64(&a.ws.stream_start[i]); } while (s1 == 0); }
-                    S = __shfl_sync(kFull, s1, 0) - 1;
+                if (first >= g0) S = f0 + 16ull * (excl + s_excl[first - g0]);
+                else if (i == 0) S = 0;
+                else {                                           // published by the tile that owns the first block
+                    do { S = ld_volatile_u64(&a.ws.stream_start[i]); } while (S == 0);
+                    S -= 1;
                 }
                 if (at + bytes <= a.out_cap) {
-                    const uint4* src = reinterpret_cast<const uint4*>(st.out[q]);
+                    const uint4* src = reinterpret_cast<const uint4*>(oq);
                     uint4* dst = reinterpret_cast<uint4*>(a.out + at);
-                    for (uint32_t x = lane; x < bytes / 16; x += 32) __stcs(dst + x, src[x]);
-                    if (lane == 0) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
-                } else if (lane == 0) {
+                    for (uint32_t x = l; x < bytes / 16; x += 4) __stcs(dst + x, src[x]);
+                    if (l == 0) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
+                } else if (l == 0) {
                     set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
                 }
-                if (lane == 0 && g == first) st_volatile_u64(&a.ws.stream_start[i], S + 1);
+                if (l == 0 && g == first) st_volatile_u64(&a.ws.stream_start[i], S + 1);
             }
             __syncwarp();
         }
@@ -444,19 +361,23 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
 
 template <int W>
 static bfsc_status launch_encode(const EncArgs& a, cudaStream_t s) {
-    static int per_sm = 0;                        // persistent grid: every CTA resident (look-back needs it)
-    if (per_sm == 0) {
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_fused<W>, kEncWarps * 32, 0) != cudaSuccess ||
+    constexpr int kThreads = EncCfg<W>::kWarps * 32;
+    constexpr size_t kSmem = sizeof(QuadStage<W>) * EncCfg<W>::kWarps;
+    static int grid = 0;                          // persistent grid: all CTAs resident
+    if (grid == 0) {
+        int per_sm = 0, dev = 0, sms = kNumSM;
+        if (cudaFuncSetAttribute(k_enc_fused<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
+            return BFSC_ERR_CUDA;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_fused<W>, kThreads, kSmem) != cudaSuccess ||
             per_sm < 1)
             per_sm = 1;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        grid = sms * per_sm;
     }
-    int dev = 0, sms = kNumSM;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int grid = sms * per_sm;
     k_enc_plan<W><<<1, 1024, 0, s>>>(a);
     BFSC_LAUNCH_CHECK();
-    k_enc_fused<W><<<grid, kEncWarps * 32, 0, s>>>(a);
+    k_enc_fused<W><<<grid, kThreads, kSmem, s>>>(a);
     BFSC_LAUNCH_CHECK();
     const uint32_t sgrid = a.n_buf < (uint32_t)(kNumSM * 8) ? a.n_buf : (uint32_t)(kNumSM * 8);
     k_enc_streams<W><<<sgrid ? sgrid : 1, 256, 0, s>>>(a);
