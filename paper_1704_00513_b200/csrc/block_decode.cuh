@@ -1,7 +1,7 @@
 // block_decode.cuh — per-block decode steps D2 (unpack), D3 (patch), D4 (scan + store) of
 // SURVEY.md §8(a). warp = block, lane r produces row r = IDs 4r..4r+3.
 #pragma once
-#include "block_encode.cuh"   // IdT
+#include "common.cuh"
 
 namespace bfsc {
 

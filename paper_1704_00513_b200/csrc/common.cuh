@@ -14,9 +14,14 @@ constexpr int kWarp = 32;
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr int kNumSM = 148;             // B200
 
+template <int W> struct IdT;
+template <> struct IdT<32> { using T = uint32_t; };
+template <> struct IdT<64> { using T = uint64_t; };
+
 // ---- workspace layout (device) -------------------------------------------------------
 // [WsHeader 256 B][blk_first u64 (n_buf+1)][fixed_prefix u64 (n_buf+1)][stream_start u64 (n_buf+1)]
-// [meta u32 (blk_cap+1)][bb16 u32 (blk_cap+1)][tile_state u64 (tile_cap)]
+// [tile_state: tile_cap entries of kStateStride u64 (one 64-byte entry per tile: the look-back polls
+//  of the tiles in flight then spread over many L2 slices instead of a few hot lines)]
 struct WsHeader {
     unsigned long long total_blocks;    // blocks of all PFOR streams of the batch
     unsigned long long fixed_total;     // sum of per-stream fixed bytes (header+directory | header+raw)
@@ -31,49 +36,38 @@ static_assert(sizeof(WsHeader) == 256, "WsHeader");
 struct WsView {
     WsHeader* hdr;
     unsigned long long* blk_first;      // n_buf+1 : first global block of each buffer
-    unsigned long long* fixed_prefix;   // n_buf+1 : exclusive prefix of fixed bytes
+    unsigned long long* fixed_prefix;   // n_buf+1 : exclusive prefix of fixed bytes (decode: of IDs)
     unsigned long long* stream_start;   // n_buf+1 : encode: 1 + byte offset of the stream (0 = not yet known)
-    uint32_t* meta;                     // blk_cap+1 : size16 | b<<8 | n_exc<<16
-    uint32_t* bb16;                     // blk_cap+1 : exclusive prefix of block sizes in 16-B units
-    unsigned long long* tile_state;     // tile_cap
+    unsigned long long* tile_state;     // tile_cap * kStateStride
     size_t blk_cap;
     size_t tile_cap;
 };
 
-constexpr int kTileBlocks = 2;          // smallest look-back tile (one warp: u64 2 blocks, u32 4) — sizes tile_state
+constexpr int kTileBlocks = 64;         // blocks per encode tile (8 worker warps x 8 blocks)
+constexpr int kStateStride = 8;         // u64 words between look-back states (64 B)
 
 __host__ __device__ inline size_t align_up(size_t x, size_t k) { return (x + k - 1) / k * k; }
 
-__host__ inline size_t ws_blk_cap_for(size_t n_ids_total, size_t n_buf) { return n_ids_total / kBlk + n_buf + 1; }
-
 __host__ inline size_t ws_bytes_for(size_t n_ids_total, size_t n_buf) {
-    size_t blk_cap = ws_blk_cap_for(n_ids_total, n_buf);
-    size_t tile_cap = blk_cap / kTileBlocks + n_buf + 2;
-    return sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + 2 * align_up(4 * (blk_cap + 1), 16)
-           + align_up(8 * tile_cap, 16) + 4096;
+    const size_t blk_cap = n_ids_total / kBlk + n_buf + 1;
+    const size_t tile_cap = blk_cap / kTileBlocks + 2;
+    return sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + 8 * kStateStride * tile_cap + 256;
 }
 
-// Carves the workspace; blk_cap is derived from the bytes actually provided.
+// Carves the workspace; the capacities are derived from the bytes actually provided.
 __host__ inline bool ws_carve(void* ws, size_t bytes, size_t n_buf, WsView* v) {
-    size_t fixed = sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + 64;
-    if (bytes < fixed + 64) return false;
-    size_t rest = bytes - fixed;
-    // per block: 8 B (meta + bb16) + 8/kTileBlocks B of tile state
-    if (rest < 128 + 8 * (n_buf + 2) + 1024) return false;
-    size_t blk_cap = (rest - 128 - 8 * (n_buf + 2)) * kTileBlocks / (8 * kTileBlocks + 8);
-    if (blk_cap < 2) return false;
-    blk_cap -= 1;
-    size_t tile_cap = blk_cap / kTileBlocks + n_buf + 2;
+    const size_t fixed = sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16);
+    if (bytes < fixed + 8 * kStateStride * 2) return false;
+    const size_t tile_cap = (bytes - fixed) / (8 * kStateStride);
     char* p = (char*)ws;
     v->hdr = (WsHeader*)p; p += sizeof(WsHeader);
     v->blk_first = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
     v->fixed_prefix = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
     v->stream_start = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
-    v->meta = (uint32_t*)p; p += align_up(4 * (blk_cap + 1), 16);
-    v->bb16 = (uint32_t*)p; p += align_up(4 * (blk_cap + 1), 16);
-    v->tile_state = (unsigned long long*)p; p += align_up(8 * tile_cap, 16);
-    v->blk_cap = blk_cap; v->tile_cap = tile_cap;
-    return (size_t)(p - (char*)ws) <= bytes;
+    v->tile_state = (unsigned long long*)p;
+    v->tile_cap = tile_cap;
+    v->blk_cap = (tile_cap - 1) * kTileBlocks;
+    return true;
 }
 
 // ---- device helpers ------------------------------------------------------------------

@@ -1,5 +1,10 @@
 // encode.cu — bfsc_compress / bfsc_compress_batch (steps E0-E5).
+//
+// Launches per call:  k_enc_plan -> k_enc_tiles [-> k_enc_streams, batch and degenerate calls only],
+// chained with programmatic dependent launch: a dependent kernel starts while its predecessor still
+// runs and executes griddepcontrol.wait before it touches what the predecessor writes.
 #include "quad_encode.cuh"
+#include "wide_encode.cuh"
 
 namespace bfsc {
 
@@ -8,6 +13,7 @@ struct EncArgs {
     const unsigned long long* in_off;   // n_buf+1 element offsets, or nullptr (single buffer of n_single IDs)
     unsigned long long n_single;
     uint32_t n_buf;
+    uint32_t pad0;
     unsigned long long thr;             // raw threshold in bytes
     unsigned char* out;
     unsigned long long out_cap;
@@ -24,13 +30,21 @@ __device__ __forceinline__ unsigned long long buf_count(const EncArgs& a, uint32
     return a.in_off ? a.in_off[i + 1] - a.in_off[i] : a.n_single;
 }
 
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+constexpr int kEncWorkers = 8;                           // worker warps per CTA
+constexpr int kTileR = kEncWorkers * kQuadBlocks;        // 64 blocks per tile
+static_assert(kTileR == kTileBlocks, "workspace sizing assumes 64-block tiles");
+constexpr int kEncThreads = (kEncWorkers + 1) * 32;      // + the scan warp
+
 // ---- E0: plan. One CTA; per buffer: mode, block count, fixed bytes; exclusive prefixes. ----
 template <int W>
 __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     __shared__ Scan2 sm[33];
     __shared__ int bad;
     constexpr unsigned long long E = W / 8;
-    constexpr unsigned long long kTile = 256;                   // = kTileR of the fused kernel
+    pdl_launch_dependents();
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
     Scan2 carry{0, 0};
@@ -55,10 +69,10 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         carry.a += tot.a; carry.b += tot.b;
     }
     __syncthreads();
-    {                                                    // look-back states of the fused kernel start invalid
-        unsigned long long nt = (carry.a + kTile - 1) / kTile;
+    {                                                    // look-back states start invalid
+        unsigned long long nt = (carry.a + kTileR - 1) / kTileR;
         if (nt > a.ws.tile_cap) nt = a.ws.tile_cap;
-        for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q] = 0;
+        for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q * kStateStride] = 0;
     }
     if (threadIdx.x == 0) {
         a.ws.blk_first[a.n_buf] = carry.a;
@@ -69,25 +83,38 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         a.ws.hdr->ticket = 0;
         a.ws.hdr->grand16 = 0;
         a.ws.hdr->total_out = carry.b;
-        const bool ok = !bad && carry.a <= a.ws.blk_cap && (carry.a + kTile - 1) / kTile <= a.ws.tile_cap;
+        const bool ok = !bad && carry.a <= a.ws.blk_cap && (carry.a + kTileR - 1) / kTileR <= a.ws.tile_cap;
         a.ws.hdr->ok = ok ? 1u : 0u;
         if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
     }
 }
 
-// ---- E1-E4 fused: one pass over HBM -----------------------------------------------------
-// A CTA pulls tiles of kTileR consecutive blocks (128 KB of u32 IDs) by ticket.
-//   pass A  (E1+E2): deltas, widths and the canonical b of every block; sizes to shared memory.
-//   scan    (E3): intra-tile exclusive scan of the sizes, tile aggregate published, decoupled
-//           look-back over the (few hundred) tiles in flight -> device-wide exclusive scan.
-//   pass B  (E1+E4): the blocks are read again — still in the 126 MB L2, so HBM is read once —
-//           packed in shared memory and stored with 128-bit stores at their final offsets, with
-//           their directory entries.
-// Both passes use four lanes per block (quad_encode.cuh): a warp works on 8 blocks at a time.
-template <int W> struct EncCfg { static constexpr int kWarps = (W == 32) ? 8 : 4; };
-constexpr int kTileR = 256;              // blocks per tile
+// ---- E1-E4 fused: one pass over HBM ------------------------------------------------------
+// CTA = 8 worker warps + 1 scan warp; tile = 64 consecutive blocks (32 KB of u32 IDs), pulled by
+// ticket. Worker warps handle 8 blocks each, four lanes per block (quad_encode.cuh):
+//   E1+E2  load (128-bit, streaming), deltas, canonical b  -> s_key, arrive on barrier 1
+//   E4     stage deltas -> column owners mask + pack the payload, exceptions, header into the
+//          warp's image area (shared memory) — overlapped with the scan warp's E3
+//   sync on barrier 2, copy the image to its final offset with 128-bit stores.
+// Scan warp (E3): while the workers run E1/E2 it draws the next ticket and prepares that tile's
+// bookkeeping; after barrier 1: intra-tile exclusive scan of the 64 sizes, aggregate published,
+// decoupled look-back over the tiles in flight (= device-wide exclusive scan of block sizes),
+// final byte offset of every block -> s_at, directory entries, stream starts, and (single-buffer
+// calls) the stream header; barrier 2.
+#ifdef BFSC_TRACE
+// Debug build only (never in libbfsc.so): per-tile phase timestamps, read back with bfsc_debug_trace.
+__device__ unsigned long long g_trace[4096 * 16];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+__device__ __forceinline__ unsigned int smid() { unsigned int r; asm volatile("mov.u32 %0, %%smid;" : "=r"(r)); return r; }
+#define TR(tile, slot_) do { if ((threadIdx.x & 31) == 0 && (tile) < 4096) g_trace[(tile) * 16 + (slot_)] = gtime(); } while (0)
+#define TRV(tile, slot_, v) do { if ((threadIdx.x & 31) == 0 && (tile) < 4096) g_trace[(tile) * 16 + (slot_)] = (v); } while (0)
+#else
+#define TR(tile, slot_) do {} while (0)
+#define TRV(tile, slot_, v) do {} while (0)
+#endif
 
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPre = 2ull << 62, kValMask = (1ull << 62) - 1;
+constexpr unsigned long long kNoTile = ~0ull, kSkip = ~0ull;
 
 __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
     unsigned long long v;
@@ -97,213 +124,288 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
 __device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned long long v) {
     asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
+__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+// Exclusive prefix (16-byte units) of tile t > 0: aggregates of t-1, t-2, ... down to the nearest
+// tile whose inclusive prefix is known. One warp. The states of the 512 nearest predecessors — more
+// than the tiles in flight — are fetched up front (16 independent loads per lane: ONE L2 round
+// trip); 32 ballots find the nearest posted prefix; every lane sums its own entries and a single
+// warp reduction ends it (a reduction per chunk of 32 made this the critical path of the kernel).
+constexpr int kLookChunks = 16;
+__device__ __forceinline__ unsigned long long lookback(const unsigned long long* __restrict__ state,
+                                                       unsigned long long t, int lane) {
+    unsigned long long acc = 0;
+    long long idx = (long long)t - 1 - lane;
+    while (true) {
+        unsigned long long s[kLookChunks];
+#pragma unroll
+        for (int r = 0; r < kLookChunks; r++)
+            s[r] = (idx - 32 * r >= 0) ? ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]) : kFlagPre;
+        int rs, stop;
+        while (true) {
+            uint32_t hit[kLookChunks], rdy[kLookChunks];
+#pragma unroll
+            for (int r = 0; r < kLookChunks; r++) {
+                hit[r] = __ballot_sync(kFull, (s[r] >> 62) == 2);
+                rdy[r] = __ballot_sync(kFull, (s[r] >> 62) != 0);
+            }
+            rs = kLookChunks; stop = 31;
+#pragma unroll
+            for (int r = kLookChunks - 1; r >= 0; r--)
+                if (hit[r]) { rs = r; stop = __ffs(hit[r]) - 1; }
+            bool ok = true;                                      // everything up to the stop entry is posted
+#pragma unroll
+            for (int r = 0; r < kLookChunks; r++) {
+                const uint32_t need = r < rs ? kFull : (r == rs ? (0xffffffffu >> (31 - stop)) : 0u);
+                ok = ok && ((rdy[r] & need) == need);
+            }
+            if (ok) break;
+            __nanosleep(64);
+#pragma unroll
+            for (int r = 0; r < kLookChunks; r++)
+                if ((s[r] >> 62) == 0) s[r] = ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]);
+        }
+#pragma unroll
+        for (int r = 0; r < kLookChunks; r++)
+            if (r < rs || (r == rs && lane <= stop)) acc += s[r] & kValMask;
+        if (rs < kLookChunks) break;
+        idx -= 32 * kLookChunks;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
+    return acc;
+}
+
+template <int W> struct EncSmem {
+    static constexpr int kStageChunks = RawCfg<W>::kAreaChunks;              // per worker warp: staged raw IDs
+    static constexpr int kWarpChunks = kStageChunks + kAreaChunks;           // + image area
+    static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
+};
 
 template <int W>
-__global__ void __launch_bounds__(EncCfg<W>::kWarps * 32) k_enc_fused(EncArgs a) {
+__global__ void __launch_bounds__(kEncThreads, (W == 32) ? 3 : 2) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
-    constexpr int kWarps = EncCfg<W>::kWarps, kThreads = kWarps * 32;
-    extern __shared__ __align__(16) unsigned char dyn_smem[];
-    QuadStage<W>* stage_all = reinterpret_cast<QuadStage<W>*>(dyn_smem);
-    __shared__ uint32_t s_key[kTileR];               // pass A result per block: size<<14 | (64-b)<<7 | n_exc
-    __shared__ uint32_t s_excl[kTileR + 1];          // exclusive scan of sizes (16-B units) inside the tile
-    __shared__ uint32_t s_buf[kTileR];               // buffer of each block
-    __shared__ int s_m[kTileR];                      // valid IDs of each block (0 = no block)
-    __shared__ unsigned long long s_xoff[kTileR];    // element offset of the block's first ID
-    __shared__ unsigned long long s_tile;
-    __shared__ unsigned long long s_lb_sum[kWarps];
-    __shared__ int s_lb_hit[kWarps];
+    extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | image area
+    __shared__ uint32_t s_key[kTileR];                   // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
+    __shared__ unsigned long long s_at[kTileR];          // scan warp: final byte offset of the block, or kSkip
+    __shared__ uint32_t s_off16[kTileR];                 // exclusive scan of the sizes inside the tile (16-B units)
+    __shared__ int s_m[2][kTileR];                       // tile bookkeeping, two parities: valid IDs of each block (0 = none)
+    __shared__ unsigned long long s_xoff[2][kTileR];     // element offset of the block's first ID
+    __shared__ uint32_t s_buf[2][kTileR];                // buffer of each block (batch calls)
+    __shared__ unsigned long long s_tile[2];             // tile of each parity, kNoTile = done
 
-    if (!a.ws.hdr->ok) return;
-    const unsigned long long total = a.ws.hdr->total_blocks;
-    const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
-    const int q = lane >> 2, l = lane & 3;
-    QuadStage<W>& st = stage_all[warp];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool batch = a.in_off != nullptr;
     const T* ids = reinterpret_cast<const T*>(a.ids);
 
-    while (true) {
-        if (tid == 0) s_tile = atomicAdd(&a.ws.hdr->ticket, 1u);
-        __syncthreads();
-        const unsigned long long t = s_tile;
-        if (t >= n_tiles) break;
-        const unsigned long long g0 = t * kTileR;
+    if (warp == kEncWorkers) {
+        // =============================== scan warp ===============================
+        pdl_wait();                                      // the plan kernel's writes are visible from here on
+        const bool ok = a.ws.hdr->ok != 0;
+        const unsigned long long total = ok ? a.ws.hdr->total_blocks : 0ull;
+        const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
+        const unsigned long long nb_single = (a.n_single + kBlk - 1) / kBlk;
+        const unsigned long long f1_single = 32ull + ((4ull * (nb_single + 1) + 15ull) & ~15ull);
 
-        for (int j = tid; j < kTileR; j += kThreads) {           // bookkeeping: block g0 + j
-            const unsigned long long g = g0 + j;
-            int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
-            if (g < total) {
-                i = find_buf(a.ws.blk_first, a.n_buf, g);
-                const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
-                m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-                xoff = buf_start(a, i) + kBlk * k;
-            }
-            s_m[j] = m; s_buf[j] = i; s_xoff[j] = xoff; s_key[j] = 0;
-        }
-        __syncthreads();
-
-        // ---- pass A: sizes
-        for (int j0 = warp * kQuadBlocks; j0 < kTileR; j0 += kWarps * kQuadBlocks) {
-            if (s_m[j0] <= 0) break;                             // blocks of a tile are dense from 0
-            const int j = j0 + q, m = s_m[j];
-            T v[8][4], d[8][4];
-            quad_load<W>(ids + s_xoff[j], m, true, v);
-            quad_deltas<W>(v, m, d);
-            uint32_t key;
-            if constexpr (W == 32) {
-                key = quad_choose_b<32, uint32_t>(d);
-            } else {
-                uint64_t o = 0;
-#pragma unroll
-                for (int i = 0; i < 8; i++) o |= d[i][0] | d[i][1] | d[i][2] | d[i][3];
-                if (__all_sync(kFull, (o >> 32) == 0)) {
-                    uint32_t d32[8][4];
-#pragma unroll
-                    for (int i = 0; i < 8; i++)
-#pragma unroll
-                        for (int c = 0; c < 4; c++) d32[i][c] = (uint32_t)d[i][c];
-                    key = quad_choose_b<64, uint32_t>(d32);
-                } else {
-                    key = quad_choose_b<64, uint64_t>(d);
-                }
-            }
-            if (l == 0) s_key[j] = m > 0 ? key : 0u;
-        }
-        __syncthreads();
-
-        // ---- E3: intra-tile scan (warp 0), then CTA-wide decoupled look-back
-        if (warp == 0) {
-            uint32_t loc[kTileR / 32], sum = 0;
-#pragma unroll
-            for (int x = 0; x < kTileR / 32; x++) { loc[x] = sum; sum += s_key[lane * (kTileR / 32) + x] >> 18; }
-            uint32_t inc = sum;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t y = __shfl_up_sync(kFull, inc, o);
-                if (lane >= o) inc += y;
-            }
-            const uint32_t base = inc - sum;
-#pragma unroll
-            for (int x = 0; x < kTileR / 32; x++) s_excl[lane * (kTileR / 32) + x] = base + loc[x];
-            if (lane == 31) {
-                s_excl[kTileR] = inc;
-                if (t > 0) st_volatile_u64(&a.ws.tile_state[t], kFlagAgg | (unsigned long long)inc);
-            }
-        }
-        unsigned long long excl = 0;
-        if (t > 0) {
-            long long idx = (long long)t - 1;
-            while (true) {                                       // kThreads predecessors per round
-                const long long mine = idx - tid;
-                unsigned long long s = kFlagPre;                 // before tile 0: prefix 0
-                if (mine >= 0) {
-                    do { s = ld_volatile_u64(&a.ws.tile_state[mine]); } while ((s >> 62) == 0);
-                }
-                const uint32_t pre = __ballot_sync(kFull, (s >> 62) == 2);
-                const int stop = __ffs(pre) - 1;
-                unsigned long long val = (stop < 0 || lane <= stop) ? (s & kValMask) : 0ull;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(kFull, val, o);
-                if (lane == 0) { s_lb_sum[warp] = val; s_lb_hit[warp] = stop >= 0; }
-                __syncthreads();
-                bool hit = false;
-#pragma unroll
-                for (int w2 = 0; w2 < kWarps; w2++) {
-                    if (!hit) { excl += s_lb_sum[w2]; hit = s_lb_hit[w2] != 0; }
-                }
-                __syncthreads();
-                if (hit) break;
-                idx -= kThreads;
-            }
-        } else {
-            __syncthreads();
-        }
-        if (tid == 0) {
-            const unsigned long long agg = s_excl[kTileR];
-            st_volatile_u64(&a.ws.tile_state[t], kFlagPre | (excl + agg));
-            if (t == n_tiles - 1) {
-                a.ws.hdr->grand16 = excl + agg;
-                a.ws.hdr->total_out = a.ws.hdr->fixed_total + 16ull * (excl + agg);
-            }
-        }
-
-        // ---- pass B: pack + emit
-        for (int j0 = warp * kQuadBlocks; j0 < kTileR; j0 += kWarps * kQuadBlocks) {
-            if (s_m[j0] <= 0) break;
-            const int j = j0 + q, m = s_m[j];
-            const uint32_t key = s_key[j];
-            const uint32_t b = m > 0 ? 64u - ((key >> 7) & 127u) : 0u, n_exc = key & 127u;
-            uint32_t* vq = st.vals + q * QuadStage<W>::kValWords;
-            unsigned char* oq = st.out + q * QuadStage<W>::kOutStride;
-            {
-                T v[8][4], d[8][4];
-                quad_load<W>(ids + s_xoff[j], m, false, v);
-                quad_deltas<W>(v, m, d);
-                if (l == 0) {                                    // block header (FORMAT.md §2)
-                    reinterpret_cast<unsigned long long*>(oq)[0] = (unsigned long long)v[0][0];
-                    reinterpret_cast<unsigned long long*>(oq)[1] = (unsigned long long)(b | (n_exc << 8));
-                }
-                if (__any_sync(kFull, n_exc > 0)) quad_exceptions<W, T>(vq, oq, d, b, n_exc);
-                if constexpr (W == 32) {
-                    quad_stage_vals<uint32_t>(vq, d, b);
-                } else {
-                    if (__any_sync(kFull, b > 32)) {             // wide payload somewhere in the batch
-                        quad_stage_vals<uint64_t>(vq, d, b);
-                        __syncwarp();
-                        quad_pack_column64(reinterpret_cast<const uint64_t*>(vq) + l,
-                                           reinterpret_cast<uint32_t*>(oq) + 4 + l, b);
+        auto draw = [&]() -> unsigned long long {
+            unsigned long long t = 0;
+            if (lane == 0) t = atomicAdd(&a.ws.hdr->ticket, 1u);
+            t = __shfl_sync(kFull, t, 0);
+            return t < n_tiles ? t : kNoTile;
+        };
+        auto prep = [&](unsigned long long t, int p) {   // bookkeeping of tile t into ring slot p
+            if (lane == 0) s_tile[p] = t;
+            if (t == kNoTile) return;
+            for (int jj = lane; jj < kTileR; jj += 32) {
+                const unsigned long long g = t * kTileR + jj;
+                int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
+                if (g < total) {
+                    if (batch) {
+                        i = find_buf(a.ws.blk_first, a.n_buf, g);
+                        const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
+                        m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+                        xoff = buf_start(a, i) + kBlk * k;
                     } else {
-                        uint32_t d32[8][4];
-#pragma unroll
-                        for (int i = 0; i < 8; i++)
-#pragma unroll
-                            for (int c = 0; c < 4; c++) d32[i][c] = (uint32_t)d[i][c];
-                        quad_stage_vals<uint32_t>(vq, d32, b);
-                        __syncwarp();
-                        quad_pack_column32(vq + l, reinterpret_cast<uint32_t*>(oq) + 4 + l, b);
+                        m = (int)min((unsigned long long)kBlk, a.n_single - kBlk * g);
+                        xoff = kBlk * g;
                     }
                 }
+                s_m[p][jj] = m; s_xoff[p][jj] = xoff; s_buf[p][jj] = i;
             }
-            if constexpr (W == 32) {
-                __syncwarp();
-                quad_pack_column32(vq + l, reinterpret_cast<uint32_t*>(oq) + 4 + l, b);
+        };
+
+        // Tickets are drawn ONE per tile and always at the same point of the pipeline (right after the
+        // previous tile's sizes are in): a lower tile number then means "sizes ready earlier", so a
+        // look-back rarely has to wait. Drawing ahead (two tickets at once) inverts that order.
+        unsigned long long t = draw();
+        prep(t, 0);
+        __syncthreads();                                 // barrier 0: the first tile is posted
+        int p = 0;
+        while (t != kNoTile) {
+            TR(t, 0);
+            bar_sync(1, kEncThreads);                    // the workers' sizes of tile t are in s_key
+            TR(t, 1);
+            unsigned int ticket = 0;                     // next tile: the atomic's latency hides behind the scan
+            if (lane == 0) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+
+            // E3: intra-tile scan (2 consecutive blocks per lane)
+            const uint32_t k0 = s_key[2 * lane], k1 = s_key[2 * lane + 1];
+            const uint32_t z0 = k0 >> 18, z1 = k1 >> 18;
+            uint32_t inc = z0 + z1;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(kFull, inc, o);
+                if (lane >= o) inc += y;
+            }
+            const uint32_t off0 = inc - z0 - z1, off1 = off0 + z0;
+            const unsigned long long agg = __shfl_sync(kFull, inc, 31);
+            s_off16[2 * lane] = off0; s_off16[2 * lane + 1] = off1;
+            if (t > 0 && lane == 0) st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagAgg | agg);
+            TR(t, 2);
+            const unsigned long long excl = t > 0 ? lookback(a.ws.tile_state, t, lane) : 0ull;
+            TR(t, 3);
+            if (lane == 0) {
+                st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagPre | (excl + agg));
+                if (t == n_tiles - 1) {
+                    a.ws.hdr->grand16 = excl + agg;
+                    a.ws.hdr->total_out = a.ws.hdr->fixed_total + 16ull * (excl + agg);
+                }
             }
             __syncwarp();
 
-            // emit: final offsets, 128-bit stores, directory entry, stream start
-            if (m > 0) {
-                const uint32_t i = s_buf[j];
-                const unsigned long long g = g0 + j;
-                const unsigned long long first = a.ws.blk_first[i];
-                const unsigned long long f0 = a.ws.fixed_prefix[i], f1 = a.ws.fixed_prefix[i + 1];
-                const unsigned long long at = f1 + 16ull * (excl + s_excl[j]);
-                const uint32_t bytes = key >> 14;
-                unsigned long long S;
-                if (first >= g0) S = f0 + 16ull * (excl + s_excl[first - g0]);
-                else if (i == 0) S = 0;
-                else {                                           // published by the tile that owns the first block
-                    do { S = ld_volatile_u64(&a.ws.stream_start[i]); } while (S == 0);
-                    S -= 1;
+            // final offsets, directory entries, stream starts
+            const unsigned long long g0 = t * kTileR;
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int jj = 2 * lane + h;
+                const unsigned long long g = g0 + jj;
+                const uint32_t key = h ? k1 : k0;
+                unsigned long long at = kSkip;
+                if (g < total) {
+                    const uint32_t off = h ? off1 : off0, bytes = key >> 14;
+                    unsigned long long first = 0, f0 = 0, f1 = f1_single, S = 0;
+                    uint32_t i = 0;
+                    if (batch) {
+                        i = s_buf[p][jj];
+                        first = a.ws.blk_first[i]; f0 = a.ws.fixed_prefix[i]; f1 = a.ws.fixed_prefix[i + 1];
+                        if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
+                        else if (i > 0) {                // published by the tile that owns the stream's first block
+                            do { S = ld_volatile_u64(&a.ws.stream_start[i]); } while (S == 0);
+                            S -= 1;
+                        }
+                        if (g == first) st_volatile_u64(&a.ws.stream_start[i], S + 1);
+                    }
+                    at = f1 + 16ull * (excl + off);
+                    if (at + bytes <= a.out_cap) {
+                        reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
+                    } else {
+                        set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+                        at = kSkip;
+                    }
+                    if (!batch && g == total - 1) {      // single buffer: stream header, dir[nb], zero pad
+                        const unsigned long long tot = f1 + 16ull * (excl + off) + bytes;
+                        if (at != kSkip) {
+                            uint4 h0, h1;
+                            h0.x = 0x43534642u;                                   // "BFSC"
+                            h0.y = 1u | ((uint32_t)W << 8) | (1u << 16);
+                            h0.z = (uint32_t)a.n_single; h0.w = (uint32_t)(a.n_single >> 32);
+                            h1.x = (uint32_t)tot; h1.y = (uint32_t)(tot >> 32);
+                            h1.z = (uint32_t)nb_single; h1.w = 0;
+                            reinterpret_cast<uint4*>(a.out)[0] = h0;
+                            reinterpret_cast<uint4*>(a.out)[1] = h1;
+                            uint32_t* dir = reinterpret_cast<uint32_t*>(a.out + 32);
+                            dir[nb_single] = (uint32_t)(tot >> 4);
+                            for (unsigned long long x = nb_single + 1; x < ((nb_single + 1 + 3) & ~3ull); x++) dir[x] = 0;
+                        }
+                        if (a.out_total) *a.out_total = at != kSkip ? tot : 0ull;
+                    }
                 }
-                if (at + bytes <= a.out_cap) {
-                    const uint4* src = reinterpret_cast<const uint4*>(oq);
-                    uint4* dst = reinterpret_cast<uint4*>(a.out + at);
-                    for (uint32_t x = l; x < bytes / 16; x += 4) __stcs(dst + x, src[x]);
-                    if (l == 0) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
-                } else if (l == 0) {
-                    set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
-                }
-                if (l == 0 && g == first) st_volatile_u64(&a.ws.stream_start[i], S + 1);
+                s_at[jj] = at;
+            }
+            TR(t, 13);
+            ticket = __shfl_sync(kFull, ticket, 0);
+            const unsigned long long nt = ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
+            prep(nt, p ^ 1);
+            TR(t, 4);
+            bar_sync(2, kEncThreads);
+            TR(t, 5);
+            TRV(t, 15, (unsigned long long)smid() | ((unsigned long long)blockIdx.x << 32));
+            t = nt; p ^= 1;
+        }
+        return;
+    }
+
+    // =============================== worker warps ===============================
+    const int q = lane >> 2, l = lane & 3;
+    uint4* area = dyn_smem + warp * EncSmem<W>::kWarpChunks;
+    uint4* slot = area + raw_slot_chunk<W>(q);                           // staging: the quad's raw IDs
+    unsigned char* img = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks + quad_slot_chunk(q));
+    const int j = warp * kQuadBlocks + q;
+    __syncthreads();                                                     // barrier 0
+    if (s_tile[0] != kNoTile) quad_prefetch<W>(slot, ids + s_xoff[0][j], s_m[0][j]);
+    int p = 0;
+    while (true) {
+        const unsigned long long t = s_tile[p];
+        if (t == kNoTile) break;
+        const int m = s_m[p][j];
+        const T* x = ids + s_xoff[p][j];
+        const T* raw = reinterpret_cast<const T*>(slot) + (reinterpret_cast<uintptr_t>(x) & 15) / sizeof(T);
+        if (warp == 0) TR(t, 6);
+        cp_async_wait_all();
+        __syncwarp();
+        if (warp == 0) TR(t, 7);
+        uint32_t key, d[32];
+        bool wide_lane = false, wide = false;
+        const T base = col_deltas<W>(raw, m, d, wide_lane);              // E1
+        if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
+        if (!wide) key = quad_choose_b<W>(d);                            // E2
+        else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(img));
+        if (m <= 0) key = 0;
+        if (l == 0) s_key[j] = key;
+        if (warp == 0) TR(t, 8);
+        bar_arrive(1, kEncThreads);
+
+        const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u, bytes = key >> 14;
+        if (!wide && __any_sync(kFull, n_exc > 0)) col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, n_exc);
+        if (!wide) {                                                     // E4 into the image area
+            if (key != 0 && b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
+            if (l == 0) {                                                // block header (FORMAT.md §2)
+                reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
+                reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
             }
             __syncwarp();
         }
+        if (warp == 0) TR(t, 9);
+        bar_sync(2, kEncThreads);                                        // s_at of tile t and the next tile are posted
+        if (warp == 0) TR(t, 10);
+
+        const unsigned long long at = key != 0 ? s_at[j] : kSkip;
+        if (s_tile[p ^ 1] != kNoTile) quad_prefetch<W>(slot, ids + s_xoff[p ^ 1][j], s_m[p ^ 1][j]);   // same slots
+        if (warp == 0) TR(t, 12);
+        if constexpr (W == 64) {
+            if (wide) {                                                  // slow path: straight to global memory
+                late_emit<64>(reinterpret_cast<const uint64_t*>(x), m, key, at != kSkip ? a.out + at : nullptr,
+                          reinterpret_cast<uint64_t*>(area + EncSmem<W>::kStageChunks));
+            }
+        }
+        if (!wide && at != kSkip) {
+            const uint4* src = reinterpret_cast<const uint4*>(img);
+            uint4* dst = reinterpret_cast<uint4*>(a.out + at);
+            for (uint32_t k = l; k < bytes / 16; k += 4) __stcs(dst + k, src[k]);
+        }
+        __syncwarp();
+        if (warp == 0) TR(t, 11);
+        p ^= 1;
     }
 }
 
-// ---- stream headers, directory tails, E5 raw passthrough, out_offsets --------------------
+// ---- stream headers, directory tails, E5 raw passthrough, out_offsets (batch / degenerate calls) ----
 template <int W>
 __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
+    pdl_wait();
     const unsigned long long total_blocks = a.ws.hdr->total_blocks, grand16 = a.ws.hdr->grand16;
     bool ok = a.ws.hdr->ok != 0;
     if (ok && a.ws.hdr->total_out > a.out_cap) {
@@ -359,29 +461,54 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     }
 }
 
+// Launch with the programmatic-stream-serialization attribute: the kernel may start before its
+// predecessor in the stream has finished; it calls griddepcontrol.wait before consuming its output.
+template <typename A>
+static cudaError_t launch_dep(void (*kern)(A), int grid, int block, size_t smem, cudaStream_t s, const A& args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args);
+}
+
 template <int W>
 static bfsc_status launch_encode(const EncArgs& a, cudaStream_t s) {
-    constexpr int kThreads = EncCfg<W>::kWarps * 32;
-    constexpr size_t kSmem = sizeof(QuadStage<W>) * EncCfg<W>::kWarps;
-    static int grid = 0;                          // persistent grid: all CTAs resident
-    if (grid == 0) {
+    constexpr size_t kSmem = EncSmem<W>::kBytes;
+    static int max_grid = 0;                      // persistent grid: all CTAs resident
+    if (max_grid == 0) {
         int per_sm = 0, dev = 0, sms = kNumSM;
-        if (cudaFuncSetAttribute(k_enc_fused<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_enc_tiles<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
             return BFSC_ERR_CUDA;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_fused<W>, kThreads, kSmem) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_tiles<W>, kEncThreads, kSmem) != cudaSuccess ||
             per_sm < 1)
             per_sm = 1;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        grid = sms * per_sm;
+        max_grid = sms * per_sm;
     }
+    constexpr unsigned long long E = W / 8;
+    const bool single = a.in_off == nullptr;
+    const bool degenerate = single && (a.n_single == 0 || a.n_single * E < a.thr);   // no block: header (+ raw copy) only
     k_enc_plan<W><<<1, 1024, 0, s>>>(a);
     BFSC_LAUNCH_CHECK();
-    k_enc_fused<W><<<grid, kThreads, kSmem, s>>>(a);
-    BFSC_LAUNCH_CHECK();
-    const uint32_t sgrid = a.n_buf < (uint32_t)(kNumSM * 8) ? a.n_buf : (uint32_t)(kNumSM * 8);
-    k_enc_streams<W><<<sgrid ? sgrid : 1, 256, 0, s>>>(a);
-    BFSC_LAUNCH_CHECK();
+    if (!degenerate) {
+        int grid = max_grid;
+        if (single) {
+            const unsigned long long n_tiles = ((a.n_single + kBlk - 1) / kBlk + kTileR - 1) / kTileR;
+            if (n_tiles < (unsigned long long)grid) grid = (int)n_tiles;
+        }
+        if (launch_dep(k_enc_tiles<W>, grid, kEncThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        BFSC_LAUNCH_CHECK();
+    }
+    if (!single || degenerate) {
+        const uint32_t sgrid = a.n_buf < (uint32_t)(kNumSM * 8) ? a.n_buf : (uint32_t)(kNumSM * 8);
+        if (launch_dep(k_enc_streams<W>, sgrid ? (int)sgrid : 1, 256, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        BFSC_LAUNCH_CHECK();
+    }
     return BFSC_OK;
 }
 
@@ -395,12 +522,18 @@ static bfsc_status encode_common(const void* d_ids, const uint64_t* d_in_off, si
     EncArgs a;
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.ids = d_ids; a.in_off = (const unsigned long long*)d_in_off; a.n_single = n_single;
-    a.n_buf = (uint32_t)n_buf; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
+    a.n_buf = (uint32_t)n_buf; a.pad0 = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
     a.out_off = (unsigned long long*)d_out_off; a.out_total = (unsigned long long*)d_out_total; a.status = d_status;
     return t == BFSC_U32 ? launch_encode<32>(a, (cudaStream_t)stream) : launch_encode<64>(a, (cudaStream_t)stream);
 }
 
 }  // namespace bfsc
+
+#ifdef BFSC_TRACE
+extern "C" int bfsc_debug_trace(unsigned long long* h_out, size_t n_words) {
+    return (int)cudaMemcpyFromSymbol(h_out, bfsc::g_trace, n_words * 8);
+}
+#endif
 
 extern "C" bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
                                      void* d_out, size_t out_capacity, uint64_t* d_out_bytes, void* d_workspace,

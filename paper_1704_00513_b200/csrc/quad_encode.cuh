@@ -9,7 +9,7 @@
 //   column owner: lane c packs column c's bit stream (FORMAT.md payload) sequentially from the
 //                 staged values in shared memory.
 #pragma once
-#include "block_encode.cuh"
+#include "common.cuh"
 
 namespace bfsc {
 
@@ -114,34 +114,24 @@ __device__ __forceinline__ uint32_t quad_max(uint32_t x) {
 // thresholds at which a value of width top-t is an exception); the chain of windows stops when
 // the exceptions above the window alone cost at least the best size, and jumps over widths no
 // value has. Returns key = size << 14 | (64 - b) << 7 | n_exc in every lane of the quad.
-template <int W, typename DT>
-__device__ __forceinline__ uint32_t quad_choose_b(const DT (&d)[8][4]) {
+template <int W>
+__device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
     const int l = quad_l();
-    constexpr int kBits = 8 * (int)sizeof(DT);
     int top;
     {
-        DT o = 0;
+        uint32_t o = 0;
 #pragma unroll
-        for (int i = 0; i < 8; i++) o |= d[i][0] | d[i][1] | d[i][2] | d[i][3];
-        uint32_t lo = (uint32_t)o, hi = 0;
-        if constexpr (sizeof(DT) == 8) hi = (uint32_t)(o >> 32);
-        lo = quad_or(lo);
-        if constexpr (sizeof(DT) == 8) hi = quad_or(hi);
-        top = hi ? 64 - __clz(hi) : 32 - __clz(lo);
+        for (int i = 0; i < 32; i++) o |= d[i];
+        top = 32 - __clz(quad_or(o));
     }
     uint32_t cnt_above = 0, best = 0xffffffffu;
     bool active = true;
     while (true) {
         uint32_t acc[3] = {0u, 0u, 0u};
-        const int off = top - kBits;                 // t = top - width = clz + off
+        const int off = top - 32;                    // t = top - width = clz + off
 #pragma unroll
-        for (int i = 0; i < 8; i++)
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-                int clz;
-                if constexpr (sizeof(DT) == 8) clz = __clzll(d[i][c]); else clz = __clz(d[i][c]);
-                acc[i / 3] += shl32(0x11111111u, (uint32_t)(4 * (clz + off)));   // t < 0 or t >= 8: shift clamps to 0
-            }
+        for (int i = 0; i < 32; i++)                 // t < 0 or t >= 8: the shift clamps to 0
+            acc[i / 12] += shl32(0x11111111u, (uint32_t)(4 * (__clz(d[i]) + off)));
         uint32_t lo = (acc[0] & 0x0f0f0f0fu) + (acc[1] & 0x0f0f0f0fu) + (acc[2] & 0x0f0f0f0fu);
         uint32_t hi = ((acc[0] >> 4) & 0x0f0f0f0fu) + ((acc[1] >> 4) & 0x0f0f0f0fu) + ((acc[2] >> 4) & 0x0f0f0f0fu);
         lo = quad_add(lo);                           // bytes: exceptions added at s = 1,3,5,7 (b = top - s)
@@ -163,171 +153,231 @@ __device__ __forceinline__ uint32_t quad_choose_b(const DT (&d)[8][4]) {
         if (!__any_sync(kFull, active)) break;
         uint32_t below = 0;                          // widest value not above top - 8
 #pragma unroll
-        for (int i = 0; i < 8; i++)
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-                const uint32_t w = (uint32_t)bitlen<DT>(d[i][c]);
-                below = max(below, (int)w <= top - 8 ? w : 0u);
-            }
+        for (int i = 0; i < 32; i++) {
+            const uint32_t w = 32u - (uint32_t)__clz(d[i]);
+            below = max(below, (int)w <= top - 8 ? w : 0u);
+        }
         below = quad_max(below);
         if (active) { top = (int)below; cnt_above = n_bot; }
     }
     return best;
 }
 
+// ---- E4: staging geometry ----------------------------------------------------------------
+// Per warp: a staging area (the batch's 128 deltas per block, row-major) and an image area (the
+// assembled block: header | payload | exceptions). Both hold 8 slots of 33 16-byte chunks; slot q
+// starts at chunk 33 q + 3 ((q + 1) >> 1) = {0,36,69,105,138,174,207,243}: the residues mod 8 are
+// {0,4,5,1,2,6,7,3}, so that (i) the 8 quads' column reads/writes (32-bit, same row) hit 8 distinct
+// 16-byte bank groups and (ii) the two quads of a 128-bit phase (2h, 2h+1) are 4 groups apart —
+// row-owner 128-bit accesses are conflict-free too.
+constexpr int kSlotChunks = 33;
+constexpr int kAreaChunks = 243 + kSlotChunks;                  // 276 chunks = 4416 B
+__device__ __forceinline__ int quad_slot_chunk(int q) { return 33 * q + 3 * ((q + 1) >> 1); }
 
-// ---- E4: staging -----------------------------------------------------------------------
-// Per-warp shared memory: the batch's masked values (row-major per block, padded stride) and the
-// batch's assembled blocks (header | payload | exceptions), canonical size <= 16 + 16 W each.
-template <int W>
-struct QuadStage {
-    static constexpr int kOutStride = 16 + 16 * W;              // bytes; /4 == 4 (mod 32) words
-    static constexpr int kValWords = kValStride * (W / 32);     // u64 values take two words
-    alignas(16) uint32_t vals[kQuadBlocks * kValWords];
-    alignas(16) unsigned char out[kQuadBlocks * kOutStride];
-};
-
-// masked low parts of the quad's rows -> vals (row owner, 128-bit stores)
-template <typename DT>
-__device__ __forceinline__ void quad_stage_vals(uint32_t* __restrict__ vq, const DT (&d)[8][4], uint32_t b) {
+// row owner -> staging: the quad's 128 deltas, row r = 4i + l at chunk r (128-bit stores)
+__device__ __forceinline__ void quad_stage_deltas(uint4* __restrict__ slot, const uint32_t (&d)[8][4]) {
     const int l = quad_l();
-    if constexpr (sizeof(DT) == 4) {
-        const uint32_t mask = b >= 32 ? 0xffffffffu : ((1u << b) - 1u);
 #pragma unroll
-        for (int i = 0; i < 8; i++)
-            reinterpret_cast<uint4*>(vq)[4 * i + l] =
-                make_uint4(d[i][0] & mask, d[i][1] & mask, d[i][2] & mask, d[i][3] & mask);
-    } else {
-        const uint64_t mask = b >= 64 ? ~0ull : ((1ull << b) - 1ull);
-#pragma unroll
-        for (int i = 0; i < 8; i++) {
-            ulonglong2* p = reinterpret_cast<ulonglong2*>(vq) + 2 * (4 * i + l);
-            p[0] = make_ulonglong2(d[i][0] & mask, d[i][1] & mask);
-            p[1] = make_ulonglong2(d[i][2] & mask, d[i][3] & mask);
-        }
-    }
+    for (int i = 0; i < 8; i++) slot[4 * i + l] = make_uint4(d[i][0], d[i][1], d[i][2], d[i][3]);
 }
 
-// Exceptions of the quad's block (n_exc > 0): positions ascending + high parts, FORMAT.md §2.
-// The quad builds the block's 128-bit exception bitmap, parks the high parts in the (not yet
-// used) vals area, then walks the bitmap: exception number e is written by lane e mod 4.
-// Must be called by the whole warp (contains __syncwarp); quads with n_exc == 0 idle through it.
-template <int W, typename DT>
-__device__ __forceinline__ void quad_exceptions(uint32_t* __restrict__ vq, unsigned char* __restrict__ oq,
-                                                const DT (&d)[8][4], uint32_t b, uint32_t n_exc) {
-    using T = typename IdT<W>::T;
-    constexpr uint32_t E = W / 8;
-    const int l = quad_l();
-    const bool on = n_exc > 0;
-    uint32_t bm[4] = {0u, 0u, 0u, 0u};
-    if (on) {
+// staging -> column owner: lane c of the quad gets u[r] = d[4r + c]
+__device__ __forceinline__ void col_load(const uint32_t* __restrict__ slot, uint32_t (&u)[32]) {
+    const int c = quad_l();
 #pragma unroll
-        for (int i = 0; i < 8; i++) {
-            DT h[4];
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-                h[c] = shr_clamp<DT>(d[i][c], b);
-                if (h[c] != 0) bm[i >> 1] |= 1u << (16 * (i & 1) + 4 * l + c);   // j = 16 i + 4 l + c
-            }
-            if constexpr (sizeof(DT) == 4) {
-                reinterpret_cast<uint4*>(vq)[4 * i + l] = make_uint4(h[0], h[1], h[2], h[3]);
-            } else {
-                ulonglong2* p = reinterpret_cast<ulonglong2*>(vq) + 2 * (4 * i + l);
-                p[0] = make_ulonglong2(h[0], h[1]);
-                p[1] = make_ulonglong2(h[2], h[3]);
-            }
-        }
-        unsigned char* e = oq + 16 + 16 * b;                     // zero the area: pads must be 0
-        const uint32_t eb = exc_bytes<W>(n_exc);
-        for (uint32_t x = l; x < eb / 16; x += 4) reinterpret_cast<uint4*>(e)[x] = make_uint4(0, 0, 0, 0);
-    }
-#pragma unroll
-    for (int w = 0; w < 4; w++) bm[w] = quad_or(bm[w]);
-    __syncwarp();
-    if (on) {
-        unsigned char* e = oq + 16 + 16 * b;
-        T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
-        const DT* hv = reinterpret_cast<const DT*>(vq);
-        uint32_t rank = 0;
-#pragma unroll
-        for (int w = 0; w < 4; w++) {
-            uint32_t mk = bm[w];
-            while (mk) {
-                const uint32_t p = 32u * w + (uint32_t)__ffs(mk) - 1u;
-                mk &= mk - 1u;
-                if ((rank & 3u) == (uint32_t)l) {
-                    e[rank] = (unsigned char)p;
-                    high[rank] = (T)hv[p];
-                }
-                rank++;
-            }
-        }
-    }
-    __syncwarp();
+    for (int r = 0; r < 32; r++) u[r] = slot[4 * r + c];
 }
 
-// One column of the payload, packed sequentially by its owner lane (b <= 32, 32-bit values).
-// For b <= 16 (<= 8) neighbouring rows are first merged into 2b- (4b-) bit items with one IMAD each,
-// which halves (quarters) the length of the sequential part.
+// One column of the payload (FORMAT.md §2 "Payload"), packed sequentially by its owner lane from
+// registers: row r's low b bits at stream bits [r b, (r+1) b); word k goes to outp[4k].
+// For b <= 8 (<= 16) four (two) neighbouring rows are first merged into one item with IMADs, which
+// quarters (halves) the sequential part. b in 1..32.
 #define BFSC_EMIT_ITEM(xv)                                               \
     {                                                                    \
         const uint32_t x_ = (xv);                                        \
         acc |= x_ << have;                                               \
-        uint32_t nh = have + bw;                                         \
-        if (nh >= 32u) {                                                 \
+        const uint32_t hi_ = __funnelshift_l(x_, 0u, have);              \
+        const uint32_t nh_ = have + bw;                                  \
+        if (nh_ >= 32u) {                                                \
             *outp = acc;                                                 \
             outp += 4;                                                   \
-            acc = shr32(x_, 32u - have);                                 \
-            nh -= 32u;                                                   \
+            acc = hi_;                                                   \
         }                                                                \
-        have = nh;                                                       \
+        have = nh_ & 31u;                                                \
     }
 
-__device__ __forceinline__ void quad_pack_column32(const uint32_t* __restrict__ col /* row r at col[4r] */,
-                                                   uint32_t* __restrict__ outp /* word k at outp[4k] */, uint32_t b) {
-    if (b == 0) return;
-    uint32_t u[32];
-#pragma unroll
-    for (int r = 0; r < 32; r++) u[r] = col[4 * r];
+__device__ __forceinline__ void col_pack32(const uint32_t (&u)[32], uint32_t b, uint32_t* __restrict__ outp) {
+    const uint32_t mask = 0xffffffffu >> (32u - b);
     uint32_t acc = 0, have = 0;
     if (b <= 8) {
         const uint32_t m1 = 1u << b, m2 = 1u << (2 * b), bw = 4 * b;
 #pragma unroll
         for (int p = 0; p < 8; p++) {
-            const uint32_t a0 = u[4 * p] + u[4 * p + 1] * m1, a1 = u[4 * p + 2] + u[4 * p + 3] * m1;
+            const uint32_t a0 = (u[4 * p] & mask) + (u[4 * p + 1] & mask) * m1;
+            const uint32_t a1 = (u[4 * p + 2] & mask) + (u[4 * p + 3] & mask) * m1;
             BFSC_EMIT_ITEM(a0 + a1 * m2)
         }
     } else if (b <= 16) {
         const uint32_t m1 = 1u << b, bw = 2 * b;
 #pragma unroll
-        for (int p = 0; p < 16; p++) BFSC_EMIT_ITEM(u[2 * p] + u[2 * p + 1] * m1)
+        for (int p = 0; p < 16; p++) BFSC_EMIT_ITEM((u[2 * p] & mask) + (u[2 * p + 1] & mask) * m1)
     } else {
         const uint32_t bw = b;
 #pragma unroll
-        for (int r = 0; r < 32; r++) BFSC_EMIT_ITEM(u[r])
+        for (int r = 0; r < 32; r++) BFSC_EMIT_ITEM(u[r] & mask)
     }
 }
 #undef BFSC_EMIT_ITEM
 
-// Wide values (u64 deltas, any b <= 64): plain sequential packer with a 128-bit window.
-__device__ __forceinline__ void quad_pack_column64(const uint64_t* __restrict__ col /* row r at col[4r] */,
-                                                   uint32_t* __restrict__ outp, uint32_t b) {
-    if (b == 0) return;
-    uint64_t lo = 0, hi = 0;
-    uint32_t have = 0;
-    for (int r = 0; r < 32; r++) {
-        const uint64_t x = col[4 * r];
-        lo |= shl64(x, have);
-        hi |= have ? shr64(x, 64u - have) : 0ull;     // have < 32 here
-        have += b;
-        while (have >= 32u) {
-            *outp = (uint32_t)lo;
-            outp += 4;
-            lo = (lo >> 32) | (hi << 32);
-            hi >>= 32;
-            have -= 32u;
+// Exceptions of the quad's block (FORMAT.md §2 "Exceptions"), column owner, 32-bit deltas (for
+// W = 64 the high parts are zero-extended). e = image + 16 + 16 b. Exception number `rank` (ascending
+// position j = 4r + c) is written by the lane that owns it: each lane builds the 32-bit mask of its
+// own exceptions (bit r), the quad exchanges the four masks, and rank = number of exceptions in
+// earlier rows plus those of lower columns in the same row. The high part comes from the staged
+// delta (dynamic index: shared memory, not registers).
+// Must be called by the whole warp (shuffles, __syncwarp); quads with n_exc == 0 idle through it.
+template <int W>
+__device__ __forceinline__ void col_exceptions(const uint32_t (&u)[32], const uint32_t* __restrict__ slot,
+                                               unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc) {
+    using T = typename IdT<W>::T;
+    constexpr uint32_t E = W / 8;
+    const int lane = threadIdx.x & 31, c = lane & 3;
+    const bool on = n_exc > 0;                               // then b < 32
+    uint32_t mk = 0;
+    if (on) {
+        const uint32_t mask = (1u << b) - 1u;
+#pragma unroll
+        for (int r = 0; r < 32; r++)
+            if (u[r] > mask) mk |= 1u << r;
+        const uint32_t eb = exc_bytes<W>(n_exc);             // zero the area: pads must be 0
+        for (uint32_t x = c; x < eb / 16; x += 4) reinterpret_cast<uint4*>(e)[x] = make_uint4(0, 0, 0, 0);
+    }
+    const uint32_t M0 = __shfl_sync(kFull, mk, (lane & ~3) + 0), M1 = __shfl_sync(kFull, mk, (lane & ~3) + 1);
+    const uint32_t M2 = __shfl_sync(kFull, mk, (lane & ~3) + 2), M3 = __shfl_sync(kFull, mk, (lane & ~3) + 3);
+    __syncwarp();
+    if (on) {
+        T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
+        uint32_t rest = mk;
+        while (rest) {
+            const uint32_t r = (uint32_t)__ffs(rest) - 1u;
+            rest &= rest - 1u;
+            const uint32_t below = (1u << r) - 1u, incl = (2u << r) - 1u;
+            const uint32_t rank = __popc(M0 & (c > 0 ? incl : below)) + __popc(M1 & (c > 1 ? incl : below)) +
+                                  __popc(M2 & (c > 2 ? incl : below)) + __popc(M3 & below);
+            const uint32_t pos = 4u * r + (uint32_t)c;
+            e[rank] = (unsigned char)pos;
+            high[rank] = (T)(slot[pos] >> b);
         }
     }
+    __syncwarp();
+}
+
+// ---- E1 (column owner): raw IDs staged by cp.async, deltas computed by the lane that packs them ----
+// The quad's block is copied global -> shared as ALIGNED 16-byte chunks (cp.async.cg, no registers,
+// any element alignment: the block's first ID sits e elements into chunk 0). A slot holds
+// kSlotChunks (u32) / 2 kSlotChunks (u64) chunks; u64 slots are dense (66 q: the residues mod 8 of
+// a 16-lane phase's four quads are {0,2,4,6}), u32 slots use quad_slot_chunk.
+template <int W> __device__ __forceinline__ int raw_slot_chunk(int q) {
+    if constexpr (W == 32) return quad_slot_chunk(q); else return 2 * kSlotChunks * q;
+}
+template <int W> struct RawCfg { static constexpr int kAreaChunks = (W == 32) ? bfsc::kAreaChunks : 16 * kSlotChunks; };
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// x = block's first ID (m valid IDs, m <= 0: nothing to copy). Lane l of the quad copies chunks l, l+4, ...
+template <int W>
+__device__ __forceinline__ void quad_prefetch(uint4* __restrict__ slot, const typename IdT<W>::T* __restrict__ x, int m) {
+    using T = typename IdT<W>::T;
+    constexpr int EPC = 16 / (int)sizeof(T);                    // elements per chunk
+    constexpr int kRounds = kBlk / EPC / 4;                      // 8 (u32) / 16 (u64) full rounds, + 1 for e > 0
+    if (m <= 0) return;
+    const int l = quad_l();
+    const uintptr_t addr = reinterpret_cast<uintptr_t>(x);
+    const int e = (int)(addr & 15) / (int)sizeof(T);
+    const uint4* src = reinterpret_cast<const uint4*>(addr & ~(uintptr_t)15) + l;
+    const int nchunk = (e + m + EPC - 1) / EPC;
+    if (nchunk == kBlk / EPC) {
+#pragma unroll
+        for (int i = 0; i < kRounds; i++) cp_async16(slot + 4 * i + l, src + 4 * i);
+    } else {
+#pragma unroll
+        for (int i = 0; i <= kRounds; i++)
+            if (4 * i + l < nchunk) cp_async16(slot + 4 * i + l, src + 4 * i);
+    }
+}
+
+// Column owner c: d[r] = delta of ID j = 4r + c (d_0 = 0, 0 beyond m), from the staged
+// raw IDs. Returns the block's first ID (valid in lane c = 0) and, for u64, whether some delta of
+// the lane does not fit 32 bits.
+template <int W>
+__device__ __forceinline__ typename IdT<W>::T col_deltas(const typename IdT<W>::T* __restrict__ raw /* slot + e */, int m,
+                                                         uint32_t (&d)[32], bool& wide_lane) {
+    using T = typename IdT<W>::T;
+    const int c = quad_l();
+    const T* p = raw + c;
+    T first = p[0];
+    uint32_t hi_or = 0;
+#pragma unroll
+    for (int r = 0; r < 32; r++) {
+        const T cur = (r == 0) ? first : p[4 * r];
+        const T prev = (r == 0) ? p[c == 0 ? 0 : -1] : p[4 * r - 1];
+        const T dd = cur - prev;
+        d[r] = (uint32_t)dd;
+        if constexpr (W == 64) hi_or |= (uint32_t)(dd >> 32);
+    }
+    if (!__all_sync(kFull, m == kBlk)) {
+        hi_or = 0;
+#pragma unroll
+        for (int r = 0; r < 32; r++) {
+            if (4 * r + c >= m) d[r] = 0;
+            if constexpr (W == 64) { if (4 * r + c < m && r > 0) hi_or |= (uint32_t)((p[4 * r] - p[4 * r - 1]) >> 32); }
+        }
+        if constexpr (W == 64) { if (c > 0 && c < m) hi_or |= (uint32_t)((p[0] - p[-1]) >> 32); }
+    }
+    wide_lane = hi_or != 0;
+    return first;
+}
+
+
+// Exceptions as col_exceptions, but the high part is recomputed from the staged RAW IDs.
+template <int W>
+__device__ __forceinline__ void col_exceptions_raw(const uint32_t (&u)[32], const typename IdT<W>::T* __restrict__ raw,
+                                                   unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc) {
+    using T = typename IdT<W>::T;
+    constexpr uint32_t E = W / 8;
+    const int lane = threadIdx.x & 31, c = lane & 3;
+    const bool on = n_exc > 0;                               // then b < 32
+    uint32_t mk = 0;
+    if (on) {
+        const uint32_t mask = (1u << b) - 1u;
+#pragma unroll
+        for (int r = 0; r < 32; r++)
+            if (u[r] > mask) mk |= 1u << r;
+        const uint32_t eb = exc_bytes<W>(n_exc);             // zero the area: pads must be 0
+        for (uint32_t x = c; x < eb / 16; x += 4) reinterpret_cast<uint4*>(e)[x] = make_uint4(0, 0, 0, 0);
+    }
+    const uint32_t M0 = __shfl_sync(kFull, mk, (lane & ~3) + 0), M1 = __shfl_sync(kFull, mk, (lane & ~3) + 1);
+    const uint32_t M2 = __shfl_sync(kFull, mk, (lane & ~3) + 2), M3 = __shfl_sync(kFull, mk, (lane & ~3) + 3);
+    __syncwarp();
+    if (on) {
+        T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
+        uint32_t rest = mk;
+        while (rest) {
+            const uint32_t r = (uint32_t)__ffs(rest) - 1u;
+            rest &= rest - 1u;
+            const uint32_t below = (1u << r) - 1u, incl = (2u << r) - 1u;
+            const uint32_t rank = __popc(M0 & (c > 0 ? incl : below)) + __popc(M1 & (c > 1 ? incl : below)) +
+                                  __popc(M2 & (c > 2 ? incl : below)) + __popc(M3 & below);
+            const uint32_t pos = 4u * r + (uint32_t)c;       // > 0: d_0 = 0 is never an exception
+            e[rank] = (unsigned char)pos;
+            high[rank] = (T)(raw[pos] - raw[pos - 1]) >> b;
+        }
+    }
+    __syncwarp();
 }
 
 }  // namespace bfsc
