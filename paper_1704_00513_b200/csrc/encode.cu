@@ -128,48 +128,40 @@ __device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.ar
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 // Exclusive prefix (16-byte units) of tile t > 0: aggregates of t-1, t-2, ... down to the nearest
-// tile whose inclusive prefix is known. One warp. The states of the 512 nearest predecessors — more
-// than the tiles in flight — are fetched up front (16 independent loads per lane: ONE L2 round
-// trip); 32 ballots find the nearest posted prefix; every lane sums its own entries and a single
-// warp reduction ends it (a reduction per chunk of 32 made this the critical path of the kernel).
-constexpr int kLookChunks = 16;
+// tile whose inclusive prefix is known. One warp. The states of the 256 nearest predecessors are
+// fetched up front (8 independent loads per lane: ONE L2 round trip), then examined 32 at a time
+// with two ballots per chunk; every lane sums its own entries and a single warp reduction ends it.
+// A chunk with an entry that is not posted yet is polled alone (a few instructions per poll).
+constexpr int kLookChunks = 8;
 __device__ __forceinline__ unsigned long long lookback(const unsigned long long* __restrict__ state,
                                                        unsigned long long t, int lane) {
     unsigned long long acc = 0;
     long long idx = (long long)t - 1 - lane;
-    while (true) {
+    bool done = false;
+    while (!done) {
         unsigned long long s[kLookChunks];
 #pragma unroll
         for (int r = 0; r < kLookChunks; r++)
             s[r] = (idx - 32 * r >= 0) ? ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]) : kFlagPre;
-        int rs, stop;
-        while (true) {
-            uint32_t hit[kLookChunks], rdy[kLookChunks];
 #pragma unroll
-            for (int r = 0; r < kLookChunks; r++) {
-                hit[r] = __ballot_sync(kFull, (s[r] >> 62) == 2);
-                rdy[r] = __ballot_sync(kFull, (s[r] >> 62) != 0);
+        for (int r = 0; r < kLookChunks; r++) {
+            if (!done) {
+                unsigned long long v = s[r];
+                while (true) {
+                    const uint32_t hit = __ballot_sync(kFull, (v >> 62) == 2);
+                    const uint32_t rdy = __ballot_sync(kFull, (v >> 62) != 0);
+                    const int stop = hit ? __ffs(hit) - 1 : 31;
+                    const uint32_t need = 0xffffffffu >> (31 - stop);
+                    if ((rdy & need) == need) {
+                        if (lane <= stop) acc += v & kValMask;
+                        done = hit != 0;
+                        break;
+                    }
+                    __nanosleep(32);
+                    if ((v >> 62) == 0) v = ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]);
+                }
             }
-            rs = kLookChunks; stop = 31;
-#pragma unroll
-            for (int r = kLookChunks - 1; r >= 0; r--)
-                if (hit[r]) { rs = r; stop = __ffs(hit[r]) - 1; }
-            bool ok = true;                                      // everything up to the stop entry is posted
-#pragma unroll
-            for (int r = 0; r < kLookChunks; r++) {
-                const uint32_t need = r < rs ? kFull : (r == rs ? (0xffffffffu >> (31 - stop)) : 0u);
-                ok = ok && ((rdy[r] & need) == need);
-            }
-            if (ok) break;
-            __nanosleep(64);
-#pragma unroll
-            for (int r = 0; r < kLookChunks; r++)
-                if ((s[r] >> 62) == 0) s[r] = ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]);
         }
-#pragma unroll
-        for (int r = 0; r < kLookChunks; r++)
-            if (r < rs || (r == rs && lane <= stop)) acc += s[r] & kValMask;
-        if (rs < kLookChunks) break;
         idx -= 32 * kLookChunks;
     }
 #pragma unroll
@@ -177,27 +169,36 @@ __device__ __forceinline__ unsigned long long lookback(const unsigned long long*
     return acc;
 }
 
+constexpr int kImgCap = 256;                                  // bytes of a block image the fast path can hold
+constexpr int kImgSlotChunks = 17;                            // slot stride (16-B chunks): 17 q mod 8 are all distinct
+constexpr int kImgBufChunks = kQuadBlocks * kImgSlotChunks;   // one image buffer of a warp
+
 template <int W> struct EncSmem {
     static constexpr int kStageChunks = RawCfg<W>::kAreaChunks;              // per worker warp: staged raw IDs
-    static constexpr int kWarpChunks = kStageChunks + kAreaChunks;           // + image area
+    static constexpr int kWarpChunks = kStageChunks + 2 * kImgBufChunks;     // + two image buffers (tile parity)
     static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
 };
+static_assert(RawCfg<32>::kAreaChunks * 16 >= 4 * kLateSlotWords64 * 8, "late_emit scratch");
+
+enum { kBarSizes = 1, kBarOffsets = 3 };                      // named barriers: +parity of the CTA's tile count
 
 template <int W>
-__global__ void __launch_bounds__(kEncThreads, (W == 32) ? 3 : 2) k_enc_tiles(EncArgs a) {
+__global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
-    extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | image area
-    __shared__ uint32_t s_key[kTileR];                   // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
-    __shared__ unsigned long long s_at[kTileR];          // scan warp: final byte offset of the block, or kSkip
+    extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | image buffer 0 | image buffer 1
+    __shared__ uint32_t s_key[2][kTileR];                // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
+    __shared__ unsigned long long s_at[2][kTileR];       // scan warp: final byte offset of the block, or kSkip
     __shared__ uint32_t s_off16[kTileR];                 // exclusive scan of the sizes inside the tile (16-B units)
-    __shared__ int s_m[2][kTileR];                       // tile bookkeeping, two parities: valid IDs of each block (0 = none)
-    __shared__ unsigned long long s_xoff[2][kTileR];     // element offset of the block's first ID
-    __shared__ uint32_t s_buf[2][kTileR];                // buffer of each block (batch calls)
-    __shared__ unsigned long long s_tile[2];             // tile of each parity, kNoTile = done
+    __shared__ int s_m[4][kTileR];                       // ring of tile bookkeeping: valid IDs of each block (0 = none)
+    __shared__ unsigned long long s_xoff[4][kTileR];     // element offset of the block's first ID
+    __shared__ uint32_t s_buf[4][kTileR];                // buffer of each block (batch calls)
+    __shared__ unsigned long long s_tile[4];             // tile of each ring slot, kNoTile = done
+    __shared__ unsigned int s_agg[2];                    // arrivals << 24 | sum of the worker warps' sizes (16-B units)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool batch = a.in_off != nullptr;
     const T* ids = reinterpret_cast<const T*>(a.ids);
+    if (threadIdx.x < 2) s_agg[threadIdx.x] = 0;
 
     if (warp == kEncWorkers) {
         // =============================== scan warp ===============================
@@ -235,22 +236,22 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 3 : 2) k_enc_tiles(En
             }
         };
 
-        // Tickets are drawn ONE per tile and always at the same point of the pipeline (right after the
-        // previous tile's sizes are in): a lower tile number then means "sizes ready earlier", so a
-        // look-back rarely has to wait. Drawing ahead (two tickets at once) inverts that order.
-        unsigned long long t = draw();
+        // A CTA works on tile k (sizes, pack) while the scan warp resolves the offsets of tile k-1, so
+        // tickets are drawn two tiles ahead: always at the same point of the pipeline, so that a lower
+        // tile number means "sizes posted earlier" and a look-back rarely has to wait.
+        unsigned long long t = draw(), t1 = t != kNoTile ? draw() : kNoTile;
         prep(t, 0);
-        __syncthreads();                                 // barrier 0: the first tile is posted
-        int p = 0;
-        while (t != kNoTile) {
+        prep(t1, 1);
+        __syncthreads();                                 // barrier 0: the first two tiles are posted
+        for (int k = 0; t != kNoTile; k++) {
+            const int kp = k & 1;
             TR(t, 0);
-            bar_sync(1, kEncThreads);                    // the workers' sizes of tile t are in s_key
-            TR(t, 1);
-            unsigned int ticket = 0;                     // next tile: the atomic's latency hides behind the scan
-            if (lane == 0) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+            bar_sync(kBarSizes + kp, kEncThreads);       // the workers' sizes of tile t are in s_key[kp]
+            unsigned int ticket = 0xffffffffu;           // tile k+2: the atomic's latency hides behind the scan
+            if (lane == 0 && t1 != kNoTile) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
 
             // E3: intra-tile scan (2 consecutive blocks per lane)
-            const uint32_t k0 = s_key[2 * lane], k1 = s_key[2 * lane + 1];
+            const uint32_t k0 = s_key[kp][2 * lane], k1 = s_key[kp][2 * lane + 1];
             const uint32_t z0 = k0 >> 18, z1 = k1 >> 18;
             uint32_t inc = z0 + z1;
 #pragma unroll
@@ -261,8 +262,7 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 3 : 2) k_enc_tiles(En
             const uint32_t off0 = inc - z0 - z1, off1 = off0 + z0;
             const unsigned long long agg = __shfl_sync(kFull, inc, 31);
             s_off16[2 * lane] = off0; s_off16[2 * lane + 1] = off1;
-            if (t > 0 && lane == 0) st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagAgg | agg);
-            TR(t, 2);
+            TR(t, 2);                                    // (the aggregate was published by the last worker warp)
             const unsigned long long excl = t > 0 ? lookback(a.ws.tile_state, t, lane) : 0ull;
             TR(t, 3);
             if (lane == 0) {
@@ -287,7 +287,7 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 3 : 2) k_enc_tiles(En
                     unsigned long long first = 0, f0 = 0, f1 = f1_single, S = 0;
                     uint32_t i = 0;
                     if (batch) {
-                        i = s_buf[p][jj];
+                        i = s_buf[k & 3][jj];
                         first = a.ws.blk_first[i]; f0 = a.ws.fixed_prefix[i]; f1 = a.ws.fixed_prefix[i + 1];
                         if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
                         else if (i > 0) {                // published by the tile that owns the stream's first block
@@ -321,82 +321,117 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 3 : 2) k_enc_tiles(En
                         if (a.out_total) *a.out_total = at != kSkip ? tot : 0ull;
                     }
                 }
-                s_at[jj] = at;
+                s_at[kp][jj] = at;
             }
-            TR(t, 13);
             ticket = __shfl_sync(kFull, ticket, 0);
-            const unsigned long long nt = ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
-            prep(nt, p ^ 1);
+            const unsigned long long t2 = ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
+            prep(t2, (k + 2) & 3);
             TR(t, 4);
-            bar_sync(2, kEncThreads);
-            TR(t, 5);
+            bar_arrive(kBarOffsets + kp, kEncThreads);   // offsets of tile k and the bookkeeping of tile k+2 are posted
             TRV(t, 15, (unsigned long long)smid() | ((unsigned long long)blockIdx.x << 32));
-            t = nt; p ^= 1;
+            t = t1; t1 = t2;
         }
         return;
     }
 
     // =============================== worker warps ===============================
+    // Iteration k: E1/E2 of tile k -> sizes posted; E4 of tile k into image buffer k&1; then the
+    // offsets of tile k-1 (resolved by the scan warp meanwhile) are awaited, the next tile's raw IDs
+    // prefetched into the (now free) staging area, and tile k-1's images copied out.
+    // Loop-carried state is kept small (registers): the bookkeeping ring is re-read where needed.
     const int q = lane >> 2, l = lane & 3;
     uint4* area = dyn_smem + warp * EncSmem<W>::kWarpChunks;
     uint4* slot = area + raw_slot_chunk<W>(q);                           // staging: the quad's raw IDs
-    unsigned char* img = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks + quad_slot_chunk(q));
+    unsigned char* img0 = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks + kImgSlotChunks * q);
     const int j = warp * kQuadBlocks + q;
+    constexpr uint32_t kLateBit = 1u << 31;                              // in key_prev: assembled by late_emit
     __syncthreads();                                                     // barrier 0
-    if (s_tile[0] != kNoTile) quad_prefetch<W>(slot, ids + s_xoff[0][j], s_m[0][j]);
-    int p = 0;
-    while (true) {
-        const unsigned long long t = s_tile[p];
-        if (t == kNoTile) break;
-        const int m = s_m[p][j];
-        const T* x = ids + s_xoff[p][j];
-        const T* raw = reinterpret_cast<const T*>(slot) + (reinterpret_cast<uintptr_t>(x) & 15) / sizeof(T);
-        if (warp == 0) TR(t, 6);
-        cp_async_wait_all();
-        __syncwarp();
-        if (warp == 0) TR(t, 7);
-        uint32_t key, d[32];
-        bool wide_lane = false, wide = false;
-        const T base = col_deltas<W>(raw, m, d, wide_lane);              // E1
-        if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
-        if (!wide) key = quad_choose_b<W>(d);                            // E2
-        else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(img));
-        if (m <= 0) key = 0;
-        if (l == 0) s_key[j] = key;
-        if (warp == 0) TR(t, 8);
-        bar_arrive(1, kEncThreads);
-
-        const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u, bytes = key >> 14;
-        if (!wide && __any_sync(kFull, n_exc > 0)) col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, n_exc);
-        if (!wide) {                                                     // E4 into the image area
-            if (key != 0 && b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
-            if (l == 0) {                                                // block header (FORMAT.md §2)
-                reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
-                reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
-            }
+    bool have = s_tile[0] != kNoTile;
+    if (have) quad_prefetch<W>(slot, ids + s_xoff[0][j], s_m[0][j]);
+    uint32_t key_prev = 0;
+    for (int k = 0;; k++) {
+        uint32_t key = 0;
+        if (have) {
+            const int m = s_m[k & 3][j];
+            const T* raw = reinterpret_cast<const T*>(slot) +
+                           (reinterpret_cast<uintptr_t>(ids + s_xoff[k & 3][j]) & 15) / sizeof(T);
+            unsigned char* img = img0 + (k & 1) * (kImgBufChunks * 16);
+            if (warp == 0) TR(s_tile[k & 3], 6);
+            cp_async_wait_all();
             __syncwarp();
-        }
-        if (warp == 0) TR(t, 9);
-        bar_sync(2, kEncThreads);                                        // s_at of tile t and the next tile are posted
-        if (warp == 0) TR(t, 10);
+            if (warp == 0) TR(s_tile[k & 3], 7);
+            uint32_t d[32];
+            bool wide_lane = false, wide = false;
+            const T base = col_deltas<W>(raw, m, d, wide_lane);          // E1
+            if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
+            if (!wide) key = quad_choose_b<W>(d);                        // E2
+            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(img));
+            if (m <= 0) key = 0;
+            if (l == 0) s_key[k & 1][j] = key;
+            {   // The tile's aggregate goes out as soon as the LAST worker warp has its sizes — not when the scan
+                // warp gets to it: that warp may still be inside the previous tile's look-back, and every
+                // later tile in flight waits for this number.
+                uint32_t z = l == 0 ? key >> 18 : 0u;
+                z += __shfl_xor_sync(kFull, z, 4); z += __shfl_xor_sync(kFull, z, 8); z += __shfl_xor_sync(kFull, z, 16);
+                if (lane == 0) {
+                    const unsigned int old = atomicAdd(&s_agg[k & 1], (1u << 24) | z);
+                    if ((old >> 24) == kEncWorkers - 1) {
+                        s_agg[k & 1] = 0;
+                        const unsigned long long t = s_tile[k & 3];
+                        if (t > 0)
+                            st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagAgg | (unsigned long long)((old & 0xffffffu) + z));
+                    }
+                }
+            }
+            if (warp == 0) TR(s_tile[k & 3], 8);
+            bar_arrive(kBarSizes + (k & 1), kEncThreads);
 
-        const unsigned long long at = key != 0 ? s_at[j] : kSkip;
-        if (s_tile[p ^ 1] != kNoTile) quad_prefetch<W>(slot, ids + s_xoff[p ^ 1][j], s_m[p ^ 1][j]);   // same slots
-        if (warp == 0) TR(t, 12);
-        if constexpr (W == 64) {
-            if (wide) {                                                  // slow path: straight to global memory
-                late_emit<64>(reinterpret_cast<const uint64_t*>(x), m, key, at != kSkip ? a.out + at : nullptr,
-                          reinterpret_cast<uint64_t*>(area + EncSmem<W>::kStageChunks));
+            const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
+            const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)kImgCap);   // slow path, in global memory later
+            if (!wide) {                                                 // E4 into the image buffer
+                const bool fast = key != 0 && !late;
+                if (__any_sync(kFull, fast && n_exc > 0))
+                    col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
+                if (fast) {
+                    if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
+                    if (l == 0) {                                        // block header (FORMAT.md §2)
+                        reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
+                        reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
+                    }
+                }
+            }
+            if (late) key |= kLateBit;
+            __syncwarp();                                                // staged IDs consumed, image complete
+            if (warp == 0) TR(s_tile[k & 3], 9);
+        }
+
+        unsigned long long at_prev = kSkip;
+        if (k > 0) {                                                     // tile k-1: offsets resolved?
+            bar_sync(kBarOffsets + ((k - 1) & 1), kEncThreads);
+            if (key_prev != 0) at_prev = s_at[(k - 1) & 1][j];
+            if (__any_sync(kFull, (key_prev & kLateBit) != 0)) {
+                const bool mine = (key_prev & kLateBit) != 0 && at_prev != kSkip;
+                late_emit<W>(ids + s_xoff[(k - 1) & 3][j], s_m[(k - 1) & 3][j], key_prev & ~kLateBit,
+                             mine ? a.out + at_prev : nullptr, reinterpret_cast<uint64_t*>(area));
             }
         }
-        if (!wide && at != kSkip) {
-            const uint4* src = reinterpret_cast<const uint4*>(img);
-            uint4* dst = reinterpret_cast<uint4*>(a.out + at);
-            for (uint32_t k = l; k < bytes / 16; k += 4) __stcs(dst + k, src[k]);
+        bool have_next = false;
+        if (have) {                                                      // next tile: posted before barrier 0 / kBarOffsets
+            have_next = s_tile[(k + 1) & 3] != kNoTile;
+            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & 3][j], s_m[(k + 1) & 3][j]);   // same slots
+        }
+        if (warp == 0 && have) TR(s_tile[k & 3], 10);
+        if ((key_prev & kLateBit) == 0 && at_prev != kSkip) {            // copy tile k-1's image to its final place
+            const uint4* src = reinterpret_cast<const uint4*>(img0 + ((k - 1) & 1) * (kImgBufChunks * 16));
+            uint4* dst = reinterpret_cast<uint4*>(a.out + at_prev);
+            const uint32_t n16 = key_prev >> 18;
+            for (uint32_t c = l; c < n16; c += 4) __stcs(dst + c, src[c]);
         }
         __syncwarp();
-        if (warp == 0) TR(t, 11);
-        p ^= 1;
+        if (warp == 0 && have) TR(s_tile[k & 3], 11);
+        if (!have) break;
+        key_prev = key;
+        have = have_next;
     }
 }
 
