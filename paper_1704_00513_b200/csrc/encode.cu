@@ -13,7 +13,7 @@ struct EncArgs {
     const unsigned long long* in_off;   // n_buf+1 element offsets, or nullptr (single buffer of n_single IDs)
     unsigned long long n_single;
     uint32_t n_buf;
-    uint32_t pad0;
+    uint32_t grid;                      // CTAs of k_enc_tiles: their first tile is blockIdx.x, tickets start here
     unsigned long long thr;             // raw threshold in bytes
     unsigned char* out;
     unsigned long long out_cap;
@@ -45,6 +45,25 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     __shared__ int bad;
     constexpr unsigned long long E = W / 8;
     pdl_launch_dependents();
+    if (a.in_off == nullptr) {                           // single buffer: no scan needed
+        const unsigned long long n = a.n_single;
+        const bool raw = n * E < a.thr;
+        const unsigned long long nb = raw ? 0ull : (n + kBlk - 1) / kBlk;
+        const unsigned long long fixed = raw ? 32ull + ((n * E + 15ull) & ~15ull) : 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull);
+        const unsigned long long nt = (nb + kTileR - 1) / kTileR;
+        const bool ok = nb <= a.ws.blk_cap && nt <= a.ws.tile_cap;
+        if (ok)
+            for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q * kStateStride] = 0;
+        if (threadIdx.x == 0) {
+            a.ws.blk_first[0] = 0; a.ws.blk_first[1] = nb;
+            a.ws.fixed_prefix[0] = 0; a.ws.fixed_prefix[1] = fixed;
+            a.ws.stream_start[0] = 0; a.ws.stream_start[1] = 0;
+            a.ws.hdr->total_blocks = nb; a.ws.hdr->fixed_total = fixed; a.ws.hdr->ticket = a.grid;
+            a.ws.hdr->grand16 = 0; a.ws.hdr->total_out = fixed; a.ws.hdr->ok = ok ? 1u : 0u;
+            if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
+        }
+        return;
+    }
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
     Scan2 carry{0, 0};
@@ -80,7 +99,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         a.ws.stream_start[a.n_buf] = 0;
         a.ws.hdr->total_blocks = carry.a;
         a.ws.hdr->fixed_total = carry.b;
-        a.ws.hdr->ticket = 0;
+        a.ws.hdr->ticket = a.grid;
         a.ws.hdr->grand16 = 0;
         a.ws.hdr->total_out = carry.b;
         const bool ok = !bad && carry.a <= a.ws.blk_cap && (carry.a + kTileR - 1) / kTileR <= a.ws.tile_cap;
@@ -180,7 +199,7 @@ template <int W> struct EncSmem {
 };
 static_assert(RawCfg<32>::kAreaChunks * 16 >= 4 * kLateSlotWords64 * 8, "late_emit scratch");
 
-enum { kBarSizes = 1, kBarOffsets = 3 };                      // named barriers: +parity of the CTA's tile count
+enum { kBarSizes = 1, kBarOffsets = 3, kBarFirst = 5 };                      // named barriers: +parity of the CTA's tile count
 
 template <int W>
 __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(EncArgs a) {
@@ -202,12 +221,16 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
 
     if (warp == kEncWorkers) {
         // =============================== scan warp ===============================
-        pdl_wait();                                      // the plan kernel's writes are visible from here on
-        const bool ok = a.ws.hdr->ok != 0;
-        const unsigned long long total = ok ? a.ws.hdr->total_blocks : 0ull;
-        const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
+        // Single-buffer calls know their geometry from the arguments: the first tile (= blockIdx.x) starts
+        // without waiting for the plan kernel; only the ticket counter and the look-back states need it.
         const unsigned long long nb_single = (a.n_single + kBlk - 1) / kBlk;
         const unsigned long long f1_single = 32ull + ((4ull * (nb_single + 1) + 15ull) & ~15ull);
+        unsigned long long total = nb_single;
+        if (batch) {
+            pdl_wait();
+            total = a.ws.hdr->ok != 0 ? a.ws.hdr->total_blocks : 0ull;
+        }
+        const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
 
         auto draw = [&]() -> unsigned long long {
             unsigned long long t = 0;
@@ -239,10 +262,13 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
         // A CTA works on tile k (sizes, pack) while the scan warp resolves the offsets of tile k-1, so
         // tickets are drawn two tiles ahead: always at the same point of the pipeline, so that a lower
         // tile number means "sizes posted earlier" and a look-back rarely has to wait.
-        unsigned long long t = draw(), t1 = t != kNoTile ? draw() : kNoTile;
+        unsigned long long t = blockIdx.x < n_tiles ? (unsigned long long)blockIdx.x : kNoTile;
         prep(t, 0);
+        __syncthreads();                                 // barrier 0: the first tile is posted
+        if (!batch) pdl_wait();                          // the plan kernel's writes are visible from here on
+        unsigned long long t1 = t != kNoTile ? draw() : kNoTile;
         prep(t1, 1);
-        __syncthreads();                                 // barrier 0: the first two tiles are posted
+        bar_arrive(kBarFirst, kEncThreads);              // the second tile is posted
         for (int k = 0; t != kNoTile; k++) {
             const int kp = k & 1;
             TR(t, 0);
@@ -378,6 +404,7 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
                     if ((old >> 24) == kEncWorkers - 1) {
                         s_agg[k & 1] = 0;
                         const unsigned long long t = s_tile[k & 3];
+                        pdl_wait();                                      // the states are zeroed by the plan kernel
                         if (t > 0)
                             st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagAgg | (unsigned long long)((old & 0xffffffu) + z));
                     }
@@ -406,6 +433,7 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
         }
 
         unsigned long long at_prev = kSkip;
+        if (k == 0) bar_sync(kBarFirst, kEncThreads);                    // the second tile is posted
         if (k > 0) {                                                     // tile k-1: offsets resolved?
             bar_sync(kBarOffsets + ((k - 1) & 1), kEncThreads);
             if (key_prev != 0) at_prev = s_at[(k - 1) & 1][j];
@@ -511,7 +539,7 @@ static cudaError_t launch_dep(void (*kern)(A), int grid, int block, size_t smem,
 }
 
 template <int W>
-static bfsc_status launch_encode(const EncArgs& a, cudaStream_t s) {
+static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     constexpr size_t kSmem = EncSmem<W>::kBytes;
     static int max_grid = 0;                      // persistent grid: all CTAs resident
     if (max_grid == 0) {
@@ -526,16 +554,19 @@ static bfsc_status launch_encode(const EncArgs& a, cudaStream_t s) {
         max_grid = sms * per_sm;
     }
     constexpr unsigned long long E = W / 8;
-    const bool single = a.in_off == nullptr;
-    const bool degenerate = single && (a.n_single == 0 || a.n_single * E < a.thr);   // no block: header (+ raw copy) only
+    const bool single = a_in.in_off == nullptr;
+    const bool degenerate = single && (a_in.n_single == 0 || a_in.n_single * E < a_in.thr);   // no block: header (+ raw copy) only
+    int grid = max_grid;
+    if (single) {
+        const unsigned long long n_tiles = ((a_in.n_single + kBlk - 1) / kBlk + kTileR - 1) / kTileR;
+        if (!degenerate && n_tiles > a_in.ws.tile_cap) return BFSC_ERR_INVALID_ARG;          // workspace too small
+        if (n_tiles < (unsigned long long)grid) grid = (int)n_tiles;
+    }
+    EncArgs a = a_in;
+    a.grid = (uint32_t)grid;
     k_enc_plan<W><<<1, 1024, 0, s>>>(a);
     BFSC_LAUNCH_CHECK();
     if (!degenerate) {
-        int grid = max_grid;
-        if (single) {
-            const unsigned long long n_tiles = ((a.n_single + kBlk - 1) / kBlk + kTileR - 1) / kTileR;
-            if (n_tiles < (unsigned long long)grid) grid = (int)n_tiles;
-        }
         if (launch_dep(k_enc_tiles<W>, grid, kEncThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
         BFSC_LAUNCH_CHECK();
     }
@@ -557,7 +588,7 @@ static bfsc_status encode_common(const void* d_ids, const uint64_t* d_in_off, si
     EncArgs a;
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.ids = d_ids; a.in_off = (const unsigned long long*)d_in_off; a.n_single = n_single;
-    a.n_buf = (uint32_t)n_buf; a.pad0 = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
+    a.n_buf = (uint32_t)n_buf; a.grid = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
     a.out_off = (unsigned long long*)d_out_off; a.out_total = (unsigned long long*)d_out_total; a.status = d_status;
     return t == BFSC_U32 ? launch_encode<32>(a, (cudaStream_t)stream) : launch_encode<64>(a, (cudaStream_t)stream);
 }
