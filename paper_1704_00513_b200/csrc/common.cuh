@@ -146,6 +146,24 @@ __device__ inline Scan2 block_scan_excl2(Scan2 v, Scan2* total, Scan2* sm /* 33 
 
 extern unsigned long long g_launches;   // host-side launch counter (api.cu)
 
+// Programmatic dependent launch: a kernel launched with launch_dep may start while its predecessor in
+// the stream still runs (once that one executed pdl_launch_dependents); it must execute pdl_wait
+// before it touches anything the predecessor writes.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename A>
+static inline cudaError_t launch_dep(void (*kern)(A), int grid, int block, size_t smem, cudaStream_t s, const A& args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args);
+}
+
 }  // namespace bfsc
 
 #define BFSC_LAUNCH_CHECK()                                        \

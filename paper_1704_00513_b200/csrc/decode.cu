@@ -1,5 +1,9 @@
 // decode.cu — bfsc_decompress / bfsc_decompress_batch (steps D0-D5).
+//
+// Launches per call: single stream: k_dec_tiles alone (it parses the stream header itself);
+// batch: k_dec_plan -> k_dec_tiles, chained with programmatic dependent launch.
 #include "block_decode.cuh"
+#include "quad_decode.cuh"
 
 namespace bfsc {
 
@@ -29,6 +33,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
     __shared__ Scan2 sm[33];
     __shared__ int bad;
     constexpr unsigned long long E = W / 8;
+    pdl_launch_dependents();
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
     Scan2 carry{0, 0};
@@ -86,68 +91,220 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
         for (uint32_t i = threadIdx.x; i <= a.n_buf; i += blockDim.x) a.id_off[i] = good ? a.ws.fixed_prefix[i] : 0ull;
 }
 
-// ---- D1-D4 per block -------------------------------------------------------------------
-template <int W>
-__global__ void __launch_bounds__(256) k_dec_blocks(DecArgs a) {
+
+// ---- D1-D5 fused -------------------------------------------------------------------------
+// Warp = batch of 8 consecutive blocks, four lanes per block (quad_decode.cuh). Per batch:
+//   locate   per quad: stream, directory entries -> block address, span, valid IDs, output address
+//   D1       cp.async the block (<= 272 B) into the warp's staging slots
+//   D2-D4    unpack from shared memory, patch through the warp's table, scan, 128-bit stores
+// Blocks over 272 B (b > 16: nearly incompressible data) take the warp-per-block path of
+// block_decode.cuh, straight from global memory. Single-stream calls parse the stream header here
+// (no plan kernel); RAW streams are copied at the end (D5).
+constexpr int kDecWarps = 8;
+constexpr int kDecThreads = kDecWarps * 32;
+
+template <int W> struct DecSmem {
     using T = typename IdT<W>::T;
-    if (!a.ws.hdr->ok) return;
-    const unsigned long long total_blocks = a.ws.hdr->total_blocks;
-    const unsigned long long nwarps = (unsigned long long)gridDim.x * (blockDim.x >> 5);
-    for (unsigned long long g = (unsigned long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-         g < total_blocks; g += nwarps) {
-        const uint32_t i = find_buf(a.ws.blk_first, a.n_buf, g);
-        const unsigned long long k = g - a.ws.blk_first[i];
-        const unsigned long long id0 = a.ws.fixed_prefix[i], n = a.ws.fixed_prefix[i + 1] - id0;
-        const unsigned char* s = a.in + s_begin(a, i);
-        const unsigned long long total16 = *reinterpret_cast<const unsigned long long*>(s + 16) >> 4;
-        const unsigned long long nb = (n + kBlk - 1) / kBlk;
+    static constexpr size_t kStageBytes = (size_t)kDecStageChunks * 16;               // per warp
+    static constexpr size_t kTabBytes = (size_t)kDecBlocks * kBlk * sizeof(T);         // per warp
+    static constexpr size_t kBytes = kDecWarps * (kStageBytes + kTabBytes);
+};
+
+template <int W>
+struct BlockAt {                       // where the quad's block is
+    const unsigned char* blk;          // first byte of the block (nullptr: no block / malformed)
+    typename IdT<W>::T* x;             // first output ID
+    uint32_t span16;                   // directory span in 16-byte units
+    int m;                             // valid IDs
+};
+
+template <int W>
+__global__ void __launch_bounds__(kDecThreads, (W == 32) ? 3 : 2) k_dec_tiles(DecArgs a) {
+    using T = typename IdT<W>::T;
+    constexpr unsigned long long E = W / 8;
+    extern __shared__ __align__(16) unsigned char dec_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, q = lane >> 2, l = lane & 3;
+    uint4* stage = reinterpret_cast<uint4*>(dec_smem + warp * DecSmem<W>::kStageBytes);
+    T* tab_w = reinterpret_cast<T*>(dec_smem + kDecWarps * DecSmem<W>::kStageBytes + warp * DecSmem<W>::kTabBytes);
+    for (int x = lane; x < kDecBlocks * kBlk; x += 32) tab_w[x] = 0;       // patch table: all zero between uses
+    __syncwarp();
+    uint4* slot = stage + kDecSlotChunks * q;
+    T* tab = tab_w + kBlk * q;
+
+    const bool batch = a.in_off != nullptr;
+    unsigned long long total_blocks, n1 = 0, total16_1 = 0, lo16_1 = 0;   // single stream: n, total/16, first block/16
+    if (batch) {
+        pdl_wait();
+        if (!a.ws.hdr->ok) return;
+        total_blocks = a.ws.hdr->total_blocks;
+    } else {                                                               // D0 for one stream (FORMAT.md §1, §4)
+        const bool first = blockIdx.x == 0 && threadIdx.x == 0;
+        bool ok = a.in_single >= 32;
+        uint32_t mode = 0;
+        unsigned long long total = 0, nb = 0;
+        if (ok) {
+            const uint4 h0 = *reinterpret_cast<const uint4*>(a.in);
+            const uint4 h1 = *reinterpret_cast<const uint4*>(a.in + 16);
+            mode = (h0.y >> 16) & 0xffu;
+            n1 = (unsigned long long)h0.w << 32 | h0.z;
+            total = (unsigned long long)h1.y << 32 | h1.x;
+            nb = h1.z;
+            if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W || mode > 1u ||
+                (h0.y >> 24) != 0u)
+                ok = false;
+            else if (total > a.in_single || (total & 15) || total < 32) ok = false;
+            else if (mode == 0) { if (nb != 0 || n1 > (total - 32) / E) ok = false; }
+            else if (nb != (n1 + kBlk - 1) / kBlk || n1 > (1ull << 40) || 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
+                ok = false;
+        }
+        if (!ok || n1 > a.ids_cap) {
+            if (first) {
+                set_status(a.status, ok ? BFSC_ERR_DST_TOO_SMALL : BFSC_ERR_CORRUPT);
+                if (a.n_ids_out) *a.n_ids_out = 0;
+            }
+            return;
+        }
+        if (first && a.n_ids_out) *a.n_ids_out = n1;
+        if (mode == 0) {                                                   // D5: raw passthrough
+            const T* xs = reinterpret_cast<const T*>(a.in + 32);
+            T* y = reinterpret_cast<T*>(a.ids);
+            for (unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; t < n1;
+                 t += (unsigned long long)gridDim.x * blockDim.x)
+                y[t] = xs[t];
+            return;
+        }
+        total_blocks = nb;
+        total16_1 = total >> 4;
+        lo16_1 = (32ull + ((4ull * (nb + 1) + 15ull) & ~15ull)) >> 4;
+    }
+
+    auto locate = [&](unsigned long long g) -> BlockAt<W> {
+        BlockAt<W> r; r.blk = nullptr; r.x = nullptr; r.span16 = 0; r.m = 0;
+        if (g >= total_blocks) return r;
+        const unsigned char* s = a.in;
+        unsigned long long k = g, id0 = 0, n = n1, total16 = total16_1, lo16 = lo16_1;
+        if (batch) {
+            const uint32_t i = find_buf(a.ws.blk_first, a.n_buf, g);
+            k = g - a.ws.blk_first[i];
+            id0 = a.ws.fixed_prefix[i]; n = a.ws.fixed_prefix[i + 1] - id0;
+            s = a.in + s_begin(a, i);
+            total16 = *reinterpret_cast<const unsigned long long*>(s + 16) >> 4;
+            lo16 = (32ull + ((4ull * ((n + kBlk - 1) / kBlk + 1) + 15ull) & ~15ull)) >> 4;
+        }
         const uint32_t* dir = reinterpret_cast<const uint32_t*>(s + 32);
         const unsigned long long o0 = dir[k], o1 = dir[k + 1];
-        const unsigned long long lo16 = (32ull + ((4ull * (nb + 1) + 15ull) & ~15ull)) >> 4;
-        if (o0 < lo16 || o1 <= o0 || o1 > total16) { set_status(a.status, BFSC_ERR_CORRUPT); continue; }
-        const unsigned char* blk = s + 16ull * o0;
-        const uint4 h = *reinterpret_cast<const uint4*>(blk);
-        const uint32_t b = h.z & 0xffu, n_exc = (h.z >> 8) & 0xffu;
-        if (b > (uint32_t)W || n_exc > 127u || 16ull + 16ull * b + exc_bytes<W>(n_exc) > 16ull * (o1 - o0)) {
-            set_status(a.status, BFSC_ERR_CORRUPT);
-            continue;
+        if (o0 < lo16 || o1 <= o0 || o1 > total16) { set_status(a.status, BFSC_ERR_CORRUPT); return r; }
+        r.blk = s + 16ull * o0;
+        r.span16 = (uint32_t)(o1 - o0);
+        r.m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+        r.x = reinterpret_cast<T*>(a.ids) + id0 + kBlk * k;
+        return r;
+    };
+
+    const unsigned long long n_batches = (total_blocks + kDecBlocks - 1) / kDecBlocks;
+    const unsigned long long n_warps = (unsigned long long)gridDim.x * kDecWarps;
+    unsigned long long bi = (unsigned long long)blockIdx.x * kDecWarps + warp;
+    BlockAt<W> cur = locate(bi * kDecBlocks + q);
+    for (; bi < n_batches; bi += n_warps) {
+        const bool big = cur.blk != nullptr && cur.span16 > (uint32_t)kDecSpanMax;
+        const bool any_big = __any_sync(kFull, big);
+        if (!any_big && cur.blk != nullptr) quad_stage_block(slot, cur.blk, cur.span16, l);
+        const BlockAt<W> nxt = locate((bi + n_warps) * kDecBlocks + q);   // the next batch's directory reads overlap the copy
+        if (!any_big) {
+            dec_cp_async_wait_all();
+            __syncwarp();
+            bool live = cur.blk != nullptr;
+            const uint4 h = slot[0];
+            const uint32_t b = h.z & 0xffu, n_exc = (h.z >> 8) & 0xffu;
+            if (live && (b > (uint32_t)W || n_exc > 127u || 1u + b + exc_bytes<W>(n_exc) / 16u > cur.span16)) {
+                set_status(a.status, BFSC_ERR_CORRUPT);
+                live = false;
+            }
+            uint32_t d[8][4];
+            quad_unpack(slot + 1, live ? b : 0u, l, d);                     // D2 (b <= 16 here: the span is <= 17 chunks)
+            T v[8][4];
+            if (__any_sync(kFull, live && n_exc > 0)) {                      // D3
+                const bool okp = quad_patch<W>(tab, reinterpret_cast<const unsigned char*>(slot + 1 + b), b,
+                                               live ? n_exc : 0u, l, v);
+                if (!okp) { set_status(a.status, BFSC_ERR_CORRUPT); live = false; }
+#pragma unroll
+                for (int i = 0; i < 8; i++)
+#pragma unroll
+                    for (int c = 0; c < 4; c++) v[i][c] |= (T)d[i][c];
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; i++)
+#pragma unroll
+                    for (int c = 0; c < 4; c++) v[i][c] = (T)d[i][c];
+            }
+            const T base = (T)((unsigned long long)h.y << 32 | h.x);
+            quad_scan_store<W>(v, base, cur.x, live ? cur.m : 0, l);         // D4
+            __syncwarp();                                                    // slots and table free again
+        } else {
+            // slow path: one block at a time, the whole warp on it, straight from global memory
+            for (int qq = 0; qq < kDecBlocks; qq++) {
+                const unsigned char* blk = reinterpret_cast<const unsigned char*>(
+                    __shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(cur.blk), 4 * qq));
+                T* x = reinterpret_cast<T*>(__shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(cur.x), 4 * qq));
+                const uint32_t span16 = __shfl_sync(kFull, cur.span16, 4 * qq);
+                const int m = __shfl_sync(kFull, cur.m, 4 * qq);
+                if (blk == nullptr) continue;
+                const uint4 h = *reinterpret_cast<const uint4*>(blk);
+                const uint32_t b = h.z & 0xffu, n_exc = (h.z >> 8) & 0xffu;
+                if (b > (uint32_t)W || n_exc > 127u || 16ull + 16ull * b + exc_bytes<W>(n_exc) > 16ull * span16) {
+                    set_status(a.status, BFSC_ERR_CORRUPT);
+                    continue;
+                }
+                const T base = (T)((unsigned long long)h.y << 32 | h.x);
+                T dd[4];
+                unpack_rows<W>(reinterpret_cast<const uint4*>(blk + 16), b, dd);
+                if (n_exc > 0 && !patch_rows<W>(blk + 16 + 16 * b, b, n_exc, dd)) {
+                    set_status(a.status, BFSC_ERR_CORRUPT);
+                    continue;
+                }
+                scan_store<W>(dd, base, x, m);
+            }
         }
-        const T base = (T)((unsigned long long)h.y << 32 | h.x);
-        T d[4];
-        unpack_rows<W>(reinterpret_cast<const uint4*>(blk + 16), b, d);
-        if (n_exc > 0 && !patch_rows<W>(blk + 16 + 16 * b, b, n_exc, d)) {
-            set_status(a.status, BFSC_ERR_CORRUPT);
-            continue;
+        cur = nxt;
+    }
+
+    if (batch) {                                                           // D5: raw streams of the batch
+        for (uint32_t i = blockIdx.x; i < a.n_buf; i += gridDim.x) {
+            const unsigned char* s = a.in + s_begin(a, i);
+            if (s[6] != 0) continue;
+            const unsigned long long id0 = a.ws.fixed_prefix[i], n = a.ws.fixed_prefix[i + 1] - id0;
+            const T* xs = reinterpret_cast<const T*>(s + 32);
+            T* y = reinterpret_cast<T*>(a.ids) + id0;
+            for (unsigned long long t = threadIdx.x; t < n; t += blockDim.x) y[t] = xs[t];
         }
-        const int m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-        scan_store<W>(d, base, reinterpret_cast<T*>(a.ids) + id0 + kBlk * k, m);
     }
 }
 
-// ---- D5 raw passthrough -----------------------------------------------------------------
 template <int W>
-__global__ void __launch_bounds__(256) k_dec_raw(DecArgs a) {
-    using T = typename IdT<W>::T;
-    if (!a.ws.hdr->ok) return;
-    for (uint32_t i = blockIdx.x; i < a.n_buf; i += gridDim.x) {
-        const unsigned char* s = a.in + s_begin(a, i);
-        if (s[6] != 0) continue;
-        const unsigned long long id0 = a.ws.fixed_prefix[i], n = a.ws.fixed_prefix[i + 1] - id0;
-        const T* x = reinterpret_cast<const T*>(s + 32);
-        T* y = reinterpret_cast<T*>(a.ids) + id0;
-        for (unsigned long long j = threadIdx.x; j < n; j += blockDim.x) y[j] = x[j];
+static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream_t s) {
+    constexpr size_t kSmem = DecSmem<W>::kBytes;
+    static int max_grid = 0;
+    if (max_grid == 0) {
+        int per_sm = 0, dev = 0, sms = kNumSM;
+        if (cudaFuncSetAttribute(k_dec_tiles<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
+            return BFSC_ERR_CUDA;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dec_tiles<W>, kDecThreads, kSmem) != cudaSuccess ||
+            per_sm < 1)
+            per_sm = 1;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        max_grid = sms * per_sm;
     }
-}
-
-template <int W>
-static bfsc_status launch_decode(const DecArgs& a, cudaStream_t s) {
-    const int grid = kNumSM * 8;
-    k_dec_plan<W><<<1, 1024, 0, s>>>(a);
-    BFSC_LAUNCH_CHECK();
-    k_dec_blocks<W><<<grid, 256, 0, s>>>(a);
-    BFSC_LAUNCH_CHECK();
-    const uint32_t rgrid = a.n_buf < (uint32_t)(kNumSM * 8) ? a.n_buf : (uint32_t)(kNumSM * 8);
-    k_dec_raw<W><<<rgrid ? rgrid : 1, 256, 0, s>>>(a);
+    const size_t want = (max_blocks + kDecBlocks * kDecWarps - 1) / (kDecBlocks * kDecWarps);
+    int grid = want < (size_t)max_grid ? (int)want : max_grid;
+    if (grid < 1) grid = 1;
+    if (a.in_off) {
+        k_dec_plan<W><<<1, 1024, 0, s>>>(a);
+        BFSC_LAUNCH_CHECK();
+        if (launch_dep(k_dec_tiles<W>, max_grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+    } else {
+        k_dec_tiles<W><<<grid, kDecThreads, kSmem, s>>>(a);
+    }
     BFSC_LAUNCH_CHECK();
     return BFSC_OK;
 }
@@ -164,7 +321,9 @@ static bfsc_status decode_common(const void* d_in, const uint64_t* d_in_off, siz
     a.in = (const unsigned char*)d_in; a.in_off = (const unsigned long long*)d_in_off; a.in_single = in_single;
     a.n_buf = (uint32_t)n_buf; a.ids = d_ids; a.ids_cap = ids_cap; a.id_off = (unsigned long long*)d_id_off;
     a.n_ids_out = (unsigned long long*)d_n_ids; a.status = d_status;
-    return t == BFSC_U32 ? launch_decode<32>(a, (cudaStream_t)stream) : launch_decode<64>(a, (cudaStream_t)stream);
+    const size_t max_blocks = ids_cap / kBlk + n_buf + 1;
+    return t == BFSC_U32 ? launch_decode<32>(a, max_blocks, (cudaStream_t)stream)
+                         : launch_decode<64>(a, max_blocks, (cudaStream_t)stream);
 }
 
 }  // namespace bfsc

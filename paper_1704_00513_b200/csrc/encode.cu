@@ -30,8 +30,6 @@ __device__ __forceinline__ unsigned long long buf_count(const EncArgs& a, uint32
     return a.in_off ? a.in_off[i + 1] - a.in_off[i] : a.n_single;
 }
 
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 constexpr int kEncWorkers = 8;                           // worker warps per CTA
 constexpr int kTileR = kEncWorkers * kQuadBlocks;        // 64 blocks per tile
@@ -522,20 +520,6 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
         if (a.out_off) a.out_off[a.n_buf] = t;
         if (a.out_total) *a.out_total = t;
     }
-}
-
-// Launch with the programmatic-stream-serialization attribute: the kernel may start before its
-// predecessor in the stream has finished; it calls griddepcontrol.wait before consuming its output.
-template <typename A>
-static cudaError_t launch_dep(void (*kern)(A), int grid, int block, size_t smem, cudaStream_t s, const A& args) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block);
-    cfg.dynamicSmemBytes = smem; cfg.stream = s;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, args);
 }
 
 template <int W>
