@@ -220,25 +220,21 @@ __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 3 : 2) k_dec_tiles(De
                 set_status(a.status, BFSC_ERR_CORRUPT);
                 live = false;
             }
-            uint32_t d[8][4];
-            quad_unpack(slot + 1, live ? b : 0u, l, d);                     // D2 (b <= 16 here: the span is <= 17 chunks)
-            T v[8][4];
-            if (__any_sync(kFull, live && n_exc > 0)) {                      // D3
-                const bool okp = quad_patch<W>(tab, reinterpret_cast<const unsigned char*>(slot + 1 + b), b,
-                                               live ? n_exc : 0u, l, v);
-                if (!okp) { set_status(a.status, BFSC_ERR_CORRUPT); live = false; }
-#pragma unroll
-                for (int i = 0; i < 8; i++)
-#pragma unroll
-                    for (int c = 0; c < 4; c++) v[i][c] |= (T)d[i][c];
-            } else {
-#pragma unroll
-                for (int i = 0; i < 8; i++)
-#pragma unroll
-                    for (int c = 0; c < 4; c++) v[i][c] = (T)d[i][c];
+            const unsigned char* e = reinterpret_cast<const unsigned char*>(slot + 1 + b);
+            const bool patch = __any_sync(kFull, live && n_exc > 0);         // D3: scatter into the patch table
+            if (patch) {
+                if (!quad_patch_scatter<W>(tab, e, b, live ? n_exc : 0u, l)) { set_status(a.status, BFSC_ERR_CORRUPT); live = false; }
+                __syncwarp();
+                const int lv = live;                                     // all four shuffles by every lane: no short-circuit
+                live = (__shfl_sync(kFull, lv, 4 * q + 0) & __shfl_sync(kFull, lv, 4 * q + 1) &
+                        __shfl_sync(kFull, lv, 4 * q + 2) & __shfl_sync(kFull, lv, 4 * q + 3)) != 0;
             }
             const T base = (T)((unsigned long long)h.y << 32 | h.x);
-            quad_scan_store<W>(v, base, cur.x, live ? cur.m : 0, l);         // D4
+            quad_decode_rows<W>(slot + 1, live ? b : 0u, tab, patch, base, cur.x, live ? cur.m : 0, l);   // D2-D4
+            if (patch) {
+                __syncwarp();
+                quad_patch_clear<W>(tab, e, (cur.blk != nullptr && b <= (uint32_t)W && n_exc <= 127u && 1u + b + exc_bytes<W>(n_exc) / 16u <= cur.span16) ? n_exc : 0u, l);
+            }
             __syncwarp();                                                    // slots and table free again
         } else {
             // slow path: one block at a time, the whole warp on it, straight from global memory

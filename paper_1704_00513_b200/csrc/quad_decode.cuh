@@ -33,32 +33,12 @@ __device__ __forceinline__ void quad_stage_block(uint4* __restrict__ slot, const
     }
 }
 
-// D2: low parts of the lane's rows from the staged payload P (b vectors of 128 bits, b <= 16; FORMAT.md §2
-// "Payload"). Row r's values sit at bits [r b, r b + b) of each column stream; the second vector read may
-// be one past the payload (slack chunk / exception area): its bits are masked off.
-__device__ __forceinline__ void quad_unpack(const uint4* __restrict__ P, uint32_t b, int l, uint32_t (&d)[8][4]) {
-    const uint32_t mask = (1u << b) - 1u;
-    uint32_t bit = (uint32_t)l * b;
-#pragma unroll
-    for (int i = 0; i < 8; i++) {
-        const uint32_t k0 = bit >> 5, sh = bit & 31u;
-        const uint4 lo = P[k0], hi = P[k0 + 1];
-        d[i][0] = __funnelshift_r(lo.x, hi.x, sh) & mask;
-        d[i][1] = __funnelshift_r(lo.y, hi.y, sh) & mask;
-        d[i][2] = __funnelshift_r(lo.z, hi.z, sh) & mask;
-        d[i][3] = __funnelshift_r(lo.w, hi.w, sh) & mask;
-        bit += 4u * b;
-    }
-}
-
-// D3: exceptions through a per-warp patch table (128 entries per block, all zero between uses): the quad
-// scatters high << b at each position, every lane ORs its rows' entries in, the scattering lanes clear
-// them again. e = staged exception area. Returns false on a malformed position. Whole warp calls;
-// quads with n_exc == 0 idle through it (their table entries are zero: tab is still read).
+// D3 (first half): exceptions go through a per-warp patch table (128 entries per block, all zero between
+// uses): the quad scatters high << b at each position here; quad_decode_rows ORs the entries in;
+// quad_patch_clear zeroes them again. e = staged exception area. Returns false on a malformed position.
 template <int W>
-__device__ __forceinline__ bool quad_patch(typename IdT<W>::T* __restrict__ tab /* the quad's 128 entries */,
-                                           const unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc, int l,
-                                           typename IdT<W>::T (&hi)[8][4]) {
+__device__ __forceinline__ bool quad_patch_scatter(typename IdT<W>::T* __restrict__ tab /* the quad's 128 entries */,
+                                                   const unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc, int l) {
     using T = typename IdT<W>::T;
     constexpr uint32_t E = W / 8;
     const T* high = reinterpret_cast<const T*>(e + ((n_exc + E - 1) & ~(E - 1)));
@@ -67,68 +47,79 @@ __device__ __forceinline__ bool quad_patch(typename IdT<W>::T* __restrict__ tab 
         const uint32_t pos = e[x];
         if (pos >= (uint32_t)kBlk) ok = false; else tab[pos] = high[x] << b;
     }
-    __syncwarp();
-#pragma unroll
-    for (int i = 0; i < 8; i++) {
-        if constexpr (W == 32) {
-            const uint4 t = reinterpret_cast<const uint4*>(tab)[4 * i + l];
-            hi[i][0] = t.x; hi[i][1] = t.y; hi[i][2] = t.z; hi[i][3] = t.w;
-        } else {
-            const ulonglong2 t0 = reinterpret_cast<const ulonglong2*>(tab)[2 * (4 * i + l)];
-            const ulonglong2 t1 = reinterpret_cast<const ulonglong2*>(tab)[2 * (4 * i + l) + 1];
-            hi[i][0] = t0.x; hi[i][1] = t0.y; hi[i][2] = t1.x; hi[i][3] = t1.y;
-        }
-    }
-    __syncwarp();
+    return ok;
+}
+template <int W>
+__device__ __forceinline__ void quad_patch_clear(typename IdT<W>::T* __restrict__ tab, const unsigned char* __restrict__ e,
+                                                 uint32_t n_exc, int l) {
     for (uint32_t x = l; x < n_exc; x += 4) {
         const uint32_t pos = e[x];
         if (pos < (uint32_t)kBlk) tab[pos] = 0;
     }
-    return ok;
 }
 
-// D4: inclusive scan of the block's 128 deltas + base (mod 2^W) and store of the first m IDs.
-// v[i][c] = delta of ID 16i + 4l + c. Order of the IDs: i major, then lane, then c.
+// D2 + D3 + D4, one row step at a time (nothing but the running sum is carried between steps):
+//   D2  low parts of row r = 4i + l from the staged payload P (b <= 16 vectors of 128 bits; FORMAT.md §2
+//       "Payload"): row r's values sit at bits [r b, r b + b) of each column stream; the second vector
+//       read may be one past the payload (slack chunk / exception area): its bits are masked off;
+//   D3  OR of the patch table's row (only if some block of the warp has exceptions);
+//   D4  inclusive scan: prefix inside the row, inclusive scan of the row sums over the quad, running
+//       carry over the steps (order of the IDs: i major, then lane, then column); + base, mod 2^W;
+//       128-bit stores of the first m IDs.
 template <int W>
-__device__ __forceinline__ void quad_scan_store(typename IdT<W>::T (&v)[8][4], typename IdT<W>::T base,
-                                                typename IdT<W>::T* __restrict__ x, int m, int l) {
+__device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, uint32_t b,
+                                                 const typename IdT<W>::T* __restrict__ tab, bool patch,
+                                                 typename IdT<W>::T base, typename IdT<W>::T* __restrict__ x, int m, int l) {
     using T = typename IdT<W>::T;
+    const uint32_t mask = (1u << b) - 1u;
+    uint32_t bit = (uint32_t)l * b;
     T carry = base;
+    const bool vec_ok = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
+    const bool vec = __all_sync(kFull, vec_ok || m <= 0);
 #pragma unroll
     for (int i = 0; i < 8; i++) {
-        v[i][1] += v[i][0]; v[i][2] += v[i][1]; v[i][3] += v[i][2];      // prefix inside the row
-        T inc = v[i][3];                                                 // inclusive scan of the row sums over the quad
+        const uint32_t k0 = bit >> 5, sh = bit & 31u;
+        const uint4 lo = P[k0], hi = P[k0 + 1];
+        bit += 4u * b;
+        T v0 = __funnelshift_r(lo.x, hi.x, sh) & mask, v1 = __funnelshift_r(lo.y, hi.y, sh) & mask;
+        T v2 = __funnelshift_r(lo.z, hi.z, sh) & mask, v3 = __funnelshift_r(lo.w, hi.w, sh) & mask;
+        if (patch) {
+            if constexpr (W == 32) {
+                const uint4 t = reinterpret_cast<const uint4*>(tab)[4 * i + l];
+                v0 |= t.x; v1 |= t.y; v2 |= t.z; v3 |= t.w;
+            } else {
+                const ulonglong2 t0 = reinterpret_cast<const ulonglong2*>(tab)[2 * (4 * i + l)];
+                const ulonglong2 t1 = reinterpret_cast<const ulonglong2*>(tab)[2 * (4 * i + l) + 1];
+                v0 |= t0.x; v1 |= t0.y; v2 |= t1.x; v3 |= t1.y;
+            }
+        }
+        v1 += v0; v2 += v1; v3 += v2;                                    // prefix inside the row
+        T inc = v3;                                                      // inclusive scan of the row sums over the quad
         T t = __shfl_up_sync(kFull, inc, 1, 4);
         if (l >= 1) inc += t;
         t = __shfl_up_sync(kFull, inc, 2, 4);
         if (l >= 2) inc += t;
         const T tot = __shfl_sync(kFull, inc, 3, 4);
-        const T off = carry + (inc - v[i][3]);
-        v[i][0] += off; v[i][1] += off; v[i][2] += off; v[i][3] += off;
+        const T off = carry + (inc - v3);
         carry += tot;
-    }
-    const bool vec_ok = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
-    if (__all_sync(kFull, vec_ok || m <= 0)) {
-        if (m > 0) {
-#pragma unroll
-            for (int i = 0; i < 8; i++) {
+        v0 += off; v1 += off; v2 += off; v3 += off;
+        if (vec) {
+            if (m > 0) {
                 if constexpr (W == 32) {
-                    __stcs(reinterpret_cast<uint4*>(x) + 4 * i + l, make_uint4(v[i][0], v[i][1], v[i][2], v[i][3]));
+                    __stcs(reinterpret_cast<uint4*>(x) + 4 * i + l, make_uint4(v0, v1, v2, v3));
                 } else {
                     ulonglong2* p = reinterpret_cast<ulonglong2*>(x) + 2 * (4 * i + l);
-                    __stcs(p, make_ulonglong2(v[i][0], v[i][1]));
-                    __stcs(p + 1, make_ulonglong2(v[i][2], v[i][3]));
+                    __stcs(p, make_ulonglong2(v0, v1));
+                    __stcs(p + 1, make_ulonglong2(v2, v3));
                 }
             }
+        } else {
+            const int jx = 16 * i + 4 * l;
+            if (jx < m) x[jx] = v0;
+            if (jx + 1 < m) x[jx + 1] = v1;
+            if (jx + 2 < m) x[jx + 2] = v2;
+            if (jx + 3 < m) x[jx + 3] = v3;
         }
-    } else {
-#pragma unroll
-        for (int i = 0; i < 8; i++)
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-                const int jx = 16 * i + 4 * l + c;
-                if (jx < m) x[jx] = v[i][c];
-            }
     }
 }
 
