@@ -119,7 +119,7 @@ struct BlockAt {                       // where the quad's block is
 };
 
 template <int W>
-__global__ void __launch_bounds__(kDecThreads, (W == 32) ? 3 : 2) k_dec_tiles(DecArgs a) {
+__global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(DecArgs a) {
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
     extern __shared__ __align__(16) unsigned char dec_smem[];

@@ -13,7 +13,7 @@ namespace bfsc {
 
 constexpr int kDecBlocks = 8;                 // blocks per warp batch
 constexpr int kDecSpanMax = 17;               // largest staged block, in 16-byte chunks (272 B)
-constexpr int kDecSlotChunks = 19;            // slot stride: one chunk of slack for the unpack's second read; 19 q mod 8 distinct
+constexpr int kDecSlotChunks = 18;            // slot stride: one chunk of slack for the unpack's second read
 constexpr int kDecStageChunks = kDecBlocks * kDecSlotChunks;
 
 __device__ __forceinline__ void dec_cp_async16(void* smem_dst, const void* gmem_src) {
