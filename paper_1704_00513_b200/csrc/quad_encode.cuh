@@ -114,6 +114,14 @@ __device__ __forceinline__ uint32_t quad_max(uint32_t x) {
 // thresholds at which a value of width top-t is an exception); the chain of windows stops when
 // the exceptions above the window alone cost at least the best size, and jumps over widths no
 // value has. Returns key = size << 14 | (64 - b) << 7 | n_exc in every lane of the quad.
+// Position of the most significant set bit (0xffffffff for 0). volatile: the widths are recomputed in
+// every window instead of being kept in 32 registers across the window loop.
+__device__ __forceinline__ uint32_t msb_pos(uint32_t x) {
+    uint32_t r;
+    asm volatile("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
+
 template <int W>
 __device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
     const int l = quad_l();
@@ -128,10 +136,10 @@ __device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
     bool active = true;
     while (true) {
         uint32_t acc[3] = {0u, 0u, 0u};
-        const int off = top - 32;                    // t = top - width = clz + off
+        const int K = 4 * (top - 1);                 // t = top - width = (top - 1) - msb_pos; msb_pos(0) = -1
 #pragma unroll
         for (int i = 0; i < 32; i++)                 // t < 0 or t >= 8: the shift clamps to 0
-            acc[i / 12] += shl32(0x11111111u, (uint32_t)(4 * (__clz(d[i]) + off)));
+            acc[i / 12] += shl32(0x11111111u, (uint32_t)(K - 4 * (int)msb_pos(d[i])));
         uint32_t lo = (acc[0] & 0x0f0f0f0fu) + (acc[1] & 0x0f0f0f0fu) + (acc[2] & 0x0f0f0f0fu);
         uint32_t hi = ((acc[0] >> 4) & 0x0f0f0f0fu) + ((acc[1] >> 4) & 0x0f0f0f0fu) + ((acc[2] >> 4) & 0x0f0f0f0fu);
         lo = quad_add(lo);                           // bytes: exceptions added at s = 1,3,5,7 (b = top - s)
@@ -151,14 +159,14 @@ __device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
         const uint32_t n_bot = cnt_above + ((hi >> 24) & 0xffu);       // exceptions at b = top - 8
         active = active && top > 8 && (16u + exc_bytes<W>(n_bot)) < (best >> 14);
         if (!__any_sync(kFull, active)) break;
-        uint32_t below = 0;                          // widest value not above top - 8
+        int below = -1;                              // widest value not above top - 8 (as msb position; d_0 = 0 gives -1)
 #pragma unroll
         for (int i = 0; i < 32; i++) {
-            const uint32_t w = 32u - (uint32_t)__clz(d[i]);
-            below = max(below, (int)w <= top - 8 ? w : 0u);
+            const int f = (int)msb_pos(d[i]);
+            below = max(below, f < top - 8 ? f : -1);
         }
-        below = quad_max(below);
-        if (active) { top = (int)below; cnt_above = n_bot; }
+        below = (int)quad_max((uint32_t)(below + 1));                  // width = position + 1
+        if (active) { top = below; cnt_above = n_bot; }
     }
     return best;
 }
