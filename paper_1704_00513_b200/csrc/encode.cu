@@ -195,9 +195,8 @@ template <int W> struct EncSmem {
     static constexpr int kWarpChunks = kStageChunks + 2 * kImgBufChunks;     // + two image buffers (tile parity)
     static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
 };
-static_assert(RawCfg<32>::kAreaChunks * 16 >= 4 * kLateSlotWords64 * 8, "late_emit scratch");
 
-enum { kBarSizes = 1, kBarOffsets = 3, kBarFirst = 5 };                      // named barriers: +parity of the CTA's tile count
+enum { kBarSizes = 1, kBarOffsets = 3, kBarInfo = 5 };                      // named barriers: +parity of the CTA's tile count
 
 template <int W>
 __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(EncArgs a) {
@@ -266,13 +265,20 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
         if (!batch) pdl_wait();                          // the plan kernel's writes are visible from here on
         unsigned long long t1 = t != kNoTile ? draw() : kNoTile;
         prep(t1, 1);
-        bar_arrive(kBarFirst, kEncThreads);              // the second tile is posted
+        if (t != kNoTile) bar_arrive(kBarInfo + 1, kEncThreads);   // the second tile is posted
+        unsigned int ticket = 0xffffffffu;               // requested one scan iteration ahead: its latency is hidden
+        if (lane == 0 && t1 != kNoTile) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
         for (int k = 0; t != kNoTile; k++) {
             const int kp = k & 1;
             TR(t, 0);
             bar_sync(kBarSizes + kp, kEncThreads);       // the workers' sizes of tile t are in s_key[kp]
-            unsigned int ticket = 0xffffffffu;           // tile k+2: the atomic's latency hides behind the scan
-            if (lane == 0 && t1 != kNoTile) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+            unsigned long long t2 = kNoTile;
+            if (t1 != kNoTile) {                         // tile k+2 goes out first: the workers prefetch it during tile k+1
+                ticket = __shfl_sync(kFull, ticket, 0);
+                t2 = ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
+                prep(t2, (k + 2) & 3);
+                bar_arrive(kBarInfo + kp, kEncThreads);
+            }
 
             // E3: intra-tile scan (2 consecutive blocks per lane)
             const uint32_t k0 = s_key[kp][2 * lane], k1 = s_key[kp][2 * lane + 1];
@@ -347,13 +353,12 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
                 }
                 s_at[kp][jj] = at;
             }
-            ticket = __shfl_sync(kFull, ticket, 0);
-            const unsigned long long t2 = ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
-            prep(t2, (k + 2) & 3);
             TR(t, 4);
-            bar_arrive(kBarOffsets + kp, kEncThreads);   // offsets of tile k and the bookkeeping of tile k+2 are posted
+            bar_arrive(kBarOffsets + kp, kEncThreads);   // offsets of tile k are posted
             TRV(t, 15, (unsigned long long)smid() | ((unsigned long long)blockIdx.x << 32));
             t = t1; t1 = t2;
+            ticket = 0xffffffffu;
+            if (lane == 0 && t1 != kNoTile) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
         }
         return;
     }
@@ -375,6 +380,7 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
     uint32_t key_prev = 0;
     for (int k = 0;; k++) {
         uint32_t key = 0;
+        bool have_next = false;
         if (have) {
             const int m = s_m[k & 3][j];
             const T* raw = reinterpret_cast<const T*>(slot) +
@@ -413,11 +419,15 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
             const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)kImgCap);   // slow path, in global memory later
-            if (!wide) {                                                 // E4 into the image buffer
-                const bool fast = key != 0 && !late;
-                if (__any_sync(kFull, fast && n_exc > 0))
-                    col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
-                if (fast) {
+            const bool fast = !wide && key != 0 && !late;
+            if (!wide && __any_sync(kFull, fast && n_exc > 0))           // E4 into the image buffer: exceptions
+                col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
+            __syncwarp();                                                // the staged IDs are consumed:
+            bar_sync(kBarInfo + ((k + 1) & 1), kEncThreads);             // next tile posted -> prefetch it into the same slots
+            have_next = s_tile[(k + 1) & 3] != kNoTile;
+            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & 3][j], s_m[(k + 1) & 3][j]);
+            {
+                if (fast) {                                              // payload + header
                     if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
                     if (l == 0) {                                        // block header (FORMAT.md §2)
                         reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
@@ -431,20 +441,14 @@ __global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(En
         }
 
         unsigned long long at_prev = kSkip;
-        if (k == 0) bar_sync(kBarFirst, kEncThreads);                    // the second tile is posted
         if (k > 0) {                                                     // tile k-1: offsets resolved?
             bar_sync(kBarOffsets + ((k - 1) & 1), kEncThreads);
             if (key_prev != 0) at_prev = s_at[(k - 1) & 1][j];
             if (__any_sync(kFull, (key_prev & kLateBit) != 0)) {
                 const bool mine = (key_prev & kLateBit) != 0 && at_prev != kSkip;
                 late_emit<W>(ids + s_xoff[(k - 1) & 3][j], s_m[(k - 1) & 3][j], key_prev & ~kLateBit,
-                             mine ? a.out + at_prev : nullptr, reinterpret_cast<uint64_t*>(area));
+                             mine ? a.out + at_prev : nullptr);
             }
-        }
-        bool have_next = false;
-        if (have) {                                                      // next tile: posted before barrier 0 / kBarOffsets
-            have_next = s_tile[(k + 1) & 3] != kNoTile;
-            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & 3][j], s_m[(k + 1) & 3][j]);   // same slots
         }
         if (warp == 0 && have) TR(s_tile[k & 3], 10);
         if ((key_prev & kLateBit) == 0 && at_prev != kSkip) {            // copy tile k-1's image to its final place

@@ -10,63 +10,51 @@
 
 namespace bfsc {
 
-constexpr int kLateSlotWords64 = 132;          // u64 deltas per scratch slot (1056 B)
-
 // Whole warp calls; lane = 4q + l. x: the quad's block (first ID, re-read from global memory), m valid
 // IDs, key = size<<14 | (64-b)<<7 | n_exc, dst = final address of the block or nullptr (nothing to do
-// for this quad). scratch: 4 slots of kLateSlotWords64 u64 (the warp's staging area).
+// for this quad). No shared memory: lane l packs column l from global memory, lane 0 lists the exceptions.
 template <int W>
 __device__ __noinline__ void late_emit(const typename IdT<W>::T* __restrict__ x, int m, uint32_t key,
-                                       unsigned char* __restrict__ dst, uint64_t* __restrict__ scratch) {
+                                       unsigned char* __restrict__ dst) {
     using T = typename IdT<W>::T;
     constexpr uint32_t E = W / 8;
-    const int lane = threadIdx.x & 31, q = lane >> 2, l = lane & 3;
+    const int l = threadIdx.x & 3;
     const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
-    for (int h = 0; h < 2; h++) {
-        const bool on = ((q >> 2) == h) && dst != nullptr && m > 0;
-        uint64_t* slot = scratch + (q & 3) * kLateSlotWords64;
-        if (on) {
-            for (int j = l; j < kBlk; j += 4)
-                slot[j] = (j > 0 && j < m) ? (uint64_t)(T)(x[j] - x[j - 1]) : 0ull;          // E1 (L979-986)
-        }
-        __syncwarp();
-        if (on) {
-            if (b > 0) {                                                             // E4: column l
-                const uint64_t mask = b >= 64 ? ~0ull : ((1ull << b) - 1ull);
-                uint32_t* outp = reinterpret_cast<uint32_t*>(dst + 16) + l;
-                uint64_t lo = 0, hi = 0;
-                uint32_t have = 0;
-                for (int r = 0; r < 32; r++) {
-                    const uint64_t v = slot[4 * r + l] & mask;
-                    lo |= shl64(v, have);
-                    hi |= have ? shr64(v, 64u - have) : 0ull;                        // have < 32 here
-                    have += b;
-                    while (have >= 32u) {
-                        *outp = (uint32_t)lo;
-                        outp += 4;
-                        lo = (lo >> 32) | (hi << 32);
-                        hi >>= 32;
-                        have -= 32u;
-                    }
-                }
-            }
-            if (l == 0) {
-                reinterpret_cast<unsigned long long*>(dst)[0] = (unsigned long long)x[0];
-                reinterpret_cast<unsigned long long*>(dst)[1] = (unsigned long long)(b | (n_exc << 8));
-                if (n_exc > 0) {                                                     // then b < W
-                    unsigned char* e = dst + 16 + 16 * b;
-                    const uint32_t eb = exc_bytes<W>(n_exc);
-                    for (uint32_t t = 0; t < eb / 16; t++) reinterpret_cast<uint4*>(e)[t] = make_uint4(0, 0, 0, 0);
-                    T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
-                    uint32_t rank = 0;
-                    for (int j = 0; j < kBlk; j++) {
-                        const uint64_t hv = slot[j] >> b;
-                        if (hv) { e[rank] = (unsigned char)j; high[rank] = (T)hv; rank++; }
-                    }
-                }
+    if (dst == nullptr || m <= 0) return;
+    auto delta = [&](int j) -> uint64_t { return (j > 0 && j < m) ? (uint64_t)(T)(x[j] - x[j - 1]) : 0ull; };   // E1 (L979-986)
+    if (b > 0) {                                                             // E4: column l
+        const uint64_t mask = b >= 64 ? ~0ull : ((1ull << b) - 1ull);
+        uint32_t* outp = reinterpret_cast<uint32_t*>(dst + 16) + l;
+        uint64_t lo = 0, hi = 0;
+        uint32_t have = 0;
+        for (int r = 0; r < 32; r++) {
+            const uint64_t v = delta(4 * r + l) & mask;
+            lo |= shl64(v, have);
+            hi |= have ? shr64(v, 64u - have) : 0ull;                        // have < 32 here
+            have += b;
+            while (have >= 32u) {
+                *outp = (uint32_t)lo;
+                outp += 4;
+                lo = (lo >> 32) | (hi << 32);
+                hi >>= 32;
+                have -= 32u;
             }
         }
-        __syncwarp();
+    }
+    if (l == 0) {
+        reinterpret_cast<unsigned long long*>(dst)[0] = (unsigned long long)x[0];
+        reinterpret_cast<unsigned long long*>(dst)[1] = (unsigned long long)(b | (n_exc << 8));
+        if (n_exc > 0) {                                                     // then b < W
+            unsigned char* e = dst + 16 + 16 * b;
+            const uint32_t eb = exc_bytes<W>(n_exc);
+            for (uint32_t t = 0; t < eb / 16; t++) reinterpret_cast<uint4*>(e)[t] = make_uint4(0, 0, 0, 0);
+            T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
+            uint32_t rank = 0;
+            for (int j = 0; j < kBlk; j++) {
+                const uint64_t hv = delta(j) >> b;
+                if (hv) { e[rank] = (unsigned char)j; high[rank] = (T)hv; rank++; }
+            }
+        }
     }
 }
 
