@@ -199,7 +199,7 @@ template <int W> struct EncSmem {
 enum { kBarSizes = 1, kBarOffsets = 3, kBarInfo = 5 };                      // named barriers: +parity of the CTA's tile count
 
 template <int W>
-__global__ void __launch_bounds__(kEncThreads, (W == 32) ? 2 : 2) k_enc_tiles(EncArgs a) {
+__global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
     extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | image buffer 0 | image buffer 1
     __shared__ uint32_t s_key[2][kTileR];                // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block

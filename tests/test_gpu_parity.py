@@ -224,3 +224,81 @@ def test_host_api_roundtrip(B, oracle_mod):
         h_back = torch.empty(n, dtype=t.dtype).pin_memory()
         assert B.decompress_host(h_out, nbytes, W, h_back, scratch) == n
         assert torch.equal(h_back, t)
+
+
+def test_rmat_config3_reduced(B, oracle_mod):
+    """config 3 recipe at scale 16: per-level frontiers, 16 buffers by contiguous vertex range, one
+    batched call per level, 1 KB raw threshold (first/last levels go RAW or empty)."""
+    G = rmat.Graph(16, 16, seed=3)
+    for root in G.roots(2, seed=3):
+        for f in G.bfs_frontiers(root):
+            vals, off = streams.split_block(f, 16, 1 << 16)
+            run_batch(B, oracle_mod, streams.as_ids(vals, 32), off, 32, 1024)
+
+
+def test_rmat_config4_reduced(B, oracle_mod):
+    """config 4 recipe at scale 16: u64 IDs, 64 destination buffers (8x8 partition read as a 64-way
+    block partition), 1 KB threshold."""
+    G = rmat.Graph(16, 16, seed=4)
+    for root in G.roots(2, seed=4):
+        for f in G.bfs_frontiers(root):
+            vals, off = streams.split_block(f, 64, 1 << 16)
+            run_batch(B, oracle_mod, streams.as_ids(vals, 64), off, 64, 1024)
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_sweep_config5_reduced(B, oracle_mod, W):
+    """config 5 recipe: single buffers of 1 KB .. 4 MB (powers of 4), gap means 1, 16, 4096; plus a batch
+    of 4096 buffers of 256 B .. 64 KB (log-uniform sizes), thresholds 0 and 1024."""
+    for k in range(5, 12):
+        n = (4 ** k) // (W // 8)
+        for mean in (1.0, 16.0, 4096.0):
+            if W == 32 and n * mean >= 2 ** 32:
+                continue                                   # exceeds the u32 ID space (DESIGN.md §1)
+            t = streams.gap_stream(n, mean, seed=5, W=W)
+            run_batch(B, oracle_mod, t, torch.tensor([0, n], dtype=torch.int64), W, 0)
+    if W == 32:
+        counts = streams.log_uniform_counts(4096, 8, 16, W, seed=5)
+        ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=W)
+        for thr in (0, 1024):
+            run_batch(B, oracle_mod, ids, off, W, thr)
+
+
+def test_config2_full_size_sampled(B, oracle_mod):
+    """BASELINE config 2 at its full size (2^24 IDs, the launch configuration bench.py times): decoded IDs
+    equal the input everywhere; directory walk (strictly increasing, sizes recomputed from the block
+    headers, total = header + directory + blocks); 256 sampled blocks per stream memcmp-equal to the
+    oracle's encoding of the same 128 IDs (blocks are independent: FORMAT.md §2)."""
+    dev = torch.device("cuda")
+    n, W = 1 << 24, 32
+    rng = np.random.default_rng(7)
+    for sub, (mean, outl) in enumerate(((2.0, 0.0), (256.0, 0.0), (256.0, 0.01))):
+        ids = streams.gap_stream(n, mean, seed=2, W=W, outlier_frac=outl, sub=sub, device=dev)
+        cap = B.compress_bound(n, W)
+        out = torch.empty(cap, dtype=torch.uint8, device=dev)
+        nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
+        ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
+        status = torch.zeros(1, dtype=torch.int32, device=dev)
+        B.compress(ids, n, W, 0, out, nbytes, ws, status)
+        back = torch.empty(n, dtype=ids.dtype, device=dev)
+        n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+        B.decompress(out, cap, W, back, n_out, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0 and int(n_out.item()) == n
+        assert torch.equal(back, ids)
+        total = int(nbytes.item())
+        s = out[:total].cpu().numpy()
+        nb = n // 128
+        assert s[:4].tobytes() == b"BFSC" and s[4] == 1 and s[5] == W and s[6] == 1
+        assert int(s[8:16].view(np.uint64)[0]) == n and int(s[16:24].view(np.uint64)[0]) == total
+        assert int(s[24:28].view(np.uint32)[0]) == nb
+        d = s[32:32 + 4 * (nb + 1)].view(np.uint32).astype(np.int64)
+        assert d[0] * 16 == 32 + ((4 * (nb + 1) + 15) // 16) * 16 and d[nb] * 16 == total
+        b = s[d[:-1] * 16 + 8].astype(np.int64)
+        ne = s[d[:-1] * 16 + 9].astype(np.int64)
+        exc = np.where(ne > 0, ((((ne + 3) // 4) * 4 + 4 * ne + 15) // 16) * 16, 0)
+        assert np.array_equal((d[1:] - d[:-1]) * 16, 16 + 16 * b + exc)
+        host = ids.cpu().numpy().view(np.uint32)
+        for k in rng.integers(0, nb, size=256):
+            ref = oracle_mod.compress(host[128 * k:128 * k + 128], 0)
+            assert np.array_equal(s[d[k] * 16:d[k + 1] * 16], ref[48:]), f"block {k} differs from the oracle"
