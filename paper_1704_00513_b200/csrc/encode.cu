@@ -13,7 +13,7 @@ struct EncArgs {
     const unsigned long long* in_off;   // n_buf+1 element offsets, or nullptr (single buffer of n_single IDs)
     unsigned long long n_single;
     uint32_t n_buf;
-    uint32_t grid;                      // CTAs of k_enc_tiles: their first tile is blockIdx.x, tickets start here
+    uint32_t grid;                      // CTAs of k_enc_tiles: their first tiles are blockIdx.x (+ grid), tickets start at 2 grid
     unsigned long long thr;             // raw threshold in bytes
     unsigned char* out;
     unsigned long long out_cap;
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
             a.ws.blk_first[0] = 0; a.ws.blk_first[1] = nb;
             a.ws.fixed_prefix[0] = 0; a.ws.fixed_prefix[1] = fixed;
             a.ws.stream_start[0] = 0; a.ws.stream_start[1] = 0;
-            a.ws.hdr->total_blocks = nb; a.ws.hdr->fixed_total = fixed; a.ws.hdr->ticket = a.grid;
+            a.ws.hdr->total_blocks = nb; a.ws.hdr->fixed_total = fixed; a.ws.hdr->ticket = 2 * a.grid;
             a.ws.hdr->grand16 = 0; a.ws.hdr->total_out = fixed; a.ws.hdr->ok = ok ? 1u : 0u;
             if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
         }
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         a.ws.stream_start[a.n_buf] = 0;
         a.ws.hdr->total_blocks = carry.a;
         a.ws.hdr->fixed_total = carry.b;
-        a.ws.hdr->ticket = a.grid;
+        a.ws.hdr->ticket = 2 * a.grid;
         a.ws.hdr->grand16 = 0;
         a.ws.hdr->total_out = carry.b;
         const bool ok = !bad && carry.a <= a.ws.blk_cap && (carry.a + kTileR - 1) / kTileR <= a.ws.tile_cap;
@@ -190,20 +190,34 @@ constexpr int kImgCap = 256;                                  // bytes of a bloc
 constexpr int kImgSlotChunks = 17;                            // slot stride (16-B chunks): 17 q mod 8 are all distinct
 constexpr int kImgBufChunks = kQuadBlocks * kImgSlotChunks;   // one image buffer of a warp
 
+constexpr int kDefer = 2;                                     // a tile's images leave kDefer tiles after they were packed
+constexpr int kNB = kDefer + 1;                               // image buffers / size and offset tables per CTA
+
 template <int W> struct EncSmem {
     static constexpr int kStageChunks = RawCfg<W>::kAreaChunks;              // per worker warp: staged raw IDs
-    static constexpr int kWarpChunks = kStageChunks + 2 * kImgBufChunks;     // + two image buffers (tile parity)
+    static constexpr int kWarpChunks = kStageChunks + kNB * kImgBufChunks;   // + the image buffers
     static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
 };
 
-enum { kBarSizes = 1, kBarOffsets = 3, kBarInfo = 5 };                      // named barriers: +parity of the CTA's tile count
+enum { kBarSizes = 1, kBarOffsets = kBarSizes + kNB, kBarWorkers = kBarOffsets + kNB };   // named barriers (+ tile count mod kNB)
 
+// k_enc_tiles: CTA = 8 worker warps + 1 scan warp; a CTA's k-th tile is "tile k" below.
+//   workers, iteration k:  E1/E2 of tile k -> sizes in s_key[k % kNB], the last warp publishes the tile's
+//       aggregate; exceptions; next tile's raw IDs prefetched (cp.async) into the staging slots; payload
+//       packed into image buffer k % kNB; then the offsets of tile k - kDefer are awaited and its images
+//       copied out. Worker warp 0 also draws the tickets and prepares the bookkeeping, two tiles ahead.
+//   scan warp, tile k: sizes -> intra-tile scan -> decoupled look-back (device-wide exclusive scan of
+//       the block sizes) -> final offsets in s_at[k % kNB], directory entries, stream starts, header.
+//       It may lag up to kDefer tiles behind the workers: a look-back that waits for a slow
+//       predecessor CTA does not stall this CTA's workers.
+// Tiles: the first two of a CTA are blockIdx.x and blockIdx.x + gridDim.x, the rest come from the ticket
+// counter, each drawn at the same point of the pipeline: a lower tile number means "sizes posted earlier".
 template <int W>
 __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
-    extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | image buffer 0 | image buffer 1
-    __shared__ uint32_t s_key[2][kTileR];                // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
-    __shared__ unsigned long long s_at[2][kTileR];       // scan warp: final byte offset of the block, or kSkip
+    extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | kNB image buffers
+    __shared__ uint32_t s_key[kNB][kTileR];              // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
+    __shared__ unsigned long long s_at[kNB][kTileR];     // scan warp: final byte offset of the block, or kSkip
     __shared__ uint32_t s_off16[kTileR];                 // exclusive scan of the sizes inside the tile (16-B units)
     __shared__ int s_m[4][kTileR];                       // ring of tile bookkeeping: valid IDs of each block (0 = none)
     __shared__ unsigned long long s_xoff[4][kTileR];     // element offset of the block's first ID
@@ -216,69 +230,48 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     const T* ids = reinterpret_cast<const T*>(a.ids);
     if (threadIdx.x < 2) s_agg[threadIdx.x] = 0;
 
+    // Single-buffer calls know their geometry from the arguments: the first tiles start without waiting
+    // for the plan kernel; only the ticket counter and the look-back states need it.
+    const unsigned long long nb_single = (a.n_single + kBlk - 1) / kBlk;
+    unsigned long long total = nb_single;
+    if (batch) {
+        pdl_wait();
+        total = a.ws.hdr->ok != 0 ? a.ws.hdr->total_blocks : 0ull;
+    }
+    const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
+
+    auto prep = [&](unsigned long long t, int p) {       // bookkeeping of tile t into ring slot p (one warp)
+        if (lane == 0) s_tile[p] = t;
+        if (t == kNoTile) return;
+        for (int jj = lane; jj < kTileR; jj += 32) {
+            const unsigned long long g = t * kTileR + jj;
+            int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
+            if (g < total) {
+                if (batch) {
+                    i = find_buf(a.ws.blk_first, a.n_buf, g);
+                    const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
+                    m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+                    xoff = buf_start(a, i) + kBlk * k;
+                } else {
+                    m = (int)min((unsigned long long)kBlk, a.n_single - kBlk * g);
+                    xoff = kBlk * g;
+                }
+            }
+            s_m[p][jj] = m; s_xoff[p][jj] = xoff; s_buf[p][jj] = i;
+        }
+    };
+
     if (warp == kEncWorkers) {
         // =============================== scan warp ===============================
-        // Single-buffer calls know their geometry from the arguments: the first tile (= blockIdx.x) starts
-        // without waiting for the plan kernel; only the ticket counter and the look-back states need it.
-        const unsigned long long nb_single = (a.n_single + kBlk - 1) / kBlk;
         const unsigned long long f1_single = 32ull + ((4ull * (nb_single + 1) + 15ull) & ~15ull);
-        unsigned long long total = nb_single;
-        if (batch) {
-            pdl_wait();
-            total = a.ws.hdr->ok != 0 ? a.ws.hdr->total_blocks : 0ull;
-        }
-        const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
-
-        auto draw = [&]() -> unsigned long long {
-            unsigned long long t = 0;
-            if (lane == 0) t = atomicAdd(&a.ws.hdr->ticket, 1u);
-            t = __shfl_sync(kFull, t, 0);
-            return t < n_tiles ? t : kNoTile;
-        };
-        auto prep = [&](unsigned long long t, int p) {   // bookkeeping of tile t into ring slot p
-            if (lane == 0) s_tile[p] = t;
-            if (t == kNoTile) return;
-            for (int jj = lane; jj < kTileR; jj += 32) {
-                const unsigned long long g = t * kTileR + jj;
-                int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
-                if (g < total) {
-                    if (batch) {
-                        i = find_buf(a.ws.blk_first, a.n_buf, g);
-                        const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
-                        m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-                        xoff = buf_start(a, i) + kBlk * k;
-                    } else {
-                        m = (int)min((unsigned long long)kBlk, a.n_single - kBlk * g);
-                        xoff = kBlk * g;
-                    }
-                }
-                s_m[p][jj] = m; s_xoff[p][jj] = xoff; s_buf[p][jj] = i;
-            }
-        };
-
-        // A CTA works on tile k (sizes, pack) while the scan warp resolves the offsets of tile k-1, so
-        // tickets are drawn two tiles ahead: always at the same point of the pipeline, so that a lower
-        // tile number means "sizes posted earlier" and a look-back rarely has to wait.
-        unsigned long long t = blockIdx.x < n_tiles ? (unsigned long long)blockIdx.x : kNoTile;
-        prep(t, 0);
-        __syncthreads();                                 // barrier 0: the first tile is posted
+        __syncthreads();                                 // barrier 0: the first two tiles are posted (by warp 0)
         if (!batch) pdl_wait();                          // the plan kernel's writes are visible from here on
-        unsigned long long t1 = t != kNoTile ? draw() : kNoTile;
-        prep(t1, 1);
-        if (t != kNoTile) bar_arrive(kBarInfo + 1, kEncThreads);   // the second tile is posted
-        unsigned int ticket = 0xffffffffu;               // requested one scan iteration ahead: its latency is hidden
-        if (lane == 0 && t1 != kNoTile) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
-        for (int k = 0; t != kNoTile; k++) {
-            const int kp = k & 1;
+        int kp = 0;                                      // k % kNB
+        for (int k = 0;; k++) {
+            const unsigned long long t = s_tile[k & 3];  // posted before the sizes of tile k-1 arrived
+            if (t == kNoTile) break;
             TR(t, 0);
             bar_sync(kBarSizes + kp, kEncThreads);       // the workers' sizes of tile t are in s_key[kp]
-            unsigned long long t2 = kNoTile;
-            if (t1 != kNoTile) {                         // tile k+2 goes out first: the workers prefetch it during tile k+1
-                ticket = __shfl_sync(kFull, ticket, 0);
-                t2 = ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
-                prep(t2, (k + 2) & 3);
-                bar_arrive(kBarInfo + kp, kEncThreads);
-            }
 
             // E3: intra-tile scan (2 consecutive blocks per lane)
             const uint32_t k0 = s_key[kp][2 * lane], k1 = s_key[kp][2 * lane + 1];
@@ -356,36 +349,46 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             TR(t, 4);
             bar_arrive(kBarOffsets + kp, kEncThreads);   // offsets of tile k are posted
             TRV(t, 15, (unsigned long long)smid() | ((unsigned long long)blockIdx.x << 32));
-            t = t1; t1 = t2;
-            ticket = 0xffffffffu;
-            if (lane == 0 && t1 != kNoTile) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+            kp = kp == kNB - 1 ? 0 : kp + 1;
         }
         return;
     }
 
     // =============================== worker warps ===============================
-    // Iteration k: E1/E2 of tile k -> sizes posted; E4 of tile k into image buffer k&1; then the
-    // offsets of tile k-1 (resolved by the scan warp meanwhile) are awaited, the next tile's raw IDs
-    // prefetched into the (now free) staging area, and tile k-1's images copied out.
-    // Loop-carried state is kept small (registers): the bookkeeping ring is re-read where needed.
     const int q = lane >> 2, l = lane & 3;
     uint4* area = dyn_smem + warp * EncSmem<W>::kWarpChunks;
     uint4* slot = area + raw_slot_chunk<W>(q);                           // staging: the quad's raw IDs
     unsigned char* img0 = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks + kImgSlotChunks * q);
     const int j = warp * kQuadBlocks + q;
-    constexpr uint32_t kLateBit = 1u << 31;                              // in key_prev: assembled by late_emit
+    constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
+    if (warp == 0) {                                                     // the CTA's first two tiles are static
+        const unsigned long long t0 = blockIdx.x, t1 = (unsigned long long)blockIdx.x + gridDim.x;
+        prep(t0 < n_tiles ? t0 : kNoTile, 0);
+        prep(t0 < n_tiles && t1 < n_tiles ? t1 : kNoTile, 1);
+    }
     __syncthreads();                                                     // barrier 0
     bool have = s_tile[0] != kNoTile;
     if (have) quad_prefetch<W>(slot, ids + s_xoff[0][j], s_m[0][j]);
-    uint32_t key_prev = 0;
+    uint32_t key_hist[kDefer] = {};                                      // keys of the tiles whose images wait in shared memory
+    unsigned int ticket = 0xffffffffu;                                   // warp 0: requested one iteration before it is used
+    int kp = 0;                                                          // k % kNB
+    int n_wait = 0, ke = 0;                                              // tiles packed but not copied out yet; next one to copy out
     for (int k = 0;; k++) {
         uint32_t key = 0;
         bool have_next = false;
         if (have) {
+            if (warp == 0 && k >= 1) {                                   // tile k+1: ticket -> bookkeeping (ring slot (k+1) & 3)
+                unsigned long long t = kNoTile;
+                if (s_tile[k & 3] != kNoTile) {
+                    ticket = __shfl_sync(kFull, ticket, 0);
+                    if (ticket < n_tiles) t = ticket;
+                }
+                prep(t, (k + 1) & 3);
+            }
             const int m = s_m[k & 3][j];
             const T* raw = reinterpret_cast<const T*>(slot) +
                            (reinterpret_cast<uintptr_t>(ids + s_xoff[k & 3][j]) & 15) / sizeof(T);
-            unsigned char* img = img0 + (k & 1) * (kImgBufChunks * 16);
+            unsigned char* img = img0 + kp * (kImgBufChunks * 16);
             if (warp == 0) TR(s_tile[k & 3], 6);
             cp_async_wait_all();
             __syncwarp();
@@ -397,9 +400,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             if (!wide) key = quad_choose_b<W>(d);                        // E2
             else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(img));
             if (m <= 0) key = 0;
-            if (l == 0) s_key[k & 1][j] = key;
+            if (l == 0) s_key[kp][j] = key;
             {   // The tile's aggregate goes out as soon as the LAST worker warp has its sizes — not when the scan
-                // warp gets to it: that warp may still be inside the previous tile's look-back, and every
+                // warp gets to it: that warp may still be inside an earlier tile's look-back, and every
                 // later tile in flight waits for this number.
                 uint32_t z = l == 0 ? key >> 18 : 0u;
                 z += __shfl_xor_sync(kFull, z, 4); z += __shfl_xor_sync(kFull, z, 8); z += __shfl_xor_sync(kFull, z, 16);
@@ -415,52 +418,67 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 }
             }
             if (warp == 0) TR(s_tile[k & 3], 8);
-            bar_arrive(kBarSizes + (k & 1), kEncThreads);
+            bar_arrive(kBarSizes + kp, kEncThreads);
+            if (warp == 0) {                                             // ticket of tile k+2 (used next iteration)
+                ticket = 0xffffffffu;
+                if (lane == 0 && s_tile[(k + 1) & 3] != kNoTile) {
+                    pdl_wait();
+                    ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+                }
+            }
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
             const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)kImgCap);   // slow path, in global memory later
             const bool fast = !wide && key != 0 && !late;
             if (!wide && __any_sync(kFull, fast && n_exc > 0))           // E4 into the image buffer: exceptions
                 col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
-            __syncwarp();                                                // the staged IDs are consumed:
-            bar_sync(kBarInfo + ((k + 1) & 1), kEncThreads);             // next tile posted -> prefetch it into the same slots
+            bar_sync(kBarWorkers, kEncWorkers * 32);                     // all staged IDs consumed; tile k+1 is posted
             have_next = s_tile[(k + 1) & 3] != kNoTile;
-            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & 3][j], s_m[(k + 1) & 3][j]);
-            {
-                if (fast) {                                              // payload + header
-                    if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
-                    if (l == 0) {                                        // block header (FORMAT.md §2)
-                        reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
-                        reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
-                    }
+            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & 3][j], s_m[(k + 1) & 3][j]);   // same slots
+            if (fast) {                                                  // payload + header
+                if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
+                if (l == 0) {                                            // block header (FORMAT.md §2)
+                    reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
+                    reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
                 }
             }
             if (late) key |= kLateBit;
-            __syncwarp();                                                // staged IDs consumed, image complete
+            __syncwarp();                                                // image complete
             if (warp == 0) TR(s_tile[k & 3], 9);
+            n_wait++;
         }
 
-        unsigned long long at_prev = kSkip;
-        if (k > 0) {                                                     // tile k-1: offsets resolved?
-            bar_sync(kBarOffsets + ((k - 1) & 1), kEncThreads);
-            if (key_prev != 0) at_prev = s_at[(k - 1) & 1][j];
-            if (__any_sync(kFull, (key_prev & kLateBit) != 0)) {
-                const bool mine = (key_prev & kLateBit) != 0 && at_prev != kSkip;
-                late_emit<W>(ids + s_xoff[(k - 1) & 3][j], s_m[(k - 1) & 3][j], key_prev & ~kLateBit,
-                             mine ? a.out + at_prev : nullptr);
+        // copy out the oldest waiting tile: tile k - kDefer while tiles keep coming, then drain
+        const int w = n_wait - (have ? 1 : 0);                           // waiting tiles older than tile k
+        if (w > 0 && (w == kDefer || !have)) {
+            static_assert(kDefer == 2, "key_hist selection below");
+            const uint32_t key_e = w == 2 ? key_hist[1] : key_hist[0];   // key of the CTA's tile ke
+            int kpe = kp - w;                                            // its buffer: ke % kNB
+            if (kpe < 0) kpe += kNB;
+            bar_sync(kBarOffsets + kpe, kEncThreads);                    // its offsets are resolved
+            unsigned long long at = kSkip;
+            if (key_e != 0) at = s_at[kpe][j];
+            if (__any_sync(kFull, (key_e & kLateBit) != 0)) {
+                const bool mine = (key_e & kLateBit) != 0 && at != kSkip;
+                late_emit<W>(ids + s_xoff[ke & 3][j], s_m[ke & 3][j], key_e & ~kLateBit, mine ? a.out + at : nullptr);
             }
+            if ((key_e & kLateBit) == 0 && at != kSkip) {                // image -> its final place
+                const uint4* src = reinterpret_cast<const uint4*>(img0 + kpe * (kImgBufChunks * 16));
+                uint4* dst = reinterpret_cast<uint4*>(a.out + at);
+                const uint32_t n16 = key_e >> 18;
+                for (uint32_t c = l; c < n16; c += 4) __stcs(dst + c, src[c]);
+            }
+            __syncwarp();
+            n_wait--;
+            ke++;
         }
-        if (warp == 0 && have) TR(s_tile[k & 3], 10);
-        if ((key_prev & kLateBit) == 0 && at_prev != kSkip) {            // copy tile k-1's image to its final place
-            const uint4* src = reinterpret_cast<const uint4*>(img0 + ((k - 1) & 1) * (kImgBufChunks * 16));
-            uint4* dst = reinterpret_cast<uint4*>(a.out + at_prev);
-            const uint32_t n16 = key_prev >> 18;
-            for (uint32_t c = l; c < n16; c += 4) __stcs(dst + c, src[c]);
+        if (!have && n_wait == 0) break;
+        if (have) {
+#pragma unroll
+            for (int x = kDefer - 1; x > 0; x--) key_hist[x] = key_hist[x - 1];
+            key_hist[0] = key;
+            kp = kp == kNB - 1 ? 0 : kp + 1;
         }
-        __syncwarp();
-        if (warp == 0 && have) TR(s_tile[k & 3], 11);
-        if (!have) break;
-        key_prev = key;
         have = have_next;
     }
 }
