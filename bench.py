@@ -37,6 +37,9 @@ SEED = 2
 W = 32
 METRIC = "codec_throughput_encode_plus_decode"
 UNIT = "GB/s"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (k_enc_tiles<32>, stream a,
+# 2^24 IDs), from the committed `ncu --set full` capture profiles/r1_enc_tiles_ncu_summary.txt (67.31 + 1.86 MB).
+NCU_TRAFFIC_BYTES = {"encode_a": 69_168_384, "decode_a": 25_263_104, "source": "profiles/r1_*_tiles_ncu_summary.txt"}
 
 
 def peaks():
@@ -271,10 +274,14 @@ def run_ours(args, rank, local_rank, world):
     # dominant call = encode of stream (a): most raw bytes per compressed byte, the headline dense frontier
     dom = STREAMS[0][0]
     alg_a = raw_bytes + comp[0] + 8
-    roof = {"bound": "hbm", "kernel": "bfsc_compress call on stream a (all its launches)", "achieved": per[dom]["encode_alg_GBps"],
+    full = args.log2n == LOG2_N
+    roof = {"bound": "hbm", "kernel": "k_enc_tiles<32> (+ its 1-CTA k_enc_plan): the bfsc_compress call on stream a",
+            "achieved": per[dom]["encode_alg_GBps"],
             "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": per[dom]["encode_alg_GBps"] / peak,
-            "algorithmic_bytes_per_launch": alg_a, "traffic": None,
-            "decode": {"achieved": per[dom]["decode_alg_GBps"], "frac": per[dom]["decode_alg_GBps"] / peak}}
+            "algorithmic_bytes_per_launch": alg_a, "traffic": NCU_TRAFFIC_BYTES["encode_a"] if full else None,
+            "traffic_source": NCU_TRAFFIC_BYTES["source"],
+            "decode": {"kernel": "k_dec_tiles<32>: the bfsc_decompress call on stream a", "achieved": per[dom]["decode_alg_GBps"],
+                       "frac": per[dom]["decode_alg_GBps"] / peak, "traffic": NCU_TRAFFIC_BYTES["decode_a"] if full else None}}
     cpu = None
     if not args.no_cpu:
         cores = len(os.sched_getaffinity(0))
@@ -301,7 +308,7 @@ def run_ours(args, rank, local_rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--steps", type=int, default=1500)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--log2n", type=int, default=LOG2_N, help="IDs per stream = 2^log2n (default: the BASELINE size)")
