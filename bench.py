@@ -121,10 +121,18 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     cores = len(os.sched_getaffinity(0))
-    n = 1 << 22                                            # bounded sample: first 2^22 IDs of each stream
-    host = [np_view(t) for t in make_streams("cpu", n)]
-    for _ in range(max(args.warmup, 0) and 1):
-        time_oracle([h[:1 << 16] for h in host], cores)
+    # Bounded sample: the first 2^p IDs of each stream, p chosen from a quick calibration so that the whole
+    # --steps K run takes about 90 s of CPU work (p in 14..22).
+    full = [np_view(t) for t in make_streams("cpu", 1 << 22)]
+    time_oracle([h[:1 << 16] for h in full], cores)                       # warm-up (builds the oracle's C library)
+    cal, _, _ = time_oracle([h[:1 << 18] for h in full], cores)
+    per_id = cal / (3 << 18)
+    budget = 90.0 / max(args.steps, 1)
+    p = 22
+    while p > 14 and per_id * (3 << p) > budget:
+        p -= 1
+    n = 1 << p
+    host = [h[:n] for h in full]
     times = []
     raw = ratio = 0
     for _ in range(args.steps):
@@ -132,7 +140,7 @@ def run_reference(args, rank, world):
         times.append(dt)
     ms = 1e3 * sum(times) / len(times)
     val = raw / (ms * 1e-3) / 1e9
-    sample = f"first 2^22 of the 2^24 IDs of each of the 3 streams, encode+decode, {cores} threads"
+    sample = f"first 2^{p} of the 2^24 IDs of each of the 3 streams, encode+decode, {cores} threads"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
