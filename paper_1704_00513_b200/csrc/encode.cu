@@ -186,8 +186,8 @@ __device__ __forceinline__ unsigned long long lookback(const unsigned long long*
     return acc;
 }
 
-constexpr int kImgCap = 256;                                  // bytes of a block image the fast path can hold
-constexpr int kImgSlotChunks = 17;                            // slot stride (16-B chunks): 17 q mod 8 are all distinct
+constexpr int kImgCap = 320;                                  // bytes of a block image the fast path can hold (b = 16 + exceptions)
+constexpr int kImgSlotChunks = 21;                            // slot stride (16-B chunks): 21 q mod 8 are all distinct
 constexpr int kImgBufChunks = kQuadBlocks * kImgSlotChunks;   // one image buffer of a warp
 
 constexpr int kDefer = 2;                                     // a tile's images leave kDefer tiles after they were packed

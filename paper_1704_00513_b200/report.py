@@ -1,0 +1,163 @@
+"""Throughput / ratio report for BASELINE.json configs 3, 4 and 5 (configs[1] is bench.py's line).
+
+    python -m paper_1704_00513_b200.report --config 3            # R-MAT 22, u32, 16 buffers/level, 1 KB threshold
+    python -m paper_1704_00513_b200.report --config 4            # R-MAT 25, u64, 64 buffers/level
+    python -m paper_1704_00513_b200.report --config 5            # message-size sweep + 4096-buffer batch
+    (--scale / --roots shrink configs 3 and 4 for a quick look)
+
+Every call goes through the C ABI (binding.py); each timed call is preceded by an L2 flush (a 256 MB
+memset outside the timed region) and timed with CUDA events; every decoded batch is compared with its
+input. Prints markdown rows: raw MB, ratio, bits/ID, encode GB/s (raw input bytes / time), decode GB/s
+(raw output bytes / time) and both as fractions of the measured HBM copy peak counted on algorithmic
+bytes (raw + compressed).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1704_00513_b200 import binding as B  # noqa: E402
+from paper_1704_00513_b200.workloads import rmat, streams  # noqa: E402
+
+
+def peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"])
+    except Exception:
+        return 6650.0
+
+
+class Runner:
+    def __init__(self, dev, reps=5):
+        self.dev, self.reps = dev, reps
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        self.peak = peak_gbs()
+
+    def _time(self, fn):
+        best = None
+        for _ in range(self.reps + 1):                       # first repetition = warm-up
+            self.flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        return best
+
+    def batch(self, ids, off, W, thr, single=False):
+        """ids: device tensor (bit pattern), off: device int64 offsets. Returns dict of results."""
+        dev = self.dev
+        n, n_buf = ids.numel(), off.numel() - 1
+        counts = (off[1:] - off[:-1]).tolist()
+        cap = B.batch_compress_bound(counts, W)
+        out = torch.empty(cap, dtype=torch.uint8, device=dev)
+        out_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+        ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+        status = torch.zeros(1, dtype=torch.int32, device=dev)
+        back = torch.empty(max(n, 4), dtype=ids.dtype, device=dev)
+        id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+        pad = torch.empty(n + 4, dtype=ids.dtype, device=dev)
+        pad[:n] = ids
+        if single:                                           # one buffer: the single-buffer entry points
+            nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
+            n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+            enc = self._time(lambda: B.compress(pad, n, W, thr, out, nbytes, ws, status))
+            dec = self._time(lambda: B.decompress(out, cap, W, back, n_out, ws, status))
+            assert int(status.item()) == 0 and int(n_out.item()) == n
+            assert torch.equal(back[:n], ids), "decode != input"
+            comp = int(nbytes.item())
+            return {"n": n, "n_buf": 1, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec}
+        enc = self._time(lambda: B.compress_batch(pad, off, n_buf, W, thr, out, out_off, ws, status))
+        dec = self._time(lambda: B.decompress_batch(out, out_off, n_buf, W, back, id_off, ws, status))
+        assert int(status.item()) == 0
+        assert torch.equal(back[:n], ids) and torch.equal(id_off, off), "decode != input"
+        comp = int(out_off[-1].item())
+        return {"n": n, "n_buf": n_buf, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec}
+
+    def row(self, label, r):
+        raw, comp = r["raw"], r["comp"]
+        alg = raw + comp
+        e, d = r["enc_ms"] * 1e-3, r["dec_ms"] * 1e-3
+        ratio = raw / comp if comp else 0.0
+        bits = 8.0 * comp / r["n"] if r["n"] else 0.0
+        return (f"| {label} | {r['n_buf']} | {raw / 1e6:.3f} | {ratio:.2f} | {bits:.2f} | {r['enc_ms'] * 1e3:.1f} | "
+                f"{raw / e / 1e9:.1f} | {100 * alg / e / 1e9 / self.peak:.1f} | {r['dec_ms'] * 1e3:.1f} | "
+                f"{raw / d / 1e9:.1f} | {100 * alg / d / 1e9 / self.peak:.1f} |")
+
+
+HDR = ("| case | buffers | raw MB | ratio | bits/ID | enc us | enc GB/s in | enc % peak | dec us | dec GB/s out | dec % peak |\n"
+       "|---|---|---|---|---|---|---|---|---|---|---|")
+
+
+def rmat_config(R, scale, seed, W, parts, n_roots, thr, per_level_roots=1):
+    dev = R.dev
+    G = rmat.Graph(scale, 16, seed=seed, device=dev)
+    print(f"R-MAT scale {scale}, edgefactor 16, seed {seed}: {G.col.numel()} directed edges after dedupe; "
+          f"{parts} buffers per level by contiguous vertex range, {'u32' if W == 32 else 'u64'} IDs, threshold {thr} B\n")
+    print(HDR)
+    for ri, root in enumerate(G.roots(n_roots, seed=seed)):
+        tot = {"n": 0, "n_buf": parts, "raw": 0, "comp": 0, "enc_ms": 0.0, "dec_ms": 0.0}
+        for level, f in enumerate(G.bfs_frontiers(root)):
+            vals, off = streams.split_block(f, parts, 1 << scale)
+            ids = streams.as_ids(vals, W).to(dev)
+            r = R.batch(ids, off.to(dev), W, thr)
+            for k in ("n", "raw", "comp", "enc_ms", "dec_ms"):
+                tot[k] += r[k]
+            if ri < per_level_roots:
+                print(R.row(f"root {root} level {level} ({r['n']} IDs)", r))
+        print(R.row(f"**root {root}, all levels** ({tot['n']} IDs)", tot))
+
+
+def sweep(R):
+    dev = R.dev
+    print("Single sorted buffers (threshold 0); n/a = the stream would exceed the u32 ID space\n")
+    print(HDR)
+    for W in (32, 64):
+        for k in range(5, 16):
+            nbytes = 4 ** k
+            n = nbytes // (W // 8)
+            for mean in (1.0, 16.0, 4096.0):
+                label = f"u{W} {nbytes >> 10} KB mean {int(mean)}"
+                if W == 32 and n * mean >= 2 ** 32:
+                    print(f"| {label} | 1 | {nbytes / 1e6:.3f} | n/a | | | | | | | |")
+                    continue
+                ids = streams.gap_stream(n, mean, seed=5, W=W, device=dev)
+                off = torch.tensor([0, n], dtype=torch.int64, device=dev)
+                print(R.row(label, R.batch(ids, off, W, 0, single=True)))
+                del ids
+    counts = streams.log_uniform_counts(4096, 8, 16, 32, seed=5)
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=32, device=dev)
+    for thr in (0, 1024):
+        print(R.row(f"batch of 4096 buffers 256 B-64 KB, mean 16, threshold {thr}", R.batch(ids.to(dev), off.to(dev), 32, thr)))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, required=True, choices=[3, 4, 5])
+    ap.add_argument("--scale", type=int, default=0)
+    ap.add_argument("--roots", type=int, default=0)
+    ap.add_argument("--reps", type=int, default=5)
+    a = ap.parse_args()
+    assert torch.cuda.is_available(), "needs a CUDA device (there is no CPU fallback)"
+    dev = torch.device("cuda:0")
+    B.lib()
+    R = Runner(dev, a.reps)
+    if a.config == 3:
+        rmat_config(R, a.scale or 22, 3, 32, 16, a.roots or 16, 1024)
+    elif a.config == 4:
+        rmat_config(R, a.scale or 25, 4, 64, 64, a.roots or 8, 1024)
+    else:
+        sweep(R)
+
+
+if __name__ == "__main__":
+    main()
