@@ -112,6 +112,38 @@ __device__ __forceinline__ uint32_t find_buf(const unsigned long long* __restric
     return lo;
 }
 
+// Same result as find_buf, starting from a hint lo with a[lo] <= g (the buffer of an earlier block): gallop,
+// then bisect. Consecutive blocks live in nearby buffers, so this touches one or two cache lines.
+__device__ __forceinline__ uint32_t find_buf_from(const unsigned long long* __restrict__ a, uint32_t n_buf,
+                                                  unsigned long long g, uint32_t lo) {
+    uint32_t hi, step = 1;
+    while (true) {
+        hi = lo + step;
+        if (hi >= n_buf) { hi = n_buf; break; }
+        if (a[hi] > g) break;
+        lo = hi; step <<= 1;
+    }
+    while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (a[mid] <= g) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// Plan kernels: buffer of the first block of every group of kTileBlocks blocks -> second word of the
+// group's workspace entry (the hint of find_buf_from). blk_first must be complete and visible.
+__device__ __forceinline__ void plan_group_hints(const unsigned long long* __restrict__ blk_first, uint32_t n_buf,
+                                                 unsigned long long total_blocks, unsigned long long* __restrict__ tile_state,
+                                                 size_t tile_cap) {
+    unsigned long long ng = (total_blocks + kTileBlocks - 1) / kTileBlocks;
+    if (ng > tile_cap) ng = tile_cap;
+    for (unsigned long long t = threadIdx.x; t < ng; t += blockDim.x)
+        tile_state[t * kStateStride + 1] = find_buf(blk_first, n_buf, t * kTileBlocks);
+}
+__device__ __forceinline__ uint32_t group_hint(const unsigned long long* __restrict__ tile_state, unsigned long long g) {
+    return (uint32_t)tile_state[(g / kTileBlocks) * kStateStride + 1];
+}
+
 // 1024-thread exclusive scan of two u64 values with running carry (plan kernels).
 struct Scan2 {
     unsigned long long a, b;

@@ -37,46 +37,60 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
     Scan2 carry{0, 0};
-    for (uint32_t i0 = 0; i0 < a.n_buf; i0 += blockDim.x) {
-        const uint32_t i = i0 + threadIdx.x;
-        Scan2 v{0, 0};
-        if (i < a.n_buf) {
-            const unsigned long long beg = s_begin(a, i);
-            unsigned long long avail = 0;
-            bool ok = true;
-            if (a.in_off && a.in_off[i + 1] < beg) ok = false; else avail = s_avail(a, i);
-            if ((beg & 15) || avail < 32) ok = false;
-            if (ok) {
-                const uint4 h0 = *reinterpret_cast<const uint4*>(a.in + beg);
-                const uint4 h1 = *reinterpret_cast<const uint4*>(a.in + beg + 16);
-                const uint32_t mode = (h0.y >> 16) & 0xffu;
-                const unsigned long long n = (unsigned long long)h0.w << 32 | h0.z;
-                const unsigned long long total = (unsigned long long)h1.y << 32 | h1.x;
-                const unsigned long long nb = h1.z;
-                if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W ||
-                    mode > 1u || (h0.y >> 24) != 0u)
-                    ok = false;
-                else if (total > avail || (total & 15) || total < 32) ok = false;
-                else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
-                else if (nb != (n + kBlk - 1) / kBlk || n > (1ull << 40) ||
-                         32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
-                    ok = false;
-                if (ok) { v.a = nb; v.b = n; }
+    constexpr int kIpt = 4;                              // streams per thread and round: 4096 streams per block scan
+    for (uint32_t i0 = 0; i0 < a.n_buf; i0 += blockDim.x * kIpt) {
+        Scan2 v[kIpt], sum{0, 0};
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            v[u] = Scan2{0, 0};
+            if (i < a.n_buf) {
+                const unsigned long long beg = s_begin(a, i);
+                unsigned long long avail = 0;
+                bool ok = true;
+                if (a.in_off && a.in_off[i + 1] < beg) ok = false; else avail = s_avail(a, i);
+                if ((beg & 15) || avail < 32) ok = false;
+                if (ok) {
+                    const uint4 h0 = *reinterpret_cast<const uint4*>(a.in + beg);
+                    const uint4 h1 = *reinterpret_cast<const uint4*>(a.in + beg + 16);
+                    const uint32_t mode = (h0.y >> 16) & 0xffu;
+                    const unsigned long long n = (unsigned long long)h0.w << 32 | h0.z;
+                    const unsigned long long total = (unsigned long long)h1.y << 32 | h1.x;
+                    const unsigned long long nb = h1.z;
+                    if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W ||
+                        mode > 1u || (h0.y >> 24) != 0u)
+                        ok = false;
+                    else if (total > avail || (total & 15) || total < 32) ok = false;
+                    else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
+                    else if (nb != (n + kBlk - 1) / kBlk || n > (1ull << 40) ||
+                             32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
+                        ok = false;
+                    if (ok) { v[u].a = nb; v[u].b = n; }
+                }
+                if (!ok) bad = 1;
             }
-            if (!ok) bad = 1;
+            sum.a += v[u].a; sum.b += v[u].b;
         }
         Scan2 tot;
-        Scan2 ex = block_scan_excl2(v, &tot, sm);
-        if (i < a.n_buf) {
-            a.ws.blk_first[i] = carry.a + ex.a;
-            a.ws.fixed_prefix[i] = carry.b + ex.b;
+        Scan2 ex = block_scan_excl2(sum, &tot, sm);
+        ex.a += carry.a; ex.b += carry.b;
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            if (i < a.n_buf) {
+                a.ws.blk_first[i] = ex.a;
+                a.ws.fixed_prefix[i] = ex.b;
+            }
+            ex.a += v[u].a; ex.b += v[u].b;
         }
         carry.a += tot.a; carry.b += tot.b;
     }
     __syncthreads();
     const bool good = !bad && carry.a <= a.ws.blk_cap && carry.b <= a.ids_cap;
+    if (threadIdx.x == 0) a.ws.blk_first[a.n_buf] = carry.a;
+    __syncthreads();
+    if (good) plan_group_hints(a.ws.blk_first, a.n_buf, carry.a, a.ws.tile_state, a.ws.tile_cap);
     if (threadIdx.x == 0) {
-        a.ws.blk_first[a.n_buf] = carry.a;
         a.ws.fixed_prefix[a.n_buf] = carry.b;
         a.ws.hdr->total_blocks = carry.a;
         a.ws.hdr->total_out = carry.b;
@@ -184,7 +198,7 @@ __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(De
         const unsigned char* s = a.in;
         unsigned long long k = g, id0 = 0, n = n1, total16 = total16_1, lo16 = lo16_1;
         if (batch) {
-            const uint32_t i = find_buf(a.ws.blk_first, a.n_buf, g);
+            const uint32_t i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
             k = g - a.ws.blk_first[i];
             id0 = a.ws.fixed_prefix[i]; n = a.ws.fixed_prefix[i + 1] - id0;
             s = a.in + s_begin(a, i);

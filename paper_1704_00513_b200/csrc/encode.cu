@@ -65,23 +65,35 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
     Scan2 carry{0, 0};
-    for (uint32_t i0 = 0; i0 < a.n_buf; i0 += blockDim.x) {
-        const uint32_t i = i0 + threadIdx.x;
-        Scan2 v{0, 0};
-        if (i < a.n_buf) {
-            if (a.in_off && a.in_off[i + 1] < a.in_off[i]) bad = 1;
-            const unsigned long long n = buf_count(a, i);
-            const bool raw = n * E < a.thr;                               // FORMAT.md §1 (L1311)
-            const unsigned long long nb = raw ? 0ull : (n + kBlk - 1) / kBlk;
-            v.a = nb;
-            v.b = raw ? 32ull + ((n * E + 15ull) & ~15ull) : 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull);
+    constexpr int kIpt = 4;                              // buffers per thread and round: 4096 buffers per block scan
+    for (uint32_t i0 = 0; i0 < a.n_buf; i0 += blockDim.x * kIpt) {
+        Scan2 v[kIpt], sum{0, 0};
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            v[u] = Scan2{0, 0};
+            if (i < a.n_buf) {
+                if (a.in_off[i + 1] < a.in_off[i]) bad = 1;
+                const unsigned long long n = buf_count(a, i);
+                const bool raw = n * E < a.thr;                           // FORMAT.md §1 (L1311)
+                const unsigned long long nb = raw ? 0ull : (n + kBlk - 1) / kBlk;
+                v[u].a = nb;
+                v[u].b = raw ? 32ull + ((n * E + 15ull) & ~15ull) : 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull);
+            }
+            sum.a += v[u].a; sum.b += v[u].b;
         }
         Scan2 tot;
-        Scan2 ex = block_scan_excl2(v, &tot, sm);
-        if (i < a.n_buf) {
-            a.ws.blk_first[i] = carry.a + ex.a;
-            a.ws.fixed_prefix[i] = carry.b + ex.b;
-            a.ws.stream_start[i] = 0;
+        Scan2 ex = block_scan_excl2(sum, &tot, sm);
+        ex.a += carry.a; ex.b += carry.b;
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            if (i < a.n_buf) {
+                a.ws.blk_first[i] = ex.a;
+                a.ws.fixed_prefix[i] = ex.b;
+                a.ws.stream_start[i] = 0;
+            }
+            ex.a += v[u].a; ex.b += v[u].b;
         }
         carry.a += tot.a; carry.b += tot.b;
     }
@@ -91,8 +103,10 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         if (nt > a.ws.tile_cap) nt = a.ws.tile_cap;
         for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q * kStateStride] = 0;
     }
+    if (threadIdx.x == 0) a.ws.blk_first[a.n_buf] = carry.a;
+    __syncthreads();
+    plan_group_hints(a.ws.blk_first, a.n_buf, carry.a, a.ws.tile_state, a.ws.tile_cap);
     if (threadIdx.x == 0) {
-        a.ws.blk_first[a.n_buf] = carry.a;
         a.ws.fixed_prefix[a.n_buf] = carry.b;
         a.ws.stream_start[a.n_buf] = 0;
         a.ws.hdr->total_blocks = carry.a;
@@ -248,7 +262,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
             if (g < total) {
                 if (batch) {
-                    i = find_buf(a.ws.blk_first, a.n_buf, g);
+                    i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
                     const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
                     m = (int)min((unsigned long long)kBlk, n - kBlk * k);
                     xoff = buf_start(a, i) + kBlk * k;
@@ -500,20 +514,22 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
         const unsigned long long q = a.ws.blk_first[i];
         unsigned long long bb = grand16;
         if (q < total_blocks) {
-            const uint32_t j = find_buf(a.ws.blk_first, a.n_buf, q);   // the buffer that owns block q
+            const uint32_t j = a.in_off ? find_buf_from(a.ws.blk_first, a.n_buf, q, group_hint(a.ws.tile_state, q))
+                                        : 0u;                               // the buffer that owns block q
             bb = (a.ws.stream_start[j] - 1 - a.ws.fixed_prefix[j]) >> 4;
         }
         return a.ws.fixed_prefix[i] + 16ull * bb;
     };
-    for (uint32_t i = blockIdx.x; i < a.n_buf; i += gridDim.x) {
+    const int lane = threadIdx.x & 31, warps = blockDim.x >> 5;
+    for (uint32_t i = blockIdx.x * warps + (threadIdx.x >> 5); i < a.n_buf; i += gridDim.x * warps) {   // warp = buffer
         const unsigned long long f0 = a.ws.blk_first[i], f1 = a.ws.blk_first[i + 1];
-        if (!ok) { if (a.out_off && threadIdx.x == 0) a.out_off[i] = 0; continue; }
+        if (!ok) { if (a.out_off && lane == 0) a.out_off[i] = 0; continue; }
         const unsigned long long s0 = stream_at(i);
         const unsigned long long s1 = (i + 1 < a.n_buf) ? stream_at(i + 1) : a.ws.hdr->total_out;
         const unsigned long long n = buf_count(a, i), total = s1 - s0;
         const bool raw = n * E < a.thr;
         unsigned char* s = a.out + s0;
-        if (threadIdx.x == 0) {
+        if (lane == 0) {
             if (a.out_off) a.out_off[i] = s0;
             const unsigned long long nb = f1 - f0;
             uint4 h0, h1;
@@ -534,7 +550,7 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
             const T* x = reinterpret_cast<const T*>(a.ids) + buf_start(a, i);
             T* y = reinterpret_cast<T*>(s + 32);
             const unsigned long long padded = (total - 32) / E;
-            for (unsigned long long j = threadIdx.x; j < padded; j += blockDim.x) y[j] = j < n ? x[j] : (T)0;
+            for (unsigned long long j = lane; j < padded; j += 32) y[j] = j < n ? x[j] : (T)0;
         }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -577,7 +593,8 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         BFSC_LAUNCH_CHECK();
     }
     if (!single || degenerate) {
-        const uint32_t sgrid = a.n_buf < (uint32_t)(kNumSM * 8) ? a.n_buf : (uint32_t)(kNumSM * 8);
+        uint32_t sgrid = (a.n_buf + 7) / 8;                      // one warp per buffer
+        if (sgrid > (uint32_t)(kNumSM * 8)) sgrid = (uint32_t)(kNumSM * 8);
         if (launch_dep(k_enc_streams<W>, sgrid ? (int)sgrid : 1, 256, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
         BFSC_LAUNCH_CHECK();
     }
