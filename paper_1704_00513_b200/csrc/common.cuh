@@ -131,14 +131,35 @@ __device__ __forceinline__ uint32_t find_buf_from(const unsigned long long* __re
 }
 
 // Plan kernels: buffer of the first block of every group of kTileBlocks blocks -> second word of the
-// group's workspace entry (the hint of find_buf_from). blk_first must be complete and visible.
-__device__ __forceinline__ void plan_group_hints(const unsigned long long* __restrict__ blk_first, uint32_t n_buf,
-                                                 unsigned long long total_blocks, unsigned long long* __restrict__ tile_state,
-                                                 size_t tile_cap) {
-    unsigned long long ng = (total_blocks + kTileBlocks - 1) / kTileBlocks;
-    if (ng > tile_cap) ng = tile_cap;
-    for (unsigned long long t = threadIdx.x; t < ng; t += blockDim.x)
-        tile_state[t * kStateStride + 1] = find_buf(blk_first, n_buf, t * kTileBlocks);
+// group's workspace entry (the hint of find_buf_from). Buffer i with blocks [first, first + nb) owns the
+// groups whose first block it contains: no search. Buffers that own many groups are queued (shared
+// list, kHintQueue entries) and written by the whole CTA in plan_hints_flush.
+constexpr int kHintQueue = 1024;
+struct HintQueue { unsigned int n; unsigned int buf[kHintQueue]; unsigned long long first[kHintQueue], nb[kHintQueue]; };
+
+__device__ __forceinline__ void plan_hints_of(uint32_t i, unsigned long long first, unsigned long long nb,
+                                              unsigned long long* __restrict__ tile_state, size_t tile_cap, HintQueue* q) {
+    if (nb == 0) return;
+    const unsigned long long t0 = (first + kTileBlocks - 1) / kTileBlocks, t1 = (first + nb - 1) / kTileBlocks;   // groups t0..t1
+    if (t1 < t0) return;
+    if (t1 - t0 < 8) {
+        for (unsigned long long t = t0; t <= t1 && t < tile_cap; t++) tile_state[t * kStateStride + 1] = i;
+    } else {
+        const unsigned int slot = atomicAdd(&q->n, 1u);
+        if (slot < (unsigned)kHintQueue) { q->buf[slot] = i; q->first[slot] = first; q->nb[slot] = nb; }
+        else for (unsigned long long t = t0; t <= t1 && t < tile_cap; t++) tile_state[t * kStateStride + 1] = i;
+    }
+}
+__device__ __forceinline__ void plan_hints_flush(unsigned long long* __restrict__ tile_state, size_t tile_cap, HintQueue* q) {
+    __syncthreads();
+    const unsigned int n = q->n < (unsigned)kHintQueue ? q->n : (unsigned)kHintQueue;
+    for (unsigned int e = 0; e < n; e++) {
+        const unsigned long long t0 = (q->first[e] + kTileBlocks - 1) / kTileBlocks, t1 = (q->first[e] + q->nb[e] - 1) / kTileBlocks;
+        for (unsigned long long t = t0 + threadIdx.x; t <= t1 && t < tile_cap; t += blockDim.x) tile_state[t * kStateStride + 1] = q->buf[e];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) q->n = 0;
+    __syncthreads();
 }
 __device__ __forceinline__ uint32_t group_hint(const unsigned long long* __restrict__ tile_state, unsigned long long g) {
     return (uint32_t)tile_state[(g / kTileBlocks) * kStateStride + 1];

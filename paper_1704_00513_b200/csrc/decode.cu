@@ -32,35 +32,52 @@ template <int W>
 __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
     __shared__ Scan2 sm[33];
     __shared__ int bad;
+    __shared__ HintQueue hq;
     constexpr unsigned long long E = W / 8;
     pdl_launch_dependents();
-    if (threadIdx.x == 0) bad = 0;
+    if (threadIdx.x == 0) { bad = 0; hq.n = 0; }
     __syncthreads();
     Scan2 carry{0, 0};
     constexpr int kIpt = 4;                              // streams per thread and round: 4096 streams per block scan
     for (uint32_t i0 = 0; i0 < a.n_buf; i0 += blockDim.x * kIpt) {
         Scan2 v[kIpt], sum{0, 0};
+        unsigned long long beg[kIpt], avail[kIpt];
+        bool rd[kIpt];
+        uint4 h0[kIpt], h1[kIpt];
 #pragma unroll
-        for (int u = 0; u < kIpt; u++) {
+        for (int u = 0; u < kIpt; u++) {                 // phase 1: extents (independent loads)
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            beg[u] = 0; avail[u] = 0; rd[u] = false;
+            if (i < a.n_buf) {
+                beg[u] = s_begin(a, i);
+                const unsigned long long end = a.in_off ? a.in_off[i + 1] : a.in_single;
+                avail[u] = end >= beg[u] ? end - beg[u] : 0;
+                rd[u] = !(beg[u] & 15) && avail[u] >= 32;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {                 // phase 2: all headers in flight at once
+            h0[u] = h1[u] = make_uint4(0, 0, 0, 0);
+            if (rd[u]) {
+                h0[u] = *reinterpret_cast<const uint4*>(a.in + beg[u]);
+                h1[u] = *reinterpret_cast<const uint4*>(a.in + beg[u] + 16);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {                 // phase 3: validation (FORMAT.md §4)
             const uint32_t i = i0 + threadIdx.x * kIpt + u;
             v[u] = Scan2{0, 0};
             if (i < a.n_buf) {
-                const unsigned long long beg = s_begin(a, i);
-                unsigned long long avail = 0;
-                bool ok = true;
-                if (a.in_off && a.in_off[i + 1] < beg) ok = false; else avail = s_avail(a, i);
-                if ((beg & 15) || avail < 32) ok = false;
+                bool ok = rd[u];
                 if (ok) {
-                    const uint4 h0 = *reinterpret_cast<const uint4*>(a.in + beg);
-                    const uint4 h1 = *reinterpret_cast<const uint4*>(a.in + beg + 16);
-                    const uint32_t mode = (h0.y >> 16) & 0xffu;
-                    const unsigned long long n = (unsigned long long)h0.w << 32 | h0.z;
-                    const unsigned long long total = (unsigned long long)h1.y << 32 | h1.x;
-                    const unsigned long long nb = h1.z;
-                    if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W ||
-                        mode > 1u || (h0.y >> 24) != 0u)
+                    const uint32_t mode = (h0[u].y >> 16) & 0xffu;
+                    const unsigned long long n = (unsigned long long)h0[u].w << 32 | h0[u].z;
+                    const unsigned long long total = (unsigned long long)h1[u].y << 32 | h1[u].x;
+                    const unsigned long long nb = h1[u].z;
+                    if (h0[u].x != 0x43534642u || (h0[u].y & 0xffu) != 1u || ((h0[u].y >> 8) & 0xffu) != (uint32_t)W ||
+                        mode > 1u || (h0[u].y >> 24) != 0u)
                         ok = false;
-                    else if (total > avail || (total & 15) || total < 32) ok = false;
+                    else if (total > avail[u] || (total & 15) || total < 32) ok = false;
                     else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
                     else if (nb != (n + kBlk - 1) / kBlk || n > (1ull << 40) ||
                              32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
@@ -80,16 +97,16 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
             if (i < a.n_buf) {
                 a.ws.blk_first[i] = ex.a;
                 a.ws.fixed_prefix[i] = ex.b;
+                plan_hints_of(i, ex.a, v[u].a, a.ws.tile_state, a.ws.tile_cap, &hq);
             }
             ex.a += v[u].a; ex.b += v[u].b;
         }
         carry.a += tot.a; carry.b += tot.b;
+        plan_hints_flush(a.ws.tile_state, a.ws.tile_cap, &hq);
     }
     __syncthreads();
     const bool good = !bad && carry.a <= a.ws.blk_cap && carry.b <= a.ids_cap;
     if (threadIdx.x == 0) a.ws.blk_first[a.n_buf] = carry.a;
-    __syncthreads();
-    if (good) plan_group_hints(a.ws.blk_first, a.n_buf, carry.a, a.ws.tile_state, a.ws.tile_cap);
     if (threadIdx.x == 0) {
         a.ws.fixed_prefix[a.n_buf] = carry.b;
         a.ws.hdr->total_blocks = carry.a;

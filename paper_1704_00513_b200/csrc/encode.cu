@@ -41,6 +41,7 @@ template <int W>
 __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     __shared__ Scan2 sm[33];
     __shared__ int bad;
+    __shared__ HintQueue hq;
     constexpr unsigned long long E = W / 8;
     pdl_launch_dependents();
     if (a.in_off == nullptr) {                           // single buffer: no scan needed
@@ -62,7 +63,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         }
         return;
     }
-    if (threadIdx.x == 0) bad = 0;
+    if (threadIdx.x == 0) { bad = 0; hq.n = 0; }
     __syncthreads();
     Scan2 carry{0, 0};
     constexpr int kIpt = 4;                              // buffers per thread and round: 4096 buffers per block scan
@@ -92,10 +93,12 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
                 a.ws.blk_first[i] = ex.a;
                 a.ws.fixed_prefix[i] = ex.b;
                 a.ws.stream_start[i] = 0;
+                plan_hints_of(i, ex.a, v[u].a, a.ws.tile_state, a.ws.tile_cap, &hq);
             }
             ex.a += v[u].a; ex.b += v[u].b;
         }
         carry.a += tot.a; carry.b += tot.b;
+        plan_hints_flush(a.ws.tile_state, a.ws.tile_cap, &hq);
     }
     __syncthreads();
     {                                                    // look-back states start invalid
@@ -104,8 +107,6 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q * kStateStride] = 0;
     }
     if (threadIdx.x == 0) a.ws.blk_first[a.n_buf] = carry.a;
-    __syncthreads();
-    plan_group_hints(a.ws.blk_first, a.n_buf, carry.a, a.ws.tile_state, a.ws.tile_cap);
     if (threadIdx.x == 0) {
         a.ws.fixed_prefix[a.n_buf] = carry.b;
         a.ws.stream_start[a.n_buf] = 0;
