@@ -205,7 +205,7 @@ constexpr int kImgCap = 320;                                  // bytes of a bloc
 constexpr int kImgSlotChunks = 21;                            // slot stride (16-B chunks): 21 q mod 8 are all distinct
 constexpr int kImgBufChunks = kQuadBlocks * kImgSlotChunks;   // one image buffer of a warp
 
-constexpr int kDefer = 2;                                     // a tile's images leave kDefer tiles after they were packed
+constexpr int kDefer = 1;                                     // a tile's images leave kDefer tiles after they were packed (1 or 2)
 constexpr int kNB = kDefer + 1;                               // image buffers / size and offset tables per CTA
 
 template <int W> struct EncSmem {
@@ -466,8 +466,8 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         // copy out the oldest waiting tile: tile k - kDefer while tiles keep coming, then drain
         const int w = n_wait - (have ? 1 : 0);                           // waiting tiles older than tile k
         if (w > 0 && (w == kDefer || !have)) {
-            static_assert(kDefer == 2, "key_hist selection below");
-            const uint32_t key_e = w == 2 ? key_hist[1] : key_hist[0];   // key of the CTA's tile ke
+            static_assert(kDefer == 1 || kDefer == 2, "key_hist selection below");
+            const uint32_t key_e = (kDefer == 2 && w == 2) ? key_hist[kDefer - 1] : key_hist[0];   // key of the CTA's tile ke
             int kpe = kp - w;                                            // its buffer: ke % kNB
             if (kpe < 0) kpe += kNB;
             bar_sync(kBarOffsets + kpe, kEncThreads);                    // its offsets are resolved
