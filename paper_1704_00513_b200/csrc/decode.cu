@@ -34,6 +34,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
     __shared__ int bad;
     __shared__ HintQueue hq;
     constexpr unsigned long long E = W / 8;
+    pdl_wait();                                          // the call before this one is complete (workspace, inputs)
     pdl_launch_dependents();
     if (threadIdx.x == 0) { bad = 0; hq.n = 0; }
     __syncthreads();
@@ -164,8 +165,9 @@ __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(De
 
     const bool batch = a.in_off != nullptr;
     unsigned long long total_blocks, n1 = 0, total16_1 = 0, lo16_1 = 0;   // single stream: n, total/16, first block/16
+    pdl_wait();                                                            // the kernel before this one is complete
+    pdl_launch_dependents();                                               // the next one may be set up; it waits for this grid
     if (batch) {
-        pdl_wait();
         if (!a.ws.hdr->ok) return;
         total_blocks = a.ws.hdr->total_blocks;
     } else {                                                               // D0 for one stream (FORMAT.md §1, §4)
@@ -326,11 +328,11 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
     if (a.in_off) {
-        k_dec_plan<W><<<1, 1024, 0, s>>>(a);
+        if (launch_dep(k_dec_plan<W>, 1, 1024, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
         BFSC_LAUNCH_CHECK();
         if (launch_dep(k_dec_tiles<W>, max_grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     } else {
-        k_dec_tiles<W><<<grid, kDecThreads, kSmem, s>>>(a);
+        if (launch_dep(k_dec_tiles<W>, grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     }
     BFSC_LAUNCH_CHECK();
     return BFSC_OK;

@@ -33,7 +33,8 @@ __device__ __forceinline__ unsigned long long buf_count(const EncArgs& a, uint32
 
 constexpr int kEncWorkers = 8;                           // worker warps per CTA
 constexpr int kTileR = kEncWorkers * kQuadBlocks;        // 64 blocks per tile
-static_assert(kTileR == kTileBlocks, "workspace sizing assumes 64-block tiles");
+static_assert(kTileR >= kTileBlocks, "workspace sizing assumes tiles of at least kTileBlocks blocks");
+constexpr int kPer = (kTileR + 31) / 32;                 // blocks per lane of the scan warp
 constexpr int kEncThreads = (kEncWorkers + 1) * 32;      // + the scan warp
 
 // ---- E0: plan. One CTA; per buffer: mode, block count, fixed bytes; exclusive prefixes. ----
@@ -43,6 +44,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     __shared__ int bad;
     __shared__ HintQueue hq;
     constexpr unsigned long long E = W / 8;
+    pdl_wait();                                          // the call before this one is complete (workspace, inputs)
     pdl_launch_dependents();
     if (a.in_off == nullptr) {                           // single buffer: no scan needed
         const unsigned long long n = a.n_single;
@@ -156,6 +158,30 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
 __device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned long long v) {
     asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
+// mbarrier (shared memory, CTA scope): one-directional "posted" signals between warps of a CTA
+__device__ __forceinline__ void mbar_init(unsigned long long* b, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {   // until the phase of that parity has completed
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(b);
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
+// Bulk (TMA) store shared -> global, issued by one lane: 16-byte aligned addresses, size a multiple of 16.
+__device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
+                 "r"((uint32_t)__cvta_generic_to_shared(ssrc)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }   // sources may be overwritten
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
@@ -214,7 +240,8 @@ template <int W> struct EncSmem {
     static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
 };
 
-enum { kBarSizes = 1, kBarOffsets = kBarSizes + kNB, kBarWorkers = kBarOffsets + kNB };   // named barriers (+ tile count mod kNB)
+enum { kBarSizes = 1 };                                       // named barriers kBarSizes + tile count mod kNB
+constexpr int kRing = 8;                                      // ring of tile bookkeeping slots (workers may be two tiles apart)
 
 // k_enc_tiles: CTA = 8 worker warps + 1 scan warp; a CTA's k-th tile is "tile k" below.
 //   workers, iteration k:  E1/E2 of tile k -> sizes in s_key[k % kNB], the last warp publishes the tile's
@@ -234,16 +261,22 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     __shared__ uint32_t s_key[kNB][kTileR];              // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
     __shared__ unsigned long long s_at[kNB][kTileR];     // scan warp: final byte offset of the block, or kSkip
     __shared__ uint32_t s_off16[kTileR];                 // exclusive scan of the sizes inside the tile (16-B units)
-    __shared__ int s_m[4][kTileR];                       // ring of tile bookkeeping: valid IDs of each block (0 = none)
-    __shared__ unsigned long long s_xoff[4][kTileR];     // element offset of the block's first ID
-    __shared__ uint32_t s_buf[4][kTileR];                // buffer of each block (batch calls)
-    __shared__ unsigned long long s_tile[4];             // tile of each ring slot, kNoTile = done
+    __shared__ int s_m[kRing][kTileR];                       // ring of tile bookkeeping: valid IDs of each block (0 = none)
+    __shared__ unsigned long long s_xoff[kRing][kTileR];     // element offset of the block's first ID
+    __shared__ uint32_t s_buf[kRing][kTileR];                // buffer of each block (batch calls)
+    __shared__ unsigned long long s_tile[kRing];             // tile of each ring slot, kNoTile = done
+    __shared__ unsigned long long mb_post[kRing];        // warp 0 -> workers: the ring slot's tile is posted (use u of a slot: parity u & 1)
+    __shared__ unsigned long long mb_off[kNB];           // scan warp -> workers: the offsets in s_at[kp] are posted
     __shared__ unsigned int s_agg[2];                    // arrivals << 24 | sum of the worker warps' sizes (16-B units)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool batch = a.in_off != nullptr;
     const T* ids = reinterpret_cast<const T*>(a.ids);
+    pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
     if (threadIdx.x < 2) s_agg[threadIdx.x] = 0;
+    if (threadIdx.x < kRing) mbar_init(&mb_post[threadIdx.x], 1);
+    if (threadIdx.x >= 32 && threadIdx.x < 32 + kNB) mbar_init(&mb_off[threadIdx.x - 32], 1);
+    __syncthreads();
 
     // Single-buffer calls know their geometry from the arguments: the first tiles start without waiting
     // for the plan kernel; only the ticket counter and the look-back states need it.
@@ -283,23 +316,32 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         if (!batch) pdl_wait();                          // the plan kernel's writes are visible from here on
         int kp = 0;                                      // k % kNB
         for (int k = 0;; k++) {
-            const unsigned long long t = s_tile[k & 3];  // posted before the sizes of tile k-1 arrived
+            const unsigned long long t = s_tile[k & (kRing - 1)];  // posted before the sizes of tile k-1 arrived
             if (t == kNoTile) break;
             TR(t, 0);
             bar_sync(kBarSizes + kp, kEncThreads);       // the workers' sizes of tile t are in s_key[kp]
 
-            // E3: intra-tile scan (2 consecutive blocks per lane)
-            const uint32_t k0 = s_key[kp][2 * lane], k1 = s_key[kp][2 * lane + 1];
-            const uint32_t z0 = k0 >> 18, z1 = k1 >> 18;
-            uint32_t inc = z0 + z1;
+            // E3: intra-tile scan (kPer consecutive blocks per lane)
+            uint32_t kk[kPer], offs[kPer], inc = 0;
+#pragma unroll
+            for (int h = 0; h < kPer; h++) {
+                const int jj = kPer * lane + h;
+                kk[h] = jj < kTileR ? s_key[kp][jj] : 0u;
+                offs[h] = inc;
+                inc += kk[h] >> 18;
+            }
+            const uint32_t own = inc;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const uint32_t y = __shfl_up_sync(kFull, inc, o);
                 if (lane >= o) inc += y;
             }
-            const uint32_t off0 = inc - z0 - z1, off1 = off0 + z0;
             const unsigned long long agg = __shfl_sync(kFull, inc, 31);
-            s_off16[2 * lane] = off0; s_off16[2 * lane + 1] = off1;
+#pragma unroll
+            for (int h = 0; h < kPer; h++) {
+                offs[h] += inc - own;
+                if (kPer * lane + h < kTileR) s_off16[kPer * lane + h] = offs[h];
+            }
             TR(t, 2);                                    // (the aggregate was published by the last worker warp)
             const unsigned long long excl = t > 0 ? lookback(a.ws.tile_state, t, lane) : 0ull;
             TR(t, 3);
@@ -315,17 +357,18 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             // final offsets, directory entries, stream starts
             const unsigned long long g0 = t * kTileR;
 #pragma unroll
-            for (int h = 0; h < 2; h++) {
-                const int jj = 2 * lane + h;
+            for (int h = 0; h < kPer; h++) {
+                const int jj = kPer * lane + h;
+                if (jj >= kTileR) continue;
                 const unsigned long long g = g0 + jj;
-                const uint32_t key = h ? k1 : k0;
+                const uint32_t key = kk[h];
                 unsigned long long at = kSkip;
                 if (g < total) {
-                    const uint32_t off = h ? off1 : off0, bytes = key >> 14;
+                    const uint32_t off = offs[h], bytes = key >> 14;
                     unsigned long long first = 0, f0 = 0, f1 = f1_single, S = 0;
                     uint32_t i = 0;
                     if (batch) {
-                        i = s_buf[k & 3][jj];
+                        i = s_buf[k & (kRing - 1)][jj];
                         first = a.ws.blk_first[i]; f0 = a.ws.fixed_prefix[i]; f1 = a.ws.fixed_prefix[i + 1];
                         if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
                         else if (i > 0) {                // published by the tile that owns the stream's first block
@@ -362,7 +405,8 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 s_at[kp][jj] = at;
             }
             TR(t, 4);
-            bar_arrive(kBarOffsets + kp, kEncThreads);   // offsets of tile k are posted
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&mb_off[kp]);     // offsets of tile k are posted
             TRV(t, 15, (unsigned long long)smid() | ((unsigned long long)blockIdx.x << 32));
             kp = kp == kNB - 1 ? 0 : kp + 1;
         }
@@ -373,47 +417,53 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     const int q = lane >> 2, l = lane & 3;
     uint4* area = dyn_smem + warp * EncSmem<W>::kWarpChunks;
     uint4* slot = area + raw_slot_chunk<W>(q);                           // staging: the quad's raw IDs
-    unsigned char* img0 = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks + kImgSlotChunks * q);
+    unsigned char* ibuf = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks);   // the warp's kNB image buffers
     const int j = warp * kQuadBlocks + q;
     constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
     if (warp == 0) {                                                     // the CTA's first two tiles are static
         const unsigned long long t0 = blockIdx.x, t1 = (unsigned long long)blockIdx.x + gridDim.x;
         prep(t0 < n_tiles ? t0 : kNoTile, 0);
         prep(t0 < n_tiles && t1 < n_tiles ? t1 : kNoTile, 1);
+        __syncwarp();
+        if (lane == 0) { mbar_arrive(&mb_post[0]); mbar_arrive(&mb_post[1]); }
     }
     __syncthreads();                                                     // barrier 0
     bool have = s_tile[0] != kNoTile;
     if (have) quad_prefetch<W>(slot, ids + s_xoff[0][j], s_m[0][j]);
-    uint32_t key_hist[kDefer] = {};                                      // keys of the tiles whose images wait in shared memory
+    static_assert(kDefer == 1, "one tile of images waits in shared memory");
+    uint32_t key_hist = 0, woff_hist = 0;                                // key and image place of the tile that waits in shared memory
     unsigned int ticket = 0xffffffffu;                                   // warp 0: requested one iteration before it is used
     int kp = 0;                                                          // k % kNB
     int n_wait = 0, ke = 0;                                              // tiles packed but not copied out yet; next one to copy out
     for (int k = 0;; k++) {
-        uint32_t key = 0;
+        uint32_t key = 0, woff = 0;
         bool have_next = false;
         if (have) {
             if (warp == 0 && k >= 1) {                                   // tile k+1: ticket -> bookkeeping (ring slot (k+1) & 3)
                 unsigned long long t = kNoTile;
-                if (s_tile[k & 3] != kNoTile) {
+                if (s_tile[k & (kRing - 1)] != kNoTile) {
                     ticket = __shfl_sync(kFull, ticket, 0);
                     if (ticket < n_tiles) t = ticket;
                 }
-                prep(t, (k + 1) & 3);
+                prep(t, (k + 1) & (kRing - 1));
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&mb_post[(k + 1) & (kRing - 1)]);
             }
-            const int m = s_m[k & 3][j];
+            const int m = s_m[k & (kRing - 1)][j];
             const T* raw = reinterpret_cast<const T*>(slot) +
-                           (reinterpret_cast<uintptr_t>(ids + s_xoff[k & 3][j]) & 15) / sizeof(T);
-            unsigned char* img = img0 + kp * (kImgBufChunks * 16);
-            if (warp == 0) TR(s_tile[k & 3], 6);
+                           (reinterpret_cast<uintptr_t>(ids + s_xoff[k & (kRing - 1)][j]) & 15) / sizeof(T);
+            unsigned char* ib = ibuf + kp * (kImgBufChunks * 16);        // this tile's image buffer
+            if (warp == 0) TR(s_tile[k & (kRing - 1)], 6);
             cp_async_wait_all();
+            if (lane == 0) bulk_wait_read();                             // the bulk store that read this image buffer is done with it
             __syncwarp();
-            if (warp == 0) TR(s_tile[k & 3], 7);
+            if (warp == 0) TR(s_tile[k & (kRing - 1)], 7);
             uint32_t d[32];
             bool wide_lane = false, wide = false;
             const T base = col_deltas<W>(raw, m, d, wide_lane);          // E1
             if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
             if (!wide) key = quad_choose_b<W>(d);                        // E2
-            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(img));
+            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (kImgSlotChunks * 16)));
             if (m <= 0) key = 0;
             if (l == 0) s_key[kp][j] = key;
             {   // The tile's aggregate goes out as soon as the LAST worker warp has its sizes — not when the scan
@@ -425,18 +475,18 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                     const unsigned int old = atomicAdd(&s_agg[k & 1], (1u << 24) | z);
                     if ((old >> 24) == kEncWorkers - 1) {
                         s_agg[k & 1] = 0;
-                        const unsigned long long t = s_tile[k & 3];
+                        const unsigned long long t = s_tile[k & (kRing - 1)];
                         pdl_wait();                                      // the states are zeroed by the plan kernel
                         if (t > 0)
                             st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagAgg | (unsigned long long)((old & 0xffffffu) + z));
                     }
                 }
             }
-            if (warp == 0) TR(s_tile[k & 3], 8);
+            if (warp == 0) TR(s_tile[k & (kRing - 1)], 8);
             bar_arrive(kBarSizes + kp, kEncThreads);
             if (warp == 0) {                                             // ticket of tile k+2 (used next iteration)
                 ticket = 0xffffffffu;
-                if (lane == 0 && s_tile[(k + 1) & 3] != kNoTile) {
+                if (lane == 0 && s_tile[(k + 1) & (kRing - 1)] != kNoTile) {
                     pdl_wait();
                     ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
                 }
@@ -445,11 +495,23 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
             const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)kImgCap);   // slow path, in global memory later
             const bool fast = !wide && key != 0 && !late;
+            // The warp's 8 images lie back to back in the buffer, as they do in the output (consecutive blocks):
+            // woff = exclusive scan of the fast blocks' sizes over the quads, in 16-byte chunks.
+            {
+                const uint32_t zf = fast ? key >> 18 : 0u;
+                uint32_t inc = zf, y;
+                y = __shfl_up_sync(kFull, inc, 4); if (lane >= 4) inc += y;
+                y = __shfl_up_sync(kFull, inc, 8); if (lane >= 8) inc += y;
+                y = __shfl_up_sync(kFull, inc, 16); if (lane >= 16) inc += y;
+                woff = inc - zf;
+            }
+            unsigned char* img = ib + 16 * woff;
             if (!wide && __any_sync(kFull, fast && n_exc > 0))           // E4 into the image buffer: exceptions
                 col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
-            bar_sync(kBarWorkers, kEncWorkers * 32);                     // all staged IDs consumed; tile k+1 is posted
-            have_next = s_tile[(k + 1) & 3] != kNoTile;
-            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & 3][j], s_m[(k + 1) & 3][j]);   // same slots
+            __syncwarp();                                                // the warp's staged IDs are consumed
+            mbar_wait(&mb_post[(k + 1) & (kRing - 1)], ((k + 1) / kRing) & 1);   // tile k+1 is posted
+            have_next = s_tile[(k + 1) & (kRing - 1)] != kNoTile;
+            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & (kRing - 1)][j], s_m[(k + 1) & (kRing - 1)][j]);   // same slots
             if (fast) {                                                  // payload + header
                 if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
                 if (l == 0) {                                            // block header (FORMAT.md §2)
@@ -459,43 +521,56 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             }
             if (late) key |= kLateBit;
             __syncwarp();                                                // image complete
-            if (warp == 0) TR(s_tile[k & 3], 9);
+            if (warp == 0) TR(s_tile[k & (kRing - 1)], 9);
             n_wait++;
         }
 
         // copy out the oldest waiting tile: tile k - kDefer while tiles keep coming, then drain
         const int w = n_wait - (have ? 1 : 0);                           // waiting tiles older than tile k
         if (w > 0 && (w == kDefer || !have)) {
-            static_assert(kDefer == 1 || kDefer == 2, "key_hist selection below");
-            const uint32_t key_e = (kDefer == 2 && w == 2) ? key_hist[kDefer - 1] : key_hist[0];   // key of the CTA's tile ke
+            const uint32_t key_e = key_hist, woff_e = woff_hist;         // key and image place of the CTA's tile ke
             int kpe = kp - w;                                            // its buffer: ke % kNB
             if (kpe < 0) kpe += kNB;
-            bar_sync(kBarOffsets + kpe, kEncThreads);                    // its offsets are resolved
+            if (warp == 0) TR(s_tile[ke & (kRing - 1)], 10);
+            mbar_wait(&mb_off[kpe], (ke / kNB) & 1);                     // its offsets are resolved
+            if (warp == 0) TR(s_tile[ke & (kRing - 1)], 11);
             unsigned long long at = kSkip;
             if (key_e != 0) at = s_at[kpe][j];
             if (__any_sync(kFull, (key_e & kLateBit) != 0)) {
                 const bool mine = (key_e & kLateBit) != 0 && at != kSkip;
-                late_emit<W>(ids + s_xoff[ke & 3][j], s_m[ke & 3][j], key_e & ~kLateBit, mine ? a.out + at : nullptr);
+                late_emit<W>(ids + s_xoff[ke & (kRing - 1)][j], s_m[ke & (kRing - 1)][j], key_e & ~kLateBit, mine ? a.out + at : nullptr);
             }
-            if ((key_e & kLateBit) == 0 && at != kSkip) {                // image -> its final place
-                const uint4* src = reinterpret_cast<const uint4*>(img0 + kpe * (kImgBufChunks * 16));
+            // images -> their final place. Usual case: the warp's blocks are consecutive in the output as well
+            // (same stream, none late, all fit): ONE bulk store of the whole buffer by lane 0.
+            const unsigned char* ib_e = ibuf + kpe * (kImgBufChunks * 16);
+            const bool valid = key_e != 0, fast_e = valid && (key_e & kLateBit) == 0;
+            const uint32_t z_e = fast_e ? key_e >> 18 : 0u;
+            const unsigned long long at_n = __shfl_down_sync(kFull, at, 4);
+            const bool valid_n = __shfl_down_sync(kFull, (int)valid, 4) != 0 && q < kQuadBlocks - 1;
+            const bool contig = !valid || (fast_e && at != kSkip && (!valid_n || at_n == at + 16ull * z_e));
+            if (__all_sync(kFull, contig)) {
+                const uint32_t tot = __shfl_sync(kFull, woff_e + z_e, 31);
+                fence_proxy_async_smem();                                // the image was written through the generic proxy
+                __syncwarp();
+                if (lane == 0 && tot > 0) bulk_store(a.out + at, ib_e, 16u * tot);
+            } else if (fast_e && at != kSkip) {
+                const uint4* src = reinterpret_cast<const uint4*>(ib_e) + woff_e;
                 uint4* dst = reinterpret_cast<uint4*>(a.out + at);
-                const uint32_t n16 = key_e >> 18;
-                for (uint32_t c = l; c < n16; c += 4) __stcs(dst + c, src[c]);
+                for (uint32_t c = l; c < z_e; c += 4) __stcs(dst + c, src[c]);
             }
             __syncwarp();
+            if (warp == 0) TR(s_tile[ke & (kRing - 1)], 12);
             n_wait--;
             ke++;
         }
         if (!have && n_wait == 0) break;
         if (have) {
-#pragma unroll
-            for (int x = kDefer - 1; x > 0; x--) key_hist[x] = key_hist[x - 1];
-            key_hist[0] = key;
+            key_hist = key; woff_hist = woff;
             kp = kp == kNB - 1 ? 0 : kp + 1;
         }
         have = have_next;
     }
+    if (lane == 0) bulk_wait_all();                                      // the bulk stores have left shared memory and landed
 }
 
 // ---- stream headers, directory tails, E5 raw passthrough, out_offsets (batch / degenerate calls) ----
@@ -504,6 +579,7 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
     pdl_wait();
+    pdl_launch_dependents();
     const unsigned long long total_blocks = a.ws.hdr->total_blocks, grand16 = a.ws.hdr->grand16;
     bool ok = a.ws.hdr->ok != 0;
     if (ok && a.ws.hdr->total_out > a.out_cap) {
@@ -587,7 +663,7 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     }
     EncArgs a = a_in;
     a.grid = (uint32_t)grid;
-    k_enc_plan<W><<<1, 1024, 0, s>>>(a);
+    if (launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     BFSC_LAUNCH_CHECK();
     if (!degenerate) {
         if (launch_dep(k_enc_tiles<W>, grid, kEncThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
