@@ -254,26 +254,28 @@ constexpr int kRing = 8;                                      // ring of tile bo
 //       predecessor CTA does not stall this CTA's workers.
 // Tiles: the first two of a CTA are blockIdx.x and blockIdx.x + gridDim.x, the rest come from the ticket
 // counter, each drawn at the same point of the pipeline: a lower tile number means "sizes posted earlier".
-template <int W>
+template <int W, bool kBatch>
 __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
     extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | kNB image buffers
     __shared__ uint32_t s_key[kNB][kTileR];              // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
     __shared__ unsigned long long s_at[kNB][kTileR];     // scan warp: final byte offset of the block, or kSkip
     __shared__ uint32_t s_off16[kTileR];                 // exclusive scan of the sizes inside the tile (16-B units)
-    __shared__ int s_m[kRing][kTileR];                       // ring of tile bookkeeping: valid IDs of each block (0 = none)
-    __shared__ unsigned long long s_xoff[kRing][kTileR];     // element offset of the block's first ID
-    __shared__ uint32_t s_buf[kRing][kTileR];                // buffer of each block (batch calls)
+    // Ring of tile bookkeeping (batch calls only: a single buffer's blocks follow from the tile number).
+    constexpr int kBk = kBatch ? kTileR : 1;
+    __shared__ int s_m[kRing][kBk];                          // valid IDs of each block (0 = none)
+    __shared__ unsigned long long s_xoff[kRing][kBk];        // element offset of the block's first ID
+    __shared__ uint32_t s_buf[kRing][kBk];                   // buffer of each block
     __shared__ unsigned long long s_tile[kRing];             // tile of each ring slot, kNoTile = done
     __shared__ unsigned long long mb_post[kRing];        // warp 0 -> workers: the ring slot's tile is posted (use u of a slot: parity u & 1)
     __shared__ unsigned long long mb_off[kNB];           // scan warp -> workers: the offsets in s_at[kp] are posted
-    __shared__ unsigned int s_agg[2];                    // arrivals << 24 | sum of the worker warps' sizes (16-B units)
+    __shared__ unsigned int s_agg[4];                    // arrivals << 24 | sum of the worker warps' sizes (16-B units)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const bool batch = a.in_off != nullptr;
+    constexpr bool batch = kBatch;
     const T* ids = reinterpret_cast<const T*>(a.ids);
     pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
-    if (threadIdx.x < 2) s_agg[threadIdx.x] = 0;
+    if (threadIdx.x < 4) s_agg[threadIdx.x] = 0;
     if (threadIdx.x < kRing) mbar_init(&mb_post[threadIdx.x], 1);
     if (threadIdx.x >= 32 && threadIdx.x < 32 + kNB) mbar_init(&mb_off[threadIdx.x - 32], 1);
     __syncthreads();
@@ -291,22 +293,31 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     auto prep = [&](unsigned long long t, int p) {       // bookkeeping of tile t into ring slot p (one warp)
         if (lane == 0) s_tile[p] = t;
         if (t == kNoTile) return;
-        for (int jj = lane; jj < kTileR; jj += 32) {
+        if constexpr (kBatch) {
+          for (int jj = lane; jj < kTileR; jj += 32) {
             const unsigned long long g = t * kTileR + jj;
             int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
             if (g < total) {
-                if (batch) {
-                    i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
-                    const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
-                    m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-                    xoff = buf_start(a, i) + kBlk * k;
-                } else {
-                    m = (int)min((unsigned long long)kBlk, a.n_single - kBlk * g);
-                    xoff = kBlk * g;
-                }
+                i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
+                const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
+                m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+                xoff = buf_start(a, i) + kBlk * k;
             }
             s_m[p][jj] = m; s_xoff[p][jj] = xoff; s_buf[p][jj] = i;
+          }
         }
+    };
+    // valid IDs / element offset of block jj of the tile in ring slot p (the tile is posted and not kNoTile)
+    auto blk_m = [&](int p, int jj) -> int {
+        if constexpr (kBatch) return s_m[p][jj];
+        else {
+            const unsigned long long g = s_tile[p] * kTileR + jj;
+            return g < nb_single ? (int)min((unsigned long long)kBlk, a.n_single - kBlk * g) : 0;
+        }
+    };
+    auto blk_xoff = [&](int p, int jj) -> unsigned long long {
+        if constexpr (kBatch) return s_xoff[p][jj];
+        else return kBlk * (s_tile[p] * kTileR + jj);
     };
 
     if (warp == kEncWorkers) {
@@ -343,7 +354,11 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 if (kPer * lane + h < kTileR) s_off16[kPer * lane + h] = offs[h];
             }
             TR(t, 2);                                    // (the aggregate was published by the last worker warp)
+#ifdef BFSC_NOLB                                             // timing experiment only (never in libbfsc.so): no look-back, wrong offsets
+            const unsigned long long excl = t * (unsigned long long)kTileR * BFSC_NOLB;
+#else
             const unsigned long long excl = t > 0 ? lookback(a.ws.tile_state, t, lane) : 0ull;
+#endif
             TR(t, 3);
             if (lane == 0) {
                 st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagPre | (excl + agg));
@@ -368,7 +383,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                     unsigned long long first = 0, f0 = 0, f1 = f1_single, S = 0;
                     uint32_t i = 0;
                     if (batch) {
-                        i = s_buf[k & (kRing - 1)][jj];
+                        if constexpr (kBatch) i = s_buf[k & (kRing - 1)][jj];
                         first = a.ws.blk_first[i]; f0 = a.ws.fixed_prefix[i]; f1 = a.ws.fixed_prefix[i + 1];
                         if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
                         else if (i > 0) {                // published by the tile that owns the stream's first block
@@ -429,9 +444,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     }
     __syncthreads();                                                     // barrier 0
     bool have = s_tile[0] != kNoTile;
-    if (have) quad_prefetch<W>(slot, ids + s_xoff[0][j], s_m[0][j]);
-    static_assert(kDefer == 1, "one tile of images waits in shared memory");
-    uint32_t key_hist = 0, woff_hist = 0;                                // key and image place of the tile that waits in shared memory
+    if (have) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));
+    static_assert(kDefer == 1 || kDefer == 2, "hist selection below");
+    uint32_t key_hist[kDefer] = {}, woff_hist[kDefer] = {};              // keys and image places of the tiles that wait in shared memory
     unsigned int ticket = 0xffffffffu;                                   // warp 0: requested one iteration before it is used
     int kp = 0;                                                          // k % kNB
     int n_wait = 0, ke = 0;                                              // tiles packed but not copied out yet; next one to copy out
@@ -449,9 +464,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&mb_post[(k + 1) & (kRing - 1)]);
             }
-            const int m = s_m[k & (kRing - 1)][j];
+            const int m = blk_m(k & (kRing - 1), j);
             const T* raw = reinterpret_cast<const T*>(slot) +
-                           (reinterpret_cast<uintptr_t>(ids + s_xoff[k & (kRing - 1)][j]) & 15) / sizeof(T);
+                           (reinterpret_cast<uintptr_t>(ids + blk_xoff(k & (kRing - 1), j)) & 15) / sizeof(T);
             unsigned char* ib = ibuf + kp * (kImgBufChunks * 16);        // this tile's image buffer
             if (warp == 0) TR(s_tile[k & (kRing - 1)], 6);
             cp_async_wait_all();
@@ -462,7 +477,14 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             bool wide_lane = false, wide = false;
             const T base = col_deltas<W>(raw, m, d, wide_lane);          // E1
             if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
+#ifdef BFSC_SKIP_CHOOSE
+            if (!wide) { uint32_t o = 0;
+#pragma unroll
+                for (int i = 0; i < 32; i++) o |= d[i];
+                const uint32_t top = 32 - __clz(quad_or(o)); key = ((16u + 16u * top) << 14) | ((64u - top) << 7); }
+#else
             if (!wide) key = quad_choose_b<W>(d);                        // E2
+#endif
             else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (kImgSlotChunks * 16)));
             if (m <= 0) key = 0;
             if (l == 0) s_key[kp][j] = key;
@@ -472,9 +494,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 uint32_t z = l == 0 ? key >> 18 : 0u;
                 z += __shfl_xor_sync(kFull, z, 4); z += __shfl_xor_sync(kFull, z, 8); z += __shfl_xor_sync(kFull, z, 16);
                 if (lane == 0) {
-                    const unsigned int old = atomicAdd(&s_agg[k & 1], (1u << 24) | z);
+                    const unsigned int old = atomicAdd(&s_agg[k & 3], (1u << 24) | z);
                     if ((old >> 24) == kEncWorkers - 1) {
-                        s_agg[k & 1] = 0;
+                        s_agg[k & 3] = 0;
                         const unsigned long long t = s_tile[k & (kRing - 1)];
                         pdl_wait();                                      // the states are zeroed by the plan kernel
                         if (t > 0)
@@ -511,9 +533,13 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             __syncwarp();                                                // the warp's staged IDs are consumed
             mbar_wait(&mb_post[(k + 1) & (kRing - 1)], ((k + 1) / kRing) & 1);   // tile k+1 is posted
             have_next = s_tile[(k + 1) & (kRing - 1)] != kNoTile;
-            if (have_next) quad_prefetch<W>(slot, ids + s_xoff[(k + 1) & (kRing - 1)][j], s_m[(k + 1) & (kRing - 1)][j]);   // same slots
+            if (have_next) quad_prefetch<W>(slot, ids + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));   // same slots
             if (fast) {                                                  // payload + header
+#ifndef BFSC_SKIP_PACK
                 if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
+#else
+                if (b > 0) reinterpret_cast<uint32_t*>(img)[4 + l] = d[0] ^ d[7] ^ d[31];
+#endif
                 if (l == 0) {                                            // block header (FORMAT.md §2)
                     reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
                     reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
@@ -528,7 +554,8 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         // copy out the oldest waiting tile: tile k - kDefer while tiles keep coming, then drain
         const int w = n_wait - (have ? 1 : 0);                           // waiting tiles older than tile k
         if (w > 0 && (w == kDefer || !have)) {
-            const uint32_t key_e = key_hist, woff_e = woff_hist;         // key and image place of the CTA's tile ke
+            const uint32_t key_e = (kDefer == 2 && w == 2) ? key_hist[kDefer - 1] : key_hist[0];     // key and image place
+            const uint32_t woff_e = (kDefer == 2 && w == 2) ? woff_hist[kDefer - 1] : woff_hist[0];  // of the CTA's tile ke
             int kpe = kp - w;                                            // its buffer: ke % kNB
             if (kpe < 0) kpe += kNB;
             if (warp == 0) TR(s_tile[ke & (kRing - 1)], 10);
@@ -538,7 +565,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             if (key_e != 0) at = s_at[kpe][j];
             if (__any_sync(kFull, (key_e & kLateBit) != 0)) {
                 const bool mine = (key_e & kLateBit) != 0 && at != kSkip;
-                late_emit<W>(ids + s_xoff[ke & (kRing - 1)][j], s_m[ke & (kRing - 1)][j], key_e & ~kLateBit, mine ? a.out + at : nullptr);
+                late_emit<W>(ids + blk_xoff(ke & (kRing - 1), j), blk_m(ke & (kRing - 1), j), key_e & ~kLateBit, mine ? a.out + at : nullptr);
             }
             // images -> their final place. Usual case: the warp's blocks are consecutive in the output as well
             // (same stream, none late, all fit): ONE bulk store of the whole buffer by lane 0.
@@ -565,7 +592,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         }
         if (!have && n_wait == 0) break;
         if (have) {
-            key_hist = key; woff_hist = woff;
+#pragma unroll
+            for (int x = kDefer - 1; x > 0; x--) { key_hist[x] = key_hist[x - 1]; woff_hist[x] = woff_hist[x - 1]; }
+            key_hist[0] = key; woff_hist[0] = woff;
             kp = kp == kNB - 1 ? 0 : kp + 1;
         }
         have = have_next;
@@ -643,9 +672,10 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     static int max_grid = 0;                      // persistent grid: all CTAs resident
     if (max_grid == 0) {
         int per_sm = 0, dev = 0, sms = kNumSM;
-        if (cudaFuncSetAttribute(k_enc_tiles<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_enc_tiles<W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess ||
+            cudaFuncSetAttribute(k_enc_tiles<W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
             return BFSC_ERR_CUDA;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_tiles<W>, kEncThreads, kSmem) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_tiles<W, true>, kEncThreads, kSmem) != cudaSuccess ||
             per_sm < 1)
             per_sm = 1;
         cudaGetDevice(&dev);
@@ -666,7 +696,8 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     if (launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     BFSC_LAUNCH_CHECK();
     if (!degenerate) {
-        if (launch_dep(k_enc_tiles<W>, grid, kEncThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        if ((single ? launch_dep(k_enc_tiles<W, false>, grid, kEncThreads, kSmem, s, a)
+                    : launch_dep(k_enc_tiles<W, true>, grid, kEncThreads, kSmem, s, a)) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
         BFSC_LAUNCH_CHECK();
     }
     if (!single || degenerate) {

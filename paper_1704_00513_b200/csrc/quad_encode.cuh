@@ -122,6 +122,14 @@ __device__ __forceinline__ uint32_t msb_pos(uint32_t x) {
     return r;
 }
 
+// a * b + c as ONE IMAD (fma pipe): the alu pipe (LOP3 / SHF / IADD3, one warp instruction per two cycles
+// and scheduler) is the busiest unit of the encoder.
+__device__ __forceinline__ uint32_t mad_fma_pipe(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+
 template <int W>
 __device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
     const int l = quad_l();
@@ -139,7 +147,7 @@ __device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
         const int K = 4 * (top - 1);                 // t = top - width = (top - 1) - msb_pos; msb_pos(0) = -1
 #pragma unroll
         for (int i = 0; i < 32; i++)                 // t < 0 or t >= 8: the shift clamps to 0
-            acc[i / 12] += shl32(0x11111111u, (uint32_t)(K - 4 * (int)msb_pos(d[i])));
+            acc[i / 12] = mad_fma_pipe(shl32(1u, (uint32_t)(K - 4 * (int)msb_pos(d[i]))), 0x11111111u, acc[i / 12]);
         uint32_t lo = (acc[0] & 0x0f0f0f0fu) + (acc[1] & 0x0f0f0f0fu) + (acc[2] & 0x0f0f0f0fu);
         uint32_t hi = ((acc[0] >> 4) & 0x0f0f0f0fu) + ((acc[1] >> 4) & 0x0f0f0f0fu) + ((acc[2] >> 4) & 0x0f0f0f0fu);
         lo = quad_add(lo);                           // bytes: exceptions added at s = 1,3,5,7 (b = top - s)
