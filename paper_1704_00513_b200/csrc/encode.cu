@@ -165,13 +165,17 @@ __device__ __forceinline__ void mbar_init(unsigned long long* b, uint32_t count)
 __device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(b)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {   // until the phase of that parity has completed
-    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(b);
+__device__ __forceinline__ bool mbar_test(uint32_t addr, uint32_t parity) {
     uint32_t ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
-    } while (!ok);
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    return ok != 0;
+}
+// Until the phase of that parity has completed. Whole warp calls. A warp that has to wait sleeps between
+// polls: a spinning warp would take issue slots from the warps it waits for.
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(b);
+    while (!mbar_test(addr, parity)) __nanosleep(64);
 }
 // Bulk (TMA) store shared -> global, issued by one lane: 16-byte aligned addresses, size a multiple of 16.
 __device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, uint32_t bytes) {
