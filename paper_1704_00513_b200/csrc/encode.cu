@@ -35,7 +35,8 @@ constexpr int kEncWorkers = 8;                           // worker warps per CTA
 constexpr int kTileR = kEncWorkers * kQuadBlocks;        // 64 blocks per tile
 static_assert(kTileR >= kTileBlocks, "workspace sizing assumes tiles of at least kTileBlocks blocks");
 constexpr int kPer = (kTileR + 31) / 32;                 // blocks per lane of the scan warp
-constexpr int kEncThreads = (kEncWorkers + 1) * 32;      // + the scan warp
+constexpr int kEncThreads = (kEncWorkers + 2) * 32;      // + the scan warp + the prep warp
+constexpr int kSizesThreads = (kEncWorkers + 1) * 32;    // threads on the "sizes posted" barrier: workers + scan warp
 
 // ---- E0: plan. One CTA; per buffer: mode, block count, fixed bytes; exclusive prefixes. ----
 template <int W>
@@ -273,6 +274,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     __shared__ unsigned long long s_tile[kRing];             // tile of each ring slot, kNoTile = done
     __shared__ unsigned long long mb_post[kRing];        // warp 0 -> workers: the ring slot's tile is posted (use u of a slot: parity u & 1)
     __shared__ unsigned long long mb_off[kNB];           // scan warp -> workers: the offsets in s_at[kp] are posted
+    __shared__ volatile unsigned int s_sized;            // scan warp: tiles of this CTA whose sizes have arrived (the prep warp follows it)
     __shared__ unsigned int s_agg[4];                    // arrivals << 24 | sum of the worker warps' sizes (16-B units)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -280,6 +282,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     const T* ids = reinterpret_cast<const T*>(a.ids);
     pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
     if (threadIdx.x < 4) s_agg[threadIdx.x] = 0;
+    if (threadIdx.x == 4) s_sized = 0;
     if (threadIdx.x < kRing) mbar_init(&mb_post[threadIdx.x], 1);
     if (threadIdx.x >= 32 && threadIdx.x < 32 + kNB) mbar_init(&mb_off[threadIdx.x - 32], 1);
     __syncthreads();
@@ -331,10 +334,12 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         if (!batch) pdl_wait();                          // the plan kernel's writes are visible from here on
         int kp = 0;                                      // k % kNB
         for (int k = 0;; k++) {
-            const unsigned long long t = s_tile[k & (kRing - 1)];  // posted before the sizes of tile k-1 arrived
+            mbar_wait(&mb_post[k & (kRing - 1)], (k / kRing) & 1);   // the prep warp has posted the CTA's tile k
+            const unsigned long long t = s_tile[k & (kRing - 1)];
             if (t == kNoTile) break;
             TR(t, 0);
-            bar_sync(kBarSizes + kp, kEncThreads);       // the workers' sizes of tile t are in s_key[kp]
+            bar_sync(kBarSizes + kp, kSizesThreads);
+            if (lane == 0) s_sized = (unsigned int)k + 1u;      // the workers' sizes of tile t are in s_key[kp]
 
             // E3: intra-tile scan (kPer consecutive blocks per lane)
             uint32_t kk[kPer], offs[kPer], inc = 0;
@@ -432,6 +437,37 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         return;
     }
 
+    if (warp == kEncWorkers + 1) {
+        // =============================== prep warp ===============================
+        // Runs ahead of the workers: draws the ticket of the CTA's tile p (p >= 2; tiles 0 and 1 are static),
+        // prepares its bookkeeping (batch calls: buffer, first ID, valid IDs of every block — a chain of
+        // dependent global loads nobody else has to wait for) and posts it. The ticket of tile p is drawn when
+        // the sizes of tile p - 2 have arrived: every CTA draws at the same point of its pipeline, so a lower
+        // tile number means "sizes posted earlier" and look-backs rarely wait; and no worker can still read the
+        // ring slot (kRing = 8) that is rewritten.
+        {
+            const unsigned long long t0 = blockIdx.x, t1 = (unsigned long long)blockIdx.x + gridDim.x;
+            prep(t0 < n_tiles ? t0 : kNoTile, 0);
+            prep(t0 < n_tiles && t1 < n_tiles ? t1 : kNoTile, 1);
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(&mb_post[0]); mbar_arrive(&mb_post[1]); }
+        }
+        __syncthreads();                                 // barrier 0
+        bool more = s_tile[1] != kNoTile;
+        if (more) pdl_wait();                            // the ticket counter is set by the plan kernel
+        for (int pt = 2; more; pt++) {
+            while ((int)s_sized + 1 < pt) __nanosleep(100);
+            unsigned int ticket = 0;
+            if (lane == 0) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+            ticket = __shfl_sync(kFull, ticket, 0);
+            more = ticket < n_tiles;
+            prep(more ? (unsigned long long)ticket : kNoTile, pt & (kRing - 1));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&mb_post[pt & (kRing - 1)]);
+        }
+        return;
+    }
+
     // =============================== worker warps ===============================
     const int q = lane >> 2, l = lane & 3;
     uint4* area = dyn_smem + warp * EncSmem<W>::kWarpChunks;
@@ -439,35 +475,17 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     unsigned char* ibuf = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks);   // the warp's kNB image buffers
     const int j = warp * kQuadBlocks + q;
     constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
-    if (warp == 0) {                                                     // the CTA's first two tiles are static
-        const unsigned long long t0 = blockIdx.x, t1 = (unsigned long long)blockIdx.x + gridDim.x;
-        prep(t0 < n_tiles ? t0 : kNoTile, 0);
-        prep(t0 < n_tiles && t1 < n_tiles ? t1 : kNoTile, 1);
-        __syncwarp();
-        if (lane == 0) { mbar_arrive(&mb_post[0]); mbar_arrive(&mb_post[1]); }
-    }
-    __syncthreads();                                                     // barrier 0
+    __syncthreads();                                                     // barrier 0: the first two tiles are posted
     bool have = s_tile[0] != kNoTile;
     if (have) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));
     static_assert(kDefer == 1 || kDefer == 2, "hist selection below");
     uint32_t key_hist[kDefer] = {}, woff_hist[kDefer] = {};              // keys and image places of the tiles that wait in shared memory
-    unsigned int ticket = 0xffffffffu;                                   // warp 0: requested one iteration before it is used
     int kp = 0;                                                          // k % kNB
     int n_wait = 0, ke = 0;                                              // tiles packed but not copied out yet; next one to copy out
     for (int k = 0;; k++) {
         uint32_t key = 0, woff = 0;
         bool have_next = false;
         if (have) {
-            if (warp == 0 && k >= 1) {                                   // tile k+1: ticket -> bookkeeping (ring slot (k+1) & 3)
-                unsigned long long t = kNoTile;
-                if (s_tile[k & (kRing - 1)] != kNoTile) {
-                    ticket = __shfl_sync(kFull, ticket, 0);
-                    if (ticket < n_tiles) t = ticket;
-                }
-                prep(t, (k + 1) & (kRing - 1));
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&mb_post[(k + 1) & (kRing - 1)]);
-            }
             const int m = blk_m(k & (kRing - 1), j);
             const T* raw = reinterpret_cast<const T*>(slot) +
                            (reinterpret_cast<uintptr_t>(ids + blk_xoff(k & (kRing - 1), j)) & 15) / sizeof(T);
@@ -509,14 +527,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 }
             }
             if (warp == 0) TR(s_tile[k & (kRing - 1)], 8);
-            bar_arrive(kBarSizes + kp, kEncThreads);
-            if (warp == 0) {                                             // ticket of tile k+2 (used next iteration)
-                ticket = 0xffffffffu;
-                if (lane == 0 && s_tile[(k + 1) & (kRing - 1)] != kNoTile) {
-                    pdl_wait();
-                    ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
-                }
-            }
+            bar_arrive(kBarSizes + kp, kSizesThreads);
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
             const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)kImgCap);   // slow path, in global memory later
@@ -581,7 +592,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             const bool contig = !valid || (fast_e && at != kSkip && (!valid_n || at_n == at + 16ull * z_e));
             if (__all_sync(kFull, contig)) {
                 const uint32_t tot = __shfl_sync(kFull, woff_e + z_e, 31);
+#ifndef BFSC_NOFENCE
                 fence_proxy_async_smem();                                // the image was written through the generic proxy
+#endif
                 __syncwarp();
                 if (lane == 0 && tot > 0) bulk_store(a.out + at, ib_e, 16u * tot);
             } else if (fast_e && at != kSkip) {
