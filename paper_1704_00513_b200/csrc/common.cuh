@@ -22,6 +22,8 @@ template <> struct IdT<64> { using T = uint64_t; };
 // [WsHeader 256 B][blk_first u64 (n_buf+1)][fixed_prefix u64 (n_buf+1)][stream_start u64 (n_buf+1)]
 // [tile_state: tile_cap entries of kStateStride u64 (one 64-byte entry per tile: the look-back polls
 //  of the tiles in flight then spread over many L2 slices instead of a few hot lines)]
+// [blk_tab: blk_cap entries of 32 B — batch calls: where each block of the batch lives (EncBlk / DecBlk),
+//  written by k_*_blocks after the plan, so that the tile kernels find a block with ONE load]
 struct WsHeader {
     unsigned long long total_blocks;    // blocks of all PFOR streams of the batch
     unsigned long long fixed_total;     // sum of per-stream fixed bytes (header+directory | header+raw)
@@ -39,32 +41,41 @@ struct WsView {
     unsigned long long* fixed_prefix;   // n_buf+1 : exclusive prefix of fixed bytes (decode: of IDs)
     unsigned long long* stream_start;   // n_buf+1 : encode: 1 + byte offset of the stream (0 = not yet known)
     unsigned long long* tile_state;     // tile_cap * kStateStride
+    uint4* blk_tab;                     // blk_cap * 2 (32 B per block), batch calls only
     size_t blk_cap;
     size_t tile_cap;
 };
 
 constexpr int kTileBlocks = 64;         // blocks per encode tile (8 worker warps x 8 blocks)
 constexpr int kStateStride = 8;         // u64 words between look-back states (64 B)
+constexpr size_t kTileWsBytes = 8 * kStateStride + 32 * kTileBlocks;   // workspace per tile: state + block table
+
+// Block table entries (batch calls). Encode: where the block's IDs are. Decode: where its stream is, which
+// block of the stream it is and where its IDs go.
+struct EncBlk { unsigned long long xoff; uint32_t m; uint32_t buf; uint4 pad; };              // first ID (element), valid IDs, buffer
+struct DecBlk { unsigned long long s_begin, x_index; uint32_t k, m, total16, nb; };           // stream start (byte), first ID (element), block, valid IDs, stream bytes / 16, blocks of the stream
+static_assert(sizeof(EncBlk) == 32 && sizeof(DecBlk) == 32, "block table entries are 32 B");
 
 __host__ __device__ inline size_t align_up(size_t x, size_t k) { return (x + k - 1) / k * k; }
 
 __host__ inline size_t ws_bytes_for(size_t n_ids_total, size_t n_buf) {
     const size_t blk_cap = n_ids_total / kBlk + n_buf + 1;
     const size_t tile_cap = blk_cap / kTileBlocks + 2;
-    return sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + 8 * kStateStride * tile_cap + 256;
+    return sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + kTileWsBytes * tile_cap + 256;
 }
 
 // Carves the workspace; the capacities are derived from the bytes actually provided.
 __host__ inline bool ws_carve(void* ws, size_t bytes, size_t n_buf, WsView* v) {
     const size_t fixed = sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16);
-    if (bytes < fixed + 8 * kStateStride * 2) return false;
-    const size_t tile_cap = (bytes - fixed) / (8 * kStateStride);
+    if (bytes < fixed + kTileWsBytes * 2) return false;
+    const size_t tile_cap = (bytes - fixed) / kTileWsBytes;
     char* p = (char*)ws;
     v->hdr = (WsHeader*)p; p += sizeof(WsHeader);
     v->blk_first = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
     v->fixed_prefix = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
     v->stream_start = (unsigned long long*)p; p += align_up(8 * (n_buf + 1), 16);
-    v->tile_state = (unsigned long long*)p;
+    v->tile_state = (unsigned long long*)p; p += 8 * kStateStride * tile_cap;
+    v->blk_tab = (uint4*)p;
     v->tile_cap = tile_cap;
     v->blk_cap = (tile_cap - 1) * kTileBlocks;
     return true;
@@ -153,9 +164,11 @@ __device__ __forceinline__ void plan_hints_of(uint32_t i, unsigned long long fir
 __device__ __forceinline__ void plan_hints_flush(unsigned long long* __restrict__ tile_state, size_t tile_cap, HintQueue* q) {
     __syncthreads();
     const unsigned int n = q->n < (unsigned)kHintQueue ? q->n : (unsigned)kHintQueue;
-    for (unsigned int e = 0; e < n; e++) {
+    const unsigned int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (unsigned int e = warp; e < n; e += nw) {        // one warp per queued buffer (not every warp through every entry)
         const unsigned long long t0 = (q->first[e] + kTileBlocks - 1) / kTileBlocks, t1 = (q->first[e] + q->nb[e] - 1) / kTileBlocks;
-        for (unsigned long long t = t0 + threadIdx.x; t <= t1 && t < tile_cap; t += blockDim.x) tile_state[t * kStateStride + 1] = q->buf[e];
+        const unsigned int b = q->buf[e];
+        for (unsigned long long t = t0 + lane; t <= t1 && t < tile_cap; t += 32) tile_state[t * kStateStride + 1] = b;
     }
     __syncthreads();
     if (threadIdx.x == 0) q->n = 0;

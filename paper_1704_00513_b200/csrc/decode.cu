@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
         Scan2 v[kIpt], sum{0, 0};
         unsigned long long beg[kIpt], avail[kIpt];
         bool rd[kIpt];
+        unsigned long long tot_bytes[kIpt];
         uint4 h0[kIpt], h1[kIpt];
 #pragma unroll
         for (int u = 0; u < kIpt; u++) {                 // phase 1: extents (independent loads)
@@ -68,6 +69,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
         for (int u = 0; u < kIpt; u++) {                 // phase 3: validation (FORMAT.md §4)
             const uint32_t i = i0 + threadIdx.x * kIpt + u;
             v[u] = Scan2{0, 0};
+            tot_bytes[u] = 0;
             if (i < a.n_buf) {
                 bool ok = rd[u];
                 if (ok) {
@@ -83,7 +85,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
                     else if (nb != (n + kBlk - 1) / kBlk || n > (1ull << 40) ||
                              32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
                         ok = false;
-                    if (ok) { v[u].a = nb; v[u].b = n; }
+                    if (ok) { v[u].a = nb; v[u].b = n; tot_bytes[u] = total; }
                 }
                 if (!ok) bad = 1;
             }
@@ -98,6 +100,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
             if (i < a.n_buf) {
                 a.ws.blk_first[i] = ex.a;
                 a.ws.fixed_prefix[i] = ex.b;
+                a.ws.stream_start[i] = tot_bytes[u];     // (decode: validated total_bytes of the stream)
                 plan_hints_of(i, ex.a, v[u].a, a.ws.tile_state, a.ws.tile_cap, &hq);
             }
             ex.a += v[u].a; ex.b += v[u].b;
@@ -121,6 +124,29 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
     __syncthreads();
     if (a.id_off)
         for (uint32_t i = threadIdx.x; i <= a.n_buf; i += blockDim.x) a.id_off[i] = good ? a.ws.fixed_prefix[i] : 0ull;
+}
+
+// ---- D0 (batch calls), second part: the block table. One thread per block of the batch: its stream
+// (search from the group hint), which block of the stream it is and where its IDs go -> ws.blk_tab, so that
+// k_dec_tiles reaches a block's directory entry with one load instead of a chain of dependent ones.
+constexpr int kBlkTabThreads = 256;
+template <int W>
+__global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
+    pdl_wait();
+    pdl_launch_dependents();
+    if (a.ws.hdr->ok == 0) return;
+    const unsigned long long total = a.ws.hdr->total_blocks;
+    for (unsigned long long g = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; g < total;
+         g += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
+        const unsigned long long k = g - a.ws.blk_first[i], id0 = a.ws.fixed_prefix[i], n = a.ws.fixed_prefix[i + 1] - id0;
+        const unsigned long long sb = s_begin(a, i), xi = id0 + kBlk * k;
+        uint4 e0, e1;
+        e0.x = (uint32_t)sb; e0.y = (uint32_t)(sb >> 32); e0.z = (uint32_t)xi; e0.w = (uint32_t)(xi >> 32);
+        e1.x = (uint32_t)k; e1.y = (uint32_t)min((unsigned long long)kBlk, n - kBlk * k);
+        e1.z = (uint32_t)(a.ws.stream_start[i] >> 4); e1.w = (uint32_t)((n + kBlk - 1) / kBlk);
+        a.ws.blk_tab[2 * g] = e0; a.ws.blk_tab[2 * g + 1] = e1;
+    }
 }
 
 
@@ -150,7 +176,7 @@ struct BlockAt {                       // where the quad's block is
     int m;                             // valid IDs
 };
 
-template <int W>
+template <int W, bool kBatch>          // kBatch: a.in_off != nullptr
 __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(DecArgs a) {
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
@@ -163,7 +189,7 @@ __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(De
     uint4* slot = stage + kDecSlotChunks * q;
     T* tab = tab_w + kBlk * q;
 
-    const bool batch = a.in_off != nullptr;
+    constexpr bool batch = kBatch;
     unsigned long long total_blocks, n1 = 0, total16_1 = 0, lo16_1 = 0;   // single stream: n, total/16, first block/16
     pdl_wait();                                                            // the kernel before this one is complete
     pdl_launch_dependents();                                               // the next one may be set up; it waits for this grid
@@ -216,21 +242,25 @@ __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(De
         if (g >= total_blocks) return r;
         const unsigned char* s = a.in;
         unsigned long long k = g, id0 = 0, n = n1, total16 = total16_1, lo16 = lo16_1;
-        if (batch) {
-            const uint32_t i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
-            k = g - a.ws.blk_first[i];
-            id0 = a.ws.fixed_prefix[i]; n = a.ws.fixed_prefix[i + 1] - id0;
-            s = a.in + s_begin(a, i);
-            total16 = *reinterpret_cast<const unsigned long long*>(s + 16) >> 4;
-            lo16 = (32ull + ((4ull * ((n + kBlk - 1) / kBlk + 1) + 15ull) & ~15ull)) >> 4;
+        int m;
+        unsigned long long xi;
+        if (batch) {                                                       // ws.blk_tab, written by k_dec_blocks
+            const uint4 e0 = __ldcg(a.ws.blk_tab + 2 * g), e1 = __ldcg(a.ws.blk_tab + 2 * g + 1);
+            s = a.in + ((unsigned long long)e0.y << 32 | e0.x);
+            xi = (unsigned long long)e0.w << 32 | e0.z;
+            k = e1.x; m = (int)e1.y; total16 = e1.z;
+            lo16 = (32ull + ((4ull * ((unsigned long long)e1.w + 1) + 15ull) & ~15ull)) >> 4;
+        } else {
+            m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+            xi = id0 + kBlk * k;
         }
         const uint32_t* dir = reinterpret_cast<const uint32_t*>(s + 32);
         const unsigned long long o0 = dir[k], o1 = dir[k + 1];
         if (o0 < lo16 || o1 <= o0 || o1 > total16) { set_status(a.status, BFSC_ERR_CORRUPT); return r; }
         r.blk = s + 16ull * o0;
         r.span16 = (uint32_t)(o1 - o0);
-        r.m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-        r.x = reinterpret_cast<T*>(a.ids) + id0 + kBlk * k;
+        r.m = m;
+        r.x = reinterpret_cast<T*>(a.ids) + xi;
         return r;
     };
 
@@ -263,7 +293,7 @@ __global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(De
                         __shfl_sync(kFull, lv, 4 * q + 2) & __shfl_sync(kFull, lv, 4 * q + 3)) != 0;
             }
             const T base = (T)((unsigned long long)h.y << 32 | h.x);
-            quad_decode_rows<W>(slot + 1, live ? b : 0u, tab, patch, base, cur.x, live ? cur.m : 0, l);   // D2-D4
+            quad_decode_rows<W, kBatch>(slot + 1, live ? b : 0u, tab, patch, base, cur.x, live ? cur.m : 0, l);   // D2-D4
             if (patch) {
                 __syncwarp();
                 quad_patch_clear<W>(tab, e, (cur.blk != nullptr && b <= (uint32_t)W && n_exc <= 127u && 1u + b + exc_bytes<W>(n_exc) / 16u <= cur.span16) ? n_exc : 0u, l);
@@ -315,9 +345,10 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     static int max_grid = 0;
     if (max_grid == 0) {
         int per_sm = 0, dev = 0, sms = kNumSM;
-        if (cudaFuncSetAttribute(k_dec_tiles<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_dec_tiles<W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess ||
+            cudaFuncSetAttribute(k_dec_tiles<W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
             return BFSC_ERR_CUDA;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dec_tiles<W>, kDecThreads, kSmem) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dec_tiles<W, true>, kDecThreads, kSmem) != cudaSuccess ||
             per_sm < 1)
             per_sm = 1;
         cudaGetDevice(&dev);
@@ -330,9 +361,13 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     if (a.in_off) {
         if (launch_dep(k_dec_plan<W>, 1, 1024, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
         BFSC_LAUNCH_CHECK();
-        if (launch_dep(k_dec_tiles<W>, max_grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        size_t bgrid = (a.ws.blk_cap + kBlkTabThreads - 1) / kBlkTabThreads;
+        if (bgrid > (size_t)(kNumSM * 8)) bgrid = (size_t)(kNumSM * 8);
+        if (launch_dep(k_dec_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        BFSC_LAUNCH_CHECK();
+        if (launch_dep(k_dec_tiles<W, true>, max_grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     } else {
-        if (launch_dep(k_dec_tiles<W>, grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        if (launch_dep(k_dec_tiles<W, false>, grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     }
     BFSC_LAUNCH_CHECK();
     return BFSC_OK;

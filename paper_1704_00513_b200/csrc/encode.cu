@@ -124,6 +124,29 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
     }
 }
 
+// ---- E0 (batch calls), second part: the block table. One thread per block of the batch: its buffer
+// (search from the group hint: one or two cached loads), first ID and valid IDs -> ws.blk_tab, so that
+// k_enc_tiles finds a block with one load instead of a chain of dependent ones.
+constexpr int kBlkTabThreads = 256;
+template <int W>
+__global__ void __launch_bounds__(kBlkTabThreads) k_enc_blocks(EncArgs a) {
+    pdl_wait();
+    pdl_launch_dependents();
+    if (a.ws.hdr->ok == 0) return;
+    const unsigned long long total = a.ws.hdr->total_blocks;
+    EncBlk* tab = reinterpret_cast<EncBlk*>(a.ws.blk_tab);
+    for (unsigned long long g = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; g < total;
+         g += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
+        const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
+        uint4 e;
+        const unsigned long long xoff = buf_start(a, i) + kBlk * k;
+        e.x = (uint32_t)xoff; e.y = (uint32_t)(xoff >> 32);
+        e.z = (uint32_t)min((unsigned long long)kBlk, n - kBlk * k); e.w = i;
+        reinterpret_cast<uint4*>(tab + g)[0] = e;        // (the second half of the entry is unused by encode)
+    }
+}
+
 // ---- E1-E4 fused: one pass over HBM ------------------------------------------------------
 // CTA = 8 worker warps + 1 scan warp; tile = 64 consecutive blocks (32 KB of u32 IDs), pulled by
 // ticket. Worker warps handle 8 blocks each, four lanes per block (quad_encode.cuh):
@@ -304,11 +327,9 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
           for (int jj = lane; jj < kTileR; jj += 32) {
             const unsigned long long g = t * kTileR + jj;
             int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
-            if (g < total) {
-                i = find_buf_from(a.ws.blk_first, a.n_buf, g, group_hint(a.ws.tile_state, g));
-                const unsigned long long k = g - a.ws.blk_first[i], n = buf_count(a, i);
-                m = (int)min((unsigned long long)kBlk, n - kBlk * k);
-                xoff = buf_start(a, i) + kBlk * k;
+            if (g < total) {                             // ws.blk_tab, written by k_enc_blocks
+                const uint4 e = __ldcg(reinterpret_cast<const uint4*>(reinterpret_cast<const EncBlk*>(a.ws.blk_tab) + g));
+                xoff = (unsigned long long)e.y << 32 | e.x; m = (int)e.z; i = e.w;
             }
             s_m[p][jj] = m; s_xoff[p][jj] = xoff; s_buf[p][jj] = i;
           }
@@ -363,6 +384,22 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                 if (kPer * lane + h < kTileR) s_off16[kPer * lane + h] = offs[h];
             }
             TR(t, 2);                                    // (the aggregate was published by the last worker warp)
+            // batch calls: the per-buffer constants of this lane's blocks, requested BEFORE the look-back (their
+            // latency hides behind it)
+            const unsigned long long g0 = t * kTileR;
+            unsigned long long bf_first[kPer], bf_f0[kPer], bf_f1[kPer];
+            uint32_t bf_i[kPer];
+            if constexpr (kBatch) {
+#pragma unroll
+                for (int h = 0; h < kPer; h++) {
+                    const int jj = kPer * lane + h;
+                    bf_i[h] = 0; bf_first[h] = 0; bf_f0[h] = 0; bf_f1[h] = 0;
+                    if (jj < kTileR && g0 + jj < total) {
+                        const uint32_t i = s_buf[k & (kRing - 1)][jj];
+                        bf_i[h] = i; bf_first[h] = a.ws.blk_first[i]; bf_f0[h] = a.ws.fixed_prefix[i]; bf_f1[h] = a.ws.fixed_prefix[i + 1];
+                    }
+                }
+            }
 #ifdef BFSC_NOLB                                             // timing experiment only (never in libbfsc.so): no look-back, wrong offsets
             const unsigned long long excl = t * (unsigned long long)kTileR * BFSC_NOLB;
 #else
@@ -379,7 +416,6 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             __syncwarp();
 
             // final offsets, directory entries, stream starts
-            const unsigned long long g0 = t * kTileR;
 #pragma unroll
             for (int h = 0; h < kPer; h++) {
                 const int jj = kPer * lane + h;
@@ -391,9 +427,8 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
                     const uint32_t off = offs[h], bytes = key >> 14;
                     unsigned long long first = 0, f0 = 0, f1 = f1_single, S = 0;
                     uint32_t i = 0;
-                    if (batch) {
-                        if constexpr (kBatch) i = s_buf[k & (kRing - 1)][jj];
-                        first = a.ws.blk_first[i]; f0 = a.ws.fixed_prefix[i]; f1 = a.ws.fixed_prefix[i + 1];
+                    if constexpr (kBatch) {
+                        i = bf_i[h]; first = bf_first[h]; f0 = bf_f0[h]; f1 = bf_f1[h];
                         if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
                         else if (i > 0) {                // published by the tile that owns the stream's first block
                             do { S = ld_volatile_u64(&a.ws.stream_start[i]); } while (S == 0);
@@ -712,6 +747,13 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     a.grid = (uint32_t)grid;
     if (launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     BFSC_LAUNCH_CHECK();
+    if (!single) {
+        const size_t cap_blocks = a.ws.blk_cap;
+        size_t bgrid = (cap_blocks + kBlkTabThreads - 1) / kBlkTabThreads;
+        if (bgrid > (size_t)(kNumSM * 8)) bgrid = (size_t)(kNumSM * 8);
+        if (launch_dep(k_enc_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        BFSC_LAUNCH_CHECK();
+    }
     if (!degenerate) {
         if ((single ? launch_dep(k_enc_tiles<W, false>, grid, kEncThreads, kSmem, s, a)
                     : launch_dep(k_enc_tiles<W, true>, grid, kEncThreads, kSmem, s, a)) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }

@@ -66,7 +66,7 @@ __device__ __forceinline__ void quad_patch_clear(typename IdT<W>::T* __restrict_
 //   D4  inclusive scan: prefix inside the row, inclusive scan of the row sums over the quad, running
 //       carry over the steps (order of the IDs: i major, then lane, then column); + base, mod 2^W;
 //       128-bit stores of the first m IDs.
-template <int W>
+template <int W, bool kWin>
 __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, uint32_t b,
                                                  const typename IdT<W>::T* __restrict__ tab, bool patch,
                                                  typename IdT<W>::T base, typename IdT<W>::T* __restrict__ x, int m, int l) {
@@ -76,6 +76,15 @@ __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, ui
     T carry = base;
     const bool vec_ok = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
     const bool vec = __all_sync(kFull, vec_ok || m <= 0);
+    // General path (some block of the warp is ragged or its output is not 16-byte aligned — buffers of a
+    // batch start at any element). kWin (batch calls): the row is shifted by e elements through the quad so
+    // that every lane still writes one ALIGNED 16/32-byte window (prev row's last e values | this row's
+    // first 4 - e); full-sector stores matter: 4- and 8-byte stores quadruple the L2 write requests.
+    // !kWin (single stream: only the warp with the ragged last block gets here): guarded element stores.
+    const int lane = threadIdx.x & 31;
+    const int e = (int)((reinterpret_cast<uintptr_t>(x) & 15) / sizeof(T));
+    const int src = (l == 0) ? lane + 3 : lane - 1;                     // owner of the previous row
+    T q1 = 0, q2 = 0, q3 = 0;                                            // this lane's previous row step
 #pragma unroll
     for (int i = 0; i < 8; i++) {
         const uint32_t k0 = bit >> 5, sh = bit & 31u;
@@ -113,12 +122,41 @@ __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, ui
                     __stcs(p + 1, make_ulonglong2(v2, v3));
                 }
             }
-        } else {
+        } else if constexpr (!kWin) {
             const int jx = 16 * i + 4 * l;
             if (jx < m) x[jx] = v0;
             if (jx + 1 < m) x[jx + 1] = v1;
             if (jx + 2 < m) x[jx + 2] = v2;
             if (jx + 3 < m) x[jx + 3] = v3;
+        } else {
+            // previous row's v1..v3: lane l-1 of this step, or lane 3 of the previous step (which publishes q*)
+            const T p1 = __shfl_sync(kFull, l == 3 ? q1 : v1, src), p2 = __shfl_sync(kFull, l == 3 ? q2 : v2, src);
+            const T p3 = __shfl_sync(kFull, l == 3 ? q3 : v3, src);
+            q1 = v1; q2 = v2; q3 = v3;
+            const T c0 = e == 0 ? v0 : (e == 1 ? p3 : (e == 2 ? p2 : p1));
+            const T c1 = e == 0 ? v1 : (e == 1 ? v0 : (e == 2 ? p3 : p2));
+            const T c2 = e == 0 ? v2 : (e == 1 ? v1 : (e == 2 ? v0 : p3));
+            const T c3 = e == 0 ? v3 : (e == 1 ? v2 : (e == 2 ? v1 : v0));
+            const int j0 = 16 * i + 4 * l - e;                           // first element of the window
+            T* w = x + j0;                                               // 16-byte aligned
+            if (j0 >= 0 && j0 + 3 < m) {
+                if constexpr (W == 32) {
+                    __stcs(reinterpret_cast<uint4*>(w), make_uint4(c0, c1, c2, c3));
+                } else {
+                    __stcs(reinterpret_cast<ulonglong2*>(w), make_ulonglong2(c0, c1));
+                    __stcs(reinterpret_cast<ulonglong2*>(w) + 1, make_ulonglong2(c2, c3));
+                }
+            } else {
+                if (j0 >= 0 && j0 < m) w[0] = c0;
+                if (j0 + 1 >= 0 && j0 + 1 < m) w[1] = c1;
+                if (j0 + 2 >= 0 && j0 + 2 < m) w[2] = c2;
+                if (j0 + 3 < m) w[3] = c3;                               // j0 + 3 >= 0 always
+            }
+            if (i == 7 && l == 3) {                                      // the block's last e elements
+                if (e >= 1 && 127 < m) x[127] = v3;
+                if (e >= 2 && 126 < m) x[126] = v2;
+                if (e >= 3 && 125 < m) x[125] = v1;
+            }
         }
     }
 }
