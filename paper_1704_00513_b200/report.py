@@ -42,46 +42,75 @@ class Runner:
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
         self.peak = peak_gbs()
 
-    def _time(self, fn):
-        best = None
-        for _ in range(self.reps + 1):                       # first repetition = warm-up
+    def _time(self, fns):
+        """fns: the same call on `len(fns)` rotating copies of its buffers. Returns (per-call ms in a run of
+        back-to-back calls, ms of one isolated call with a cold L2, host-bound flag: enqueueing the run took the
+        host at least 90 % of the time the GPU needed, i.e. the figure is the host's, not the kernels')."""
+        import time
+        for f in fns:                                        # warm-up
+            f()
+        torch.cuda.synchronize()
+        rounds = max(self.reps, -(-40 // len(fns)))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(rounds):
+            for f in fns:
+                f()
+        e1.record()
+        host_ms = 1e3 * (time.perf_counter() - t0)
+        torch.cuda.synchronize()
+        gpu_ms = e0.elapsed_time(e1)
+        stream_ms = gpu_ms / (rounds * len(fns))
+        self.host_bound = self.host_bound or host_ms >= 0.9 * gpu_ms
+        iso = None
+        for _ in range(3):
             self.flush.zero_()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(); fn(); e1.record()
+            e0.record(); fns[0](); e1.record()
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
-            best = ms if best is None else min(best, ms)
-        return best
+            iso = ms if iso is None else min(iso, ms)
+        return stream_ms, iso
 
     def batch(self, ids, off, W, thr, single=False):
-        """ids: device tensor (bit pattern), off: device int64 offsets. Returns dict of results."""
+        """ids: device tensor (bit pattern), off: device int64 offsets. Returns dict of results. Timed on
+        `copies` rotating copies of every buffer (working set >= 256 MB, 2..8 copies)."""
         dev = self.dev
+        self.host_bound = False
         n, n_buf = ids.numel(), off.numel() - 1
         counts = (off[1:] - off[:-1]).tolist()
         cap = B.batch_compress_bound(counts, W)
-        out = torch.empty(cap, dtype=torch.uint8, device=dev)
+        per_copy = 2 * n * (W // 8) + 1
+        copies = int(max(2, min(8, -(-(256 << 20) // per_copy))))
+        outs = [torch.empty(cap, dtype=torch.uint8, device=dev) for _ in range(copies)]
         out_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
         ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
         status = torch.zeros(1, dtype=torch.int32, device=dev)
-        back = torch.empty(max(n, 4), dtype=ids.dtype, device=dev)
+        backs = [torch.empty(max(n, 4), dtype=ids.dtype, device=dev) for _ in range(copies)]
         id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
-        pad = torch.empty(n + 4, dtype=ids.dtype, device=dev)
-        pad[:n] = ids
+        pads = []
+        for _ in range(copies):
+            pad = torch.empty(n + 4, dtype=ids.dtype, device=dev)
+            pad[:n] = ids
+            pads.append(pad)
         if single:                                           # one buffer: the single-buffer entry points
             nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
             n_out = torch.zeros(1, dtype=torch.int64, device=dev)
-            enc = self._time(lambda: B.compress(pad, n, W, thr, out, nbytes, ws, status))
-            dec = self._time(lambda: B.decompress(out, cap, W, back, n_out, ws, status))
+            enc, enc_iso = self._time([(lambda c=c: B.compress(pads[c], n, W, thr, outs[c], nbytes, ws, status)) for c in range(copies)])
+            dec, dec_iso = self._time([(lambda c=c: B.decompress(outs[c], cap, W, backs[c], n_out, ws, status)) for c in range(copies)])
             assert int(status.item()) == 0 and int(n_out.item()) == n
-            assert torch.equal(back[:n], ids), "decode != input"
+            assert torch.equal(backs[copies - 1][:n], ids), "decode != input"
             comp = int(nbytes.item())
-            return {"n": n, "n_buf": 1, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec}
-        enc = self._time(lambda: B.compress_batch(pad, off, n_buf, W, thr, out, out_off, ws, status))
-        dec = self._time(lambda: B.decompress_batch(out, out_off, n_buf, W, back, id_off, ws, status))
+            return {"n": n, "n_buf": 1, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec,
+                    "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound}
+        enc, enc_iso = self._time([(lambda c=c: B.compress_batch(pads[c], off, n_buf, W, thr, outs[c], out_off, ws, status)) for c in range(copies)])
+        dec, dec_iso = self._time([(lambda c=c: B.decompress_batch(outs[c], out_off, n_buf, W, backs[c], id_off, ws, status)) for c in range(copies)])
         assert int(status.item()) == 0
-        assert torch.equal(back[:n], ids) and torch.equal(id_off, off), "decode != input"
+        assert torch.equal(backs[copies - 1][:n], ids) and torch.equal(id_off, off), "decode != input"
         comp = int(out_off[-1].item())
-        return {"n": n, "n_buf": n_buf, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec}
+        return {"n": n, "n_buf": n_buf, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec,
+                "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound}
 
     def row(self, label, r):
         raw, comp = r["raw"], r["comp"]
@@ -89,13 +118,19 @@ class Runner:
         e, d = r["enc_ms"] * 1e-3, r["dec_ms"] * 1e-3
         ratio = raw / comp if comp else 0.0
         bits = 8.0 * comp / r["n"] if r["n"] else 0.0
+        if r.get("host_bound"):
+            label += " (*)"
         return (f"| {label} | {r['n_buf']} | {raw / 1e6:.3f} | {ratio:.2f} | {bits:.2f} | {r['enc_ms'] * 1e3:.1f} | "
                 f"{raw / e / 1e9:.1f} | {100 * alg / e / 1e9 / self.peak:.1f} | {r['dec_ms'] * 1e3:.1f} | "
-                f"{raw / d / 1e9:.1f} | {100 * alg / d / 1e9 / self.peak:.1f} |")
+                f"{raw / d / 1e9:.1f} | {100 * alg / d / 1e9 / self.peak:.1f} | {r['enc_iso_ms'] * 1e3:.1f} | {r['dec_iso_ms'] * 1e3:.1f} |")
 
 
-HDR = ("| case | buffers | raw MB | ratio | bits/ID | enc us | enc GB/s in | enc % peak | dec us | dec GB/s out | dec % peak |\n"
-       "|---|---|---|---|---|---|---|---|---|---|---|")
+HDR = ("enc us / dec us: per call, in a run of back-to-back calls on rotating copies of the buffers (working set >= 256 MB or 8 copies); "
+       "isolated: ONE call between two events after an L2 flush (launch latency and cold caches included); "
+       "(*) = the host needed as long to enqueue the run as the GPU to execute it (9-15 us per call from Python): "
+       "the back-to-back figure is then the host's\n\n"
+       "| case | buffers | raw MB | ratio | bits/ID | enc us | enc GB/s in | enc % peak | dec us | dec GB/s out | dec % peak | isolated enc us | isolated dec us |\n"
+       "|---|---|---|---|---|---|---|---|---|---|---|---|---|")
 
 
 def rmat_config(R, scale, seed, W, parts, n_roots, thr, per_level_roots=1):
@@ -105,13 +140,14 @@ def rmat_config(R, scale, seed, W, parts, n_roots, thr, per_level_roots=1):
           f"{parts} buffers per level by contiguous vertex range, {'u32' if W == 32 else 'u64'} IDs, threshold {thr} B\n")
     print(HDR)
     for ri, root in enumerate(G.roots(n_roots, seed=seed)):
-        tot = {"n": 0, "n_buf": parts, "raw": 0, "comp": 0, "enc_ms": 0.0, "dec_ms": 0.0}
+        tot = {"n": 0, "n_buf": parts, "raw": 0, "comp": 0, "enc_ms": 0.0, "dec_ms": 0.0, "enc_iso_ms": 0.0, "dec_iso_ms": 0.0}
         for level, f in enumerate(G.bfs_frontiers(root)):
             vals, off = streams.split_block(f, parts, 1 << scale)
             ids = streams.as_ids(vals, W).to(dev)
             r = R.batch(ids, off.to(dev), W, thr)
-            for k in ("n", "raw", "comp", "enc_ms", "dec_ms"):
+            for k in ("n", "raw", "comp", "enc_ms", "dec_ms", "enc_iso_ms", "dec_iso_ms"):
                 tot[k] += r[k]
+            tot["host_bound"] = tot.get("host_bound", False) or r["host_bound"]
             if ri < per_level_roots:
                 print(R.row(f"root {root} level {level} ({r['n']} IDs)", r))
         print(R.row(f"**root {root}, all levels** ({tot['n']} IDs)", tot))
@@ -128,7 +164,7 @@ def sweep(R):
             for mean in (1.0, 16.0, 4096.0):
                 label = f"u{W} {nbytes >> 10} KB mean {int(mean)}"
                 if W == 32 and n * mean >= 2 ** 32:
-                    print(f"| {label} | 1 | {nbytes / 1e6:.3f} | n/a | | | | | | | |")
+                    print(f"| {label} | 1 | {nbytes / 1e6:.3f} | n/a | | | | | | | | | |")
                     continue
                 ids = streams.gap_stream(n, mean, seed=5, W=W, device=dev)
                 off = torch.tensor([0, n], dtype=torch.int64, device=dev)

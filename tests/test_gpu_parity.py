@@ -149,6 +149,29 @@ def test_batch_ragged(B, oracle_mod, W):
     run_batch(B, oracle_mod, ids2, off2, W, 0)
 
 
+@pytest.mark.parametrize("W", [32, 64])
+def test_batch_alignments_and_many_buffers(B, oracle_mod, W):
+    """Buffers that start at every element alignment (decode writes aligned windows shifted through the
+    quad; encode stages unaligned chunks), blocks on the slow paths inside a batch, buffers that straddle
+    tiles, and more buffers than one round of the plan kernels' scan (4096)."""
+    g = torch.Generator().manual_seed(11)
+    counts = torch.tensor([128 * 70 + e for e in (0, 1, 2, 3, 5, 6, 7, 9)] + [257, 3, 0, 129, 8191, 64 * 128, 1, 127])
+    ids, off = streams.batch_of_streams(counts, 2.0, seed=9, W=W)
+    ids = ids.clone()
+    lo, hi = int(off[3]), int(off[4])                     # one buffer of incompressible values: blocks over the image cap
+    ids[lo:hi] = torch.randint(-(2 ** 31), 2 ** 31 - 1, (hi - lo,), generator=g, dtype=torch.int64).to(ids.dtype) if W == 32 \
+        else torch.randint(-(2 ** 62), 2 ** 62, (hi - lo,), generator=g, dtype=torch.int64)
+    lo, hi = int(off[5]), int(off[6])                     # outliers: exceptions in most blocks
+    sel = torch.rand(hi - lo, generator=g) < 0.02
+    ids[lo:hi][sel] += 1 << 20
+    for thr in (0, 1024):
+        run_batch(B, oracle_mod, ids, off, W, thr)
+    many = torch.randint(0, 300, (9000,), generator=g)
+    ids2, off2 = streams.batch_of_streams(many, 16.0, seed=10, W=W)
+    for thr in (0, 1024):
+        run_batch(B, oracle_mod, ids2, off2, W, thr)
+
+
 def test_tiny_rmat_config1(B, oracle_mod):
     """BASELINE config 1: scale 12, 8 roots, 4 buffers by v mod 4, threshold 0, single + batch API."""
     G = rmat.Graph(12, 16, seed=1)
