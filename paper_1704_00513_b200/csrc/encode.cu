@@ -300,7 +300,12 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     __shared__ volatile unsigned int s_sized;            // scan warp: tiles of this CTA whose sizes have arrived (the prep warp follows it)
     __shared__ unsigned int s_agg[4];                    // arrivals << 24 | sum of the worker warps' sizes (16-B units)
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // Roles by hardware warp: 0 = prep warp, 1..kEncWorkers = workers, kEncWorkers + 1 = scan warp. The schedulers
+    // favour the highest warp number among eligible warps: the scan warp (every later tile waits for its prefix)
+    // goes first, the prep warp (runs ahead, polls) last. `warp` below is the ROLE: workers 0..kEncWorkers-1,
+    // scan warp kEncWorkers, prep warp kEncWorkers + 1.
+    const int hw_warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = hw_warp == 0 ? kEncWorkers + 1 : hw_warp - 1;
     constexpr bool batch = kBatch;
     const T* ids = reinterpret_cast<const T*>(a.ids);
     pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
@@ -491,7 +496,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
         bool more = s_tile[1] != kNoTile;
         if (more) pdl_wait();                            // the ticket counter is set by the plan kernel
         for (int pt = 2; more; pt++) {
-            while ((int)s_sized + 1 < pt) __nanosleep(100);
+            while ((int)s_sized + 1 < pt) __nanosleep(400);   // (a tile period is 3-4 us: polling faster only takes issue slots)
             unsigned int ticket = 0;
             if (lane == 0) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
             ticket = __shfl_sync(kFull, ticket, 0);
