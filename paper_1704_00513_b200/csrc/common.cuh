@@ -234,6 +234,6 @@ static inline cudaError_t launch_dep(void (*kern)(A), int grid, int block, size_
 
 #define BFSC_LAUNCH_CHECK()                                        \
     do {                                                           \
-        ::bfsc::g_launches++;                                      \
+        __atomic_fetch_add(&::bfsc::g_launches, 1ull, __ATOMIC_RELAXED); /* calls may come from several host threads */ \
         if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; } \
     } while (0)
