@@ -269,6 +269,34 @@ def test_rmat_config4_reduced(B, oracle_mod):
             run_batch(B, oracle_mod, streams.as_ids(vals, 64), off, 64, 1024)
 
 
+def test_rmat_config3_full_size_one_root(B, oracle_mod):
+    """config 3 at its BASELINE size (R-MAT scale 22, 16 buffers per level, u32, 1 KB threshold), one root:
+    every level's batch byte-for-byte against the oracle (the graph and the BFS are built on the GPU by the
+    workload module; the codec calls are the ones report.py times)."""
+    G = rmat.Graph(22, 16, seed=3, device=torch.device("cuda"))
+    root = G.roots(1, seed=3)[0]
+    total = 0
+    for f in G.bfs_frontiers(root):
+        vals, off = streams.split_block(f, 16, 1 << 22)
+        run_batch(B, oracle_mod, streams.as_ids(vals, 32).cpu(), off.cpu(), 32, 1024)
+        total += vals.numel()
+    assert total > 2_000_000                                  # the giant component
+
+
+def test_rmat_config4_full_size_one_root(B, oracle_mod):
+    """config 4 at its BASELINE size (R-MAT scale 25, 64 buffers per level, u64, 1 KB threshold), one root."""
+    G = rmat.Graph(25, 16, seed=4, device=torch.device("cuda"))
+    root = G.roots(1, seed=4)[0]
+    total = 0
+    for f in G.bfs_frontiers(root):
+        vals, off = streams.split_block(f, 64, 1 << 25)
+        run_batch(B, oracle_mod, streams.as_ids(vals, 64).cpu(), off.cpu(), 64, 1024)
+        total += vals.numel()
+    del G
+    torch.cuda.empty_cache()
+    assert total > 16_000_000
+
+
 @pytest.mark.parametrize("W", [32, 64])
 def test_sweep_config5_reduced(B, oracle_mod, W):
     """config 5 recipe: single buffers of 1 KB .. 4 MB (powers of 4), gap means 1, 16, 4096; plus a batch
