@@ -315,41 +315,60 @@ def test_sweep_config5_reduced(B, oracle_mod, W):
             run_batch(B, oracle_mod, ids, off, W, thr)
 
 
-def test_config2_full_size_sampled(B, oracle_mod):
-    """BASELINE config 2 at its full size (2^24 IDs, the launch configuration bench.py times): decoded IDs
-    equal the input everywhere; directory walk (strictly increasing, sizes recomputed from the block
-    headers, total = header + directory + blocks); 256 sampled blocks per stream memcmp-equal to the
-    oracle's encoding of the same 128 IDs (blocks are independent: FORMAT.md §2)."""
+def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256):
+    """One large single stream through bfsc_compress / bfsc_decompress: decoded IDs equal the input everywhere;
+    directory walk (strictly increasing, sizes recomputed from the block headers, total = header + directory +
+    blocks); `samples` blocks memcmp-equal to the oracle's encoding of the same 128 IDs (blocks are
+    independent: FORMAT.md §2)."""
     dev = torch.device("cuda")
-    n, W = 1 << 24, 32
+    n = ids.numel()
+    E = W // 8
+    cap = B.compress_bound(n, W)
+    out = torch.empty(cap, dtype=torch.uint8, device=dev)
+    nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress(ids, n, W, 0, out, nbytes, ws, status)
+    back = torch.empty(n, dtype=ids.dtype, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+    B.decompress(out, cap, W, back, n_out, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and int(n_out.item()) == n
+    assert torch.equal(back, ids)
+    del back
+    total = int(nbytes.item())
+    s = out[:total].cpu().numpy()
+    nb = (n + 127) // 128
+    assert s[:4].tobytes() == b"BFSC" and s[4] == 1 and s[5] == W and s[6] == 1
+    assert int(s[8:16].view(np.uint64)[0]) == n and int(s[16:24].view(np.uint64)[0]) == total
+    assert int(s[24:28].view(np.uint32)[0]) == nb
+    d = s[32:32 + 4 * (nb + 1)].view(np.uint32).astype(np.int64)
+    assert d[0] * 16 == 32 + ((4 * (nb + 1) + 15) // 16) * 16 and d[nb] * 16 == total
+    b = s[d[:-1] * 16 + 8].astype(np.int64)
+    ne = s[d[:-1] * 16 + 9].astype(np.int64)
+    exc = np.where(ne > 0, ((((ne + E - 1) // E) * E + E * ne + 15) // 16) * 16, 0)
+    assert np.array_equal((d[1:] - d[:-1]) * 16, 16 + 16 * b + exc)
+    host = ids.cpu().numpy().view(np.uint32 if W == 32 else np.uint64)
+    for k in rng.integers(0, nb, size=samples):
+        ref = oracle_mod.compress(host[128 * k:128 * k + 128], 0)
+        assert np.array_equal(s[d[k] * 16:d[k + 1] * 16], ref[48:]), f"block {k} differs from the oracle"
+
+
+def test_config2_full_size_sampled(B, oracle_mod):
+    """BASELINE config 2 at its full size (2^24 IDs, the launch configuration bench.py times)."""
     rng = np.random.default_rng(7)
     for sub, (mean, outl) in enumerate(((2.0, 0.0), (256.0, 0.0), (256.0, 0.01))):
-        ids = streams.gap_stream(n, mean, seed=2, W=W, outlier_frac=outl, sub=sub, device=dev)
-        cap = B.compress_bound(n, W)
-        out = torch.empty(cap, dtype=torch.uint8, device=dev)
-        nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
-        ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
-        status = torch.zeros(1, dtype=torch.int32, device=dev)
-        B.compress(ids, n, W, 0, out, nbytes, ws, status)
-        back = torch.empty(n, dtype=ids.dtype, device=dev)
-        n_out = torch.zeros(1, dtype=torch.int64, device=dev)
-        B.decompress(out, cap, W, back, n_out, ws, status)
-        torch.cuda.synchronize()
-        assert int(status.item()) == 0 and int(n_out.item()) == n
-        assert torch.equal(back, ids)
-        total = int(nbytes.item())
-        s = out[:total].cpu().numpy()
-        nb = n // 128
-        assert s[:4].tobytes() == b"BFSC" and s[4] == 1 and s[5] == W and s[6] == 1
-        assert int(s[8:16].view(np.uint64)[0]) == n and int(s[16:24].view(np.uint64)[0]) == total
-        assert int(s[24:28].view(np.uint32)[0]) == nb
-        d = s[32:32 + 4 * (nb + 1)].view(np.uint32).astype(np.int64)
-        assert d[0] * 16 == 32 + ((4 * (nb + 1) + 15) // 16) * 16 and d[nb] * 16 == total
-        b = s[d[:-1] * 16 + 8].astype(np.int64)
-        ne = s[d[:-1] * 16 + 9].astype(np.int64)
-        exc = np.where(ne > 0, ((((ne + 3) // 4) * 4 + 4 * ne + 15) // 16) * 16, 0)
-        assert np.array_equal((d[1:] - d[:-1]) * 16, 16 + 16 * b + exc)
-        host = ids.cpu().numpy().view(np.uint32)
-        for k in rng.integers(0, nb, size=256):
-            ref = oracle_mod.compress(host[128 * k:128 * k + 128], 0)
-            assert np.array_equal(s[d[k] * 16:d[k + 1] * 16], ref[48:]), f"block {k} differs from the oracle"
+        ids = streams.gap_stream(1 << 24, mean, seed=2, W=32, outlier_frac=outl, sub=sub, device=torch.device("cuda"))
+        _full_size_sampled(B, oracle_mod, ids, 32, rng)
+
+
+def test_config5_largest_buffers_sampled(B, oracle_mod):
+    """The 1 GB ends of the config-5 sweep (2^28 u32 IDs with gaps of 1; 2^27 u64 IDs with gaps of mean 4096):
+    tile counts, offsets and directory entries far beyond the 2^24-ID case (1 GB streams: offsets over 2^32 / 16
+    are still exact)."""
+    rng = np.random.default_rng(8)
+    dev = torch.device("cuda")
+    _full_size_sampled(B, oracle_mod, streams.gap_stream(1 << 28, 1.0, seed=5, W=32, device=dev), 32, rng, samples=64)
+    torch.cuda.empty_cache()
+    _full_size_sampled(B, oracle_mod, streams.gap_stream(1 << 27, 4096.0, seed=5, W=64, device=dev), 64, rng, samples=64)
+    torch.cuda.empty_cache()
