@@ -95,6 +95,22 @@ def np_view(t):
     return t.cpu().numpy().view(np.uint32 if W == 32 else np.uint64)
 
 
+def max_over_ranks(x: float, world: int, device) -> float:
+    """Replicas only: the job's time is the slowest rank's. MAX all-reduce over whatever backend
+    the process group was initialised with (nccl on GPUs; gloo in the CPU test of this function)."""
+    if world <= 1:
+        return float(x)
+    import torch.distributed as dist
+    tt = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(per_rank_units: float, world: int, seconds: float) -> float:
+    """value = units all ranks processed / max-over-ranks time (weak scaling: every rank does the same work)."""
+    return world * per_rank_units / seconds
+
+
 # --------------------------------------------------------------------------- oracle arm
 def time_oracle(host_ids, threads, reps=1):
     """oracle encode+decode of every stream; returns (seconds, raw_bytes_processed, ratio)."""
@@ -122,12 +138,12 @@ def run_reference(args, rank, world):
         return
     cores = len(os.sched_getaffinity(0))
     # Bounded sample: the first 2^p IDs of each stream, p chosen from a quick calibration so that the whole
-    # --steps K run takes about 90 s of CPU work (p in 14..22).
+    # --steps K run takes about --ref-budget-s (default 90) seconds of CPU work (p in 14..22).
     full = [np_view(t) for t in make_streams("cpu", 1 << 22)]
     time_oracle([h[:1 << 16] for h in full], cores)                       # warm-up (builds the oracle's C library)
     cal, _, _ = time_oracle([h[:1 << 18] for h in full], cores)
     per_id = cal / (3 << 18)
-    budget = 90.0 / max(args.steps, 1)
+    budget = args.ref_budget_s / max(args.steps, 1)
     p = 22
     while p > 14 and per_id * (3 << p) > budget:
         p -= 1
@@ -214,10 +230,7 @@ def run_ours(args, rank, local_rank, world):
     clocks = sampler.stop()
     launches_timed = B.kernel_launches() - launches0
     ms_total = t0.elapsed_time(t1)
-    if world > 1:
-        tt = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
     # ---- per-call durations (roofline): CUDA events around a run of back-to-back launches of ONE call on
     # kCopies distinct copies of the stream (inputs and outputs rotate: > 250 MB of other traffic between a
@@ -254,7 +267,7 @@ def run_ours(args, rank, local_rank, world):
         dec_ms.append(d0.elapsed_time(d1) / (reps * kCopies))
         del c_ids
     assert int(status.item()) == 0, f"device status {int(status.item())}"
-    value = world * (2 * S * raw_bytes) / (ms_step * 1e-3) / 1e9
+    value = whole_job_value(2 * S * raw_bytes, world, ms_step * 1e-3) / 1e9
 
     # ---- end to end through the host-buffer C-ABI calls (pinned host memory) ----
     e2e = None
@@ -314,12 +327,9 @@ def run_ours(args, rank, local_rank, world):
             e2e_step()
         torch.cuda.synchronize()
         e_ms = 1e3 * (time.perf_counter() - w0) / e_steps
-        if world > 1:
-            tt = torch.tensor([e_ms], device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e_ms = float(tt.item())
+        e_ms = max_over_ranks(e_ms, world, dev)
         assert torch.equal(h_back, h_ids[S - 1])
-        e2e = {"value": world * (2 * S * raw_bytes) / (e_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": e_ms,
+        e2e = {"value": whole_job_value(2 * S * raw_bytes, world, e_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": e_ms,
                "h2d_bytes_per_step": S * raw_bytes + sum(comp), "d2h_bytes_per_step": sum(comp) + S * raw_bytes + 32 * S,
                "api": "bfsc_compress_host + bfsc_decompress_host, pinned host buffers; compress calls and decompress calls "
                       "from two host threads on two streams (stream s is decompressed as soon as its compress call returned)"}
@@ -353,7 +363,10 @@ def run_ours(args, rank, local_rank, world):
         m = 1 << min(args.log2n, 22)
         host = [np_view(t[:m]) for t in ids]
         dt, raw, _ = time_oracle(host, cores)
+        m1 = 1 << min(args.log2n, 20)
+        dt1, raw1, _ = time_oracle([np_view(t[:m1]) for t in ids], 1)
         cpu = {"value": raw / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "single_thread": {"value": raw1 / dt1 / 1e9, "unit": UNIT, "sample": f"first 2^{min(args.log2n, 20)} IDs of each stream"},
                "sample": f"first 2^{min(args.log2n, 22)} IDs of each of the 3 streams, encode+decode, {cores} threads, 1 pass"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -380,6 +393,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=LOG2_N, help="IDs per stream = 2^log2n (default: the BASELINE size)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for the whole run")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
