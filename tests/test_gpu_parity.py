@@ -315,6 +315,35 @@ def test_sweep_config5_reduced(B, oracle_mod, W):
             run_batch(B, oracle_mod, ids, off, W, thr)
 
 
+def test_random_batches_soak(B, oracle_mod):
+    """Seeded random batches (buffer counts 1..6000, sizes 0..3 M IDs, u32/u64, gaps of mean 1..70000, optional
+    outliers, both thresholds) byte-for-byte against the oracle: shakes the hand-overs between the warps of the
+    encoder (tickets, look-back, deferred copy-out) and the plan / block-table kernels under varied timing."""
+    g = torch.Generator().manual_seed(20261104)
+    for _ in range(150):
+        W = 32 if torch.rand(1, generator=g) < 0.6 else 64
+        kind = int(torch.randint(0, 4, (1,), generator=g))
+        if kind == 0:
+            nbuf, hi = int(torch.randint(1, 40, (1,), generator=g)), 200000
+        elif kind == 1:
+            nbuf, hi = int(torch.randint(1000, 6000, (1,), generator=g)), 400
+        elif kind == 2:
+            nbuf, hi = int(torch.randint(1, 300, (1,), generator=g)), 20000
+        else:
+            nbuf, hi = 1, 3000000
+        counts = torch.randint(0, hi, (nbuf,), generator=g)
+        mean = [1.0, 2.0, 16.0, 256.0, 4096.0, 70000.0][int(torch.randint(0, 6, (1,), generator=g))]
+        ids, off = streams.batch_of_streams(counts, mean, seed=int(torch.randint(0, 1 << 30, (1,), generator=g)), W=W)
+        if torch.rand(1, generator=g) < 0.3 and ids.numel() > 10:
+            sel = torch.rand(ids.numel(), generator=g) < 0.01
+            ids = ids.clone()
+            ids[sel] += 1 << 22
+        thr = [0, 1024][int(torch.randint(0, 2, (1,), generator=g))]
+        run_batch(B, oracle_mod, ids, off, W, thr)
+        if nbuf == 1:
+            run_single(B, oracle_mod, ids, W, thr)
+
+
 def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256):
     """One large single stream through bfsc_compress / bfsc_decompress: decoded IDs equal the input everywhere;
     directory walk (strictly increasing, sizes recomputed from the block headers, total = header + directory +
