@@ -309,6 +309,17 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     constexpr bool batch = kBatch;
     const T* ids = reinterpret_cast<const T*>(a.ids);
     pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
+    if constexpr (!kBatch) {
+        // Single-buffer calls: a worker's share of the CTA's first tile (tile blockIdx.x) follows from the
+        // arguments: its loads go out before anything else in the kernel (barriers, mbarrier set-up, plan).
+        if (warp < kEncWorkers) {
+            const unsigned long long g = (unsigned long long)blockIdx.x * kTileR + warp * kQuadBlocks + (lane >> 2);
+            const unsigned long long nb0 = (a.n_single + kBlk - 1) / kBlk;
+            if (g < nb0)
+                quad_prefetch<W>(dyn_smem + warp * EncSmem<W>::kWarpChunks + raw_slot_chunk<W>(lane >> 2), ids + kBlk * g,
+                                 (int)min((unsigned long long)kBlk, a.n_single - kBlk * g));
+        }
+    }
     if (threadIdx.x < 4) s_agg[threadIdx.x] = 0;
     if (threadIdx.x == 4) s_sized = 0;
     if (threadIdx.x < kRing) mbar_init(&mb_post[threadIdx.x], 1);
@@ -517,7 +528,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
     constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
     __syncthreads();                                                     // barrier 0: the first two tiles are posted
     bool have = s_tile[0] != kNoTile;
-    if (have) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));
+    if constexpr (kBatch) { if (have) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j)); }   // (single: see the top)
     static_assert(kDefer == 1 || kDefer == 2, "hist selection below");
     uint32_t key_hist[kDefer] = {}, woff_hist[kDefer] = {};              // keys and image places of the tiles that wait in shared memory
     int kp = 0;                                                          // k % kNB
