@@ -255,16 +255,21 @@ __device__ __forceinline__ unsigned long long lookback(const unsigned long long*
     return acc;
 }
 
-constexpr int kImgCap = 320;                                  // bytes of a block image the fast path can hold (b = 16 + exceptions)
-constexpr int kImgSlotChunks = 21;                            // slot stride (16-B chunks): 21 q mod 8 are all distinct
-constexpr int kImgBufChunks = kQuadBlocks * kImgSlotChunks;   // one image buffer of a warp
+// Image buffer of a warp: room for 8 block images of at most kCap bytes, back to back. u32: 320 B (b = 16 with
+// exceptions, b = 19 without); u64: 288 B, so that two CTAs of the batch instantiation (1 KB blocks staged, 10 KB
+// of bookkeeping) still fit one SM.
+template <int W> struct ImgCfg {
+    static constexpr int kSlotChunks = (W == 32) ? 21 : 18;   // 16-byte chunks per block
+    static constexpr int kCap = (W == 32) ? 320 : 288;        // bytes of a block image the fast path can hold
+    static constexpr int kBufChunks = kQuadBlocks * kSlotChunks;
+};
 
 constexpr int kDefer = 1;                                     // a tile's images leave kDefer tiles after they were packed (1 or 2)
 constexpr int kNB = kDefer + 1;                               // image buffers / size and offset tables per CTA
 
 template <int W> struct EncSmem {
     static constexpr int kStageChunks = RawCfg<W>::kAreaChunks;              // per worker warp: staged raw IDs
-    static constexpr int kWarpChunks = kStageChunks + kNB * kImgBufChunks;   // + the image buffers
+    static constexpr int kWarpChunks = kStageChunks + kNB * ImgCfg<W>::kBufChunks;   // + the image buffers
     static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
 };
 
@@ -540,7 +545,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             const int m = blk_m(k & (kRing - 1), j);
             const T* raw = reinterpret_cast<const T*>(slot) +
                            (reinterpret_cast<uintptr_t>(ids + blk_xoff(k & (kRing - 1), j)) & 15) / sizeof(T);
-            unsigned char* ib = ibuf + kp * (kImgBufChunks * 16);        // this tile's image buffer
+            unsigned char* ib = ibuf + kp * (ImgCfg<W>::kBufChunks * 16);        // this tile's image buffer
             if (warp == 0) TR(s_tile[k & (kRing - 1)], 6);
             cp_async_wait_all();
             if (lane == 0) bulk_wait_read();                             // the bulk store that read this image buffer is done with it
@@ -558,7 +563,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
 #else
             if (!wide) key = quad_choose_b<W>(d);                        // E2
 #endif
-            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (kImgSlotChunks * 16)));
+            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (ImgCfg<W>::kSlotChunks * 16)));
             if (m <= 0) key = 0;
             if (l == 0) s_key[kp][j] = key;
             {   // The tile's aggregate goes out as soon as the LAST worker warp has its sizes — not when the scan
@@ -581,7 +586,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             bar_arrive(kBarSizes + kp, kSizesThreads);
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
-            const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)kImgCap);   // slow path, in global memory later
+            const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)ImgCfg<W>::kCap);   // slow path, in global memory later
             const bool fast = !wide && key != 0 && !late;
             // The warp's 8 images lie back to back in the buffer, as they do in the output (consecutive blocks):
             // woff = exclusive scan of the fast blocks' sizes over the quads, in 16-byte chunks.
@@ -635,7 +640,7 @@ __global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
             }
             // images -> their final place. Usual case: the warp's blocks are consecutive in the output as well
             // (same stream, none late, all fit): ONE bulk store of the whole buffer by lane 0.
-            const unsigned char* ib_e = ibuf + kpe * (kImgBufChunks * 16);
+            const unsigned char* ib_e = ibuf + kpe * (ImgCfg<W>::kBufChunks * 16);
             const bool valid = key_e != 0, fast_e = valid && (key_e & kLateBit) == 0;
             const uint32_t z_e = fast_e ? key_e >> 18 : 0u;
             const unsigned long long at_n = __shfl_down_sync(kFull, at, 4);
