@@ -47,7 +47,10 @@ struct WsView {
 };
 
 constexpr int kTileBlocks = 64;         // blocks per encode tile (8 worker warps x 8 blocks)
-constexpr int kStateStride = 8;         // u64 words between look-back states (64 B)
+#ifndef BFSC_STATE_STRIDE
+#define BFSC_STATE_STRIDE 8
+#endif
+constexpr int kStateStride = BFSC_STATE_STRIDE;         // u64 words between look-back states (64 B)
 constexpr size_t kTileWsBytes = 8 * kStateStride + 32 * kTileBlocks;   // workspace per tile: state + block table
 
 // Block table entries (batch calls). Encode: where the block's IDs are. Decode: where its stream is, which

@@ -213,41 +213,59 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 __device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// Exclusive prefix (16-byte units) of tile t > 0: aggregates of t-1, t-2, ... down to the nearest
-// tile whose inclusive prefix is known. One warp. The states of the 256 nearest predecessors are
-// fetched up front (8 independent loads per lane: ONE L2 round trip), then examined 32 at a time
-// with two ballots per chunk; every lane sums its own entries and a single warp reduction ends it.
-// A chunk with an entry that is not posted yet is polled alone (a few instructions per poll).
-constexpr int kLookChunks = 8;
+// Decoupled look-back (one warp): the exclusive prefix of tile t > 0 = aggregates of t-1, t-2, ... down to the
+// nearest tile whose inclusive prefix is known. Every lane sums its own entries, a single warp reduction ends it.
+#ifndef BFSC_LOOK_CHUNKS
+#define BFSC_LOOK_CHUNKS 1
+#endif
+constexpr int kLookChunks = BFSC_LOOK_CHUNKS;
+#ifndef BFSC_LOOK_SLEEP
+#define BFSC_LOOK_SLEEP 32
+#endif
+constexpr unsigned kLookSleepNs = BFSC_LOOK_SLEEP;   // back-off between polls of a look-back that has to wait
+// One round of the look-back: the states of the 32 * N predecessors below idx0 (lane i: idx0 - i, - 32, ...) are
+// requested at once, then examined 32 at a time with two ballots; an entry that is not posted yet is polled alone.
+template <int N>
+__device__ __forceinline__ bool lookback_round(const unsigned long long* __restrict__ state, long long idx, int lane,
+                                               unsigned long long& acc) {
+    unsigned long long s[N];
+    bool done = false;
+#pragma unroll
+    for (int r = 0; r < N; r++)
+        s[r] = (idx - 32 * r >= 0) ? ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]) : kFlagPre;
+#pragma unroll
+    for (int r = 0; r < N; r++) {
+        if (!done) {
+            unsigned long long v = s[r];
+            while (true) {
+                const uint32_t hit = __ballot_sync(kFull, (v >> 62) == 2);
+                const uint32_t rdy = __ballot_sync(kFull, (v >> 62) != 0);
+                const int stop = hit ? __ffs(hit) - 1 : 31;
+                const uint32_t need = 0xffffffffu >> (31 - stop);
+                if ((rdy & need) == need) {
+                    if (lane <= stop) acc += v & kValMask;
+                    done = hit != 0;
+                    break;
+                }
+                __nanosleep(kLookSleepNs);
+                if ((v >> 62) == 0) v = ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]);
+            }
+        }
+    }
+    return done;
+}
+
+// Exclusive prefix (16-byte units) of tile t > 0: rounds of kLookChunks x 32 predecessor states. One chunk per
+// round is the measured optimum (swept 1..24, also with a larger window after the first round, and 4..32
+// lanes in the first round): the nearest tile with a known inclusive prefix is usually a few tiles back, and every
+// speculative load of a state that other SMs are about to write slows the call (8 chunks: + 1.3 us per call).
 __device__ __forceinline__ unsigned long long lookback(const unsigned long long* __restrict__ state,
                                                        unsigned long long t, int lane) {
     unsigned long long acc = 0;
     long long idx = (long long)t - 1 - lane;
     bool done = false;
     while (!done) {
-        unsigned long long s[kLookChunks];
-#pragma unroll
-        for (int r = 0; r < kLookChunks; r++)
-            s[r] = (idx - 32 * r >= 0) ? ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]) : kFlagPre;
-#pragma unroll
-        for (int r = 0; r < kLookChunks; r++) {
-            if (!done) {
-                unsigned long long v = s[r];
-                while (true) {
-                    const uint32_t hit = __ballot_sync(kFull, (v >> 62) == 2);
-                    const uint32_t rdy = __ballot_sync(kFull, (v >> 62) != 0);
-                    const int stop = hit ? __ffs(hit) - 1 : 31;
-                    const uint32_t need = 0xffffffffu >> (31 - stop);
-                    if ((rdy & need) == need) {
-                        if (lane <= stop) acc += v & kValMask;
-                        done = hit != 0;
-                        break;
-                    }
-                    __nanosleep(32);
-                    if ((v >> 62) == 0) v = ld_volatile_u64(&state[(idx - 32 * r) * kStateStride]);
-                }
-            }
-        }
+        done = lookback_round<kLookChunks>(state, idx, lane, acc);
         idx -= 32 * kLookChunks;
     }
 #pragma unroll
@@ -264,7 +282,10 @@ template <int W> struct ImgCfg {
     static constexpr int kBufChunks = kQuadBlocks * kSlotChunks;
 };
 
-constexpr int kDefer = 1;                                     // a tile's images leave kDefer tiles after they were packed (1 or 2)
+#ifndef BFSC_DEFER
+#define BFSC_DEFER 1
+#endif
+constexpr int kDefer = BFSC_DEFER;                                     // a tile's images leave kDefer tiles after they were packed (1 or 2)
 constexpr int kNB = kDefer + 1;                               // image buffers / size and offset tables per CTA
 
 template <int W> struct EncSmem {
