@@ -36,6 +36,7 @@ constexpr int kTileR = kEncWorkers * kQuadBlocks;        // 64 blocks per tile
 static_assert(kTileR >= kTileBlocks, "workspace sizing assumes tiles of at least kTileBlocks blocks");
 constexpr int kPer = (kTileR + 31) / 32;                 // blocks per lane of the scan warp
 constexpr int kEncThreads = (kEncWorkers + 2) * 32;      // + the scan warp + the prep warp
+constexpr int kEncCtasPerSm = (kEncWorkers >= 16) ? 1 : 2;
 constexpr int kSizesThreads = (kEncWorkers + 1) * 32;    // threads on the "sizes posted" barrier: workers + scan warp
 
 // ---- E0: plan. One CTA; per buffer: mode, block count, fixed bytes; exclusive prefixes. ----
@@ -309,7 +310,7 @@ constexpr int kRing = 8;                                      // ring of tile bo
 // Tiles: the first two of a CTA are blockIdx.x and blockIdx.x + gridDim.x, the rest come from the ticket
 // counter, each drawn at the same point of the pipeline: a lower tile number means "sizes posted earlier".
 template <int W, bool kBatch>
-__global__ void __launch_bounds__(kEncThreads, 2) k_enc_tiles(EncArgs a) {
+__global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
     extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | kNB image buffers
     __shared__ uint32_t s_key[kNB][kTileR];              // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
