@@ -177,11 +177,11 @@ constexpr unsigned long long kNoTile = ~0ull, kSkip = ~0ull;
 
 __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
     unsigned long long v;
-    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");   // gpu scope: the writers are CTAs of this grid
     return v;
 }
 __device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned long long v) {
-    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 // mbarrier (shared memory, CTA scope): one-directional "posted" signals between warps of a CTA
 __device__ __forceinline__ void mbar_init(unsigned long long* b, uint32_t count) {
