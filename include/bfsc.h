@@ -17,9 +17,14 @@
  *    The library allocates nothing, frees nothing and never synchronises (except the *_host
  *    convenience calls, which synchronise `cuda_stream` before returning).
  *  - Every call enqueues its kernels on `cuda_stream` (a cudaStream_t passed as void*;
- *    NULL = the legacy default stream) and returns immediately.
+ *    NULL = the legacy default stream) and returns immediately. Stream order holds for
+ *    everything a call reads or writes. The kernels are launched with programmatic dependent
+ *    launch: a kernel may become resident while its predecessor in the stream still runs, but
+ *    waits for that predecessor to complete before it touches memory (back-to-back calls pay
+ *    no launch gap).
  *  - d_ids / d_out / d_in must be 16-byte aligned; element offsets inside a batch may be
- *    arbitrary (unaligned buffers take a scalar load/store path).
+ *    arbitrary (buffers that start off a 16-byte boundary are staged / written through
+ *    aligned 16-byte chunks all the same).
  *  - IDs are little-endian unsigned integers of W = 32 or 64 bits (bfsc_dtype).
  *  - Return value: host-detectable errors only (null / misaligned pointer, bad dtype,
  *    workspace too small, launch failure -> BFSC_ERR_CUDA).
@@ -32,8 +37,10 @@
  *    access occurs. d_status may be NULL (errors are then dropped).
  *  - raw_threshold_bytes: a buffer is sent RAW iff n*W/8 < raw_threshold_bytes
  *    (FORMAT.md §1); 0 = always compress.
- *  - Workspace: bfsc_workspace_bytes(n_ids_total, n_buf, t) bytes, 16-byte aligned, any
- *    content on entry, clobbered by the call; one workspace per in-flight call.
+ *  - Workspace: bfsc_workspace_bytes(n_ids_total, n_buf, t) bytes (about 33 bytes per 128 IDs
+ *    + 24 per buffer: scan states and, for batch calls, a table of where every block lives),
+ *    16-byte aligned, any content on entry, clobbered by the call; one workspace per in-flight
+ *    call (calls on the same stream may share one).
  *  - Compressed output is canonical: byte-identical to the scalar oracle (oracle/), pads
  *    included. The decoder accepts any well-formed stream.
  */
