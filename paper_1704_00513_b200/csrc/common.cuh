@@ -115,19 +115,8 @@ __device__ __forceinline__ uint32_t exc_bytes(uint32_t n) {
     return n ? ((a + 15u) & ~15u) : 0u;
 }
 
-// first index i in [0, n_buf] with a[i] > g, minus 1  (buffers without blocks are skipped)
-__device__ __forceinline__ uint32_t find_buf(const unsigned long long* __restrict__ a, uint32_t n_buf,
-                                             unsigned long long g) {
-    uint32_t lo = 0, hi = n_buf;        // invariant: a[lo] <= g < a[hi]  (a[0] = 0, a[n_buf] = total > g)
-    while (hi - lo > 1) {
-        uint32_t mid = (lo + hi) >> 1;
-        if (a[mid] <= g) lo = mid; else hi = mid;
-    }
-    return lo;
-}
-
-// Same result as find_buf, starting from a hint lo with a[lo] <= g (the buffer of an earlier block): gallop,
-// then bisect. Consecutive blocks live in nearby buffers, so this touches one or two cache lines.
+// Buffer of global block g: the last i with a[i] <= g (buffers without blocks are skipped), searched from a
+// hint lo with a[lo] <= g (the buffer of an earlier block): gallop, then bisect. Consecutive blocks live in nearby buffers, so this touches one or two cache lines.
 __device__ __forceinline__ uint32_t find_buf_from(const unsigned long long* __restrict__ a, uint32_t n_buf,
                                                   unsigned long long g, uint32_t lo) {
     uint32_t hi, step = 1;

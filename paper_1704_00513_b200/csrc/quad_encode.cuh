@@ -3,92 +3,17 @@
 // of the quad. Per-block scalar work (sizes, offsets, headers) then costs 1/8 of a warp
 // instruction per block instead of a whole one, and nothing needs a full-warp reduction.
 //
-// Two ownerships of a block's 128 values (j = 4r + c, row r = 0..31, column c = 0..3):
-//   row owner   : lane l holds rows r = 4i + l, i = 0..7 (v[i][c] = x[16i + 4l + c]): the quad
-//                 reads 64 contiguous bytes per load instruction (128-bit loads, coalesced);
-//   column owner: lane c packs column c's bit stream (FORMAT.md payload) sequentially from the
-//                 staged values in shared memory.
+// Ownership of a block's 128 values (j = 4r + c, row r = 0..31, column c = 0..3): lane c of the quad is the
+// COLUMN OWNER of column c. The raw IDs are staged in shared memory by cp.async; lane c forms the 32 deltas of
+// its column there (E1), counts widths (E2) and packs the column's bit stream (E4, FORMAT.md payload)
+// sequentially from registers — the values never change hands between E1 and E4.
 #pragma once
 #include "common.cuh"
 
 namespace bfsc {
 
 constexpr int kQuadBlocks = 8;                       // blocks per warp batch
-constexpr int kValStride = 132;                      // words between blocks' staged rows (== 4 mod 32: conflict-free column reads)
-
-__device__ __forceinline__ int quad_q() { return (threadIdx.x & 31) >> 2; }
 __device__ __forceinline__ int quad_l() { return threadIdx.x & 3; }
-
-template <typename DT> __device__ __forceinline__ int bitlen(DT v);
-template <> __device__ __forceinline__ int bitlen<uint32_t>(uint32_t v) { return 32 - __clz(v); }
-template <> __device__ __forceinline__ int bitlen<uint64_t>(uint64_t v) { return 64 - __clzll(v); }
-
-template <typename DT> __device__ __forceinline__ DT shr_clamp(DT v, uint32_t s);
-template <> __device__ __forceinline__ uint32_t shr_clamp<uint32_t>(uint32_t v, uint32_t s) { return shr32(v, s); }
-template <> __device__ __forceinline__ uint64_t shr_clamp<uint64_t>(uint64_t v, uint32_t s) { return shr64(v, s); }
-
-// ---- E1: row-owner load of the quad's block. x = block's first ID, m = valid IDs (0..128).
-template <int W>
-__device__ __forceinline__ void quad_load(const typename IdT<W>::T* __restrict__ x, int m, bool keep_in_l2,
-                                          typename IdT<W>::T (&v)[8][4]) {
-    using T = typename IdT<W>::T;
-    const int l = quad_l();
-    const bool fast = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
-    if (__all_sync(kFull, fast)) {
-        if constexpr (W == 32) {
-            const uint4* p = reinterpret_cast<const uint4*>(x) + l;
-#pragma unroll
-            for (int i = 0; i < 8; i++) {
-                const uint4 t = keep_in_l2 ? __ldg(p + 4 * i) : __ldcs(p + 4 * i);
-                v[i][0] = t.x; v[i][1] = t.y; v[i][2] = t.z; v[i][3] = t.w;
-            }
-        } else {
-            const ulonglong2* p = reinterpret_cast<const ulonglong2*>(x) + 2 * l;
-#pragma unroll
-            for (int i = 0; i < 8; i++) {
-                const ulonglong2 t0 = keep_in_l2 ? __ldg(p + 8 * i) : __ldcs(p + 8 * i);
-                const ulonglong2 t1 = keep_in_l2 ? __ldg(p + 8 * i + 1) : __ldcs(p + 8 * i + 1);
-                v[i][0] = t0.x; v[i][1] = t0.y; v[i][2] = t1.x; v[i][3] = t1.y;
-            }
-        }
-    } else {                                         // ragged / unaligned / missing blocks: guarded scalar loads
-#pragma unroll
-        for (int i = 0; i < 8; i++)
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-                const int j = 16 * i + 4 * l + c;
-                v[i][c] = (j < m) ? x[j] : (T)0;
-            }
-    }
-}
-
-// ---- E1: deltas, d_0 = 0, zero beyond m. One shuffle per row step:
-// a lane needs the last ID of the previous row, which lives in lane-1 (same step) or, for l = 0,
-// in lane+3 (previous step) — lane l = 3 publishes its previous step's value for that purpose.
-template <int W>
-__device__ __forceinline__ void quad_deltas(const typename IdT<W>::T (&v)[8][4], int m,
-                                            typename IdT<W>::T (&d)[8][4]) {
-    using T = typename IdT<W>::T;
-    const int lane = threadIdx.x & 31, l = lane & 3;
-    const int src = (l == 0) ? lane + 3 : lane - 1;
-#pragma unroll
-    for (int i = 0; i < 8; i++) {
-        const T pub = (l == 3 && i > 0) ? v[i - 1][3] : v[i][3];
-        T prev = __shfl_sync(kFull, pub, src);
-        if (i == 0 && l == 0) prev = v[0][0];
-        d[i][0] = v[i][0] - prev;
-        d[i][1] = v[i][1] - v[i][0];
-        d[i][2] = v[i][2] - v[i][1];
-        d[i][3] = v[i][3] - v[i][2];
-    }
-    if (!__all_sync(kFull, m == kBlk)) {
-#pragma unroll
-        for (int i = 0; i < 8; i++)
-#pragma unroll
-            for (int c = 0; c < 4; c++)
-                if (16 * i + 4 * l + c >= m) d[i][c] = 0;
-    }
-}
 
 // quad-wide reductions (lanes 4q..4q+3)
 __device__ __forceinline__ uint32_t quad_or(uint32_t x) {
@@ -109,7 +34,7 @@ __device__ __forceinline__ uint32_t quad_max(uint32_t x) {
 }
 
 // ---- E2: canonical b of the quad's block (FORMAT.md §2: exact argmin of the block size over
-// b in 0..maxw, ties to the largest b). Same window argument as choose_b in block_encode.cuh:
+// b in 0..maxw, ties to the largest b). Window argument:
 // the 9 candidates [top-8, top] are costed from nibble counters (pattern 0x11111111 << 4t marks the
 // thresholds at which a value of width top-t is an exception); the chain of windows stops when
 // the exceptions above the window alone cost at least the best size, and jumps over widths no
@@ -190,20 +115,6 @@ constexpr int kSlotChunks = 33;
 constexpr int kAreaChunks = 243 + kSlotChunks;                  // 276 chunks = 4416 B
 __device__ __forceinline__ int quad_slot_chunk(int q) { return 33 * q + 3 * ((q + 1) >> 1); }
 
-// row owner -> staging: the quad's 128 deltas, row r = 4i + l at chunk r (128-bit stores)
-__device__ __forceinline__ void quad_stage_deltas(uint4* __restrict__ slot, const uint32_t (&d)[8][4]) {
-    const int l = quad_l();
-#pragma unroll
-    for (int i = 0; i < 8; i++) slot[4 * i + l] = make_uint4(d[i][0], d[i][1], d[i][2], d[i][3]);
-}
-
-// staging -> column owner: lane c of the quad gets u[r] = d[4r + c]
-__device__ __forceinline__ void col_load(const uint32_t* __restrict__ slot, uint32_t (&u)[32]) {
-    const int c = quad_l();
-#pragma unroll
-    for (int r = 0; r < 32; r++) u[r] = slot[4 * r + c];
-}
-
 // One column of the payload (FORMAT.md §2 "Payload"), packed sequentially by its owner lane from
 // registers: row r's low b bits at stream bits [r b, (r+1) b); word k goes to outp[4k].
 // For b <= 8 (<= 16) four (two) neighbouring rows are first merged into one item with IMADs, which
@@ -244,49 +155,6 @@ __device__ __forceinline__ void col_pack32(const uint32_t (&u)[32], uint32_t b, 
     }
 }
 #undef BFSC_EMIT_ITEM
-
-// Exceptions of the quad's block (FORMAT.md §2 "Exceptions"), column owner, 32-bit deltas (for
-// W = 64 the high parts are zero-extended). e = image + 16 + 16 b. Exception number `rank` (ascending
-// position j = 4r + c) is written by the lane that owns it: each lane builds the 32-bit mask of its
-// own exceptions (bit r), the quad exchanges the four masks, and rank = number of exceptions in
-// earlier rows plus those of lower columns in the same row. The high part comes from the staged
-// delta (dynamic index: shared memory, not registers).
-// Must be called by the whole warp (shuffles, __syncwarp); quads with n_exc == 0 idle through it.
-template <int W>
-__device__ __forceinline__ void col_exceptions(const uint32_t (&u)[32], const uint32_t* __restrict__ slot,
-                                               unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc) {
-    using T = typename IdT<W>::T;
-    constexpr uint32_t E = W / 8;
-    const int lane = threadIdx.x & 31, c = lane & 3;
-    const bool on = n_exc > 0;                               // then b < 32
-    uint32_t mk = 0;
-    if (on) {
-        const uint32_t mask = (1u << b) - 1u;
-#pragma unroll
-        for (int r = 0; r < 32; r++)
-            if (u[r] > mask) mk |= 1u << r;
-        const uint32_t eb = exc_bytes<W>(n_exc);             // zero the area: pads must be 0
-        for (uint32_t x = c; x < eb / 16; x += 4) reinterpret_cast<uint4*>(e)[x] = make_uint4(0, 0, 0, 0);
-    }
-    const uint32_t M0 = __shfl_sync(kFull, mk, (lane & ~3) + 0), M1 = __shfl_sync(kFull, mk, (lane & ~3) + 1);
-    const uint32_t M2 = __shfl_sync(kFull, mk, (lane & ~3) + 2), M3 = __shfl_sync(kFull, mk, (lane & ~3) + 3);
-    __syncwarp();
-    if (on) {
-        T* high = reinterpret_cast<T*>(e + ((n_exc + E - 1) & ~(E - 1)));
-        uint32_t rest = mk;
-        while (rest) {
-            const uint32_t r = (uint32_t)__ffs(rest) - 1u;
-            rest &= rest - 1u;
-            const uint32_t below = (1u << r) - 1u, incl = (2u << r) - 1u;
-            const uint32_t rank = __popc(M0 & (c > 0 ? incl : below)) + __popc(M1 & (c > 1 ? incl : below)) +
-                                  __popc(M2 & (c > 2 ? incl : below)) + __popc(M3 & below);
-            const uint32_t pos = 4u * r + (uint32_t)c;
-            e[rank] = (unsigned char)pos;
-            high[rank] = (T)(slot[pos] >> b);
-        }
-    }
-    __syncwarp();
-}
 
 // ---- E1 (column owner): raw IDs staged by cp.async, deltas computed by the lane that packs them ----
 // The quad's block is copied global -> shared as ALIGNED 16-byte chunks (cp.async.cg, no registers,
@@ -359,7 +227,12 @@ __device__ __forceinline__ typename IdT<W>::T col_deltas(const typename IdT<W>::
 }
 
 
-// Exceptions as col_exceptions, but the high part is recomputed from the staged RAW IDs.
+// Exceptions of the quad's block (FORMAT.md §2 "Exceptions"), column owner, 32-bit deltas (for W = 64 the high
+// parts are zero-extended). e = image + 16 + 16 b. Exception number `rank` (ascending position j = 4r + c) is
+// written by the lane that owns it: each lane builds the 32-bit mask of its own exceptions (bit r), the quad
+// exchanges the four masks, and rank = number of exceptions in earlier rows plus those of lower columns in the
+// same row. The high part is recomputed from the staged RAW IDs.
+// Must be called by the whole warp (shuffles, __syncwarp); quads with n_exc == 0 idle through it.
 template <int W>
 __device__ __forceinline__ void col_exceptions_raw(const uint32_t (&u)[32], const typename IdT<W>::T* __restrict__ raw,
                                                    unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc) {
