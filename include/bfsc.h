@@ -22,6 +22,12 @@
  *    launch: a kernel may become resident while its predecessor in the stream still runs, but
  *    waits for that predecessor to complete before it touches memory (back-to-back calls pay
  *    no launch gap).
+ *  - Concurrency: bfsc_compress / bfsc_compress_batch run a persistent grid that fills the GPU
+ *    and whose CTAs wait for one another (device-wide scan of block sizes). Issue compress
+ *    calls of one device on ONE stream at a time: two compress grids that become resident
+ *    half each (two streams racing for the same SMs) can wait for each other forever.
+ *    Decompress calls have no such dependency and may run on any stream, also next to a
+ *    compress call.
  *  - d_ids / d_out / d_in must be 16-byte aligned; element offsets inside a batch may be
  *    arbitrary (buffers that start off a 16-byte boundary are staged / written through
  *    aligned 16-byte chunks all the same).
