@@ -274,12 +274,14 @@ __device__ __forceinline__ unsigned long long lookback(const unsigned long long*
     return acc;
 }
 
-// Image buffer of a warp: room for 8 block images of at most kCap bytes, back to back. u32: 320 B (b = 16 with
-// exceptions, b = 19 without); u64: 288 B, so that two CTAs of the batch instantiation (1 KB blocks staged, 10 KB
-// of bookkeeping) still fit one SM.
+// Image buffer of a warp: room for 8 block images of at most kCap bytes, back to back. u32: 544 B — EVERY u32
+// block fits (b = 32 costs 528 B and the argmin never exceeds it): nearly incompressible u32 input stays on the
+// fast path (with 320-byte slots a stream of 22-bit gaps took 141 us instead of 37). u64: 288 B (b = 17), so that
+// two CTAs of the batch instantiation (1 KB blocks staged, 10 KB of bookkeeping) still fit one SM; larger u64
+// blocks (gaps over 2^17 between sorted 64-bit IDs) take the slow path.
 template <int W> struct ImgCfg {
-    static constexpr int kSlotChunks = (W == 32) ? 21 : 18;   // 16-byte chunks per block
-    static constexpr int kCap = (W == 32) ? 320 : 288;        // bytes of a block image the fast path can hold
+    static constexpr int kSlotChunks = (W == 32) ? 34 : 18;   // 16-byte chunks per block
+    static constexpr int kCap = (W == 32) ? 544 : 288;        // bytes of a block image the fast path can hold
     static constexpr int kBufChunks = kQuadBlocks * kSlotChunks;
 };
 
