@@ -158,14 +158,18 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
 // Blocks over 272 B (b > 16: nearly incompressible data) take the warp-per-block path of
 // block_decode.cuh, straight from global memory. Single-stream calls parse the stream header here
 // (no plan kernel); RAW streams are copied at the end (D5).
-constexpr int kDecWarps = 8;
-constexpr int kDecThreads = kDecWarps * 32;
+// CTA shape: u32 3 CTAs of 10 warps per SM (7.4 KB of shared memory per warp), u64 2 CTAs of 8 warps (11.5 KB per warp)
+template <int W> struct DecCfg {
+    static constexpr int kWarps = (W == 32) ? 10 : 8;
+    static constexpr int kThreads = kWarps * 32;
+    static constexpr int kCtasPerSm = (W == 32) ? 3 : 2;
+};
 
 template <int W> struct DecSmem {
     using T = typename IdT<W>::T;
     static constexpr size_t kStageBytes = (size_t)kDecStageChunks * 16;               // per warp
     static constexpr size_t kTabBytes = (size_t)kDecBlocks * kBlk * sizeof(T);         // per warp
-    static constexpr size_t kBytes = kDecWarps * (kStageBytes + kTabBytes);
+    static constexpr size_t kBytes = DecCfg<W>::kWarps * (kStageBytes + kTabBytes);
 };
 
 template <int W>
@@ -177,7 +181,8 @@ struct BlockAt {                       // where the quad's block is
 };
 
 template <int W, bool kBatch>          // kBatch: a.in_off != nullptr
-__global__ void __launch_bounds__(kDecThreads, (W == 32) ? 4 : 2) k_dec_tiles(DecArgs a) {
+__global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_dec_tiles(DecArgs a) {
+    constexpr int kDecWarps = DecCfg<W>::kWarps;
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
     extern __shared__ __align__(16) unsigned char dec_smem[];
@@ -348,14 +353,14 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
         if (cudaFuncSetAttribute(k_dec_tiles<W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess ||
             cudaFuncSetAttribute(k_dec_tiles<W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
             return BFSC_ERR_CUDA;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dec_tiles<W, true>, kDecThreads, kSmem) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dec_tiles<W, true>, DecCfg<W>::kThreads, kSmem) != cudaSuccess ||
             per_sm < 1)
             per_sm = 1;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         max_grid = sms * per_sm;
     }
-    const size_t want = (max_blocks + kDecBlocks * kDecWarps - 1) / (kDecBlocks * kDecWarps);
+    const size_t want = (max_blocks + kDecBlocks * DecCfg<W>::kWarps - 1) / (kDecBlocks * DecCfg<W>::kWarps);
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
     if (a.in_off) {
@@ -365,9 +370,9 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
         if (bgrid > (size_t)(kNumSM * 8)) bgrid = (size_t)(kNumSM * 8);
         if (launch_dep(k_dec_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
         BFSC_LAUNCH_CHECK();
-        if (launch_dep(k_dec_tiles<W, true>, max_grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        if (launch_dep(k_dec_tiles<W, true>, max_grid, DecCfg<W>::kThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     } else {
-        if (launch_dep(k_dec_tiles<W, false>, grid, kDecThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        if (launch_dep(k_dec_tiles<W, false>, grid, DecCfg<W>::kThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
     }
     BFSC_LAUNCH_CHECK();
     return BFSC_OK;
