@@ -158,11 +158,11 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
 // Blocks over 272 B (b > 16: nearly incompressible data) take the warp-per-block path of
 // block_decode.cuh, straight from global memory. Single-stream calls parse the stream header here
 // (no plan kernel); RAW streams are copied at the end (D5).
-// CTA shape: u32 3 CTAs of 10 warps per SM (7.4 KB of shared memory per warp), u64 2 CTAs of 8 warps (11.5 KB per warp)
+// CTA shape: u32 2 CTAs of 14 warps per SM (7.4 KB of shared memory per warp), u64 2 CTAs of 8 warps (11.5 KB per warp)
 template <int W> struct DecCfg {
-    static constexpr int kWarps = (W == 32) ? 10 : 8;
+    static constexpr int kWarps = (W == 32) ? 14 : 8;
     static constexpr int kThreads = kWarps * 32;
-    static constexpr int kCtasPerSm = (W == 32) ? 3 : 2;
+    static constexpr int kCtasPerSm = (W == 32) ? 2 : 2;
 };
 
 template <int W> struct DecSmem {
@@ -270,8 +270,20 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
     };
 
     const unsigned long long n_batches = (total_blocks + kDecBlocks - 1) / kDecBlocks;
-    const unsigned long long n_warps = (unsigned long long)gridDim.x * kDecWarps;
+    // Every working warp gets the same number of batches: with R = rounds the grid's warps need, only
+    // ceil(n_batches / R) warps work, spread evenly over the CTAs (CTA c has base or base + 1 working warps,
+    // numbered consecutively: neighbouring batches, i.e. neighbouring bytes of the stream, stay on one SM).
+    // 2^24 IDs = 16384 batches on 296 x 14 warps: 4 rounds, 4096 warps with 4 batches each.
+    const uint32_t cap_warps = gridDim.x * kDecWarps;
+    unsigned long long n_warps = cap_warps;
     unsigned long long bi = (unsigned long long)blockIdx.x * kDecWarps + warp;
+    if (n_batches > cap_warps && n_batches < 0xffffffffull) {             // (32-bit arithmetic: 64-bit divisions cost more than they save)
+        const uint32_t nb32 = (uint32_t)n_batches, rounds = (nb32 + cap_warps - 1) / cap_warps;
+        const uint32_t nw = (nb32 + rounds - 1) / rounds, base_w = nw / gridDim.x, rem_w = nw - base_w * gridDim.x;
+        n_warps = nw;
+        bi = blockIdx.x * base_w + min(blockIdx.x, rem_w) + warp;
+        if ((uint32_t)warp >= base_w + (blockIdx.x < rem_w ? 1u : 0u)) bi = n_batches;   // this warp sits the call out
+    }
     BlockAt<W> cur = locate(bi * kDecBlocks + q);
     for (; bi < n_batches; bi += n_warps) {
         const bool big = cur.blk != nullptr && cur.span16 > (uint32_t)kDecSpanMax;
