@@ -158,9 +158,9 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
 // Blocks over 272 B (b > 16: nearly incompressible data) take the warp-per-block path of
 // block_decode.cuh, straight from global memory. Single-stream calls parse the stream header here
 // (no plan kernel); RAW streams are copied at the end (D5).
-// CTA shape: u32 2 CTAs of 14 warps per SM (7.4 KB of shared memory per warp), u64 2 CTAs of 8 warps (11.5 KB per warp)
+// CTA shape: u32 2 CTAs of 16 warps per SM (6.9 KB of shared memory per warp), u64 2 CTAs of 8 warps (11 KB per warp)
 template <int W> struct DecCfg {
-    static constexpr int kWarps = (W == 32) ? 14 : 8;
+    static constexpr int kWarps = (W == 32) ? 16 : 8;
     static constexpr int kThreads = kWarps * 32;
     static constexpr int kCtasPerSm = (W == 32) ? 2 : 2;
 };
@@ -273,7 +273,7 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
     // Every working warp gets the same number of batches: with R = rounds the grid's warps need, only
     // ceil(n_batches / R) warps work, spread evenly over the CTAs (CTA c has base or base + 1 working warps,
     // numbered consecutively: neighbouring batches, i.e. neighbouring bytes of the stream, stay on one SM).
-    // 2^24 IDs = 16384 batches on 296 x 14 warps: 4 rounds, 4096 warps with 4 batches each.
+    // 2^24 IDs = 16384 batches on 296 x 16 warps: 4 rounds, 4096 warps with 4 batches each instead of 4736 with 3 or 4.
     const uint32_t cap_warps = gridDim.x * kDecWarps;
     unsigned long long n_warps = cap_warps;
     unsigned long long bi = (unsigned long long)blockIdx.x * kDecWarps + warp;

@@ -4,7 +4,7 @@
 // 64 (u32) / 128 (u64) contiguous bytes, so loads and stores are coalesced 128-bit accesses, and the
 // per-block scalar work (header, directory, validation) costs 1/8 of a warp instruction per block.
 //
-// Fast path only: blocks of at most kDecSpanMax 16-byte chunks (b <= 24 without exceptions),
+// Fast path only: blocks of at most kDecSpanMax 16-byte chunks (b <= 20 without exceptions),
 // staged in shared memory by cp.async. Larger blocks take the warp-per-block path of block_decode.cuh.
 #pragma once
 #include "common.cuh"
@@ -12,8 +12,8 @@
 namespace bfsc {
 
 constexpr int kDecBlocks = 8;                 // blocks per warp batch
-constexpr int kDecSpanMax = 25;               // largest staged block, in 16-byte chunks (400 B: b = 24)
-constexpr int kDecSlotChunks = 26;            // slot stride: one chunk of slack for the unpack's second read
+constexpr int kDecSpanMax = 21;               // largest staged block, in 16-byte chunks (336 B: b = 20)
+constexpr int kDecSlotChunks = 22;            // slot stride: one chunk of slack for the unpack's second read
 constexpr int kDecStageChunks = kDecBlocks * kDecSlotChunks;
 
 __device__ __forceinline__ void dec_cp_async16(void* smem_dst, const void* gmem_src) {
