@@ -153,9 +153,9 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
 // ---- D1-D5 fused -------------------------------------------------------------------------
 // Warp = batch of 8 consecutive blocks, four lanes per block (quad_decode.cuh). Per batch:
 //   locate   per quad: stream, directory entries -> block address, span, valid IDs, output address
-//   D1       cp.async the block (<= 272 B) into the warp's staging slots
+//   D1       cp.async the block (<= 336 B) into the warp's staging slots
 //   D2-D4    unpack from shared memory, patch through the warp's table, scan, 128-bit stores
-// Blocks over 272 B (b > 16: nearly incompressible data) take the warp-per-block path of
+// Blocks over 336 B (b > 20: nearly incompressible data) take the warp-per-block path of
 // block_decode.cuh, straight from global memory. Single-stream calls parse the stream header here
 // (no plan kernel); RAW streams are copied at the end (D5).
 // CTA shape: u32 2 CTAs of 16 warps per SM (6.9 KB of shared memory per warp), u64 2 CTAs of 8 warps (11 KB per warp)
