@@ -38,8 +38,8 @@ W = 32
 METRIC = "codec_throughput_encode_plus_decode"
 UNIT = "GB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (k_enc_tiles<32>, stream a,
-# 2^24 IDs), from the committed `ncu --set full` capture profiles/r1_enc_tiles_ncu_summary.txt (67.30 + 2.04 MB).
-NCU_TRAFFIC_BYTES = {"encode_a": 69_342_464, "decode_a": 24_857_600, "source": "profiles/r1_*_tiles_ncu_summary.txt"}
+# 2^24 IDs), from the committed `ncu --set full` capture profiles/r1_enc_tiles_ncu_summary.txt (67.30 + 1.73 MB).
+NCU_TRAFFIC_BYTES = {"encode_a": 69_034_240, "decode_a": 24_271_872, "source": "profiles/r1_*_tiles_ncu_summary.txt"}
 
 
 def peaks():
