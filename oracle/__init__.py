@@ -20,6 +20,7 @@ _HDR = os.path.join(_HERE, "bfsc_ref.h")
 _lib = None
 
 OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT = 0, 1, 2, 3
+CODEC_PFOR, CODEC_BP128 = 1, 2          # encoder rule = mode byte of the stream (FORMAT.md §1, §7)
 
 
 class OracleError(RuntimeError):
@@ -60,6 +61,12 @@ def lib():
         L.bfsc_ref_emit_block.argtypes = [vp, c.c_uint64, i32, i32, vp]
         L.bfsc_ref_compress.restype = i32
         L.bfsc_ref_compress.argtypes = [vp, sz, i32, sz, vp, sz, c.POINTER(sz)]
+        L.bfsc_ref_choose_b_bp128.restype = i32
+        L.bfsc_ref_choose_b_bp128.argtypes = [vp]
+        L.bfsc_ref_compress_codec.restype = i32
+        L.bfsc_ref_compress_codec.argtypes = [i32, vp, sz, i32, sz, vp, sz, c.POINTER(sz)]
+        L.bfsc_ref_compress_batch_codec.restype = i32
+        L.bfsc_ref_compress_batch_codec.argtypes = [i32, vp, vp, sz, i32, sz, vp, sz, vp]
         L.bfsc_ref_decompress.restype = i32
         L.bfsc_ref_decompress.argtypes = [vp, sz, i32, vp, sz, c.POINTER(sz)]
         L.bfsc_ref_compress_batch.restype = i32
@@ -118,6 +125,12 @@ def choose_b(d: np.ndarray, W: int):
     return b, n_exc.value
 
 
+def choose_b_bp128(d: np.ndarray) -> int:
+    d = np.ascontiguousarray(d, dtype=np.uint64)
+    assert d.shape == (128,)
+    return lib().bfsc_ref_choose_b_bp128(_p(d))
+
+
 def emit_block(d: np.ndarray, base: int, b: int, W: int) -> bytes:
     d = np.ascontiguousarray(d, dtype=np.uint64)
     out = np.zeros(2304, dtype=np.uint8)
@@ -125,13 +138,14 @@ def emit_block(d: np.ndarray, base: int, b: int, W: int) -> bytes:
     return out[:n].tobytes()
 
 
-def compress(ids: np.ndarray, raw_threshold_bytes: int = 0) -> np.ndarray:
+def compress(ids: np.ndarray, raw_threshold_bytes: int = 0, codec: int = CODEC_PFOR) -> np.ndarray:
     ids = np.ascontiguousarray(ids)
     W = _W(ids)
     cap = max(compress_bound(len(ids), W), 32 + (len(ids) * W // 8 + 15) // 16 * 16)
     out = np.empty(cap, dtype=np.uint8)
     nbytes = ctypes.c_size_t(0)
-    rc = lib().bfsc_ref_compress(_p(ids), len(ids), W, raw_threshold_bytes, _p(out), cap, ctypes.byref(nbytes))
+    rc = lib().bfsc_ref_compress_codec(codec, _p(ids), len(ids), W, raw_threshold_bytes, _p(out), cap,
+                                       ctypes.byref(nbytes))
     if rc:
         raise OracleError(rc)
     return out[:nbytes.value].copy()
@@ -155,8 +169,9 @@ def batch_bound(in_offsets: np.ndarray, W: int) -> int:
     return int(sum(max(compress_bound(int(c), W), 32 + (int(c) * W // 8 + 15) // 16 * 16) for c in counts))
 
 
-def compress_batch(ids: np.ndarray, in_offsets: np.ndarray, raw_threshold_bytes: int = 0, threads: int = 0):
-    """-> (out bytes, out_offsets[n_buf+1]); threads > 0 uses the pthread driver."""
+def compress_batch(ids: np.ndarray, in_offsets: np.ndarray, raw_threshold_bytes: int = 0, threads: int = 0,
+                   codec: int = CODEC_PFOR):
+    """-> (out bytes, out_offsets[n_buf+1]); threads > 0 uses the pthread driver (PFOR only)."""
     ids = np.ascontiguousarray(ids)
     W = _W(ids)
     in_offsets = np.ascontiguousarray(in_offsets, dtype=np.uint64)
@@ -169,11 +184,12 @@ def compress_batch(ids: np.ndarray, in_offsets: np.ndarray, raw_threshold_bytes:
     out = np.empty(max(cap, 16), dtype=np.uint8)
     out_off = np.zeros(n_buf + 1, dtype=np.uint64)
     if threads > 0:
+        assert codec == CODEC_PFOR
         rc = lib().bfsc_ref_compress_batch_mt(_p(ids), _p(in_offsets), n_buf, W, raw_threshold_bytes,
                                               _p(out), cap, _p(out_off), threads)
     else:
-        rc = lib().bfsc_ref_compress_batch(_p(ids), _p(in_offsets), n_buf, W, raw_threshold_bytes,
-                                           _p(out), cap, _p(out_off))
+        rc = lib().bfsc_ref_compress_batch_codec(codec, _p(ids), _p(in_offsets), n_buf, W, raw_threshold_bytes,
+                                                 _p(out), cap, _p(out_off))
     if rc:
         raise OracleError(rc)
     return out[:int(out_off[-1])], out_off

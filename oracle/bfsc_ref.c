@@ -76,6 +76,15 @@ int bfsc_ref_choose_b(const uint64_t d[128], int W, int *n_exc_out) {
     return best_b;
 }
 
+/* FORMAT.md §7 (mode 2, BP128-D1): plain binary packing, the codec class the thesis ran (S4-BP128,
+ * blocks of 128, b in 0..32, no exceptions). b = the frame-of-reference width of
+ * the block's deltas (eq. 6 L969 with min = 0; "driven by b of the worst value", L987-998). */
+int bfsc_ref_choose_b_bp128(const uint64_t d[128]) {
+    int maxw = 0;
+    for (int j = 0; j < BLK; j++) { int w = bfsc_ref_width(d[j]); if (w > maxw) maxw = w; }
+    return maxw;
+}
+
 /* O6: header, payload (4-column interleave), exceptions, pads — FORMAT.md §2. */
 size_t bfsc_ref_emit_block(const uint64_t d[128], uint64_t base, int b, int W, uint8_t *out) {
     int pos[BLK], n_exc = 0;
@@ -125,7 +134,13 @@ static int is_raw(size_t n, int W, size_t thr) { return n * (size_t)(W / 8) < th
 
 int bfsc_ref_compress(const void *ids, size_t n, int W, size_t thr,
                       uint8_t *out, size_t cap, size_t *out_bytes) {
+    return bfsc_ref_compress_codec(BFSC_REF_CODEC_PFOR, ids, n, W, thr, out, cap, out_bytes);
+}
+
+int bfsc_ref_compress_codec(int codec, const void *ids, size_t n, int W, size_t thr,
+                            uint8_t *out, size_t cap, size_t *out_bytes) {
     if ((W != 32 && W != 64) || !out || !out_bytes || (n && !ids)) return BFSC_REF_ERR_INVALID_ARG;
+    if (codec != BFSC_REF_CODEC_PFOR && codec != BFSC_REF_CODEC_BP128) return BFSC_REF_ERR_INVALID_ARG;
     if (is_raw(n, W, thr)) {
         size_t body = n * (size_t)(W / 8), total = 32 + align_up(body, 16);
         if (total > cap) return BFSC_REF_ERR_DST_TOO_SMALL;
@@ -145,7 +160,10 @@ int bfsc_ref_compress(const void *ids, size_t n, int W, size_t thr,
         uint64_t d[BLK];
         const uint8_t *xb = (const uint8_t *)ids + BLK * k * (size_t)(W / 8);
         uint64_t base = bfsc_ref_block_deltas(xb, m, W, d);   /* O3 */
-        int n_exc, b = bfsc_ref_choose_b(d, W, &n_exc);       /* O4, O5 */
+        int n_exc = 0, b;
+        if (codec == BFSC_REF_CODEC_BP128) b = bfsc_ref_choose_b_bp128(d);   /* FORMAT.md §7 */
+        else b = bfsc_ref_choose_b(d, W, &n_exc);             /* O4, O5 */
+        (void)n_exc;
         size_t sz = bfsc_ref_emit_block(d, base, b, W, tmp);  /* O6 */
         if (off + sz > cap) return BFSC_REF_ERR_DST_TOO_SMALL;
         memcpy(out + off, tmp, sz);
@@ -153,7 +171,7 @@ int bfsc_ref_compress(const void *ids, size_t n, int W, size_t thr,
         off += sz;
     }
     st_le(out + 32 + 4 * nb, off / 16, 4);
-    write_header(out, W, 1, n, off, (uint32_t)nb);
+    write_header(out, W, codec, n, off, (uint32_t)nb);     /* mode byte = codec (1 PFOR-D1, 2 BP128-D1) */
     *out_bytes = off;
     return BFSC_REF_OK;
 }
@@ -196,7 +214,7 @@ static int parse_header(const uint8_t *in, size_t in_bytes, int W,
                         int *mode, uint64_t *n, uint64_t *total, uint64_t *nb) {
     if (in_bytes < 32) return BFSC_REF_ERR_CORRUPT;
     if (in[0] != 'B' || in[1] != 'F' || in[2] != 'S' || in[3] != 'C') return BFSC_REF_ERR_CORRUPT;
-    if (in[4] != 1 || in[5] != W || in[6] > 1) return BFSC_REF_ERR_CORRUPT;
+    if (in[4] != 1 || in[5] != W || in[6] > 2) return BFSC_REF_ERR_CORRUPT;
     *mode = in[6];
     *n = ld_le(in + 8, 8); *total = ld_le(in + 16, 8); *nb = ld_le(in + 24, 4);
     if (*total > in_bytes || *total % 16 || *total < 32) return BFSC_REF_ERR_CORRUPT;
@@ -237,12 +255,17 @@ int bfsc_ref_decompress(const uint8_t *in, size_t in_bytes, int W,
 
 int bfsc_ref_compress_batch(const void *ids, const uint64_t *in_off, size_t n_buf, int W,
                             size_t thr, uint8_t *out, size_t cap, uint64_t *out_off) {
+    return bfsc_ref_compress_batch_codec(BFSC_REF_CODEC_PFOR, ids, in_off, n_buf, W, thr, out, cap, out_off);
+}
+
+int bfsc_ref_compress_batch_codec(int codec, const void *ids, const uint64_t *in_off, size_t n_buf, int W,
+                                  size_t thr, uint8_t *out, size_t cap, uint64_t *out_off) {
     if (!in_off || !out_off) return BFSC_REF_ERR_INVALID_ARG;
     size_t off = 0;
     for (size_t i = 0; i < n_buf; i++) {
         size_t bytes = 0;
         const uint8_t *src = (const uint8_t *)ids + in_off[i] * (size_t)(W / 8);
-        int rc = bfsc_ref_compress(src, in_off[i + 1] - in_off[i], W, thr, out + off, cap - off, &bytes);
+        int rc = bfsc_ref_compress_codec(codec, src, in_off[i + 1] - in_off[i], W, thr, out + off, cap - off, &bytes);
         if (rc) return rc;
         out_off[i] = off;
         off += bytes;

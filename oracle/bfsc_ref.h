@@ -21,7 +21,9 @@
  * closed-form sizes for constant-gap sequences, brute-force choice of b written
  * independently in Python, an independent pure-Python big-integer decoder
  * (oracle/witness.py) built from FORMAT.md alone, hand-computed byte vectors,
- * round-trip identity and the walk-the-headers invariants.
+ * round-trip identity and the walk-the-headers invariants. Mode 2 (BP128-D1, FORMAT.md §7): hand-evaluated
+ * sizes (tests/golden/bp128_sizes.txt), b = int.bit_length of the widest delta, blocks byte-equal to the
+ * witness builder with that b, witness decode, equality with mode 1 where no exception pays.
  * Parity vs the thesis's own codec (S4-BP128 bytes / ratios): parity unpinned — the
  * thesis ships no byte layout and its sample data are not available.
  *
@@ -44,6 +46,9 @@ enum {
     BFSC_REF_ERR_CORRUPT = 3
 };
 
+/* Encoder rule = mode byte of the stream it writes (FORMAT.md §1, §7). */
+enum { BFSC_REF_CODEC_PFOR = 1, BFSC_REF_CODEC_BP128 = 2 };
+
 /* bit length of v: 0 for 0, floor(log2 v)+1 otherwise. For a range [min,max] the FOR
  * width of eq. (6) is bfsc_ref_width(max - min). */
 int bfsc_ref_width(uint64_t v);
@@ -62,6 +67,10 @@ uint64_t bfsc_ref_block_deltas(const void *x, int m, int W, uint64_t d[128]);
  * b in 0..maxw, ties to the largest b. Writes n_exc(b). */
 int bfsc_ref_choose_b(const uint64_t d[128], int W, int *n_exc);
 
+/* b of the no-exception codec (FORMAT.md §7, mode 2 = BP128-D1; the thesis's codec class S4-BP128,
+ * PAPER.md L1052-1056): the width of the block's widest delta; n_exc = 0. */
+int bfsc_ref_choose_b_bp128(const uint64_t d[128]);
+
 /* Emit one block with a GIVEN b (any 0..W): header, payload, exceptions, pads.
  * Returns its byte count (= block_bytes(b, n_exc(b))). out must hold 16+16W+... bytes
  * (<= 16 + 16*64 + 16 + 127*9 rounded; 2304 is always enough). */
@@ -70,6 +79,14 @@ size_t bfsc_ref_emit_block(const uint64_t d[128], uint64_t base, int b, int W, u
 /* One stream. Returns BFSC_REF_OK and *out_bytes, or an error. */
 int bfsc_ref_compress(const void *ids, size_t n, int W, size_t raw_threshold_bytes,
                       uint8_t *out, size_t out_capacity, size_t *out_bytes);
+
+/* Same, with the encoder rule given: BFSC_REF_CODEC_PFOR (what bfsc_ref_compress does) or
+ * BFSC_REF_CODEC_BP128 (every block b = maxw, no exceptions; header mode 2). */
+int bfsc_ref_compress_codec(int codec, const void *ids, size_t n, int W, size_t raw_threshold_bytes,
+                            uint8_t *out, size_t out_capacity, size_t *out_bytes);
+int bfsc_ref_compress_batch_codec(int codec, const void *ids, const uint64_t *in_offsets, size_t n_buf, int W,
+                                  size_t raw_threshold_bytes,
+                                  uint8_t *out, size_t out_capacity, uint64_t *out_offsets);
 
 /* One stream. in_bytes = bytes available at `in` (may exceed the stream's total_bytes).
  * Writes *n_ids; ids must hold ids_capacity elements of W bits. */

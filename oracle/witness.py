@@ -69,9 +69,20 @@ def brute_force_b(d, W: int):
     return best
 
 
+def stream_mode(s: bytes) -> int:
+    return s[6]
+
+
+def stream_blocks(s: bytes):
+    """(b, n_exc) of every block of a mode 1 / mode 2 stream, by walking the directory."""
+    nb = int.from_bytes(s[24:28], "little")
+    dir_ = [int.from_bytes(s[32 + 4 * k:36 + 4 * k], "little") for k in range(nb + 1)]
+    return [(s[16 * dir_[k] + 8], s[16 * dir_[k] + 9]) for k in range(nb)]
+
+
 def decode_stream(s: bytes, W: int):
     """-> list of python ints. Raises ValueError on anything FORMAT.md §4 rejects."""
-    if len(s) < 32 or s[0:4] != b"BFSC" or s[4] != 1 or s[5] != W or s[6] not in (0, 1):
+    if len(s) < 32 or s[0:4] != b"BFSC" or s[4] != 1 or s[5] != W or s[6] not in (0, 1, 2):      # 2 = BP128-D1: decoded like 1 (FORMAT.md §7)
         raise ValueError("bad header")
     n = int.from_bytes(s[8:16], "little")
     total = int.from_bytes(s[16:24], "little")

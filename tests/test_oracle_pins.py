@@ -161,3 +161,98 @@ def test_forced_b_blocks_decode(oracle_mod):
             got = oracle_mod.decompress(np.frombuffer(s, np.uint8), W)
             assert [int(v) for v in got] == [int(v) for v in want]
             assert witness.decode_stream(s, W) == [int(v) for v in want]
+
+
+# ---------------------------------------------------------------- mode 2: BP128-D1 (FORMAT.md §7)
+def _bp128_case(name, W, n):
+    dt = _dt(W)
+    if name == "gap1":
+        return (1000 + np.arange(n, dtype=np.uint64)).astype(dt)
+    if name == "gap3":
+        return (1000 + 3 * np.arange(n, dtype=np.uint64)).astype(dt)
+    if name == "step20":
+        x = 7 + np.arange(n, dtype=np.uint64)
+        x[51:] += (1 << 20) - 1                        # delta of ID 51 = 2^20
+        return x.astype(dt)
+    if name == "seq8":
+        return np.array([int(v) for v in _rows("paper_seq8.txt")[0]], dtype=dt)
+    if name == "range7":
+        return np.arange(2000, 2128, dtype=dt)
+    raise KeyError(name)
+
+
+def test_bp128_sizes_and_witness(oracle_mod):
+    for name, W, n, total in _rows("bp128_sizes.txt"):
+        W, n, total = int(W), int(n), int(total)
+        x = _bp128_case(name, W, n)
+        s = oracle_mod.compress(x, codec=oracle_mod.CODEC_BP128)
+        assert len(s) == total, name
+        assert witness.stream_mode(s.tobytes()) == 2
+        assert all(ne == 0 for _, ne in witness.stream_blocks(s.tobytes()))
+        assert witness.decode_stream(s.tobytes(), W) == [int(v) for v in x]          # second witness
+        assert np.array_equal(oracle_mod.decompress(s, W), x)
+        assert len(s) <= oracle_mod.compress_bound(n, W)
+
+
+def test_bp128_b_is_max_width_and_blocks_match_forced_b(oracle_mod):
+    """b = bit length of the widest delta (eq. 6, min = 0), found here with Python's int.bit_length;
+    the stream = header(mode 2) | directory | witness.build_block(d, base, b) for every block."""
+    rng = np.random.default_rng(11)
+    for W in (32, 64):
+        for trial in range(12):
+            n = int(rng.integers(1, 700))
+            hi = int(rng.integers(1, W))
+            gaps = rng.integers(0, 1 << int(rng.integers(1, hi + 1)), size=n, dtype=np.uint64)
+            gaps[rng.random(n) < 0.03] = rng.integers(0, 1 << hi, dtype=np.uint64)   # outliers: would be exceptions in PFOR
+            x = np.cumsum(gaps, dtype=np.uint64).astype(_dt(W))
+            s = oracle_mod.compress(x, codec=oracle_mod.CODEC_BP128).tobytes()
+            nb = -(-n // 128)
+            blocks = witness.stream_blocks(s)
+            at = 32 + -(-4 * (nb + 1) // 16) * 16
+            for k in range(nb):
+                xs = [int(v) for v in x[128 * k:128 * (k + 1)]]
+                base, d = witness.deltas_of_block(xs, W)
+                b = max(v.bit_length() for v in d)
+                assert blocks[k] == (b, 0)
+                assert oracle_mod.choose_b_bp128(np.array(d, dtype=np.uint64)) == b
+                img = witness.build_block(d, base, b, W)
+                assert s[at:at + len(img)] == img
+                assert int.from_bytes(s[32 + 4 * k:36 + 4 * k], "little") == at // 16
+                at += len(img)
+            assert at == len(s) and int.from_bytes(s[16:24], "little") == at
+            assert witness.decode_stream(s, W) == [int(v) for v in x]
+
+
+def test_bp128_equals_pfor_when_no_exception_pays(oracle_mod):
+    """Where the PFOR argmin keeps b = maxw in every block the two modes differ in byte 6 only;
+    BP128 is never smaller than PFOR (PFOR minimises over a set that contains b = maxw)."""
+    x = (5 + 3 * np.arange(5000, dtype=np.uint64)).astype(np.uint32)
+    a, b = oracle_mod.compress(x), oracle_mod.compress(x, codec=oracle_mod.CODEC_BP128)
+    assert len(a) == len(b) and a[6] == 1 and b[6] == 2
+    assert np.array_equal(np.delete(a, 6), np.delete(b, 6))
+    rng = np.random.default_rng(5)
+    for W in (32, 64):
+        g = rng.geometric(1 / 200, size=3000).astype(np.uint64)
+        g[rng.random(3000) < 0.01] = 1 << 22
+        y = np.cumsum(g, dtype=np.uint64).astype(_dt(W))
+        p, q = oracle_mod.compress(y), oracle_mod.compress(y, codec=oracle_mod.CODEC_BP128)
+        assert len(p) < len(q)
+        assert np.array_equal(oracle_mod.decompress(q, W), y)
+
+
+def test_bp128_threshold_batch_and_roundtrip(oracle_mod):
+    rng = np.random.default_rng(3)
+    for W in (32, 64):
+        counts = np.array([0, 1, 127, 128, 129, 300, 1000, 5], dtype=np.uint64)
+        off = np.concatenate([[0], np.cumsum(counts)]).astype(np.uint64)
+        ids = np.cumsum(rng.integers(1, 50, size=int(off[-1]), dtype=np.uint64)).astype(_dt(W))
+        for thr in (0, 1024):
+            out, out_off = oracle_mod.compress_batch(ids, off, thr, codec=oracle_mod.CODEC_BP128)
+            for i, c in enumerate(counts):
+                s = out[int(out_off[i]):int(out_off[i + 1])]
+                raw = int(c) * W // 8 < thr
+                assert s[6] == (0 if raw else 2)                 # RAW selection is independent of the codec
+                one = oracle_mod.compress(ids[int(off[i]):int(off[i + 1])], thr, codec=oracle_mod.CODEC_BP128)
+                assert np.array_equal(s, one)
+            back, id_off = oracle_mod.decompress_batch(out, out_off, W, len(ids))
+            assert np.array_equal(back, ids) and np.array_equal(id_off, off)
