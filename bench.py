@@ -242,6 +242,8 @@ def run_ours(args, rank, local_rank, world):
     c_back = backs + [torch.empty(n, dtype=ids[0].dtype, device=dev) for _ in range(kCopies - S)]
     kTrials = 5                                              # runs per call: median reported, min alongside
     enc_ms, dec_ms, enc_min, dec_min = [], [], [], []
+    bp_enc_ms, bp_dec_ms = [], []                            # the same calls under the BP128 rule (FORMAT.md §7)
+    nbytes_bp = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(S)]
     for s in range(S):
         c_ids = [ids[s]] + [ids[s].clone() for _ in range(kCopies - 1)]
         for c in range(kCopies):
@@ -270,6 +272,14 @@ def run_ours(args, rank, local_rank, world):
         dec_ms.append(float(np.median(dec_runs)))
         enc_min.append(min(enc_runs))
         dec_min.append(min(dec_runs))
+        bp_call = lambda c: B.compress_codec(B.CODEC_BP128, c_ids[c], n, W, 0, c_out[c], nbytes_bp[s], ws, status)   # noqa: E731
+        for c in range(kCopies):
+            bp_call(c)
+        torch.cuda.synchronize()
+        bp_enc_ms.append(float(np.median([run_of(bp_call) for _ in range(kTrials)])))
+        c_back[kCopies - 1].zero_()
+        bp_dec_ms.append(float(np.median([run_of(dec_call) for _ in range(kTrials)])))
+        assert torch.equal(c_back[kCopies - 1], ids[s]), "BP128: decode != input"
         del c_ids
     assert int(status.item()) == 0, f"device status {int(status.item())}"
     value = whole_job_value(2 * S * raw_bytes, world, ms_step * 1e-3) / 1e9
@@ -351,6 +361,12 @@ def run_ours(args, rank, local_rank, world):
                      "encode_alg_GBps": alg / enc_ms[s] / 1e6, "decode_alg_GBps": alg / dec_ms[s] / 1e6,
                      "encode_frac_of_peak": alg / enc_ms[s] / 1e6 / peak, "decode_frac_of_peak": alg / dec_ms[s] / 1e6 / peak,
                      "encode_frac_of_8TBps": alg / enc_ms[s] / 1e6 / 8000.0, "decode_frac_of_8TBps": alg / dec_ms[s] / 1e6 / 8000.0}
+        cb = int(nbytes_bp[s].item())
+        alg_bp = raw_bytes + cb + 8
+        per[name]["bp128"] = {"ratio": raw_bytes / cb, "bits_per_id": 8 * cb / n, "encode_ms": bp_enc_ms[s], "decode_ms": bp_dec_ms[s],
+                              "encode_alg_GBps": alg_bp / bp_enc_ms[s] / 1e6, "decode_alg_GBps": alg_bp / bp_dec_ms[s] / 1e6,
+                              "encode_frac_of_peak": alg_bp / bp_enc_ms[s] / 1e6 / peak, "decode_frac_of_peak": alg_bp / bp_dec_ms[s] / 1e6 / peak,
+                              "encode_frac_of_8TBps": alg_bp / bp_enc_ms[s] / 1e6 / 8000.0, "decode_frac_of_8TBps": alg_bp / bp_dec_ms[s] / 1e6 / 8000.0}
     # dominant call = encode of stream (a): most raw bytes per compressed byte, the headline dense frontier
     dom = STREAMS[0][0]
     alg_a = raw_bytes + comp[0] + 8

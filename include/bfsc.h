@@ -71,6 +71,17 @@ typedef enum {
 
 typedef enum { BFSC_U32 = 32, BFSC_U64 = 64 } bfsc_dtype;
 
+/* Encoder rule of a compress call = mode byte of the streams it writes (FORMAT.md §1, §7):
+ *   BFSC_CODEC_PFOR  (1) patched frame of reference: per block the b that minimises the block size,
+ *                        values >= 2^b stored apart as exceptions — what
+ *                        bfsc_compress / bfsc_compress_batch do;
+ *   BFSC_CODEC_BP128 (2) plain binary packing, the codec class the thesis ran (S4-BP128, L1052-1056):
+ *                        b = width of the block's widest delta (eq. 6), no exceptions. Skips
+ *                        step E2's size argmin; one outlier widens its whole block (L1000).
+ * Buffers below the raw threshold are RAW (mode 0) under either rule. bfsc_decompress[_batch] read
+ * the mode from each stream header and decode every mode. */
+typedef enum { BFSC_CODEC_PFOR = 1, BFSC_CODEC_BP128 = 2 } bfsc_codec;
+
 /* library / format version: (format_version << 16) | abi_revision */
 uint32_t bfsc_version(void);
 
@@ -91,6 +102,12 @@ bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t 
                           void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                           void* cuda_stream);
 
+/* bfsc_compress with the encoder rule given (any other value: BFSC_ERR_INVALID_ARG). */
+bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, size_t n_ids, bfsc_dtype t,
+                                size_t raw_threshold_bytes, void* d_out, size_t out_capacity,
+                                uint64_t* d_out_bytes, void* d_workspace, size_t workspace_bytes,
+                                uint32_t* d_status, void* cuda_stream);
+
 /* ONE stream at d_in (in_bytes available, >= its total_bytes) -> d_ids[0..n); *d_n_ids
  * (device) = n. Steps D0-D5. */
 bfsc_status bfsc_decompress(const void* d_in, size_t in_bytes, bfsc_dtype t,
@@ -106,6 +123,13 @@ bfsc_status bfsc_compress_batch(const void* d_ids, const uint64_t* d_in_offsets,
                                 void* d_out, size_t out_capacity, uint64_t* d_out_offsets,
                                 void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                                 void* cuda_stream);
+
+/* bfsc_compress_batch with the encoder rule given (one rule for all buffers of the batch). */
+bfsc_status bfsc_compress_batch_codec(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_offsets,
+                                      size_t n_buf, bfsc_dtype t, size_t raw_threshold_bytes,
+                                      void* d_out, size_t out_capacity, uint64_t* d_out_offsets,
+                                      void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                      void* cuda_stream);
 
 /* d_in_offsets: n_buf+1 BYTE offsets of the streams inside d_in (each a multiple of 16).
  * IDs are written back to back at d_ids; d_id_offsets[0..n_buf] (device, written) are

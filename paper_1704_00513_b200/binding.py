@@ -17,10 +17,12 @@ _lib = None
 
 OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED = range(6)
 U32, U64 = 32, 64
+CODEC_PFOR, CODEC_BP128 = 1, 2          # bfsc_codec (include/bfsc.h)
 
 EXPORTS = [
     "bfsc_version", "bfsc_compress_bound", "bfsc_batch_compress_bound", "bfsc_workspace_bytes",
     "bfsc_compress", "bfsc_decompress", "bfsc_compress_batch", "bfsc_decompress_batch",
+    "bfsc_compress_codec", "bfsc_compress_batch_codec",
     "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
 ]
 
@@ -53,6 +55,10 @@ def lib():
         L.bfsc_host_scratch_bytes.argtypes = [sz, i32]
         L.bfsc_compress.restype = i32
         L.bfsc_compress.argtypes = [vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_compress_codec.restype = i32
+        L.bfsc_compress_codec.argtypes = [i32, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_compress_batch_codec.restype = i32
+        L.bfsc_compress_batch_codec.argtypes = [i32, vp, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_decompress.restype = i32
         L.bfsc_decompress.argtypes = [vp, sz, i32, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_compress_batch.restype = i32
@@ -117,6 +123,13 @@ def compress(d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_bytes, d_workspa
                                ctypes.c_void_p(_stream())), "bfsc_compress")
 
 
+def compress_codec(codec, d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_bytes, d_workspace, d_status):
+    """bfsc_compress_codec: bfsc_compress with the encoder rule given (CODEC_PFOR / CODEC_BP128)."""
+    _check(lib().bfsc_compress_codec(codec, _ptr(d_ids), n_ids, W, raw_threshold_bytes, _ptr(d_out), d_out.numel(),
+                                     _ptr(d_out_bytes), _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
+                                     ctypes.c_void_p(_stream())), "bfsc_compress_codec")
+
+
 def decompress(d_in, in_bytes, W, d_ids, d_n_ids, d_workspace, d_status):
     _check(lib().bfsc_decompress(_ptr(d_in), in_bytes, W, _ptr(d_ids), d_ids.numel(), _ptr(d_n_ids),
                                  _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
@@ -127,6 +140,14 @@ def compress_batch(d_ids, d_in_offsets, n_buf, W, raw_threshold_bytes, d_out, d_
     _check(lib().bfsc_compress_batch(_ptr(d_ids), _ptr(d_in_offsets), n_buf, W, raw_threshold_bytes, _ptr(d_out),
                                      d_out.numel(), _ptr(d_out_offsets), _ptr(d_workspace), d_workspace.numel(),
                                      _ptr(d_status), ctypes.c_void_p(_stream())), "bfsc_compress_batch")
+
+
+def compress_batch_codec(codec, d_ids, d_in_offsets, n_buf, W, raw_threshold_bytes, d_out, d_out_offsets, d_workspace,
+                         d_status):
+    _check(lib().bfsc_compress_batch_codec(codec, _ptr(d_ids), _ptr(d_in_offsets), n_buf, W, raw_threshold_bytes,
+                                           _ptr(d_out), d_out.numel(), _ptr(d_out_offsets), _ptr(d_workspace),
+                                           d_workspace.numel(), _ptr(d_status), ctypes.c_void_p(_stream())),
+           "bfsc_compress_batch_codec")
 
 
 def decompress_batch(d_in, d_in_offsets, n_buf, W, d_ids, d_id_offsets, d_workspace, d_status):

@@ -12,7 +12,7 @@ static size_t bound_one(size_t n, int W) {
 }
 }  // namespace bfsc
 
-extern "C" uint32_t bfsc_version(void) { return (1u << 16) | 1u; }
+extern "C" uint32_t bfsc_version(void) { return (1u << 16) | 2u; }   // abi revision 2: bfsc_compress[_batch]_codec, mode 2
 
 extern "C" uint64_t bfsc_kernel_launches(void) { return bfsc::g_launches; }
 

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
                     const unsigned long long total = (unsigned long long)h1[u].y << 32 | h1[u].x;
                     const unsigned long long nb = h1[u].z;
                     if (h0[u].x != 0x43534642u || (h0[u].y & 0xffu) != 1u || ((h0[u].y >> 8) & 0xffu) != (uint32_t)W ||
-                        mode > 1u || (h0[u].y >> 24) != 0u)
+                        mode > 2u || (h0[u].y >> 24) != 0u)                  // mode 2 (BP128-D1) decodes as mode 1: FORMAT.md §7
                         ok = false;
                     else if (total > avail[u] || (total & 15) || total < 32) ok = false;
                     else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
             n1 = (unsigned long long)h0.w << 32 | h0.z;
             total = (unsigned long long)h1.y << 32 | h1.x;
             nb = h1.z;
-            if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W || mode > 1u ||
+            if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W || mode > 2u ||
                 (h0.y >> 24) != 0u)
                 ok = false;
             else if (total > a.in_single || (total & 15) || total < 32) ok = false;

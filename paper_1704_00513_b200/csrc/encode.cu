@@ -14,6 +14,7 @@ struct EncArgs {
     unsigned long long n_single;
     uint32_t n_buf;
     uint32_t grid;                      // CTAs of k_enc_tiles: their first tiles are blockIdx.x (+ grid), tickets start at 2 grid
+    uint32_t codec;                     // encoder rule = mode byte: 1 PFOR-D1 (E2: size argmin), 2 BP128-D1 (b = maxw, no exceptions; FORMAT.md §7)
     unsigned long long thr;             // raw threshold in bytes
     unsigned char* out;
     unsigned long long out_cap;
@@ -493,7 +494,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                         if (at != kSkip) {
                             uint4 h0, h1;
                             h0.x = 0x43534642u;                                   // "BFSC"
-                            h0.y = 1u | ((uint32_t)W << 8) | (1u << 16);
+                            h0.y = 1u | ((uint32_t)W << 8) | (a.codec << 16);     // mode = the encoder rule
                             h0.z = (uint32_t)a.n_single; h0.w = (uint32_t)(a.n_single >> 32);
                             h1.x = (uint32_t)tot; h1.y = (uint32_t)(tot >> 32);
                             h1.z = (uint32_t)nb_single; h1.w = 0;
@@ -585,9 +586,10 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 for (int i = 0; i < 32; i++) o |= d[i];
                 const uint32_t top = 32 - __clz(quad_or(o)); key = ((16u + 16u * top) << 14) | ((64u - top) << 7); }
 #else
-            if (!wide) key = quad_choose_b<W>(d);                        // E2
+            if (!wide) key = a.codec == BFSC_CODEC_BP128 ? quad_max_width_key(d) : quad_choose_b<W>(d);   // E2
 #endif
-            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (ImgCfg<W>::kSlotChunks * 16)));
+            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (ImgCfg<W>::kSlotChunks * 16)),
+                                     a.codec == BFSC_CODEC_BP128);
             if (m <= 0) key = 0;
             if (l == 0) s_key[kp][j] = key;
             {   // The tile's aggregate goes out as soon as the LAST worker warp has its sizes — not when the scan
@@ -737,7 +739,7 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
             const unsigned long long nb = f1 - f0;
             uint4 h0, h1;
             h0.x = 0x43534642u;                                           // "BFSC"
-            h0.y = 1u | ((uint32_t)W << 8) | ((raw ? 0u : 1u) << 16);
+            h0.y = 1u | ((uint32_t)W << 8) | ((raw ? 0u : a.codec) << 16);
             h0.z = (uint32_t)n; h0.w = (uint32_t)(n >> 32);
             h1.x = (uint32_t)total; h1.y = (uint32_t)(total >> 32);
             h1.z = (uint32_t)nb; h1.w = 0;
@@ -813,17 +815,18 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     return BFSC_OK;
 }
 
-static bfsc_status encode_common(const void* d_ids, const uint64_t* d_in_off, size_t n_single, size_t n_buf,
+static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_off, size_t n_single, size_t n_buf,
                                  bfsc_dtype t, size_t thr, void* d_out, size_t out_cap, uint64_t* d_out_off,
                                  uint64_t* d_out_total, void* ws, size_t ws_bytes, uint32_t* d_status, void* stream) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
+    if (codec != BFSC_CODEC_PFOR && codec != BFSC_CODEC_BP128) return BFSC_ERR_INVALID_ARG;
     if (!d_out || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
     if (((uintptr_t)d_ids & 15) || ((uintptr_t)d_out & 15) || ((uintptr_t)ws & 15)) return BFSC_ERR_INVALID_ARG;
     if (!d_ids && (d_in_off || n_single)) return BFSC_ERR_INVALID_ARG;
     EncArgs a;
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.ids = d_ids; a.in_off = (const unsigned long long*)d_in_off; a.n_single = n_single;
-    a.n_buf = (uint32_t)n_buf; a.grid = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
+    a.n_buf = (uint32_t)n_buf; a.grid = 0; a.codec = (uint32_t)codec; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
     a.out_off = (unsigned long long*)d_out_off; a.out_total = (unsigned long long*)d_out_total; a.status = d_status;
     return t == BFSC_U32 ? launch_encode<32>(a, (cudaStream_t)stream) : launch_encode<64>(a, (cudaStream_t)stream);
 }
@@ -836,19 +839,35 @@ extern "C" int bfsc_debug_trace(unsigned long long* h_out, size_t n_words) {
 }
 #endif
 
+extern "C" bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, size_t n_ids, bfsc_dtype t,
+                                           size_t raw_threshold_bytes, void* d_out, size_t out_capacity,
+                                           uint64_t* d_out_bytes, void* d_workspace, size_t workspace_bytes,
+                                           uint32_t* d_status, void* cuda_stream) {
+    if (!d_out_bytes) return BFSC_ERR_INVALID_ARG;
+    return bfsc::encode_common(codec, d_ids, nullptr, n_ids, 1, t, raw_threshold_bytes, d_out, out_capacity, nullptr,
+                               d_out_bytes, d_workspace, workspace_bytes, d_status, cuda_stream);
+}
+
 extern "C" bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
                                      void* d_out, size_t out_capacity, uint64_t* d_out_bytes, void* d_workspace,
                                      size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
-    if (!d_out_bytes) return BFSC_ERR_INVALID_ARG;
-    return bfsc::encode_common(d_ids, nullptr, n_ids, 1, t, raw_threshold_bytes, d_out, out_capacity, nullptr,
-                               d_out_bytes, d_workspace, workspace_bytes, d_status, cuda_stream);
+    return bfsc_compress_codec(BFSC_CODEC_PFOR, d_ids, n_ids, t, raw_threshold_bytes, d_out, out_capacity, d_out_bytes,
+                               d_workspace, workspace_bytes, d_status, cuda_stream);
+}
+
+extern "C" bfsc_status bfsc_compress_batch_codec(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_offsets,
+                                                 size_t n_buf, bfsc_dtype t, size_t raw_threshold_bytes, void* d_out,
+                                                 size_t out_capacity, uint64_t* d_out_offsets, void* d_workspace,
+                                                 size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
+    if (!d_in_offsets || !d_out_offsets) return BFSC_ERR_INVALID_ARG;
+    return bfsc::encode_common(codec, d_ids, d_in_offsets, 0, n_buf, t, raw_threshold_bytes, d_out, out_capacity,
+                               d_out_offsets, nullptr, d_workspace, workspace_bytes, d_status, cuda_stream);
 }
 
 extern "C" bfsc_status bfsc_compress_batch(const void* d_ids, const uint64_t* d_in_offsets, size_t n_buf,
                                            bfsc_dtype t, size_t raw_threshold_bytes, void* d_out,
                                            size_t out_capacity, uint64_t* d_out_offsets, void* d_workspace,
                                            size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
-    if (!d_in_offsets || !d_out_offsets) return BFSC_ERR_INVALID_ARG;
-    return bfsc::encode_common(d_ids, d_in_offsets, 0, n_buf, t, raw_threshold_bytes, d_out, out_capacity,
-                               d_out_offsets, nullptr, d_workspace, workspace_bytes, d_status, cuda_stream);
+    return bfsc_compress_batch_codec(BFSC_CODEC_PFOR, d_ids, d_in_offsets, n_buf, t, raw_threshold_bytes, d_out,
+                                     out_capacity, d_out_offsets, d_workspace, workspace_bytes, d_status, cuda_stream);
 }

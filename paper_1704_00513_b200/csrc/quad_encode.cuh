@@ -104,6 +104,16 @@ __device__ __forceinline__ uint32_t quad_choose_b(const uint32_t (&d)[32]) {
     return best;
 }
 
+// ---- E2 of the no-exception codec (FORMAT.md §7, mode 2 = BP128-D1; the thesis's codec class S4-BP128,
+// PAPER.md L1052-1056): b = width of the block's widest delta (eq. 6), n_exc = 0. Same key layout.
+__device__ __forceinline__ uint32_t quad_max_width_key(const uint32_t (&d)[32]) {
+    uint32_t o = 0;
+#pragma unroll
+    for (int i = 0; i < 32; i++) o |= d[i];
+    const uint32_t top = 32u - (uint32_t)__clz(quad_or(o));
+    return ((16u + 16u * top) << 14) | ((64u - top) << 7);
+}
+
 // ---- E4: staging geometry ----------------------------------------------------------------
 // Per warp: a staging area (the batch's 128 deltas per block, row-major) and an image area (the
 // assembled block: header | payload | exceptions). Both hold 8 slots of 33 16-byte chunks; slot q

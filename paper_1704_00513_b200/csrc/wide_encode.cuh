@@ -61,7 +61,9 @@ __device__ __noinline__ void late_emit(const typename IdT<W>::T* __restrict__ x,
 // E2 for a warp batch with wide deltas: exact argmin of the block size over b in 0..maxw, ties to
 // the largest b (FORMAT.md §2), from a 65-bin histogram of the widths in shared memory. Whole warp
 // calls; raw = the quad's staged IDs (block's first ID at raw[0]); hist = 65 words of scratch per quad.
-__device__ __noinline__ uint32_t wide_choose_b(const uint64_t* __restrict__ raw, int m, uint32_t* __restrict__ hist) {
+// no_exc: the BP128 rule (FORMAT.md §7): b = maxw, n_exc = 0.
+__device__ __noinline__ uint32_t wide_choose_b(const uint64_t* __restrict__ raw, int m, uint32_t* __restrict__ hist,
+                                               bool no_exc) {
     const int lane = threadIdx.x & 31, l = lane & 3;
     for (int k = l; k < 65; k += 4) hist[k] = 0;
     __syncwarp();
@@ -75,7 +77,7 @@ __device__ __noinline__ uint32_t wide_choose_b(const uint64_t* __restrict__ raw,
         int maxw = 64;
         while (maxw > 0 && hist[maxw] == 0) maxw--;
         uint32_t n = 0;
-        for (int b = maxw; b >= 0; b--) {                        // descending: a tie keeps the larger b
+        for (int b = maxw; b >= (no_exc ? maxw : 0); b--) {      // descending: a tie keeps the larger b
             const uint32_t key = ((16u + 16u * (uint32_t)b + exc_bytes<64>(n)) << 14) | ((64u - (uint32_t)b) << 7) | n;
             if ((key >> 14) < (best >> 14)) best = key;
             n += hist[b];

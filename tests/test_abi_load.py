@@ -37,7 +37,7 @@ def test_bounds_match_format(L, oracle_mod):
             assert binding.compress_bound(n, W) >= oracle_mod.compress_bound(n, W)
     assert binding.batch_compress_bound([0, 5, 300], 32) == sum(binding.compress_bound(n, 32) for n in (0, 5, 300))
     assert binding.workspace_bytes(1 << 24, 1, 32) > (1 << 24) // 128 // 64 * 64   # one 64-byte look-back state per 64-block tile
-    assert L.bfsc_version() >> 16 == 1
+    assert L.bfsc_version() >> 16 == 1 and L.bfsc_version() & 0xffff >= 2
 
 
 def test_host_arg_validation(L):
@@ -48,6 +48,9 @@ def test_host_arg_validation(L):
     assert rc == 1
     rc = L.bfsc_decompress(None, 0, 32, None, 0, None, None, 0, None, None)
     assert rc == 1
+    for bad_codec in (0, 3):                       # bfsc_codec: 1 = PFOR, 2 = BP128 (include/bfsc.h)
+        assert L.bfsc_compress_codec(bad_codec, None, 0, 32, 0, None, 0, None, None, 0, None, None) == 1
+        assert L.bfsc_compress_batch_codec(bad_codec, None, None, 1, 32, 0, None, 0, None, None, 0, None, None) == 1
 
 
 def test_no_fallback_when_library_missing(monkeypatch):

@@ -24,7 +24,11 @@ def _np(t, W):
     return a.view(np.uint32) if W == 32 else a.view(np.uint64)
 
 
-def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True):
+PFOR, BP128 = 1, 2           # bfsc_codec: encoder rule (FORMAT.md §7)
+CODECS = [PFOR, BP128]
+
+
+def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True, codec=PFOR):
     """ids_t: CPU tensor (int32/int64 bit pattern), off_t: int64 offsets. Returns GPU bytes."""
     dev = torch.device("cuda")
     n, n_buf = ids_t.numel(), off_t.numel() - 1
@@ -37,7 +41,10 @@ def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True):
     out_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
     ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
     status = torch.zeros(1, dtype=torch.int32, device=dev)
-    B.compress_batch(d_ids, d_off, n_buf, W, thr, out, out_off, ws, status)
+    if codec == PFOR:
+        B.compress_batch(d_ids, d_off, n_buf, W, thr, out, out_off, ws, status)
+    else:
+        B.compress_batch_codec(codec, d_ids, d_off, n_buf, W, thr, out, out_off, ws, status)
     torch.cuda.synchronize()
     assert int(status.item()) == 0
     total = int(out_off[-1].item())
@@ -46,7 +53,8 @@ def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True):
     gpu_bytes = out[:total].cpu().numpy()
     gpu_off = out_off.cpu().numpy().astype(np.uint64)
     if check_oracle:
-        ref, ref_off = oracle_mod.compress_batch(_np(ids_t, W), off_t.numpy().astype(np.uint64), thr, threads=8)
+        ref, ref_off = oracle_mod.compress_batch(_np(ids_t, W), off_t.numpy().astype(np.uint64), thr,
+                                                 threads=8 if codec == PFOR else 0, codec=codec)
         assert np.array_equal(gpu_off, ref_off)
         if not np.array_equal(gpu_bytes, ref):
             bad = int(np.nonzero(gpu_bytes != ref)[0][0])
@@ -64,7 +72,7 @@ def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True):
     return gpu_bytes, gpu_off
 
 
-def run_single(B, oracle_mod, ids_t, W, thr):
+def run_single(B, oracle_mod, ids_t, W, thr, codec=PFOR):
     dev = torch.device("cuda")
     n = ids_t.numel()
     cap = B.compress_bound(n, W)
@@ -73,11 +81,14 @@ def run_single(B, oracle_mod, ids_t, W, thr):
     nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
     ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
     status = torch.zeros(1, dtype=torch.int32, device=dev)
-    B.compress(d_ids, n, W, thr, out, nbytes, ws, status)
+    if codec == PFOR:
+        B.compress(d_ids, n, W, thr, out, nbytes, ws, status)
+    else:
+        B.compress_codec(codec, d_ids, n, W, thr, out, nbytes, ws, status)
     torch.cuda.synchronize()
     assert int(status.item()) == 0
     total = int(nbytes.item())
-    ref = oracle_mod.compress(_np(ids_t, W), thr)
+    ref = oracle_mod.compress(_np(ids_t, W), thr, codec=codec)
     assert total == len(ref)
     assert np.array_equal(out[:total].cpu().numpy(), ref)
     back = torch.empty(max(n, 4), dtype=ids_t.dtype, device=dev)
@@ -88,18 +99,20 @@ def run_single(B, oracle_mod, ids_t, W, thr):
     assert torch.equal(back[:n].cpu(), ids_t)
 
 
+@pytest.mark.parametrize("codec", CODECS)
 @pytest.mark.parametrize("W", [32, 64])
-def test_single_edge_sizes(B, oracle_mod, W):
+def test_single_edge_sizes(B, oracle_mod, W, codec):
     for n in (0, 1, 2, 127, 128, 129, 255, 256, 257, 1000, 4097, 128 * 300 + 5):
         for mean in (1.0, 2.0, 256.0):
             t = streams.gap_stream(n, mean, seed=11, W=W)
-            run_single(B, oracle_mod, t, W, 0)
-    run_single(B, oracle_mod, streams.gap_stream(100, 2.0, seed=1, W=W), W, 1024)   # RAW
-    run_single(B, oracle_mod, streams.gap_stream(300, 2.0, seed=1, W=W), W, 1024)
+            run_single(B, oracle_mod, t, W, 0, codec=codec)
+    run_single(B, oracle_mod, streams.gap_stream(100, 2.0, seed=1, W=W), W, 1024, codec=codec)   # RAW
+    run_single(B, oracle_mod, streams.gap_stream(300, 2.0, seed=1, W=W), W, 1024, codec=codec)
 
 
+@pytest.mark.parametrize("codec", CODECS)
 @pytest.mark.parametrize("W", [32, 64])
-def test_adversarial_values(B, oracle_mod, W):
+def test_adversarial_values(B, oracle_mod, W, codec):
     rng = np.random.default_rng(W)
     n = 128 * 40 + 77
     dt = np.uint32 if W == 32 else np.uint64
@@ -127,13 +140,14 @@ def test_adversarial_values(B, oracle_mod, W):
         t = torch.from_numpy(arr.view(np.int32 if W == 32 else np.int64).copy()).to(tdt)
         off = torch.tensor([0, n], dtype=torch.int64)
         try:
-            run_batch(B, oracle_mod, t, off, W, 0)
+            run_batch(B, oracle_mod, t, off, W, 0, codec=codec)
         except AssertionError as e:
             raise AssertionError(f"{name}: {e}")
 
 
+@pytest.mark.parametrize("codec", CODECS)
 @pytest.mark.parametrize("W", [32, 64])
-def test_batch_ragged(B, oracle_mod, W):
+def test_batch_ragged(B, oracle_mod, W, codec):
     counts = streams.log_uniform_counts(300, 6, 14, W, seed=5)
     counts[0] = 0
     counts[5] = 0
@@ -143,10 +157,10 @@ def test_batch_ragged(B, oracle_mod, W):
     counts[299] = 0
     ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=W)
     for thr in (0, 1024):
-        run_batch(B, oracle_mod, ids, off, W, thr)
+        run_batch(B, oracle_mod, ids, off, W, thr, codec=codec)
     # unaligned buffer starts (odd element offsets) exercise the scalar load/store path
     ids2, off2 = streams.batch_of_streams(torch.tensor([3, 130, 257, 1, 1000]), 2.0, seed=6, W=W)
-    run_batch(B, oracle_mod, ids2, off2, W, 0)
+    run_batch(B, oracle_mod, ids2, off2, W, 0, codec=codec)
 
 
 @pytest.mark.parametrize("W", [32, 64])
@@ -165,32 +179,37 @@ def test_batch_alignments_and_many_buffers(B, oracle_mod, W):
     sel = torch.rand(hi - lo, generator=g) < 0.02
     ids[lo:hi][sel] += 1 << 20
     for thr in (0, 1024):
-        run_batch(B, oracle_mod, ids, off, W, thr)
+        for codec in CODECS:
+            run_batch(B, oracle_mod, ids, off, W, thr, codec=codec)
     many = torch.randint(0, 300, (9000,), generator=g)
     ids2, off2 = streams.batch_of_streams(many, 16.0, seed=10, W=W)
     for thr in (0, 1024):
-        run_batch(B, oracle_mod, ids2, off2, W, thr)
+        for codec in CODECS:
+            run_batch(B, oracle_mod, ids2, off2, W, thr, codec=codec)
 
 
-def test_tiny_rmat_config1(B, oracle_mod):
+@pytest.mark.parametrize("codec", CODECS)
+def test_tiny_rmat_config1(B, oracle_mod, codec):
     """BASELINE config 1: scale 12, 8 roots, 4 buffers by v mod 4, threshold 0, single + batch API."""
     G = rmat.Graph(12, 16, seed=1)
     for root in G.roots(8, seed=1):
         for f in G.bfs_frontiers(root):
             vals, off = streams.split_mod(f, 4)
             ids = streams.as_ids(vals, 32)
-            run_batch(B, oracle_mod, ids, off, 32, 0)
+            run_batch(B, oracle_mod, ids, off, 32, 0, codec=codec)
             for q in range(4):
-                run_single(B, oracle_mod, ids[int(off[q]):int(off[q + 1])].clone(), 32, 0)
+                run_single(B, oracle_mod, ids[int(off[q]):int(off[q + 1])].clone(), 32, 0, codec=codec)
 
 
-def test_streams_config2_reduced(B, oracle_mod):
+@pytest.mark.parametrize("codec", CODECS)
+def test_streams_config2_reduced(B, oracle_mod, codec):
     """config 2 recipes at 2^18 IDs (several thousand blocks, oracle in seconds)."""
     n = (1 << 18) + 37
     for mean, outl in ((2.0, 0.0), (256.0, 0.0), (256.0, 0.01)):
         for W in (32, 64):
             t = streams.gap_stream(n, mean, seed=2, W=W, outlier_frac=outl)
-            run_batch(B, oracle_mod, t, torch.tensor([0, n], dtype=torch.int64), W, 0)
+            run_batch(B, oracle_mod, t, torch.tensor([0, n], dtype=torch.int64), W, 0, codec=codec)
+            run_single(B, oracle_mod, t, W, 0, codec=codec)
 
 
 def test_errors_reported_on_device(B):
@@ -249,24 +268,26 @@ def test_host_api_roundtrip(B, oracle_mod):
         assert torch.equal(h_back, t)
 
 
-def test_rmat_config3_reduced(B, oracle_mod):
+@pytest.mark.parametrize("codec", CODECS)
+def test_rmat_config3_reduced(B, oracle_mod, codec):
     """config 3 recipe at scale 16: per-level frontiers, 16 buffers by contiguous vertex range, one
     batched call per level, 1 KB raw threshold (first/last levels go RAW or empty)."""
     G = rmat.Graph(16, 16, seed=3)
     for root in G.roots(2, seed=3):
         for f in G.bfs_frontiers(root):
             vals, off = streams.split_block(f, 16, 1 << 16)
-            run_batch(B, oracle_mod, streams.as_ids(vals, 32), off, 32, 1024)
+            run_batch(B, oracle_mod, streams.as_ids(vals, 32), off, 32, 1024, codec=codec)
 
 
-def test_rmat_config4_reduced(B, oracle_mod):
+@pytest.mark.parametrize("codec", CODECS)
+def test_rmat_config4_reduced(B, oracle_mod, codec):
     """config 4 recipe at scale 16: u64 IDs, 64 destination buffers (8x8 partition read as a 64-way
     block partition), 1 KB threshold."""
     G = rmat.Graph(16, 16, seed=4)
     for root in G.roots(2, seed=4):
         for f in G.bfs_frontiers(root):
             vals, off = streams.split_block(f, 64, 1 << 16)
-            run_batch(B, oracle_mod, streams.as_ids(vals, 64), off, 64, 1024)
+            run_batch(B, oracle_mod, streams.as_ids(vals, 64), off, 64, 1024, codec=codec)
 
 
 def test_rmat_config3_full_size_one_root(B, oracle_mod):
@@ -344,7 +365,7 @@ def test_random_batches_soak(B, oracle_mod):
             run_single(B, oracle_mod, ids, W, thr)
 
 
-def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256):
+def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256, codec=PFOR):
     """One large single stream through bfsc_compress / bfsc_decompress: decoded IDs equal the input everywhere;
     directory walk (strictly increasing, sizes recomputed from the block headers, total = header + directory +
     blocks); `samples` blocks memcmp-equal to the oracle's encoding of the same 128 IDs (blocks are
@@ -357,7 +378,10 @@ def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256):
     nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
     ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
     status = torch.zeros(1, dtype=torch.int32, device=dev)
-    B.compress(ids, n, W, 0, out, nbytes, ws, status)
+    if codec == PFOR:
+        B.compress(ids, n, W, 0, out, nbytes, ws, status)
+    else:
+        B.compress_codec(codec, ids, n, W, 0, out, nbytes, ws, status)
     back = torch.empty(n, dtype=ids.dtype, device=dev)
     n_out = torch.zeros(1, dtype=torch.int64, device=dev)
     B.decompress(out, cap, W, back, n_out, ws, status)
@@ -368,7 +392,7 @@ def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256):
     total = int(nbytes.item())
     s = out[:total].cpu().numpy()
     nb = (n + 127) // 128
-    assert s[:4].tobytes() == b"BFSC" and s[4] == 1 and s[5] == W and s[6] == 1
+    assert s[:4].tobytes() == b"BFSC" and s[4] == 1 and s[5] == W and s[6] == codec
     assert int(s[8:16].view(np.uint64)[0]) == n and int(s[16:24].view(np.uint64)[0]) == total
     assert int(s[24:28].view(np.uint32)[0]) == nb
     d = s[32:32 + 4 * (nb + 1)].view(np.uint32).astype(np.int64)
@@ -379,16 +403,17 @@ def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256):
     assert np.array_equal((d[1:] - d[:-1]) * 16, 16 + 16 * b + exc)
     host = ids.cpu().numpy().view(np.uint32 if W == 32 else np.uint64)
     for k in rng.integers(0, nb, size=samples):
-        ref = oracle_mod.compress(host[128 * k:128 * k + 128], 0)
+        ref = oracle_mod.compress(host[128 * k:128 * k + 128], 0, codec=codec)
         assert np.array_equal(s[d[k] * 16:d[k + 1] * 16], ref[48:]), f"block {k} differs from the oracle"
 
 
-def test_config2_full_size_sampled(B, oracle_mod):
+@pytest.mark.parametrize("codec", CODECS)
+def test_config2_full_size_sampled(B, oracle_mod, codec):
     """BASELINE config 2 at its full size (2^24 IDs, the launch configuration bench.py times)."""
     rng = np.random.default_rng(7)
     for sub, (mean, outl) in enumerate(((2.0, 0.0), (256.0, 0.0), (256.0, 0.01))):
         ids = streams.gap_stream(1 << 24, mean, seed=2, W=32, outlier_frac=outl, sub=sub, device=torch.device("cuda"))
-        _full_size_sampled(B, oracle_mod, ids, 32, rng)
+        _full_size_sampled(B, oracle_mod, ids, 32, rng, codec=codec)
 
 
 def test_config5_largest_buffers_sampled(B, oracle_mod):
