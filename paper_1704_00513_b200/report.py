@@ -3,7 +3,8 @@
     python -m paper_1704_00513_b200.report --config 3            # R-MAT 22, u32, 16 buffers/level, 1 KB threshold
     python -m paper_1704_00513_b200.report --config 4            # R-MAT 25, u64, 64 buffers/level
     python -m paper_1704_00513_b200.report --config 5            # message-size sweep + 4096-buffer batch
-    (--scale / --roots shrink configs 3 and 4 for a quick look)
+    (--scale / --roots shrink configs 3 and 4 for a quick look; --codec bp128 runs the same cases under the
+     no-exception rule, FORMAT.md §7 — the codec class the thesis ran)
 
 Every call goes through the C ABI (binding.py); each timed call is preceded by an L2 flush (a 256 MB
 memset outside the timed region) and timed with CUDA events; every decoded batch is compared with its
@@ -37,8 +38,8 @@ def peak_gbs():
 
 
 class Runner:
-    def __init__(self, dev, reps=5):
-        self.dev, self.reps = dev, reps
+    def __init__(self, dev, reps=5, codec=B.CODEC_PFOR):
+        self.dev, self.reps, self.codec = dev, reps, codec
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
         self.peak = peak_gbs()
 
@@ -97,14 +98,14 @@ class Runner:
         if single:                                           # one buffer: the single-buffer entry points
             nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
             n_out = torch.zeros(1, dtype=torch.int64, device=dev)
-            enc, enc_iso = self._time([(lambda c=c: B.compress(pads[c], n, W, thr, outs[c], nbytes, ws, status)) for c in range(copies)])
+            enc, enc_iso = self._time([(lambda c=c: B.compress_codec(self.codec, pads[c], n, W, thr, outs[c], nbytes, ws, status)) for c in range(copies)])
             dec, dec_iso = self._time([(lambda c=c: B.decompress(outs[c], cap, W, backs[c], n_out, ws, status)) for c in range(copies)])
             assert int(status.item()) == 0 and int(n_out.item()) == n
             assert torch.equal(backs[copies - 1][:n], ids), "decode != input"
             comp = int(nbytes.item())
             return {"n": n, "n_buf": 1, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec,
                     "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound}
-        enc, enc_iso = self._time([(lambda c=c: B.compress_batch(pads[c], off, n_buf, W, thr, outs[c], out_off, ws, status)) for c in range(copies)])
+        enc, enc_iso = self._time([(lambda c=c: B.compress_batch_codec(self.codec, pads[c], off, n_buf, W, thr, outs[c], out_off, ws, status)) for c in range(copies)])
         dec, dec_iso = self._time([(lambda c=c: B.decompress_batch(outs[c], out_off, n_buf, W, backs[c], id_off, ws, status)) for c in range(copies)])
         assert int(status.item()) == 0
         assert torch.equal(backs[copies - 1][:n], ids) and torch.equal(id_off, off), "decode != input"
@@ -182,11 +183,13 @@ def main():
     ap.add_argument("--scale", type=int, default=0)
     ap.add_argument("--roots", type=int, default=0)
     ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--codec", default="pfor", choices=["pfor", "bp128"], help="encoder rule (bfsc_codec)")
     a = ap.parse_args()
     assert torch.cuda.is_available(), "needs a CUDA device (there is no CPU fallback)"
     dev = torch.device("cuda:0")
     B.lib()
-    R = Runner(dev, a.reps)
+    R = Runner(dev, a.reps, B.CODEC_BP128 if a.codec == "bp128" else B.CODEC_PFOR)
+    print(f"encoder rule: {'BP128-D1 (mode 2, no exceptions)' if a.codec == 'bp128' else 'PFOR-D1 (mode 1)'}\n")
     if a.config == 3:
         rmat_config(R, a.scale or 22, 3, 32, 16, a.roots or 16, 1024)
     elif a.config == 4:
