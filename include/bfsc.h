@@ -21,7 +21,9 @@
  *    everything a call reads or writes. The kernels are launched with programmatic dependent
  *    launch: a kernel may become resident while its predecessor in the stream still runs, but
  *    waits for that predecessor to complete before it touches memory (back-to-back calls pay
- *    no launch gap).
+ *    no launch gap). Because a call only enqueues kernels, a sequence of calls may be captured
+ *    in a CUDA graph (stream capture) and replayed, after one call of each kind outside the
+ *    capture (one-time function attributes); the launch counter then counts the capture only.
  *  - Concurrency: bfsc_compress / bfsc_compress_batch run a persistent grid that fills the GPU
  *    and whose CTAs wait for one another (device-wide scan of block sizes). Issue compress
  *    calls of one device on ONE stream at a time: two compress grids that become resident

@@ -365,6 +365,64 @@ def test_random_batches_soak(B, oracle_mod):
             run_single(B, oracle_mod, ids, W, thr)
 
 
+@pytest.mark.parametrize("W", [32, 64])
+def test_calls_replay_from_a_cuda_graph(B, oracle_mod, W):
+    """include/bfsc.h: the device calls only enqueue kernels on the given stream (no allocation, no
+    synchronisation), so a caller may capture them in a CUDA graph. One graph holding compress_batch +
+    decompress_batch + compress + decompress is replayed on three different contents of the same buffers;
+    every replay must give the oracle's bytes and the input back."""
+    dev = torch.device("cuda")
+    counts = torch.tensor([5000, 0, 129, 40000, 1, 300, 12800])
+    n, n_buf = int(counts.sum()), counts.numel()
+    off = torch.zeros(n_buf + 1, dtype=torch.int64)
+    off[1:] = torch.cumsum(counts, 0)
+    dt = torch.int32 if W == 32 else torch.int64
+    d_ids = torch.zeros(n + 4, dtype=dt, device=dev)
+    d_off = off.to(dev)
+    cap = B.batch_compress_bound(counts.tolist(), W)
+    out = torch.zeros(cap, dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    back = torch.zeros(n + 4, dtype=dt, device=dev)
+    id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    cap1 = B.compress_bound(n, W)
+    out1 = torch.zeros(cap1, dtype=torch.uint8, device=dev)
+    nbytes1 = torch.zeros(1, dtype=torch.int64, device=dev)
+    back1 = torch.zeros(n + 4, dtype=dt, device=dev)
+    n_out1 = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    def calls():
+        B.compress_batch(d_ids, d_off, n_buf, W, 1024, out, out_off, ws, status)
+        B.decompress_batch(out, out_off, n_buf, W, back, id_off, ws, status)
+        B.compress(d_ids, n, W, 0, out1, nbytes1, ws, status)
+        B.decompress(out1, cap1, W, back1, n_out1, ws, status)
+
+    calls()                                                  # first use outside the capture (one-time attribute set-up)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream(device=dev)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            calls()
+    torch.cuda.synchronize()
+    for rep, mean in enumerate((2.0, 300.0, 70000.0)):
+        ids, off2 = streams.batch_of_streams(counts, mean, seed=100 + rep, W=W)
+        assert torch.equal(off2, off)
+        d_ids[:n] = ids.to(dev)
+        out.zero_(); back.fill_(-1); out1.zero_(); back1.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0
+        ref, ref_off = oracle_mod.compress_batch(_np(ids, W), off.numpy().astype(np.uint64), 1024)
+        assert np.array_equal(out_off.cpu().numpy().astype(np.uint64), ref_off)
+        assert np.array_equal(out[:len(ref)].cpu().numpy(), ref)
+        assert torch.equal(back[:n].cpu(), ids) and torch.equal(id_off.cpu(), off)
+        ref1 = oracle_mod.compress(_np(ids, W), 0)
+        assert int(nbytes1.item()) == len(ref1) and np.array_equal(out1[:len(ref1)].cpu().numpy(), ref1)
+        assert int(n_out1.item()) == n and torch.equal(back1[:n].cpu(), ids)
+
+
 def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256, codec=PFOR):
     """One large single stream through bfsc_compress / bfsc_decompress: decoded IDs equal the input everywhere;
     directory walk (strictly increasing, sizes recomputed from the block headers, total = header + directory +
