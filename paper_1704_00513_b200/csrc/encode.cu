@@ -461,7 +461,17 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             }
             __syncwarp();
 
-            // final offsets, directory entries, stream starts
+            // Stream starts of the streams that BEGIN in this tile go out first, before any lane below polls for
+            // the start of a stream that began in an earlier tile: a publish never waits behind a poll.
+            if constexpr (kBatch) {
+#pragma unroll
+                for (int h = 0; h < kPer; h++) {
+                    const int jj = kPer * lane + h;
+                    if (jj < kTileR && g0 + jj < total && bf_first[h] == g0 + jj)
+                        st_volatile_u64(&a.ws.stream_start[bf_i[h]], bf_f0[h] + 16ull * (excl + offs[h]) + 1);
+                }
+            }
+            // final offsets, directory entries
 #pragma unroll
             for (int h = 0; h < kPer; h++) {
                 const int jj = kPer * lane + h;
@@ -480,7 +490,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                             do { S = ld_volatile_u64(&a.ws.stream_start[i]); } while (S == 0);
                             S -= 1;
                         }
-                        if (g == first) st_volatile_u64(&a.ws.stream_start[i], S + 1);
                     }
                     at = f1 + 16ull * (excl + off);
                     if (at + bytes <= a.out_cap) {
