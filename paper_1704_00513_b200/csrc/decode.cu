@@ -1,7 +1,7 @@
 // decode.cu — bfsc_decompress / bfsc_decompress_batch (steps D0-D5).
 //
 // Launches per call: single stream: k_dec_tiles alone (it parses the stream header itself);
-// batch: k_dec_plan -> k_dec_tiles, chained with programmatic dependent launch.
+// batch: [k_dec_headers ->] k_dec_plan -> k_dec_blocks -> k_dec_tiles, chained with programmatic dependent launch.
 #include "block_decode.cuh"
 #include "quad_decode.cuh"
 
