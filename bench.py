@@ -284,6 +284,47 @@ def run_ours(args, rank, local_rank, world):
     assert int(status.item()) == 0, f"device status {int(status.item())}"
     value = whole_job_value(2 * S * raw_bytes, world, ms_step * 1e-3) / 1e9
 
+    # ---- the batched path (BASELINE configs[4], batch part): 4096 buffers of 256 B - 64 KB (log-uniform), gaps of
+    # mean 16, u32, one bfsc_compress_batch / bfsc_decompress_batch per call; reported beside the headline, not in it
+    batch = None
+    if rank == 0 and args.log2n == LOG2_N:
+        counts = streams.log_uniform_counts(4096, 8, 16, 32, seed=5)
+        b_ids, b_off = streams.batch_of_streams(counts, 16.0, seed=5, W=W, device=dev)
+        b_ids, b_off = b_ids.to(dev), b_off.to(dev)
+        bn, nbuf = b_ids.numel(), b_off.numel() - 1
+        bcap = B.batch_compress_bound(counts.tolist(), W)
+        kB = 6                                               # rotating copies: 6 x (49 MB in + out) > 2 x L2
+        bi = [b_ids] + [b_ids.clone() for _ in range(kB - 1)]
+        bo = [torch.empty(bcap, dtype=torch.uint8, device=dev) for _ in range(kB)]
+        bb = [torch.empty(bn, dtype=b_ids.dtype, device=dev) for _ in range(kB)]
+        b_out_off = torch.zeros(nbuf + 1, dtype=torch.int64, device=dev)
+        b_id_off = torch.zeros(nbuf + 1, dtype=torch.int64, device=dev)
+        bws = torch.empty(B.workspace_bytes(bn, nbuf, W), dtype=torch.uint8, device=dev)
+
+        def run_b(call, reps_b=10):
+            for c in range(kB):
+                call(c)
+            torch.cuda.synchronize()
+            a0, a1 = mk(), mk()
+            a0.record()
+            for _ in range(reps_b):
+                for c in range(kB):
+                    call(c)
+            a1.record()
+            torch.cuda.synchronize()
+            return a0.elapsed_time(a1) / (reps_b * kB)
+
+        b_enc = float(np.median([run_b(lambda c: B.compress_batch(bi[c], b_off, nbuf, W, 0, bo[c], b_out_off, bws, status)) for _ in range(3)]))
+        b_dec = float(np.median([run_b(lambda c: B.decompress_batch(bo[c], b_out_off, nbuf, W, bb[c], b_id_off, bws, status)) for _ in range(3)]))
+        assert int(status.item()) == 0 and torch.equal(bb[kB - 1], b_ids) and torch.equal(b_id_off, b_off), "batch: decode != input"
+        b_raw, b_comp = bn * (W // 8), int(b_out_off[-1].item())
+        batch = {"workload": "configs[4] batch: 4096 buffers of 256 B-64 KB (log-uniform), gaps mean 16, u32, threshold 0, seed 5",
+                 "n_buf": nbuf, "raw_bytes": b_raw, "ratio": b_raw / b_comp, "encode_ms": b_enc, "decode_ms": b_dec,
+                 "encode_GBps_in": b_raw / b_enc / 1e6, "decode_GBps_out": b_raw / b_dec / 1e6,
+                 "encode_frac_of_peak": (b_raw + b_comp) / b_enc / 1e6 / peaks()[0], "decode_frac_of_peak": (b_raw + b_comp) / b_dec / 1e6 / peaks()[0],
+                 "note": "per call incl. the host's enqueue time when that is the longer one (4 kernels per compress call)"}
+        del bi, bo, bb
+
     # ---- end to end through the host-buffer C-ABI calls (pinned host memory) ----
     e2e = None
     if not args.no_e2e:
@@ -401,7 +442,7 @@ def run_ours(args, rank, local_rank, world):
                                       "average per launch; median of 5 runs (min alongside)"},
         "ratio": {k: v["ratio"] for k, v in per.items()},
         "encode_GBps_in": S * raw_bytes / sum(enc_ms) / 1e6, "decode_GBps_out": S * raw_bytes / sum(dec_ms) / 1e6,
-        "per_stream": per, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
+        "per_stream": per, "batch": batch, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
     }
     print(json.dumps(line))
 
