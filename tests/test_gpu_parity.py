@@ -253,6 +253,43 @@ def test_errors_reported_on_device(B):
     assert int(status.item()) == B.ERR_DST_TOO_SMALL
 
 
+def test_batch_of_many_streams_rejects_corrupt_headers(B):
+    """Batches of >= 512 streams read their headers through k_dec_headers (gathered by the whole GPU, then parsed
+    by the one-CTA plan): the same rejections as the direct path (FORMAT.md §4), no crash, nothing decoded
+    beyond capacity; and an intact batch of that size still round-trips."""
+    dev = torch.device("cuda")
+    W = 32
+    counts = torch.randint(0, 600, (700,), generator=torch.Generator().manual_seed(5))
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=11, W=W)
+    n, n_buf = ids.numel(), counts.numel()
+    out = torch.empty(B.batch_compress_bound(counts.tolist(), W), dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress_batch(ids.to(dev), off.to(dev), n_buf, W, 1024, out, out_off, ws, status)
+    back = torch.full((n + 4,), -1, dtype=ids.dtype, device=dev)
+    id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    B.decompress_batch(out, out_off, n_buf, W, back, id_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and torch.equal(back[:n].cpu(), ids) and torch.equal(id_off.cpu(), off)
+    starts = out_off.cpu()
+    for which, (rel, val) in ((3, (0, 0x41)), (350, (5, 64)), (699, (4, 9)), (512, (17, 0xFF))):   # magic, W, version, total_bytes
+        bad = out.clone()
+        bad[int(starts[which]) + rel] = val
+        status.zero_()
+        back.fill_(-1)
+        B.decompress_batch(bad, out_off, n_buf, W, back, id_off, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == B.ERR_CORRUPT, which
+        assert bool((back[n:] == -1).all())
+    bad_off = out_off.clone()
+    bad_off[100] += 8                                        # a stream that does not start on a 16-byte boundary
+    status.zero_()
+    B.decompress_batch(out, bad_off, n_buf, W, back, id_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_CORRUPT
+
+
 def test_host_api_roundtrip(B, oracle_mod):
     dev = torch.device("cuda")
     for W in (32, 64):
