@@ -24,15 +24,16 @@
  *    no launch gap). Because a call only enqueues kernels, a sequence of calls may be captured
  *    in a CUDA graph (stream capture) and replayed, after one call of each kind outside the
  *    capture (one-time function attributes); the launch counter then counts the capture only.
- *  - Concurrency: bfsc_compress / bfsc_compress_batch run a persistent grid that fills the GPU
- *    and whose CTAs wait for one another (device-wide scan of block sizes). Issue compress
- *    calls of one device on ONE stream at a time: two compress grids that become resident
- *    half each (two streams racing for the same SMs) can wait for each other forever.
- *    Decompress calls have no such dependency and may run on any stream, also next to a
- *    compress call.
+ *  - Concurrency: calls may be issued from several host threads and on any streams of a device, also
+ *    at the same time, each with a workspace of its own. The compress kernels run a device-wide scan of
+ *    block sizes in which CTAs wait for one another; every tile of work is handed out by an atomic ticket,
+ *    in order, so whatever a CTA waits for is held by a CTA that is already running: no kernel of this
+ *    library assumes that its whole grid is resident (two compress grids, or a compress grid next to a
+ *    foreign persistent kernel, cannot deadlock). Opt-out: BFSC_CODEC_FLAG_EXCLUSIVE (see bfsc_codec).
  *  - d_ids / d_out / d_in must be 16-byte aligned; element offsets inside a batch may be
  *    arbitrary (buffers that start off a 16-byte boundary are staged / written through
- *    aligned 16-byte chunks all the same).
+ *    aligned 16-byte chunks all the same). Nothing is read beyond the last ID of a buffer
+ *    (its last, ragged 16-byte chunk is fetched partially) and nothing before d_ids.
  *  - IDs are little-endian unsigned integers of W = 32 or 64 bits (bfsc_dtype).
  *  - Return value: host-detectable errors only (null / misaligned pointer, bad dtype,
  *    workspace too small, launch failure -> BFSC_ERR_CUDA).
@@ -81,8 +82,16 @@ typedef enum { BFSC_U32 = 32, BFSC_U64 = 64 } bfsc_dtype;
  *                        b = width of the block's widest delta (eq. 6), no exceptions. Skips
  *                        step E2's size argmin; one outlier widens its whole block (L1000).
  * Buffers below the raw threshold are RAW (mode 0) under either rule. bfsc_decompress[_batch] read
- * the mode from each stream header and decode every mode. */
-typedef enum { BFSC_CODEC_PFOR = 1, BFSC_CODEC_BP128 = 2 } bfsc_codec;
+ * the mode from each stream header and decode every mode.
+ *
+ * Launch flag, OR-ed into the codec argument of the *_codec calls:
+ *   BFSC_CODEC_FLAG_EXCLUSIVE  the caller vouches that nothing else occupies the device while the call runs
+ *                        (no kernel on another stream, no second compress call in flight), so that the
+ *                        whole compress grid becomes resident at once. The first two tiles of every CTA are
+ *                        then assigned statically and start before the call's plan kernel has finished
+ *                        (about 2 us less per call). If the promise is broken the call can deadlock.
+ *                        Output bytes are the same with or without the flag. */
+typedef enum { BFSC_CODEC_PFOR = 1, BFSC_CODEC_BP128 = 2, BFSC_CODEC_FLAG_EXCLUSIVE = 0x100 } bfsc_codec;
 
 /* library / format version: (format_version << 16) | abi_revision */
 uint32_t bfsc_version(void);
@@ -98,7 +107,9 @@ size_t bfsc_batch_compress_bound(const uint64_t* h_counts, size_t n_buf, bfsc_dt
 size_t bfsc_workspace_bytes(size_t n_ids_total, size_t n_buf, bfsc_dtype t);
 
 /* ONE buffer: d_ids[0..n_ids) -> one stream at d_out; *d_out_bytes (device) = its
- * total_bytes. Steps E0-E5 of SURVEY.md §8(a). */
+ * total_bytes. Steps E0-E5 of SURVEY.md §8(a): compress() of Algorithm 4 lines 5 / 9 and Algorithm 5
+ * — D1 deltas (L979-986), per-block width (eq. 6),
+ * exceptions (L1000-1011), RAW below the threshold (L1309-1334); layout FORMAT.md §1-§3. */
 bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
                           void* d_out, size_t out_capacity, uint64_t* d_out_bytes,
                           void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
@@ -111,15 +122,18 @@ bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, size_t n_id
                                 uint32_t* d_status, void* cuda_stream);
 
 /* ONE stream at d_in (in_bytes available, >= its total_bytes) -> d_ids[0..n); *d_n_ids
- * (device) = n. Steps D0-D5. */
+ * (device) = n. Steps D0-D5: decompress() of Algorithm 4 lines 7 / 11: unpack
+ * (L987-998), patch the exceptions (L1011), prefix-sum the deltas (L979-986); FORMAT.md §4. */
 bfsc_status bfsc_decompress(const void* d_in, size_t in_bytes, bfsc_dtype t,
                             void* d_ids, size_t ids_capacity, uint64_t* d_n_ids,
                             void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                             void* cuda_stream);
 
-/* n_buf buffers in one launch sequence. d_in_offsets: n_buf+1 non-decreasing ELEMENT
- * offsets into d_ids (device). Streams are written back to back at d_out;
- * d_out_offsets[0..n_buf] (device, written) are their BYTE offsets, [n_buf] = total. */
+/* n_buf buffers in one launch sequence — the send buffers of one exchange (ALLGATHERV / ALLTOALLV counts and
+ * displacements; "data transfer grouping", L1786-1800). d_in_offsets: n_buf+1
+ * non-decreasing ELEMENT offsets into d_ids (device). Streams are written back to back at d_out (FORMAT.md §5);
+ * d_out_offsets[0..n_buf] (device, written) are their BYTE offsets, [n_buf] = total: the size metadata
+ * the caller exchanges first (L1790). */
 bfsc_status bfsc_compress_batch(const void* d_ids, const uint64_t* d_in_offsets, size_t n_buf,
                                 bfsc_dtype t, size_t raw_threshold_bytes,
                                 void* d_out, size_t out_capacity, uint64_t* d_out_offsets,
@@ -133,9 +147,9 @@ bfsc_status bfsc_compress_batch_codec(bfsc_codec codec, const void* d_ids, const
                                       void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                                       void* cuda_stream);
 
-/* d_in_offsets: n_buf+1 BYTE offsets of the streams inside d_in (each a multiple of 16).
- * IDs are written back to back at d_ids; d_id_offsets[0..n_buf] (device, written) are
- * their ELEMENT offsets. */
+/* The receive side of the same exchange. d_in_offsets: n_buf+1 BYTE offsets
+ * of the streams inside d_in (each a multiple of 16). IDs are written back to back at d_ids;
+ * d_id_offsets[0..n_buf] (device, written) are their ELEMENT offsets. */
 bfsc_status bfsc_decompress_batch(const void* d_in, const uint64_t* d_in_offsets, size_t n_buf,
                                   bfsc_dtype t,
                                   void* d_ids, size_t ids_capacity, uint64_t* d_id_offsets,

@@ -200,6 +200,7 @@ static int decode_block(const uint8_t *blk, size_t avail, int W, int m, void *id
         for (int i = 0; i < n_exc; i++) {
             int p = e[i];
             if (p >= BLK) return BFSC_REF_ERR_CORRUPT;
+            if (i > 0 && p <= e[i - 1]) return BFSC_REF_ERR_CORRUPT;   /* FORMAT.md §4: strictly ascending */
             uint64_t high = ld_le(h + (size_t)i * (W / 8), W / 8);
             if (b < 64) d[p] |= high << b;
         }
@@ -214,7 +215,7 @@ static int parse_header(const uint8_t *in, size_t in_bytes, int W,
                         int *mode, uint64_t *n, uint64_t *total, uint64_t *nb) {
     if (in_bytes < 32) return BFSC_REF_ERR_CORRUPT;
     if (in[0] != 'B' || in[1] != 'F' || in[2] != 'S' || in[3] != 'C') return BFSC_REF_ERR_CORRUPT;
-    if (in[4] != 1 || in[5] != W || in[6] > 2) return BFSC_REF_ERR_CORRUPT;
+    if (in[4] != 1 || in[5] != W || in[6] > 2 || in[7] != 0) return BFSC_REF_ERR_CORRUPT;   /* FORMAT.md §4: reserved byte 7 */
     *mode = in[6];
     *n = ld_le(in + 8, 8); *total = ld_le(in + 16, 8); *nb = ld_le(in + 24, 4);
     if (*total > in_bytes || *total % 16 || *total < 32) return BFSC_REF_ERR_CORRUPT;

@@ -82,7 +82,7 @@ def stream_blocks(s: bytes):
 
 def decode_stream(s: bytes, W: int):
     """-> list of python ints. Raises ValueError on anything FORMAT.md §4 rejects."""
-    if len(s) < 32 or s[0:4] != b"BFSC" or s[4] != 1 or s[5] != W or s[6] not in (0, 1, 2):      # 2 = BP128-D1: decoded like 1 (FORMAT.md §7)
+    if len(s) < 32 or s[0:4] != b"BFSC" or s[4] != 1 or s[5] != W or s[6] not in (0, 1, 2) or s[7] != 0:   # 2 = BP128-D1: decoded like 1 (FORMAT.md §7)
         raise ValueError("bad header")
     n = int.from_bytes(s[8:16], "little")
     total = int.from_bytes(s[16:24], "little")
@@ -118,6 +118,8 @@ def decode_stream(s: bytes, W: int):
             e = blk[16 + 16 * b:]
             pos = list(e[:n_exc])
             hoff = _align(n_exc, W // 8)
+            if any(pos[i] <= pos[i - 1] for i in range(1, n_exc)):
+                raise ValueError("exception positions not strictly ascending")
             for i, p in enumerate(pos):
                 if p >= 128:
                     raise ValueError("bad exception position")

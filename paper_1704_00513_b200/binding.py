@@ -18,6 +18,7 @@ _lib = None
 OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED = range(6)
 U32, U64 = 32, 64
 CODEC_PFOR, CODEC_BP128 = 1, 2          # bfsc_codec (include/bfsc.h)
+CODEC_FLAG_EXCLUSIVE = 0x100            # launch flag, OR-ed into the codec (include/bfsc.h)
 
 EXPORTS = [
     "bfsc_version", "bfsc_compress_bound", "bfsc_batch_compress_bound", "bfsc_workspace_bytes",
@@ -171,25 +172,3 @@ def decompress_host(h_in, in_bytes, W, h_ids, d_scratch) -> int:
                                       _ptr(d_scratch), d_scratch.numel(), ctypes.c_void_p(_stream())),
            "bfsc_decompress_host")
     return n.value
-
-
-class Codec:
-    """Convenience holder of the device buffers one (batched) call needs. Still marshalling
-    only: sizes the buffers with the library's own bound functions and forwards."""
-
-    def __init__(self, max_ids: int, max_buf: int, W: int, device="cuda"):
-        self.W, self.max_ids, self.max_buf = W, max_ids, max_buf
-        dev = torch.device(device)
-        bound = max_buf * compress_bound(0, W) + compress_bound(max_ids, W) + 48 * max_buf
-        self.out = torch.empty(bound + 256, dtype=torch.uint8, device=dev)
-        self.ws = torch.empty(workspace_bytes(max_ids, max_buf, W), dtype=torch.uint8, device=dev)
-        self.out_off = torch.zeros(max_buf + 1, dtype=torch.int64, device=dev)
-        self.id_off = torch.zeros(max_buf + 1, dtype=torch.int64, device=dev)
-        self.status = torch.zeros(1, dtype=torch.int32, device=dev)
-        self.ids = torch.empty(max_ids + 4, dtype=torch.int32 if W == 32 else torch.int64, device=dev)
-
-    def encode(self, d_ids, d_in_off, n_buf, thr):
-        compress_batch(d_ids, d_in_off, n_buf, self.W, thr, self.out, self.out_off, self.ws, self.status)
-
-    def decode(self, n_buf):
-        decompress_batch(self.out, self.out_off, n_buf, self.W, self.ids, self.id_off, self.ws, self.status)

@@ -1,8 +1,26 @@
 // api.cu — host-only entry points of the C ABI: bounds, workspace size, host-buffer calls.
 #include "common.cuh"
 
+#include <mutex>
+
 namespace bfsc {
 unsigned long long g_launches = 0;
+
+bool current_device(DeviceInfo* d) {
+    static std::mutex mu;
+    static int sms[kMaxDevices] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return false;
+    std::lock_guard<std::mutex> lock(mu);
+    if (sms[dev] == 0) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) return false;
+        sms[dev] = n;
+    }
+    d->device = dev;
+    d->sms = sms[dev];
+    return true;
+}
 
 static size_t bound_one(size_t n, int W) {
     const size_t nb = (n + kBlk - 1) / kBlk;

@@ -41,7 +41,7 @@ __device__ __forceinline__ void unpack_rows(const uint4* __restrict__ P, uint32_
 }
 
 // D3: OR the exceptions' high parts into place. e = exception area (pos bytes, pad, highs).
-// Returns false on a malformed position.
+// Returns false on a malformed position (>= 128, or not above its predecessor).
 template <int W>
 __device__ __forceinline__ bool patch_rows(const unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc,
                                            typename IdT<W>::T d[4]) {
@@ -53,7 +53,10 @@ __device__ __forceinline__ bool patch_rows(const unsigned char* __restrict__ e, 
     for (uint32_t i0 = 0; i0 < n_exc; i0 += 32) {
         const uint32_t i = i0 + lane;
         uint32_t pos = 0xffffffffu; T hv = 0;
-        if (i < n_exc) { pos = e[i]; hv = high[i]; if (pos >= (uint32_t)kBlk) ok = false; }
+        if (i < n_exc) {
+            pos = e[i]; hv = high[i];
+            if (pos >= (uint32_t)kBlk || (i > 0 && pos <= e[i - 1])) ok = false;   // FORMAT.md §4: < 128, strictly ascending
+        }
         const uint32_t cnt = min(32u, n_exc - i0);
         for (uint32_t q = 0; q < cnt; q++) {
             const uint32_t p = __shfl_sync(kFull, pos, q);

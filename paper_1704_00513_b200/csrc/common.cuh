@@ -12,7 +12,6 @@ namespace bfsc {
 constexpr int kBlk = 128;               // IDs per block
 constexpr int kWarp = 32;
 constexpr uint32_t kFull = 0xffffffffu;
-constexpr int kNumSM = 148;             // B200
 
 template <int W> struct IdT;
 template <> struct IdT<32> { using T = uint32_t; };
@@ -47,10 +46,7 @@ struct WsView {
 };
 
 constexpr int kTileBlocks = 64;         // blocks per encode tile (8 worker warps x 8 blocks)
-#ifndef BFSC_STATE_STRIDE
-#define BFSC_STATE_STRIDE 8
-#endif
-constexpr int kStateStride = BFSC_STATE_STRIDE;         // u64 words between look-back states (64 B)
+constexpr int kStateStride = 8;         // u64 words between look-back states (64 B)
 constexpr size_t kTileWsBytes = 8 * kStateStride + 32 * kTileBlocks;   // workspace per tile: state + block table
 
 // Block table entries (batch calls). Encode: where the block's IDs are. Decode: where its stream is, which
@@ -204,6 +200,12 @@ __device__ inline Scan2 block_scan_excl2(Scan2 v, Scan2* total, Scan2* sm /* 33 
 
 extern unsigned long long g_launches;   // host-side launch counter (api.cu)
 
+// Per-device launch set-up (api.cu): the SM count of the CURRENT device and a once-per-device flag table, so
+// that every device of the process gets its cudaFuncSetAttribute / occupancy query (thread-safe).
+constexpr int kMaxDevices = 64;
+struct DeviceInfo { int device; int sms; };
+bool current_device(DeviceInfo* d);      // false: no current device
+
 // Programmatic dependent launch: a kernel launched with launch_dep may start while its predecessor in
 // the stream still runs (once that one executed pdl_launch_dependents); it must execute pdl_wait
 // before it touches anything the predecessor writes.
@@ -224,8 +226,10 @@ static inline cudaError_t launch_dep(void (*kern)(A), int grid, int block, size_
 
 }  // namespace bfsc
 
-#define BFSC_LAUNCH_CHECK()                                        \
-    do {                                                           \
-        __atomic_fetch_add(&::bfsc::g_launches, 1ull, __ATOMIC_RELAXED); /* calls may come from several host threads */ \
-        if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; } \
+// One launch through launch_dep: its own return value decides (an earlier, unrelated error of the process is
+// neither reported here nor cleared); counts the launch (calls may come from several host threads).
+#define BFSC_LAUNCH(expr)                                                        \
+    do {                                                                         \
+        if ((expr) != cudaSuccess) return BFSC_ERR_CUDA;                         \
+        __atomic_fetch_add(&::bfsc::g_launches, 1ull, __ATOMIC_RELAXED);         \
     } while (0)

@@ -2,6 +2,8 @@
 //
 // Launches per call: single stream: k_dec_tiles alone (it parses the stream header itself);
 // batch: [k_dec_headers ->] k_dec_plan -> k_dec_blocks -> k_dec_tiles, chained with programmatic dependent launch.
+#include <mutex>
+
 #include "block_decode.cuh"
 #include "quad_decode.cuh"
 
@@ -109,8 +111,7 @@ __global__ void __launch_bounds__(1024) k_dec_plan(DecArgs a) {
                         ok = false;
                     else if (total > avail[u] || (total & 15) || total < 32) ok = false;
                     else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
-                    else if (nb != (n + kBlk - 1) / kBlk || n > (1ull << 40) ||
-                             32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
+                    else if (nb != (n + kBlk - 1) / kBlk || 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)   // (nb is 32 bits wide: n < 2^39)
                         ok = false;
                     if (ok) { v[u].a = nb; v[u].b = n; tot_bytes[u] = total; }
                 }
@@ -256,7 +257,7 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
                 ok = false;
             else if (total > a.in_single || (total & 15) || total < 32) ok = false;
             else if (mode == 0) { if (nb != 0 || n1 > (total - 32) / E) ok = false; }
-            else if (nb != (n1 + kBlk - 1) / kBlk || n1 > (1ull << 40) || 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
+            else if (nb != (n1 + kBlk - 1) / kBlk || 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
                 ok = false;
         }
         if (!ok || n1 > a.ids_cap) {
@@ -394,22 +395,31 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
     }
 }
 
+// Once per device and instantiation: the dynamic shared memory attribute and the resident CTAs per SM.
+template <int W, bool kBatch>
+static int dec_ctas_per_sm(int device) {
+    static std::mutex mu;
+    static int per_sm[kMaxDevices] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    if (per_sm[device] == 0) {
+        int n = 0;
+        if (cudaFuncSetAttribute(k_dec_tiles<W, kBatch>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DecSmem<W>::kBytes) != cudaSuccess)
+            return 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_dec_tiles<W, kBatch>, DecCfg<W>::kThreads, DecSmem<W>::kBytes) != cudaSuccess || n < 1)
+            return 0;
+        per_sm[device] = n;
+    }
+    return per_sm[device];
+}
+
 template <int W>
 static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream_t s) {
     constexpr size_t kSmem = DecSmem<W>::kBytes;
-    static int max_grid = 0;
-    if (max_grid == 0) {
-        int per_sm = 0, dev = 0, sms = kNumSM;
-        if (cudaFuncSetAttribute(k_dec_tiles<W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess ||
-            cudaFuncSetAttribute(k_dec_tiles<W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
-            return BFSC_ERR_CUDA;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dec_tiles<W, true>, DecCfg<W>::kThreads, kSmem) != cudaSuccess ||
-            per_sm < 1)
-            per_sm = 1;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        max_grid = sms * per_sm;
-    }
+    DeviceInfo dev;
+    if (!current_device(&dev)) return BFSC_ERR_CUDA;
+    const int per_sm = a.in_off ? dec_ctas_per_sm<W, true>(dev.device) : dec_ctas_per_sm<W, false>(dev.device);
+    if (per_sm < 1) return BFSC_ERR_CUDA;
+    const int max_grid = dev.sms * per_sm;
     const size_t want = (max_blocks + kDecBlocks * DecCfg<W>::kWarps - 1) / (kDecBlocks * DecCfg<W>::kWarps);
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
@@ -417,21 +427,18 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
         const bool gather = a.n_buf >= kHeaderGatherMin && a.ws.blk_cap >= a.n_buf;
         if (gather) {
             int hgrid = (int)((a.n_buf + 255) / 256);
-            if (hgrid > kNumSM * 4) hgrid = kNumSM * 4;
-            if (launch_dep(k_dec_headers<W>, hgrid, 256, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-            BFSC_LAUNCH_CHECK();
+            if (hgrid > dev.sms * 4) hgrid = dev.sms * 4;
+            BFSC_LAUNCH(launch_dep(k_dec_headers<W>, hgrid, 256, 0, s, a));
         }
-        if ((gather ? launch_dep(k_dec_plan<W, true>, 1, 1024, 0, s, a) : launch_dep(k_dec_plan<W, false>, 1, 1024, 0, s, a)) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-        BFSC_LAUNCH_CHECK();
+        if (gather) BFSC_LAUNCH(launch_dep(k_dec_plan<W, true>, 1, 1024, 0, s, a));
+        else BFSC_LAUNCH(launch_dep(k_dec_plan<W, false>, 1, 1024, 0, s, a));
         size_t bgrid = (a.ws.blk_cap + kBlkTabThreads - 1) / kBlkTabThreads;
-        if (bgrid > (size_t)(kNumSM * 8)) bgrid = (size_t)(kNumSM * 8);
-        if (launch_dep(k_dec_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-        BFSC_LAUNCH_CHECK();
-        if (launch_dep(k_dec_tiles<W, true>, max_grid, DecCfg<W>::kThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        if (bgrid > (size_t)dev.sms * 8) bgrid = (size_t)dev.sms * 8;
+        BFSC_LAUNCH(launch_dep(k_dec_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a));
+        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true>, max_grid, DecCfg<W>::kThreads, kSmem, s, a));
     } else {
-        if (launch_dep(k_dec_tiles<W, false>, grid, DecCfg<W>::kThreads, kSmem, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
+        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
     }
-    BFSC_LAUNCH_CHECK();
     return BFSC_OK;
 }
 

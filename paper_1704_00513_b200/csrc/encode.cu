@@ -3,6 +3,8 @@
 // Launches per call:  k_enc_plan -> k_enc_tiles [-> k_enc_streams, batch and degenerate calls only],
 // chained with programmatic dependent launch: a dependent kernel starts while its predecessor still
 // runs and executes griddepcontrol.wait before it touches what the predecessor writes.
+#include <mutex>
+
 #include "quad_encode.cuh"
 #include "wide_encode.cuh"
 
@@ -13,8 +15,9 @@ struct EncArgs {
     const unsigned long long* in_off;   // n_buf+1 element offsets, or nullptr (single buffer of n_single IDs)
     unsigned long long n_single;
     uint32_t n_buf;
-    uint32_t grid;                      // CTAs of k_enc_tiles: their first tiles are blockIdx.x (+ grid), tickets start at 2 grid
     uint32_t codec;                     // encoder rule = mode byte: 1 PFOR-D1 (E2: size argmin), 2 BP128-D1 (b = maxw, no exceptions; FORMAT.md §7)
+    uint32_t exclusive;                 // BFSC_CODEC_FLAG_EXCLUSIVE: the CTAs' first two tiles are static (grid CTAs; tickets start at 2 grid)
+    uint32_t grid;                      // CTAs of k_enc_tiles
     unsigned long long thr;             // raw threshold in bytes
     unsigned char* out;
     unsigned long long out_cap;
@@ -62,7 +65,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
             a.ws.blk_first[0] = 0; a.ws.blk_first[1] = nb;
             a.ws.fixed_prefix[0] = 0; a.ws.fixed_prefix[1] = fixed;
             a.ws.stream_start[0] = 0; a.ws.stream_start[1] = 0;
-            a.ws.hdr->total_blocks = nb; a.ws.hdr->fixed_total = fixed; a.ws.hdr->ticket = 2 * a.grid;
+            a.ws.hdr->total_blocks = nb; a.ws.hdr->fixed_total = fixed; a.ws.hdr->ticket = a.exclusive ? 2 * a.grid : 0;
             a.ws.hdr->grand16 = 0; a.ws.hdr->total_out = fixed; a.ws.hdr->ok = ok ? 1u : 0u;
             if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
         }
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(1024) k_enc_plan(EncArgs a) {
         a.ws.stream_start[a.n_buf] = 0;
         a.ws.hdr->total_blocks = carry.a;
         a.ws.hdr->fixed_total = carry.b;
-        a.ws.hdr->ticket = 2 * a.grid;
+        a.ws.hdr->ticket = a.exclusive ? 2 * a.grid : 0;
         a.ws.hdr->grand16 = 0;
         a.ws.hdr->total_out = carry.b;
         const bool ok = !bad && carry.a <= a.ws.blk_cap && (carry.a + kTileR - 1) / kTileR <= a.ws.tile_cap;
@@ -173,18 +176,6 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_enc_blocks(EncArgs a) {
 // decoupled look-back over the tiles in flight (= device-wide exclusive scan of block sizes),
 // final byte offset of every block -> s_at, directory entries, stream starts, and (single-buffer
 // calls) the stream header; barrier 2.
-#ifdef BFSC_TRACE
-// Debug build only (never in libbfsc.so): per-tile phase timestamps, read back with bfsc_debug_trace.
-__device__ unsigned long long g_trace[4096 * 16];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-__device__ __forceinline__ unsigned int smid() { unsigned int r; asm volatile("mov.u32 %0, %%smid;" : "=r"(r)); return r; }
-#define TR(tile, slot_) do { if ((threadIdx.x & 31) == 0 && (tile) < 4096) g_trace[(tile) * 16 + (slot_)] = gtime(); } while (0)
-#define TRV(tile, slot_, v) do { if ((threadIdx.x & 31) == 0 && (tile) < 4096) g_trace[(tile) * 16 + (slot_)] = (v); } while (0)
-#else
-#define TR(tile, slot_) do {} while (0)
-#define TRV(tile, slot_, v) do {} while (0)
-#endif
-
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPre = 2ull << 62, kValMask = (1ull << 62) - 1;
 constexpr unsigned long long kNoTile = ~0ull, kSkip = ~0ull;
 
@@ -224,19 +215,16 @@ __device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, uint32_
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }   // sources may be overwritten
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2_bulk(const void* gsrc, uint32_t bytes) {   // 16-byte aligned, a multiple of 16
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 // Decoupled look-back (one warp): the exclusive prefix of tile t > 0 = aggregates of t-1, t-2, ... down to the
 // nearest tile whose inclusive prefix is known. Every lane sums its own entries, a single warp reduction ends it.
-#ifndef BFSC_LOOK_CHUNKS
-#define BFSC_LOOK_CHUNKS 1
-#endif
-constexpr int kLookChunks = BFSC_LOOK_CHUNKS;
-#ifndef BFSC_LOOK_SLEEP
-#define BFSC_LOOK_SLEEP 32
-#endif
-constexpr unsigned kLookSleepNs = BFSC_LOOK_SLEEP;   // back-off between polls of a look-back that has to wait
+constexpr int kLookChunks = 1;                       // rounds of 32 predecessor states (the measured optimum, see lookback)
+constexpr unsigned kLookSleepNs = 32;                // back-off between polls of a look-back that has to wait
 // One round of the look-back: the states of the 32 * N predecessors below idx0 (lane i: idx0 - i, - 32, ...) are
 // requested at once, then examined 32 at a time with two ballots; an entry that is not posted yet is polled alone.
 template <int N>
@@ -298,10 +286,7 @@ template <int W> struct ImgCfg {
     static constexpr int kBufChunks = kQuadBlocks * kSlotChunks;
 };
 
-#ifndef BFSC_DEFER
-#define BFSC_DEFER 1
-#endif
-constexpr int kDefer = BFSC_DEFER;                                     // a tile's images leave kDefer tiles after they were packed (1 or 2)
+constexpr int kDefer = 1;                                     // a tile's images leave kDefer tiles after they were packed
 constexpr int kNB = kDefer + 1;                               // image buffers / size and offset tables per CTA
 
 template <int W> struct EncSmem {
@@ -322,8 +307,8 @@ constexpr int kRing = 8;                                      // ring of tile bo
 //       the block sizes) -> final offsets in s_at[k % kNB], directory entries, stream starts, header.
 //       It may lag up to kDefer tiles behind the workers: a look-back that waits for a slow
 //       predecessor CTA does not stall this CTA's workers.
-// Tiles: the first two of a CTA are blockIdx.x and blockIdx.x + gridDim.x, the rest come from the ticket
-// counter, each drawn at the same point of the pipeline: a lower tile number means "sizes posted earlier".
+// Tiles: every one comes from the ticket counter (prep warp), each drawn at the same point of the pipeline: a lower
+// tile number means "sizes posted earlier" — and is held by a running CTA, whatever else occupies the device.
 template <int W, bool kBatch>
 __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
@@ -352,14 +337,25 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     const T* ids = reinterpret_cast<const T*>(a.ids);
     pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
     if constexpr (!kBatch) {
-        // Single-buffer calls: a worker's share of the CTA's first tile (tile blockIdx.x) follows from the
-        // arguments: its loads go out before anything else in the kernel (barriers, mbarrier set-up, plan).
-        if (warp < kEncWorkers) {
-            const unsigned long long g = (unsigned long long)blockIdx.x * kTileR + warp * kQuadBlocks + (lane >> 2);
+        // Single-buffer calls: the plan kernel (ticket counter, zeroed look-back states) is still running.
+        if (a.exclusive) {
+            // static first tile (tile blockIdx.x): its loads go out before anything else in the kernel
+            if (warp < kEncWorkers) {
+                const unsigned long long g = (unsigned long long)blockIdx.x * kTileR + warp * kQuadBlocks + (lane >> 2);
+                const unsigned long long nb0 = (a.n_single + kBlk - 1) / kBlk;
+                if (g < nb0)
+                    quad_prefetch<W>(dyn_smem + warp * EncSmem<W>::kWarpChunks + raw_slot_chunk<W>(lane >> 2), ids + kBlk * g,
+                                     (int)min((unsigned long long)kBlk, a.n_single - kBlk * g));
+            }
+        } else if (warp < kEncWorkers && lane == 0) {
+            // Meanwhile pull the tile this CTA will most likely draw first (tickets go out in launch order) into L2.
+            const unsigned long long g = (unsigned long long)blockIdx.x * kTileR + warp * kQuadBlocks;
             const unsigned long long nb0 = (a.n_single + kBlk - 1) / kBlk;
-            if (g < nb0)
-                quad_prefetch<W>(dyn_smem + warp * EncSmem<W>::kWarpChunks + raw_slot_chunk<W>(lane >> 2), ids + kBlk * g,
-                                 (int)min((unsigned long long)kBlk, a.n_single - kBlk * g));
+            if (g < nb0) {
+                const unsigned long long n_el = min((unsigned long long)(kQuadBlocks * kBlk), a.n_single - kBlk * g);
+                const uint32_t bytes = (uint32_t)(n_el * sizeof(T)) & ~15u;
+                if (bytes) prefetch_l2_bulk(ids + kBlk * g, bytes);
+            }
         }
     }
     if (threadIdx.x < 4) s_agg[threadIdx.x] = 0;
@@ -368,8 +364,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     if (threadIdx.x >= 32 && threadIdx.x < 32 + kNB) mbar_init(&mb_off[threadIdx.x - 32], 1);
     __syncthreads();
 
-    // Single-buffer calls know their geometry from the arguments: the first tiles start without waiting
-    // for the plan kernel; only the ticket counter and the look-back states need it.
     const unsigned long long nb_single = (a.n_single + kBlk - 1) / kBlk;
     unsigned long long total = nb_single;
     if (batch) {
@@ -409,14 +403,12 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     if (warp == kEncWorkers) {
         // =============================== scan warp ===============================
         const unsigned long long f1_single = 32ull + ((4ull * (nb_single + 1) + 15ull) & ~15ull);
-        __syncthreads();                                 // barrier 0: the first two tiles are posted (by warp 0)
         if (!batch) pdl_wait();                          // the plan kernel's writes are visible from here on
         int kp = 0;                                      // k % kNB
         for (int k = 0;; k++) {
             mbar_wait(&mb_post[k & (kRing - 1)], (k / kRing) & 1);   // the prep warp has posted the CTA's tile k
             const unsigned long long t = s_tile[k & (kRing - 1)];
             if (t == kNoTile) break;
-            TR(t, 0);
             bar_sync(kBarSizes + kp, kSizesThreads);
             if (lane == 0) s_sized = (unsigned int)k + 1u;      // the workers' sizes of tile t are in s_key[kp]
 
@@ -441,7 +433,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 offs[h] += inc - own;
                 if (kPer * lane + h < kTileR) s_off16[kPer * lane + h] = offs[h];
             }
-            TR(t, 2);                                    // (the aggregate was published by the last worker warp)
             // batch calls: the per-buffer constants of this lane's blocks, requested BEFORE the look-back (their
             // latency hides behind it)
             const unsigned long long g0 = t * kTileR;
@@ -458,12 +449,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                     }
                 }
             }
-#ifdef BFSC_NOLB                                             // timing experiment only (never in libbfsc.so): no look-back, wrong offsets
-            const unsigned long long excl = t * (unsigned long long)kTileR * BFSC_NOLB;
-#else
             const unsigned long long excl = t > 0 ? lookback(a.ws.tile_state, t, lane) : 0ull;
-#endif
-            TR(t, 3);
             if (lane == 0) {
                 st_volatile_u64(&a.ws.tile_state[t * kStateStride], kFlagPre | (excl + agg));
                 if (t == n_tiles - 1) {
@@ -530,10 +516,8 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 }
                 s_at[kp][jj] = at;
             }
-            TR(t, 4);
             __syncwarp();
             if (lane == 0) mbar_arrive(&mb_off[kp]);     // offsets of tile k are posted
-            TRV(t, 15, (unsigned long long)smid() | ((unsigned long long)blockIdx.x << 32));
             kp = kp == kNB - 1 ? 0 : kp + 1;
         }
         return;
@@ -541,29 +525,49 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
 
     if (warp == kEncWorkers + 1) {
         // =============================== prep warp ===============================
-        // Runs ahead of the workers: draws the ticket of the CTA's tile p (p >= 2; tiles 0 and 1 are static),
-        // prepares its bookkeeping (batch calls: buffer, first ID, valid IDs of every block — a chain of
-        // dependent global loads nobody else has to wait for) and posts it. The ticket of tile p is drawn when
-        // the sizes of tile p - 2 have arrived: every CTA draws at the same point of its pipeline, so a lower
-        // tile number means "sizes posted earlier" and look-backs rarely wait; and no worker can still read the
-        // ring slot (kRing = 8) that is rewritten.
-        {
+        // Runs ahead of the workers: draws the ticket of the CTA's tile p, prepares its bookkeeping (batch calls:
+        // buffer, first ID, valid IDs of every block — a chain of dependent global loads nobody else has to wait
+        // for) and posts it. EVERY tile comes from the ticket counter, in order: whatever a CTA waits for (look-back)
+        // belongs to a tile with a lower ticket, which a RUNNING CTA holds — no co-residency assumption (two
+        // compress grids, or a compress grid next to any other kernel, cannot deadlock). The CTA's second ticket is
+        // drawn a moment after its first, when every CTA of the wave has its first (a CTA holding two neighbouring
+        // tiles would publish the second one a tile period late, and the tiles above wait for it); from then on
+        // the ticket of tile p is drawn when the sizes of tile p - 2 have arrived: every CTA draws at the same
+        // point of its pipeline, so a lower tile number means "sizes posted earlier" and look-backs rarely wait;
+        // and no worker can still read the ring slot (kRing = 8) that is rewritten.
+        // BFSC_CODEC_FLAG_EXCLUSIVE (the caller vouches that every CTA of the grid becomes resident): the first two
+        // tiles are blockIdx.x and blockIdx.x + gridDim.x and need neither the plan kernel nor an atomic.
+        auto draw = [&]() -> unsigned long long {
+            unsigned int ticket = 0;
+            if (lane == 0) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
+            ticket = __shfl_sync(kFull, ticket, 0);
+            return ticket < n_tiles ? (unsigned long long)ticket : kNoTile;
+        };
+        if (a.exclusive) {
             const unsigned long long t0 = blockIdx.x, t1 = (unsigned long long)blockIdx.x + gridDim.x;
             prep(t0 < n_tiles ? t0 : kNoTile, 0);
             prep(t0 < n_tiles && t1 < n_tiles ? t1 : kNoTile, 1);
             __syncwarp();
             if (lane == 0) { mbar_arrive(&mb_post[0]); mbar_arrive(&mb_post[1]); }
+            if (!batch) pdl_wait();                      // the ticket counter is set by the plan kernel
+        } else {
+            if (!batch) pdl_wait();                      // the ticket counter is set by the plan kernel
+            const unsigned long long t0 = draw();
+            prep(t0, 0);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&mb_post[0]);
+            __nanosleep(1000);
+            const unsigned long long t1 = t0 != kNoTile ? draw() : kNoTile;
+            prep(t1, 1);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&mb_post[1]);
         }
-        __syncthreads();                                 // barrier 0
         bool more = s_tile[1] != kNoTile;
-        if (more) pdl_wait();                            // the ticket counter is set by the plan kernel
         for (int pt = 2; more; pt++) {
             while ((int)s_sized + 1 < pt) __nanosleep(400);   // (a tile period is 3-4 us: polling faster only takes issue slots)
-            unsigned int ticket = 0;
-            if (lane == 0) ticket = atomicAdd(&a.ws.hdr->ticket, 1u);
-            ticket = __shfl_sync(kFull, ticket, 0);
-            more = ticket < n_tiles;
-            prep(more ? (unsigned long long)ticket : kNoTile, pt & (kRing - 1));
+            const unsigned long long t = draw();
+            more = t != kNoTile;
+            prep(t, pt & (kRing - 1));
             __syncwarp();
             if (lane == 0) mbar_arrive(&mb_post[pt & (kRing - 1)]);
         }
@@ -577,9 +581,9 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     unsigned char* ibuf = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks);   // the warp's kNB image buffers
     const int j = warp * kQuadBlocks + q;
     constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
-    __syncthreads();                                                     // barrier 0: the first two tiles are posted
+    mbar_wait(&mb_post[0], 0);                                           // the CTA's first tile is posted (by the prep warp)
     bool have = s_tile[0] != kNoTile;
-    if constexpr (kBatch) { if (have) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j)); }   // (single: see the top)
+    if (have && (kBatch || !a.exclusive)) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));   // (exclusive single-buffer calls: see the top)
     static_assert(kDefer == 1 || kDefer == 2, "hist selection below");
     uint32_t key_hist[kDefer] = {}, woff_hist[kDefer] = {};              // keys and image places of the tiles that wait in shared memory
     int kp = 0;                                                          // k % kNB
@@ -592,24 +596,18 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             const T* raw = reinterpret_cast<const T*>(slot) +
                            (reinterpret_cast<uintptr_t>(ids + blk_xoff(k & (kRing - 1), j)) & 15) / sizeof(T);
             unsigned char* ib = ibuf + kp * (ImgCfg<W>::kBufChunks * 16);        // this tile's image buffer
-            if (warp == 0) TR(s_tile[k & (kRing - 1)], 6);
             cp_async_wait_all();
-            if (lane == 0) bulk_wait_read();                             // the bulk store that read this image buffer is done with it
             __syncwarp();
-            if (warp == 0) TR(s_tile[k & (kRing - 1)], 7);
             uint32_t d[32];
             bool wide_lane = false, wide = false;
             const T base = col_deltas<W>(raw, m, d, wide_lane);          // E1
             if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
-#ifdef BFSC_SKIP_CHOOSE
-            if (!wide) { uint32_t o = 0;
-#pragma unroll
-                for (int i = 0; i < 32; i++) o |= d[i];
-                const uint32_t top = 32 - __clz(quad_or(o)); key = ((16u + 16u * top) << 14) | ((64u - top) << 7); }
-#else
             if (!wide) key = a.codec == BFSC_CODEC_BP128 ? quad_max_width_key(d) : quad_choose_b<W>(d);   // E2
-#endif
-            else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (ImgCfg<W>::kSlotChunks * 16)),
+            // The bulk store that read this image buffer (issued when the previous iteration ended) is done with it.
+            // Not waited for before E2: the copy engine needs half a microsecond to fetch its source.
+            if (lane == 0) bulk_wait_read();
+            __syncwarp();
+            if (wide) key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (ImgCfg<W>::kSlotChunks * 16)),
                                      a.codec == BFSC_CODEC_BP128);
             if (m <= 0) key = 0;
             if (l == 0) s_key[kp][j] = key;
@@ -629,7 +627,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                     }
                 }
             }
-            if (warp == 0) TR(s_tile[k & (kRing - 1)], 8);
             bar_arrive(kBarSizes + kp, kSizesThreads);
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
@@ -653,11 +650,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             have_next = s_tile[(k + 1) & (kRing - 1)] != kNoTile;
             if (have_next) quad_prefetch<W>(slot, ids + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));   // same slots
             if (fast) {                                                  // payload + header
-#ifndef BFSC_SKIP_PACK
                 if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
-#else
-                if (b > 0) reinterpret_cast<uint32_t*>(img)[4 + l] = d[0] ^ d[7] ^ d[31];
-#endif
                 if (l == 0) {                                            // block header (FORMAT.md §2)
                     reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
                     reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
@@ -665,7 +658,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             }
             if (late) key |= kLateBit;
             __syncwarp();                                                // image complete
-            if (warp == 0) TR(s_tile[k & (kRing - 1)], 9);
             n_wait++;
         }
 
@@ -676,9 +668,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             const uint32_t woff_e = (kDefer == 2 && w == 2) ? woff_hist[kDefer - 1] : woff_hist[0];  // of the CTA's tile ke
             int kpe = kp - w;                                            // its buffer: ke % kNB
             if (kpe < 0) kpe += kNB;
-            if (warp == 0) TR(s_tile[ke & (kRing - 1)], 10);
             mbar_wait(&mb_off[kpe], (ke / kNB) & 1);                     // its offsets are resolved
-            if (warp == 0) TR(s_tile[ke & (kRing - 1)], 11);
             unsigned long long at = kSkip;
             if (key_e != 0) at = s_at[kpe][j];
             if (__any_sync(kFull, (key_e & kLateBit) != 0)) {
@@ -695,9 +685,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             const bool contig = !valid || (fast_e && at != kSkip && (!valid_n || at_n == at + 16ull * z_e));
             if (__all_sync(kFull, contig)) {
                 const uint32_t tot = __shfl_sync(kFull, woff_e + z_e, 31);
-#ifndef BFSC_NOFENCE
                 fence_proxy_async_smem();                                // the image was written through the generic proxy
-#endif
                 __syncwarp();
                 if (lane == 0 && tot > 0) bulk_store(a.out + at, ib_e, 16u * tot);
             } else if (fast_e && at != kSkip) {
@@ -706,7 +694,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 for (uint32_t c = l; c < z_e; c += 4) __stcs(dst + c, src[c]);
             }
             __syncwarp();
-            if (warp == 0) TR(s_tile[ke & (kRing - 1)], 12);
             n_wait--;
             ke++;
         }
@@ -788,52 +775,55 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     }
 }
 
+// Once per device and instantiation: the dynamic shared memory attribute and the resident CTAs per SM.
+template <int W, bool kBatch>
+static int enc_ctas_per_sm(int device) {
+    static std::mutex mu;
+    static int per_sm[kMaxDevices] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    if (per_sm[device] == 0) {
+        int n = 0;
+        if (cudaFuncSetAttribute(k_enc_tiles<W, kBatch>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EncSmem<W>::kBytes) != cudaSuccess)
+            return 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_enc_tiles<W, kBatch>, kEncThreads, EncSmem<W>::kBytes) != cudaSuccess || n < 1)
+            return 0;
+        per_sm[device] = n;
+    }
+    return per_sm[device];
+}
+
 template <int W>
 static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     constexpr size_t kSmem = EncSmem<W>::kBytes;
-    static int max_grid = 0;                      // persistent grid: all CTAs resident
-    if (max_grid == 0) {
-        int per_sm = 0, dev = 0, sms = kNumSM;
-        if (cudaFuncSetAttribute(k_enc_tiles<W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess ||
-            cudaFuncSetAttribute(k_enc_tiles<W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem) != cudaSuccess)
-            return BFSC_ERR_CUDA;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_enc_tiles<W, true>, kEncThreads, kSmem) != cudaSuccess ||
-            per_sm < 1)
-            per_sm = 1;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        max_grid = sms * per_sm;
-    }
+    DeviceInfo dev;
+    if (!current_device(&dev)) return BFSC_ERR_CUDA;
     constexpr unsigned long long E = W / 8;
     const bool single = a_in.in_off == nullptr;
     const bool degenerate = single && (a_in.n_single == 0 || a_in.n_single * E < a_in.thr);   // no block: header (+ raw copy) only
-    int grid = max_grid;
+    const int per_sm = single ? enc_ctas_per_sm<W, false>(dev.device) : enc_ctas_per_sm<W, true>(dev.device);
+    if (per_sm < 1) return BFSC_ERR_CUDA;
+    int grid = dev.sms * per_sm;                                 // one resident wave (every tile is drawn by ticket: any grid size is correct)
     if (single) {
         const unsigned long long n_tiles = ((a_in.n_single + kBlk - 1) / kBlk + kTileR - 1) / kTileR;
         if (!degenerate && n_tiles > a_in.ws.tile_cap) return BFSC_ERR_INVALID_ARG;          // workspace too small
-        if (n_tiles < (unsigned long long)grid) grid = (int)n_tiles;
+        if (n_tiles < (unsigned long long)grid) grid = n_tiles ? (int)n_tiles : 1;
     }
     EncArgs a = a_in;
     a.grid = (uint32_t)grid;
-    if (launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-    BFSC_LAUNCH_CHECK();
+    BFSC_LAUNCH(launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a));
     if (!single) {
-        const size_t cap_blocks = a.ws.blk_cap;
-        size_t bgrid = (cap_blocks + kBlkTabThreads - 1) / kBlkTabThreads;
-        if (bgrid > (size_t)(kNumSM * 8)) bgrid = (size_t)(kNumSM * 8);
-        if (launch_dep(k_enc_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-        BFSC_LAUNCH_CHECK();
+        size_t bgrid = (a.ws.blk_cap + kBlkTabThreads - 1) / kBlkTabThreads;
+        if (bgrid > (size_t)dev.sms * 8) bgrid = (size_t)dev.sms * 8;
+        BFSC_LAUNCH(launch_dep(k_enc_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a));
     }
     if (!degenerate) {
-        if ((single ? launch_dep(k_enc_tiles<W, false>, grid, kEncThreads, kSmem, s, a)
-                    : launch_dep(k_enc_tiles<W, true>, grid, kEncThreads, kSmem, s, a)) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-        BFSC_LAUNCH_CHECK();
+        if (single) BFSC_LAUNCH(launch_dep(k_enc_tiles<W, false>, grid, kEncThreads, kSmem, s, a));
+        else BFSC_LAUNCH(launch_dep(k_enc_tiles<W, true>, grid, kEncThreads, kSmem, s, a));
     }
     if (!single || degenerate) {
         uint32_t sgrid = (a.n_buf + 7) / 8;                      // one warp per buffer
-        if (sgrid > (uint32_t)(kNumSM * 8)) sgrid = (uint32_t)(kNumSM * 8);
-        if (launch_dep(k_enc_streams<W>, sgrid ? (int)sgrid : 1, 256, 0, s, a) != cudaSuccess) { cudaGetLastError(); return BFSC_ERR_CUDA; }
-        BFSC_LAUNCH_CHECK();
+        if (sgrid > (uint32_t)dev.sms * 8) sgrid = (uint32_t)dev.sms * 8;
+        BFSC_LAUNCH(launch_dep(k_enc_streams<W>, sgrid ? (int)sgrid : 1, 256, 0, s, a));
     }
     return BFSC_OK;
 }
@@ -842,6 +832,8 @@ static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint
                                  bfsc_dtype t, size_t thr, void* d_out, size_t out_cap, uint64_t* d_out_off,
                                  uint64_t* d_out_total, void* ws, size_t ws_bytes, uint32_t* d_status, void* stream) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
+    const uint32_t exclusive = ((uint32_t)codec & (uint32_t)BFSC_CODEC_FLAG_EXCLUSIVE) ? 1u : 0u;
+    codec = (bfsc_codec)((uint32_t)codec & ~(uint32_t)BFSC_CODEC_FLAG_EXCLUSIVE);
     if (codec != BFSC_CODEC_PFOR && codec != BFSC_CODEC_BP128) return BFSC_ERR_INVALID_ARG;
     if (!d_out || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
     if (((uintptr_t)d_ids & 15) || ((uintptr_t)d_out & 15) || ((uintptr_t)ws & 15)) return BFSC_ERR_INVALID_ARG;
@@ -849,18 +841,12 @@ static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint
     EncArgs a;
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.ids = d_ids; a.in_off = (const unsigned long long*)d_in_off; a.n_single = n_single;
-    a.n_buf = (uint32_t)n_buf; a.grid = 0; a.codec = (uint32_t)codec; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
+    a.n_buf = (uint32_t)n_buf; a.codec = (uint32_t)codec; a.exclusive = exclusive; a.grid = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
     a.out_off = (unsigned long long*)d_out_off; a.out_total = (unsigned long long*)d_out_total; a.status = d_status;
     return t == BFSC_U32 ? launch_encode<32>(a, (cudaStream_t)stream) : launch_encode<64>(a, (cudaStream_t)stream);
 }
 
 }  // namespace bfsc
-
-#ifdef BFSC_TRACE
-extern "C" int bfsc_debug_trace(unsigned long long* h_out, size_t n_words) {
-    return (int)cudaMemcpyFromSymbol(h_out, bfsc::g_trace, n_words * 8);
-}
-#endif
 
 extern "C" bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, size_t n_ids, bfsc_dtype t,
                                            size_t raw_threshold_bytes, void* d_out, size_t out_capacity,

@@ -35,7 +35,8 @@ __device__ __forceinline__ void quad_stage_block(uint4* __restrict__ slot, const
 
 // D3 (first half): exceptions go through a per-warp patch table (128 entries per block, all zero between
 // uses): the quad scatters high << b at each position here; quad_decode_rows ORs the entries in;
-// quad_patch_clear zeroes them again. e = staged exception area. Returns false on a malformed position.
+// quad_patch_clear zeroes them again. e = staged exception area. Returns false on a malformed position
+// (>= 128, or not above its predecessor: FORMAT.md §4).
 template <int W>
 __device__ __forceinline__ bool quad_patch_scatter(typename IdT<W>::T* __restrict__ tab /* the quad's 128 entries */,
                                                    const unsigned char* __restrict__ e, uint32_t b, uint32_t n_exc, int l) {
@@ -45,7 +46,8 @@ __device__ __forceinline__ bool quad_patch_scatter(typename IdT<W>::T* __restric
     bool ok = true;
     for (uint32_t x = l; x < n_exc; x += 4) {
         const uint32_t pos = e[x];
-        if (pos >= (uint32_t)kBlk) ok = false; else tab[pos] = high[x] << b;
+        if (pos >= (uint32_t)kBlk || (x > 0 && pos <= e[x - 1])) ok = false;   // FORMAT.md §4: < 128, strictly ascending
+        else tab[pos] = high[x] << b;
     }
     return ok;
 }

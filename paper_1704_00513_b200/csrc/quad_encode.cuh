@@ -180,7 +180,14 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+// Same, reading only the first src_bytes (1..16) of the chunk; the rest of the 16 bytes is zero-filled.
+__device__ __forceinline__ void cp_async16_part(void* smem_dst, const void* gmem_src, int src_bytes) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gmem_src), "r"(src_bytes) : "memory");
+}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }   // all but the newest N groups
 
 // x = block's first ID (m valid IDs, m <= 0: nothing to copy). Lane l of the quad copies chunks l, l+4, ...
 template <int W>
@@ -197,10 +204,11 @@ __device__ __forceinline__ void quad_prefetch(uint4* __restrict__ slot, const ty
     if (nchunk == kBlk / EPC) {
 #pragma unroll
         for (int i = 0; i < kRounds; i++) cp_async16(slot + 4 * i + l, src + 4 * i);
-    } else {
+    } else {                                                     // ragged block (the last one of its buffer), or e > 0:
+        const int tail = (e + m) * (int)sizeof(T) - 16 * (nchunk - 1);   // nothing is read beyond the block's last ID
 #pragma unroll
         for (int i = 0; i <= kRounds; i++)
-            if (4 * i + l < nchunk) cp_async16(slot + 4 * i + l, src + 4 * i);
+            if (4 * i + l < nchunk) cp_async16_part(slot + 4 * i + l, src + 4 * i, 4 * i + l == nchunk - 1 ? tail : 16);
     }
 }
 

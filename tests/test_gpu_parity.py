@@ -53,8 +53,7 @@ def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True, codec=PFOR
     gpu_bytes = out[:total].cpu().numpy()
     gpu_off = out_off.cpu().numpy().astype(np.uint64)
     if check_oracle:
-        ref, ref_off = oracle_mod.compress_batch(_np(ids_t, W), off_t.numpy().astype(np.uint64), thr,
-                                                 threads=8 if codec == PFOR else 0, codec=codec)
+        ref, ref_off = oracle_mod.compress_batch(_np(ids_t, W), off_t.numpy().astype(np.uint64), thr, codec=codec)   # the plain serial oracle
         assert np.array_equal(gpu_off, ref_off)
         if not np.array_equal(gpu_bytes, ref):
             bad = int(np.nonzero(gpu_bytes != ref)[0][0])
@@ -327,32 +326,37 @@ def test_rmat_config4_reduced(B, oracle_mod, codec):
             run_batch(B, oracle_mod, streams.as_ids(vals, 64), off, 64, 1024, codec=codec)
 
 
-def test_rmat_config3_full_size_one_root(B, oracle_mod):
-    """config 3 at its BASELINE size (R-MAT scale 22, 16 buffers per level, u32, 1 KB threshold), one root:
+def test_rmat_config3_full_size_all_roots(B, oracle_mod):
+    """config 3 at its BASELINE size (R-MAT scale 22, 16 buffers per level, u32, 1 KB threshold), ALL 16 roots:
     every level's batch byte-for-byte against the oracle (the graph and the BFS are built on the GPU by the
     workload module; the codec calls are the ones report.py times)."""
     G = rmat.Graph(22, 16, seed=3, device=torch.device("cuda"))
-    root = G.roots(1, seed=3)[0]
-    total = 0
-    for f in G.bfs_frontiers(root):
-        vals, off = streams.split_block(f, 16, 1 << 22)
-        run_batch(B, oracle_mod, streams.as_ids(vals, 32).cpu(), off.cpu(), 32, 1024)
-        total += vals.numel()
-    assert total > 2_000_000                                  # the giant component
-
-
-def test_rmat_config4_full_size_one_root(B, oracle_mod):
-    """config 4 at its BASELINE size (R-MAT scale 25, 64 buffers per level, u64, 1 KB threshold), one root."""
-    G = rmat.Graph(25, 16, seed=4, device=torch.device("cuda"))
-    root = G.roots(1, seed=4)[0]
-    total = 0
-    for f in G.bfs_frontiers(root):
-        vals, off = streams.split_block(f, 64, 1 << 25)
-        run_batch(B, oracle_mod, streams.as_ids(vals, 64).cpu(), off.cpu(), 64, 1024)
-        total += vals.numel()
+    roots = G.roots(16, seed=3)
+    assert len(roots) == 16
+    for root in roots:
+        total = 0
+        for f in G.bfs_frontiers(root):
+            vals, off = streams.split_block(f, 16, 1 << 22)
+            run_batch(B, oracle_mod, streams.as_ids(vals, 32).cpu(), off.cpu(), 32, 1024)
+            total += vals.numel()
+        assert total > 2_000_000                              # the giant component
     del G
     torch.cuda.empty_cache()
-    assert total > 16_000_000
+
+
+def test_rmat_config4_full_size_three_roots(B, oracle_mod):
+    """config 4 at its BASELINE size (R-MAT scale 25, 64 buffers per level, u64, 1 KB threshold), three of the 8 roots
+    (the graph is built once)."""
+    G = rmat.Graph(25, 16, seed=4, device=torch.device("cuda"))
+    for root in G.roots(8, seed=4)[:3]:
+        total = 0
+        for f in G.bfs_frontiers(root):
+            vals, off = streams.split_block(f, 64, 1 << 25)
+            run_batch(B, oracle_mod, streams.as_ids(vals, 64).cpu(), off.cpu(), 64, 1024)
+            total += vals.numel()
+        assert total > 16_000_000
+    del G
+    torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("W", [32, 64])
@@ -460,11 +464,11 @@ def test_calls_replay_from_a_cuda_graph(B, oracle_mod, W):
         assert int(n_out1.item()) == n and torch.equal(back1[:n].cpu(), ids)
 
 
-def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256, codec=PFOR):
-    """One large single stream through bfsc_compress / bfsc_decompress: decoded IDs equal the input everywhere;
-    directory walk (strictly increasing, sizes recomputed from the block headers, total = header + directory +
-    blocks); `samples` blocks memcmp-equal to the oracle's encoding of the same 128 IDs (blocks are
-    independent: FORMAT.md §2)."""
+def _full_size(B, oracle_mod, ids, W, codec=PFOR):
+    """One large single stream through bfsc_compress / bfsc_decompress (the launch configuration bench.py and
+    report.py time): decoded IDs equal the input; the WHOLE compressed stream memcmp-equal to the serial oracle's;
+    and, independently of the oracle, the directory walk (strictly increasing, sizes recomputed from the block
+    headers, total = header + directory + blocks)."""
     dev = torch.device("cuda")
     n = ids.numel()
     E = W // 8
@@ -486,6 +490,7 @@ def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256, codec=PFOR):
     del back
     total = int(nbytes.item())
     s = out[:total].cpu().numpy()
+    del out
     nb = (n + 127) // 128
     assert s[:4].tobytes() == b"BFSC" and s[4] == 1 and s[5] == W and s[6] == codec
     assert int(s[8:16].view(np.uint64)[0]) == n and int(s[16:24].view(np.uint64)[0]) == total
@@ -497,27 +502,191 @@ def _full_size_sampled(B, oracle_mod, ids, W, rng, samples=256, codec=PFOR):
     exc = np.where(ne > 0, ((((ne + E - 1) // E) * E + E * ne + 15) // 16) * 16, 0)
     assert np.array_equal((d[1:] - d[:-1]) * 16, 16 + 16 * b + exc)
     host = ids.cpu().numpy().view(np.uint32 if W == 32 else np.uint64)
-    for k in rng.integers(0, nb, size=samples):
-        ref = oracle_mod.compress(host[128 * k:128 * k + 128], 0, codec=codec)
-        assert np.array_equal(s[d[k] * 16:d[k + 1] * 16], ref[48:]), f"block {k} differs from the oracle"
+    ref = oracle_mod.compress(host, 0, codec=codec)              # serial oracle, whole stream
+    assert len(ref) == total
+    if not np.array_equal(s, ref):
+        bad = int(np.nonzero(s != ref)[0][0])
+        raise AssertionError(f"compressed bytes differ from the oracle at byte {bad} of {total}")
 
 
 @pytest.mark.parametrize("codec", CODECS)
-def test_config2_full_size_sampled(B, oracle_mod, codec):
-    """BASELINE config 2 at its full size (2^24 IDs, the launch configuration bench.py times)."""
-    rng = np.random.default_rng(7)
+def test_config2_full_size(B, oracle_mod, codec):
+    """BASELINE config 2 at its full size (3 streams of 2^24 IDs, the launch configuration bench.py times): every
+    byte of every stream against the serial oracle, under both encoder rules."""
     for sub, (mean, outl) in enumerate(((2.0, 0.0), (256.0, 0.0), (256.0, 0.01))):
         ids = streams.gap_stream(1 << 24, mean, seed=2, W=32, outlier_frac=outl, sub=sub, device=torch.device("cuda"))
-        _full_size_sampled(B, oracle_mod, ids, 32, rng, codec=codec)
+        _full_size(B, oracle_mod, ids, 32, codec=codec)
 
 
-def test_config5_largest_buffers_sampled(B, oracle_mod):
-    """The 1 GB ends of the config-5 sweep (2^28 u32 IDs with gaps of 1; 2^27 u64 IDs with gaps of mean 4096):
-    tile counts, offsets and directory entries far beyond the 2^24-ID case (1 GB streams: offsets over 2^32 / 16
-    are still exact)."""
-    rng = np.random.default_rng(8)
+def test_config5_large_cells_full(B, oracle_mod):
+    """The upper half of the config-5 sweep, every byte against the serial oracle: single buffers of 16 MB, 64 MB
+    and 256 MB (u32 and u64; gap means 1, 16, 4096 where the IDs fit the type), plus ragged sizes around 2^23 IDs
+    (the kernel is then several waves deep: every warp draws many tiles, look-backs span hundreds of super-tiles)."""
     dev = torch.device("cuda")
-    _full_size_sampled(B, oracle_mod, streams.gap_stream(1 << 28, 1.0, seed=5, W=32, device=dev), 32, rng, samples=64)
+    for W in (32, 64):
+        for k in (12, 13, 14):
+            n = (4 ** k) // (W // 8)
+            for mean in (1.0, 16.0, 4096.0):
+                if W == 32 and n * mean >= 2 ** 32:
+                    continue                               # exceeds the u32 ID space (DESIGN.md §1)
+                _full_size(B, oracle_mod, streams.gap_stream(n, mean, seed=5, W=W, device=dev), W)
+                torch.cuda.empty_cache()
+        _full_size(B, oracle_mod, streams.gap_stream((1 << 23) + 77, 256.0, seed=6, W=W, outlier_frac=0.01, device=dev), W)
+        _full_size(B, oracle_mod, streams.gap_stream((1 << 23) - 129, 2.0, seed=7, W=W, device=dev), W, codec=BP128)
+
+
+def test_config5_largest_buffers_full(B, oracle_mod):
+    """The 1 GB ends of the config-5 sweep (2^28 u32 IDs with gaps of 1; 2^27 u64 IDs with gaps of mean 4096): tile
+    counts, offsets and directory entries far beyond the 2^24-ID case (offsets over 2^32 / 16 are still exact)."""
+    dev = torch.device("cuda")
+    _full_size(B, oracle_mod, streams.gap_stream(1 << 28, 1.0, seed=5, W=32, device=dev), 32)
     torch.cuda.empty_cache()
-    _full_size_sampled(B, oracle_mod, streams.gap_stream(1 << 27, 4096.0, seed=5, W=64, device=dev), 64, rng, samples=64)
+    _full_size(B, oracle_mod, streams.gap_stream(1 << 27, 4096.0, seed=5, W=64, device=dev), 64)
     torch.cuda.empty_cache()
+
+
+def test_exclusive_flag_same_bytes(B, oracle_mod):
+    """BFSC_CODEC_FLAG_EXCLUSIVE (static first tiles, include/bfsc.h) changes the schedule, not the bytes: single and
+    batch calls, both encoder rules, against the oracle."""
+    dev = torch.device("cuda")
+    for W in (32, 64):
+        n = 128 * 64 * 700 + 99                                  # more tiles than one resident wave of CTAs
+        x = streams.gap_stream(n, 16.0, seed=41, W=W, outlier_frac=0.01)
+        for codec in CODECS:
+            ref = oracle_mod.compress(_np(x, W), 0, codec=codec)
+            cap = B.compress_bound(n, W)
+            out = torch.empty(cap, dtype=torch.uint8, device=dev)
+            nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
+            ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
+            status = torch.zeros(1, dtype=torch.int32, device=dev)
+            B.compress_codec(codec | B.CODEC_FLAG_EXCLUSIVE, x.to(dev), n, W, 0, out, nbytes, ws, status)
+            torch.cuda.synchronize()
+            assert int(status.item()) == 0 and int(nbytes.item()) == len(ref)
+            assert np.array_equal(out[:len(ref)].cpu().numpy(), ref)
+        counts = streams.log_uniform_counts(500, 6, 15, W, seed=42)
+        ids, off = streams.batch_of_streams(counts, 16.0, seed=42, W=W)
+        ref, ref_off = oracle_mod.compress_batch(_np(ids, W), off.numpy().astype(np.uint64), 1024)
+        out = torch.empty(B.batch_compress_bound(counts.tolist(), W), dtype=torch.uint8, device=dev)
+        out_off = torch.zeros(counts.numel() + 1, dtype=torch.int64, device=dev)
+        ws = torch.empty(B.workspace_bytes(ids.numel(), counts.numel(), W), dtype=torch.uint8, device=dev)
+        status = torch.zeros(1, dtype=torch.int32, device=dev)
+        B.compress_batch_codec(PFOR | B.CODEC_FLAG_EXCLUSIVE, ids.to(dev), off.to(dev), counts.numel(), W, 1024, out, out_off, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0 and np.array_equal(out_off.cpu().numpy().astype(np.uint64), ref_off)
+        assert np.array_equal(out[:len(ref)].cpu().numpy(), ref)
+
+
+def test_two_compress_calls_run_concurrently(B, oracle_mod):
+    """Two bfsc_compress calls on two CUDA streams of one device at the same time, 200 times (every tile is
+    drawn by ticket: no co-residency assumption), each with its own workspace; bytes vs the
+    oracle every time (the inputs alternate, so a stale result cannot pass)."""
+    dev = torch.device("cuda")
+    W = 32
+    n = (1 << 21) + 333
+    xs = [streams.gap_stream(n, m, seed=31 + i, W=W, outlier_frac=o, device=dev) for i, (m, o) in enumerate(((2.0, 0.0), (256.0, 0.01)))]
+    refs = [oracle_mod.compress(_np(x, W), 0) for x in xs]
+    cap = B.compress_bound(n, W)
+    outs = [torch.empty(cap, dtype=torch.uint8, device=dev) for _ in range(2)]
+    nbs = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(2)]
+    wss = [torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev) for _ in range(2)]
+    sts = [torch.zeros(1, dtype=torch.int32, device=dev) for _ in range(2)]
+    cs = [torch.cuda.Stream(device=dev) for _ in range(2)]
+    torch.cuda.synchronize()
+    for rep in range(200):
+        for k in range(2):
+            with torch.cuda.stream(cs[k]):
+                B.compress(xs[(k + rep) % 2], n, W, 0, outs[k], nbs[k], wss[k], sts[k])
+        if rep % 20 == 19 or rep < 2:
+            torch.cuda.synchronize()
+            for k in range(2):
+                ref = refs[(k + rep) % 2]
+                assert int(sts[k].item()) == 0 and int(nbs[k].item()) == len(ref)
+                assert np.array_equal(outs[k][:len(ref)].cpu().numpy(), ref), (rep, k)
+    torch.cuda.synchronize()
+
+
+def _mutations(rng, good, W, n_mut):
+    """Seeded single-byte (and a few two-byte) mutations of a stream, biased to the bytes a decoder reads as
+    structure: stream header, directory, block headers, exception areas."""
+    nb = int(good[24:28].view(np.uint32)[0])
+    d = good[32:32 + 4 * (nb + 1)].view(np.uint32).astype(np.int64)
+    spots = list(range(4, 28)) + list(range(32, 32 + 4 * (nb + 1)))
+    for k in range(nb):
+        o = 16 * int(d[k])
+        b, ne = int(good[o + 8]), int(good[o + 9])
+        spots += [o + 8, o + 9]
+        if ne:
+            spots += list(range(o + 16 + 16 * b, o + 16 + 16 * b + ne + 2))
+    spots = [x for x in spots if x < len(good)]
+    for _ in range(n_mut):
+        s = good.copy()
+        for _ in range(1 if rng.random() < 0.8 else 2):
+            p = spots[int(rng.integers(0, len(spots)))]
+            s[p] = int(rng.integers(0, 256)) if rng.random() < 0.5 else (int(s[p]) + int(rng.choice([1, -1, 2, 16, 128]))) % 256
+        yield s
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_decoder_fuzz_matches_oracle_verdict(B, oracle_mod, W):
+    """FORMAT.md §4 on the GPU, single and batch calls, staged fast path and wide (> 336 B) blocks: for seeded
+    mutations of header, directory, block-header and exception bytes the device status equals the oracle's verdict
+    (OK / CORRUPT / DST_TOO_SMALL); when both accept, the IDs are equal; guard elements behind the output are never
+    written; truncated input is rejected."""
+    dev = torch.device("cuda")
+    rng = np.random.default_rng(1000 + W)
+    dt = np.uint32 if W == 32 else np.uint64
+    tdt = torch.int32 if W == 32 else torch.int64
+    n = 128 * 9 + 50
+    g = rng.integers(1, 40, size=n).astype(np.uint64)
+    g[rng.integers(0, n, size=40)] = np.uint64(1) << np.uint64(21)                       # exceptions in most blocks
+    g[128 * 4:128 * 6] = rng.integers(1 << 24, 1 << 26, size=256).astype(np.uint64)      # two blocks over the staged size (b = 26)
+    x = (np.cumsum(g) & np.uint64((1 << W) - 1)).astype(dt)
+    good = oracle_mod.compress(x, 0)
+    cap_ids = n + 64
+    ws = torch.empty(B.workspace_bytes(cap_ids + 200, 2, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+    cap_b = cap_ids + 200                                            # the batch call decodes a 200-ID stream in front of the mutated one
+    back = torch.empty(cap_b + 16, dtype=tdt, device=dev)
+    id_off = torch.zeros(3, dtype=torch.int64, device=dev)
+    small = oracle_mod.compress(x[:200], 0)
+    verdicts = {0: 0, 2: 0, 3: 0}
+
+    def oracle_verdict(s):
+        try:
+            return 0, oracle_mod.decompress(s, W, capacity=cap_ids)
+        except oracle_mod.OracleError as ex:
+            return ex.code, None
+
+    def check(s, in_bytes=None):
+        code, ids = oracle_verdict(s if in_bytes is None else s[:in_bytes])
+        d_in = torch.from_numpy(s).to(dev)
+        # single call
+        back.fill_(-7); status.zero_()
+        B.decompress(d_in, len(s) if in_bytes is None else in_bytes, W, back[:cap_ids], n_out, ws, status)
+        torch.cuda.synchronize()
+        st = int(status.item())
+        assert st == code, f"single: device status {st}, oracle {code}"
+        assert bool((back[cap_ids:] == -7).all())
+        if code == 0:
+            assert int(n_out.item()) == len(ids) and np.array_equal(_np(back[:len(ids)], W), ids)
+        verdicts[code] = verdicts.get(code, 0) + 1
+        # batch call: [intact small stream | s]
+        if in_bytes is None:
+            both = torch.from_numpy(np.concatenate([small, s])).to(dev)
+            offs = torch.tensor([0, len(small), len(small) + len(s)], dtype=torch.int64, device=dev)
+            back.fill_(-7); status.zero_()
+            B.decompress_batch(both, offs, 2, W, back[:cap_b], id_off, ws, status)
+            torch.cuda.synchronize()
+            st = int(status.item())
+            assert st == code, f"batch: device status {st}, oracle {code}"
+            assert bool((back[cap_b:] == -7).all())
+            if code == 0:
+                assert np.array_equal(_np(back[200:200 + len(ids)], W), ids)
+
+    check(good)
+    for s in _mutations(rng, good, W, 400):
+        check(s)
+    for cut in (16, 31, 32, 48, len(good) - 16, len(good) - 1):
+        check(good, in_bytes=cut)
+    assert verdicts[0] > 20 and verdicts[3] > 100            # the mutations reach both outcomes

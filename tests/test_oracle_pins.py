@@ -256,3 +256,22 @@ def test_bp128_threshold_batch_and_roundtrip(oracle_mod):
                 assert np.array_equal(s, one)
             back, id_off = oracle_mod.decompress_batch(out, out_off, W, len(ids))
             assert np.array_equal(back, ids) and np.array_equal(id_off, off)
+
+
+def test_compress_bound_closed_form(oracle_mod):
+    """FORMAT.md §3, pinned from BOTH sides: bound(n, W) == 32 + align16(4 (nb + 1)) + nb (16 + 16 W), typed out
+    here, and attained exactly by an incompressible buffer of full blocks (every delta needs W bits)."""
+    hand = {(0, 32): 48, (1, 32): 32 + 16 + 528, (128, 32): 32 + 16 + 528, (129, 32): 32 + 16 + 2 * 528,
+            (1000, 32): 32 + 48 + 8 * 528, (16384, 32): 32 + 528 + 128 * 528, (1 << 24, 64): 32 + 524304 + 131072 * 1040,
+            (0, 64): 48, (127, 64): 32 + 16 + 1040, (385, 64): 32 + 32 + 4 * 1040, (1 << 20, 64): 32 + 32784 + 8192 * 1040,
+            (3 * 128, 32): 32 + 16 + 3 * 528}
+    for (n, W), want in hand.items():
+        nb = -(-n // 128)
+        assert want == 32 + -(-4 * (nb + 1) // 16) * 16 + nb * (16 + 16 * W)
+        assert oracle_mod.compress_bound(n, W) == want, (n, W)
+    for W in (32, 64):                                             # tight: constant gap 2^(W-1) + 1 (mod 2^W) -> every delta is W bits wide
+        n = 128 * 5
+        x = np.array([(j * ((1 << (W - 1)) + 1)) % (1 << W) for j in range(n)], dtype=np.uint32 if W == 32 else np.uint64)
+        s = oracle_mod.compress(x)
+        # the first delta of each block is 0, the other 127 have W bits: b = W, no exceptions
+        assert len(s) == oracle_mod.compress_bound(n, W)

@@ -179,6 +179,7 @@ def test_corrupt_streams_rejected(oracle_mod):
     bad(lambda s: s.__setitem__(4, 2))                             # version
     bad(lambda s: s.__setitem__(5, 64))                            # W
     bad(lambda s: s.__setitem__(6, 9))                             # mode
+    bad(lambda s: s.__setitem__(7, 1))                             # reserved header byte (FORMAT.md §4)
     bad(lambda s: s.__setitem__(slice(16, 24), np.frombuffer(struct.pack("<Q", len(good) + 16), np.uint8)))
     bad(lambda s: s.__setitem__(slice(24, 28), np.frombuffer(struct.pack("<I", 99), np.uint8)))
     bad(lambda s: s.__setitem__(slice(36, 40), np.frombuffer(struct.pack("<I", 1), np.uint8)))      # dir[1] backwards
@@ -187,3 +188,32 @@ def test_corrupt_streams_rejected(oracle_mod):
     bad(lambda s: s.__setitem__(first_blk + 9, 127))               # block larger than its span
     with pytest.raises(oracle_mod.OracleError):
         oracle_mod.decompress(good[:-16], 32)                      # truncated
+
+
+def test_exception_positions_must_ascend(oracle_mod):
+    """FORMAT.md §4: an exception list whose positions are not strictly ascending (a duplicate, or two swapped
+    entries) is rejected by both decoders; the untouched stream and a stream whose positions were replaced by
+    OTHER ascending ones still decode (to different IDs: positions are data)."""
+    for W in (32, 64):
+        d = np.ones(128, dtype=np.uint64)
+        d[0] = 0
+        d[[9, 40, 41, 100]] = np.uint64(1 << 20)
+        x = (np.uint64(7) + np.cumsum(d)).astype(np.uint32 if W == 32 else np.uint64)
+        good = oracle_mod.compress(x)
+        blk = 16 * struct.unpack("<I", good[32:36].tobytes())[0]
+        assert good[blk + 8] == 1 and good[blk + 9] == 4           # b = 1, four exceptions
+        e = blk + 16 + 16
+        assert list(good[e:e + 4]) == [9, 40, 41, 100]
+        assert np.array_equal(oracle_mod.decompress(good, W), x)
+        assert witness.decode_stream(good.tobytes(), W) == [int(v) for v in x]
+        for pos in ([9, 40, 40, 100], [9, 41, 40, 100], [100, 41, 40, 9], [9, 9, 9, 9]):
+            s = good.copy()
+            s[e:e + 4] = pos
+            with pytest.raises(oracle_mod.OracleError):
+                oracle_mod.decompress(s, W)
+            with pytest.raises(ValueError):
+                witness.decode_stream(s.tobytes(), W)
+        s = good.copy()
+        s[e:e + 4] = [1, 2, 3, 127]                                # other ascending positions: well-formed
+        y = oracle_mod.decompress(s, W)
+        assert witness.decode_stream(s.tobytes(), W) == [int(v) for v in y] and not np.array_equal(y, x)
