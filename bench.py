@@ -37,9 +37,26 @@ SEED = 2
 W = 32
 METRIC = "codec_throughput_encode_plus_decode"
 UNIT = "GB/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (k_enc_tiles<32>, stream a,
-# 2^24 IDs), from the committed `ncu --set full` capture profiles/r1_enc_tiles_ncu_summary.txt (67.30 + 1.73 MB).
-NCU_TRAFFIC_BYTES = {"encode_a": 69_034_240, "decode_a": 24_271_872, "source": "profiles/r1_*_tiles_ncu_summary.txt"}
+NCU_SUMMARIES = {"encode": "profiles/r2_enc_tiles_ncu_summary.txt", "decode": "profiles/r2_dec_tiles_ncu_summary.txt"}
+
+
+def ncu_traffic(kind: str, stream: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum (bytes) of ONE launch of the encode / decode kernel on stream
+    'a' | 'b' | 'c', read from the committed `ncu --set full` summary (profiles/README.md names the command that
+    made it); None when the file or the section is missing."""
+    path = os.path.join(ROOT, NCU_SUMMARIES[kind])
+    try:
+        sec, rd, wr = None, None, None
+        for line in open(path):
+            if line.startswith("== stream "):
+                sec = line.split()[2]
+            elif sec == stream and line.startswith("dram__bytes_read.sum "):
+                rd = float(line.split()[1])
+            elif sec == stream and line.startswith("dram__bytes_write.sum "):
+                wr = float(line.split()[1])
+        return None if rd is None or wr is None else int(round((rd + wr) * 1e6))     # ncu prints MB
+    except OSError:
+        return None
 
 
 def peaks():
@@ -134,21 +151,24 @@ def time_oracle(host_ids, threads, reps=1):
 
 
 def run_reference(args, rank, world):
+    """This tier's reference arm: the oracle, as it stands, on the host cores — on the FULL workload (3 streams of
+    2^log2n IDs, encode + decode per step: about 0.3 s at 16 threads), unless --steps of them would exceed
+    --ref-budget-s; then, and only then, on the first 2^p IDs of every stream (said in config.sample)."""
     if rank != 0:
         return
     cores = len(os.sched_getaffinity(0))
-    # Bounded sample: the first 2^p IDs of each stream, p chosen from a quick calibration so that the whole
-    # --steps K run takes about --ref-budget-s (default 90) seconds of CPU work (p in 14..22).
-    full = [np_view(t) for t in make_streams("cpu", 1 << 22)]
+    full = [np_view(t) for t in make_streams("cpu", 1 << args.log2n)]
     time_oracle([h[:1 << 16] for h in full], cores)                       # warm-up (builds the oracle's C library)
-    cal, _, _ = time_oracle([h[:1 << 18] for h in full], cores)
-    per_id = cal / (3 << 18)
-    budget = args.ref_budget_s / max(args.steps, 1)
-    p = 22
+    cal, _, _ = time_oracle([h[:1 << 20] for h in full], cores)
+    per_id = cal / (3 << 20)
+    budget = args.ref_budget_s / max(args.steps + args.warmup, 1)
+    p = args.log2n
     while p > 14 and per_id * (3 << p) > budget:
         p -= 1
     n = 1 << p
     host = [h[:n] for h in full]
+    for _ in range(args.warmup):
+        time_oracle(host, cores)
     times = []
     raw = ratio = 0
     for _ in range(args.steps):
@@ -156,16 +176,25 @@ def run_reference(args, rank, world):
         times.append(dt)
     ms = 1e3 * sum(times) / len(times)
     val = raw / (ms * 1e-3) / 1e9
-    sample = f"first 2^{p} of the 2^24 IDs of each of the 3 streams, encode+decode, {cores} threads"
+    sample = (f"the full workload: all 2^{p} IDs of each of the 3 streams" if p == args.log2n else
+              f"first 2^{p} of the 2^{args.log2n} IDs of each of the 3 streams (the full workload would exceed --ref-budget-s)")
+    sample += f", encode+decode, {cores} threads"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u32", "data": "synthetic", "ratio": ratio,
-        "config": {"workload": "configs[1]: 3 sorted u32 streams (a,b,c), seed 2; oracle on a bounded sample", "sample": sample},
+        "config": workload_config(args.log2n, world) | {"sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
+
+
+def workload_config(log2n, world):
+    """config of the JSON line: the same for both arms (the driver compares them)."""
+    return {"workload": f"configs[1]: 3 sorted u32 streams of 2^{log2n} IDs (a: geometric gaps mean 2, b: mean 256, "
+                        "c: mean 256 + 1% outliers in [2^16,2^24)), seed 2; step = compress a,b,c then decompress a,b,c",
+            "raw_threshold_bytes": 0, "parallelism": "replicas only" if world > 1 else "single GPU"}
 
 
 # --------------------------------------------------------------------------- CUDA arm
@@ -227,7 +256,6 @@ def run_ours(args, rank, local_rank, world):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    clocks = sampler.stop()
     launches_timed = B.kernel_launches() - launches0
     ms_total = t0.elapsed_time(t1)
     ms_total = max_over_ranks(ms_total, world, dev)
@@ -243,6 +271,7 @@ def run_ours(args, rank, local_rank, world):
     kTrials = 5                                              # runs per call: median reported, min alongside
     enc_ms, dec_ms, enc_min, dec_min = [], [], [], []
     bp_enc_ms, bp_dec_ms = [], []                            # the same calls under the BP128 rule (FORMAT.md §7)
+    ex_enc_ms = []                                           # bfsc_compress with BFSC_CODEC_FLAG_EXCLUSIVE (static first tiles, include/bfsc.h)
     nbytes_bp = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(S)]
     for s in range(S):
         c_ids = [ids[s]] + [ids[s].clone() for _ in range(kCopies - 1)]
@@ -272,6 +301,11 @@ def run_ours(args, rank, local_rank, world):
         dec_ms.append(float(np.median(dec_runs)))
         enc_min.append(min(enc_runs))
         dec_min.append(min(dec_runs))
+        ex_call = lambda c: B.compress_codec(B.CODEC_PFOR | B.CODEC_FLAG_EXCLUSIVE, c_ids[c], n, W, 0, c_out[c], nbytes[s], ws, status)   # noqa: E731
+        for c in range(kCopies):
+            ex_call(c)
+        torch.cuda.synchronize()
+        ex_enc_ms.append(float(np.median([run_of(ex_call) for _ in range(kTrials)])))
         bp_call = lambda c: B.compress_codec(B.CODEC_BP128, c_ids[c], n, W, 0, c_out[c], nbytes_bp[s], ws, status)   # noqa: E731
         for c in range(kCopies):
             bp_call(c)
@@ -283,47 +317,100 @@ def run_ours(args, rank, local_rank, world):
         del c_ids
     assert int(status.item()) == 0, f"device status {int(status.item())}"
     value = whole_job_value(2 * S * raw_bytes, world, ms_step * 1e-3) / 1e9
+    # nvidia-smi is sampled every 20 ms from before the timed region (a few milliseconds long) to the end of the per-call
+    # runs above (the same calls, a few seconds of them): the clocks under this load, not of one idle instant
+    clocks = sampler.stop()
+    clocks["window"] = "timed region + the per-call runs of the same calls that follow it"
 
-    # ---- the batched path (BASELINE configs[4], batch part): 4096 buffers of 256 B - 64 KB (log-uniform), gaps of
-    # mean 16, u32, one bfsc_compress_batch / bfsc_decompress_batch per call; reported beside the headline, not in it
+    # ---- the batched path, reported beside the headline, not in it: (1) BASELINE configs[4]'s batch of 4096 buffers of
+    # 256 B - 64 KB (log-uniform), gaps of mean 16, u32, threshold 0; (2) the largest BFS level of configs[3] (R-MAT 25,
+    # u64 IDs, 64 destination buffers by contiguous vertex range, 1 KB threshold). One bfsc_compress_batch /
+    # bfsc_decompress_batch per call, on rotating copies (> 2 x L2 between a buffer's write and its re-read); timed
+    # twice: enqueued from Python (host time included when it is the longer one) and replayed from a CUDA graph
+    # captured around the same C-ABI calls (device-side time of the kernel chain).
     batch = None
-    if rank == 0 and args.log2n == LOG2_N:
-        counts = streams.log_uniform_counts(4096, 8, 16, 32, seed=5)
-        b_ids, b_off = streams.batch_of_streams(counts, 16.0, seed=5, W=W, device=dev)
-        b_ids, b_off = b_ids.to(dev), b_off.to(dev)
-        bn, nbuf = b_ids.numel(), b_off.numel() - 1
-        bcap = B.batch_compress_bound(counts.tolist(), W)
-        kB = 6                                               # rotating copies: 6 x (49 MB in + out) > 2 x L2
-        bi = [b_ids] + [b_ids.clone() for _ in range(kB - 1)]
-        bo = [torch.empty(bcap, dtype=torch.uint8, device=dev) for _ in range(kB)]
-        bb = [torch.empty(bn, dtype=b_ids.dtype, device=dev) for _ in range(kB)]
-        b_out_off = torch.zeros(nbuf + 1, dtype=torch.int64, device=dev)
-        b_id_off = torch.zeros(nbuf + 1, dtype=torch.int64, device=dev)
-        bws = torch.empty(B.workspace_bytes(bn, nbuf, W), dtype=torch.uint8, device=dev)
+    if rank == 0 and args.log2n == LOG2_N and not args.no_batch:
+        def measure_batch(b_ids, b_off, Wb, thr, label):
+            bn, nbuf = b_ids.numel(), b_off.numel() - 1
+            counts_l = (b_off[1:] - b_off[:-1]).tolist()
+            bcap = B.batch_compress_bound(counts_l, Wb)
+            kB = int(max(3, min(8, -(-(300 << 20) // (2 * bn * (Wb // 8) + 1)))))
+            bi = [b_ids] + [b_ids.clone() for _ in range(kB - 1)]
+            bo = [torch.empty(bcap, dtype=torch.uint8, device=dev) for _ in range(kB)]
+            bb = [torch.empty(bn, dtype=b_ids.dtype, device=dev) for _ in range(kB)]
+            b_out_off = torch.zeros(nbuf + 1, dtype=torch.int64, device=dev)
+            b_id_off = torch.zeros(nbuf + 1, dtype=torch.int64, device=dev)
+            bws = torch.empty(B.workspace_bytes(bn, nbuf, Wb), dtype=torch.uint8, device=dev)
+            enc = lambda c: B.compress_batch(bi[c], b_off, nbuf, Wb, thr, bo[c], b_out_off, bws, status)         # noqa: E731
+            dec = lambda c: B.decompress_batch(bo[c], b_out_off, nbuf, Wb, bb[c], b_id_off, bws, status)      # noqa: E731
 
-        def run_b(call, reps_b=10):
-            for c in range(kB):
-                call(c)
-            torch.cuda.synchronize()
-            a0, a1 = mk(), mk()
-            a0.record()
-            for _ in range(reps_b):
+            def run_b(call, reps_b=10):
                 for c in range(kB):
                     call(c)
-            a1.record()
-            torch.cuda.synchronize()
-            return a0.elapsed_time(a1) / (reps_b * kB)
+                torch.cuda.synchronize()
+                a0, a1 = mk(), mk()
+                a0.record()
+                for _ in range(reps_b):
+                    for c in range(kB):
+                        call(c)
+                a1.record()
+                torch.cuda.synchronize()
+                return a0.elapsed_time(a1) / (reps_b * kB)
 
-        b_enc = float(np.median([run_b(lambda c: B.compress_batch(bi[c], b_off, nbuf, W, 0, bo[c], b_out_off, bws, status)) for _ in range(3)]))
-        b_dec = float(np.median([run_b(lambda c: B.decompress_batch(bo[c], b_out_off, nbuf, W, bb[c], b_id_off, bws, status)) for _ in range(3)]))
-        assert int(status.item()) == 0 and torch.equal(bb[kB - 1], b_ids) and torch.equal(b_id_off, b_off), "batch: decode != input"
-        b_raw, b_comp = bn * (W // 8), int(b_out_off[-1].item())
-        batch = {"workload": "configs[4] batch: 4096 buffers of 256 B-64 KB (log-uniform), gaps mean 16, u32, threshold 0, seed 5",
-                 "n_buf": nbuf, "raw_bytes": b_raw, "ratio": b_raw / b_comp, "encode_ms": b_enc, "decode_ms": b_dec,
-                 "encode_GBps_in": b_raw / b_enc / 1e6, "decode_GBps_out": b_raw / b_dec / 1e6,
-                 "encode_frac_of_peak": (b_raw + b_comp) / b_enc / 1e6 / peaks()[0], "decode_frac_of_peak": (b_raw + b_comp) / b_dec / 1e6 / peaks()[0],
-                 "note": "per call incl. the host's enqueue time when that is the longer one (4 kernels per compress call)"}
-        del bi, bo, bb
+            def run_graph(call, reps_b=10):
+                side = torch.cuda.Stream(device=dev)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.stream(side):
+                    with torch.cuda.graph(g, stream=side):
+                        for c in range(kB):
+                            call(c)
+                torch.cuda.synchronize()
+                g.replay()
+                torch.cuda.synchronize()
+                a0, a1 = mk(), mk()
+                a0.record()
+                for _ in range(reps_b):
+                    g.replay()
+                a1.record()
+                torch.cuda.synchronize()
+                return a0.elapsed_time(a1) / (reps_b * kB)
+
+            b_enc = float(np.median([run_b(enc) for _ in range(3)]))
+            b_dec = float(np.median([run_b(dec) for _ in range(3)]))
+            g_enc = float(np.median([run_graph(enc) for _ in range(3)]))
+            g_dec = float(np.median([run_graph(dec) for _ in range(3)]))
+            assert int(status.item()) == 0 and torch.equal(bb[kB - 1], b_ids) and torch.equal(b_id_off, b_off), "batch: decode != input"
+            b_raw, b_comp = bn * (Wb // 8), int(b_out_off[-1].item())
+            pk = peaks()[0]
+            return {"workload": label, "n_buf": nbuf, "raw_bytes": b_raw, "ratio": b_raw / b_comp,
+                    "encode_ms": b_enc, "decode_ms": b_dec, "encode_graph_ms": g_enc, "decode_graph_ms": g_dec,
+                    "encode_GBps_in": b_raw / g_enc / 1e6, "decode_GBps_out": b_raw / g_dec / 1e6,
+                    "encode_frac_of_peak": (b_raw + b_comp) / g_enc / 1e6 / pk, "decode_frac_of_peak": (b_raw + b_comp) / g_dec / 1e6 / pk,
+                    "encode_frac_of_peak_enqueued": (b_raw + b_comp) / b_enc / 1e6 / pk,
+                    "decode_frac_of_peak_enqueued": (b_raw + b_comp) / b_dec / 1e6 / pk,
+                    "note": "*_graph_ms and the fractions: replayed from a CUDA graph (device-side time of the call's kernel chain); "
+                            "encode_ms / decode_ms: enqueued from Python, per call incl. the host's time when that is the longer one"}
+
+        counts = streams.log_uniform_counts(4096, 8, 16, 32, seed=5)
+        b_ids, b_off = streams.batch_of_streams(counts, 16.0, seed=5, W=W, device=dev)
+        batch = {"b4096": measure_batch(b_ids.to(dev), b_off.to(dev), W, 0,
+                                        "configs[4] batch: 4096 buffers of 256 B-64 KB (log-uniform), gaps mean 16, u32, threshold 0, seed 5")}
+        del b_ids, b_off
+        try:
+            from paper_1704_00513_b200.workloads import rmat
+            G = rmat.Graph(25, 16, seed=4, device=dev)
+            root = G.roots(1, seed=4)[0]
+            big = max(G.bfs_frontiers(root), key=lambda f: f.numel())
+            del G
+            torch.cuda.empty_cache()
+            vals, off64 = streams.split_block(big, 64, 1 << 25)
+            batch["rmat25_level"] = measure_batch(streams.as_ids(vals, 64).to(dev), off64.to(dev), 64, 1024,
+                                                  f"configs[3]: largest BFS level of R-MAT 25 (seed 4, first root), {vals.numel()} u64 IDs "
+                                                  "in 64 buffers by contiguous vertex range, threshold 1 KB")
+            del vals, off64, big
+            torch.cuda.empty_cache()
+        except torch.cuda.OutOfMemoryError:
+            batch["rmat25_level"] = None
 
     # ---- end to end through the host-buffer C-ABI calls (pinned host memory) ----
     e2e = None
@@ -408,35 +495,43 @@ def run_ours(args, rank, local_rank, world):
                               "encode_alg_GBps": alg_bp / bp_enc_ms[s] / 1e6, "decode_alg_GBps": alg_bp / bp_dec_ms[s] / 1e6,
                               "encode_frac_of_peak": alg_bp / bp_enc_ms[s] / 1e6 / peak, "decode_frac_of_peak": alg_bp / bp_dec_ms[s] / 1e6 / peak,
                               "encode_frac_of_8TBps": alg_bp / bp_enc_ms[s] / 1e6 / 8000.0, "decode_frac_of_8TBps": alg_bp / bp_dec_ms[s] / 1e6 / 8000.0}
-    # dominant call = encode of stream (a): most raw bytes per compressed byte, the headline dense frontier
-    dom = STREAMS[0][0]
-    alg_a = raw_bytes + comp[0] + 8
+        per[name]["encode_exclusive_flag"] = {"encode_ms": ex_enc_ms[s], "encode_alg_GBps": alg / ex_enc_ms[s] / 1e6,
+                                              "encode_frac_of_peak": alg / ex_enc_ms[s] / 1e6 / peak,
+                                              "encode_frac_of_8TBps": alg / ex_enc_ms[s] / 1e6 / 8000.0,
+                                              "note": "BFSC_CODEC_FLAG_EXCLUSIVE: the caller vouches that nothing else runs on the device (include/bfsc.h)"}
+    # dominant kernel = k_enc_tiles<32> (96 of the 160 us of a step); the roofline object is that of its SLOWEST call,
+    # the one furthest from the roofline (stream c: exceptions); a and b beside it
+    names = [nm for nm, _, _ in STREAMS]
+    dom_i = int(np.argmax(enc_ms))
+    dom = names[dom_i]
+    key = "abc"[dom_i]
     full = args.log2n == LOG2_N
-    roof = {"bound": "hbm", "kernel": "k_enc_tiles<32> (+ its 1-CTA k_enc_plan): the bfsc_compress call on stream a",
+    roof = {"bound": "hbm", "kernel": f"k_enc_tiles<32, false> (+ its 1-CTA k_enc_plan): the bfsc_compress call on stream {key}, the slowest of a, b, c",
             "achieved": per[dom]["encode_alg_GBps"],
             "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": per[dom]["encode_alg_GBps"] / peak,
-            "algorithmic_bytes_per_launch": alg_a, "traffic": NCU_TRAFFIC_BYTES["encode_a"] if full else None,
-            "traffic_source": NCU_TRAFFIC_BYTES["source"],
-            "decode": {"kernel": "k_dec_tiles<32>: the bfsc_decompress call on stream a", "achieved": per[dom]["decode_alg_GBps"],
-                       "frac": per[dom]["decode_alg_GBps"] / peak, "traffic": NCU_TRAFFIC_BYTES["decode_a"] if full else None}}
+            "algorithmic_bytes_per_launch": raw_bytes + comp[dom_i] + 8,
+            "traffic": ncu_traffic("encode", key) if full else None, "traffic_source": NCU_SUMMARIES["encode"],
+            "per_stream": {"abc"[i]: {"encode_frac": per[names[i]]["encode_frac_of_peak"], "decode_frac": per[names[i]]["decode_frac_of_peak"],
+                                      "encode_traffic": ncu_traffic("encode", "abc"[i]) if full else None,
+                                      "decode_traffic": ncu_traffic("decode", "abc"[i]) if full else None} for i in range(S)},
+            "decode": {"kernel": f"k_dec_tiles<32, false>: the bfsc_decompress call on stream {key}", "achieved": per[dom]["decode_alg_GBps"],
+                       "frac": per[dom]["decode_alg_GBps"] / peak, "traffic": ncu_traffic("decode", key) if full else None,
+                       "traffic_source": NCU_SUMMARIES["decode"]}}
     cpu = None
     if not args.no_cpu:
         cores = len(os.sched_getaffinity(0))
-        m = 1 << min(args.log2n, 22)
-        host = [np_view(t[:m]) for t in ids]
+        host = [np_view(t) for t in ids]                     # the whole workload: same config as the GPU line
         dt, raw, _ = time_oracle(host, cores)
         m1 = 1 << min(args.log2n, 20)
-        dt1, raw1, _ = time_oracle([np_view(t[:m1]) for t in ids], 1)
+        dt1, raw1, _ = time_oracle([h[:m1] for h in host], 1)
         cpu = {"value": raw / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "single_thread": {"value": raw1 / dt1 / 1e9, "unit": UNIT, "sample": f"first 2^{min(args.log2n, 20)} IDs of each stream"},
-               "sample": f"first 2^{min(args.log2n, 22)} IDs of each of the 3 streams, encode+decode, {cores} threads, 1 pass"}
+               "single_thread": {"value": raw1 / dt1 / 1e9, "unit": UNIT, "sample": f"first 2^{min(args.log2n, 20)} IDs of each stream, 1 thread"},
+               "sample": f"the full workload: all 2^{args.log2n} IDs of each of the 3 streams, encode+decode, {cores} threads, 1 pass"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
         "data": "synthetic",
-        "config": {"workload": f"configs[1]: 3 sorted u32 streams of 2^{args.log2n} IDs (a: geometric gaps mean 2, b: mean 256, "
-                               "c: mean 256 + 1% outliers in [2^16,2^24)), seed 2; step = compress a,b,c then decompress a,b,c",
-                   "raw_threshold_bytes": 0, "parallelism": "replicas only" if world > 1 else "single GPU",
+        "config": workload_config(args.log2n, world) | {
                    "l2_policy": "inputs larger than L2: >=170 MB of other streams' traffic between any write and its re-read",
                    "per_call_timing": "events around runs of back-to-back launches of one call on 4 rotating copies of the stream, "
                                       "average per launch; median of 5 runs (min alongside)"},
@@ -456,6 +551,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=LOG2_N, help="IDs per stream = 2^log2n (default: the BASELINE size)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-batch", action="store_true", help="skip the batched-path section (4096-buffer batch, R-MAT 25 level)")
     ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for the whole run")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
