@@ -21,6 +21,7 @@ _lib = None
 
 OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT = 0, 1, 2, 3
 CODEC_PFOR, CODEC_BP128 = 1, 2          # encoder rule = mode byte of the stream (FORMAT.md §1, §7)
+FLAG_RAW_FALLBACK = 0x200               # OR-ed into the rule: RAW when the rule does not shrink the stream (FORMAT.md §8)
 
 
 class OracleError(RuntimeError):
@@ -77,6 +78,10 @@ def lib():
         L.bfsc_ref_compress_batch_mt.argtypes = [vp, vp, sz, i32, sz, vp, sz, vp, i32]
         L.bfsc_ref_decompress_batch_mt.restype = i32
         L.bfsc_ref_decompress_batch_mt.argtypes = [vp, vp, sz, i32, vp, sz, vp, i32]
+        L.bfsc_ref_compress_bitmap.restype = i32
+        L.bfsc_ref_compress_bitmap.argtypes = [i32, vp, sz, c.c_uint64, i32, sz, vp, sz, c.POINTER(sz)]
+        L.bfsc_ref_decompress_to_bitmap.restype = i32
+        L.bfsc_ref_decompress_to_bitmap.argtypes = [vp, sz, i32, c.c_uint64, vp, sz, c.POINTER(sz)]
         _lib = L
     return _lib
 
@@ -210,3 +215,30 @@ def decompress_batch(stream: np.ndarray, in_offsets: np.ndarray, W: int, capacit
     if rc:
         raise OracleError(rc)
     return ids[:int(id_off[-1])], id_off
+
+
+def compress_bitmap(bitmap: np.ndarray, n_bits: int, W: int, id_base: int = 0, raw_threshold_bytes: int = 0,
+                    codec: int = CODEC_PFOR) -> np.ndarray:
+    """bitmap: uint32 words (bit v = bit v % 32 of word v // 32) -> the stream of the IDs id_base + v of its set bits."""
+    bitmap = np.ascontiguousarray(bitmap, dtype=np.uint32)
+    assert len(bitmap) * 32 >= n_bits
+    cap = max(compress_bound(n_bits, W), 32 + (n_bits * W // 8 + 15) // 16 * 16)
+    out = np.empty(cap, dtype=np.uint8)
+    nbytes = ctypes.c_size_t(0)
+    rc = lib().bfsc_ref_compress_bitmap(codec, _p(bitmap), n_bits, ctypes.c_uint64(id_base), W, raw_threshold_bytes,
+                                        _p(out), cap, ctypes.byref(nbytes))
+    if rc:
+        raise OracleError(rc)
+    return out[:nbytes.value].copy()
+
+
+def decompress_to_bitmap(stream: np.ndarray, W: int, bitmap: np.ndarray, n_bits: int, id_base: int = 0) -> int:
+    """ORs the decoded IDs into `bitmap` (uint32 words, modified in place); returns the number of IDs decoded."""
+    stream = np.ascontiguousarray(stream, dtype=np.uint8)
+    assert bitmap.dtype == np.uint32 and bitmap.flags["C_CONTIGUOUS"] and len(bitmap) * 32 >= n_bits
+    n = ctypes.c_size_t(0)
+    rc = lib().bfsc_ref_decompress_to_bitmap(_p(stream), len(stream), W, ctypes.c_uint64(id_base), _p(bitmap), n_bits,
+                                             ctypes.byref(n))
+    if rc:
+        raise OracleError(rc)
+    return n.value

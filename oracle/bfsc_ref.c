@@ -137,8 +137,27 @@ int bfsc_ref_compress(const void *ids, size_t n, int W, size_t thr,
     return bfsc_ref_compress_codec(BFSC_REF_CODEC_PFOR, ids, n, W, thr, out, cap, out_bytes);
 }
 
+static int compress_rule(int codec, const void *ids, size_t n, int W, size_t thr,
+                         uint8_t *out, size_t cap, size_t *out_bytes);
+
+/* FORMAT.md §8: with BFSC_REF_FLAG_RAW_FALLBACK the stream is encoded under the rule, and sent RAW after all when that
+ * did not make it smaller than the RAW stream of the same IDs ("Compression -> Transmission -> Decompression slower
+ * than Transmission"; the thesis sets its threshold by hand, L2086, L2164). Written the plain way:
+ * encode, compare, encode again as RAW. */
 int bfsc_ref_compress_codec(int codec, const void *ids, size_t n, int W, size_t thr,
                             uint8_t *out, size_t cap, size_t *out_bytes) {
+    int fallback = codec & BFSC_REF_FLAG_RAW_FALLBACK;
+    codec &= ~BFSC_REF_FLAG_RAW_FALLBACK;
+    int rc = compress_rule(codec, ids, n, W, thr, out, cap, out_bytes);
+    if (rc || !fallback) return rc;
+    size_t raw_total = 32 + align_up(n * (size_t)(W / 8), 16);
+    if (*out_bytes >= raw_total)                               /* did not shrink: RAW (threshold above any size) */
+        return compress_rule(codec, ids, n, W, (size_t)-1, out, cap, out_bytes);
+    return BFSC_REF_OK;
+}
+
+static int compress_rule(int codec, const void *ids, size_t n, int W, size_t thr,
+                         uint8_t *out, size_t cap, size_t *out_bytes) {
     if ((W != 32 && W != 64) || !out || !out_bytes || (n && !ids)) return BFSC_REF_ERR_INVALID_ARG;
     if (codec != BFSC_REF_CODEC_PFOR && codec != BFSC_REF_CODEC_BP128) return BFSC_REF_ERR_INVALID_ARG;
     if (is_raw(n, W, thr)) {
@@ -289,6 +308,49 @@ int bfsc_ref_decompress_batch(const uint8_t *in, const uint64_t *in_off, size_t 
     }
     id_off[n_buf] = at;
     return BFSC_REF_OK;
+}
+
+/* ---- frontier bitmaps (FORMAT.md §9; "32-bit-word bitmap", Algorithm 4 line 11, L1381-1392, L2080) ----
+ * A frontier given as a bitmap: bit v of the bitmap (bit v % 32 of 32-bit little-endian word v / 32) set <=> vertex
+ * id_base + v is in the frontier. The stream of a bitmap is, by definition, the stream of its sorted ID list. */
+int bfsc_ref_compress_bitmap(int codec, const uint32_t *bitmap, size_t n_bits, uint64_t id_base, int W, size_t thr,
+                             uint8_t *out, size_t cap, size_t *out_bytes) {
+    if ((W != 32 && W != 64) || (n_bits && !bitmap)) return BFSC_REF_ERR_INVALID_ARG;
+    size_t n = 0;
+    for (size_t v = 0; v < n_bits; v++) n += (bitmap[v / 32] >> (v % 32)) & 1u;
+    void *ids = malloc((n ? n : 1) * (size_t)(W / 8));
+    if (!ids) return BFSC_REF_ERR_INVALID_ARG;
+    size_t k = 0;
+    for (size_t v = 0; v < n_bits; v++)                        /* ascending bit index = ascending ID */
+        if ((bitmap[v / 32] >> (v % 32)) & 1u) store_id(ids, k++, W, (id_base + v) & wmask(W));
+    int rc = bfsc_ref_compress_codec(codec, ids, n, W, thr, out, cap, out_bytes);
+    free(ids);
+    return rc;
+}
+
+/* Decode, then OR bit (x - id_base) into the bitmap for every decoded ID x (the "t ⊙ ¬Π" consumer of Algorithm 4
+ * works on bitmaps). An ID outside [id_base, id_base + n_bits) does not fit the bitmap: DST_TOO_SMALL. *n_ids = IDs decoded. */
+int bfsc_ref_decompress_to_bitmap(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,
+                                  uint32_t *bitmap, size_t n_bits, size_t *n_ids) {
+    if ((W != 32 && W != 64) || !in || !n_ids) return BFSC_REF_ERR_INVALID_ARG;
+    int mode; uint64_t n, total, nb;
+    int rc = parse_header(in, in_bytes, W, &mode, &n, &total, &nb);
+    if (rc) return rc;
+    void *ids = malloc((n ? n : 1) * (size_t)(W / 8));
+    if (!ids) return BFSC_REF_ERR_INVALID_ARG;
+    size_t got = 0;
+    rc = bfsc_ref_decompress(in, in_bytes, W, ids, n, &got);
+    for (size_t i = 0; !rc && i < got; i++) {
+        uint64_t v = (load_id(ids, i, W) - id_base) & wmask(W);
+        if (v >= n_bits) rc = BFSC_REF_ERR_DST_TOO_SMALL;
+    }
+    for (size_t i = 0; !rc && i < got; i++) {
+        uint64_t v = (load_id(ids, i, W) - id_base) & wmask(W);
+        bitmap[v / 32] |= 1u << (v % 32);
+    }
+    free(ids);
+    if (!rc) *n_ids = got;
+    return rc;
 }
 
 /* ------------------------------------------------------------------------------------

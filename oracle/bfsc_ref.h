@@ -46,8 +46,9 @@ enum {
     BFSC_REF_ERR_CORRUPT = 3
 };
 
-/* Encoder rule = mode byte of the stream it writes (FORMAT.md §1, §7). */
-enum { BFSC_REF_CODEC_PFOR = 1, BFSC_REF_CODEC_BP128 = 2 };
+/* Encoder rule = mode byte of the stream it writes (FORMAT.md §1, §7). BFSC_REF_FLAG_RAW_FALLBACK, OR-ed into
+ * the rule: a stream that the rule does not make smaller than its RAW form is sent RAW (FORMAT.md §8). */
+enum { BFSC_REF_CODEC_PFOR = 1, BFSC_REF_CODEC_BP128 = 2, BFSC_REF_FLAG_RAW_FALLBACK = 0x200 };
 
 /* bit length of v: 0 for 0, floor(log2 v)+1 otherwise. For a range [min,max] the FOR
  * width of eq. (6) is bfsc_ref_width(max - min). */
@@ -102,6 +103,14 @@ int bfsc_ref_compress_batch(const void *ids, const uint64_t *in_offsets, size_t 
 /* in_offsets: n_buf+1 byte offsets into `in`; id_offsets: n_buf+1 element offsets, written. */
 int bfsc_ref_decompress_batch(const uint8_t *in, const uint64_t *in_offsets, size_t n_buf, int W,
                               void *ids, size_t ids_capacity, uint64_t *id_offsets);
+
+/* Frontier bitmaps (FORMAT.md §9): bit v (bit v % 32 of word v / 32) <=> ID id_base + v. compress_bitmap = compress
+ * of the ascending ID list of the set bits; decompress_to_bitmap ORs the decoded IDs' bits into the bitmap
+ * (DST_TOO_SMALL if an ID lies outside [id_base, id_base + n_bits)). */
+int bfsc_ref_compress_bitmap(int codec, const uint32_t *bitmap, size_t n_bits, uint64_t id_base, int W,
+                             size_t raw_threshold_bytes, uint8_t *out, size_t out_capacity, size_t *out_bytes);
+int bfsc_ref_decompress_to_bitmap(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,
+                                  uint32_t *bitmap, size_t n_bits, size_t *n_ids);
 
 /* Multi-threaded drivers used only by bench.py's cpu_baseline leg: independent buffers
  * are spread over `threads` pthreads; each buffer goes through the same scalar routines

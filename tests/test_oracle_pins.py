@@ -275,3 +275,88 @@ def test_compress_bound_closed_form(oracle_mod):
         s = oracle_mod.compress(x)
         # the first delta of each block is 0, the other 127 have W bits: b = W, no exceptions
         assert len(s) == oracle_mod.compress_bound(n, W)
+
+
+# ---------------------------------------------------------------- FORMAT.md §8: RAW fallback
+def test_raw_fallback_rule(oracle_mod):
+    """FORMAT.md §8: with the fallback flag a stream is never larger than its RAW form; it is
+    the rule's stream, byte for byte, when that is smaller, and the RAW stream otherwise (ties: RAW). Sizes typed out."""
+    F = oracle_mod.FLAG_RAW_FALLBACK
+    for W in (32, 64):
+        E = W // 8
+        dt = _dt(W)
+        assert len(oracle_mod.compress(np.zeros(0, dtype=dt), 0, codec=oracle_mod.CODEC_PFOR | F)) == 32          # 48 without
+        assert len(oracle_mod.compress(np.array([7], dtype=dt), 0, codec=oracle_mod.CODEC_PFOR | F)) == 32 + 16   # 64 without
+        x = (2000 + np.arange(128)).astype(dt)                      # the paper's eq. (7) range: 80 bytes either way
+        a, b = oracle_mod.compress(x, 0), oracle_mod.compress(x, 0, codec=oracle_mod.CODEC_PFOR | F)
+        assert len(a) == 80 and np.array_equal(a, b)
+        inc = np.array([(j * ((1 << (W - 1)) + 1)) % (1 << W) for j in range(640)], dtype=dt)   # every delta W bits wide
+        s = oracle_mod.compress(inc, 0, codec=oracle_mod.CODEC_PFOR | F)
+        assert len(s) == 32 + 640 * E and s[6] == 0 and s[24:28].view(np.uint32)[0] == 0
+        assert np.array_equal(s[32:].view(dt), inc)
+        assert len(oracle_mod.compress(inc, 0)) == oracle_mod.compress_bound(640, W) > len(s)
+        assert np.array_equal(oracle_mod.decompress(s, W), inc)
+        assert witness.decode_stream(s.tobytes(), W) == [int(v) for v in inc]
+    # a tie: 128 u32 IDs with a constant gap of 2^29 (30 bits): 32 + 16 + (16 + 16 * 30) = 544 = 32 + 512 -> RAW
+    tie = ((np.arange(128, dtype=np.uint64) << np.uint64(29)) & np.uint64(0xFFFFFFFF)).astype(np.uint32)
+    assert len(oracle_mod.compress(tie, 0)) == 544
+    s = oracle_mod.compress(tie, 0, codec=oracle_mod.CODEC_PFOR | F)
+    assert len(s) == 544 and s[6] == 0
+    rng = np.random.default_rng(99)
+    for _ in range(40):
+        W = int(rng.choice([32, 64]))
+        n = int(rng.integers(0, 700))
+        bits = int(rng.integers(1, W + 1))
+        g = rng.integers(0, 1 << min(bits, 63), size=n, dtype=np.uint64)
+        x = (np.cumsum(g) & np.uint64((1 << W) - 1)).astype(_dt(W))
+        for rule in (oracle_mod.CODEC_PFOR, oracle_mod.CODEC_BP128):
+            plain, fb = oracle_mod.compress(x, 0, codec=rule), oracle_mod.compress(x, 0, codec=rule | F)
+            raw_total = 32 + -(-n * (W // 8) // 16) * 16
+            assert len(fb) == min(len(plain), raw_total) and len(fb) <= raw_total
+            assert (fb[6] == 0) == (len(plain) >= raw_total)
+            if len(plain) < raw_total:
+                assert np.array_equal(fb, plain)
+            assert np.array_equal(oracle_mod.decompress(fb, W), x)
+
+
+# ---------------------------------------------------------------- FORMAT.md §9: frontier bitmaps
+def test_bitmap_hand_vector(oracle_mod):
+    """The paper's eq. (7) range 2000..2127 as a bitmap, words typed by hand (bit v = bit v % 32 of word v / 32):
+    its stream is the hand-typed 80-byte vector of tests/golden/hand_vector_2000_2127.hex; the same bits at
+    0..127 with id_base = 2000 give the same bytes."""
+    gold = bytes.fromhex("".join(ln.split("#")[0] for ln in open(os.path.join(GOLD, "hand_vector_2000_2127.hex"))).replace(" ", "").replace("\n", ""))
+    words = np.zeros(67, dtype=np.uint32)
+    words[62] = 0xFFFF0000                                          # bits 2000..2015
+    words[63] = words[64] = words[65] = 0xFFFFFFFF                  # bits 2016..2111
+    words[66] = 0x0000FFFF                                          # bits 2112..2127
+    s = oracle_mod.compress_bitmap(words, 67 * 32, 32)
+    assert s.tobytes() == gold
+    assert oracle_mod.compress_bitmap(np.full(4, 0xFFFFFFFF, dtype=np.uint32), 128, 32, id_base=2000).tobytes() == gold
+    back = np.zeros(67, dtype=np.uint32)
+    assert oracle_mod.decompress_to_bitmap(s, 32, back, 67 * 32) == 128 and np.array_equal(back, words)
+
+
+def test_bitmap_matches_id_list_and_round_trips(oracle_mod):
+    """compress_bitmap(bits) == compress(IDs of the set bits), the IDs derived here by numpy (unpackbits, nonzero),
+    not by the oracle; n in the header = popcount; decompress_to_bitmap ORs (old bits stay); an ID outside the
+    bitmap is DST_TOO_SMALL and leaves the bitmap alone."""
+    rng = np.random.default_rng(7)
+    for W in (32, 64):
+        for n_bits, density in ((1, 1.0), (31, 0.5), (32, 0.5), (1000, 0.5), (4096, 0.02), (70000, 0.3), (5000, 0.0)):
+            for id_base in (0, 12345):
+                bits = rng.random(n_bits) < density
+                words = np.packbits(np.concatenate([bits, np.zeros(-n_bits % 32, dtype=bool)]), bitorder="little").view(np.uint32).copy()
+                ids = (np.nonzero(bits)[0].astype(np.uint64) + np.uint64(id_base)).astype(_dt(W))
+                s = oracle_mod.compress_bitmap(words, n_bits, W, id_base=id_base)
+                assert np.array_equal(s, oracle_mod.compress(ids, 0))
+                assert int(s[8:16].view(np.uint64)[0]) == int(bits.sum())
+                old = rng.integers(0, 1 << 32, size=len(words), dtype=np.uint64).astype(np.uint32)
+                old[-1] &= np.uint32((1 << ((n_bits - 1) % 32 + 1)) - 1)
+                back = old.copy()
+                assert oracle_mod.decompress_to_bitmap(s, W, back, n_bits, id_base=id_base) == len(ids)
+                assert np.array_equal(back, old | words)
+                if len(ids) and n_bits > 1:
+                    small = old.copy()
+                    with pytest.raises(oracle_mod.OracleError) as ei:
+                        oracle_mod.decompress_to_bitmap(s, W, small, int(ids[-1]) - id_base, id_base=id_base)   # last ID does not fit
+                    assert ei.value.code == oracle_mod.ERR_DST_TOO_SMALL and np.array_equal(small, old)
