@@ -90,8 +90,15 @@ typedef enum { BFSC_U32 = 32, BFSC_U64 = 64 } bfsc_dtype;
  *                        whole compress grid becomes resident at once. The first two tiles of every CTA are
  *                        then assigned statically and start before the call's plan kernel has finished
  *                        (about 2 us less per call). If the promise is broken the call can deadlock.
- *                        Output bytes are the same with or without the flag. */
-typedef enum { BFSC_CODEC_PFOR = 1, BFSC_CODEC_BP128 = 2, BFSC_CODEC_FLAG_EXCLUSIVE = 0x100 } bfsc_codec;
+ *                        Output bytes are the same with or without the flag.
+ *   BFSC_CODEC_FLAG_RAW_FALLBACK  FORMAT.md §8: a stream that the rule does not make smaller than
+ *                        its RAW form is sent RAW (mode 0) after all: total_bytes <= 32 + align16(n W / 8) always.
+ *                        Single-buffer calls (bfsc_compress_codec, bfsc_compress_bitmap); the batch calls return
+ *                        BFSC_ERR_UNSUPPORTED (streams of a batch lie back to back: a stream that shrinks after the
+ *                        fact would move every stream behind it). The input is read a second time only for the
+ *                        streams that fall back. */
+typedef enum { BFSC_CODEC_PFOR = 1, BFSC_CODEC_BP128 = 2, BFSC_CODEC_FLAG_EXCLUSIVE = 0x100,
+               BFSC_CODEC_FLAG_RAW_FALLBACK = 0x200 } bfsc_codec;
 
 /* library / format version: (format_version << 16) | abi_revision */
 uint32_t bfsc_version(void);
@@ -155,6 +162,23 @@ bfsc_status bfsc_decompress_batch(const void* d_in, const uint64_t* d_in_offsets
                                   void* d_ids, size_t ids_capacity, uint64_t* d_id_offsets,
                                   void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                                   void* cuda_stream);
+
+/* Frontier bitmaps (FORMAT.md §9; Algorithm 4 line 11, Algorithm 5): the codec fused
+ * with the conversion on either side of it. d_bitmap: 32-bit words, bit v = bit v % 32 of word v / 32 <=> ID id_base + v;
+ * 16-byte aligned, readable / writable up to a whole number of words.
+ * bfsc_compress_bitmap: the stream of the ascending IDs of the set bits of d_bitmap[0 .. n_bits) — byte-identical to
+ *   bfsc_compress_codec on that ID list, which is never materialised (the input read is n_bits / 8 bytes).
+ *   out_capacity >= bfsc_compress_bound(number of set bits) (n_bits is always enough); workspace:
+ *   bfsc_bitmap_workspace_bytes(n_bits, t).
+ * bfsc_decompress_to_bitmap: ORs the bits of the stream's IDs into d_bitmap (old bits stay); *d_n_ids = IDs decoded.
+ *   An ID outside [id_base, id_base + n_bits): BFSC_ERR_DST_TOO_SMALL in *d_status (bits of other IDs may have been set). */
+size_t bfsc_bitmap_workspace_bytes(size_t n_bits, bfsc_dtype t);
+bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_bitmap, size_t n_bits, uint64_t id_base, bfsc_dtype t,
+                                 size_t raw_threshold_bytes, void* d_out, size_t out_capacity, uint64_t* d_out_bytes,
+                                 void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream);
+bfsc_status bfsc_decompress_to_bitmap(const void* d_in, size_t in_bytes, bfsc_dtype t, uint64_t id_base,
+                                      uint32_t* d_bitmap, size_t n_bits, uint64_t* d_n_ids,
+                                      void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream);
 
 /* End-to-end convenience calls with HOST buffers (pinned memory recommended): copy in,
  * run the device call above, copy the result out, synchronise the stream. d_scratch is a

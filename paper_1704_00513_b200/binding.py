@@ -19,11 +19,13 @@ OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED =
 U32, U64 = 32, 64
 CODEC_PFOR, CODEC_BP128 = 1, 2          # bfsc_codec (include/bfsc.h)
 CODEC_FLAG_EXCLUSIVE = 0x100            # launch flag, OR-ed into the codec (include/bfsc.h)
+CODEC_FLAG_RAW_FALLBACK = 0x200         # FORMAT.md §8, OR-ed into the codec of a single-buffer call
 
 EXPORTS = [
     "bfsc_version", "bfsc_compress_bound", "bfsc_batch_compress_bound", "bfsc_workspace_bytes",
     "bfsc_compress", "bfsc_decompress", "bfsc_compress_batch", "bfsc_decompress_batch",
     "bfsc_compress_codec", "bfsc_compress_batch_codec",
+    "bfsc_bitmap_workspace_bytes", "bfsc_compress_bitmap", "bfsc_decompress_to_bitmap",
     "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
 ]
 
@@ -52,6 +54,12 @@ def lib():
         L.bfsc_batch_compress_bound.argtypes = [vp, sz, i32]
         L.bfsc_workspace_bytes.restype = sz
         L.bfsc_workspace_bytes.argtypes = [sz, sz, i32]
+        L.bfsc_bitmap_workspace_bytes.restype = sz
+        L.bfsc_bitmap_workspace_bytes.argtypes = [sz, i32]
+        L.bfsc_compress_bitmap.restype = i32
+        L.bfsc_compress_bitmap.argtypes = [i32, vp, sz, c.c_uint64, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_decompress_to_bitmap.restype = i32
+        L.bfsc_decompress_to_bitmap.argtypes = [vp, sz, i32, c.c_uint64, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_host_scratch_bytes.restype = sz
         L.bfsc_host_scratch_bytes.argtypes = [sz, i32]
         L.bfsc_compress.restype = i32
@@ -103,6 +111,10 @@ def workspace_bytes(n_ids_total: int, n_buf: int, W: int) -> int:
     return lib().bfsc_workspace_bytes(n_ids_total, n_buf, W)
 
 
+def bitmap_workspace_bytes(n_bits: int, W: int) -> int:
+    return lib().bfsc_bitmap_workspace_bytes(n_bits, W)
+
+
 def host_scratch_bytes(n_ids: int, W: int) -> int:
     return lib().bfsc_host_scratch_bytes(n_ids, W)
 
@@ -129,6 +141,20 @@ def compress_codec(codec, d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_byt
     _check(lib().bfsc_compress_codec(codec, _ptr(d_ids), n_ids, W, raw_threshold_bytes, _ptr(d_out), d_out.numel(),
                                      _ptr(d_out_bytes), _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
                                      ctypes.c_void_p(_stream())), "bfsc_compress_codec")
+
+
+def compress_bitmap(codec, d_bitmap, n_bits, id_base, W, raw_threshold_bytes, d_out, d_out_bytes, d_workspace, d_status):
+    """bfsc_compress_bitmap (FORMAT.md §9): d_bitmap int32/uint32 words, bit v = ID id_base + v."""
+    _check(lib().bfsc_compress_bitmap(codec, _ptr(d_bitmap), n_bits, id_base, W, raw_threshold_bytes, _ptr(d_out),
+                                      d_out.numel(), _ptr(d_out_bytes), _ptr(d_workspace), d_workspace.numel(),
+                                      _ptr(d_status), ctypes.c_void_p(_stream())), "bfsc_compress_bitmap")
+
+
+def decompress_to_bitmap(d_in, in_bytes, W, id_base, d_bitmap, n_bits, d_n_ids, d_workspace, d_status):
+    """bfsc_decompress_to_bitmap (FORMAT.md §9): ORs the bits of the stream's IDs into d_bitmap."""
+    _check(lib().bfsc_decompress_to_bitmap(_ptr(d_in), in_bytes, W, id_base, _ptr(d_bitmap), n_bits, _ptr(d_n_ids),
+                                           _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
+                                           ctypes.c_void_p(_stream())), "bfsc_decompress_to_bitmap")
 
 
 def decompress(d_in, in_bytes, W, d_ids, d_n_ids, d_workspace, d_status):

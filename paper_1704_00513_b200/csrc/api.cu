@@ -30,7 +30,7 @@ static size_t bound_one(size_t n, int W) {
 }
 }  // namespace bfsc
 
-extern "C" uint32_t bfsc_version(void) { return (1u << 16) | 2u; }   // abi revision 2: bfsc_compress[_batch]_codec, mode 2
+extern "C" uint32_t bfsc_version(void) { return (1u << 16) | 3u; }   // abi revision 2: bfsc_compress[_batch]_codec, mode 2; 3: codec flags, bitmap calls
 
 extern "C" uint64_t bfsc_kernel_launches(void) { return bfsc::g_launches; }
 
@@ -49,6 +49,12 @@ extern "C" size_t bfsc_batch_compress_bound(const uint64_t* h_counts, size_t n_b
 extern "C" size_t bfsc_workspace_bytes(size_t n_ids_total, size_t n_buf, bfsc_dtype t) {
     (void)t;
     return bfsc::align_up(bfsc::ws_bytes_for(n_ids_total, n_buf), 256);
+}
+
+// standard workspace of one stream of at most n_bits IDs | set bits before every 1024-bit chunk (u64, + the total)
+extern "C" size_t bfsc_bitmap_workspace_bytes(size_t n_bits, bfsc_dtype t) {
+    (void)t;
+    return bfsc::align_up(bfsc::align_up(bfsc::ws_bytes_for(n_bits, 1), 16) + 8 * ((n_bits + 1023) / 1024 + 1), 256);
 }
 
 // ---- host-buffer convenience calls ------------------------------------------------------

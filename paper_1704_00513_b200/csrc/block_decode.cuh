@@ -74,9 +74,10 @@ __device__ __forceinline__ bool patch_rows(const unsigned char* __restrict__ e, 
 
 // D4: inclusive scan of the 128 deltas (4 local adds + warp scan of row totals) + base, then store
 // the first m IDs. x: block's first output ID.
-template <int W>
+template <int W, bool kBits = false>
 __device__ __forceinline__ void scan_store(typename IdT<W>::T d[4], typename IdT<W>::T base,
-                                           typename IdT<W>::T* __restrict__ x, int m) {
+                                           typename IdT<W>::T* __restrict__ x, int m,
+                                           const BitSink& sink = BitSink{nullptr, 0, 0, nullptr}) {
     using T = typename IdT<W>::T;
     const int lane = lane_id();
     d[1] += d[0]; d[2] += d[1]; d[3] += d[2];
@@ -88,6 +89,10 @@ __device__ __forceinline__ void scan_store(typename IdT<W>::T d[4], typename IdT
     }
     const T off = base + (inc - d[3]);
     d[0] += off; d[1] += off; d[2] += off; d[3] += off;
+    if constexpr (kBits) {
+        set_bits4<T>(sink, d[0], d[1], d[2], d[3], m - 4 * lane);
+        return;
+    }
     const bool vec_ok = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
     if (vec_ok) {
         if constexpr (W == 32) {

@@ -30,7 +30,8 @@ struct WsHeader {
     unsigned int ok;                    // 1 = plan valid and capacity sufficient
     unsigned int ticket;                // tile ticket counter (fused encode)
     unsigned long long grand16;         // encode: sum of all block sizes in 16-B units (written by the last tile)
-    unsigned long long pad[27];
+    unsigned long long n_ids;           // bfsc_compress_bitmap: set bits of the bitmap = IDs of the stream (k_bm_plan)
+    unsigned long long pad[26];
 };
 static_assert(sizeof(WsHeader) == 256, "WsHeader");
 
@@ -109,6 +110,31 @@ __device__ __forceinline__ uint32_t exc_bytes(uint32_t n) {
     constexpr uint32_t E = W / 8;
     uint32_t a = ((n + E - 1) & ~(E - 1)) + n * E;
     return n ? ((a + 15u) & ~15u) : 0u;
+}
+
+// Decoding into a frontier bitmap (FORMAT.md §9): bit (x - id_base) of bm for every decoded ID x. bm == nullptr: IDs go to
+// the ID array as usual.
+struct BitSink { uint32_t* bm; unsigned long long id_base, n_bits; uint32_t* status; };
+// Four consecutive decoded IDs (the first nvalid of them count). Neighbours that fall into the same 32-bit word go
+// out as ONE atomic OR (sorted dense frontiers: usually all four). An ID outside the bitmap: DST_TOO_SMALL, not set.
+template <typename T>
+__device__ __forceinline__ void set_bits4(const BitSink& s, T v0, T v1, T v2, T v3, int nvalid) {
+    const T v[4] = {v0, v1, v2, v3};
+    uint32_t w[4], mk[4];
+#pragma unroll
+    for (int c = 0; c < 4; c++) {
+        const unsigned long long rel = (unsigned long long)(T)(v[c] - (T)s.id_base);
+        bool ok = c < nvalid;
+        if (ok && rel >= s.n_bits) { set_status(s.status, BFSC_ERR_DST_TOO_SMALL); ok = false; }
+        w[c] = ok ? (uint32_t)(rel >> 5) : 0xffffffffu;
+        mk[c] = ok ? 1u << ((uint32_t)rel & 31u) : 0u;
+    }
+#pragma unroll
+    for (int c = 1; c < 4; c++)
+        if (w[c] == w[c - 1]) { mk[c] |= mk[c - 1]; mk[c - 1] = 0u; }
+#pragma unroll
+    for (int c = 0; c < 4; c++)
+        if (mk[c]) atomicOr(s.bm + w[c], mk[c]);
 }
 
 // Buffer of global block g: the last i with a[i] <= g (buffers without blocks are skipped), searched from a

@@ -2,6 +2,7 @@
 //
 // Launches per call: single stream: k_dec_tiles alone (it parses the stream header itself);
 // batch: [k_dec_headers ->] k_dec_plan -> k_dec_blocks -> k_dec_tiles, chained with programmatic dependent launch.
+#include <cstdlib>
 #include <mutex>
 
 #include "block_decode.cuh"
@@ -19,6 +20,7 @@ struct DecArgs {
     unsigned long long* id_off;         // n_buf+1 (batch, written) or nullptr
     unsigned long long* n_ids_out;      // single: *d_n_ids, or nullptr
     uint32_t* status;
+    BitSink sink;                       // bfsc_decompress_to_bitmap: where the IDs' bits go (ids == nullptr then)
     WsView ws;                          // blk_first, fixed_prefix (= id offsets)
 };
 
@@ -197,18 +199,20 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
 // Blocks over 336 B (b > 20: nearly incompressible data) take the warp-per-block path of
 // block_decode.cuh, straight from global memory. Single-stream calls parse the stream header here
 // (no plan kernel); RAW streams are copied at the end (D5).
-// CTA shape: u32 2 CTAs of 16 warps per SM (6.9 KB of shared memory per warp), u64 2 CTAs of 8 warps (11 KB per warp)
-template <int W> struct DecCfg {
-    static constexpr int kWarps = (W == 32) ? 16 : 8;
+// CTA shape: u32 2 CTAs of 16 warps per SM (6.9 KB of shared memory per warp), u64 2 CTAs of 8 warps (11 KB per warp);
+// the TMA variant (two staging buffers per warp: 9.7 KB) fits 2 CTAs of 11 warps
+template <int W, bool kTma = false> struct DecCfg {
+    static constexpr int kStages = kTma ? 2 : 1;                                      // staging buffers per warp
+    static constexpr int kWarps = (W == 32) ? (kTma ? 11 : 16) : 8;
     static constexpr int kThreads = kWarps * 32;
-    static constexpr int kCtasPerSm = (W == 32) ? 2 : 2;
+    static constexpr int kCtasPerSm = 2;
 };
 
-template <int W> struct DecSmem {
+template <int W, bool kTma = false> struct DecSmem {
     using T = typename IdT<W>::T;
-    static constexpr size_t kStageBytes = (size_t)kDecStageChunks * 16;               // per warp
+    static constexpr size_t kStageBytes = (size_t)DecCfg<W, kTma>::kStages * kDecStageChunks * 16;   // per warp
     static constexpr size_t kTabBytes = (size_t)kDecBlocks * kBlk * sizeof(T);         // per warp
-    static constexpr size_t kBytes = DecCfg<W>::kWarps * (kStageBytes + kTabBytes);
+    static constexpr size_t kBytes = DecCfg<W, kTma>::kWarps * (kStageBytes + kTabBytes);
 };
 
 template <int W>
@@ -219,19 +223,28 @@ struct BlockAt {                       // where the quad's block is
     int m;                             // valid IDs
 };
 
-template <int W, bool kBatch>          // kBatch: a.in_off != nullptr
-__global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_dec_tiles(DecArgs a) {
-    constexpr int kDecWarps = DecCfg<W>::kWarps;
+// kTma (single-stream calls): D1 as ONE bulk copy (TMA, cp.async.bulk + mbarrier) of the warp batch's contiguous span
+// [dir[8k], dir[8k+8)) * 16 issued by lane 0, the blocks unpacked where they land; else every lane copies 16-byte
+// chunks of its quad's block into the quad's slot (cp.async). The measured A/B is in DESIGN.md §5.2.
+template <int W, bool kBatch, bool kTma, bool kBits = false>   // kBatch: a.in_off != nullptr; kBits: bits into a.sink instead of IDs into a.ids
+__global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kCtasPerSm) k_dec_tiles(DecArgs a) {
+    constexpr int kDecWarps = DecCfg<W, kTma>::kWarps;
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
     extern __shared__ __align__(16) unsigned char dec_smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, q = lane >> 2, l = lane & 3;
-    uint4* stage = reinterpret_cast<uint4*>(dec_smem + warp * DecSmem<W>::kStageBytes);
-    T* tab_w = reinterpret_cast<T*>(dec_smem + kDecWarps * DecSmem<W>::kStageBytes + warp * DecSmem<W>::kTabBytes);
+    uint4* stage = reinterpret_cast<uint4*>(dec_smem + warp * DecSmem<W, kTma>::kStageBytes);
+    T* tab_w = reinterpret_cast<T*>(dec_smem + kDecWarps * DecSmem<W, kTma>::kStageBytes + warp * DecSmem<W, kTma>::kTabBytes);
     for (int x = lane; x < kDecBlocks * kBlk; x += 32) tab_w[x] = 0;       // patch table: all zero between uses
     __syncwarp();
     uint4* slot = stage + kDecSlotChunks * q;
     T* tab = tab_w + kBlk * q;
+    __shared__ unsigned long long s_mbar[kTma ? 2 * kDecWarps : 1];       // kTma: "the span in stage s of warp w has landed"
+    if constexpr (kTma) {
+        if (lane < 2) dec_mbar_init(&s_mbar[2 * warp + lane], 1);
+        dec_fence_mbar_init();
+        __syncwarp();
+    }
 
     constexpr bool batch = kBatch;
     unsigned long long total_blocks, n1 = 0, total16_1 = 0, lo16_1 = 0;   // single stream: n, total/16, first block/16
@@ -273,7 +286,8 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
             T* y = reinterpret_cast<T*>(a.ids);
             for (unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; t < n1;
                  t += (unsigned long long)gridDim.x * blockDim.x)
-                y[t] = xs[t];
+                if constexpr (kBits) set_bits4<T>(a.sink, xs[t], (T)0, (T)0, (T)0, 1);
+                else y[t] = xs[t];
             return;
         }
         total_blocks = nb;
@@ -323,64 +337,121 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
         bi = blockIdx.x * base_w + min(blockIdx.x, rem_w) + warp;
         if ((uint32_t)warp >= base_w + (blockIdx.x < rem_w ? 1u : 0u)) bi = n_batches;   // this warp sits the call out
     }
-    BlockAt<W> cur = locate(bi * kDecBlocks + q);
-    for (; bi < n_batches; bi += n_warps) {
-        const bool big = cur.blk != nullptr && cur.span16 > (uint32_t)kDecSpanMax;
-        const bool any_big = __any_sync(kFull, big);
-        if (!any_big && cur.blk != nullptr) quad_stage_block(slot, cur.blk, cur.span16, l);
-        const BlockAt<W> nxt = locate((bi + n_warps) * kDecBlocks + q);   // the next batch's directory reads overlap the copy
-        if (!any_big) {
-            dec_cp_async_wait_all();
+    // D2-D4 of the quad's block, staged at `slot` (header chunk first)
+    auto decode_staged = [&](const BlockAt<W>& cur, uint4* slot) {
+        bool live = cur.blk != nullptr;
+        const uint4 h = slot[0];
+        const uint32_t b = h.z & 0xffu, n_exc = (h.z >> 8) & 0xffu;
+        if (live && (b > (uint32_t)W || n_exc > 127u || 1u + b + exc_bytes<W>(n_exc) / 16u > cur.span16)) {
+            set_status(a.status, BFSC_ERR_CORRUPT);
+            live = false;
+        }
+        const unsigned char* e = reinterpret_cast<const unsigned char*>(slot + 1 + b);
+        const bool patch = __any_sync(kFull, live && n_exc > 0);         // D3: scatter into the patch table
+        if (patch) {
+            if (!quad_patch_scatter<W>(tab, e, b, live ? n_exc : 0u, l)) { set_status(a.status, BFSC_ERR_CORRUPT); live = false; }
             __syncwarp();
-            bool live = cur.blk != nullptr;
-            const uint4 h = slot[0];
+            const int lv = live;                                     // all four shuffles by every lane: no short-circuit
+            live = (__shfl_sync(kFull, lv, 4 * q + 0) & __shfl_sync(kFull, lv, 4 * q + 1) &
+                    __shfl_sync(kFull, lv, 4 * q + 2) & __shfl_sync(kFull, lv, 4 * q + 3)) != 0;
+        }
+        const T base = (T)((unsigned long long)h.y << 32 | h.x);
+        quad_decode_rows<W, kBatch, kBits>(slot + 1, live ? b : 0u, tab, patch, base, cur.x, live ? cur.m : 0, l, a.sink);   // D2-D4
+        if (patch) {
+            __syncwarp();
+            quad_patch_clear<W>(tab, e, (cur.blk != nullptr && b <= (uint32_t)W && n_exc <= 127u && 1u + b + exc_bytes<W>(n_exc) / 16u <= cur.span16) ? n_exc : 0u, l);
+        }
+    };
+    // slow path: the batch's blocks one at a time, the whole warp on each, straight from global memory
+    auto decode_direct = [&](const BlockAt<W>& cur) {
+        // slow path: one block at a time, the whole warp on it, straight from global memory
+        for (int qq = 0; qq < kDecBlocks; qq++) {
+            const unsigned char* blk = reinterpret_cast<const unsigned char*>(
+                __shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(cur.blk), 4 * qq));
+            T* x = reinterpret_cast<T*>(__shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(cur.x), 4 * qq));
+            const uint32_t span16 = __shfl_sync(kFull, cur.span16, 4 * qq);
+            const int m = __shfl_sync(kFull, cur.m, 4 * qq);
+            if (blk == nullptr) continue;
+            const uint4 h = *reinterpret_cast<const uint4*>(blk);
             const uint32_t b = h.z & 0xffu, n_exc = (h.z >> 8) & 0xffu;
-            if (live && (b > (uint32_t)W || n_exc > 127u || 1u + b + exc_bytes<W>(n_exc) / 16u > cur.span16)) {
+            if (b > (uint32_t)W || n_exc > 127u || 16ull + 16ull * b + exc_bytes<W>(n_exc) > 16ull * span16) {
                 set_status(a.status, BFSC_ERR_CORRUPT);
-                live = false;
-            }
-            const unsigned char* e = reinterpret_cast<const unsigned char*>(slot + 1 + b);
-            const bool patch = __any_sync(kFull, live && n_exc > 0);         // D3: scatter into the patch table
-            if (patch) {
-                if (!quad_patch_scatter<W>(tab, e, b, live ? n_exc : 0u, l)) { set_status(a.status, BFSC_ERR_CORRUPT); live = false; }
-                __syncwarp();
-                const int lv = live;                                     // all four shuffles by every lane: no short-circuit
-                live = (__shfl_sync(kFull, lv, 4 * q + 0) & __shfl_sync(kFull, lv, 4 * q + 1) &
-                        __shfl_sync(kFull, lv, 4 * q + 2) & __shfl_sync(kFull, lv, 4 * q + 3)) != 0;
+                continue;
             }
             const T base = (T)((unsigned long long)h.y << 32 | h.x);
-            quad_decode_rows<W, kBatch>(slot + 1, live ? b : 0u, tab, patch, base, cur.x, live ? cur.m : 0, l);   // D2-D4
-            if (patch) {
-                __syncwarp();
-                quad_patch_clear<W>(tab, e, (cur.blk != nullptr && b <= (uint32_t)W && n_exc <= 127u && 1u + b + exc_bytes<W>(n_exc) / 16u <= cur.span16) ? n_exc : 0u, l);
+            T dd[4];
+            unpack_rows<W>(reinterpret_cast<const uint4*>(blk + 16), b, dd);
+            if (n_exc > 0 && !patch_rows<W>(blk + 16 + 16 * b, b, n_exc, dd)) {
+                set_status(a.status, BFSC_ERR_CORRUPT);
+                continue;
             }
-            __syncwarp();                                                    // slots and table free again
-        } else {
-            // slow path: one block at a time, the whole warp on it, straight from global memory
-            for (int qq = 0; qq < kDecBlocks; qq++) {
-                const unsigned char* blk = reinterpret_cast<const unsigned char*>(
-                    __shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(cur.blk), 4 * qq));
-                T* x = reinterpret_cast<T*>(__shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(cur.x), 4 * qq));
-                const uint32_t span16 = __shfl_sync(kFull, cur.span16, 4 * qq);
-                const int m = __shfl_sync(kFull, cur.m, 4 * qq);
-                if (blk == nullptr) continue;
-                const uint4 h = *reinterpret_cast<const uint4*>(blk);
-                const uint32_t b = h.z & 0xffu, n_exc = (h.z >> 8) & 0xffu;
-                if (b > (uint32_t)W || n_exc > 127u || 16ull + 16ull * b + exc_bytes<W>(n_exc) > 16ull * span16) {
-                    set_status(a.status, BFSC_ERR_CORRUPT);
-                    continue;
-                }
-                const T base = (T)((unsigned long long)h.y << 32 | h.x);
-                T dd[4];
-                unpack_rows<W>(reinterpret_cast<const uint4*>(blk + 16), b, dd);
-                if (n_exc > 0 && !patch_rows<W>(blk + 16 + 16 * b, b, n_exc, dd)) {
-                    set_status(a.status, BFSC_ERR_CORRUPT);
-                    continue;
-                }
-                scan_store<W>(dd, base, x, m);
-            }
+            scan_store<W, kBits>(dd, base, x, m, a.sink);
         }
-        cur = nxt;
+    };
+
+    if constexpr (!kTma) {
+        BlockAt<W> cur = locate(bi * kDecBlocks + q);
+        for (; bi < n_batches; bi += n_warps) {
+            const bool big = cur.blk != nullptr && cur.span16 > (uint32_t)kDecSpanMax;
+            const bool any_big = __any_sync(kFull, big);
+            if (!any_big && cur.blk != nullptr) quad_stage_block(slot, cur.blk, cur.span16, l);
+            const BlockAt<W> nxt = locate((bi + n_warps) * kDecBlocks + q);   // the next batch's directory reads overlap the copy
+            if (!any_big) {
+                dec_cp_async_wait_all();
+                __syncwarp();
+                decode_staged(cur, slot);
+                __syncwarp();                                                // slots and table free again
+            } else {
+                decode_direct(cur);
+            }
+            cur = nxt;
+        }
+    } else {
+        // Two stages per warp: while batch i is unpacked from one, the span of batch i + 1 lands in the other — ONE bulk
+        // copy (TMA) per batch, issued by lane 0: the batch's blocks are one contiguous piece of the stream (entry k + 1
+        // of the directory ends block k and starts block k + 1). A quad whose directory entries were rejected breaks
+        // the span: nothing of that batch is decoded (the status word says CORRUPT already).
+        struct Staged { uint32_t rel; bool direct; bool skip; };
+        auto issue = [&](BlockAt<W>& c, unsigned long long batch_i, int st) -> Staged {
+            Staged r{0u, false, true};
+            if (batch_i >= n_batches) return r;
+            const bool expect = batch_i * kDecBlocks + q < total_blocks;
+            const bool whole = __all_sync(kFull, !expect || c.blk != nullptr);
+            const bool any_big = __any_sync(kFull, c.blk != nullptr && c.span16 > (uint32_t)kDecSpanMax);
+            const unsigned long long base_p = __shfl_sync(kFull, (unsigned long long)reinterpret_cast<uintptr_t>(c.blk), 0);
+            const int n_live = __popc(__ballot_sync(kFull, expect)) >> 2;
+            r.rel = c.blk != nullptr ? (uint32_t)((reinterpret_cast<uintptr_t>(c.blk) - base_p) >> 4) : 0u;
+            const uint32_t span_all = __shfl_sync(kFull, r.rel + c.span16, 4 * (n_live > 0 ? n_live - 1 : 0));
+            if (!whole) { c.blk = nullptr; return r; }
+            r.skip = false;
+            r.direct = any_big;
+            if (!any_big && lane == 0) {
+                dec_mbar_expect_tx(&s_mbar[2 * warp + st], 16u * span_all);
+                dec_bulk_load(stage + st * kDecStageChunks, reinterpret_cast<const void*>(static_cast<uintptr_t>(base_p)), 16u * span_all,
+                              &s_mbar[2 * warp + st]);
+            }
+            return r;
+        };
+        BlockAt<W> cur = locate(bi * kDecBlocks + q);
+        Staged sc = issue(cur, bi, 0);
+        BlockAt<W> nxt = locate((bi + n_warps) * kDecBlocks + q);
+        uint32_t phase[2] = {0u, 0u};
+        int st = 0;
+        for (; bi < n_batches; bi += n_warps) {
+            const Staged sn = issue(nxt, bi + n_warps, st ^ 1);                  // lands while this batch is unpacked
+            const BlockAt<W> nxt2 = locate((bi + 2 * n_warps) * kDecBlocks + q); // directory reads two batches ahead
+            if (!sc.skip) {
+                if (!sc.direct) {
+                    dec_mbar_wait(&s_mbar[2 * warp + st], phase[st]);
+                    phase[st] ^= 1u;
+                    decode_staged(cur, stage + st * kDecStageChunks + sc.rel);
+                    __syncwarp();                                            // stage and table free again
+                } else {
+                    decode_direct(cur);
+                }
+            }
+            cur = nxt; nxt = nxt2; sc = sn; st ^= 1;
+        }
     }
 
     if (batch) {                                                           // D5: raw streams of the batch
@@ -396,16 +467,16 @@ __global__ void __launch_bounds__(DecCfg<W>::kThreads, DecCfg<W>::kCtasPerSm) k_
 }
 
 // Once per device and instantiation: the dynamic shared memory attribute and the resident CTAs per SM.
-template <int W, bool kBatch>
+template <int W, bool kBatch, bool kTma, bool kBits = false>
 static int dec_ctas_per_sm(int device) {
     static std::mutex mu;
     static int per_sm[kMaxDevices] = {};
     std::lock_guard<std::mutex> lock(mu);
     if (per_sm[device] == 0) {
         int n = 0;
-        if (cudaFuncSetAttribute(k_dec_tiles<W, kBatch>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DecSmem<W>::kBytes) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_dec_tiles<W, kBatch, kTma, kBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DecSmem<W, kTma>::kBytes) != cudaSuccess)
             return 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_dec_tiles<W, kBatch>, DecCfg<W>::kThreads, DecSmem<W>::kBytes) != cudaSuccess || n < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_dec_tiles<W, kBatch, kTma, kBits>, DecCfg<W, kTma>::kThreads, DecSmem<W, kTma>::kBytes) != cudaSuccess || n < 1)
             return 0;
         per_sm[device] = n;
     }
@@ -417,10 +488,17 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     constexpr size_t kSmem = DecSmem<W>::kBytes;
     DeviceInfo dev;
     if (!current_device(&dev)) return BFSC_ERR_CUDA;
-    const int per_sm = a.in_off ? dec_ctas_per_sm<W, true>(dev.device) : dec_ctas_per_sm<W, false>(dev.device);
+    // D1 staging of single-stream calls: per-lane cp.async (default) or, with BFSC_DEC_STAGING=tma in the environment,
+    // one bulk copy (TMA) per warp batch into a two-stage ring. Both are bit-exact (tests run both); the measured
+    // A/B (profiles/r2_dec_staging_ab.md) is why cp.async is the default.
+    const char* staging = getenv("BFSC_DEC_STAGING");
+    const bool use_tma = staging != nullptr && staging[0] == 't';
+    const int per_sm = a.in_off ? dec_ctas_per_sm<W, true, false>(dev.device)
+                                : (use_tma ? dec_ctas_per_sm<W, false, true>(dev.device) : dec_ctas_per_sm<W, false, false>(dev.device));
     if (per_sm < 1) return BFSC_ERR_CUDA;
     const int max_grid = dev.sms * per_sm;
-    const size_t want = (max_blocks + kDecBlocks * DecCfg<W>::kWarps - 1) / (kDecBlocks * DecCfg<W>::kWarps);
+    const int warps = a.in_off || !use_tma ? DecCfg<W, false>::kWarps : DecCfg<W, true>::kWarps;
+    const size_t want = (max_blocks + kDecBlocks * warps - 1) / (kDecBlocks * warps);
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
     if (a.in_off) {
@@ -435,26 +513,33 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
         size_t bgrid = (a.ws.blk_cap + kBlkTabThreads - 1) / kBlkTabThreads;
         if (bgrid > (size_t)dev.sms * 8) bgrid = (size_t)dev.sms * 8;
         BFSC_LAUNCH(launch_dep(k_dec_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a));
-        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true>, max_grid, DecCfg<W>::kThreads, kSmem, s, a));
+        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false>, max_grid, DecCfg<W>::kThreads, kSmem, s, a));
+    } else if (a.sink.bm != nullptr) {
+        const int psm = dec_ctas_per_sm<W, false, false, true>(dev.device);
+        if (psm < 1) return BFSC_ERR_CUDA;
+        const int g = want < (size_t)(dev.sms * psm) ? (want ? (int)want : 1) : dev.sms * psm;
+        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, false, false, true>, g, DecCfg<W>::kThreads, kSmem, s, a));
     } else {
-        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
+        if (use_tma) BFSC_LAUNCH(launch_dep(k_dec_tiles<W, false, true>, grid, DecCfg<W, true>::kThreads, DecSmem<W, true>::kBytes, s, a));
+        else BFSC_LAUNCH(launch_dep(k_dec_tiles<W, false, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
     }
     return BFSC_OK;
 }
 
 static bfsc_status decode_common(const void* d_in, const uint64_t* d_in_off, size_t in_single, size_t n_buf,
                                  bfsc_dtype t, void* d_ids, size_t ids_cap, uint64_t* d_id_off, uint64_t* d_n_ids,
-                                 void* ws, size_t ws_bytes, uint32_t* d_status, void* stream) {
+                                 void* ws, size_t ws_bytes, uint32_t* d_status, void* stream,
+                                 BitSink sink = BitSink{nullptr, 0, 0, nullptr}) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
     if (!d_in || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
-    if (!d_ids && ids_cap) return BFSC_ERR_INVALID_ARG;
+    if (!d_ids && ids_cap && !sink.bm) return BFSC_ERR_INVALID_ARG;
     if (((uintptr_t)d_in & 15) || ((uintptr_t)d_ids & 15) || ((uintptr_t)ws & 15)) return BFSC_ERR_INVALID_ARG;
     DecArgs a;
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.in = (const unsigned char*)d_in; a.in_off = (const unsigned long long*)d_in_off; a.in_single = in_single;
     a.n_buf = (uint32_t)n_buf; a.ids = d_ids; a.ids_cap = ids_cap; a.id_off = (unsigned long long*)d_id_off;
-    a.n_ids_out = (unsigned long long*)d_n_ids; a.status = d_status;
-    const size_t max_blocks = ids_cap / kBlk + n_buf + 1;
+    a.n_ids_out = (unsigned long long*)d_n_ids; a.status = d_status; a.sink = sink;
+    const size_t max_blocks = (sink.bm ? (size_t)sink.n_bits : ids_cap) / kBlk + n_buf + 1;
     return t == BFSC_U32 ? launch_decode<32>(a, max_blocks, (cudaStream_t)stream)
                          : launch_decode<64>(a, max_blocks, (cudaStream_t)stream);
 }
@@ -476,4 +561,13 @@ extern "C" bfsc_status bfsc_decompress_batch(const void* d_in, const uint64_t* d
     if (!d_in_offsets || !d_id_offsets) return BFSC_ERR_INVALID_ARG;
     return bfsc::decode_common(d_in, d_in_offsets, 0, n_buf, t, d_ids, ids_capacity, d_id_offsets, nullptr,
                                d_workspace, workspace_bytes, d_status, cuda_stream);
+}
+
+extern "C" bfsc_status bfsc_decompress_to_bitmap(const void* d_in, size_t in_bytes, bfsc_dtype t, uint64_t id_base,
+                                                 uint32_t* d_bitmap, size_t n_bits, uint64_t* d_n_ids,
+                                                 void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                                 void* cuda_stream) {
+    if (!d_n_ids || !d_bitmap || ((uintptr_t)d_bitmap & 15) || n_bits > (1ull << 32)) return BFSC_ERR_INVALID_ARG;
+    return bfsc::decode_common(d_in, nullptr, in_bytes, 1, t, nullptr, ~(size_t)0, nullptr, d_n_ids, d_workspace,
+                               workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_bitmap, id_base, n_bits, d_status});
 }

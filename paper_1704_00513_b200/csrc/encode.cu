@@ -5,6 +5,7 @@
 // runs and executes griddepcontrol.wait before it touches what the predecessor writes.
 #include <mutex>
 
+#include "bitmap_stage.cuh"
 #include "quad_encode.cuh"
 #include "wide_encode.cuh"
 
@@ -14,6 +15,11 @@ struct EncArgs {
     const void* ids;
     const unsigned long long* in_off;   // n_buf+1 element offsets, or nullptr (single buffer of n_single IDs)
     unsigned long long n_single;
+    const uint32_t* bitmap;             // bfsc_compress_bitmap (FORMAT.md §9): the IDs are the set bits of bitmap[0 .. n_bits), + id_base;
+    unsigned long long n_bits, id_base; //   their number is counted on the device (ws.hdr->n_ids); ids == nullptr then
+    unsigned long long* chunk;          //   bitmap: set bits before every 1024-bit chunk (n_chunks + 1 entries, after the standard workspace)
+    unsigned long long n_chunks;
+    uint32_t fallback;                  // BFSC_CODEC_FLAG_RAW_FALLBACK (FORMAT.md §8), single-buffer calls
     uint32_t n_buf;
     uint32_t codec;                     // encoder rule = mode byte: 1 PFOR-D1 (E2: size argmin), 2 BP128-D1 (b = maxw, no exceptions; FORMAT.md §7)
     uint32_t exclusive;                 // BFSC_CODEC_FLAG_EXCLUSIVE: the CTAs' first two tiles are static (grid CTAs; tickets start at 2 grid)
@@ -280,18 +286,22 @@ __device__ __forceinline__ unsigned long long lookback(const unsigned long long*
 // fast path (with 320-byte slots a stream of 22-bit gaps took 141 us instead of 37). u64: 288 B (b = 17), so that
 // two CTAs of the batch instantiation (1 KB blocks staged, 10 KB of bookkeeping) still fit one SM; larger u64
 // blocks (gaps over 2^17 between sorted 64-bit IDs) take the slow path.
-template <int W> struct ImgCfg {
-    static constexpr int kSlotChunks = (W == 32) ? 34 : 18;   // 16-byte chunks per block
-    static constexpr int kCap = (W == 32) ? 544 : 288;        // bytes of a block image the fast path can hold
+// kSrc: where the IDs come from — 0: one ID array, 1: a batch of ID arrays, 2: a frontier bitmap (FORMAT.md §9). A bitmap
+// has no ID array for the slow path to re-read, so its image slots hold every block (544 B) for both widths (deltas of a
+// bitmap of < 2^32 bits fit 32 bits), and each worker warp gets a landing area for the bitmap words of its 8 blocks.
+template <int W, int kSrc = 0> struct ImgCfg {
+    static constexpr int kSlotChunks = (W == 32 || kSrc == 2) ? 34 : 18;   // 16-byte chunks per block
+    static constexpr int kCap = kSlotChunks * 16;                          // bytes of a block image the fast path can hold
     static constexpr int kBufChunks = kQuadBlocks * kSlotChunks;
 };
 
 constexpr int kDefer = 1;                                     // a tile's images leave kDefer tiles after they were packed
 constexpr int kNB = kDefer + 1;                               // image buffers / size and offset tables per CTA
+constexpr int kLandChunks = 32;                               // bitmap words of a warp batch staged by cp.async: 512 B = 4096 bits (denser than 1 ID in 4 bits on average; sparser batches are read from global memory)
 
-template <int W> struct EncSmem {
+template <int W, int kSrc = 0> struct EncSmem {
     static constexpr int kStageChunks = RawCfg<W>::kAreaChunks;              // per worker warp: staged raw IDs
-    static constexpr int kWarpChunks = kStageChunks + kNB * ImgCfg<W>::kBufChunks;   // + the image buffers
+    static constexpr int kWarpChunks = kStageChunks + kNB * ImgCfg<W, kSrc>::kBufChunks + (kSrc == 2 ? kLandChunks : 0);   // + the image buffers (+ landing area)
     static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
 };
 
@@ -309,9 +319,12 @@ constexpr int kRing = 8;                                      // ring of tile bo
 //       predecessor CTA does not stall this CTA's workers.
 // Tiles: every one comes from the ticket counter (prep warp), each drawn at the same point of the pipeline: a lower
 // tile number means "sizes posted earlier" — and is held by a running CTA, whatever else occupies the device.
-template <int W, bool kBatch>
+template <int W, int kSrc>
 __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
+    constexpr bool kBatch = kSrc == 1, kBits = kSrc == 2;
+    using Img = ImgCfg<W, kSrc>;
+    using Smem = EncSmem<W, kSrc>;
     extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | kNB image buffers
     __shared__ uint32_t s_key[kNB][kTileR];              // workers: size<<14 | (64-b)<<7 | n_exc, 0 = no block
     __shared__ unsigned long long s_at[kNB][kTileR];     // scan warp: final byte offset of the block, or kSkip
@@ -336,7 +349,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     constexpr bool batch = kBatch;
     const T* ids = reinterpret_cast<const T*>(a.ids);
     pdl_launch_dependents();                             // the next call's first kernel may be set up; it waits for this grid
-    if constexpr (!kBatch) {
+    if constexpr (kSrc == 0) {
         // Single-buffer calls: the plan kernel (ticket counter, zeroed look-back states) is still running.
         if (a.exclusive) {
             // static first tile (tile blockIdx.x): its loads go out before anything else in the kernel
@@ -344,7 +357,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 const unsigned long long g = (unsigned long long)blockIdx.x * kTileR + warp * kQuadBlocks + (lane >> 2);
                 const unsigned long long nb0 = (a.n_single + kBlk - 1) / kBlk;
                 if (g < nb0)
-                    quad_prefetch<W>(dyn_smem + warp * EncSmem<W>::kWarpChunks + raw_slot_chunk<W>(lane >> 2), ids + kBlk * g,
+                    quad_prefetch<W>(dyn_smem + warp * Smem::kWarpChunks + raw_slot_chunk<W>(lane >> 2), ids + kBlk * g,
                                      (int)min((unsigned long long)kBlk, a.n_single - kBlk * g));
             }
         } else if (warp < kEncWorkers && lane == 0) {
@@ -364,13 +377,25 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     if (threadIdx.x >= 32 && threadIdx.x < 32 + kNB) mbar_init(&mb_off[threadIdx.x - 32], 1);
     __syncthreads();
 
-    const unsigned long long nb_single = (a.n_single + kBlk - 1) / kBlk;
+    // n_ids: IDs of the one stream of a single-buffer call — an argument, or (bitmap) counted by the kernels before
+    unsigned long long n_ids = a.n_single;
+    if constexpr (kBits) {
+        pdl_wait();
+        n_ids = a.ws.hdr->ok != 0 ? a.ws.hdr->n_ids : 0ull;
+    }
+    unsigned long long nb_single = (n_ids + kBlk - 1) / kBlk;
+    if constexpr (kBits) nb_single = a.ws.hdr->ok != 0 ? a.ws.hdr->total_blocks : 0ull;    // (0: RAW by the threshold, k_bm_finish)
     unsigned long long total = nb_single;
     if (batch) {
         pdl_wait();
         total = a.ws.hdr->ok != 0 ? a.ws.hdr->total_blocks : 0ull;
     }
     const unsigned long long n_tiles = (total + kTileR - 1) / kTileR;
+    // bitmap source: ring of the tiles' block starts (bit index of each block's first ID; entry 64 = end of the tile's
+    // last block), copied from ws.blk_tab (k_bm_starts) by the prep warp
+    constexpr int kSt = kBits ? kTileR + 1 : 1;
+    __shared__ uint32_t s_start[kRing][kSt];
+    const uint32_t* starts = reinterpret_cast<const uint32_t*>(a.ws.blk_tab);
 
     auto prep = [&](unsigned long long t, int p) {       // bookkeeping of tile t into ring slot p (one warp)
         if (lane == 0) s_tile[p] = t;
@@ -386,13 +411,19 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             s_m[p][jj] = m; s_xoff[p][jj] = xoff; s_buf[p][jj] = i;
           }
         }
+        if constexpr (kBits) {
+            for (int jj = lane; jj <= kTileR; jj += 32) {
+                const unsigned long long g = min(t * kTileR + jj, total);        // starts[total] = n_bits
+                s_start[p][jj] = __ldcg(starts + g);
+            }
+        }
     };
     // valid IDs / element offset of block jj of the tile in ring slot p (the tile is posted and not kNoTile)
     auto blk_m = [&](int p, int jj) -> int {
         if constexpr (kBatch) return s_m[p][jj];
         else {
             const unsigned long long g = s_tile[p] * kTileR + jj;
-            return g < nb_single ? (int)min((unsigned long long)kBlk, a.n_single - kBlk * g) : 0;
+            return g < nb_single ? (int)min((unsigned long long)kBlk, n_ids - kBlk * g) : 0;
         }
     };
     auto blk_xoff = [&](int p, int jj) -> unsigned long long {
@@ -502,7 +533,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                             uint4 h0, h1;
                             h0.x = 0x43534642u;                                   // "BFSC"
                             h0.y = 1u | ((uint32_t)W << 8) | (a.codec << 16);     // mode = the encoder rule
-                            h0.z = (uint32_t)a.n_single; h0.w = (uint32_t)(a.n_single >> 32);
+                            h0.z = (uint32_t)n_ids; h0.w = (uint32_t)(n_ids >> 32);
                             h1.x = (uint32_t)tot; h1.y = (uint32_t)(tot >> 32);
                             h1.z = (uint32_t)nb_single; h1.w = 0;
                             reinterpret_cast<uint4*>(a.out)[0] = h0;
@@ -576,14 +607,20 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
 
     // =============================== worker warps ===============================
     const int q = lane >> 2, l = lane & 3;
-    uint4* area = dyn_smem + warp * EncSmem<W>::kWarpChunks;
+    uint4* area = dyn_smem + warp * Smem::kWarpChunks;
     uint4* slot = area + raw_slot_chunk<W>(q);                           // staging: the quad's raw IDs
-    unsigned char* ibuf = reinterpret_cast<unsigned char*>(area + EncSmem<W>::kStageChunks);   // the warp's kNB image buffers
+    unsigned char* ibuf = reinterpret_cast<unsigned char*>(area + Smem::kStageChunks);   // the warp's kNB image buffers
     const int j = warp * kQuadBlocks + q;
     constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
     mbar_wait(&mb_post[0], 0);                                           // the CTA's first tile is posted (by the prep warp)
     bool have = s_tile[0] != kNoTile;
-    if (have && (kBatch || !a.exclusive)) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));   // (exclusive single-buffer calls: see the top)
+    uint4* land = area + Smem::kStageChunks + kNB * Img::kBufChunks;      // bitmap source: the words of the warp's 8 blocks
+    if constexpr (kBits) {
+        static_assert(!kBits || Img::kCap >= 16 + 16 * 32 + 16, "a bitmap has no ID array for the slow path: every block must fit its image slot");
+        if (have) bm_prefetch<kLandChunks>(land, a.bitmap, s_start[0], warp, lane);
+    } else {
+        if (have && (kBatch || !a.exclusive)) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));   // (exclusive single-buffer calls: see the top)
+    }
     static_assert(kDefer == 1 || kDefer == 2, "hist selection below");
     uint32_t key_hist[kDefer] = {}, woff_hist[kDefer] = {};              // keys and image places of the tiles that wait in shared memory
     int kp = 0;                                                          // k % kNB
@@ -593,21 +630,25 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
         bool have_next = false;
         if (have) {
             const int m = blk_m(k & (kRing - 1), j);
-            const T* raw = reinterpret_cast<const T*>(slot) +
-                           (reinterpret_cast<uintptr_t>(ids + blk_xoff(k & (kRing - 1), j)) & 15) / sizeof(T);
-            unsigned char* ib = ibuf + kp * (ImgCfg<W>::kBufChunks * 16);        // this tile's image buffer
+            const T* raw = reinterpret_cast<const T*>(slot);
+            if constexpr (!kBits) raw += (reinterpret_cast<uintptr_t>(ids + blk_xoff(k & (kRing - 1), j)) & 15) / sizeof(T);
+            unsigned char* ib = ibuf + kp * (Img::kBufChunks * 16);        // this tile's image buffer
             cp_async_wait_all();
             __syncwarp();
+            if constexpr (kBits) {                                       // E1, first half: the block's set bits -> raw IDs in the slot
+                bm_expand<T, kLandChunks>(reinterpret_cast<T*>(slot), s_start[k & (kRing - 1)], warp, q, l, land, a.bitmap, a.id_base);
+                __syncwarp();
+            }
             uint32_t d[32];
             bool wide_lane = false, wide = false;
             const T base = col_deltas<W>(raw, m, d, wide_lane);          // E1
-            if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
+            if constexpr (W == 64 && !kBits) wide = __any_sync(kFull, wide_lane);   // (a bitmap of < 2^32 bits: every delta fits 32 bits)
             if (!wide) key = a.codec == BFSC_CODEC_BP128 ? quad_max_width_key(d) : quad_choose_b<W>(d);   // E2
             // The bulk store that read this image buffer (issued when the previous iteration ended) is done with it.
             // Not waited for before E2: the copy engine needs half a microsecond to fetch its source.
             if (lane == 0) bulk_wait_read();
             __syncwarp();
-            if (wide) key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (ImgCfg<W>::kSlotChunks * 16)),
+            if (wide) key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(ib + q * (Img::kSlotChunks * 16)),
                                      a.codec == BFSC_CODEC_BP128);
             if (m <= 0) key = 0;
             if (l == 0) s_key[kp][j] = key;
@@ -630,7 +671,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             bar_arrive(kBarSizes + kp, kSizesThreads);
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
-            const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)ImgCfg<W>::kCap);   // slow path, in global memory later
+            const bool late = !kBits && key != 0 && (wide || (key >> 14) > (uint32_t)Img::kCap);   // slow path, in global memory later
             const bool fast = !wide && key != 0 && !late;
             // The warp's 8 images lie back to back in the buffer, as they do in the output (consecutive blocks):
             // woff = exclusive scan of the fast blocks' sizes over the quads, in 16-byte chunks.
@@ -648,7 +689,11 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             __syncwarp();                                                // the warp's staged IDs are consumed
             mbar_wait(&mb_post[(k + 1) & (kRing - 1)], ((k + 1) / kRing) & 1);   // tile k+1 is posted
             have_next = s_tile[(k + 1) & (kRing - 1)] != kNoTile;
-            if (have_next) quad_prefetch<W>(slot, ids + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));   // same slots
+            if constexpr (kBits) {
+                if (have_next) bm_prefetch<kLandChunks>(land, a.bitmap, s_start[(k + 1) & (kRing - 1)], warp, lane);
+            } else {
+                if (have_next) quad_prefetch<W>(slot, ids + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));   // same slots
+            }
             if (fast) {                                                  // payload + header
                 if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
                 if (l == 0) {                                            // block header (FORMAT.md §2)
@@ -673,11 +718,11 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             if (key_e != 0) at = s_at[kpe][j];
             if (__any_sync(kFull, (key_e & kLateBit) != 0)) {
                 const bool mine = (key_e & kLateBit) != 0 && at != kSkip;
-                late_emit<W>(ids + blk_xoff(ke & (kRing - 1), j), blk_m(ke & (kRing - 1), j), key_e & ~kLateBit, mine ? a.out + at : nullptr);
+                if constexpr (!kBits) late_emit<W>(ids + blk_xoff(ke & (kRing - 1), j), blk_m(ke & (kRing - 1), j), key_e & ~kLateBit, mine ? a.out + at : nullptr);
             }
             // images -> their final place. Usual case: the warp's blocks are consecutive in the output as well
             // (same stream, none late, all fit): ONE bulk store of the whole buffer by lane 0.
-            const unsigned char* ib_e = ibuf + kpe * (ImgCfg<W>::kBufChunks * 16);
+            const unsigned char* ib_e = ibuf + kpe * (Img::kBufChunks * 16);
             const bool valid = key_e != 0, fast_e = valid && (key_e & kLateBit) == 0;
             const uint32_t z_e = fast_e ? key_e >> 18 : 0u;
             const unsigned long long at_n = __shfl_down_sync(kFull, at, 4);
@@ -775,17 +820,218 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     }
 }
 
+// ---- FORMAT.md §8: RAW fallback of a single-buffer call (ID array source). After the stream is complete (its size is
+// in ws.hdr->total_out): if it is not smaller than the RAW stream of the same IDs, it is overwritten by that one
+// (header, verbatim IDs, zero pad) and *out_total follows. The input is read a second time only then.
+template <int W>
+__global__ void __launch_bounds__(256) k_enc_fallback(EncArgs a) {
+    using T = typename IdT<W>::T;
+    constexpr unsigned long long E = W / 8;
+    pdl_wait();
+    pdl_launch_dependents();
+    const unsigned long long n = a.n_single, body = (n * E + 15ull) & ~15ull, raw_total = 32ull + body;
+    if (a.ws.hdr->ok == 0 || n * E < a.thr) return;                          // RAW already (by the threshold)
+    const unsigned long long have = a.ws.hdr->total_out;
+    if (have > a.out_cap || have < raw_total) return;                        // (an error was flagged) | smaller: keep
+    const T* x = reinterpret_cast<const T*>(a.ids);
+    T* y = reinterpret_cast<T*>(a.out + 32);
+    const unsigned long long padded = body / E;
+    for (unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < padded;
+         j += (unsigned long long)gridDim.x * blockDim.x)
+        y[j] = j < n ? x[j] : (T)0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        uint4 h0, h1;
+        h0.x = 0x43534642u; h0.y = 1u | ((uint32_t)W << 8);                  // mode 0
+        h0.z = (uint32_t)n; h0.w = (uint32_t)(n >> 32);
+        h1.x = (uint32_t)raw_total; h1.y = (uint32_t)(raw_total >> 32); h1.z = 0; h1.w = 0;
+        reinterpret_cast<uint4*>(a.out)[0] = h0;
+        reinterpret_cast<uint4*>(a.out)[1] = h1;
+        if (a.out_total) *a.out_total = raw_total;
+    }
+}
+
+// ---- FORMAT.md §9: a frontier bitmap as the source. Chunk = 32 words = 1024 bits.
+constexpr int kChunkBits = 1024;
+
+// set bits of every chunk -> a.chunk[c] (bits at positions >= n_bits do not count). One warp per chunk.
+__global__ void __launch_bounds__(256) k_bm_count(EncArgs a) {
+    pdl_wait();                                          // the call before this one is complete (workspace, inputs)
+    pdl_launch_dependents();
+    const int lane = threadIdx.x & 31;
+    for (unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); c < a.n_chunks; c += (unsigned long long)gridDim.x * 8) {
+        const unsigned long long bit0 = c * kChunkBits + 32ull * lane;
+        uint32_t x = bit0 < a.n_bits ? a.bitmap[c * 32 + lane] : 0u;
+        if (bit0 < a.n_bits && a.n_bits - bit0 < 32) x &= (1u << (uint32_t)(a.n_bits - bit0)) - 1u;
+        const uint32_t k = __reduce_add_sync(kFull, (uint32_t)__popc(x));
+        if (lane == 0) a.chunk[c] = k;
+    }
+}
+
+// One CTA: exclusive scan of the chunk counts (in place; entry n_chunks = n), then the plan of the one stream (E0).
+template <int W>
+__global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
+    __shared__ Scan2 sm[33];
+    constexpr unsigned long long E = W / 8;
+    pdl_wait();
+    pdl_launch_dependents();
+    Scan2 carry{0, 0};
+    constexpr int kIpt = 8;
+    for (unsigned long long c0 = 0; c0 < a.n_chunks; c0 += 1024ull * kIpt) {
+        unsigned long long v[kIpt];
+        Scan2 sum{0, 0};
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const unsigned long long c = c0 + (unsigned long long)threadIdx.x * kIpt + u;
+            v[u] = c < a.n_chunks ? a.chunk[c] : 0ull;
+            sum.a += v[u];
+        }
+        Scan2 tot;
+        Scan2 ex = block_scan_excl2(sum, &tot, sm);
+        unsigned long long run = carry.a + ex.a;
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const unsigned long long c = c0 + (unsigned long long)threadIdx.x * kIpt + u;
+            if (c < a.n_chunks) a.chunk[c] = run;
+            run += v[u];
+        }
+        carry.a += tot.a;
+    }
+    const unsigned long long n = carry.a;
+    const bool raw = n * E < a.thr;
+    const unsigned long long nb_all = (n + kBlk - 1) / kBlk, nb = raw ? 0ull : nb_all;
+    const unsigned long long fixed = raw ? 32ull + ((n * E + 15ull) & ~15ull) : 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull);
+    const unsigned long long nt = (nb + kTileR - 1) / kTileR;
+    const bool ok = nb_all + 1 <= a.ws.blk_cap && nt <= a.ws.tile_cap;
+    if (ok)
+        for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q * kStateStride] = 0;
+    if (threadIdx.x == 0) {
+        a.chunk[a.n_chunks] = n;
+        a.ws.blk_first[0] = 0; a.ws.blk_first[1] = nb;
+        a.ws.fixed_prefix[0] = 0; a.ws.fixed_prefix[1] = fixed;
+        a.ws.stream_start[0] = 0; a.ws.stream_start[1] = 0;
+        a.ws.hdr->total_blocks = nb; a.ws.hdr->fixed_total = fixed; a.ws.hdr->ticket = 0;
+        a.ws.hdr->grand16 = 0; a.ws.hdr->total_out = fixed; a.ws.hdr->ok = ok ? 1u : 0u; a.ws.hdr->n_ids = n;
+        if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
+        if (a.out_total) *a.out_total = 0;               // (the last tile, or k_bm_finish, writes the size)
+    }
+}
+
+// Where every block begins: starts[g] = bit index of the (128 g)-th set bit (u32, in ws.blk_tab), starts[nb_all] = n_bits.
+// One warp per chunk: the chunk holds the block starts 128 g in [prefix, prefix + count): at most 8.
+__global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
+    pdl_wait();
+    pdl_launch_dependents();
+    if (a.ws.hdr->ok == 0) return;
+    uint32_t* starts = reinterpret_cast<uint32_t*>(a.ws.blk_tab);
+    const int lane = threadIdx.x & 31;
+    const unsigned long long n = a.ws.hdr->n_ids;
+    if (blockIdx.x == 0 && threadIdx.x == 0) starts[(n + kBlk - 1) / kBlk] = (uint32_t)a.n_bits;
+    for (unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); c < a.n_chunks; c += (unsigned long long)gridDim.x * 8) {
+        const unsigned long long p0 = a.chunk[c], p1 = a.chunk[c + 1];
+        unsigned long long g = (p0 + kBlk - 1) / kBlk;   // first block that starts at or after rank p0
+        if (g * kBlk >= p1) continue;                    // no block starts in this chunk
+        const unsigned long long bit0 = c * kChunkBits + 32ull * lane;
+        uint32_t x = bit0 < a.n_bits ? a.bitmap[c * 32 + lane] : 0u;
+        if (bit0 < a.n_bits && a.n_bits - bit0 < 32) x &= (1u << (uint32_t)(a.n_bits - bit0)) - 1u;
+        const uint32_t k = (uint32_t)__popc(x);
+        uint32_t inc = k;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        const uint32_t excl = inc - k;
+        for (; g * kBlk < p1; g++) {
+            const uint32_t r = (uint32_t)(g * kBlk - p0);            // rank inside the chunk
+            if (r >= excl && r < excl + k) starts[g] = (uint32_t)(bit0 + __fns(x, 0, (int)(r - excl) + 1));
+        }
+    }
+}
+
+// After the tiles: the streams the tile kernel does not write. (i) RAW by the threshold, (ii) RAW by the fallback rule
+// (FORMAT.md §8), both expanded from the bitmap block by block (one warp per block); (iii) the empty stream (no tile
+// ran). The decision reads the size the plan / the last tile has left in ws.hdr->total_out; *out_total is written
+// by one thread (nobody reads it).
+template <int W>
+__global__ void __launch_bounds__(256) k_bm_finish(EncArgs a) {
+    using T = typename IdT<W>::T;
+    constexpr unsigned long long E = W / 8;
+    pdl_wait();
+    pdl_launch_dependents();
+    if (a.ws.hdr->ok == 0) return;                                           // (*out_total = 0 since the plan)
+    const unsigned long long n = a.ws.hdr->n_ids, body = (n * E + 15ull) & ~15ull, raw_total = 32ull + body;
+    const bool raw_thr = n * E < a.thr;
+    const unsigned long long have = a.ws.hdr->total_out;                     // raw_thr: = raw_total; n = 0: 48
+    const bool first = blockIdx.x == 0 && threadIdx.x == 0;
+    if (!raw_thr && have > a.out_cap) {                                      // flagged by the tiles, except when there was none
+        if (n == 0 && first) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+        return;
+    }
+    const bool to_raw = raw_thr || (a.fallback && have >= raw_total);
+    if (!to_raw) {
+        if (n == 0 && first) {                                               // (iii) 48 bytes: header, dir[0] = 3
+            uint4 h0, h1;
+            h0.x = 0x43534642u; h0.y = 1u | ((uint32_t)W << 8) | (a.codec << 16); h0.z = 0; h0.w = 0;
+            h1.x = 48u; h1.y = 0; h1.z = 0; h1.w = 0;
+            reinterpret_cast<uint4*>(a.out)[0] = h0;
+            reinterpret_cast<uint4*>(a.out)[1] = h1;
+            reinterpret_cast<uint4*>(a.out)[2] = make_uint4(3u, 0u, 0u, 0u);
+            if (a.out_total) *a.out_total = 48ull;
+        }
+        return;
+    }
+    if (raw_total > a.out_cap) {
+        if (first) { set_status(a.status, BFSC_ERR_DST_TOO_SMALL); if (a.out_total) *a.out_total = 0; }
+        return;
+    }
+    const uint32_t* starts = reinterpret_cast<const uint32_t*>(a.ws.blk_tab);
+    const unsigned long long nb_all = (n + kBlk - 1) / kBlk;
+    const int lane = threadIdx.x & 31;
+    T* y = reinterpret_cast<T*>(a.out + 32);
+    for (unsigned long long g = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); g < nb_all; g += (unsigned long long)gridDim.x * 8) {
+        const uint32_t s = starts[g], e = starts[g + 1];
+        if (e <= s) continue;
+        const uint32_t w_first = s >> 5, w_last = (e - 1u) >> 5;
+        uint32_t rank = 0;
+        for (uint32_t w = w_first; w <= w_last && w >= w_first; w += 32) {
+            const uint32_t wi = w + (uint32_t)lane;
+            uint32_t x = (wi <= w_last && wi >= w) ? a.bitmap[wi] : 0u;
+            if (wi == w_first) x &= 0xffffffffu << (s & 31u);
+            if (wi == w_last && (e & 31u)) x &= (1u << (e & 31u)) - 1u;
+            const uint32_t k = (uint32_t)__popc(x);
+            uint32_t inc = k;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += t; }
+            uint32_t pos = rank + inc - k;
+            rank += __shfl_sync(kFull, inc, 31);
+            while (x) {
+                const uint32_t b = (uint32_t)__ffs((int)x) - 1u;
+                x &= x - 1u;
+                y[g * kBlk + pos++] = (T)(a.id_base + 32ull * wi + b);
+            }
+        }
+    }
+    for (unsigned long long j = n + (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < body / E; j += (unsigned long long)gridDim.x * blockDim.x)
+        y[j] = (T)0;                                                         // zero pad
+    if (first) {
+        uint4 h0, h1;
+        h0.x = 0x43534642u; h0.y = 1u | ((uint32_t)W << 8);                  // mode 0
+        h0.z = (uint32_t)n; h0.w = (uint32_t)(n >> 32);
+        h1.x = (uint32_t)raw_total; h1.y = (uint32_t)(raw_total >> 32); h1.z = 0; h1.w = 0;
+        reinterpret_cast<uint4*>(a.out)[0] = h0;
+        reinterpret_cast<uint4*>(a.out)[1] = h1;
+        if (a.out_total) *a.out_total = raw_total;
+    }
+}
+
 // Once per device and instantiation: the dynamic shared memory attribute and the resident CTAs per SM.
-template <int W, bool kBatch>
+template <int W, int kSrc>
 static int enc_ctas_per_sm(int device) {
     static std::mutex mu;
     static int per_sm[kMaxDevices] = {};
     std::lock_guard<std::mutex> lock(mu);
     if (per_sm[device] == 0) {
         int n = 0;
-        if (cudaFuncSetAttribute(k_enc_tiles<W, kBatch>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EncSmem<W>::kBytes) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_enc_tiles<W, kSrc>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EncSmem<W, kSrc>::kBytes) != cudaSuccess)
             return 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_enc_tiles<W, kBatch>, kEncThreads, EncSmem<W>::kBytes) != cudaSuccess || n < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_enc_tiles<W, kSrc>, kEncThreads, EncSmem<W, kSrc>::kBytes) != cudaSuccess || n < 1)
             return 0;
         per_sm[device] = n;
     }
@@ -800,7 +1046,7 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     constexpr unsigned long long E = W / 8;
     const bool single = a_in.in_off == nullptr;
     const bool degenerate = single && (a_in.n_single == 0 || a_in.n_single * E < a_in.thr);   // no block: header (+ raw copy) only
-    const int per_sm = single ? enc_ctas_per_sm<W, false>(dev.device) : enc_ctas_per_sm<W, true>(dev.device);
+    const int per_sm = single ? enc_ctas_per_sm<W, 0>(dev.device) : enc_ctas_per_sm<W, 1>(dev.device);
     if (per_sm < 1) return BFSC_ERR_CUDA;
     int grid = dev.sms * per_sm;                                 // one resident wave (every tile is drawn by ticket: any grid size is correct)
     if (single) {
@@ -817,14 +1063,45 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         BFSC_LAUNCH(launch_dep(k_enc_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a));
     }
     if (!degenerate) {
-        if (single) BFSC_LAUNCH(launch_dep(k_enc_tiles<W, false>, grid, kEncThreads, kSmem, s, a));
-        else BFSC_LAUNCH(launch_dep(k_enc_tiles<W, true>, grid, kEncThreads, kSmem, s, a));
+        if (single) BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 0>, grid, kEncThreads, kSmem, s, a));
+        else BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 1>, grid, kEncThreads, kSmem, s, a));
     }
     if (!single || degenerate) {
         uint32_t sgrid = (a.n_buf + 7) / 8;                      // one warp per buffer
         if (sgrid > (uint32_t)dev.sms * 8) sgrid = (uint32_t)dev.sms * 8;
         BFSC_LAUNCH(launch_dep(k_enc_streams<W>, sgrid ? (int)sgrid : 1, 256, 0, s, a));
     }
+    if (single && a.fallback) {
+        size_t fgrid = (a.n_single * E / (256 * 16 * 4)) + 1;    // 16 bytes per thread and round, a few rounds
+        if (fgrid > (size_t)dev.sms * 8) fgrid = (size_t)dev.sms * 8;
+        BFSC_LAUNCH(launch_dep(k_enc_fallback<W>, (int)fgrid, 256, 0, s, a));
+    }
+    return BFSC_OK;
+}
+
+// bfsc_compress_bitmap: count -> plan -> starts -> tiles -> finish (the tile count is known on the device only: one
+// resident wave of CTAs, or fewer when even a full bitmap has fewer tiles; tiles are drawn by ticket).
+template <int W>
+static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
+    constexpr size_t kSmem = EncSmem<W, 2>::kBytes;
+    DeviceInfo dev;
+    if (!current_device(&dev)) return BFSC_ERR_CUDA;
+    const int per_sm = enc_ctas_per_sm<W, 2>(dev.device);
+    if (per_sm < 1) return BFSC_ERR_CUDA;
+    EncArgs a = a_in;
+    int grid = dev.sms * per_sm;
+    const unsigned long long max_tiles = ((a.n_bits + kBlk - 1) / kBlk + kTileR - 1) / kTileR;
+    if (max_tiles > a.ws.tile_cap) return BFSC_ERR_INVALID_ARG;              // workspace too small
+    if (max_tiles < (unsigned long long)grid) grid = max_tiles ? (int)max_tiles : 1;
+    a.grid = (uint32_t)grid;
+    size_t cgrid = (size_t)((a.n_chunks + 7) / 8);
+    if (cgrid > (size_t)dev.sms * 8) cgrid = (size_t)dev.sms * 8;
+    if (cgrid < 1) cgrid = 1;
+    BFSC_LAUNCH(launch_dep(k_bm_count, (int)cgrid, 256, 0, s, a));
+    BFSC_LAUNCH(launch_dep(k_bm_plan<W>, 1, 1024, 0, s, a));
+    BFSC_LAUNCH(launch_dep(k_bm_starts, (int)cgrid, 256, 0, s, a));
+    BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 2>, grid, kEncThreads, kSmem, s, a));
+    BFSC_LAUNCH(launch_dep(k_bm_finish<W>, (int)cgrid, 256, 0, s, a));
     return BFSC_OK;
 }
 
@@ -833,13 +1110,16 @@ static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint
                                  uint64_t* d_out_total, void* ws, size_t ws_bytes, uint32_t* d_status, void* stream) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
     const uint32_t exclusive = ((uint32_t)codec & (uint32_t)BFSC_CODEC_FLAG_EXCLUSIVE) ? 1u : 0u;
-    codec = (bfsc_codec)((uint32_t)codec & ~(uint32_t)BFSC_CODEC_FLAG_EXCLUSIVE);
+    const uint32_t fallback = ((uint32_t)codec & (uint32_t)BFSC_CODEC_FLAG_RAW_FALLBACK) ? 1u : 0u;
+    codec = (bfsc_codec)((uint32_t)codec & ~(uint32_t)(BFSC_CODEC_FLAG_EXCLUSIVE | BFSC_CODEC_FLAG_RAW_FALLBACK));
     if (codec != BFSC_CODEC_PFOR && codec != BFSC_CODEC_BP128) return BFSC_ERR_INVALID_ARG;
+    if (fallback && d_in_off) return BFSC_ERR_UNSUPPORTED;                  // FORMAT.md §8: single-buffer calls
     if (!d_out || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
     if (((uintptr_t)d_ids & 15) || ((uintptr_t)d_out & 15) || ((uintptr_t)ws & 15)) return BFSC_ERR_INVALID_ARG;
     if (!d_ids && (d_in_off || n_single)) return BFSC_ERR_INVALID_ARG;
-    EncArgs a;
+    EncArgs a = {};
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
+    a.fallback = fallback;
     a.ids = d_ids; a.in_off = (const unsigned long long*)d_in_off; a.n_single = n_single;
     a.n_buf = (uint32_t)n_buf; a.codec = (uint32_t)codec; a.exclusive = exclusive; a.grid = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
     a.out_off = (unsigned long long*)d_out_off; a.out_total = (unsigned long long*)d_out_total; a.status = d_status;
@@ -855,6 +1135,29 @@ extern "C" bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, 
     if (!d_out_bytes) return BFSC_ERR_INVALID_ARG;
     return bfsc::encode_common(codec, d_ids, nullptr, n_ids, 1, t, raw_threshold_bytes, d_out, out_capacity, nullptr,
                                d_out_bytes, d_workspace, workspace_bytes, d_status, cuda_stream);
+}
+
+extern "C" bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_bitmap, size_t n_bits, uint64_t id_base,
+                                            bfsc_dtype t, size_t raw_threshold_bytes, void* d_out, size_t out_capacity,
+                                            uint64_t* d_out_bytes, void* d_workspace, size_t workspace_bytes,
+                                            uint32_t* d_status, void* cuda_stream) {
+    using namespace bfsc;
+    if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
+    const uint32_t fallback = ((uint32_t)codec & (uint32_t)BFSC_CODEC_FLAG_RAW_FALLBACK) ? 1u : 0u;
+    codec = (bfsc_codec)((uint32_t)codec & ~(uint32_t)(BFSC_CODEC_FLAG_EXCLUSIVE | BFSC_CODEC_FLAG_RAW_FALLBACK));   // (exclusive: no effect here)
+    if (codec != BFSC_CODEC_PFOR && codec != BFSC_CODEC_BP128) return BFSC_ERR_INVALID_ARG;
+    if (!d_out || !d_out_bytes || !d_workspace || (n_bits && !d_bitmap)) return BFSC_ERR_INVALID_ARG;
+    if ((unsigned long long)n_bits >= (1ull << 32)) return BFSC_ERR_INVALID_ARG;
+    if (((uintptr_t)d_bitmap & 15) || ((uintptr_t)d_out & 15) || ((uintptr_t)d_workspace & 15)) return BFSC_ERR_INVALID_ARG;
+    const size_t std_bytes = align_up(ws_bytes_for(n_bits, 1), 16), n_chunks = (n_bits + kChunkBits - 1) / kChunkBits;
+    if (workspace_bytes < std_bytes + 8 * (n_chunks + 1)) return BFSC_ERR_INVALID_ARG;
+    EncArgs a = {};
+    if (!ws_carve(d_workspace, std_bytes, 1, &a.ws)) return BFSC_ERR_INVALID_ARG;
+    a.bitmap = d_bitmap; a.n_bits = n_bits; a.id_base = id_base;
+    a.chunk = reinterpret_cast<unsigned long long*>(static_cast<char*>(d_workspace) + std_bytes); a.n_chunks = n_chunks;
+    a.fallback = fallback; a.n_buf = 1; a.codec = (uint32_t)codec; a.thr = raw_threshold_bytes;
+    a.out = (unsigned char*)d_out; a.out_cap = out_capacity; a.out_total = (unsigned long long*)d_out_bytes; a.status = d_status;
+    return t == BFSC_U32 ? launch_encode_bitmap<32>(a, (cudaStream_t)cuda_stream) : launch_encode_bitmap<64>(a, (cudaStream_t)cuda_stream);
 }
 
 extern "C" bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,

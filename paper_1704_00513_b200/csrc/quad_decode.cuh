@@ -22,6 +22,27 @@ __device__ __forceinline__ void dec_cp_async16(void* smem_dst, const void* gmem_
 }
 __device__ __forceinline__ void dec_cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// D1, bulk variant: mbarrier + cp.async.bulk (TMA), one copy per warp batch, issued by one lane.
+__device__ __forceinline__ void dec_mbar_init(unsigned long long* b, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void dec_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void dec_mbar_expect_tx(unsigned long long* b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void dec_bulk_load(void* sdst, const void* gsrc, uint32_t bytes, unsigned long long* b) {   // 16-byte aligned, multiple of 16
+    asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"((uint32_t)__cvta_generic_to_shared(sdst)),
+                 "l"(gsrc), "r"(bytes), "r"((uint32_t)__cvta_generic_to_shared(b)) : "memory");
+}
+__device__ __forceinline__ void dec_mbar_wait(unsigned long long* b, uint32_t parity) {      // whole warp
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(b);
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
+
 // D1: stage the quad's block (span16 <= kDecSpanMax chunks at blk) into its slot; lane l copies chunks l, l+4, ...
 __device__ __forceinline__ void quad_stage_block(uint4* __restrict__ slot, const unsigned char* __restrict__ blk,
                                                  uint32_t span16, int l) {
@@ -68,10 +89,12 @@ __device__ __forceinline__ void quad_patch_clear(typename IdT<W>::T* __restrict_
 //   D4  inclusive scan: prefix inside the row, inclusive scan of the row sums over the quad, running
 //       carry over the steps (order of the IDs: i major, then lane, then column); + base, mod 2^W;
 //       128-bit stores of the first m IDs.
-template <int W, bool kWin>
+// kBits: the IDs are not stored; their bits go into the bitmap of `sink` (FORMAT.md §9).
+template <int W, bool kWin, bool kBits = false>
 __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, uint32_t b,
                                                  const typename IdT<W>::T* __restrict__ tab, bool patch,
-                                                 typename IdT<W>::T base, typename IdT<W>::T* __restrict__ x, int m, int l) {
+                                                 typename IdT<W>::T base, typename IdT<W>::T* __restrict__ x, int m, int l,
+                                                 const BitSink& sink = BitSink{nullptr, 0, 0, nullptr}) {
     using T = typename IdT<W>::T;
     const uint32_t mask = (1u << b) - 1u;
     uint32_t bit = (uint32_t)l * b;
@@ -114,7 +137,9 @@ __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, ui
         const T off = carry + (inc - v3);
         carry += tot;
         v0 += off; v1 += off; v2 += off; v3 += off;
-        if (vec) {
+        if constexpr (kBits) {
+            set_bits4<T>(sink, v0, v1, v2, v3, m - (16 * i + 4 * l));
+        } else if (vec) {
             if (m > 0) {
                 if constexpr (W == 32) {
                     __stcs(reinterpret_cast<uint4*>(x) + 4 * i + l, make_uint4(v0, v1, v2, v3));

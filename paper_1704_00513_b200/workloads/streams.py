@@ -109,3 +109,25 @@ def split_block(frontier: torch.Tensor, parts: int, n_vertices: int):
     off = torch.searchsorted(frontier, bounds, right=False)
     off[-1] = frontier.numel()
     return frontier, off.to(torch.int64)
+
+
+_S_BIT, _S_JUNK = 0x15, 0x16
+
+
+def frontier_bitmap(n_bits: int, density: float, seed: int, run: int = 1) -> torch.Tensor:
+    """A frontier bitmap (32-bit words): int32 words, whole 16-byte groups. Cells of `run` consecutive
+    bits are set together w.p. `density` (run > 1: clustered frontiers); bits at positions >= n_bits of the padded
+    words are random junk the codec must ignore (FORMAT.md §9). density 0 / 1: empty / full."""
+    words = (n_bits + 31) // 32
+    padded = max(4, (words + 3) // 4 * 4)
+    pos = torch.arange(padded * 32, dtype=torch.int64)
+    if density >= 1.0:
+        bits = torch.ones_like(pos, dtype=torch.bool)
+    elif density <= 0.0:
+        bits = torch.zeros_like(pos, dtype=torch.bool)
+    else:
+        bits = rng.below(seed, _S_BIT, pos // run, 1_000_000) < int(density * 1_000_000)
+    junk = rng.below(seed, _S_JUNK, pos, 2) == 1
+    bits = torch.where(pos < n_bits, bits, junk)
+    w = (bits.view(padded, 32).to(torch.int64) << torch.arange(32, dtype=torch.int64)).sum(1)
+    return (w & 0xFFFFFFFF).to(torch.uint32).view(torch.int32)

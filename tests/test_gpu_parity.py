@@ -545,6 +545,21 @@ def test_config5_largest_buffers_full(B, oracle_mod):
     torch.cuda.empty_cache()
 
 
+def test_decode_tma_staging_variant(B, oracle_mod, monkeypatch):
+    """BFSC_DEC_STAGING=tma: single-stream decode stages every warp batch with one bulk copy (TMA) into a two-stage
+    ring instead of per-lane cp.async (measured, slower, kept selectable). Same results: edge sizes,
+    exceptions, blocks over the staged size, corrupt streams."""
+    monkeypatch.setenv("BFSC_DEC_STAGING", "tma")
+    for W in (32, 64):
+        for n in (0, 1, 127, 128, 129, 1000, 128 * 300 + 5, (1 << 20) + 77):
+            for mean, outl in ((2.0, 0.0), (256.0, 0.01), (70000.0, 0.0)):
+                run_single(B, oracle_mod, streams.gap_stream(n, mean, seed=13, W=W, outlier_frac=outl), W, 0)
+    rng = np.random.default_rng(5)
+    x = np.cumsum(rng.integers(0, 1 << 26, size=128 * 20 + 3, dtype=np.uint64)).astype(np.uint32)   # b = 26: blocks over the staged size
+    run_single(B, oracle_mod, torch.from_numpy(x.view(np.int32).copy()), 32, 0)
+    test_errors_reported_on_device(B)
+
+
 def test_exclusive_flag_same_bytes(B, oracle_mod):
     """BFSC_CODEC_FLAG_EXCLUSIVE (static first tiles, include/bfsc.h) changes the schedule, not the bytes: single and
     batch calls, both encoder rules, against the oracle."""
@@ -690,3 +705,181 @@ def test_decoder_fuzz_matches_oracle_verdict(B, oracle_mod, W):
     for cut in (16, 31, 32, 48, len(good) - 16, len(good) - 1):
         check(good, in_bytes=cut)
     assert verdicts[0] > 20 and verdicts[3] > 100            # the mutations reach both outcomes
+
+
+# ---- FORMAT.md §9: frontier bitmaps; §8: RAW fallback ------------------------------------------------------------
+FALLBACK = 0x200
+
+
+def _bitmap_ids(bm_np, n_bits, id_base, W):
+    """numpy, independent of both sides: the ascending IDs of the set bits."""
+    bits = np.unpackbits(bm_np.view(np.uint8), bitorder="little")[:n_bits]
+    v = np.nonzero(bits)[0].astype(np.uint64)
+    ids = v + np.uint64(id_base & 0xFFFFFFFFFFFFFFFF)
+    return (ids & np.uint64(0xFFFFFFFF)).astype(np.uint32) if W == 32 else ids
+
+
+def run_bitmap(B, oracle_mod, bm_t, n_bits, W, id_base=0, thr=0, codec=PFOR, check_list=True):
+    dev = torch.device("cuda")
+    bm_np = bm_t.numpy().view(np.uint32)
+    d_bm = bm_t.to(dev)
+    cap = B.compress_bound(n_bits, W)
+    out = torch.full((cap + 64,), 0xAB, dtype=torch.uint8, device=dev)
+    nbytes = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.bitmap_workspace_bytes(n_bits, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress_bitmap(codec, d_bm, n_bits, id_base, W, thr, out, nbytes, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    total = int(nbytes.item())
+    ref = oracle_mod.compress_bitmap(bm_np, n_bits, W, id_base, thr, codec)
+    got = out[:total].cpu().numpy()
+    assert total == len(ref), (total, len(ref))
+    if not np.array_equal(got, ref):
+        raise AssertionError(f"bitmap stream differs at byte {int(np.nonzero(got != ref)[0][0])} of {len(ref)}")
+    assert bool((out[cap:] == 0xAB).all()), "wrote beyond capacity"
+    assert torch.equal(d_bm.cpu(), bm_t), "the bitmap is an input"
+    if check_list:                                   # FORMAT.md §9: it IS the stream of the ID list
+        ids = _bitmap_ids(bm_np, n_bits, id_base, W)
+        assert np.array_equal(ref, oracle_mod.compress(ids, thr, codec=codec))
+    # decode into a bitmap that already holds other bits: OR semantics, nothing beyond n_bits touched
+    words = bm_t.numel()
+    old = streams.frontier_bitmap(words * 32, 0.1, seed=77)[:words].clone()
+    d_back = old.to(dev)
+    n_out = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    ws2 = torch.empty(B.workspace_bytes(max(n_bits, 1), 1, W), dtype=torch.uint8, device=dev)
+    B.decompress_to_bitmap(out, total, W, id_base, d_back, n_bits, n_out, ws2, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    exp = old.numpy().view(np.uint32).copy()
+    n_ref = oracle_mod.decompress_to_bitmap(ref, W, exp, n_bits, id_base)
+    assert int(n_out.item()) == n_ref
+    assert np.array_equal(d_back.cpu().numpy().view(np.uint32), exp)
+    return total
+
+
+@pytest.mark.parametrize("codec", CODECS)
+@pytest.mark.parametrize("W", [32, 64])
+def test_bitmap_edge_sizes(B, oracle_mod, W, codec):
+    bases = (0, 12345, (1 << 32) - 100) if W == 32 else (0, (1 << 40) + 7, (1 << 64) - 50)
+    for n_bits in (0, 1, 31, 32, 33, 127, 128, 129, 1000, 1023, 1024, 1025, 4096 + 7, 128 * 64 * 3 + 5):
+        for dens in (0.0, 1.0, 0.5, 0.03):
+            bm = streams.frontier_bitmap(n_bits, dens, seed=n_bits + 1)
+            run_bitmap(B, oracle_mod, bm, n_bits, W, id_base=bases[n_bits % 3], codec=codec)
+    run_bitmap(B, oracle_mod, streams.frontier_bitmap(3000, 0.05, seed=2), 3000, W, thr=4096, codec=codec)   # RAW by the threshold
+    run_bitmap(B, oracle_mod, streams.frontier_bitmap(3000, 0.9, seed=2), 3000, W, thr=4096, codec=codec)
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_bitmap_densities_many_tiles(B, oracle_mod, W):
+    """Several tiles per CTA and a ragged tail; dense (landing area), sparse (blocks that span many words: read from
+    global memory), clustered, and one block spread over the whole bitmap."""
+    n_bits = (1 << 22) + 4321
+    for dens, run in ((0.5, 1), (0.25, 1), (0.03, 1), (0.002, 1), (0.3, 64), (0.01, 1024)):
+        run_bitmap(B, oracle_mod, streams.frontier_bitmap(n_bits, dens, seed=5, run=run), n_bits, W, id_base=3,
+                   check_list=dens >= 0.25)
+    run_bitmap(B, oracle_mod, streams.frontier_bitmap(n_bits, 0.00002, seed=6), n_bits, W)     # ~84 IDs: one ragged block
+    run_bitmap(B, oracle_mod, streams.frontier_bitmap(n_bits, 1.0, seed=6), n_bits, W)          # full
+
+
+def test_bitmap_frontier_scale24(B, oracle_mod):
+    """A frontier bitmap of a scale-24 graph (2^24 vertices), a quarter of the vertices in it."""
+    n_bits = 1 << 24
+    total = run_bitmap(B, oracle_mod, streams.frontier_bitmap(n_bits, 0.25, seed=24), n_bits, 32, check_list=False)
+    assert total < n_bits // 8 * 3                   # (gap ~4: about 3.6 bits per ID)
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_bitmap_decode_rejects_ids_outside(B, oracle_mod, W):
+    dev = torch.device("cuda")
+    ids = _np(streams.gap_stream(5000, 3.0, seed=4, W=W), W)
+    stream = oracle_mod.compress(ids, 0)
+    lo, hi = int(ids.min()), int(ids.max())
+    for id_base, n_bits, ok in ((lo, hi - lo + 1, True), (lo + 1, hi - lo, False), (lo, hi - lo, False), (0, hi + 1, True)):
+        words = max(4, ((n_bits + 31) // 32 + 3) // 4 * 4)
+        d_bm = torch.zeros(words, dtype=torch.int32, device=dev)
+        d_in = torch.from_numpy(np.concatenate([stream, np.zeros(16, np.uint8)])).to(dev)
+        n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+        status = torch.zeros(1, dtype=torch.int32, device=dev)
+        ws = torch.empty(B.workspace_bytes(len(ids), 1, W), dtype=torch.uint8, device=dev)
+        B.decompress_to_bitmap(d_in, len(stream), W, id_base, d_bm, n_bits, n_out, ws, status)
+        torch.cuda.synchronize()
+        exp = np.zeros(words, np.uint32)
+        try:
+            oracle_mod.decompress_to_bitmap(stream, W, exp, n_bits, id_base)
+            ref_ok = True
+        except oracle_mod.OracleError as e:
+            ref_ok = False
+            assert e.code == 2                       # DST_TOO_SMALL
+        assert ref_ok == ok
+        assert (int(status.item()) == 0) == ok
+        if ok:
+            assert np.array_equal(d_bm.cpu().numpy().view(np.uint32), exp)
+        else:
+            assert int(status.item()) == 2
+
+
+def _fallback_single(B, oracle_mod, ids_t, W, thr=0, codec=PFOR):
+    dev = torch.device("cuda")
+    n = ids_t.numel()
+    cap = B.compress_bound(n, W)
+    d_ids = ids_t.to(dev) if n else torch.empty(4, dtype=ids_t.dtype, device=dev)
+    out = torch.full((cap + 64,), 0xAB, dtype=torch.uint8, device=dev)
+    nbytes = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, 1, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress_codec(codec | FALLBACK, d_ids, n, W, thr, out, nbytes, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    total = int(nbytes.item())
+    ref = oracle_mod.compress(_np(ids_t, W), thr, codec=codec | oracle_mod.FLAG_RAW_FALLBACK)
+    assert total == len(ref) and total <= 32 + (n * W // 8 + 15) // 16 * 16
+    assert np.array_equal(out[:total].cpu().numpy(), ref)
+    assert bool((out[cap:] == 0xAB).all())
+    back = torch.empty(max(n, 4), dtype=ids_t.dtype, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+    B.decompress(out, total, W, back, n_out, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and int(n_out.item()) == n
+    assert torch.equal(back[:n].cpu(), ids_t)
+    return int(ref[6])                                # mode byte
+
+
+@pytest.mark.parametrize("codec", CODECS)
+@pytest.mark.parametrize("W", [32, 64])
+def test_raw_fallback_single(B, oracle_mod, W, codec):
+    rng = np.random.default_rng(W + codec)
+    tdt = torch.int32 if W == 32 else torch.int64
+    dt = np.uint32 if W == 32 else np.uint64
+    modes = set()
+    for n in (0, 1, 2, 3, 127, 128, 129, 1000, 128 * 64 + 3, 128 * 64 * 40 + 77):
+        rnd = torch.from_numpy(rng.integers(0, 1 << W, size=n, dtype=np.uint64, endpoint=False).astype(dt).view(
+            np.int32 if W == 32 else np.int64))
+        modes.add(_fallback_single(B, oracle_mod, rnd, W, codec=codec))              # incompressible: RAW
+        modes.add(_fallback_single(B, oracle_mod, streams.gap_stream(n, 3.0, seed=n, W=W), W, codec=codec))
+        modes.add(_fallback_single(B, oracle_mod, streams.gap_stream(n, 3.0, seed=n, W=W), W, thr=2048, codec=codec))
+    assert modes == {0, codec}
+    # around the tie (FORMAT.md §8: a tie goes to RAW): one block of 128 IDs with a constant gap of 2^g packs into
+    # 48 + 16 + 16 (g + 1) bytes against 32 + 16 W RAW — equal at g = W - 3, smaller below, larger above
+    for gap_bits in (W - 4, W - 3, W - 2, W - 1):
+        v = (np.arange(128, dtype=np.uint64) * np.uint64(1 << gap_bits)) & np.uint64((1 << W) - 1 if W < 64 else 0xFFFFFFFFFFFFFFFF)
+        t = torch.from_numpy(v.astype(dt).view(np.int32 if W == 32 else np.int64))
+        _fallback_single(B, oracle_mod, t, W, codec=codec)
+
+
+def test_raw_fallback_batch_is_unsupported_and_bitmap_follows_the_rule(B, oracle_mod):
+    dev = torch.device("cuda")
+    ids = streams.gap_stream(1000, 2.0, seed=1, W=32).to(dev)
+    off = torch.tensor([0, 400, 1000], dtype=torch.int64, device=dev)
+    out = torch.empty(B.batch_compress_bound([400, 600], 32), dtype=torch.uint8, device=dev)
+    out_off = torch.zeros(3, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(1000, 2, 32), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    with pytest.raises(B.BfscError) as e:
+        B.compress_batch_codec(PFOR | FALLBACK, ids, off, 2, 32, 0, out, out_off, ws, status)
+    assert e.value.code == B.ERR_UNSUPPORTED
+    # bitmaps: a handful of set bits far apart do not shrink (n = 1: 64 bytes against 48 RAW); dense ones do
+    for W in (32, 64):
+        for n_bits, dens in ((0, 0.0), (5000, 0.0002), (5000, 0.001), (1 << 20, 0.000003), (1 << 20, 0.3)):
+            bm = streams.frontier_bitmap(n_bits, dens, seed=9)
+            run_bitmap(B, oracle_mod, bm, n_bits, W, codec=PFOR | FALLBACK)
