@@ -238,6 +238,24 @@ def run_ours(args, rank, local_rank, world):
     for s in range(S):                                       # untimed sanity: decode == input
         assert torch.equal(backs[s], ids[s]), "decode != input"
 
+    if args.ncu:
+        # Capture mode (profiles/README.md): between cudaProfilerStart / Stop, ONE compress and ONE decompress call per
+        # stream, in the order a, b, c — run under `ncu --profile-from-start off`; no number is reported from here.
+        sampler.stop()
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        torch.cuda.synchronize()
+        torch.cuda.profiler.start()
+        for s in range(S):
+            flush.zero_()
+            B.compress(ids[s], n, W, 0, outs[s], nbytes[s], ws, status)
+            flush.zero_()
+            B.decompress(outs[s], cap, W, backs[s], n_out, ws, status)
+        torch.cuda.synchronize()
+        torch.cuda.profiler.stop()
+        if rank == 0:
+            print(json.dumps({"ncu_capture": "compress + decompress of streams a, b, c, one call each", "status": int(status.item())}))
+        return
+
     mk = lambda: torch.cuda.Event(enable_timing=True)       # noqa: E731
     t0, t1 = mk(), mk()
     launches0 = B.kernel_launches()
@@ -551,6 +569,8 @@ def main():
     ap.add_argument("--log2n", type=int, default=LOG2_N, help="IDs per stream = 2^log2n (default: the BASELINE size)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--ncu", action="store_true", help="capture mode for ncu --profile-from-start off: one compress + one "
+                    "decompress per stream between cudaProfilerStart/Stop, nothing timed (profiles/README.md)")
     ap.add_argument("--no-batch", action="store_true", help="skip the batched-path section (4096-buffer batch, R-MAT 25 level)")
     ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for the whole run")
     args = ap.parse_args()

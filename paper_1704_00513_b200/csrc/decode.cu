@@ -191,6 +191,137 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_dec_blocks(DecArgs a) {
 }
 
 
+// ---- D0 (batch calls of up to kFusedMaxStreams streams): plan AND block table in ONE launch of a few CTAs, as on the
+// encode side (k_enc_planblocks): every CTA parses all the headers and scans for itself (no inter-CTA dependency, no
+// gather / plan / table chain of three launches), keeps first block, first ID and size of every stream in shared
+// memory, and writes its slice of the per-stream tables, of d_id_offsets and of the block table.
+constexpr uint32_t kFusedMaxStreams = 8192;
+constexpr int kFusedPlanCtas = 32;                        // (every CTA reads every header: 32 CTAs x 4096 streams x 64 B = 8 MB from L2)
+__host__ __device__ inline size_t dec_planblocks_smem(size_t n_buf) { return 8 * (n_buf + 1) + 4 * (n_buf + 2) + 4 * (n_buf + 2); }
+// The scan of both fused plans (any CTA size): headers of all streams parsed and validated (FORMAT.md §4), per stream
+// first block, first ID and total_bytes / 16 -> shared memory; kTables: the per-stream workspace tables as well, the
+// entries of the threads with `mine`. Returns the totals (blocks, IDs); *bad is set when a header is rejected.
+template <int W, bool kTables>
+__device__ __forceinline__ Scan2 dec_plan_scan(const DecArgs& a, unsigned long long* s_idpre, uint32_t* s_first, uint32_t* s_tot16,
+                                               Scan2* sm, int* bad_p, bool mine) {
+    constexpr unsigned long long E = W / 8;
+    Scan2 carry{0, 0};
+    constexpr int kIpt = 4;
+    for (uint32_t i0 = 0; i0 < a.n_buf; i0 += blockDim.x * kIpt) {
+        Scan2 v[kIpt], sum{0, 0};
+        unsigned long long beg[kIpt], avail[kIpt], tot_bytes[kIpt];
+        bool rd[kIpt];
+        uint4 h0[kIpt], h1[kIpt];
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {                 // extents (independent loads)
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            beg[u] = 0; avail[u] = 0; rd[u] = false;
+            if (i < a.n_buf) {
+                beg[u] = a.in_off[i];
+                const unsigned long long end = a.in_off[i + 1];
+                avail[u] = end >= beg[u] ? end - beg[u] : 0;
+                rd[u] = !(beg[u] & 15) && avail[u] >= 32;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {                 // all headers in flight at once
+            h0[u] = h1[u] = make_uint4(0, 0, 0, 0);
+            if (rd[u]) {
+                h0[u] = __ldcg(reinterpret_cast<const uint4*>(a.in + beg[u]));
+                h1[u] = __ldcg(reinterpret_cast<const uint4*>(a.in + beg[u] + 16));
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {                 // validation (FORMAT.md §4), as in k_dec_plan
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            v[u] = Scan2{0, 0};
+            tot_bytes[u] = 0;
+            if (i < a.n_buf) {
+                bool ok = rd[u];
+                if (ok) {
+                    const uint32_t mode = (h0[u].y >> 16) & 0xffu;
+                    const unsigned long long n = (unsigned long long)h0[u].w << 32 | h0[u].z;
+                    const unsigned long long total = (unsigned long long)h1[u].y << 32 | h1[u].x;
+                    const unsigned long long nb = h1[u].z;
+                    if (h0[u].x != 0x43534642u || (h0[u].y & 0xffu) != 1u || ((h0[u].y >> 8) & 0xffu) != (uint32_t)W ||
+                        mode > 2u || (h0[u].y >> 24) != 0u)
+                        ok = false;
+                    else if (total > avail[u] || (total & 15) || total < 32) ok = false;
+                    else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
+                    else if (nb != (n + kBlk - 1) / kBlk || 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total)
+                        ok = false;
+                    if (ok) { v[u].a = nb; v[u].b = n; tot_bytes[u] = total; }
+                }
+                if (!ok) *bad_p = 1;
+            }
+            sum.a += v[u].a; sum.b += v[u].b;
+        }
+        Scan2 tot;
+        Scan2 ex = block_scan_excl2(sum, &tot, sm);
+        ex.a += carry.a; ex.b += carry.b;
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = i0 + threadIdx.x * kIpt + u;
+            if (i < a.n_buf) {
+                s_first[i] = (uint32_t)ex.a; s_idpre[i] = ex.b; s_tot16[i] = (uint32_t)(tot_bytes[u] >> 4);
+                if (kTables && mine) { a.ws.blk_first[i] = ex.a; a.ws.fixed_prefix[i] = ex.b; a.ws.stream_start[i] = tot_bytes[u]; }
+            }
+            ex.a += v[u].a; ex.b += v[u].b;
+        }
+        carry.a += tot.a; carry.b += tot.b;
+    }
+    return carry;
+}
+
+template <int W>
+__global__ void __launch_bounds__(1024) k_dec_planblocks(DecArgs a) {
+    extern __shared__ __align__(16) unsigned char pb_smem[];
+    unsigned long long* s_idpre = reinterpret_cast<unsigned long long*>(pb_smem);      // n_buf + 1: first ID of every stream
+    uint32_t* s_first = reinterpret_cast<uint32_t*>(s_idpre + a.n_buf + 1);            // n_buf + 1: first block
+    uint32_t* s_tot16 = s_first + a.n_buf + 2;                                         // n_buf: validated total_bytes / 16
+    __shared__ Scan2 sm[33];
+    __shared__ int bad;
+    pdl_wait();                                          // the call before this one is complete (workspace, inputs)
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) bad = 0;
+    __syncthreads();
+    const bool mine = threadIdx.x % gridDim.x == blockIdx.x;
+    const Scan2 carry = dec_plan_scan<W, true>(a, s_idpre, s_first, s_tot16, sm, &bad, mine);
+    if (threadIdx.x == 0) { s_first[a.n_buf] = (uint32_t)carry.a; s_idpre[a.n_buf] = carry.b; }
+    __syncthreads();
+    const bool good = !bad && carry.a <= a.ws.blk_cap && carry.b <= a.ids_cap && carry.a < (1ull << 32);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        a.ws.blk_first[a.n_buf] = carry.a;
+        a.ws.fixed_prefix[a.n_buf] = carry.b;
+        a.ws.hdr->total_blocks = carry.a;
+        a.ws.hdr->total_out = carry.b;
+        a.ws.hdr->ok = good ? 1u : 0u;
+        if (bad) set_status(a.status, BFSC_ERR_CORRUPT);
+        else if (carry.b > a.ids_cap) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+        else if (!good) set_status(a.status, BFSC_ERR_INVALID_ARG);
+        if (a.n_ids_out) *a.n_ids_out = good ? carry.b : 0ull;
+    }
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x, me = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a.id_off)
+        for (unsigned long long i = me; i <= a.n_buf; i += stride) a.id_off[i] = good ? s_idpre[i] : 0ull;
+    if (!good) return;
+    for (unsigned long long g = me; g < carry.a; g += stride) {
+        uint32_t lo = 0, hi = a.n_buf;                   // the last i with s_first[i] <= g
+        while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (s_first[mid] <= (uint32_t)g) lo = mid; else hi = mid;
+        }
+        const uint32_t i = lo;
+        const unsigned long long k = g - s_first[i], id0 = s_idpre[i], n = s_idpre[i + 1] - id0;
+        const unsigned long long sb = a.in_off[i], xi = id0 + kBlk * k;
+        uint4 e0, e1;
+        e0.x = (uint32_t)sb; e0.y = (uint32_t)(sb >> 32); e0.z = (uint32_t)xi; e0.w = (uint32_t)(xi >> 32);
+        e1.x = (uint32_t)k; e1.y = (uint32_t)min((unsigned long long)kBlk, n - kBlk * k);
+        e1.z = s_tot16[i]; e1.w = (uint32_t)((n + kBlk - 1) / kBlk);
+        a.ws.blk_tab[2 * g] = e0; a.ws.blk_tab[2 * g + 1] = e1;
+    }
+}
+
 // ---- D1-D5 fused -------------------------------------------------------------------------
 // Warp = batch of 8 consecutive blocks, four lanes per block (quad_decode.cuh). Per batch:
 //   locate   per quad: stream, directory entries -> block address, span, valid IDs, output address
@@ -226,8 +357,17 @@ struct BlockAt {                       // where the quad's block is
 // kTma (single-stream calls): D1 as ONE bulk copy (TMA, cp.async.bulk + mbarrier) of the warp batch's contiguous span
 // [dir[8k], dir[8k+8)) * 16 issued by lane 0, the blocks unpacked where they land; else every lane copies 16-byte
 // chunks of its quad's block into the quad's slot (cp.async). The measured A/B is in DESIGN.md §5.2.
-template <int W, bool kBatch, bool kTma, bool kBits = false>   // kBatch: a.in_off != nullptr; kBits: bits into a.sink instead of IDs into a.ids
+// kSelf (small batches: up to kSelfMaxStreams streams, kSelfMaxBlocks blocks): the whole call in ONE launch — every CTA
+// runs D0 for itself (dec_plan_scan, tables in shared memory) instead of reading what a plan kernel left in the workspace.
+constexpr uint32_t kSelfMaxStreams = 1024, kSelfMaxBlocks = 2048;
+template <int W, bool kBatch, bool kTma, bool kBits = false, bool kSelf = false>   // kBatch: a.in_off != nullptr; kBits: bits into a.sink instead of IDs into a.ids
 __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kCtasPerSm) k_dec_tiles(DecArgs a) {
+    static_assert(!kSelf || (kBatch && !kTma && !kBits), "kSelf: batch calls");
+    constexpr uint32_t kSelfN = kSelf ? kSelfMaxStreams : 0;
+    __shared__ unsigned long long s_idpre[kSelfN + 1];                     // kSelf: first ID of every stream (entry n_buf: total)
+    __shared__ uint32_t s_first[kSelfN + 2], s_tot16[kSelfN + 1];          //        first block, total_bytes / 16
+    __shared__ Scan2 s_scan[kSelf ? 33 : 1];
+    __shared__ int s_bad;
     constexpr int kDecWarps = DecCfg<W, kTma>::kWarps;
     using T = typename IdT<W>::T;
     constexpr unsigned long long E = W / 8;
@@ -250,7 +390,25 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
     unsigned long long total_blocks, n1 = 0, total16_1 = 0, lo16_1 = 0;   // single stream: n, total/16, first block/16
     pdl_wait();                                                            // the kernel before this one is complete
     pdl_launch_dependents();                                               // the next one may be set up; it waits for this grid
-    if (batch) {
+    if constexpr (kSelf) {                                                 // D0 of the batch, by every CTA for itself
+        if (threadIdx.x == 0) s_bad = 0;
+        __syncthreads();
+        const Scan2 tot = dec_plan_scan<W, false>(a, s_idpre, s_first, s_tot16, s_scan, &s_bad, false);
+        if (threadIdx.x == 0) { s_first[a.n_buf] = (uint32_t)tot.a; s_idpre[a.n_buf] = tot.b; }
+        __syncthreads();
+        const bool good = !s_bad && tot.b <= a.ids_cap && tot.a < (1ull << 32);
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            if (s_bad) set_status(a.status, BFSC_ERR_CORRUPT);
+            else if (tot.b > a.ids_cap) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+            else if (!good) set_status(a.status, BFSC_ERR_INVALID_ARG);
+            if (a.n_ids_out) *a.n_ids_out = good ? tot.b : 0ull;
+        }
+        if (a.id_off)
+            for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i <= a.n_buf; i += gridDim.x * blockDim.x)
+                a.id_off[i] = good ? s_idpre[i] : 0ull;
+        if (!good) return;
+        total_blocks = tot.a;
+    } else if (batch) {
         if (!a.ws.hdr->ok) return;
         total_blocks = a.ws.hdr->total_blocks;
     } else {                                                               // D0 for one stream (FORMAT.md §1, §4)
@@ -302,7 +460,18 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         unsigned long long k = g, id0 = 0, n = n1, total16 = total16_1, lo16 = lo16_1;
         int m;
         unsigned long long xi;
-        if (batch) {                                                       // ws.blk_tab, written by k_dec_blocks
+        if constexpr (kSelf) {                                             // the CTA's own tables
+            uint32_t lo = 0, hi = a.n_buf;                                 // the last i with s_first[i] <= g
+            while (hi - lo > 1) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (s_first[mid] <= (uint32_t)g) lo = mid; else hi = mid;
+            }
+            s = a.in + a.in_off[lo];
+            k = g - s_first[lo]; id0 = s_idpre[lo]; n = s_idpre[lo + 1] - id0; total16 = s_tot16[lo];
+            m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+            xi = id0 + kBlk * k;
+            lo16 = (32ull + ((4ull * ((n + kBlk - 1) / kBlk + 1) + 15ull) & ~15ull)) >> 4;
+        } else if (batch) {                                                // ws.blk_tab, written by k_dec_blocks / k_dec_planblocks
             const uint4 e0 = __ldcg(a.ws.blk_tab + 2 * g), e1 = __ldcg(a.ws.blk_tab + 2 * g + 1);
             s = a.in + ((unsigned long long)e0.y << 32 | e0.x);
             xi = (unsigned long long)e0.w << 32 | e0.z;
@@ -458,7 +627,9 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         for (uint32_t i = blockIdx.x; i < a.n_buf; i += gridDim.x) {
             const unsigned char* s = a.in + s_begin(a, i);
             if (s[6] != 0) continue;
-            const unsigned long long id0 = a.ws.fixed_prefix[i], n = a.ws.fixed_prefix[i + 1] - id0;
+            unsigned long long id0, n;
+            if constexpr (kSelf) { id0 = s_idpre[i]; n = s_idpre[i + 1] - id0; }
+            else { id0 = a.ws.fixed_prefix[i]; n = a.ws.fixed_prefix[i + 1] - id0; }
             const T* xs = reinterpret_cast<const T*>(s + 32);
             T* y = reinterpret_cast<T*>(a.ids) + id0;
             for (unsigned long long t = threadIdx.x; t < n; t += blockDim.x) y[t] = xs[t];
@@ -467,20 +638,34 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
 }
 
 // Once per device and instantiation: the dynamic shared memory attribute and the resident CTAs per SM.
-template <int W, bool kBatch, bool kTma, bool kBits = false>
+template <int W, bool kBatch, bool kTma, bool kBits = false, bool kSelf = false>
 static int dec_ctas_per_sm(int device) {
     static std::mutex mu;
     static int per_sm[kMaxDevices] = {};
     std::lock_guard<std::mutex> lock(mu);
     if (per_sm[device] == 0) {
         int n = 0;
-        if (cudaFuncSetAttribute(k_dec_tiles<W, kBatch, kTma, kBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DecSmem<W, kTma>::kBytes) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_dec_tiles<W, kBatch, kTma, kBits, kSelf>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DecSmem<W, kTma>::kBytes) != cudaSuccess)
             return 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_dec_tiles<W, kBatch, kTma, kBits>, DecCfg<W, kTma>::kThreads, DecSmem<W, kTma>::kBytes) != cudaSuccess || n < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_dec_tiles<W, kBatch, kTma, kBits, kSelf>, DecCfg<W, kTma>::kThreads, DecSmem<W, kTma>::kBytes) != cudaSuccess || n < 1)
             return 0;
         per_sm[device] = n;
     }
     return per_sm[device];
+}
+
+template <int W>
+static bool dec_planblocks_init(int device) {            // once per device: the fused plan's shared memory (up to 128 KB)
+    static std::mutex mu;
+    static bool done[kMaxDevices] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!done[device]) {
+        if (cudaFuncSetAttribute(k_dec_planblocks<W>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)dec_planblocks_smem(kFusedMaxStreams)) != cudaSuccess)
+            return false;
+        done[device] = true;
+    }
+    return true;
 }
 
 template <int W>
@@ -498,10 +683,27 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     if (per_sm < 1) return BFSC_ERR_CUDA;
     const int max_grid = dev.sms * per_sm;
     const int warps = a.in_off || !use_tma ? DecCfg<W, false>::kWarps : DecCfg<W, true>::kWarps;
-    const size_t want = (max_blocks + kDecBlocks * warps - 1) / (kDecBlocks * warps);
+    if (a.in_off && a.ws.blk_cap < max_blocks) max_blocks = a.ws.blk_cap;          // (more blocks than that: INVALID_ARG on the device)
+    // CTAs: one per warp batch while the device has room for them (a small call is spread over the SMs, one working
+    // warp each: k_dec_tiles balances the working warps over the CTAs), at most one resident wave
+    (void)warps;
+    const size_t want = (max_blocks + kDecBlocks - 1) / kDecBlocks;
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
-    if (a.in_off) {
+    if (a.in_off && a.n_buf <= kSelfMaxStreams && max_blocks <= kSelfMaxBlocks) {
+        // a small batch (both bounds known on the host: stream count, and blocks by the ID capacity / the workspace size):
+        // one launch, no plan kernel
+        const int psm = dec_ctas_per_sm<W, true, false, false, true>(dev.device);
+        if (psm < 1) return BFSC_ERR_CUDA;
+        const int g = want < (size_t)(dev.sms * psm) ? (want ? (int)want : 1) : dev.sms * psm;
+        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false, false, true>, g, DecCfg<W>::kThreads, kSmem, s, a));
+    } else if (a.in_off && a.n_buf <= kFusedMaxStreams && a.ws.blk_cap < (1ull << 32)) {
+        if (!dec_planblocks_init<W>(dev.device)) return BFSC_ERR_CUDA;
+        size_t pgrid = (a.ws.blk_cap + 1023) / 1024;
+        if (pgrid > (size_t)kFusedPlanCtas) pgrid = kFusedPlanCtas;
+        BFSC_LAUNCH(launch_dep(k_dec_planblocks<W>, pgrid ? (int)pgrid : 1, 1024, dec_planblocks_smem(a.n_buf), s, a));
+        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
+    } else if (a.in_off) {
         const bool gather = a.n_buf >= kHeaderGatherMin && a.ws.blk_cap >= a.n_buf;
         if (gather) {
             int hgrid = (int)((a.n_buf + 255) / 256);

@@ -170,6 +170,88 @@ __global__ void __launch_bounds__(kBlkTabThreads) k_enc_blocks(EncArgs a) {
     }
 }
 
+// ---- E0 (batch calls of up to kFusedMaxBuf buffers): plan AND block table in ONE launch of many CTAs. Every CTA
+// repeats the whole scan over the buffers for itself (n_buf + 1 offsets from L2, one block scan: no inter-CTA
+// dependency, no second launch whose start has to wait for the first one's end) and keeps the buffers' first blocks
+// in shared memory; it then writes ITS slice of everything: per-buffer tables, look-back states, group hints, and
+// the block table (buffer of a block: bisection in shared memory). Replaces k_enc_plan -> k_enc_blocks.
+constexpr uint32_t kFusedMaxBuf = 8192;
+constexpr int kFusedIpt = 8;                             // buffers per thread (1024 threads)
+__device__ __forceinline__ uint32_t bisect_first(const uint32_t* __restrict__ first, uint32_t n_buf, uint32_t g) {
+    uint32_t lo = 0, hi = n_buf;                         // the last i in [0, n_buf) with first[i] <= g (first[0] = 0)
+    while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (first[mid] <= g) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+template <int W>
+__global__ void __launch_bounds__(1024) k_enc_planblocks(EncArgs a) {
+    __shared__ Scan2 sm[33];
+    __shared__ uint32_t s_first[kFusedMaxBuf + 1];
+    __shared__ int bad;
+    constexpr unsigned long long E = W / 8;
+    pdl_wait();                                          // the call before this one is complete (workspace, inputs)
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) bad = 0;
+    __syncthreads();
+    const uint32_t ib = threadIdx.x * kFusedIpt;
+    Scan2 v[kFusedIpt], sum{0, 0};
+#pragma unroll
+    for (int u = 0; u < kFusedIpt; u++) {
+        const uint32_t i = ib + u;
+        v[u] = Scan2{0, 0};
+        if (i < a.n_buf) {
+            const unsigned long long o0 = a.in_off[i], o1 = a.in_off[i + 1];
+            if (o1 < o0) bad = 1;
+            const unsigned long long n = o1 - o0;
+            const bool raw = n * E < a.thr;                               // FORMAT.md §1 (L1311)
+            const unsigned long long nb = raw ? 0ull : (n + kBlk - 1) / kBlk;
+            v[u].a = nb;
+            v[u].b = raw ? 32ull + ((n * E + 15ull) & ~15ull) : 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull);
+        }
+        sum.a += v[u].a; sum.b += v[u].b;
+    }
+    Scan2 tot;
+    Scan2 ex = block_scan_excl2(sum, &tot, sm);
+    const bool mine = threadIdx.x % gridDim.x == blockIdx.x;              // table entries of this thread's buffers: this CTA's
+#pragma unroll
+    for (int u = 0; u < kFusedIpt; u++) {
+        const uint32_t i = ib + u;
+        if (i < a.n_buf) {
+            s_first[i] = (uint32_t)ex.a;
+            if (mine) { a.ws.blk_first[i] = ex.a; a.ws.fixed_prefix[i] = ex.b; a.ws.stream_start[i] = 0; }
+        }
+        ex.a += v[u].a; ex.b += v[u].b;
+    }
+    if (threadIdx.x == 0) s_first[a.n_buf] = (uint32_t)tot.a;
+    __syncthreads();
+    const unsigned long long total = tot.a, nt = (total + kTileR - 1) / kTileR;
+    const bool ok = !bad && total <= a.ws.blk_cap && nt <= a.ws.tile_cap && total < (1ull << 32);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        a.ws.blk_first[a.n_buf] = total; a.ws.fixed_prefix[a.n_buf] = tot.b; a.ws.stream_start[a.n_buf] = 0;
+        a.ws.hdr->total_blocks = total; a.ws.hdr->fixed_total = tot.b; a.ws.hdr->ticket = a.exclusive ? 2 * a.grid : 0;
+        a.ws.hdr->grand16 = 0; a.ws.hdr->total_out = tot.b; a.ws.hdr->ok = ok ? 1u : 0u;
+        if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
+    }
+    if (!ok) return;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; t < nt; t += stride) {
+        a.ws.tile_state[t * kStateStride] = 0;                            // look-back states start invalid
+        a.ws.tile_state[t * kStateStride + 1] = bisect_first(s_first, a.n_buf, (uint32_t)(t * kTileR));   // group hint
+    }
+    EncBlk* tab = reinterpret_cast<EncBlk*>(a.ws.blk_tab);
+    for (unsigned long long g = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += stride) {
+        const uint32_t i = bisect_first(s_first, a.n_buf, (uint32_t)g);
+        const unsigned long long k = g - s_first[i], o0 = a.in_off[i], n = a.in_off[i + 1] - o0;
+        const unsigned long long xoff = o0 + kBlk * k;
+        uint4 e;
+        e.x = (uint32_t)xoff; e.y = (uint32_t)(xoff >> 32);
+        e.z = (uint32_t)min((unsigned long long)kBlk, n - kBlk * k); e.w = i;
+        reinterpret_cast<uint4*>(tab + g)[0] = e;        // (the second half of the entry is unused by encode)
+    }
+}
+
 // ---- E1-E4 fused: one pass over HBM ------------------------------------------------------
 // CTA = 8 worker warps + 1 scan warp; tile = 64 consecutive blocks (32 KB of u32 IDs), pulled by
 // ticket. Worker warps handle 8 blocks each, four lanes per block (quad_encode.cuh):
@@ -440,6 +522,24 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             mbar_wait(&mb_post[k & (kRing - 1)], (k / kRing) & 1);   // the prep warp has posted the CTA's tile k
             const unsigned long long t = s_tile[k & (kRing - 1)];
             if (t == kNoTile) break;
+            // batch calls: the per-buffer constants of this lane's blocks (and the start of a stream that began in an
+            // earlier tile, if it is published already) are requested BEFORE the sizes are waited for: the tile was
+            // posted two tiles ahead, so their latency hides behind the workers' E1/E2
+            const unsigned long long g0 = t * kTileR;
+            unsigned long long bf_first[kPer], bf_f0[kPer], bf_f1[kPer], bf_S[kPer];
+            uint32_t bf_i[kPer];
+            if constexpr (kBatch) {
+#pragma unroll
+                for (int h = 0; h < kPer; h++) {
+                    const int jj = kPer * lane + h;
+                    bf_i[h] = 0; bf_first[h] = 0; bf_f0[h] = 0; bf_f1[h] = 0; bf_S[h] = 0;
+                    if (jj < kTileR && g0 + jj < total) {
+                        const uint32_t i = s_buf[k & (kRing - 1)][jj];
+                        bf_i[h] = i; bf_first[h] = a.ws.blk_first[i]; bf_f0[h] = a.ws.fixed_prefix[i]; bf_f1[h] = a.ws.fixed_prefix[i + 1];
+                        if (i > 0) bf_S[h] = ld_volatile_u64(&a.ws.stream_start[i]);     // (0: not known yet, or the stream begins in this tile)
+                    }
+                }
+            }
             bar_sync(kBarSizes + kp, kSizesThreads);
             if (lane == 0) s_sized = (unsigned int)k + 1u;      // the workers' sizes of tile t are in s_key[kp]
 
@@ -463,22 +563,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             for (int h = 0; h < kPer; h++) {
                 offs[h] += inc - own;
                 if (kPer * lane + h < kTileR) s_off16[kPer * lane + h] = offs[h];
-            }
-            // batch calls: the per-buffer constants of this lane's blocks, requested BEFORE the look-back (their
-            // latency hides behind it)
-            const unsigned long long g0 = t * kTileR;
-            unsigned long long bf_first[kPer], bf_f0[kPer], bf_f1[kPer];
-            uint32_t bf_i[kPer];
-            if constexpr (kBatch) {
-#pragma unroll
-                for (int h = 0; h < kPer; h++) {
-                    const int jj = kPer * lane + h;
-                    bf_i[h] = 0; bf_first[h] = 0; bf_f0[h] = 0; bf_f1[h] = 0;
-                    if (jj < kTileR && g0 + jj < total) {
-                        const uint32_t i = s_buf[k & (kRing - 1)][jj];
-                        bf_i[h] = i; bf_first[h] = a.ws.blk_first[i]; bf_f0[h] = a.ws.fixed_prefix[i]; bf_f1[h] = a.ws.fixed_prefix[i + 1];
-                    }
-                }
             }
             const unsigned long long excl = t > 0 ? lookback(a.ws.tile_state, t, lane) : 0ull;
             if (lane == 0) {
@@ -516,7 +600,8 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                         i = bf_i[h]; first = bf_first[h]; f0 = bf_f0[h]; f1 = bf_f1[h];
                         if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
                         else if (i > 0) {                // published by the tile that owns the stream's first block
-                            do { S = ld_volatile_u64(&a.ws.stream_start[i]); } while (S == 0);
+                            S = bf_S[h];
+                            while (S == 0) S = ld_volatile_u64(&a.ws.stream_start[i]);
                             S -= 1;
                         }
                     }
@@ -1054,10 +1139,18 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         if (!degenerate && n_tiles > a_in.ws.tile_cap) return BFSC_ERR_INVALID_ARG;          // workspace too small
         if (n_tiles < (unsigned long long)grid) grid = n_tiles ? (int)n_tiles : 1;
     }
+    if (!single && (unsigned long long)grid > a_in.ws.tile_cap) grid = (int)a_in.ws.tile_cap;   // (tile_cap >= 2: no more tiles than that)
     EncArgs a = a_in;
     a.grid = (uint32_t)grid;
-    BFSC_LAUNCH(launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a));
-    if (!single) {
+    const bool fused = !single && a.n_buf <= kFusedMaxBuf;
+    if (fused) {                                                 // plan + block table in one launch
+        size_t pgrid = (a.ws.blk_cap + 1023) / 1024;
+        if (pgrid > (size_t)dev.sms) pgrid = (size_t)dev.sms;
+        BFSC_LAUNCH(launch_dep(k_enc_planblocks<W>, pgrid ? (int)pgrid : 1, 1024, 0, s, a));
+    } else {
+        BFSC_LAUNCH(launch_dep(k_enc_plan<W>, 1, 1024, 0, s, a));
+    }
+    if (!single && !fused) {
         size_t bgrid = (a.ws.blk_cap + kBlkTabThreads - 1) / kBlkTabThreads;
         if (bgrid > (size_t)dev.sms * 8) bgrid = (size_t)dev.sms * 8;
         BFSC_LAUNCH(launch_dep(k_enc_blocks<W>, bgrid ? (int)bgrid : 1, kBlkTabThreads, 0, s, a));

@@ -180,11 +180,14 @@ def test_batch_alignments_and_many_buffers(B, oracle_mod, W):
     for thr in (0, 1024):
         for codec in CODECS:
             run_batch(B, oracle_mod, ids, off, W, thr, codec=codec)
-    many = torch.randint(0, 300, (9000,), generator=g)
-    ids2, off2 = streams.batch_of_streams(many, 16.0, seed=10, W=W)
-    for thr in (0, 1024):
-        for codec in CODECS:
-            run_batch(B, oracle_mod, ids2, off2, W, thr, codec=codec)
+    # 9000 buffers: the one-CTA plan + block-table chain; 5000 and 8192: the fused plan of up to 8192 buffers
+    # (two rounds of its decode-side scan, and the limit itself)
+    for n_buf in (9000, 5000, 8192):
+        many = torch.randint(0, 300, (n_buf,), generator=g)
+        ids2, off2 = streams.batch_of_streams(many, 16.0, seed=10, W=W)
+        for thr in (0, 1024):
+            for codec in CODECS:
+                run_batch(B, oracle_mod, ids2, off2, W, thr, codec=codec)
 
 
 @pytest.mark.parametrize("codec", CODECS)
