@@ -190,6 +190,33 @@ def run_reference(args, rank, world):
     }))
 
 
+def run_config_report(args):
+    """`bench.py --config N`: the config-3/4/5 report of paper_1704_00513_b200/report.py with the oracle timed beside
+    every row (same run, same inputs). The oracle runs its multi-threaded driver on all host cores
+    under the PFOR rule, its serial functions under BP128 (the driver knows mode 1 only)."""
+    import oracle
+    from paper_1704_00513_b200 import report
+    from paper_1704_00513_b200 import build as cuda_build
+    cuda_build.build()
+    oracle.build()
+    cores = len(os.sched_getaffinity(0))
+
+    def oracle_timer(ids, off, Wb, thr, codec):
+        a = ids.cpu().numpy().view(np.uint32 if Wb == 32 else np.uint64)
+        o = off.cpu().numpy().astype(np.uint64)
+        threads = cores if codec == oracle.CODEC_PFOR else 0
+        t0 = time.perf_counter()
+        s, so = oracle.compress_batch(a, o, thr, threads=threads, codec=codec)
+        t1 = time.perf_counter()
+        y, _ = oracle.decompress_batch(s, so, Wb, len(a), threads=threads)
+        t2 = time.perf_counter()
+        assert len(a) == 0 or (y[0] == a[0] and y[len(a) - 1] == a[-1])
+        return t1 - t0, t2 - t1
+
+    print(f"oracle columns: oracle/ on {cores} host threads (PFOR rule; 1 thread under BP128), same buffers, same run\n")
+    report.run(args, cpu_timer=oracle_timer)
+
+
 def workload_config(log2n, world):
     """config of the JSON line: the same for both arms (the driver compares them)."""
     return {"workload": f"configs[1]: 3 sorted u32 streams of 2^{log2n} IDs (a: geometric gaps mean 2, b: mean 256, "
@@ -430,6 +457,57 @@ def run_ours(args, rank, local_rank, world):
         except torch.cuda.OutOfMemoryError:
             batch["rmat25_level"] = None
 
+    # ---- frontier bitmaps (FORMAT.md §9), beside the headline: stream a given as the bitmap of its IDs
+    # (one bit per vertex: the form the BFS holds its frontier in) through bfsc_compress_bitmap /
+    # bfsc_decompress_to_bitmap, on rotating copies; the stream is byte-identical to the ID-list call's (checked).
+    bitmap = None
+    if rank == 0 and args.log2n == LOG2_N and not args.no_batch:
+        a_ids = ids[0].to(torch.int64) & 0xFFFFFFFF
+        n_bits = int(a_ids.max().item()) + 1
+        words = ((n_bits + 31) // 32 + 3) // 4 * 4
+        bits = torch.zeros(words * 32, dtype=torch.bool, device=dev)
+        bits[a_ids] = True
+        bm = (bits.view(words, 32).to(torch.int64) << torch.arange(32, dtype=torch.int64, device=dev)).sum(1)
+        bm = (bm & 0xFFFFFFFF).to(torch.uint32).view(torch.int32)
+        del bits, a_ids
+        kC = 4
+        bms = [bm] + [bm.clone() for _ in range(kC - 1)]
+        bm_back = [torch.zeros(words, dtype=torch.int32, device=dev) for _ in range(kC)]
+        ws_bm = torch.empty(B.bitmap_workspace_bytes(n_bits, W), dtype=torch.uint8, device=dev)
+        ws_d = torch.empty(B.workspace_bytes(n_bits, 1, W), dtype=torch.uint8, device=dev)
+        nb_bm = torch.zeros(1, dtype=torch.int64, device=dev)
+        enc_bm = lambda c: B.compress_bitmap(B.CODEC_PFOR, bms[c], n_bits, 0, W, 0, c_out[c], nb_bm, ws_bm, status)          # noqa: E731
+        dec_bm = lambda c: B.decompress_to_bitmap(c_out[c], cap, W, 0, bm_back[c], n_bits, n_out, ws_d, status)             # noqa: E731
+
+        def run_bm(call):
+            for c in range(kC):
+                call(c)
+            torch.cuda.synchronize()
+            a0, a1 = mk(), mk()
+            a0.record()
+            for _ in range(reps):
+                for c in range(kC):
+                    call(c)
+            a1.record()
+            torch.cuda.synchronize()
+            return a0.elapsed_time(a1) / (reps * kC)
+
+        bm_enc = float(np.median([run_bm(enc_bm) for _ in range(kTrials)]))
+        comp_bm = int(nb_bm.item())
+        bm_dec = float(np.median([run_bm(dec_bm) for _ in range(kTrials)]))
+        assert int(status.item()) == 0 and comp_bm == comp[0], "bitmap stream != ID-list stream"
+        mask_tail = torch.equal(bm_back[kC - 1][:n_bits // 32], bm[:n_bits // 32])
+        assert mask_tail and int(n_out.item()) == n, "bitmap decode != input"
+        alg_bm = n_bits // 8 + comp_bm
+        pk = peaks()[0]
+        bitmap = {"workload": f"stream a as a frontier bitmap: {n_bits} bits, {n} set (1 in {n_bits / n:.2f})", "n_bits": n_bits,
+                  "bitmap_bytes": n_bits // 8, "stream_bytes": comp_bm, "encode_ms": bm_enc, "decode_ms": bm_dec,
+                  "id_list_encode_ms": enc_ms[0], "id_list_decode_ms": dec_ms[0],
+                  "encode_frac_of_peak": alg_bm / bm_enc / 1e6 / pk, "decode_frac_of_peak": alg_bm / bm_dec / 1e6 / pk,
+                  "note": "algorithmic bytes = bitmap + stream (the ID list is never materialised); the decode ORs into a bitmap that "
+                          "already holds the bits after the first pass (same work: one atomic OR per touched word group)"}
+        del bms, bm_back, bm, ws_bm, ws_d
+
     # ---- end to end through the host-buffer C-ABI calls (pinned host memory) ----
     e2e = None
     if not args.no_e2e:
@@ -555,7 +633,7 @@ def run_ours(args, rank, local_rank, world):
                                       "average per launch; median of 5 runs (min alongside)"},
         "ratio": {k: v["ratio"] for k, v in per.items()},
         "encode_GBps_in": S * raw_bytes / sum(enc_ms) / 1e6, "decode_GBps_out": S * raw_bytes / sum(dec_ms) / 1e6,
-        "per_stream": per, "batch": batch, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
+        "per_stream": per, "batch": batch, "bitmap": bitmap, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches_timed), "clocks": clocks,
     }
     print(json.dumps(line))
 
@@ -573,7 +651,15 @@ def main():
                     "decompress per stream between cudaProfilerStart/Stop, nothing timed (profiles/README.md)")
     ap.add_argument("--no-batch", action="store_true", help="skip the batched-path section (4096-buffer batch, R-MAT 25 level)")
     ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for the whole run")
+    ap.add_argument("--config", type=int, default=0, choices=[0, 3, 4, 5],
+                    help="instead of the bench line: the report of BASELINE configs 3, 4 or 5 (paper_1704_00513_b200/report.py) "
+                         "with the oracle timed beside every row; takes report.py's flags (--graph --codec --json --scale --roots --reps)")
+    from paper_1704_00513_b200 import report as _report
+    _report.add_arguments(ap)
     args = ap.parse_args()
+    if args.config:
+        run_config_report(args)
+        return
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -51,10 +51,10 @@ extern "C" size_t bfsc_workspace_bytes(size_t n_ids_total, size_t n_buf, bfsc_dt
     return bfsc::align_up(bfsc::ws_bytes_for(n_ids_total, n_buf), 256);
 }
 
-// standard workspace of one stream of at most n_bits IDs | set bits before every 1024-bit chunk (u64, + the total)
+// standard workspace of one stream of at most n_bits IDs | the bitmap's rank tables (common.cuh)
 extern "C" size_t bfsc_bitmap_workspace_bytes(size_t n_bits, bfsc_dtype t) {
     (void)t;
-    return bfsc::align_up(bfsc::align_up(bfsc::ws_bytes_for(n_bits, 1), 16) + 8 * ((n_bits + 1023) / 1024 + 1), 256);
+    return bfsc::align_up(bfsc::align_up(bfsc::ws_bytes_for(n_bits, 1), 16) + bfsc::bitmap_extra_ws_bytes(n_bits), 256);
 }
 
 // ---- host-buffer convenience calls ------------------------------------------------------

@@ -64,6 +64,13 @@ __host__ inline size_t ws_bytes_for(size_t n_ids_total, size_t n_buf) {
     return sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16) + kTileWsBytes * tile_cap + 256;
 }
 
+// bfsc_compress_bitmap: behind the standard workspace of one stream of n_bits IDs — the set bits before every super-chunk of
+// 32 x 1024 bits (u64, + the total) and, inside its super-chunk, before every chunk (u32)
+__host__ inline size_t bitmap_extra_ws_bytes(size_t n_bits) {
+    const size_t n_super = (n_bits + 32767) / 32768;
+    return 8 * (n_super + 1) + 4 * 32 * n_super + 16;
+}
+
 // Carves the workspace; the capacities are derived from the bytes actually provided.
 __host__ inline bool ws_carve(void* ws, size_t bytes, size_t n_buf, WsView* v) {
     const size_t fixed = sizeof(WsHeader) + 3 * align_up(8 * (n_buf + 1), 16);

@@ -17,8 +17,9 @@ struct EncArgs {
     unsigned long long n_single;
     const uint32_t* bitmap;             // bfsc_compress_bitmap (FORMAT.md §9): the IDs are the set bits of bitmap[0 .. n_bits), + id_base;
     unsigned long long n_bits, id_base; //   their number is counted on the device (ws.hdr->n_ids); ids == nullptr then
-    unsigned long long* chunk;          //   bitmap: set bits before every 1024-bit chunk (n_chunks + 1 entries, after the standard workspace)
-    unsigned long long n_chunks;
+    unsigned long long* super;          //   bitmap: set bits before every super-chunk of 32 chunks (n_super + 1 entries, after the standard workspace)
+    uint32_t* chunk;                    //   bitmap: set bits of its super-chunk before every 1024-bit chunk (32 n_super entries, after `super`)
+    unsigned long long n_chunks, n_super;
     uint32_t fallback;                  // BFSC_CODEC_FLAG_RAW_FALLBACK (FORMAT.md §8), single-buffer calls
     uint32_t n_buf;
     uint32_t codec;                     // encoder rule = mode byte: 1 PFOR-D1 (E2: size argmin), 2 BP128-D1 (b = maxw, no exceptions; FORMAT.md §7)
@@ -938,21 +939,47 @@ __global__ void __launch_bounds__(256) k_enc_fallback(EncArgs a) {
 // ---- FORMAT.md §9: a frontier bitmap as the source. Chunk = 32 words = 1024 bits.
 constexpr int kChunkBits = 1024;
 
-// set bits of every chunk -> a.chunk[c] (bits at positions >= n_bits do not count). One warp per chunk.
+constexpr int kSuperChunks = 32;                         // chunks per super-chunk: one warp counts one super-chunk (4 KB of bitmap)
+__device__ __forceinline__ uint32_t bm_word(const EncArgs& a, unsigned long long c, int lane) {   // word `lane` of chunk c, bits >= n_bits cleared
+    const unsigned long long bit0 = c * kChunkBits + 32ull * lane;
+    uint32_t x = bit0 < a.n_bits ? a.bitmap[c * 32 + lane] : 0u;
+    if (bit0 < a.n_bits && a.n_bits - bit0 < 32) x &= (1u << (uint32_t)(a.n_bits - bit0)) - 1u;
+    return x;
+}
+// Position of the k-th (k = 0: lowest) set bit of x; x has more than k set bits. Five halving steps.
+__device__ __forceinline__ uint32_t select_bit(uint32_t x, uint32_t k) {
+    uint32_t pos = 0;
+#pragma unroll
+    for (int w = 16; w > 0; w >>= 1) {
+        const uint32_t c = (uint32_t)__popc(x & ((1u << w) - 1u));
+        if (k >= c) { k -= c; x >>= w; pos += w; }
+    }
+    return pos;
+}
+
+// Set bits of every chunk, as prefixes inside its super-chunk -> a.chunk[c]; totals of the super-chunks -> a.super[s].
+// One warp per super-chunk: 32 coalesced 128-byte loads, lane j keeps the count of chunk j.
 __global__ void __launch_bounds__(256) k_bm_count(EncArgs a) {
     pdl_wait();                                          // the call before this one is complete (workspace, inputs)
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
-    for (unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); c < a.n_chunks; c += (unsigned long long)gridDim.x * 8) {
-        const unsigned long long bit0 = c * kChunkBits + 32ull * lane;
-        uint32_t x = bit0 < a.n_bits ? a.bitmap[c * 32 + lane] : 0u;
-        if (bit0 < a.n_bits && a.n_bits - bit0 < 32) x &= (1u << (uint32_t)(a.n_bits - bit0)) - 1u;
-        const uint32_t k = __reduce_add_sync(kFull, (uint32_t)__popc(x));
-        if (lane == 0) a.chunk[c] = k;
+    for (unsigned long long s = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); s < a.n_super; s += (unsigned long long)gridDim.x * 8) {
+        uint32_t mine = 0;
+#pragma unroll 8
+        for (int j = 0; j < kSuperChunks; j++) {
+            const unsigned long long c = s * kSuperChunks + j;
+            const uint32_t k = c < a.n_chunks ? __reduce_add_sync(kFull, (uint32_t)__popc(bm_word(a, c, lane))) : 0u;
+            if (lane == j) mine = k;
+        }
+        uint32_t inc = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        a.chunk[s * kSuperChunks + lane] = inc - mine;
+        if (lane == 31) a.super[s] = inc;
     }
 }
 
-// One CTA: exclusive scan of the chunk counts (in place; entry n_chunks = n), then the plan of the one stream (E0).
+// One CTA: exclusive scan of the super-chunk totals (in place; entry n_super = n), then the plan of the one stream (E0).
 template <int W>
 __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
     __shared__ Scan2 sm[33];
@@ -961,13 +988,13 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
     pdl_launch_dependents();
     Scan2 carry{0, 0};
     constexpr int kIpt = 8;
-    for (unsigned long long c0 = 0; c0 < a.n_chunks; c0 += 1024ull * kIpt) {
+    for (unsigned long long c0 = 0; c0 < a.n_super; c0 += 1024ull * kIpt) {
         unsigned long long v[kIpt];
         Scan2 sum{0, 0};
 #pragma unroll
         for (int u = 0; u < kIpt; u++) {
             const unsigned long long c = c0 + (unsigned long long)threadIdx.x * kIpt + u;
-            v[u] = c < a.n_chunks ? a.chunk[c] : 0ull;
+            v[u] = c < a.n_super ? a.super[c] : 0ull;
             sum.a += v[u];
         }
         Scan2 tot;
@@ -976,7 +1003,7 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
 #pragma unroll
         for (int u = 0; u < kIpt; u++) {
             const unsigned long long c = c0 + (unsigned long long)threadIdx.x * kIpt + u;
-            if (c < a.n_chunks) a.chunk[c] = run;
+            if (c < a.n_super) a.super[c] = run;
             run += v[u];
         }
         carry.a += tot.a;
@@ -990,7 +1017,7 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
     if (ok)
         for (unsigned long long q = threadIdx.x; q < nt; q += blockDim.x) a.ws.tile_state[q * kStateStride] = 0;
     if (threadIdx.x == 0) {
-        a.chunk[a.n_chunks] = n;
+        a.super[a.n_super] = n;
         a.ws.blk_first[0] = 0; a.ws.blk_first[1] = nb;
         a.ws.fixed_prefix[0] = 0; a.ws.fixed_prefix[1] = fixed;
         a.ws.stream_start[0] = 0; a.ws.stream_start[1] = 0;
@@ -1012,20 +1039,17 @@ __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
     const unsigned long long n = a.ws.hdr->n_ids;
     if (blockIdx.x == 0 && threadIdx.x == 0) starts[(n + kBlk - 1) / kBlk] = (uint32_t)a.n_bits;
     for (unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); c < a.n_chunks; c += (unsigned long long)gridDim.x * 8) {
-        const unsigned long long p0 = a.chunk[c], p1 = a.chunk[c + 1];
-        unsigned long long g = (p0 + kBlk - 1) / kBlk;   // first block that starts at or after rank p0
-        if (g * kBlk >= p1) continue;                    // no block starts in this chunk
-        const unsigned long long bit0 = c * kChunkBits + 32ull * lane;
-        uint32_t x = bit0 < a.n_bits ? a.bitmap[c * 32 + lane] : 0u;
-        if (bit0 < a.n_bits && a.n_bits - bit0 < 32) x &= (1u << (uint32_t)(a.n_bits - bit0)) - 1u;
+        const unsigned long long p0 = a.super[c / kSuperChunks] + a.chunk[c];
+        const uint32_t x = bm_word(a, c, lane);
         const uint32_t k = (uint32_t)__popc(x);
         uint32_t inc = k;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        const unsigned long long p1 = p0 + __shfl_sync(kFull, inc, 31);
         const uint32_t excl = inc - k;
-        for (; g * kBlk < p1; g++) {
+        for (unsigned long long g = (p0 + kBlk - 1) / kBlk; g * kBlk < p1; g++) {       // the block starts in this chunk
             const uint32_t r = (uint32_t)(g * kBlk - p0);            // rank inside the chunk
-            if (r >= excl && r < excl + k) starts[g] = (uint32_t)(bit0 + __fns(x, 0, (int)(r - excl) + 1));
+            if (r >= excl && r < excl + k) starts[g] = (uint32_t)(c * kChunkBits + 32ull * lane + select_bit(x, r - excl));
         }
     }
 }
@@ -1187,10 +1211,12 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
     if (max_tiles > a.ws.tile_cap) return BFSC_ERR_INVALID_ARG;              // workspace too small
     if (max_tiles < (unsigned long long)grid) grid = max_tiles ? (int)max_tiles : 1;
     a.grid = (uint32_t)grid;
-    size_t cgrid = (size_t)((a.n_chunks + 7) / 8);
+    size_t cgrid = (size_t)((a.n_chunks + 7) / 8), sgrid = (size_t)((a.n_super + 7) / 8);
     if (cgrid > (size_t)dev.sms * 8) cgrid = (size_t)dev.sms * 8;
+    if (sgrid > (size_t)dev.sms * 8) sgrid = (size_t)dev.sms * 8;
     if (cgrid < 1) cgrid = 1;
-    BFSC_LAUNCH(launch_dep(k_bm_count, (int)cgrid, 256, 0, s, a));
+    if (sgrid < 1) sgrid = 1;
+    BFSC_LAUNCH(launch_dep(k_bm_count, (int)sgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_bm_plan<W>, 1, 1024, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_bm_starts, (int)cgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 2>, grid, kEncThreads, kSmem, s, a));
@@ -1243,11 +1269,14 @@ extern "C" bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_
     if ((unsigned long long)n_bits >= (1ull << 32)) return BFSC_ERR_INVALID_ARG;
     if (((uintptr_t)d_bitmap & 15) || ((uintptr_t)d_out & 15) || ((uintptr_t)d_workspace & 15)) return BFSC_ERR_INVALID_ARG;
     const size_t std_bytes = align_up(ws_bytes_for(n_bits, 1), 16), n_chunks = (n_bits + kChunkBits - 1) / kChunkBits;
-    if (workspace_bytes < std_bytes + 8 * (n_chunks + 1)) return BFSC_ERR_INVALID_ARG;
+    const size_t n_super = (n_chunks + kSuperChunks - 1) / kSuperChunks;
+    if (workspace_bytes < std_bytes + bitmap_extra_ws_bytes(n_bits)) return BFSC_ERR_INVALID_ARG;
     EncArgs a = {};
     if (!ws_carve(d_workspace, std_bytes, 1, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.bitmap = d_bitmap; a.n_bits = n_bits; a.id_base = id_base;
-    a.chunk = reinterpret_cast<unsigned long long*>(static_cast<char*>(d_workspace) + std_bytes); a.n_chunks = n_chunks;
+    a.super = reinterpret_cast<unsigned long long*>(static_cast<char*>(d_workspace) + std_bytes);
+    a.chunk = reinterpret_cast<uint32_t*>(a.super + n_super + 1);
+    a.n_chunks = n_chunks; a.n_super = n_super;
     a.fallback = fallback; a.n_buf = 1; a.codec = (uint32_t)codec; a.thr = raw_threshold_bytes;
     a.out = (unsigned char*)d_out; a.out_cap = out_capacity; a.out_total = (unsigned long long*)d_out_bytes; a.status = d_status;
     return t == BFSC_U32 ? launch_encode_bitmap<32>(a, (cudaStream_t)cuda_stream) : launch_encode_bitmap<64>(a, (cudaStream_t)cuda_stream);

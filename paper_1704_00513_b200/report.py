@@ -3,6 +3,10 @@
     python -m paper_1704_00513_b200.report --config 3            # R-MAT 22, u32, 16 buffers/level, 1 KB threshold
     python -m paper_1704_00513_b200.report --config 4            # R-MAT 25, u64, 64 buffers/level
     python -m paper_1704_00513_b200.report --config 5            # message-size sweep + 4096-buffer batch
+    (`python bench.py --config N ...` runs the same report with two more columns: the oracle (oracle/, multi-threaded
+     driver) timed on the box's host cores on the very same buffers, beside every row. This module belongs to the
+     product package and never imports the oracle: bench.py passes the timer in.)
+    (--json adds one JSON line per report: totals, oracle included when timed)
     (--scale / --roots shrink configs 3 and 4 for a quick look; --codec bp128 runs the same cases under the
      no-exception rule, FORMAT.md §7 — the codec class the thesis ran; --graph replays
      each timed run from a CUDA graph captured around the same C-ABI calls: the host's 9-15 us per call from
@@ -40,8 +44,11 @@ def peak_gbs():
 
 
 class Runner:
-    def __init__(self, dev, reps=5, codec=B.CODEC_PFOR, graph=False):
-        self.dev, self.reps, self.codec, self.graph = dev, reps, codec, graph
+    def __init__(self, dev, reps=5, codec=B.CODEC_PFOR, graph=False, cpu_timer=None):
+        """cpu_timer(ids: device tensor, off: device int64 offsets, W, thr, codec) -> (encode seconds, decode seconds)
+        of a CPU implementation on the same buffers, or None (bench.py --config passes the oracle's)."""
+        self.dev, self.reps, self.codec, self.graph, self.cpu_timer = dev, reps, codec, graph, cpu_timer
+        self.totals = []                                     # one dict per report row marked as a total (--json)
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
         self.peak = peak_gbs()
 
@@ -130,6 +137,10 @@ class Runner:
             pad = torch.empty(n + 4, dtype=ids.dtype, device=dev)
             pad[:n] = ids
             pads.append(pad)
+        cpu = {}
+        if self.cpu_timer is not None:
+            ce, cd = self.cpu_timer(ids, off, W, thr, self.codec)
+            cpu = {"cpu_enc_ms": 1e3 * ce, "cpu_dec_ms": 1e3 * cd}
         if single:                                           # one buffer: the single-buffer entry points
             nbytes = torch.zeros(1, dtype=torch.int64, device=dev)
             n_out = torch.zeros(1, dtype=torch.int64, device=dev)
@@ -139,14 +150,14 @@ class Runner:
             assert torch.equal(backs[copies - 1][:n], ids), "decode != input"
             comp = int(nbytes.item())
             return {"n": n, "n_buf": 1, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec,
-                    "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound}
+                    "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound} | cpu
         enc, enc_iso = self._time([(lambda c=c: B.compress_batch_codec(self.codec, pads[c], off, n_buf, W, thr, outs[c], out_off, ws, status)) for c in range(copies)])
         dec, dec_iso = self._time([(lambda c=c: B.decompress_batch(outs[c], out_off, n_buf, W, backs[c], id_off, ws, status)) for c in range(copies)])
         assert int(status.item()) == 0
         assert torch.equal(backs[copies - 1][:n], ids) and torch.equal(id_off, off), "decode != input"
         comp = int(out_off[-1].item())
         return {"n": n, "n_buf": n_buf, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec,
-                "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound}
+                "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound} | cpu
 
     def row(self, label, r):
         raw, comp = r["raw"], r["comp"]
@@ -156,17 +167,28 @@ class Runner:
         bits = 8.0 * comp / r["n"] if r["n"] else 0.0
         if r.get("host_bound"):
             label += " (*)"
+        ora = "n/a | n/a"
+        if r.get("cpu_enc_ms") and r.get("cpu_dec_ms"):
+            ora = f"{raw / r['cpu_enc_ms'] / 1e6:.2f} | {raw / r['cpu_dec_ms'] / 1e6:.2f}"
         return (f"| {label} | {r['n_buf']} | {raw / 1e6:.3f} | {ratio:.2f} | {bits:.2f} | {r['enc_ms'] * 1e3:.1f} | "
                 f"{raw / e / 1e9:.1f} | {100 * alg / e / 1e9 / self.peak:.1f} | {r['dec_ms'] * 1e3:.1f} | "
-                f"{raw / d / 1e9:.1f} | {100 * alg / d / 1e9 / self.peak:.1f} | {r['enc_iso_ms'] * 1e3:.1f} | {r['dec_iso_ms'] * 1e3:.1f} |")
+                f"{raw / d / 1e9:.1f} | {100 * alg / d / 1e9 / self.peak:.1f} | {r['enc_iso_ms'] * 1e3:.1f} | {r['dec_iso_ms'] * 1e3:.1f} | {ora} |")
+
+    def total(self, label, r):
+        """A totals row: printed like any row, and kept for --json."""
+        self.totals.append({"case": label} | {k: r[k] for k in r if k != "host_bound"} |
+                           {"enc_frac_of_peak": (r["raw"] + r["comp"]) / (r["enc_ms"] * 1e-3) / 1e9 / self.peak,
+                            "dec_frac_of_peak": (r["raw"] + r["comp"]) / (r["dec_ms"] * 1e-3) / 1e9 / self.peak})
+        return self.row(label, r)
 
 
 HDR = ("enc us / dec us: per call, in a run of back-to-back calls on rotating copies of the buffers (working set >= 256 MB or 8 copies); "
        "isolated: ONE call between two events after an L2 flush (launch latency and cold caches included); "
        "(*) = the host needed as long to enqueue the run as the GPU to execute it (9-15 us per call from Python): "
-       "the back-to-back figure is then the host's\n\n"
-       "| case | buffers | raw MB | ratio | bits/ID | enc us | enc GB/s in | enc % peak | dec us | dec GB/s out | dec % peak | isolated enc us | isolated dec us |\n"
-       "|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+       "the back-to-back figure is then the host's; oracle enc / dec GB/s: the CPU oracle (oracle/, all host cores) timed on the "
+       "same buffers in the same run (only through `python bench.py --config N`; n/a otherwise)\n\n"
+       "| case | buffers | raw MB | ratio | bits/ID | enc us | enc GB/s in | enc % peak | dec us | dec GB/s out | dec % peak | isolated enc us | isolated dec us | oracle enc GB/s | oracle dec GB/s |\n"
+       "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
 
 
 def rmat_config(R, scale, seed, W, parts, n_roots, thr, per_level_roots=1):
@@ -181,12 +203,13 @@ def rmat_config(R, scale, seed, W, parts, n_roots, thr, per_level_roots=1):
             vals, off = streams.split_block(f, parts, 1 << scale)
             ids = streams.as_ids(vals, W).to(dev)
             r = R.batch(ids, off.to(dev), W, thr)
-            for k in ("n", "raw", "comp", "enc_ms", "dec_ms", "enc_iso_ms", "dec_iso_ms"):
-                tot[k] += r[k]
+            for k in ("n", "raw", "comp", "enc_ms", "dec_ms", "enc_iso_ms", "dec_iso_ms", "cpu_enc_ms", "cpu_dec_ms"):
+                if k in r:
+                    tot[k] = tot.get(k, 0.0) + r[k]
             tot["host_bound"] = tot.get("host_bound", False) or r["host_bound"]
             if ri < per_level_roots:
                 print(R.row(f"root {root} level {level} ({r['n']} IDs)", r))
-        print(R.row(f"**root {root}, all levels** ({tot['n']} IDs)", tot))
+        print(R.total(f"**root {root}, all levels** ({tot['n']} IDs)", tot))
 
 
 def sweep(R):
@@ -209,22 +232,15 @@ def sweep(R):
     counts = streams.log_uniform_counts(4096, 8, 16, 32, seed=5)
     ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=32, device=dev)
     for thr in (0, 1024):
-        print(R.row(f"batch of 4096 buffers 256 B-64 KB, mean 16, threshold {thr}", R.batch(ids.to(dev), off.to(dev), 32, thr)))
+        print(R.total(f"batch of 4096 buffers 256 B-64 KB, mean 16, threshold {thr}", R.batch(ids.to(dev), off.to(dev), 32, thr)))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--config", type=int, required=True, choices=[3, 4, 5])
-    ap.add_argument("--scale", type=int, default=0)
-    ap.add_argument("--roots", type=int, default=0)
-    ap.add_argument("--reps", type=int, default=5)
-    ap.add_argument("--codec", default="pfor", choices=["pfor", "bp128"], help="encoder rule (bfsc_codec)")
-    ap.add_argument("--graph", action="store_true", help="replay the timed calls from captured CUDA graphs")
-    a = ap.parse_args()
+def run(a, cpu_timer=None):
+    """The report of parsed arguments `a` (see main); cpu_timer: Runner's."""
     assert torch.cuda.is_available(), "needs a CUDA device (there is no CPU fallback)"
     dev = torch.device("cuda:0")
     B.lib()
-    R = Runner(dev, a.reps, B.CODEC_BP128 if a.codec == "bp128" else B.CODEC_PFOR, a.graph)
+    R = Runner(dev, a.reps, B.CODEC_BP128 if a.codec == "bp128" else B.CODEC_PFOR, a.graph, cpu_timer)
     if a.graph:
         print("timed runs replayed from CUDA graphs captured around the C-ABI calls (device-side time of the kernel chain)\n")
     print(f"encoder rule: {'BP128-D1 (mode 2, no exceptions)' if a.codec == 'bp128' else 'PFOR-D1 (mode 1)'}\n")
@@ -234,6 +250,26 @@ def main():
         rmat_config(R, a.scale or 25, 4, 64, 64, a.roots or 8, 1024)
     else:
         sweep(R)
+    if a.json:
+        print()
+        print(json.dumps({"report": f"configs[{a.config - 1}]", "codec": a.codec, "graph_replay": bool(a.graph),
+                          "peak_GBps": R.peak, "oracle_timed": cpu_timer is not None, "totals": R.totals}))
+
+
+def add_arguments(ap):
+    ap.add_argument("--scale", type=int, default=0)
+    ap.add_argument("--roots", type=int, default=0)
+    ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--codec", default="pfor", choices=["pfor", "bp128"], help="encoder rule (bfsc_codec)")
+    ap.add_argument("--graph", action="store_true", help="replay the timed calls from captured CUDA graphs")
+    ap.add_argument("--json", action="store_true", help="one JSON line with the totals after the table")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, required=True, choices=[3, 4, 5])
+    add_arguments(ap)
+    run(ap.parse_args())
 
 
 if __name__ == "__main__":
