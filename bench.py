@@ -602,7 +602,7 @@ def run_ours(args, rank, local_rank, world):
     dom = names[dom_i]
     key = "abc"[dom_i]
     full = args.log2n == LOG2_N
-    roof = {"bound": "hbm", "kernel": f"k_enc_tiles<32, false> (+ its 1-CTA k_enc_plan): the bfsc_compress call on stream {key}, the slowest of a, b, c",
+    roof = {"bound": "hbm", "kernel": f"k_enc_tiles<32, 0> (+ its 1-CTA k_enc_plan): the bfsc_compress call on stream {key}, the slowest of a, b, c",
             "achieved": per[dom]["encode_alg_GBps"],
             "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": per[dom]["encode_alg_GBps"] / peak,
             "algorithmic_bytes_per_launch": raw_bytes + comp[dom_i] + 8,
@@ -610,7 +610,7 @@ def run_ours(args, rank, local_rank, world):
             "per_stream": {"abc"[i]: {"encode_frac": per[names[i]]["encode_frac_of_peak"], "decode_frac": per[names[i]]["decode_frac_of_peak"],
                                       "encode_traffic": ncu_traffic("encode", "abc"[i]) if full else None,
                                       "decode_traffic": ncu_traffic("decode", "abc"[i]) if full else None} for i in range(S)},
-            "decode": {"kernel": f"k_dec_tiles<32, false>: the bfsc_decompress call on stream {key}", "achieved": per[dom]["decode_alg_GBps"],
+            "decode": {"kernel": f"k_dec_tiles<32, 0, 0, 0, 0>: the bfsc_decompress call on stream {key}", "achieved": per[dom]["decode_alg_GBps"],
                        "frac": per[dom]["decode_alg_GBps"] / peak, "traffic": ncu_traffic("decode", key) if full else None,
                        "traffic_source": NCU_SUMMARIES["decode"]}}
     cpu = None
