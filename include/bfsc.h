@@ -122,6 +122,22 @@ bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t 
                           void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                           void* cuda_stream);
 
+/* bfsc_compress for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same kernels, with the workspace in a device array that is part of the library image
+ * (a file-scope `static __device__` array of BFSC_NOALLOC_SCRATCH_BYTES bytes: every GPU that loads the library holds it
+ * until the process exits). The call allocates nothing, on the host or on the device.
+ *   n_ids <= BFSC_NOALLOC_MAX_IDS, else BFSC_ERR_INVALID_ARG (nothing is enqueued); everything else as bfsc_compress,
+ *   output bytes included.
+ *   ALL no-alloc calls of a device share that one array: two of them that overlap on the GPU (two streams, or two host
+ *   threads on two streams) race on it and produce garbage — issue them on one stream at a time. The array keeps the
+ *   last call's contents; whatever must start at zero (tile states, ticket counter) is reset by the call's own plan
+ *   kernel, as for a caller-owned workspace. */
+#define BFSC_NOALLOC_MAX_IDS ((size_t)1 << 22)
+#define BFSC_NOALLOC_SCRATCH_BYTES ((size_t)1088 * 1024)
+bfsc_status bfsc_compress_noalloc(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
+                                  void* d_out, size_t out_capacity, uint64_t* d_out_bytes, uint32_t* d_status,
+                                  void* cuda_stream);
+
 /* bfsc_compress with the encoder rule given (any other value: BFSC_ERR_INVALID_ARG). */
 bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, size_t n_ids, bfsc_dtype t,
                                 size_t raw_threshold_bytes, void* d_out, size_t out_capacity,

@@ -19,13 +19,14 @@ OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED =
 U32, U64 = 32, 64
 CODEC_PFOR, CODEC_BP128 = 1, 2          # bfsc_codec (include/bfsc.h)
 CODEC_FLAG_EXCLUSIVE = 0x100            # launch flag, OR-ed into the codec (include/bfsc.h)
+NOALLOC_MAX_IDS = 1 << 22               # bfsc_compress_noalloc: BFSC_NOALLOC_MAX_IDS (include/bfsc.h)
 CODEC_FLAG_RAW_FALLBACK = 0x200         # FORMAT.md §8, OR-ed into the codec of a single-buffer call
 
 EXPORTS = [
     "bfsc_version", "bfsc_compress_bound", "bfsc_batch_compress_bound", "bfsc_workspace_bytes",
     "bfsc_compress", "bfsc_decompress", "bfsc_compress_batch", "bfsc_decompress_batch",
     "bfsc_compress_codec", "bfsc_compress_batch_codec",
-    "bfsc_bitmap_workspace_bytes", "bfsc_compress_bitmap", "bfsc_decompress_to_bitmap",
+    "bfsc_bitmap_workspace_bytes", "bfsc_compress_bitmap", "bfsc_decompress_to_bitmap", "bfsc_compress_noalloc",
     "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
 ]
 
@@ -64,6 +65,8 @@ def lib():
         L.bfsc_host_scratch_bytes.argtypes = [sz, i32]
         L.bfsc_compress.restype = i32
         L.bfsc_compress.argtypes = [vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_compress_noalloc.restype = i32
+        L.bfsc_compress_noalloc.argtypes = [vp, sz, i32, sz, vp, sz, vp, vp, vp]
         L.bfsc_compress_codec.restype = i32
         L.bfsc_compress_codec.argtypes = [i32, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_compress_batch_codec.restype = i32
@@ -134,6 +137,13 @@ def compress(d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_bytes, d_workspa
     _check(lib().bfsc_compress(_ptr(d_ids), n_ids, W, raw_threshold_bytes, _ptr(d_out), d_out.numel(),
                                _ptr(d_out_bytes), _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
                                ctypes.c_void_p(_stream())), "bfsc_compress")
+
+
+def compress_noalloc(d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_bytes, d_status):
+    """bfsc_compress_noalloc: bfsc_compress with the workspace in the library's own device array (no allocation anywhere;
+    n_ids <= NOALLOC_MAX_IDS; calls that overlap on the GPU race on that array)."""
+    _check(lib().bfsc_compress_noalloc(_ptr(d_ids), n_ids, W, raw_threshold_bytes, _ptr(d_out), d_out.numel(),
+                                       _ptr(d_out_bytes), _ptr(d_status), ctypes.c_void_p(_stream())), "bfsc_compress_noalloc")
 
 
 def compress_codec(codec, d_ids, n_ids, W, raw_threshold_bytes, d_out, d_out_bytes, d_workspace, d_status):

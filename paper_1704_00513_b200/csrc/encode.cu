@@ -1289,6 +1289,41 @@ extern "C" bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype
                                d_workspace, workspace_bytes, d_status, cuda_stream);
 }
 
+// ---- bfsc_compress_noalloc (include/bfsc.h): the workspace of a single-buffer call of up to BFSC_NOALLOC_MAX_IDS IDs
+// lives in the library image. In HOST code the array's name is a host-side stand-in, not a device address: the address
+// the kernels get comes from cudaGetSymbolAddress, once per device, with that device current.
+namespace bfsc {
+static __device__ __align__(256) unsigned char g_noalloc_scratch[BFSC_NOALLOC_SCRATCH_BYTES];
+
+static void* noalloc_scratch(int device) {               // device address of the array on `device` (the current one), or nullptr
+    static std::mutex mu;
+    static void* addr[kMaxDevices] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    if (addr[device] == nullptr) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || p == nullptr) return nullptr;
+        addr[device] = p;
+    }
+    return addr[device];
+}
+}  // namespace bfsc
+
+extern "C" bfsc_status bfsc_compress_noalloc(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
+                                             void* d_out, size_t out_capacity, uint64_t* d_out_bytes,
+                                             uint32_t* d_status, void* cuda_stream) {
+    using namespace bfsc;
+    if (!d_out_bytes) return BFSC_ERR_INVALID_ARG;
+    if (n_ids > BFSC_NOALLOC_MAX_IDS) return BFSC_ERR_INVALID_ARG;       // beyond what the built-in scratch array holds
+    static_assert(BFSC_NOALLOC_SCRATCH_BYTES % 256 == 0, "scratch size");
+    if (ws_bytes_for(BFSC_NOALLOC_MAX_IDS, 1) > BFSC_NOALLOC_SCRATCH_BYTES) return BFSC_ERR_INVALID_ARG;   // (a build-time property)
+    DeviceInfo dev;
+    if (!current_device(&dev)) return BFSC_ERR_CUDA;
+    void* ws = noalloc_scratch(dev.device);
+    if (ws == nullptr) return BFSC_ERR_CUDA;
+    return encode_common(BFSC_CODEC_PFOR, d_ids, nullptr, n_ids, 1, t, raw_threshold_bytes, d_out, out_capacity, nullptr,
+                         d_out_bytes, ws, BFSC_NOALLOC_SCRATCH_BYTES, d_status, cuda_stream);
+}
+
 extern "C" bfsc_status bfsc_compress_batch_codec(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_offsets,
                                                  size_t n_buf, bfsc_dtype t, size_t raw_threshold_bytes, void* d_out,
                                                  size_t out_capacity, uint64_t* d_out_offsets, void* d_workspace,
