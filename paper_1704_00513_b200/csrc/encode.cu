@@ -585,34 +585,51 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                         st_volatile_u64(&a.ws.stream_start[bf_i[h]], bf_f0[h] + 16ull * (excl + offs[h]) + 1);
                 }
             }
-            // final offsets, directory entries
+            // Final offsets first: they need the look-back's result and the plan's tables only, and the workers wait
+            // for nothing else. The directory entries follow AFTER the offsets are posted: a batch call's entry also
+            // needs the start of its stream, which a stream that spans in from an earlier tile gets from that tile's
+            // scan warp (a poll) — that wait is now off the workers' path.
+            unsigned long long at_h[kPer];
+#pragma unroll
+            for (int h = 0; h < kPer; h++) {
+                const int jj = kPer * lane + h;
+                at_h[h] = kSkip;
+                if (jj >= kTileR) continue;
+                if (g0 + jj < total) {
+                    unsigned long long f1 = f1_single;
+                    if constexpr (kBatch) f1 = bf_f1[h];
+                    const unsigned long long at = f1 + 16ull * (excl + offs[h]);
+                    if (at + (kk[h] >> 14) <= a.out_cap) at_h[h] = at;
+                    else set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+                }
+                s_at[kp][jj] = at_h[h];
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&mb_off[kp]);     // offsets of tile k are posted
+            // directory entries, stream header of a single-buffer call
 #pragma unroll
             for (int h = 0; h < kPer; h++) {
                 const int jj = kPer * lane + h;
                 if (jj >= kTileR) continue;
                 const unsigned long long g = g0 + jj;
                 const uint32_t key = kk[h];
-                unsigned long long at = kSkip;
+                const unsigned long long at = at_h[h];
                 if (g < total) {
                     const uint32_t off = offs[h], bytes = key >> 14;
                     unsigned long long first = 0, f0 = 0, f1 = f1_single, S = 0;
                     uint32_t i = 0;
                     if constexpr (kBatch) {
                         i = bf_i[h]; first = bf_first[h]; f0 = bf_f0[h]; f1 = bf_f1[h];
-                        if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
-                        else if (i > 0) {                // published by the tile that owns the stream's first block
-                            S = bf_S[h];
-                            while (S == 0) S = ld_volatile_u64(&a.ws.stream_start[i]);
-                            S -= 1;
+                        if (at != kSkip) {
+                            if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
+                            else if (i > 0) {            // published by the tile that owns the stream's first block
+                                S = bf_S[h];
+                                while (S == 0) S = ld_volatile_u64(&a.ws.stream_start[i]);
+                                S -= 1;
+                            }
                         }
                     }
-                    at = f1 + 16ull * (excl + off);
-                    if (at + bytes <= a.out_cap) {
-                        reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
-                    } else {
-                        set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
-                        at = kSkip;
-                    }
+                    if (at != kSkip) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
                     if (!batch && g == total - 1) {      // single buffer: stream header, dir[nb], zero pad
                         const unsigned long long tot = f1 + 16ull * (excl + off) + bytes;
                         if (at != kSkip) {
@@ -631,10 +648,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                         if (a.out_total) *a.out_total = at != kSkip ? tot : 0ull;
                     }
                 }
-                s_at[kp][jj] = at;
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&mb_off[kp]);     // offsets of tile k are posted
             kp = kp == kNB - 1 ? 0 : kp + 1;
         }
         return;
