@@ -45,13 +45,20 @@ __device__ __forceinline__ void bm_expand(T* __restrict__ raw, const uint32_t* _
         uint32_t inc = c, y;
         y = __shfl_up_sync(qmask, inc, 1, 4); if (l >= 1) inc += y;
         y = __shfl_up_sync(qmask, inc, 2, 4); if (l >= 2) inc += y;
-        uint32_t pos = rank + inc - c;
+        // the word's set bits from the top down (one bfind per bit, no bit reversal), written backwards from the rank
+        // behind the word's last ID; four bits per trip, the stores predicated
+        T* out = raw + (rank + inc);
         rank += __shfl_sync(qmask, inc, 3, 4);
-        const unsigned long long id0 = id_base + 32ull * wi;
+        const T id0 = (T)(id_base + 32ull * wi);
         while (x) {
-            const uint32_t b = (uint32_t)__ffs((int)x) - 1u;
-            x &= x - 1u;
-            raw[pos++] = (T)(id0 + b);
+#pragma unroll
+            for (int u = 1; u <= 4; u++) {
+                uint32_t b;
+                asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(x));               // 0xffffffff for x == 0
+                if (x) out[-u] = id0 + (T)b;
+                x &= ~(1u << (b & 31u));
+            }
+            out -= 4;
         }
     }
 }

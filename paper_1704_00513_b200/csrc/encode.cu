@@ -17,8 +17,8 @@ struct EncArgs {
     unsigned long long n_single;
     const uint32_t* bitmap;             // bfsc_compress_bitmap (FORMAT.md §9): the IDs are the set bits of bitmap[0 .. n_bits), + id_base;
     unsigned long long n_bits, id_base; //   their number is counted on the device (ws.hdr->n_ids); ids == nullptr then
-    unsigned long long* super;          //   bitmap: set bits before every super-chunk of 32 chunks (n_super + 1 entries, after the standard workspace)
-    uint32_t* chunk;                    //   bitmap: set bits of its super-chunk before every 1024-bit chunk (32 n_super entries, after `super`)
+    unsigned long long* super;          //   bitmap: set bits before every super-chunk of 32 chunks (n_super + 1 entries, behind the standard workspace and `chunk`)
+    uint32_t* chunk;                    //   bitmap: set bits of every 1024-bit chunk (32 n_super entries, before `super`)
     unsigned long long n_chunks, n_super;
     uint32_t fallback;                  // BFSC_CODEC_FLAG_RAW_FALLBACK (FORMAT.md §8), single-buffer calls
     uint32_t n_buf;
@@ -971,55 +971,56 @@ __device__ __forceinline__ uint32_t select_bit(uint32_t x, uint32_t k) {
     return pos;
 }
 
-// Set bits of every chunk, as prefixes inside its super-chunk -> a.chunk[c]; totals of the super-chunks -> a.super[s].
-// One warp per super-chunk: 32 coalesced 128-byte loads, lane j keeps the count of chunk j.
+// Set bits of every chunk -> a.chunk[c] (plain counts; entries up to the end of the last super-chunk: 0). Eight lanes per
+// chunk, one 16-byte load each (the bitmap is 16-byte aligned and readable up to a multiple of 16 bytes).
 __global__ void __launch_bounds__(256) k_bm_count(EncArgs a) {
     pdl_wait();                                          // the call before this one is complete (workspace, inputs)
     pdl_launch_dependents();
-    const int lane = threadIdx.x & 31;
-    for (unsigned long long s = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); s < a.n_super; s += (unsigned long long)gridDim.x * 8) {
-        uint32_t mine = 0;
-#pragma unroll 8
-        for (int j = 0; j < kSuperChunks; j++) {
-            const unsigned long long c = s * kSuperChunks + j;
-            const uint32_t k = c < a.n_chunks ? __reduce_add_sync(kFull, (uint32_t)__popc(bm_word(a, c, lane))) : 0u;
-            if (lane == j) mine = k;
-        }
-        uint32_t inc = mine;
+    const int lane = threadIdx.x & 31, sub = lane & 7;
+    const unsigned long long n_pad = a.n_super * kSuperChunks;
+    for (unsigned long long c = ((unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * 4 + (lane >> 3); c < n_pad;
+         c += (unsigned long long)gridDim.x * 32) {      // (the 4 chunks of a warp lie below n_pad together: n_pad is a multiple of 32)
+        const unsigned long long bit0 = c * kChunkBits + 128ull * sub;
+        uint32_t k = 0;
+        if (bit0 < a.n_bits) {
+            const uint4 v = reinterpret_cast<const uint4*>(a.bitmap)[c * 8 + sub];
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
-        a.chunk[s * kSuperChunks + lane] = inc - mine;
-        if (lane == 31) a.super[s] = inc;
+            for (int u = 0; u < 4; u++) {
+                const unsigned long long b0 = bit0 + 32ull * u;
+                uint32_t x = b0 < a.n_bits ? w[u] : 0u;
+                if (b0 < a.n_bits && a.n_bits - b0 < 32) x &= (1u << (uint32_t)(a.n_bits - b0)) - 1u;
+                k += (uint32_t)__popc(x);
+            }
+        }
+        k += __shfl_xor_sync(kFull, k, 1); k += __shfl_xor_sync(kFull, k, 2); k += __shfl_xor_sync(kFull, k, 4);
+        if (sub == 0) a.chunk[c] = k;
     }
 }
 
-// One CTA: exclusive scan of the super-chunk totals (in place; entry n_super = n), then the plan of the one stream (E0).
+// One CTA: totals of the super-chunks (warp w, step i: the 32 chunk counts of super-chunk s0 + 32 w + i in one coalesced
+// load, reduced; lane i keeps the total — thread t then holds super-chunk s0 + t), block scan -> a.super (entry n_super =
+// n = the number of set bits); then the plan of the one stream (E0).
 template <int W>
 __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
     __shared__ Scan2 sm[33];
     constexpr unsigned long long E = W / 8;
     pdl_wait();
     pdl_launch_dependents();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     Scan2 carry{0, 0};
-    constexpr int kIpt = 8;
-    for (unsigned long long c0 = 0; c0 < a.n_super; c0 += 1024ull * kIpt) {
-        unsigned long long v[kIpt];
-        Scan2 sum{0, 0};
-#pragma unroll
-        for (int u = 0; u < kIpt; u++) {
-            const unsigned long long c = c0 + (unsigned long long)threadIdx.x * kIpt + u;
-            v[u] = c < a.n_super ? a.super[c] : 0ull;
-            sum.a += v[u];
+    for (unsigned long long s0 = 0; s0 < a.n_super; s0 += 1024ull) {
+        uint32_t mine = 0;
+#pragma unroll 8
+        for (int i = 0; i < 32; i++) {
+            const unsigned long long sc = s0 + 32ull * warp + i;
+            const uint32_t t = __reduce_add_sync(kFull, sc < a.n_super ? a.chunk[sc * kSuperChunks + lane] : 0u);
+            if (lane == i) mine = t;
         }
+        const unsigned long long sc = s0 + threadIdx.x;
         Scan2 tot;
-        Scan2 ex = block_scan_excl2(sum, &tot, sm);
-        unsigned long long run = carry.a + ex.a;
-#pragma unroll
-        for (int u = 0; u < kIpt; u++) {
-            const unsigned long long c = c0 + (unsigned long long)threadIdx.x * kIpt + u;
-            if (c < a.n_super) a.super[c] = run;
-            run += v[u];
-        }
+        const Scan2 ex = block_scan_excl2(Scan2{mine, 0}, &tot, sm);
+        if (sc < a.n_super) a.super[sc] = carry.a + ex.a;
         carry.a += tot.a;
     }
     const unsigned long long n = carry.a;
@@ -1043,29 +1044,65 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
 }
 
 // Where every block begins: starts[g] = bit index of the (128 g)-th set bit (u32, in ws.blk_tab), starts[nb_all] = n_bits.
-// One warp per chunk: the chunk holds the block starts 128 g in [prefix, prefix + count): at most 8.
+// A warp takes kStartsPer chunks at a time: a chunk holds the block starts 128 g in [prefix, prefix + count), at most 8.
+// The bitmap words (the caller's input, stable since this call's first kernel) are loaded and ranked BEFORE the wait for
+// the plan kernel, all kStartsPer loads in flight at once; after it only the two prefix tables are read.
+constexpr int kStartsPer = 4;
 __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
-    pdl_wait();
     pdl_launch_dependents();
-    if (a.ws.hdr->ok == 0) return;
-    uint32_t* starts = reinterpret_cast<uint32_t*>(a.ws.blk_tab);
     const int lane = threadIdx.x & 31;
-    const unsigned long long n = a.ws.hdr->n_ids;
-    if (blockIdx.x == 0 && threadIdx.x == 0) starts[(n + kBlk - 1) / kBlk] = (uint32_t)a.n_bits;
-    for (unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); c < a.n_chunks; c += (unsigned long long)gridDim.x * 8) {
-        const unsigned long long p0 = a.super[c / kSuperChunks] + a.chunk[c];
-        const uint32_t x = bm_word(a, c, lane);
-        const uint32_t k = (uint32_t)__popc(x);
-        uint32_t inc = k;
+    const unsigned long long stride = (unsigned long long)gridDim.x * 8 * kStartsPer;
+    unsigned long long c0 = ((unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * kStartsPer;
+    bool waited = false;
+    for (; c0 < a.n_chunks; c0 += stride) {
+        uint32_t x[kStartsPer], k[kStartsPer], inc[kStartsPer];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
-        const unsigned long long p1 = p0 + __shfl_sync(kFull, inc, 31);
-        const uint32_t excl = inc - k;
-        for (unsigned long long g = (p0 + kBlk - 1) / kBlk; g * kBlk < p1; g++) {       // the block starts in this chunk
-            const uint32_t r = (uint32_t)(g * kBlk - p0);            // rank inside the chunk
-            if (r >= excl && r < excl + k) starts[g] = (uint32_t)(c * kChunkBits + 32ull * lane + select_bit(x, r - excl));
+        for (int u = 0; u < kStartsPer; u++) x[u] = c0 + u < a.n_chunks ? bm_word(a, c0 + u, lane) : 0u;
+#pragma unroll
+        for (int u = 0; u < kStartsPer; u++) {
+            k[u] = (uint32_t)__popc(x[u]);
+            inc[u] = k[u];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc[u], o); if (lane >= o) inc[u] += y; }
+        }
+        if (!waited) { pdl_wait(); waited = true; }
+        if (a.ws.hdr->ok == 0) return;
+        // set bits before each of the warp's chunks: its super-chunk's prefix + the counts of the chunks before it in
+        // the super-chunk (the warp's chunks share one: one coalesced load of its 32 counts, scanned here)
+        unsigned long long p0[kStartsPer];
+        {
+            const unsigned long long sc = c0 / kSuperChunks;
+            const uint32_t cnt = a.chunk[sc * kSuperChunks + lane];
+            uint32_t ci = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, ci, o); if (lane >= o) ci += y; }
+            const unsigned long long sp = a.super[sc];
+#pragma unroll
+            for (int u = 0; u < kStartsPer; u++) p0[u] = sp + __shfl_sync(kFull, ci - cnt, (int)((c0 + u) % kSuperChunks));
+        }
+        uint32_t* starts = reinterpret_cast<uint32_t*>(a.ws.blk_tab);
+#pragma unroll
+        for (int u = 0; u < kStartsPer; u++) {
+            // lane j takes the j-th block start of the chunk: rank r inside the chunk -> the word that holds it (the
+            // number of words whose inclusive count is <= r: five shuffle steps) -> the bit inside that word
+            const unsigned long long p1 = p0[u] + __shfl_sync(kFull, inc[u], 31);
+            const unsigned long long g = (p0[u] + kBlk - 1) / kBlk + (unsigned)lane;
+            const uint32_t r = (uint32_t)(g * kBlk - p0[u]);
+            uint32_t pos = 0;
+#pragma unroll
+            for (int st = 16; st > 0; st >>= 1) {
+                const uint32_t v = __shfl_sync(kFull, inc[u], (int)(pos + st - 1));
+                if (v <= r) pos += st;
+            }
+            pos &= 31u;                                                  // (lanes beyond the chunk's last start: anything valid)
+            const uint32_t xo = __shfl_sync(kFull, x[u], (int)pos);
+            const uint32_t eo = __shfl_sync(kFull, inc[u] - k[u], (int)pos);
+            if (g * kBlk < p1) starts[g] = (uint32_t)((c0 + u) * kChunkBits + 32ull * pos + select_bit(xo, r - eo));
         }
     }
+    if (!waited) pdl_wait();
+    if (blockIdx.x == 0 && threadIdx.x == 0 && a.ws.hdr->ok != 0)
+        reinterpret_cast<uint32_t*>(a.ws.blk_tab)[(a.ws.hdr->n_ids + kBlk - 1) / kBlk] = (uint32_t)a.n_bits;
 }
 
 // After the tiles: the streams the tile kernel does not write. (i) RAW by the threshold, (ii) RAW by the fallback rule
@@ -1227,12 +1264,16 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
     a.grid = (uint32_t)grid;
     size_t cgrid = (size_t)((a.n_chunks + 7) / 8), sgrid = (size_t)((a.n_super + 7) / 8);
     if (cgrid > (size_t)dev.sms * 8) cgrid = (size_t)dev.sms * 8;
+    sgrid = (size_t)((a.n_super * kSuperChunks + 31) / 32);          // k_bm_count: a warp takes 4 chunks
     if (sgrid > (size_t)dev.sms * 8) sgrid = (size_t)dev.sms * 8;
     if (cgrid < 1) cgrid = 1;
     if (sgrid < 1) sgrid = 1;
     BFSC_LAUNCH(launch_dep(k_bm_count, (int)sgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_bm_plan<W>, 1, 1024, 0, s, a));
-    BFSC_LAUNCH(launch_dep(k_bm_starts, (int)cgrid, 256, 0, s, a));
+    size_t tgrid = (size_t)((a.n_chunks + 8 * kStartsPer - 1) / (8 * kStartsPer));
+    if (tgrid > (size_t)dev.sms * 8) tgrid = (size_t)dev.sms * 8;
+    if (tgrid < 1) tgrid = 1;
+    BFSC_LAUNCH(launch_dep(k_bm_starts, (int)tgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 2>, grid, kEncThreads, kSmem, s, a));
     BFSC_LAUNCH(launch_dep(k_bm_finish<W>, (int)cgrid, 256, 0, s, a));
     return BFSC_OK;
@@ -1288,8 +1329,8 @@ extern "C" bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_
     EncArgs a = {};
     if (!ws_carve(d_workspace, std_bytes, 1, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.bitmap = d_bitmap; a.n_bits = n_bits; a.id_base = id_base;
-    a.super = reinterpret_cast<unsigned long long*>(static_cast<char*>(d_workspace) + std_bytes);
-    a.chunk = reinterpret_cast<uint32_t*>(a.super + n_super + 1);
+    a.chunk = reinterpret_cast<uint32_t*>(static_cast<char*>(d_workspace) + std_bytes);       // 16-byte aligned: read as uint4
+    a.super = reinterpret_cast<unsigned long long*>(a.chunk + n_super * kSuperChunks);
     a.n_chunks = n_chunks; a.n_super = n_super;
     a.fallback = fallback; a.n_buf = 1; a.codec = (uint32_t)codec; a.thr = raw_threshold_bytes;
     a.out = (unsigned char*)d_out; a.out_cap = out_capacity; a.out_total = (unsigned long long*)d_out_bytes; a.status = d_status;
