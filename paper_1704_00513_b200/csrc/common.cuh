@@ -127,6 +127,22 @@ struct BitSink { uint32_t* bm; unsigned long long id_base, n_bits; uint32_t* sta
 template <typename T>
 __device__ __forceinline__ void set_bits4(const BitSink& s, T v0, T v1, T v2, T v3, int nvalid) {
     const T v[4] = {v0, v1, v2, v3};
+    {   // Usual case (a sorted, dense frontier): all four count, all lie inside the bitmap, in the word of the first one or
+        // the word after it: one range test for the four, one or two atomics. Anything else takes the general path below.
+        const T r0 = (T)(v0 - (T)s.id_base), r1 = (T)(v1 - (T)s.id_base), r2 = (T)(v2 - (T)s.id_base), r3 = (T)(v3 - (T)s.id_base);
+        if (nvalid >= 4 && (unsigned long long)(r0 | r1 | r2 | r3) < s.n_bits) {       // (the OR is >= each of them)
+            const uint32_t q0 = (uint32_t)r0, w0 = q0 >> 5;                            // n_bits <= 2^32: the offsets fit 32 bits
+            const uint32_t d1 = ((uint32_t)r1 >> 5) - w0, d2 = ((uint32_t)r2 >> 5) - w0, d3 = ((uint32_t)r3 >> 5) - w0;
+            if ((d1 | d2 | d3) <= 1u) {
+                const uint32_t b1 = 1u << ((uint32_t)r1 & 31u), b2 = 1u << ((uint32_t)r2 & 31u), b3 = 1u << ((uint32_t)r3 & 31u);
+                const uint32_t lo = (1u << (q0 & 31u)) | (d1 ? 0u : b1) | (d2 ? 0u : b2) | (d3 ? 0u : b3);
+                const uint32_t hi = (d1 ? b1 : 0u) | (d2 ? b2 : 0u) | (d3 ? b3 : 0u);
+                atomicOr(s.bm + w0, lo);
+                if (hi) atomicOr(s.bm + w0 + 1, hi);
+                return;
+            }
+        }
+    }
     uint32_t w[4], mk[4];
 #pragma unroll
     for (int c = 0; c < 4; c++) {
