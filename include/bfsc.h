@@ -90,7 +90,11 @@ typedef enum { BFSC_U32 = 32, BFSC_U64 = 64 } bfsc_dtype;
  *                        whole compress grid becomes resident at once. The first two tiles of every CTA are
  *                        then assigned statically and start before the call's plan kernel has finished
  *                        (about 2 us less per call). If the promise is broken the call can deadlock.
- *                        Output bytes are the same with or without the flag.
+ *                        The first tiles' IDs are also read BEFORE the call waits for the kernel enqueued before it
+ *                        on the stream: d_ids must not be the output of the bfsc call enqueued immediately before
+ *                        this one (bfsc kernels release their successor early; after any other kernel, an event
+ *                        or a synchronisation the IDs are complete). Output bytes are the same with or without
+ *                        the flag.
  *   BFSC_CODEC_FLAG_RAW_FALLBACK  FORMAT.md §8: a stream that the rule does not make smaller than
  *                        its RAW form is sent RAW (mode 0) after all: total_bytes <= 32 + align16(n W / 8) always.
  *                        Single-buffer calls (bfsc_compress_codec, bfsc_compress_bitmap); the batch calls return
