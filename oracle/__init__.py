@@ -82,6 +82,8 @@ def lib():
         L.bfsc_ref_compress_bitmap.argtypes = [i32, vp, sz, c.c_uint64, i32, sz, vp, sz, c.POINTER(sz)]
         L.bfsc_ref_decompress_to_bitmap.restype = i32
         L.bfsc_ref_decompress_to_bitmap.argtypes = [vp, sz, i32, c.c_uint64, vp, sz, c.POINTER(sz)]
+        L.bfsc_ref_decompress_to_frontier.restype = i32
+        L.bfsc_ref_decompress_to_frontier.argtypes = [vp, sz, i32, c.c_uint64, vp, vp, sz, c.POINTER(sz)]
         _lib = L
     return _lib
 
@@ -239,6 +241,21 @@ def decompress_to_bitmap(stream: np.ndarray, W: int, bitmap: np.ndarray, n_bits:
     n = ctypes.c_size_t(0)
     rc = lib().bfsc_ref_decompress_to_bitmap(_p(stream), len(stream), W, ctypes.c_uint64(id_base), _p(bitmap), n_bits,
                                              ctypes.byref(n))
+    if rc:
+        raise OracleError(rc)
+    return n.value
+
+
+def decompress_to_frontier(stream: np.ndarray, W: int, frontier: np.ndarray, visited: np.ndarray, n_bits: int,
+                           id_base: int = 0) -> int:
+    """Algorithm 4 lines 10-13 on bitmaps (uint32 words, both modified in place): frontier |= decoded & ~visited,
+    visited |= decoded. Returns the number of IDs decoded."""
+    stream = np.ascontiguousarray(stream, dtype=np.uint8)
+    for b in (frontier, visited):
+        assert b.dtype == np.uint32 and b.flags["C_CONTIGUOUS"] and len(b) * 32 >= n_bits
+    n = ctypes.c_size_t(0)
+    rc = lib().bfsc_ref_decompress_to_frontier(_p(stream), len(stream), W, ctypes.c_uint64(id_base), _p(frontier),
+                                               _p(visited), n_bits, ctypes.byref(n))
     if rc:
         raise OracleError(rc)
     return n.value

@@ -353,6 +353,39 @@ int bfsc_ref_decompress_to_bitmap(const uint8_t *in, size_t in_bytes, int W, uin
     return rc;
 }
 
+/* Algorithm 4, lines 10-13, with the frontier t and the visited set of Pi as bitmaps:
+ *   line 10  t <- decompress(t'')          the decoded IDs
+ *   line 11  t <- t (.) not Pi             keep those not visited yet
+ *   line 12  Pi <- Pi + t                  mark them visited
+ *   line 13  f <- t                        they are (part of) the next frontier: OR-ed into `frontier`
+ * One ID at a time, in stream order; an ID met a second time is visited by then and changes nothing. */
+int bfsc_ref_decompress_to_frontier(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,
+                                    uint32_t *frontier, uint32_t *visited, size_t n_bits, size_t *n_ids) {
+    if ((W != 32 && W != 64) || !in || !n_ids || !frontier || !visited) return BFSC_REF_ERR_INVALID_ARG;
+    int mode; uint64_t n, total, nb;
+    int rc = parse_header(in, in_bytes, W, &mode, &n, &total, &nb);
+    if (rc) return rc;
+    void *ids = malloc((n ? n : 1) * (size_t)(W / 8));
+    if (!ids) return BFSC_REF_ERR_INVALID_ARG;
+    size_t got = 0;
+    rc = bfsc_ref_decompress(in, in_bytes, W, ids, n, &got);
+    for (size_t i = 0; !rc && i < got; i++) {
+        uint64_t v = (load_id(ids, i, W) - id_base) & wmask(W);
+        if (v >= n_bits) rc = BFSC_REF_ERR_DST_TOO_SMALL;
+    }
+    for (size_t i = 0; !rc && i < got; i++) {
+        uint64_t v = (load_id(ids, i, W) - id_base) & wmask(W);
+        uint32_t bit = 1u << (v % 32);
+        if (!(visited[v / 32] & bit)) {                          /* line 11 */
+            visited[v / 32] |= bit;                              /* line 12 */
+            frontier[v / 32] |= bit;                             /* line 13 */
+        }
+    }
+    free(ids);
+    if (!rc) *n_ids = got;
+    return rc;
+}
+
 /* ------------------------------------------------------------------------------------
  * Multi-threaded drivers (bench.py cpu_baseline only). Work unit = one 128-ID block, run
  * through the very same scalar routines; three phases: block sizes -> serial prefix ->

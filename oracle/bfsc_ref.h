@@ -111,6 +111,10 @@ int bfsc_ref_compress_bitmap(int codec, const uint32_t *bitmap, size_t n_bits, u
                              size_t raw_threshold_bytes, uint8_t *out, size_t out_capacity, size_t *out_bytes);
 int bfsc_ref_decompress_to_bitmap(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,
                                   uint32_t *bitmap, size_t n_bits, size_t *n_ids);
+/* Algorithm 4 lines 10-13 on bitmaps: for the decoded IDs S,
+ * frontier |= S \ visited and visited |= S (FORMAT.md §9, last item). Nothing is changed on an error. */
+int bfsc_ref_decompress_to_frontier(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,
+                                    uint32_t *frontier, uint32_t *visited, size_t n_bits, size_t *n_ids);
 
 /* Multi-threaded drivers used only by bench.py's cpu_baseline leg: independent buffers
  * are spread over `threads` pthreads; each buffer goes through the same scalar routines

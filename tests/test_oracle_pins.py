@@ -360,3 +360,34 @@ def test_bitmap_matches_id_list_and_round_trips(oracle_mod):
                     with pytest.raises(oracle_mod.OracleError) as ei:
                         oracle_mod.decompress_to_bitmap(s, W, small, int(ids[-1]) - id_base, id_base=id_base)   # last ID does not fit
                     assert ei.value.code == oracle_mod.ERR_DST_TOO_SMALL and np.array_equal(small, old)
+
+
+def test_frontier_update_hand_example_and_set_algebra(oracle_mod):
+    """FORMAT.md §9, last item (Algorithm 4 lines 10-13). Hand example: IDs {3, 5, 5, 40}, visited =
+    {5, 6}, frontier = {0}: line 11 keeps {3, 40}, line 12 gives visited {3, 5, 6, 40}, line 13 frontier {0, 3, 40}.
+    Then the set identities on random inputs, with numpy sets: frontier' = frontier | (S & ~visited),
+    visited' = visited | S; the visited bits of other IDs and an out-of-range ID leave everything alone."""
+    s = oracle_mod.compress(np.array([3, 5, 5, 40], dtype=np.uint32), 0)
+    vis = np.array([(1 << 5) | (1 << 6), 0], dtype=np.uint32)
+    fr = np.array([1, 0], dtype=np.uint32)
+    assert oracle_mod.decompress_to_frontier(s, 32, fr, vis, 64) == 4
+    assert fr.tolist() == [1 | (1 << 3), 1 << 8] and vis.tolist() == [(1 << 3) | (1 << 5) | (1 << 6), 1 << 8]
+    rng = np.random.default_rng(11)
+    for W in (32, 64):
+        for n_bits, dens, id_base in ((1, 1.0, 0), (33, 0.5, 7), (5000, 0.3, 12345), (70000, 0.05, 0)):
+            bits = rng.random(n_bits) < dens
+            ids = (np.nonzero(bits)[0].astype(np.uint64) + np.uint64(id_base)).astype(_dt(W))
+            S = np.packbits(np.concatenate([bits, np.zeros(-n_bits % 32, dtype=bool)]), bitorder="little").view(np.uint32).copy()
+            s = oracle_mod.compress(ids, 0)
+            tail = np.uint32((1 << ((n_bits - 1) % 32 + 1)) - 1)
+            vis0 = rng.integers(0, 1 << 32, size=len(S), dtype=np.uint64).astype(np.uint32); vis0[-1] &= tail
+            fr0 = rng.integers(0, 1 << 32, size=len(S), dtype=np.uint64).astype(np.uint32); fr0[-1] &= tail
+            vis, fr = vis0.copy(), fr0.copy()
+            assert oracle_mod.decompress_to_frontier(s, W, fr, vis, n_bits, id_base=id_base) == len(ids)
+            assert np.array_equal(fr, fr0 | (S & ~vis0)) and np.array_equal(vis, vis0 | S)
+            if len(ids) and n_bits > 1:
+                vis, fr = vis0.copy(), fr0.copy()
+                with pytest.raises(oracle_mod.OracleError) as ei:
+                    oracle_mod.decompress_to_frontier(s, W, fr, vis, int(ids[-1]) - id_base, id_base=id_base)
+                assert ei.value.code == oracle_mod.ERR_DST_TOO_SMALL
+                assert np.array_equal(fr, fr0) and np.array_equal(vis, vis0)
