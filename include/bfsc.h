@@ -191,7 +191,13 @@ bfsc_status bfsc_decompress_batch(const void* d_in, const uint64_t* d_in_offsets
  *   out_capacity >= bfsc_compress_bound(number of set bits) (n_bits is always enough); workspace:
  *   bfsc_bitmap_workspace_bytes(n_bits, t).
  * bfsc_decompress_to_bitmap: ORs the bits of the stream's IDs into d_bitmap (old bits stay); *d_n_ids = IDs decoded.
- *   An ID outside [id_base, id_base + n_bits): BFSC_ERR_DST_TOO_SMALL in *d_status (bits of other IDs may have been set). */
+ *   An ID outside [id_base, id_base + n_bits): BFSC_ERR_DST_TOO_SMALL in *d_status (bits of other IDs may have been set).
+ * bfsc_decompress_to_frontier: Algorithm 4 lines 10-13 (t <- decompress(t''), t <- t (.) not Pi,
+ *   Pi <- Pi + t, f <- t) in the decode kernel, with the next frontier and the visited set of Pi as two bitmaps of the
+ *   same geometry: every decoded ID that is not in d_visited yet is set in d_visited and in d_frontier (both OR-ed:
+ *   old bits stay); an ID that is visited already changes nothing. d_frontier != d_visited. Several calls of one BFS
+ *   level (one per received stream) may run concurrently on the same pair of bitmaps: the updates are atomic and a
+ *   vertex received twice enters the frontier once. Same error behaviour as bfsc_decompress_to_bitmap. */
 size_t bfsc_bitmap_workspace_bytes(size_t n_bits, bfsc_dtype t);
 bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_bitmap, size_t n_bits, uint64_t id_base, bfsc_dtype t,
                                  size_t raw_threshold_bytes, void* d_out, size_t out_capacity, uint64_t* d_out_bytes,
@@ -199,6 +205,9 @@ bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_bitmap, siz
 bfsc_status bfsc_decompress_to_bitmap(const void* d_in, size_t in_bytes, bfsc_dtype t, uint64_t id_base,
                                       uint32_t* d_bitmap, size_t n_bits, uint64_t* d_n_ids,
                                       void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream);
+bfsc_status bfsc_decompress_to_frontier(const void* d_in, size_t in_bytes, bfsc_dtype t, uint64_t id_base,
+                                        uint32_t* d_frontier, uint32_t* d_visited, size_t n_bits, uint64_t* d_n_ids,
+                                        void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream);
 
 /* End-to-end convenience calls with HOST buffers (pinned memory recommended): copy in,
  * run the device call above, copy the result out, synchronise the stream. d_scratch is a

@@ -77,7 +77,7 @@ __device__ __forceinline__ bool patch_rows(const unsigned char* __restrict__ e, 
 template <int W, bool kBits = false>
 __device__ __forceinline__ void scan_store(typename IdT<W>::T d[4], typename IdT<W>::T base,
                                            typename IdT<W>::T* __restrict__ x, int m,
-                                           const BitSink& sink = BitSink{nullptr, 0, 0, nullptr}) {
+                                           const BitSink& sink = BitSink{nullptr, 0, 0, nullptr, nullptr}) {
     using T = typename IdT<W>::T;
     const int lane = lane_id();
     d[1] += d[0]; d[2] += d[1]; d[3] += d[2];

@@ -731,7 +731,7 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
 static bfsc_status decode_common(const void* d_in, const uint64_t* d_in_off, size_t in_single, size_t n_buf,
                                  bfsc_dtype t, void* d_ids, size_t ids_cap, uint64_t* d_id_off, uint64_t* d_n_ids,
                                  void* ws, size_t ws_bytes, uint32_t* d_status, void* stream,
-                                 BitSink sink = BitSink{nullptr, 0, 0, nullptr}) {
+                                 BitSink sink = BitSink{nullptr, 0, 0, nullptr, nullptr}) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
     if (!d_in || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
     if (!d_ids && ids_cap && !sink.bm) return BFSC_ERR_INVALID_ARG;
@@ -771,5 +771,16 @@ extern "C" bfsc_status bfsc_decompress_to_bitmap(const void* d_in, size_t in_byt
                                                  void* cuda_stream) {
     if (!d_n_ids || !d_bitmap || ((uintptr_t)d_bitmap & 15) || n_bits > (1ull << 32)) return BFSC_ERR_INVALID_ARG;
     return bfsc::decode_common(d_in, nullptr, in_bytes, 1, t, nullptr, ~(size_t)0, nullptr, d_n_ids, d_workspace,
-                               workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_bitmap, id_base, n_bits, d_status});
+                               workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_bitmap, id_base, n_bits, d_status, nullptr});
+}
+
+extern "C" bfsc_status bfsc_decompress_to_frontier(const void* d_in, size_t in_bytes, bfsc_dtype t, uint64_t id_base,
+                                                   uint32_t* d_frontier, uint32_t* d_visited, size_t n_bits,
+                                                   uint64_t* d_n_ids, void* d_workspace, size_t workspace_bytes,
+                                                   uint32_t* d_status, void* cuda_stream) {
+    if (!d_n_ids || !d_frontier || !d_visited || d_frontier == d_visited || ((uintptr_t)d_frontier & 15) ||
+        ((uintptr_t)d_visited & 15) || n_bits > (1ull << 32))
+        return BFSC_ERR_INVALID_ARG;
+    return bfsc::decode_common(d_in, nullptr, in_bytes, 1, t, nullptr, ~(size_t)0, nullptr, d_n_ids, d_workspace,
+                               workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_frontier, id_base, n_bits, d_status, d_visited});
 }

@@ -94,7 +94,7 @@ template <int W, bool kWin, bool kBits = false>
 __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, uint32_t b,
                                                  const typename IdT<W>::T* __restrict__ tab, bool patch,
                                                  typename IdT<W>::T base, typename IdT<W>::T* __restrict__ x, int m, int l,
-                                                 const BitSink& sink = BitSink{nullptr, 0, 0, nullptr}) {
+                                                 const BitSink& sink = BitSink{nullptr, 0, 0, nullptr, nullptr}) {
     using T = typename IdT<W>::T;
     const uint32_t mask = (1u << b) - 1u;
     uint32_t bit = (uint32_t)l * b;

@@ -886,3 +886,57 @@ def test_raw_fallback_batch_is_unsupported_and_bitmap_follows_the_rule(B, oracle
         for n_bits, dens in ((0, 0.0), (5000, 0.0002), (5000, 0.001), (1 << 20, 0.000003), (1 << 20, 0.3)):
             bm = streams.frontier_bitmap(n_bits, dens, seed=9)
             run_bitmap(B, oracle_mod, bm, n_bits, W, codec=PFOR | FALLBACK)
+
+
+# ---- FORMAT.md §9, last item: decode into the next frontier against the visited bitmap (Algorithm 4 lines 10-13) ----
+def _frontier_case(B, oracle_mod, ids_np, W, n_bits, id_base, thr=0, seed=0, expect_ok=True):
+    dev = torch.device("cuda")
+    stream = oracle_mod.compress(ids_np, thr)
+    words = max(4, ((n_bits + 31) // 32 + 3) // 4 * 4)
+    vis0 = streams.frontier_bitmap(words * 32, 0.4, seed=seed + 1)[:words].numpy().view(np.uint32).copy()
+    fr0 = streams.frontier_bitmap(words * 32, 0.1, seed=seed + 2)[:words].numpy().view(np.uint32).copy()
+    d_in = torch.from_numpy(np.concatenate([stream, np.zeros(16, np.uint8)])).to(dev)
+    d_vis = torch.from_numpy(vis0.view(np.int32).copy()).to(dev)
+    d_fr = torch.from_numpy(fr0.view(np.int32).copy()).to(dev)
+    n_out = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    ws = torch.empty(B.workspace_bytes(max(len(ids_np), 1), 1, W), dtype=torch.uint8, device=dev)
+    B.decompress_to_frontier(d_in, len(stream), W, id_base, d_fr, d_vis, n_bits, n_out, ws, status)
+    torch.cuda.synchronize()
+    vis, fr = vis0.copy(), fr0.copy()
+    try:
+        n_ref = oracle_mod.decompress_to_frontier(stream, W, fr, vis, n_bits, id_base)
+        ref_ok = True
+    except oracle_mod.OracleError as e:
+        assert e.code == 2
+        ref_ok = False
+    assert ref_ok == expect_ok
+    if not ref_ok:
+        assert int(status.item()) == 2                 # DST_TOO_SMALL; the bitmaps may hold the bits of other IDs
+        return
+    assert int(status.item()) == 0 and int(n_out.item()) == n_ref
+    assert np.array_equal(d_vis.cpu().numpy().view(np.uint32), vis), "visited bitmap differs from the oracle"
+    assert np.array_equal(d_fr.cpu().numpy().view(np.uint32), fr), "frontier bitmap differs from the oracle"
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_decompress_to_frontier(B, oracle_mod, W):
+    dt = np.uint32 if W == 32 else np.uint64
+    rng = np.random.default_rng(W)
+    bases = (0, 777, (1 << W) - 50)
+    for k, (n, mean) in enumerate(((0, 1.0), (1, 1.0), (127, 2.0), (128, 2.0), (1000, 3.0), (128 * 64 * 3 + 5, 2.0), (50000, 40.0), (3000, 5000.0))):
+        rel = _np(streams.gap_stream(n, mean, seed=40 + k, W=W), W).astype(np.uint64) if n else np.zeros(0, np.uint64)
+        rel = rel - (rel[0] if n else 0)                                   # bit indices from 0
+        n_bits = int(rel[-1]) + 1 + k if n else 100
+        id_base = bases[k % 3]
+        ids = ((rel + np.uint64(id_base)) & np.uint64((1 << W) - 1 if W < 64 else 0xFFFFFFFFFFFFFFFF)).astype(dt)
+        _frontier_case(B, oracle_mod, ids, W, n_bits, id_base, seed=k)
+        if n > 200:
+            _frontier_case(B, oracle_mod, ids, W, n_bits, id_base, thr=1 << 30, seed=k)          # a RAW stream
+            _frontier_case(B, oracle_mod, ids, W, n_bits - k - 1, id_base, seed=k, expect_ok=False)   # the last ID does not fit
+    # IDs in any order and more than once (the codec takes any sequence): a vertex received twice counts once
+    pool = rng.integers(0, 5000, size=20000, dtype=np.uint64)
+    _frontier_case(B, oracle_mod, (pool + np.uint64(9)).astype(dt), W, 5000, 9, seed=99)
+    # a 2^22-bit level: many tiles, all warps
+    bits = rng.random(1 << 22) < 0.3
+    _frontier_case(B, oracle_mod, np.nonzero(bits)[0].astype(dt), W, 1 << 22, 0, seed=5)
