@@ -113,9 +113,7 @@ __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, ui
 #pragma unroll
     for (int i = 0; i < 8; i++) {
         const uint32_t k0 = bit >> 5, sh = bit & 31u;
-        const uint4 lo = P[k0];
-        uint4 hi = lo;                                                   // the next chunk only if the value straddles it
-        if (sh + b > 32u) hi = P[k0 + 1];
+        const uint4 lo = P[k0], hi = P[k0 + 1];                          // (loading hi only when a value straddles the chunk: +9 % instructions, same time)
         bit += 4u * b;
         T v0 = __funnelshift_r(lo.x, hi.x, sh) & mask, v1 = __funnelshift_r(lo.y, hi.y, sh) & mask;
         T v2 = __funnelshift_r(lo.z, hi.z, sh) & mask, v3 = __funnelshift_r(lo.w, hi.w, sh) & mask;
