@@ -267,6 +267,7 @@ __global__ void __launch_bounds__(1024) k_enc_planblocks(EncArgs a) {
 // calls) the stream header; barrier 2.
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPre = 2ull << 62, kValMask = (1ull << 62) - 1;
 constexpr unsigned long long kNoTile = ~0ull, kSkip = ~0ull;
+constexpr uint32_t kLateBit = 1u << 31;                  // in a stored key: the block is assembled by late_emit, not in an image buffer
 
 __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
     unsigned long long v;
@@ -711,7 +712,6 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     uint4* slot = area + raw_slot_chunk<W>(q);                           // staging: the quad's raw IDs
     unsigned char* ibuf = reinterpret_cast<unsigned char*>(area + Smem::kStageChunks);   // the warp's kNB image buffers
     const int j = warp * kQuadBlocks + q;
-    constexpr uint32_t kLateBit = 1u << 31;                              // in a stored key: assembled by late_emit
     mbar_wait(&mb_post[0], 0);                                           // the CTA's first tile is posted (by the prep warp)
     bool have = s_tile[0] != kNoTile;
     uint4* land = area + Smem::kStageChunks + kNB * Img::kBufChunks;      // bitmap source: the words of the warp's 8 blocks
@@ -917,6 +917,269 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
         const unsigned long long t = ok ? a.ws.hdr->total_out : 0ull;
         if (a.out_off) a.out_off[a.n_buf] = t;
         if (a.out_total) *a.out_total = t;
+    }
+}
+
+// ---- Small batches (a BFS level of up to ~1 MB): the WHOLE compress call in one launch of one thread-block cluster ----
+// kSmallCtas CTAs that the hardware schedules together, so that a CTA may wait for another one of the grid without any
+// residency assumption, and that exchange their tile sums through distributed shared memory instead of a look-back
+// through L2. Every CTA runs E0 for itself (the plan of up to kSmallMaxBuf buffers, tables in shared memory), then
+//   pass 1   E1 + E2 of its tiles (tile T = 8 r + cluster rank, r = 0 .. kSmallIters - 1): sizes in shared memory,
+//            tile sums written into every CTA of the cluster;                          -- cluster barrier --
+//            exclusive scan of the <= 32 tile sums (every CTA the same), scans inside the own tiles; the starts of
+//            the streams whose first block is in an own tile -> ws.stream_start, out_offsets;  -- cluster barrier --
+//   pass 2   E1 + E4 of its tiles (IDs staged again: they come from L2), blocks and directory entries written to
+//            their final place; stream headers, directory tails, RAW copies (E5) of its share of the streams.
+// No plan kernel, no look-back states, no ticket, no k_enc_streams: one launch latency instead of three.
+constexpr int kSmallCtas = 8;                            // portable cluster size
+constexpr int kSmallIters = 4;                           // tiles per CTA
+constexpr uint32_t kSmallMaxBuf = 1024;
+constexpr uint32_t kSmallMaxBlocks = kSmallCtas * kTileR * kSmallIters;      // 2048 blocks = 262144 IDs
+constexpr int kSmallThreads = kEncWorkers * 32;
+
+template <int W> struct SmallSmem {
+    static constexpr int kStageChunks = RawCfg<W>::kAreaChunks;              // per warp: staged raw IDs
+    static constexpr int kSlotChunks = 34;                                   // per quad: one block image (every block with 32-bit deltas fits: 16 + 16 * 32 + 16)
+    static constexpr int kWarpChunks = kStageChunks + kQuadBlocks * kSlotChunks;
+    static constexpr size_t kBytes = (size_t)kEncWorkers * kWarpChunks * 16;
+};
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {     // every thread of every CTA of the cluster; orders shared AND global memory
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void st_cluster_u32(uint32_t* local_ptr, uint32_t rank, uint32_t v) {   // the same variable in CTA `rank` of the cluster
+    const uint32_t la = (uint32_t)__cvta_generic_to_shared(local_ptr);
+    uint32_t ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(rank));
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(ra), "r"(v) : "memory");
+}
+
+template <int W>
+__global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
+    using T = typename IdT<W>::T;
+    using Smem = SmallSmem<W>;
+    constexpr unsigned long long E = W / 8;
+    extern __shared__ __align__(16) uint4 dyn_smem[];
+    __shared__ uint32_t s_first[kSmallMaxBuf + 1];                   // first block of every buffer (entry n_buf: total)
+    __shared__ unsigned long long s_fixed[kSmallMaxBuf + 1];         // exclusive prefix of the fixed bytes
+    __shared__ uint32_t s_key[kSmallIters][kTileR];                  // size<<14 | (64-b)<<7 | n_exc (| kLateBit), 0 = no block
+    __shared__ uint32_t s_off16[kSmallIters][kTileR];                // exclusive scan of the sizes inside the tile (16-B units)
+    __shared__ uint32_t s_buf[kSmallIters][kTileR];                  // buffer, valid IDs, first ID (element) of every own block
+    __shared__ int s_m[kSmallIters][kTileR];
+    __shared__ unsigned long long s_xoff[kSmallIters][kTileR];
+    __shared__ uint32_t s_sum[kSmallIters];                          // sums of the own tiles
+    __shared__ uint32_t s_tsum[kSmallCtas * kSmallIters];            // sums of ALL tiles (written by their CTAs), then their exclusive scan
+    __shared__ Scan2 sm[33];
+    __shared__ int bad;
+    pdl_wait();                                                      // the call before this one is complete (workspace, inputs)
+    pdl_launch_dependents();
+    const uint32_t rank = cluster_ctarank();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, q = lane >> 2, l = lane & 3;
+    const T* ids = reinterpret_cast<const T*>(a.ids);
+
+    // ---- E0, by every CTA for itself
+    if (threadIdx.x == 0) bad = 0;
+    if (threadIdx.x < kSmallIters) s_sum[threadIdx.x] = 0;
+    __syncthreads();
+    {
+        constexpr int kIpt = kSmallMaxBuf / kSmallThreads;           // 4
+        Scan2 v[kIpt], sum{0, 0};
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = threadIdx.x * kIpt + u;
+            v[u] = Scan2{0, 0};
+            if (i < a.n_buf) {
+                const unsigned long long o0 = a.in_off[i], o1 = a.in_off[i + 1];
+                if (o1 < o0) bad = 1;
+                const unsigned long long n = o1 - o0;
+                const bool raw = n * E < a.thr;                      // FORMAT.md §1 (L1311)
+                const unsigned long long nb = raw ? 0ull : (n + kBlk - 1) / kBlk;
+                v[u].a = nb;
+                v[u].b = raw ? 32ull + ((n * E + 15ull) & ~15ull) : 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull);
+            }
+            sum.a += v[u].a; sum.b += v[u].b;
+        }
+        Scan2 tot;
+        Scan2 ex = block_scan_excl2(sum, &tot, sm);
+#pragma unroll
+        for (int u = 0; u < kIpt; u++) {
+            const uint32_t i = threadIdx.x * kIpt + u;
+            if (i < a.n_buf) { s_first[i] = (uint32_t)min(ex.a, 0xffffffffull); s_fixed[i] = ex.b; }
+            ex.a += v[u].a; ex.b += v[u].b;
+        }
+        if (threadIdx.x == 0) { s_first[a.n_buf] = (uint32_t)min(tot.a, 0xffffffffull); s_fixed[a.n_buf] = tot.b; }
+        __syncthreads();
+        if (bad || tot.a > a.ws.blk_cap || tot.a > kSmallMaxBlocks) {        // (the same decision in every CTA of the cluster)
+            if (rank == 0 && threadIdx.x == 0) set_status(a.status, BFSC_ERR_INVALID_ARG);
+            for (uint32_t i = rank * kSmallThreads + threadIdx.x; i <= a.n_buf; i += kSmallCtas * kSmallThreads) a.out_off[i] = 0;
+            return;
+        }
+    }
+    const uint32_t total = s_first[a.n_buf];
+    const int R = (int)((total + kSmallCtas * kTileR - 1) / (kSmallCtas * kTileR));      // tiles per CTA that hold blocks
+    uint4* area = dyn_smem + warp * Smem::kWarpChunks;
+    uint4* slot = area + raw_slot_chunk<W>(q);
+    unsigned char* img = reinterpret_cast<unsigned char*>(area + Smem::kStageChunks) + q * (Smem::kSlotChunks * 16);
+    const int j = warp * kQuadBlocks + q;                            // the quad's block inside a tile
+
+    // ---- pass 1: E1 + E2
+    for (int r = 0; r < R; r++) {
+        const uint32_t g = (uint32_t)r * (kSmallCtas * kTileR) + rank * kTileR + (uint32_t)j;
+        int m = 0; uint32_t i = 0; unsigned long long xoff = 0;
+        if (g < total) {
+            i = bisect_first(s_first, a.n_buf, g);
+            const unsigned long long o0 = a.in_off[i], n = a.in_off[i + 1] - o0, k = g - s_first[i];
+            m = (int)min((unsigned long long)kBlk, n - kBlk * k);
+            xoff = o0 + kBlk * k;
+        }
+        if (l == 0) { s_buf[r][j] = i; s_m[r][j] = m; s_xoff[r][j] = xoff; }
+        quad_prefetch<W>(slot, ids + xoff, m);
+        cp_async_wait_all();
+        __syncwarp();
+        const T* raw = reinterpret_cast<const T*>(slot) + (reinterpret_cast<uintptr_t>(ids + xoff) & 15) / sizeof(T);
+        uint32_t d[32];
+        bool wide_lane = false, wide = false;
+        col_deltas<W>(raw, m, d, wide_lane);
+        if constexpr (W == 64) wide = __any_sync(kFull, wide_lane);
+        uint32_t key;
+        if (!wide) key = a.codec == BFSC_CODEC_BP128 ? quad_max_width_key(d) : quad_choose_b<W>(d);
+        else key = wide_choose_b(reinterpret_cast<const uint64_t*>(raw), m, reinterpret_cast<uint32_t*>(img), a.codec == BFSC_CODEC_BP128);
+        if (m <= 0) key = 0;
+        const bool late = key != 0 && (wide || (key >> 14) > (uint32_t)(Smem::kSlotChunks * 16));
+        if (l == 0) s_key[r][j] = key | (late ? kLateBit : 0u);
+        uint32_t z = l == 0 ? key >> 18 : 0u;
+        z += __shfl_xor_sync(kFull, z, 4); z += __shfl_xor_sync(kFull, z, 8); z += __shfl_xor_sync(kFull, z, 16);
+        if (lane == 0) atomicAdd(&s_sum[r], z);
+        __syncwarp();                                                // the staged IDs are consumed (the next tile overwrites them)
+    }
+    __syncthreads();
+    if (threadIdx.x < kSmallIters * kSmallCtas) {                    // thread (r, c): the sum of the own tile r -> CTA c
+        const int r = threadIdx.x / kSmallCtas, c = threadIdx.x % kSmallCtas;
+        st_cluster_u32(&s_tsum[r * kSmallCtas + (int)rank], (uint32_t)c, r < R ? s_sum[r] : 0u);
+    }
+    cluster_sync_all();
+    // ---- E3: every CTA scans the tile sums (tile T = 8 r + c, T in block order) and its own tiles
+    if (warp == 0) {
+        const uint32_t v = lane < kSmallCtas * kSmallIters ? s_tsum[lane] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        if (lane < kSmallCtas * kSmallIters) s_tsum[lane] = inc - v;             // exclusive
+        if (lane == 31) s_sum[0] = inc;                                          // grand total (16-B units); the own sums are no longer needed
+    }
+    if (warp >= 1 && warp <= R) {                                                // warp r + 1: the 64 sizes of own tile r (R <= 4 < 8 warps)
+        const int r = warp - 1;
+        const uint32_t k0 = s_key[r][2 * lane] & ~kLateBit, k1 = s_key[r][2 * lane + 1] & ~kLateBit;
+        const uint32_t own = (k0 >> 18) + (k1 >> 18);
+        uint32_t inc = own;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        s_off16[r][2 * lane] = inc - own;
+        s_off16[r][2 * lane + 1] = inc - own + (k0 >> 18);
+    }
+    __syncthreads();
+    const unsigned long long grand16 = s_sum[0];
+    const unsigned long long total_out = s_fixed[a.n_buf] + 16ull * grand16;
+    if (total_out > a.out_cap) {                                                 // (the same decision in every CTA)
+        if (rank == 0 && threadIdx.x == 0) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+        for (uint32_t i = rank * kSmallThreads + threadIdx.x; i <= a.n_buf; i += kSmallCtas * kSmallThreads) a.out_off[i] = 0;
+        return;
+    }
+    // scan value G at block g of one of the own tiles (16-B units of block bytes before it)
+    auto scan_at = [&](uint32_t g) -> unsigned long long {
+        const uint32_t r = g / (kSmallCtas * kTileR), jj = g % kTileR;
+        return (unsigned long long)s_tsum[r * kSmallCtas + rank] + s_off16[r][jj];
+    };
+    // stream i starts at fixed_prefix[i] + 16 G(first block of i); streams without blocks: at the next block, or at the
+    // end (G = grand total: rank 0). The CTA that owns that block publishes the start.
+    for (uint32_t i = threadIdx.x; i < a.n_buf; i += kSmallThreads) {
+        const uint32_t g = s_first[i];
+        unsigned long long S = ~0ull;
+        if (g >= total) { if (rank == 0) S = s_fixed[i] + 16ull * grand16; }
+        else if ((g / kTileR) % kSmallCtas == rank) S = s_fixed[i] + 16ull * scan_at(g);
+        if (S != ~0ull) { a.ws.stream_start[i] = S; a.out_off[i] = S; }
+    }
+    if (rank == 0 && threadIdx.x == 0) { a.ws.stream_start[a.n_buf] = total_out; a.out_off[a.n_buf] = total_out; }
+    __threadfence();
+    cluster_sync_all();
+
+    // ---- pass 2: E1 + E4, blocks and directory entries to their final place
+    for (int r = 0; r < R; r++) {
+        const uint32_t g = (uint32_t)r * (kSmallCtas * kTileR) + rank * kTileR + (uint32_t)j;
+        const int m = s_m[r][j];
+        const uint32_t i = s_buf[r][j];
+        const unsigned long long xoff = s_xoff[r][j];
+        if (R > 1) {                                                 // (R == 1: the tile is still staged)
+            quad_prefetch<W>(slot, ids + xoff, m);
+            cp_async_wait_all();
+            __syncwarp();
+        }
+        const T* raw = reinterpret_cast<const T*>(slot) + (reinterpret_cast<uintptr_t>(ids + xoff) & 15) / sizeof(T);
+        const uint32_t stored = s_key[r][j], key = stored & ~kLateBit;
+        const bool late = (stored & kLateBit) != 0, fast = key != 0 && !late;
+        const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
+        unsigned long long at = 0;
+        if (key != 0) {
+            at = s_fixed[i + 1] + 16ull * scan_at(g);
+            if (l == 0) {                                            // directory entry (FORMAT.md §1)
+                const unsigned long long S = __ldcg(&a.ws.stream_start[i]);
+                reinterpret_cast<uint32_t*>(a.out + S + 32)[g - s_first[i]] = (uint32_t)((at - S) >> 4);
+            }
+        }
+        uint32_t d[32];
+        bool wide_lane = false;
+        const T base = col_deltas<W>(raw, m, d, wide_lane);
+        if (__any_sync(kFull, fast && n_exc > 0)) col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
+        if (fast) {
+            if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
+            if (l == 0) {                                            // block header (FORMAT.md §2)
+                reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
+                reinterpret_cast<unsigned long long*>(img)[1] = (unsigned long long)(b | (n_exc << 8));
+            }
+        }
+        __syncwarp();
+        if (fast) {
+            const uint4* src = reinterpret_cast<const uint4*>(img);
+            uint4* dst = reinterpret_cast<uint4*>(a.out + at);
+            for (uint32_t c = l; c < (key >> 18); c += 4) __stcs(dst + c, src[c]);
+        }
+        if (__any_sync(kFull, late)) late_emit<W>(ids + xoff, m, key, late ? a.out + at : nullptr);
+        __syncwarp();                                                // image and staged IDs are free again
+    }
+
+    // ---- stream headers, directory tails, E5 (RAW copies): a warp per stream, the streams dealt round the cluster
+    for (uint32_t i = rank * kEncWorkers + warp; i < a.n_buf; i += kSmallCtas * kEncWorkers) {
+        const unsigned long long s0 = __ldcg(&a.ws.stream_start[i]), s1 = __ldcg(&a.ws.stream_start[i + 1]);
+        const unsigned long long o0 = a.in_off[i], n = a.in_off[i + 1] - o0, tot = s1 - s0;
+        const bool raw_s = n * E < a.thr;
+        unsigned char* s = a.out + s0;
+        if (lane == 0) {
+            const unsigned long long nb = s_first[i + 1] - s_first[i];
+            uint4 h0, h1;
+            h0.x = 0x43534642u;                                      // "BFSC"
+            h0.y = 1u | ((uint32_t)W << 8) | ((raw_s ? 0u : a.codec) << 16);
+            h0.z = (uint32_t)n; h0.w = (uint32_t)(n >> 32);
+            h1.x = (uint32_t)tot; h1.y = (uint32_t)(tot >> 32);
+            h1.z = (uint32_t)nb; h1.w = 0;
+            reinterpret_cast<uint4*>(s)[0] = h0;
+            reinterpret_cast<uint4*>(s)[1] = h1;
+            if (!raw_s) {                                            // dir[nb] and the zero pad
+                uint32_t* dir = reinterpret_cast<uint32_t*>(s + 32);
+                dir[nb] = (uint32_t)(tot >> 4);
+                for (unsigned long long x = nb + 1; x < ((nb + 1 + 3) & ~3ull); x++) dir[x] = 0;
+            }
+        }
+        if (raw_s) {                                                 // E5: verbatim copy + zero pad
+            const T* x = ids + o0;
+            T* y = reinterpret_cast<T*>(s + 32);
+            const unsigned long long padded = (tot - 32) / E;
+            for (unsigned long long t = lane; t < padded; t += 32) y[t] = t < n ? x[t] : (T)0;
+        }
     }
 }
 
@@ -1199,6 +1462,19 @@ static int enc_ctas_per_sm(int device) {
 }
 
 template <int W>
+static bool enc_small_init(int device) {                 // once per device: the small-batch kernel's dynamic shared memory
+    static std::mutex mu;
+    static bool done[kMaxDevices] = {};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!done[device]) {
+        if (cudaFuncSetAttribute(k_enc_small<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SmallSmem<W>::kBytes) != cudaSuccess)
+            return false;
+        done[device] = true;
+    }
+    return true;
+}
+
+template <int W>
 static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     constexpr size_t kSmem = EncSmem<W>::kBytes;
     DeviceInfo dev;
@@ -1213,6 +1489,24 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         const unsigned long long n_tiles = ((a_in.n_single + kBlk - 1) / kBlk + kTileR - 1) / kTileR;
         if (!degenerate && n_tiles > a_in.ws.tile_cap) return BFSC_ERR_INVALID_ARG;          // workspace too small
         if (n_tiles < (unsigned long long)grid) grid = n_tiles ? (int)n_tiles : 1;
+    }
+    if (!single && a_in.n_buf <= kSmallMaxBuf && a_in.ws.blk_cap <= kSmallMaxBlocks) {
+        // a small batch (both bounds known on the host: buffer count, and blocks by the workspace size the caller derived
+        // from the total ID count): one launch of one cluster
+        if (!enc_small_init<W>(dev.device)) return BFSC_ERR_CUDA;
+        EncArgs a = a_in;
+        a.grid = kSmallCtas;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(kSmallCtas); cfg.blockDim = dim3(kSmallThreads);
+        cfg.dynamicSmemBytes = SmallSmem<W>::kBytes; cfg.stream = s;
+        cudaLaunchAttribute at[2];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        at[1].id = cudaLaunchAttributeClusterDimension;
+        at[1].val.clusterDim.x = kSmallCtas; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 2;
+        BFSC_LAUNCH(cudaLaunchKernelEx(&cfg, k_enc_small<W>, a));
+        return BFSC_OK;
     }
     if (!single && (unsigned long long)grid > a_in.ws.tile_cap) grid = (int)a_in.ws.tile_cap;   // (tile_cap >= 2: no more tiles than that)
     EncArgs a = a_in;

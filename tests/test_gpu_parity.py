@@ -940,3 +940,64 @@ def test_decompress_to_frontier(B, oracle_mod, W):
     # a 2^22-bit level: many tiles, all warps
     bits = rng.random(1 << 22) < 0.3
     _frontier_case(B, oracle_mod, np.nonzero(bits)[0].astype(dt), W, 1 << 22, 0, seed=5)
+
+
+# ---- the one-launch cluster kernel of small batches (k_enc_small: <= 1024 buffers, <= 2048 blocks by the workspace size) ----
+@pytest.mark.parametrize("W", [32, 64])
+def test_small_batch_cluster_kernel_boundaries(B, oracle_mod, W):
+    """Batches around the limits of the small-batch path and inside it: 1 .. 4 tiles per CTA, exactly 2048 blocks and one
+    more (the general path), 1024 buffers and 1025, empty / RAW / one-ID buffers between full ones, buffers at every
+    element alignment, outliers (exceptions), incompressible blocks (largest images), u64 deltas over 2^32 (the wide
+    path), both encoder rules, thresholds 0 and 1 KB."""
+    g = torch.Generator().manual_seed(W)
+    cases = []
+    for nblk in (1, 63, 64, 65, 511, 512, 513, 1024, 1536, 2047, 2048, 2049):           # one buffer of nblk blocks (ragged tail)
+        cases.append(torch.tensor([128 * nblk - 5]))
+    cases.append(torch.randint(0, 300, (1024,), generator=g))                               # 1024 small buffers
+    cases.append(torch.randint(0, 300, (1025,), generator=g))                               # one too many: the general path
+    cases.append(torch.tensor([0, 0, 1, 0, 129, 0, 0, 127, 128, 0, 5000, 1, 1, 0, 255, 256, 257, 0]))
+    cases.append(torch.tensor([128 * 3 + e for e in range(1, 40)]))                        # every alignment
+    cases.append(torch.randint(100, 3000, (100,), generator=g))                             # ~ 1200 blocks in 100 buffers
+    for ci, counts in enumerate(cases):
+        ids, off = streams.batch_of_streams(counts, 2.0 if ci % 2 else 300.0, seed=60 + ci, W=W)
+        ids = ids.clone()
+        n = ids.numel()
+        if n > 4000:                                                                         # outliers and an incompressible stretch
+            sel = torch.rand(n, generator=g) < 0.01
+            ids[sel] += 1 << 20
+            lo = n // 3
+            ids[lo:lo + 700] = torch.randint(-(2 ** 31), 2 ** 31 - 1, (700,), generator=g, dtype=torch.int64).to(ids.dtype) if W == 32 \
+                else torch.randint(-(2 ** 62), 2 ** 62, (700,), generator=g, dtype=torch.int64)
+        for thr in (0, 1024):
+            for codec in CODECS:
+                run_batch(B, oracle_mod, ids, off, W, thr, codec=codec)
+
+
+def test_small_batch_cluster_kernel_errors(B):
+    dev = torch.device("cuda")
+    counts = torch.tensor([1000, 0, 77, 4096, 129])
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=7, W=32)
+    n, n_buf = ids.numel(), counts.numel()
+    d_ids, d_off = ids.to(dev), off.to(dev)
+    ws = torch.empty(B.workspace_bytes(n, n_buf, 32), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    out_off = torch.full((n_buf + 1,), -1, dtype=torch.int64, device=dev)
+    small = torch.full((1024,), 0xAB, dtype=torch.uint8, device=dev)                        # far too small an output buffer
+    B.compress_batch(d_ids, d_off, n_buf, 32, 0, small[:512], out_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_DST_TOO_SMALL and bool((out_off == 0).all()) and bool((small[512:] == 0xAB).all())
+    status.zero_()
+    bad = off.clone(); bad[2] = bad[1] - 1                                                   # decreasing offsets
+    out = torch.empty(B.batch_compress_bound(counts.tolist(), 32), dtype=torch.uint8, device=dev)
+    B.compress_batch(d_ids, bad.to(dev), n_buf, 32, 0, out, out_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_INVALID_ARG and bool((out_off == 0).all())
+    status.zero_()
+    counts2 = torch.tensor([1000, 0, 77, 4096, 129, 20000])                                 # 199 blocks
+    ids2, off2 = streams.batch_of_streams(counts2, 16.0, seed=7, W=32)
+    tiny_ws = torch.empty(B.workspace_bytes(200, 6, 32), dtype=torch.uint8, device=dev)      # a workspace for far fewer IDs: 64 blocks
+    out2 = torch.empty(B.batch_compress_bound(counts2.tolist(), 32), dtype=torch.uint8, device=dev)
+    out_off2 = torch.full((7,), -1, dtype=torch.int64, device=dev)
+    B.compress_batch(ids2.to(dev), off2.to(dev), 6, 32, 0, out2, out_off2, tiny_ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_INVALID_ARG and bool((out_off2 == 0).all())
