@@ -854,6 +854,19 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     if (lane == 0) bulk_wait_all();                                      // the bulk stores have left shared memory and landed
 }
 
+// E5 by one warp: y[0 .. padded) = x[0 .. n), zeros behind. Eight loads in flight per lane (a plain loop waits for every
+// load before it issues the next: a 1 KB RAW stream then costs eight round trips to L2).
+template <typename T>
+__device__ __forceinline__ void raw_copy(T* __restrict__ y, const T* __restrict__ x, unsigned long long n, unsigned long long padded, int lane) {
+    for (unsigned long long t0 = 0; t0 < padded; t0 += 32 * 8) {
+        T v[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) { const unsigned long long t = t0 + 32 * u + lane; v[u] = t < n ? x[t] : (T)0; }
+#pragma unroll
+        for (int u = 0; u < 8; u++) { const unsigned long long t = t0 + 32 * u + lane; if (t < padded) y[t] = v[u]; }
+    }
+}
+
 // ---- stream headers, directory tails, E5 raw passthrough, out_offsets (batch / degenerate calls) ----
 template <int W>
 __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
@@ -910,7 +923,7 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
             const T* x = reinterpret_cast<const T*>(a.ids) + buf_start(a, i);
             T* y = reinterpret_cast<T*>(s + 32);
             const unsigned long long padded = (total - 32) / E;
-            for (unsigned long long j = lane; j < padded; j += 32) y[j] = j < n ? x[j] : (T)0;
+            raw_copy<T>(y, x, n, padded, lane);
         }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -924,12 +937,13 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
 // kSmallCtas CTAs that the hardware schedules together, so that a CTA may wait for another one of the grid without any
 // residency assumption, and that exchange their tile sums through distributed shared memory instead of a look-back
 // through L2. Every CTA runs E0 for itself (the plan of up to kSmallMaxBuf buffers, tables in shared memory), then
-//   pass 1   E1 + E2 of its tiles (tile T = 8 r + cluster rank, r = 0 .. kSmallIters - 1): sizes in shared memory,
-//            tile sums written into every CTA of the cluster;                          -- cluster barrier --
-//            exclusive scan of the <= 32 tile sums (every CTA the same), scans inside the own tiles; the starts of
-//            the streams whose first block is in an own tile -> ws.stream_start, out_offsets;  -- cluster barrier --
-//   pass 2   E1 + E4 of its tiles (IDs staged again: they come from L2), blocks and directory entries written to
-//            their final place; stream headers, directory tails, RAW copies (E5) of its share of the streams.
+//   pass 1   E1 + E2 of its tiles (tile T = 8 r + cluster rank, r = 0 .. kSmallIters - 1): sizes in shared memory; the
+//            scan inside each own tile and its sum written into every CTA of the cluster;   -- ONE cluster barrier --
+//            exclusive scan of the <= 32 tile sums (every CTA the same): every CTA now has the output offset of every
+//            block and every stream of the batch in its own shared memory;
+//   pass 2   E1 + E4 of its tiles (IDs staged again if there are several: they come from L2), blocks and directory
+//            entries written to their final place; stream headers, directory tails, RAW copies (E5), out_offsets
+//            of its share of the streams.
 // No plan kernel, no look-back states, no ticket, no k_enc_streams: one launch latency instead of three.
 constexpr int kSmallCtas = 8;                            // portable cluster size
 constexpr int kSmallIters = 4;                           // tiles per CTA
@@ -968,7 +982,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
     __shared__ uint32_t s_first[kSmallMaxBuf + 1];                   // first block of every buffer (entry n_buf: total)
     __shared__ unsigned long long s_fixed[kSmallMaxBuf + 1];         // exclusive prefix of the fixed bytes
     __shared__ uint32_t s_key[kSmallIters][kTileR];                  // size<<14 | (64-b)<<7 | n_exc (| kLateBit), 0 = no block
-    __shared__ uint32_t s_off16[kSmallIters][kTileR];                // exclusive scan of the sizes inside the tile (16-B units)
+    __shared__ uint32_t s_off16[kSmallCtas * kSmallIters][kTileR];   // exclusive scan of the sizes inside EVERY tile of the cluster (16-B units; tile T = block / 64), each row written by its CTA
     __shared__ uint32_t s_buf[kSmallIters][kTileR];                  // buffer, valid IDs, first ID (element) of every own block
     __shared__ int s_m[kSmallIters][kTileR];
     __shared__ unsigned long long s_xoff[kSmallIters][kTileR];
@@ -1058,55 +1072,50 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         __syncwarp();                                                // the staged IDs are consumed (the next tile overwrites them)
     }
     __syncthreads();
-    if (threadIdx.x < kSmallIters * kSmallCtas) {                    // thread (r, c): the sum of the own tile r -> CTA c
-        const int r = threadIdx.x / kSmallCtas, c = threadIdx.x % kSmallCtas;
-        st_cluster_u32(&s_tsum[r * kSmallCtas + (int)rank], (uint32_t)c, r < R ? s_sum[r] : 0u);
-    }
-    cluster_sync_all();
-    // ---- E3: every CTA scans the tile sums (tile T = 8 r + c, T in block order) and its own tiles
-    if (warp == 0) {
-        const uint32_t v = lane < kSmallCtas * kSmallIters ? s_tsum[lane] : 0u;
-        uint32_t inc = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
-        if (lane < kSmallCtas * kSmallIters) s_tsum[lane] = inc - v;             // exclusive
-        if (lane == 31) s_sum[0] = inc;                                          // grand total (16-B units); the own sums are no longer needed
-    }
-    if (warp >= 1 && warp <= R) {                                                // warp r + 1: the 64 sizes of own tile r (R <= 4 < 8 warps)
-        const int r = warp - 1;
+    // ---- E3. Warp r: exclusive scan of the 64 sizes of own tile r (tile T = 8 r + rank = first block / 64); the row and the
+    // tile's sum go into EVERY CTA of the cluster (distributed shared memory), so that after ONE cluster barrier every CTA
+    // knows the scan value at every block of the batch: no look-back, no exchange through global memory.
+    if (warp < R) {
+        const int r = warp, Tl = r * kSmallCtas + (int)rank;
         const uint32_t k0 = s_key[r][2 * lane] & ~kLateBit, k1 = s_key[r][2 * lane + 1] & ~kLateBit;
         const uint32_t own = (k0 >> 18) + (k1 >> 18);
         uint32_t inc = own;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
-        s_off16[r][2 * lane] = inc - own;
-        s_off16[r][2 * lane + 1] = inc - own + (k0 >> 18);
+        const uint32_t e0 = inc - own, e1 = e0 + (k0 >> 18), sum = __shfl_sync(kFull, inc, 31);
+#pragma unroll
+        for (int c = 0; c < kSmallCtas; c++) {
+            st_cluster_u32(&s_off16[Tl][2 * lane], (uint32_t)c, e0);
+            st_cluster_u32(&s_off16[Tl][2 * lane + 1], (uint32_t)c, e1);
+            if (lane == 0) st_cluster_u32(&s_tsum[Tl], (uint32_t)c, sum);
+        }
+    }
+    cluster_sync_all();
+    if (warp == 0) {                                                 // exclusive scan of the tile sums (tiles beyond the last block: never written, never read)
+        const int nT = R * kSmallCtas;
+        const uint32_t v = lane < nT ? s_tsum[lane] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        if (lane < nT) s_tsum[lane] = inc - v;
+        if (lane == 31) s_sum[0] = inc;                              // grand total (16-B units); the own sums are no longer needed
     }
     __syncthreads();
     const unsigned long long grand16 = s_sum[0];
     const unsigned long long total_out = s_fixed[a.n_buf] + 16ull * grand16;
-    if (total_out > a.out_cap) {                                                 // (the same decision in every CTA)
+    if (total_out > a.out_cap) {                                     // (the same decision in every CTA)
         if (rank == 0 && threadIdx.x == 0) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
         for (uint32_t i = rank * kSmallThreads + threadIdx.x; i <= a.n_buf; i += kSmallCtas * kSmallThreads) a.out_off[i] = 0;
         return;
     }
-    // scan value G at block g of one of the own tiles (16-B units of block bytes before it)
+    // scan value at block g: 16-B units of block bytes before it (g = total: all of them)
     auto scan_at = [&](uint32_t g) -> unsigned long long {
-        const uint32_t r = g / (kSmallCtas * kTileR), jj = g % kTileR;
-        return (unsigned long long)s_tsum[r * kSmallCtas + rank] + s_off16[r][jj];
+        return g >= total ? grand16 : (unsigned long long)s_tsum[g / kTileR] + s_off16[g / kTileR][g % kTileR];
     };
-    // stream i starts at fixed_prefix[i] + 16 G(first block of i); streams without blocks: at the next block, or at the
-    // end (G = grand total: rank 0). The CTA that owns that block publishes the start.
-    for (uint32_t i = threadIdx.x; i < a.n_buf; i += kSmallThreads) {
-        const uint32_t g = s_first[i];
-        unsigned long long S = ~0ull;
-        if (g >= total) { if (rank == 0) S = s_fixed[i] + 16ull * grand16; }
-        else if ((g / kTileR) % kSmallCtas == rank) S = s_fixed[i] + 16ull * scan_at(g);
-        if (S != ~0ull) { a.ws.stream_start[i] = S; a.out_off[i] = S; }
-    }
-    if (rank == 0 && threadIdx.x == 0) { a.ws.stream_start[a.n_buf] = total_out; a.out_off[a.n_buf] = total_out; }
-    __threadfence();
-    cluster_sync_all();
+    // stream i starts at fixed_prefix[i] + 16 * (scan value at its first block; streams without blocks: at the next block)
+    auto stream_at = [&](uint32_t i) -> unsigned long long {
+        return i >= a.n_buf ? total_out : s_fixed[i] + 16ull * scan_at(s_first[i]);
+    };
 
     // ---- pass 2: E1 + E4, blocks and directory entries to their final place
     for (int r = 0; r < R; r++) {
@@ -1127,7 +1136,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         if (key != 0) {
             at = s_fixed[i + 1] + 16ull * scan_at(g);
             if (l == 0) {                                            // directory entry (FORMAT.md §1)
-                const unsigned long long S = __ldcg(&a.ws.stream_start[i]);
+                const unsigned long long S = stream_at(i);
                 reinterpret_cast<uint32_t*>(a.out + S + 32)[g - s_first[i]] = (uint32_t)((at - S) >> 4);
             }
         }
@@ -1152,10 +1161,12 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         __syncwarp();                                                // image and staged IDs are free again
     }
 
-    // ---- stream headers, directory tails, E5 (RAW copies): a warp per stream, the streams dealt round the cluster
+    if (a.n_buf == 0 && rank == 0 && threadIdx.x == 0) a.out_off[0] = total_out;
+    // ---- stream headers, directory tails, E5 (RAW copies), out_offsets: a warp per stream, the streams dealt round the cluster
     for (uint32_t i = rank * kEncWorkers + warp; i < a.n_buf; i += kSmallCtas * kEncWorkers) {
-        const unsigned long long s0 = __ldcg(&a.ws.stream_start[i]), s1 = __ldcg(&a.ws.stream_start[i + 1]);
+        const unsigned long long s0 = stream_at(i), s1 = stream_at(i + 1);
         const unsigned long long o0 = a.in_off[i], n = a.in_off[i + 1] - o0, tot = s1 - s0;
+        if (lane == 0) { a.out_off[i] = s0; if (i + 1 == a.n_buf) a.out_off[a.n_buf] = s1; }
         const bool raw_s = n * E < a.thr;
         unsigned char* s = a.out + s0;
         if (lane == 0) {
@@ -1178,7 +1189,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
             const T* x = ids + o0;
             T* y = reinterpret_cast<T*>(s + 32);
             const unsigned long long padded = (tot - 32) / E;
-            for (unsigned long long t = lane; t < padded; t += 32) y[t] = t < n ? x[t] : (T)0;
+            raw_copy<T>(y, x, n, padded, lane);
         }
     }
 }
