@@ -937,7 +937,7 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
 // kSmallCtas CTAs that the hardware schedules together, so that a CTA may wait for another one of the grid without any
 // residency assumption, and that exchange their tile sums through distributed shared memory instead of a look-back
 // through L2. Every CTA runs E0 for itself (the plan of up to kSmallMaxBuf buffers, tables in shared memory), then
-//   pass 1   E1 + E2 of its tiles (tile T = 8 r + cluster rank, r = 0 .. kSmallIters - 1): sizes in shared memory; the
+//   pass 1   E1 + E2 of its tiles (tile T = kSmallCtas r + cluster rank, r = 0 .. kSmallIters - 1): sizes in shared memory; the
 //            scan inside each own tile and its sum written into every CTA of the cluster;   -- ONE cluster barrier --
 //            exclusive scan of the <= 32 tile sums (every CTA the same): every CTA now has the output offset of every
 //            block and every stream of the batch in its own shared memory;
@@ -945,10 +945,11 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
 //            entries written to their final place; stream headers, directory tails, RAW copies (E5), out_offsets
 //            of its share of the streams.
 // No plan kernel, no look-back states, no ticket, no k_enc_streams: one launch latency instead of three.
-constexpr int kSmallCtas = 8;                            // portable cluster size
-constexpr int kSmallIters = 4;                           // tiles per CTA
+constexpr int kSmallCtas = 16;                           // CTAs of the cluster (above the portable 8: opt-in, checked once per device)
+constexpr int kSmallIters = 2;                           // tiles per CTA (measured: with 4 the general path is faster from 3 tiles on)
 constexpr uint32_t kSmallMaxBuf = 1024;
 constexpr uint32_t kSmallMaxBlocks = kSmallCtas * kTileR * kSmallIters;      // 2048 blocks = 262144 IDs
+static_assert(kSmallCtas * kSmallIters <= 32, "one warp scans the tile sums");
 constexpr int kSmallThreads = kEncWorkers * 32;
 
 template <int W> struct SmallSmem {
@@ -1072,7 +1073,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         __syncwarp();                                                // the staged IDs are consumed (the next tile overwrites them)
     }
     __syncthreads();
-    // ---- E3. Warp r: exclusive scan of the 64 sizes of own tile r (tile T = 8 r + rank = first block / 64); the row and the
+    // ---- E3. Warp r: exclusive scan of the 64 sizes of own tile r (tile T = kSmallCtas r + rank = first block / 64); the row and the
     // tile's sum go into EVERY CTA of the cluster (distributed shared memory), so that after ONE cluster barrier every CTA
     // knows the scan value at every block of the batch: no look-back, no exchange through global memory.
     if (warp < R) {
@@ -1472,17 +1473,29 @@ static int enc_ctas_per_sm(int device) {
     return per_sm[device];
 }
 
+// Once per device: the small-batch kernel's dynamic shared memory and its cluster size. 1 = usable, -1 = this device
+// cannot run a cluster of kSmallCtas such CTAs (small batches then take the general path), 0 = a CUDA error.
 template <int W>
-static bool enc_small_init(int device) {                 // once per device: the small-batch kernel's dynamic shared memory
+static int enc_small_init(int device) {
     static std::mutex mu;
-    static bool done[kMaxDevices] = {};
+    static int state[kMaxDevices] = {};
     std::lock_guard<std::mutex> lock(mu);
-    if (!done[device]) {
+    if (state[device] == 0) {
         if (cudaFuncSetAttribute(k_enc_small<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SmallSmem<W>::kBytes) != cudaSuccess)
-            return false;
-        done[device] = true;
+            return 0;
+        int n = 0;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(kSmallCtas); cfg.blockDim = dim3(kSmallThreads); cfg.dynamicSmemBytes = SmallSmem<W>::kBytes;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = kSmallCtas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        const bool ok = cudaFuncSetAttribute(k_enc_small<W>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess &&
+                        cudaOccupancyMaxActiveClusters(&n, k_enc_small<W>, &cfg) == cudaSuccess && n >= 1;
+        if (!ok) (void)cudaGetLastError();               // (not an error of the call: the general path runs)
+        state[device] = ok ? 1 : -1;
     }
-    return true;
+    return state[device];
 }
 
 template <int W>
@@ -1501,10 +1514,14 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         if (!degenerate && n_tiles > a_in.ws.tile_cap) return BFSC_ERR_INVALID_ARG;          // workspace too small
         if (n_tiles < (unsigned long long)grid) grid = n_tiles ? (int)n_tiles : 1;
     }
+    int small = 0;
     if (!single && a_in.n_buf <= kSmallMaxBuf && a_in.ws.blk_cap <= kSmallMaxBlocks) {
+        small = enc_small_init<W>(dev.device);
+        if (small == 0) return BFSC_ERR_CUDA;
+    }
+    if (small == 1) {
         // a small batch (both bounds known on the host: buffer count, and blocks by the workspace size the caller derived
         // from the total ID count): one launch of one cluster
-        if (!enc_small_init<W>(dev.device)) return BFSC_ERR_CUDA;
         EncArgs a = a_in;
         a.grid = kSmallCtas;
         cudaLaunchConfig_t cfg = {};
