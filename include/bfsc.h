@@ -114,7 +114,9 @@ size_t bfsc_compress_bound(size_t n_ids, bfsc_dtype t);
 size_t bfsc_batch_compress_bound(const uint64_t* h_counts, size_t n_buf, bfsc_dtype t);
 
 /* Workspace bytes sufficient for any of the four device calls on a batch of n_buf buffers
- * holding n_ids_total IDs in total (single-buffer calls: n_buf = 1). Host. */
+ * holding n_ids_total IDs in total (single-buffer calls: n_buf = 1). Host. The batch calls size their launches by the
+ * workspace they are given: a small batch (a BFS level of up to ~1 MB) with a workspace sized for ITS total runs in one
+ * launch; the same batch with a workspace sized for the largest level of the run takes the general three-launch path. */
 size_t bfsc_workspace_bytes(size_t n_ids_total, size_t n_buf, bfsc_dtype t);
 
 /* ONE buffer: d_ids[0..n_ids) -> one stream at d_out; *d_out_bytes (device) = its

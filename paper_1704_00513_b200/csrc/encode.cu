@@ -1,8 +1,11 @@
 // encode.cu — bfsc_compress / bfsc_compress_batch (steps E0-E5).
 //
-// Launches per call:  k_enc_plan -> k_enc_tiles [-> k_enc_streams, batch and degenerate calls only],
-// chained with programmatic dependent launch: a dependent kernel starts while its predecessor still
-// runs and executes griddepcontrol.wait before it touches what the predecessor writes.
+// Launches per call, chained with programmatic dependent launch (a dependent kernel starts while its predecessor still
+// runs and executes griddepcontrol.wait before it touches what the predecessor writes):
+//   one buffer              k_enc_plan -> k_enc_tiles<W, 0> [-> k_enc_streams: no block at all] [-> k_enc_fallback: FORMAT.md §8]
+//   small batch             k_enc_small (one cluster; <= 1024 buffers, <= 2048 blocks by the workspace size)
+//   batch                   k_enc_planblocks (<= 8192 buffers; else k_enc_plan -> k_enc_blocks) -> k_enc_tiles<W, 1> -> k_enc_streams
+//   frontier bitmap         k_bm_count -> k_bm_plan -> k_bm_starts -> k_enc_tiles<W, 2> -> k_bm_finish
 #include <mutex>
 
 #include "bitmap_stage.cuh"
