@@ -1318,6 +1318,17 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
         a.ws.hdr->grand16 = 0; a.ws.hdr->total_out = fixed; a.ws.hdr->ok = ok ? 1u : 0u; a.ws.hdr->n_ids = n;
         if (!ok) set_status(a.status, BFSC_ERR_INVALID_ARG);
         if (a.out_total) *a.out_total = 0;               // (the last tile, or k_bm_finish, writes the size)
+        if (ok && n == 0 && !raw) {                      // the empty stream (no tile runs; k_bm_finish is not launched when the
+            if (48 <= a.out_cap) {                       //  call has neither a threshold nor the fallback option): 48 bytes
+                uint4 h0, h1;
+                h0.x = 0x43534642u; h0.y = 1u | ((uint32_t)W << 8) | (a.codec << 16); h0.z = 0; h0.w = 0;
+                h1.x = 48u; h1.y = 0; h1.z = 0; h1.w = 0;
+                reinterpret_cast<uint4*>(a.out)[0] = h0;
+                reinterpret_cast<uint4*>(a.out)[1] = h1;
+                reinterpret_cast<uint4*>(a.out)[2] = make_uint4(3u, 0u, 0u, 0u);
+                if (a.out_total) *a.out_total = 48ull;
+            } else set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+        }
     }
 }
 
@@ -1600,7 +1611,8 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
     if (tgrid < 1) tgrid = 1;
     BFSC_LAUNCH(launch_dep(k_bm_starts, (int)tgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 2>, grid, kEncThreads, kSmem, s, a));
-    BFSC_LAUNCH(launch_dep(k_bm_finish<W>, (int)cgrid, 256, 0, s, a));
+    if (a.thr > 0 || a.fallback)                                     // (else no stream can end up RAW, and the plan wrote the empty one)
+        BFSC_LAUNCH(launch_dep(k_bm_finish<W>, (int)cgrid, 256, 0, s, a));
     return BFSC_OK;
 }
 
