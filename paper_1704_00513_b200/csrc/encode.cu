@@ -1249,15 +1249,16 @@ __device__ __forceinline__ uint32_t select_bit(uint32_t x, uint32_t k) {
     return pos;
 }
 
-// Set bits of every chunk -> a.chunk[c] (plain counts; entries up to the end of the last super-chunk: 0). Eight lanes per
-// chunk, one 16-byte load each (the bitmap is 16-byte aligned and readable up to a multiple of 16 bytes).
+// Set bits of every chunk -> a.chunk[c] (plain counts; entries up to the end of the last super-chunk: 0) and of every
+// super-chunk -> a.super[s]. A CTA takes a super-chunk at a time (8 warps x 4 chunks), eight lanes per chunk, one 16-byte
+// load each (the bitmap is 16-byte aligned and readable up to a multiple of 16 bytes).
 __global__ void __launch_bounds__(256) k_bm_count(EncArgs a) {
+    __shared__ uint32_t s_w[8];
     pdl_wait();                                          // the call before this one is complete (workspace, inputs)
     pdl_launch_dependents();
-    const int lane = threadIdx.x & 31, sub = lane & 7;
-    const unsigned long long n_pad = a.n_super * kSuperChunks;
-    for (unsigned long long c = ((unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * 4 + (lane >> 3); c < n_pad;
-         c += (unsigned long long)gridDim.x * 32) {      // (the 4 chunks of a warp lie below n_pad together: n_pad is a multiple of 32)
+    const int lane = threadIdx.x & 31, sub = lane & 7, warp = threadIdx.x >> 5;
+    for (unsigned long long sc = blockIdx.x; sc < a.n_super; sc += gridDim.x) {
+        const unsigned long long c = sc * kSuperChunks + 4 * warp + (lane >> 3);
         const unsigned long long bit0 = c * kChunkBits + 128ull * sub;
         uint32_t k = 0;
         if (bit0 < a.n_bits) {
@@ -1273,29 +1274,27 @@ __global__ void __launch_bounds__(256) k_bm_count(EncArgs a) {
         }
         k += __shfl_xor_sync(kFull, k, 1); k += __shfl_xor_sync(kFull, k, 2); k += __shfl_xor_sync(kFull, k, 4);
         if (sub == 0) a.chunk[c] = k;
+        const uint32_t kw = k + __shfl_xor_sync(kFull, k, 8);                    // the warp's four chunks
+        const uint32_t kq = kw + __shfl_xor_sync(kFull, kw, 16);
+        if (lane == 0) s_w[warp] = kq;
+        __syncthreads();
+        if (threadIdx.x == 0) a.super[sc] = (unsigned long long)s_w[0] + s_w[1] + s_w[2] + s_w[3] + s_w[4] + s_w[5] + s_w[6] + s_w[7];
+        __syncthreads();
     }
 }
 
-// One CTA: totals of the super-chunks (warp w, step i: the 32 chunk counts of super-chunk s0 + 32 w + i in one coalesced
-// load, reduced; lane i keeps the total — thread t then holds super-chunk s0 + t), block scan -> a.super (entry n_super =
-// n = the number of set bits); then the plan of the one stream (E0).
+// One CTA: block scan of the super-chunk totals, in place -> set bits before every super-chunk (entry n_super = n = the
+// number of set bits); then the plan of the one stream (E0).
 template <int W>
 __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
     __shared__ Scan2 sm[33];
     constexpr unsigned long long E = W / 8;
     pdl_wait();
     pdl_launch_dependents();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     Scan2 carry{0, 0};
     for (unsigned long long s0 = 0; s0 < a.n_super; s0 += 1024ull) {
-        uint32_t mine = 0;
-#pragma unroll 8
-        for (int i = 0; i < 32; i++) {
-            const unsigned long long sc = s0 + 32ull * warp + i;
-            const uint32_t t = __reduce_add_sync(kFull, sc < a.n_super ? a.chunk[sc * kSuperChunks + lane] : 0u);
-            if (lane == i) mine = t;
-        }
         const unsigned long long sc = s0 + threadIdx.x;
+        const unsigned long long mine = sc < a.n_super ? a.super[sc] : 0ull;
         Scan2 tot;
         const Scan2 ex = block_scan_excl2(Scan2{mine, 0}, &tot, sm);
         if (sc < a.n_super) a.super[sc] = carry.a + ex.a;
@@ -1600,7 +1599,7 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
     a.grid = (uint32_t)grid;
     size_t cgrid = (size_t)((a.n_chunks + 7) / 8), sgrid = (size_t)((a.n_super + 7) / 8);
     if (cgrid > (size_t)dev.sms * 8) cgrid = (size_t)dev.sms * 8;
-    sgrid = (size_t)((a.n_super * kSuperChunks + 31) / 32);          // k_bm_count: a warp takes 4 chunks
+    sgrid = (size_t)a.n_super;                                       // k_bm_count: a CTA takes a super-chunk
     if (sgrid > (size_t)dev.sms * 8) sgrid = (size_t)dev.sms * 8;
     if (cgrid < 1) cgrid = 1;
     if (sgrid < 1) sgrid = 1;
