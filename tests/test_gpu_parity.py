@@ -1001,3 +1001,53 @@ def test_small_batch_cluster_kernel_errors(B):
     B.compress_batch(ids2.to(dev), off2.to(dev), 6, 32, 0, out2, out_off2, tiny_ws, status)
     torch.cuda.synchronize()
     assert int(status.item()) == B.ERR_INVALID_ARG and bool((out_off2 == 0).all())
+
+
+def test_mixed_calls_overlap_on_four_streams(B, oracle_mod):
+    """Large single-buffer calls, small batches (the one-cluster kernel) and mid-size batches enqueued on four streams
+    without any synchronisation between them, three passes over the same buffers: every tile of every compress grid comes
+    from a ticket and a cluster is scheduled as a whole, so whatever shares the device, nothing can wait for a CTA that
+    is not running. Bytes against the oracle, decode against the input."""
+    dev = torch.device("cuda")
+    rng = np.random.default_rng(17)
+    cu = [torch.cuda.Stream() for _ in range(4)]
+    for rnd in range(12):
+        jobs = []
+        for s in range(4):
+            W = int(rng.choice([32, 64])); thr = int(rng.choice([0, 1024])); kind = (rnd + s) % 3
+            if kind == 0:
+                n = int(rng.choice([1 << 20, (1 << 22) + 5])); n_buf = 1; off = None
+                ids = streams.gap_stream(n, float(rng.choice([2.0, 256.0])), seed=100 * rnd + s, W=W, outlier_frac=0.01, device=dev)
+            else:
+                n_buf = int(rng.choice([16, 64])) if kind == 1 else 500
+                counts = torch.randint(0, 3000 if kind == 1 else 400, (n_buf,), generator=torch.Generator().manual_seed(100 * rnd + s))
+                ids, off = streams.batch_of_streams(counts, 16.0, seed=100 * rnd + s, W=W, device=dev)
+                ids, off = ids.to(dev), off.to(dev); n = ids.numel()
+            cap = B.compress_bound(n, W) if off is None else B.batch_compress_bound((off[1:] - off[:-1]).tolist(), W)
+            jobs.append(dict(W=W, thr=thr, ids=ids, off=off, n=n, n_buf=n_buf, cap=cap,
+                             out=torch.empty(cap, dtype=torch.uint8, device=dev),
+                             ws=torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev),
+                             st=torch.zeros(1, dtype=torch.int32, device=dev), oo=torch.zeros(n_buf + 1, dtype=torch.int64, device=dev),
+                             back=torch.empty(max(n, 4), dtype=ids.dtype, device=dev), io=torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)))
+        torch.cuda.synchronize()
+        for _ in range(3):
+            for s, j in enumerate(jobs):
+                with torch.cuda.stream(cu[s]):
+                    if j["off"] is None:
+                        B.compress(j["ids"], j["n"], j["W"], j["thr"], j["out"], j["oo"][1:2], j["ws"], j["st"])
+                        B.decompress(j["out"], j["cap"], j["W"], j["back"], j["io"][1:2], j["ws"], j["st"])
+                    else:
+                        B.compress_batch(j["ids"], j["off"], j["n_buf"], j["W"], j["thr"], j["out"], j["oo"], j["ws"], j["st"])
+                        B.decompress_batch(j["out"], j["oo"], j["n_buf"], j["W"], j["back"], j["io"], j["ws"], j["st"])
+        torch.cuda.synchronize()
+        for j in jobs:
+            assert int(j["st"].item()) == 0
+            host = _np(j["ids"], j["W"])
+            if j["off"] is None:
+                ref = oracle_mod.compress(host, j["thr"])
+                assert int(j["oo"][1].item()) == len(ref)
+            else:
+                ref, ro = oracle_mod.compress_batch(host, j["off"].cpu().numpy().astype(np.uint64), j["thr"])
+                assert np.array_equal(j["oo"].cpu().numpy().astype(np.uint64), ro)
+            assert np.array_equal(j["out"][:len(ref)].cpu().numpy(), ref)
+            assert torch.equal(j["back"][:j["n"]], j["ids"])
