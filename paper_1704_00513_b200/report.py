@@ -229,6 +229,14 @@ def sweep(R):
                 off = torch.tensor([0, n], dtype=torch.int64, device=dev)
                 print(R.row(label, R.batch(ids, off, W, 0, single=True)))
                 del ids
+    # BFS levels of up to ~1 MB (the one-launch paths of both directions) and just above (the general path)
+    for n_buf, per in ((16, 2000), (16, 8000), (16, 16000), (16, 20000), (16, 100000)):
+        counts = torch.full((n_buf,), per, dtype=torch.int64)
+        ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=32, device=dev)
+        print(R.total(f"level of {n_buf} buffers x {per} IDs, mean 16, threshold 1024", R.batch(ids.to(dev), off.to(dev), 32, 1024)))
+    counts = streams.log_uniform_counts(64, 8, 12, 32, seed=5)
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=32, device=dev)
+    print(R.total("level of 64 buffers 1 KB-16 KB (log-uniform), mean 16, threshold 1024", R.batch(ids.to(dev), off.to(dev), 32, 1024)))
     counts = streams.log_uniform_counts(4096, 8, 16, 32, seed=5)
     ids, off = streams.batch_of_streams(counts, 16.0, seed=5, W=32, device=dev)
     for thr in (0, 1024):
