@@ -12,7 +12,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-SO_PATH = os.path.join(_HERE, "libbfsc.so")
+CHECKED = os.environ.get("BFSC_CHECKED", "") == "1"      # the bounds-asserting build (build.py)
+SO_PATH = os.path.join(_HERE, "libbfsc_checked.so" if CHECKED else "libbfsc.so")
 _lib = None
 
 OK, ERR_INVALID_ARG, ERR_DST_TOO_SMALL, ERR_CORRUPT, ERR_CUDA, ERR_UNSUPPORTED = range(6)
@@ -123,6 +124,16 @@ def bitmap_workspace_bytes(n_bits: int, W: int) -> int:
 
 def host_scratch_bytes(n_ids: int, W: int) -> int:
     return lib().bfsc_host_scratch_bytes(n_ids, W)
+
+
+def check_failures():
+    """BFSC_CHECKED build only: (violations, first failing source line) of the encode and of the decode kernels so far."""
+    out = []
+    for name in ("bfsc_debug_checks_encode", "bfsc_debug_checks_decode"):
+        buf = (ctypes.c_uint * 2)()
+        getattr(lib(), name)(buf)
+        out.append((int(buf[0]), int(buf[1])))
+    return out
 
 
 def kernel_launches() -> int:

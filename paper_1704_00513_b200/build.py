@@ -1,5 +1,8 @@
 """Builds csrc/*.cu into paper_1704_00513_b200/libbfsc.so for sm_100a (in-tree, so the .so
-travels to the GPU box with the repo snapshot). `python -m paper_1704_00513_b200.build`."""
+travels to the GPU box with the repo snapshot). `python -m paper_1704_00513_b200.build`.
+With BFSC_CHECKED=1 in the environment: libbfsc_checked.so, compiled with -DBFSC_CHECKED (every BFSC_CHECK of the kernels
+counted instead of compiled away); binding.py loads that one under the same variable, and tests/conftest.py asserts at
+the end of a run that no check failed: `BFSC_CHECKED=1 python -m pytest tests -m gpu`."""
 from __future__ import annotations
 
 import glob
@@ -8,7 +11,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SO = os.path.join(HERE, "libbfsc.so")
+CHECKED = os.environ.get("BFSC_CHECKED", "") == "1"      # the bounds-asserting build (csrc/common.cuh: BFSC_CHECK), a library of its own
+SO = os.path.join(HERE, "libbfsc_checked.so" if CHECKED else "libbfsc.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-shared", "--use_fast_math", "-Xptxas", "-v"]
@@ -27,7 +31,7 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        cmd = [NVCC] + FLAGS + ["-o", SO] + sources()
+        cmd = [NVCC] + FLAGS + (["-DBFSC_CHECKED"] if CHECKED else []) + ["-o", SO] + sources()
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode:
             print(r.stdout + r.stderr)

@@ -55,6 +55,7 @@ __device__ __forceinline__ void bm_expand(T* __restrict__ raw, const uint32_t* _
             for (int u = 1; u <= 4; u++) {
                 uint32_t b;
                 asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(x));               // 0xffffffff for x == 0
+                BFSC_CHECK(!x || (out - u >= raw && out - u < raw + kBlk));
                 if (x) out[-u] = id0 + (T)b;
                 x &= ~(1u << (b & 31u));
             }

@@ -88,6 +88,22 @@ __host__ inline bool ws_carve(void* ws, size_t bytes, size_t n_buf, WsView* v) {
     return true;
 }
 
+// ---- -DBFSC_CHECKED (python -m paper_1704_00513_b200.build --checked, or BFSC_CHECKED=1 in the environment of the tests):
+// every BFSC_CHECK in the kernels is evaluated — shared-memory slot indices, global stores against out_capacity /
+// ids_capacity / the bitmap — and a violation is counted (first failing source line kept) instead of trapping, so that a
+// whole test run can be made under it and asked for the count at the end (bfsc_debug_checks_encode / _decode; one
+// counter per translation unit). The normal build compiles the checks away. compute-sanitizer is not available on
+// the GPU pool this library is developed on; this is its stand-in.
+#ifdef BFSC_CHECKED
+static __device__ unsigned int g_bfsc_check[2];          // failures, first failing line
+#define BFSC_CHECK(cond)                                                                     \
+    do {                                                                                     \
+        if (!(cond)) { atomicAdd(&g_bfsc_check[0], 1u); atomicCAS(&g_bfsc_check[1], 0u, (unsigned)__LINE__); } \
+    } while (0)
+#else
+#define BFSC_CHECK(cond) do { } while (0)
+#endif
+
 // ---- device helpers ------------------------------------------------------------------
 __device__ __forceinline__ void set_status(uint32_t* st, uint32_t code) {
     if (st) atomicCAS(st, 0u, code);
@@ -125,6 +141,7 @@ struct BitSink { uint32_t* bm; unsigned long long id_base, n_bits; uint32_t* sta
 // The bits `mask` of word w: plain OR into the bitmap, or (bfsc_decompress_to_frontier, Algorithm 4 lines 11-13) OR into
 // the visited bitmap first — what was not visited before goes into the frontier bitmap.
 __device__ __forceinline__ void sink_or(const BitSink& s, uint32_t w, uint32_t mask) {
+    BFSC_CHECK((unsigned long long)w < (s.n_bits + 31) / 32);
     if (s.visited != nullptr) {
         // The atomic's return value says which of the bits were visited before (exactly once per vertex, whoever else
         // updates the same word). It costs the warp a round trip to L2 per word. Measured alternative: a plain load of

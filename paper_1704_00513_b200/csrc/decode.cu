@@ -488,6 +488,7 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         r.span16 = (uint32_t)(o1 - o0);
         r.m = m;
         r.x = reinterpret_cast<T*>(a.ids) + xi;
+        BFSC_CHECK(kBits || xi + (unsigned long long)m <= a.ids_cap);
         return r;
     };
 
@@ -563,6 +564,7 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         for (; bi < n_batches; bi += n_warps) {
             const bool big = cur.blk != nullptr && cur.span16 > (uint32_t)kDecSpanMax;
             const bool any_big = __any_sync(kFull, big);
+            BFSC_CHECK(any_big || cur.blk == nullptr || cur.span16 <= (uint32_t)kDecSpanMax);
             if (!any_big && cur.blk != nullptr) quad_stage_block(slot, cur.blk, cur.span16, l);
             const BlockAt<W> nxt = locate((bi + n_warps) * kDecBlocks + q);   // the next batch's directory reads overlap the copy
             if (!any_big) {
@@ -764,6 +766,13 @@ extern "C" bfsc_status bfsc_decompress_batch(const void* d_in, const uint64_t* d
     return bfsc::decode_common(d_in, d_in_offsets, 0, n_buf, t, d_ids, ids_capacity, d_id_offsets, nullptr,
                                d_workspace, workspace_bytes, d_status, cuda_stream);
 }
+
+#ifdef BFSC_CHECKED
+extern "C" void bfsc_debug_checks_decode(unsigned int* h_failures_and_line) {      // BFSC_CHECK violations of the decode kernels so far
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(h_failures_and_line, bfsc::g_bfsc_check, 2 * sizeof(unsigned int));
+}
+#endif
 
 extern "C" bfsc_status bfsc_decompress_to_bitmap(const void* d_in, size_t in_bytes, bfsc_dtype t, uint64_t id_base,
                                                  uint32_t* d_bitmap, size_t n_bits, uint64_t* d_n_ids,

@@ -633,6 +633,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                             }
                         }
                     }
+                    BFSC_CHECK(at == kSkip || (at >= S && S + 32 + 4 * (g - first) + 4 <= a.out_cap));
                     if (at != kSkip) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
                     if (!batch && g == total - 1) {      // single buffer: stream header, dir[nb], zero pad
                         const unsigned long long tot = f1 + 16ull * (excl + off) + bytes;
@@ -787,6 +788,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 woff = inc - zf;
             }
             unsigned char* img = ib + 16 * woff;
+            BFSC_CHECK(!fast || 16u * woff + (key >> 14) <= (uint32_t)(Img::kBufChunks * 16));
             if (!wide && __any_sync(kFull, fast && n_exc > 0))           // E4 into the image buffer: exceptions
                 col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
             __syncwarp();                                                // the warp's staged IDs are consumed
@@ -835,10 +837,12 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 const uint32_t tot = __shfl_sync(kFull, woff_e + z_e, 31);
                 fence_proxy_async_smem();                                // the image was written through the generic proxy
                 __syncwarp();
+                BFSC_CHECK(lane != 0 || tot == 0 || (at + 16ull * tot <= a.out_cap && 16u * tot <= (uint32_t)(Img::kBufChunks * 16)));
                 if (lane == 0 && tot > 0) bulk_store(a.out + at, ib_e, 16u * tot);
             } else if (fast_e && at != kSkip) {
                 const uint4* src = reinterpret_cast<const uint4*>(ib_e) + woff_e;
                 uint4* dst = reinterpret_cast<uint4*>(a.out + at);
+                BFSC_CHECK(at + 16ull * z_e <= a.out_cap);
                 for (uint32_t c = l; c < z_e; c += 4) __stcs(dst + c, src[c]);
             }
             __syncwarp();
@@ -1156,6 +1160,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
             }
         }
         __syncwarp();
+        BFSC_CHECK(key == 0 || at + (key >> 14) <= a.out_cap);
+        BFSC_CHECK(!fast || (key >> 14) <= (uint32_t)(Smem::kSlotChunks * 16));
         if (fast) {
             const uint4* src = reinterpret_cast<const uint4*>(img);
             uint4* dst = reinterpret_cast<uint4*>(a.out + at);
@@ -1169,6 +1175,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
     // ---- stream headers, directory tails, E5 (RAW copies), out_offsets: a warp per stream, the streams dealt round the cluster
     for (uint32_t i = rank * kEncWorkers + warp; i < a.n_buf; i += kSmallCtas * kEncWorkers) {
         const unsigned long long s0 = stream_at(i), s1 = stream_at(i + 1);
+        BFSC_CHECK(s0 + 32 <= s1 && s1 <= a.out_cap);
         const unsigned long long o0 = a.in_off[i], n = a.in_off[i + 1] - o0, tot = s1 - s0;
         if (lane == 0) { a.out_off[i] = s0; if (i + 1 == a.n_buf) a.out_off[a.n_buf] = s1; }
         const bool raw_s = n * E < a.thr;
@@ -1637,6 +1644,30 @@ static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint
 }
 
 }  // namespace bfsc
+
+#ifdef BFSC_CHECKED
+extern "C" void bfsc_debug_checks_encode(unsigned int* h_failures_and_line) {      // BFSC_CHECK violations of the encode kernels so far
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(h_failures_and_line, bfsc::g_bfsc_check, 2 * sizeof(unsigned int));
+}
+namespace bfsc {
+__global__ void k_check_selftest() { BFSC_CHECK(threadIdx.x != 3); }               // one violation, on purpose
+}
+// Proves that a violated BFSC_CHECK is seen: runs one, returns what the counters then say in h_seen[0..1] (failures added,
+// line recorded), and puts the counters back as they were.
+extern "C" void bfsc_debug_check_selftest(unsigned int* h_seen) {
+    unsigned int before[2], after[2];
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(before, bfsc::g_bfsc_check, sizeof(before));
+    const unsigned int zero[2] = {0u, 0u};
+    cudaMemcpyToSymbol(bfsc::g_bfsc_check, zero, sizeof(zero));
+    bfsc::k_check_selftest<<<1, 32>>>();
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(after, bfsc::g_bfsc_check, sizeof(after));
+    cudaMemcpyToSymbol(bfsc::g_bfsc_check, before, sizeof(before));
+    h_seen[0] = after[0]; h_seen[1] = after[1];
+}
+#endif
 
 extern "C" bfsc_status bfsc_compress_codec(bfsc_codec codec, const void* d_ids, size_t n_ids, bfsc_dtype t,
                                            size_t raw_threshold_bytes, void* d_out, size_t out_capacity,

@@ -69,3 +69,15 @@ def test_noalloc_rejects_sizes_beyond_the_scratch(B):
     assert e.value.code == B.ERR_INVALID_ARG
     torch.cuda.synchronize()
     assert int(nbytes.item()) == -1 and int(status.item()) == 0          # nothing was enqueued
+
+
+def test_checked_build_sees_a_violation(B):
+    """Only under BFSC_CHECKED=1 (libbfsc_checked.so): a deliberately violated BFSC_CHECK is counted with its source line —
+    the end-of-run assertion of tests/conftest.py would see a real one."""
+    import ctypes
+    if not B.CHECKED:
+        pytest.skip("normal build: BFSC_CHECK compiles away")
+    seen = (ctypes.c_uint * 2)()
+    B.lib().bfsc_debug_check_selftest(seen)
+    assert seen[0] == 1 and seen[1] > 0
+    assert B.check_failures()[0][0] == 0                 # the selftest put the counters back
