@@ -176,6 +176,26 @@ bfsc_status bfsc_compress_batch_codec(bfsc_codec codec, const void* d_ids, const
                                       void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
                                       void* cuda_stream);
 
+/* The send side of the exchange with the transfer fused into the encoder (PAPER.md L1361-1369:
+ * Algorithm 4 lines 5 and 9, the row / column exchanges of compressed frontiers; L1792-1800, L1834: overlap of compression
+ * and communication, the thesis's future work). As bfsc_compress_batch_codec, except that stream i is not appended to a
+ * common output: it is written at the device address d_dst[i] — a device array of n_buf addresses, each a multiple of 16
+ * with dst_capacity writable bytes behind it. An address may lie in ANOTHER GPU's memory (peer access enabled / an
+ * NVLink-mapped symmetric buffer): the encoder's own stores are then the transfer, there is no packed send buffer, no
+ * size exchange and no copy; the receiver finds the stream's size in its header (total_bytes, FORMAT.md §1) and decodes
+ * its slots with bfsc_decompress_batch (d_in_offsets = the slots' offsets: a stream may be shorter than its span). The
+ * bytes at d_dst[i] are identical to stream i of bfsc_compress_batch_codec. d_out_bytes[0..n_buf) (device, written):
+ * total_bytes of each stream, 0 for a stream that did not fit dst_capacity (BFSC_ERR_DST_TOO_SMALL in *d_status; nothing
+ * is written beyond a destination's capacity) or whose address is 0 or misaligned (BFSC_ERR_INVALID_ARG in *d_status).
+ * Workspace: bfsc_workspace_bytes(total IDs, n_buf). Complete (visible to the owner of the destination) when the call's
+ * last kernel has finished: order the receiver's decode behind it with an event, a stream-ordered collective or a
+ * symmetric-memory barrier. BFSC_CODEC_FLAG_RAW_FALLBACK: BFSC_ERR_UNSUPPORTED as for every batch call. */
+bfsc_status bfsc_compress_batch_scatter(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_offsets, size_t n_buf,
+                                        bfsc_dtype t, size_t raw_threshold_bytes,
+                                        void* const* d_dst, size_t dst_capacity, uint64_t* d_out_bytes,
+                                        void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                        void* cuda_stream);
+
 /* The receive side of the same exchange. d_in_offsets: n_buf+1 BYTE offsets
  * of the streams inside d_in (each a multiple of 16). IDs are written back to back at d_ids;
  * d_id_offsets[0..n_buf] (device, written) are their ELEMENT offsets. */

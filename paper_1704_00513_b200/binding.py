@@ -26,7 +26,7 @@ CODEC_FLAG_RAW_FALLBACK = 0x200         # FORMAT.md §8, OR-ed into the codec of
 EXPORTS = [
     "bfsc_version", "bfsc_compress_bound", "bfsc_batch_compress_bound", "bfsc_workspace_bytes",
     "bfsc_compress", "bfsc_decompress", "bfsc_compress_batch", "bfsc_decompress_batch",
-    "bfsc_compress_codec", "bfsc_compress_batch_codec",
+    "bfsc_compress_codec", "bfsc_compress_batch_codec", "bfsc_compress_batch_scatter",
     "bfsc_bitmap_workspace_bytes", "bfsc_compress_bitmap", "bfsc_decompress_to_bitmap", "bfsc_compress_noalloc",
     "bfsc_decompress_to_frontier",
     "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
@@ -75,6 +75,8 @@ def lib():
         L.bfsc_compress_codec.argtypes = [i32, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_compress_batch_codec.restype = i32
         L.bfsc_compress_batch_codec.argtypes = [i32, vp, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_compress_batch_scatter.restype = i32
+        L.bfsc_compress_batch_scatter.argtypes = [i32, vp, vp, sz, i32, sz, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_decompress.restype = i32
         L.bfsc_decompress.argtypes = [vp, sz, i32, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_compress_batch.restype = i32
@@ -206,6 +208,15 @@ def compress_batch_codec(codec, d_ids, d_in_offsets, n_buf, W, raw_threshold_byt
                                            _ptr(d_out), d_out.numel(), _ptr(d_out_offsets), _ptr(d_workspace),
                                            d_workspace.numel(), _ptr(d_status), ctypes.c_void_p(_stream())),
            "bfsc_compress_batch_codec")
+
+
+def compress_batch_scatter(codec, d_ids, d_in_offsets, n_buf, W, raw_threshold_bytes, d_dst, dst_capacity, d_out_bytes,
+                           d_workspace, d_status):
+    """d_dst: int64 device tensor of n_buf device addresses (tensor.data_ptr() values; may be peer-mapped)."""
+    _check(lib().bfsc_compress_batch_scatter(codec, _ptr(d_ids), _ptr(d_in_offsets), n_buf, W, raw_threshold_bytes,
+                                             _ptr(d_dst), dst_capacity, _ptr(d_out_bytes), _ptr(d_workspace),
+                                             d_workspace.numel(), _ptr(d_status), ctypes.c_void_p(_stream())),
+           "bfsc_compress_batch_scatter")
 
 
 def decompress_batch(d_in, d_in_offsets, n_buf, W, d_ids, d_id_offsets, d_workspace, d_status):

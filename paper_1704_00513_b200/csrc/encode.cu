@@ -33,6 +33,9 @@ struct EncArgs {
     unsigned long long out_cap;
     unsigned long long* out_off;        // n_buf+1 (batch) or nullptr
     unsigned long long* out_total;      // single: *d_out_bytes, or nullptr
+    const unsigned long long* dst;      // bfsc_compress_batch_scatter: n_buf device ADDRESSES, stream i is written at dst[i] (out == nullptr,
+    unsigned long long dst_cap;         //   out_cap == ~0: `out + offset` below is the address itself); bytes behind every dst[i]
+    unsigned long long* out_sizes;      //   n_buf stream sizes (0: the stream did not fit / bad address)
     uint32_t* status;
     WsView ws;
 };
@@ -373,7 +376,8 @@ __device__ __forceinline__ unsigned long long lookback(const unsigned long long*
 // fast path (with 320-byte slots a stream of 22-bit gaps took 141 us instead of 37). u64: 288 B (b = 17), so that
 // two CTAs of the batch instantiation (1 KB blocks staged, 10 KB of bookkeeping) still fit one SM; larger u64
 // blocks (gaps over 2^17 between sorted 64-bit IDs) take the slow path.
-// kSrc: where the IDs come from — 0: one ID array, 1: a batch of ID arrays, 2: a frontier bitmap (FORMAT.md §9). A bitmap
+// kSrc: where the IDs come from — 0: one ID array, 1: a batch of ID arrays, 2: a frontier bitmap (FORMAT.md §9), 3: a batch
+// whose streams go to one destination address each (bfsc_compress_batch_scatter) instead of back to back. A bitmap
 // has no ID array for the slow path to re-read, so its image slots hold every block (544 B) for both widths (deltas of a
 // bitmap of < 2^32 bits fit 32 bits), and each worker warp gets a landing area for the bitmap words of its 8 blocks.
 template <int W, int kSrc = 0> struct ImgCfg {
@@ -409,7 +413,7 @@ constexpr int kRing = 8;                                      // ring of tile bo
 template <int W, int kSrc>
 __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArgs a) {
     using T = typename IdT<W>::T;
-    constexpr bool kBatch = kSrc == 1, kBits = kSrc == 2;
+    constexpr bool kBatch = kSrc == 1 || kSrc == 3, kBits = kSrc == 2, kScatter = kSrc == 3;
     using Img = ImgCfg<W, kSrc>;
     using Smem = EncSmem<W, kSrc>;
     extern __shared__ __align__(16) uint4 dyn_smem[];    // per worker warp: staging area | kNB image buffers
@@ -531,17 +535,18 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             // earlier tile, if it is published already) are requested BEFORE the sizes are waited for: the tile was
             // posted two tiles ahead, so their latency hides behind the workers' E1/E2
             const unsigned long long g0 = t * kTileR;
-            unsigned long long bf_first[kPer], bf_f0[kPer], bf_f1[kPer], bf_S[kPer];
+            unsigned long long bf_first[kPer], bf_f0[kPer], bf_f1[kPer], bf_S[kPer], bf_dst[kPer];
             uint32_t bf_i[kPer];
             if constexpr (kBatch) {
 #pragma unroll
                 for (int h = 0; h < kPer; h++) {
                     const int jj = kPer * lane + h;
-                    bf_i[h] = 0; bf_first[h] = 0; bf_f0[h] = 0; bf_f1[h] = 0; bf_S[h] = 0;
+                    bf_i[h] = 0; bf_first[h] = 0; bf_f0[h] = 0; bf_f1[h] = 0; bf_S[h] = 0; bf_dst[h] = 0;
                     if (jj < kTileR && g0 + jj < total) {
                         const uint32_t i = s_buf[k & (kRing - 1)][jj];
                         bf_i[h] = i; bf_first[h] = a.ws.blk_first[i]; bf_f0[h] = a.ws.fixed_prefix[i]; bf_f1[h] = a.ws.fixed_prefix[i + 1];
                         if (i > 0) bf_S[h] = ld_volatile_u64(&a.ws.stream_start[i]);     // (0: not known yet, or the stream begins in this tile)
+                        if constexpr (kScatter) bf_dst[h] = a.dst[i];
                     }
                 }
             }
@@ -593,6 +598,8 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             // for nothing else. The directory entries follow AFTER the offsets are posted: a batch call's entry also
             // needs the start of its stream, which a stream that spans in from an earlier tile gets from that tile's
             // scan warp (a poll) — that wait is now off the workers' path.
+            // Scatter calls: a block's place is its offset INSIDE its stream, behind the stream's own destination — so the
+            // start of the stream (in the back-to-back layout the scan runs over) is needed before the offsets can be posted.
             unsigned long long at_h[kPer];
 #pragma unroll
             for (int h = 0; h < kPer; h++) {
@@ -603,8 +610,22 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                     unsigned long long f1 = f1_single;
                     if constexpr (kBatch) f1 = bf_f1[h];
                     const unsigned long long at = f1 + 16ull * (excl + offs[h]);
-                    if (at + (kk[h] >> 14) <= a.out_cap) at_h[h] = at;
-                    else set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+                    if constexpr (kScatter) {
+                        unsigned long long S = 0;
+                        if (bf_first[h] >= g0) S = bf_f0[h] + 16ull * (excl + s_off16[bf_first[h] - g0]);
+                        else if (bf_i[h] > 0) {
+                            S = bf_S[h];
+                            while (S == 0) S = ld_volatile_u64(&a.ws.stream_start[bf_i[h]]);
+                            S -= 1;
+                        }
+                        const unsigned long long rel = at - S;
+                        if (bf_dst[h] == 0 || (bf_dst[h] & 15)) set_status(a.status, BFSC_ERR_INVALID_ARG);
+                        else if (rel + (kk[h] >> 14) <= a.dst_cap) at_h[h] = bf_dst[h] + rel;
+                        else set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+                    } else {
+                        if (at + (kk[h] >> 14) <= a.out_cap) at_h[h] = at;
+                        else set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+                    }
                 }
                 s_at[kp][jj] = at_h[h];
             }
@@ -624,7 +645,8 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                     uint32_t i = 0;
                     if constexpr (kBatch) {
                         i = bf_i[h]; first = bf_first[h]; f0 = bf_f0[h]; f1 = bf_f1[h];
-                        if (at != kSkip) {
+                        if constexpr (kScatter) S = bf_dst[h];           // (`at` is an address here: at - S = the offset in the stream)
+                        else if (at != kSkip) {
                             if (first >= g0) S = f0 + 16ull * (excl + s_off16[first - g0]);
                             else if (i > 0) {            // published by the tile that owns the stream's first block
                                 S = bf_S[h];
@@ -633,7 +655,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                             }
                         }
                     }
-                    BFSC_CHECK(at == kSkip || (at >= S && S + 32 + 4 * (g - first) + 4 <= a.out_cap));
+                    BFSC_CHECK(at == kSkip || (at >= S && (kScatter ? 32 + 4 * (g - first) + 4 <= a.dst_cap : S + 32 + 4 * (g - first) + 4 <= a.out_cap)));
                     if (at != kSkip) reinterpret_cast<uint32_t*>(a.out + S + 32)[g - first] = (uint32_t)((at - S) >> 4);
                     if (!batch && g == total - 1) {      // single buffer: stream header, dir[nb], zero pad
                         const unsigned long long tot = f1 + 16ull * (excl + off) + bytes;
@@ -903,12 +925,22 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     for (uint32_t i = blockIdx.x * warps + (threadIdx.x >> 5); i < a.n_buf; i += gridDim.x * warps) {   // warp = buffer
         const unsigned long long f0 = a.ws.blk_first[i], f1 = a.ws.blk_first[i + 1];
         const unsigned long long f2 = (i + 1 < a.n_buf) ? a.ws.blk_first[i + 2] : f1;
-        if (!ok) { if (a.out_off && lane == 0) a.out_off[i] = 0; continue; }
+        if (!ok) { if (lane == 0) { if (a.out_off) a.out_off[i] = 0; if (a.out_sizes) a.out_sizes[i] = 0; } continue; }
         const unsigned long long s0 = stream_at(i, f0, f1);
         const unsigned long long s1 = (i + 1 < a.n_buf) ? stream_at(i + 1, f1, f2) : a.ws.hdr->total_out;
         const unsigned long long n = buf_count(a, i), total = s1 - s0;
         const bool raw = n * E < a.thr;
         unsigned char* s = a.out + s0;
+        if (a.dst) {                                                      // scatter call: the stream has its own destination
+            const unsigned long long d = a.dst[i];
+            const bool fits = d != 0 && !(d & 15) && total <= a.dst_cap;
+            if (lane == 0) {
+                a.out_sizes[i] = fits ? total : 0ull;
+                if (!fits) set_status(a.status, (d == 0 || (d & 15)) ? BFSC_ERR_INVALID_ARG : BFSC_ERR_DST_TOO_SMALL);
+            }
+            if (!fits) continue;
+            s = reinterpret_cast<unsigned char*>(d);
+        }
         if (lane == 0) {
             if (a.out_off) a.out_off[i] = s0;
             const unsigned long long nb = f1 - f0;
@@ -1526,7 +1558,8 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     constexpr unsigned long long E = W / 8;
     const bool single = a_in.in_off == nullptr;
     const bool degenerate = single && (a_in.n_single == 0 || a_in.n_single * E < a_in.thr);   // no block: header (+ raw copy) only
-    const int per_sm = single ? enc_ctas_per_sm<W, 0>(dev.device) : enc_ctas_per_sm<W, 1>(dev.device);
+    const bool scatter = a_in.dst != nullptr;
+    const int per_sm = single ? enc_ctas_per_sm<W, 0>(dev.device) : scatter ? enc_ctas_per_sm<W, 3>(dev.device) : enc_ctas_per_sm<W, 1>(dev.device);
     if (per_sm < 1) return BFSC_ERR_CUDA;
     int grid = dev.sms * per_sm;                                 // one resident wave (every tile is drawn by ticket: any grid size is correct)
     if (single) {
@@ -1535,7 +1568,7 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         if (n_tiles < (unsigned long long)grid) grid = n_tiles ? (int)n_tiles : 1;
     }
     int small = 0;
-    if (!single && a_in.n_buf <= kSmallMaxBuf && a_in.ws.blk_cap <= kSmallMaxBlocks) {
+    if (!single && !scatter && a_in.n_buf <= kSmallMaxBuf && a_in.ws.blk_cap <= kSmallMaxBlocks) {
         small = enc_small_init<W>(dev.device);
         if (small == 0) return BFSC_ERR_CUDA;
     }
@@ -1574,6 +1607,7 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
     }
     if (!degenerate) {
         if (single) BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 0>, grid, kEncThreads, kSmem, s, a));
+        else if (scatter) BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 3>, grid, kEncThreads, kSmem, s, a));
         else BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 1>, grid, kEncThreads, kSmem, s, a));
     }
     if (!single || degenerate) {
@@ -1624,14 +1658,16 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
 
 static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_off, size_t n_single, size_t n_buf,
                                  bfsc_dtype t, size_t thr, void* d_out, size_t out_cap, uint64_t* d_out_off,
-                                 uint64_t* d_out_total, void* ws, size_t ws_bytes, uint32_t* d_status, void* stream) {
+                                 uint64_t* d_out_total, void* ws, size_t ws_bytes, uint32_t* d_status, void* stream,
+                                 void* const* d_dst = nullptr, uint64_t* d_out_sizes = nullptr) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
     const uint32_t exclusive = ((uint32_t)codec & (uint32_t)BFSC_CODEC_FLAG_EXCLUSIVE) ? 1u : 0u;
     const uint32_t fallback = ((uint32_t)codec & (uint32_t)BFSC_CODEC_FLAG_RAW_FALLBACK) ? 1u : 0u;
     codec = (bfsc_codec)((uint32_t)codec & ~(uint32_t)(BFSC_CODEC_FLAG_EXCLUSIVE | BFSC_CODEC_FLAG_RAW_FALLBACK));
     if (codec != BFSC_CODEC_PFOR && codec != BFSC_CODEC_BP128) return BFSC_ERR_INVALID_ARG;
     if (fallback && d_in_off) return BFSC_ERR_UNSUPPORTED;                  // FORMAT.md §8: single-buffer calls
-    if (!d_out || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
+    if ((!d_out && !d_dst) || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
+    if (d_dst && (d_out || !d_in_off || !d_out_sizes)) return BFSC_ERR_INVALID_ARG;     // scatter: batch calls, no common output
     if (((uintptr_t)d_ids & 15) || ((uintptr_t)d_out & 15) || ((uintptr_t)ws & 15)) return BFSC_ERR_INVALID_ARG;
     if (!d_ids && (d_in_off || n_single)) return BFSC_ERR_INVALID_ARG;
     EncArgs a = {};
@@ -1640,6 +1676,10 @@ static bfsc_status encode_common(bfsc_codec codec, const void* d_ids, const uint
     a.ids = d_ids; a.in_off = (const unsigned long long*)d_in_off; a.n_single = n_single;
     a.n_buf = (uint32_t)n_buf; a.codec = (uint32_t)codec; a.exclusive = exclusive; a.grid = 0; a.thr = thr; a.out = (unsigned char*)d_out; a.out_cap = out_cap;
     a.out_off = (unsigned long long*)d_out_off; a.out_total = (unsigned long long*)d_out_total; a.status = d_status;
+    if (d_dst) {                                         // out == nullptr: offsets into it are addresses
+        a.dst = reinterpret_cast<const unsigned long long*>(d_dst); a.dst_cap = out_cap; a.out_cap = ~0ull;
+        a.out_sizes = (unsigned long long*)d_out_sizes;
+    }
     return t == BFSC_U32 ? launch_encode<32>(a, (cudaStream_t)stream) : launch_encode<64>(a, (cudaStream_t)stream);
 }
 
@@ -1761,4 +1801,14 @@ extern "C" bfsc_status bfsc_compress_batch(const void* d_ids, const uint64_t* d_
                                            size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
     return bfsc_compress_batch_codec(BFSC_CODEC_PFOR, d_ids, d_in_offsets, n_buf, t, raw_threshold_bytes, d_out,
                                      out_capacity, d_out_offsets, d_workspace, workspace_bytes, d_status, cuda_stream);
+}
+
+extern "C" bfsc_status bfsc_compress_batch_scatter(bfsc_codec codec, const void* d_ids, const uint64_t* d_in_offsets,
+                                                   size_t n_buf, bfsc_dtype t, size_t raw_threshold_bytes,
+                                                   void* const* d_dst, size_t dst_capacity, uint64_t* d_out_bytes,
+                                                   void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                                   void* cuda_stream) {
+    if (!d_in_offsets || !d_dst || !d_out_bytes) return BFSC_ERR_INVALID_ARG;
+    return bfsc::encode_common(codec, d_ids, d_in_offsets, 0, n_buf, t, raw_threshold_bytes, nullptr, dst_capacity,
+                               nullptr, nullptr, d_workspace, workspace_bytes, d_status, cuda_stream, d_dst, d_out_bytes);
 }

@@ -68,7 +68,47 @@ def run_batch(B, oracle_mod, ids_t, off_t, W, thr, check_oracle=True, codec=PFOR
     assert torch.equal(id_off.cpu(), off_t)
     assert torch.equal(back[:n].cpu(), ids_t)
     assert bool((back[n:] == -1).all())
+    run_scatter(B, d_ids, d_off, counts, W, thr, codec, out, out_off, ids_t, off_t)
     return gpu_bytes, gpu_off
+
+
+def run_scatter(B, d_ids, d_off, counts, W, thr, codec, out, out_off, ids_t, off_t):
+    """bfsc_compress_batch_scatter on the same batch: stream i lands in slot i of a slotted receive buffer (a guard
+    zone behind every slot), byte-identical to stream i of the back-to-back output `out` (which the caller has compared
+    with the oracle); then bfsc_decompress_batch straight from the slots."""
+    dev = d_ids.device
+    n, n_buf = ids_t.numel(), len(counts)
+    slot = max([B.compress_bound(c, W) for c in set(counts)] + [32])
+    pitch = slot + 48                                          # (a multiple of 16; 48 guard bytes)
+    if n_buf == 0 or n_buf * pitch > (1 << 28):
+        return
+    recv = torch.full((n_buf * pitch,), 0xCD, dtype=torch.uint8, device=dev)
+    dst = recv.data_ptr() + pitch * torch.arange(n_buf, dtype=torch.int64, device=dev)
+    sizes = torch.full((n_buf,), -1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress_batch_scatter(codec, d_ids, d_off, n_buf, W, thr, dst, slot, sizes, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    assert torch.equal(sizes, out_off[1:] - out_off[:-1])
+    # every slot: the stream, then untouched bytes up to the next slot
+    col = torch.arange(pitch, device=dev).unsqueeze(0)
+    live = col < sizes.unsqueeze(1)
+    src_idx = (out_off[:-1].unsqueeze(1) + col).clamp_(max=out.numel() - 1)
+    expect = torch.where(live, out[src_idx], torch.full_like(out[:1], 0xCD))
+    got = recv.view(n_buf, pitch)
+    if not torch.equal(got, expect):
+        bad = torch.nonzero(got != expect)[0].tolist()
+        raise AssertionError(f"scatter: slot {bad[0]} differs at byte {bad[1]} (stream of {int(sizes[bad[0]])} bytes)")
+    # the receive side: decode the slots where they lie (a stream is shorter than its span)
+    slot_off = pitch * torch.arange(n_buf + 1, dtype=torch.int64, device=dev)
+    back = torch.full((n + 4,), -1, dtype=ids_t.dtype, device=dev)
+    id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    B.decompress_batch(recv, slot_off, n_buf, W, back, id_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    assert torch.equal(id_off.cpu(), off_t)
+    assert torch.equal(back[:n].cpu(), ids_t)
 
 
 def run_single(B, oracle_mod, ids_t, W, thr, codec=PFOR):
@@ -1051,3 +1091,57 @@ def test_mixed_calls_overlap_on_four_streams(B, oracle_mod):
                 assert np.array_equal(j["oo"].cpu().numpy().astype(np.uint64), ro)
             assert np.array_equal(j["out"][:len(ref)].cpu().numpy(), ref)
             assert torch.equal(j["back"][:j["n"]], j["ids"])
+
+
+def test_batch_scatter_errors(B, oracle_mod):
+    """bfsc_compress_batch_scatter: a stream that does not fit its destination is reported (size 0, DST_TOO_SMALL) and
+    nothing is written beyond any destination's capacity while the other streams arrive intact; a null or misaligned
+    destination is INVALID_ARG on the device; host-side argument errors; the RAW-fallback flag is UNSUPPORTED."""
+    dev = torch.device("cuda")
+    W = 32
+    counts = torch.tensor([1000, 128 * 64 * 3 + 5, 40, 0, 128 * 70])
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=77, W=W)
+    n, n_buf = ids.numel(), counts.numel()
+    d_ids, d_off = ids.to(dev), off.to(dev)
+    ref, ref_off = oracle_mod.compress_batch(_np(ids, W), off.numpy().astype(np.uint64), 0)
+    sizes_ref = np.diff(ref_off.astype(np.int64))
+    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    cap = int(sizes_ref[4])                                    # stream 4 fits exactly, stream 1 (three tiles) does not
+    assert sizes_ref[1] > cap > sizes_ref[0]
+    pitch = (cap + 15) // 16 * 16 + 64
+    recv = torch.full((n_buf * pitch,), 0xCD, dtype=torch.uint8, device=dev)
+    dst = recv.data_ptr() + pitch * torch.arange(n_buf, dtype=torch.int64, device=dev)
+    sizes = torch.full((n_buf,), -1, dtype=torch.int64, device=dev)
+    B.compress_batch_scatter(PFOR, d_ids, d_off, n_buf, W, 0, dst, cap, sizes, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_DST_TOO_SMALL
+    got = recv.view(n_buf, pitch).cpu().numpy()
+    for i in range(n_buf):
+        if i == 1:
+            assert int(sizes[i]) == 0
+        else:
+            assert int(sizes[i]) == sizes_ref[i]
+            assert np.array_equal(got[i, :sizes_ref[i]], ref[int(ref_off[i]):int(ref_off[i + 1])]), f"stream {i}"
+            assert (got[i, sizes_ref[i]:] == 0xCD).all()
+        assert (got[i, cap:] == 0xCD).all(), f"slot {i}: wrote beyond its capacity"
+    # a null and a misaligned destination
+    cap2 = int(sizes_ref.max())
+    pitch2 = cap2 + 64
+    recv2 = torch.empty(n_buf * pitch2, dtype=torch.uint8, device=dev)
+    for bad_addr in (0, recv2.data_ptr() + 2 * pitch2 + 4):
+        recv2.fill_(0xCD); status.zero_(); sizes.fill_(-1)
+        dst2 = recv2.data_ptr() + pitch2 * torch.arange(n_buf, dtype=torch.int64, device=dev)
+        dst2[2] = bad_addr
+        B.compress_batch_scatter(PFOR, d_ids, d_off, n_buf, W, 0, dst2, cap2, sizes, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == B.ERR_INVALID_ARG
+        assert int(sizes[2]) == 0 and [int(sizes[i]) for i in (0, 1, 3, 4)] == [int(sizes_ref[i]) for i in (0, 1, 3, 4)]
+        assert bool((recv2.view(n_buf, pitch2)[2] == 0xCD).all())
+    # host-side rejections: nothing is enqueued
+    status.zero_()
+    for kwargs in (dict(dst=None), dict(sizes=None), dict(codec=PFOR | B.CODEC_FLAG_RAW_FALLBACK, code=B.ERR_UNSUPPORTED)):
+        with pytest.raises(B.BfscError) as e:
+            B.compress_batch_scatter(kwargs.get("codec", PFOR), d_ids, d_off, n_buf, W, 0, kwargs.get("dst", dst), cap,
+                                     kwargs.get("sizes", sizes), ws, status)
+        assert e.value.code == kwargs.get("code", B.ERR_INVALID_ARG)
