@@ -1040,6 +1040,12 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
     if (threadIdx.x == 0) bad = 0;
     if (threadIdx.x < kSmallIters) s_sum[threadIdx.x] = 0;
     __syncthreads();
+    auto zero_outputs = [&]() {                                      // an error of the whole call: every offset / size reads 0
+        for (uint32_t i = rank * kSmallThreads + threadIdx.x; i <= a.n_buf; i += kSmallCtas * kSmallThreads) {
+            if (a.out_off) a.out_off[i] = 0;
+            if (a.out_sizes && i < a.n_buf) a.out_sizes[i] = 0;
+        }
+    };
     {
         constexpr int kIpt = kSmallMaxBuf / kSmallThreads;           // 4
         Scan2 v[kIpt], sum{0, 0};
@@ -1070,7 +1076,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         __syncthreads();
         if (bad || tot.a > a.ws.blk_cap || tot.a > kSmallMaxBlocks) {        // (the same decision in every CTA of the cluster)
             if (rank == 0 && threadIdx.x == 0) set_status(a.status, BFSC_ERR_INVALID_ARG);
-            for (uint32_t i = rank * kSmallThreads + threadIdx.x; i <= a.n_buf; i += kSmallCtas * kSmallThreads) a.out_off[i] = 0;
+            zero_outputs();
             return;
         }
     }
@@ -1145,9 +1151,12 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
     const unsigned long long total_out = s_fixed[a.n_buf] + 16ull * grand16;
     if (total_out > a.out_cap) {                                     // (the same decision in every CTA)
         if (rank == 0 && threadIdx.x == 0) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
-        for (uint32_t i = rank * kSmallThreads + threadIdx.x; i <= a.n_buf; i += kSmallCtas * kSmallThreads) a.out_off[i] = 0;
+        zero_outputs();
         return;
     }
+    auto dst_ok = [&](unsigned long long d, unsigned long long stream_bytes) -> bool {   // scatter calls: a usable destination that holds the stream
+        return d != 0 && !(d & 15) && stream_bytes <= a.dst_cap;
+    };
     // scan value at block g: 16-B units of block bytes before it (g = total: all of them)
     auto scan_at = [&](uint32_t g) -> unsigned long long {
         return g >= total ? grand16 : (unsigned long long)s_tsum[g / kTileR] + s_off16[g / kTileR][g % kTileR];
@@ -1173,12 +1182,18 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         const bool late = (stored & kLateBit) != 0, fast = key != 0 && !late;
         const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
         unsigned long long at = 0;
+        bool placed = key != 0;                                      // (scatter calls: and the stream fits its destination)
         if (key != 0) {
             at = s_fixed[i + 1] + 16ull * scan_at(g);
-            if (l == 0) {                                            // directory entry (FORMAT.md §1)
-                const unsigned long long S = stream_at(i);
-                reinterpret_cast<uint32_t*>(a.out + S + 32)[g - s_first[i]] = (uint32_t)((at - S) >> 4);
+            unsigned long long S = stream_at(i);
+            if (a.dst) {                                             // the stream has its own destination: `at` becomes an address
+                const unsigned long long dsti = a.dst[i];
+                placed = dst_ok(dsti, stream_at(i + 1) - S);
+                at = dsti + (at - S);
+                S = dsti;
             }
+            if (l == 0 && placed)                                    // directory entry (FORMAT.md §1)
+                reinterpret_cast<uint32_t*>(a.out + S + 32)[g - s_first[i]] = (uint32_t)((at - S) >> 4);
         }
         uint32_t d[32];
         bool wide_lane = false;
@@ -1194,24 +1209,34 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_enc_small(EncArgs a) {
         __syncwarp();
         BFSC_CHECK(key == 0 || at + (key >> 14) <= a.out_cap);
         BFSC_CHECK(!fast || (key >> 14) <= (uint32_t)(Smem::kSlotChunks * 16));
-        if (fast) {
+        if (fast && placed) {
             const uint4* src = reinterpret_cast<const uint4*>(img);
             uint4* dst = reinterpret_cast<uint4*>(a.out + at);
             for (uint32_t c = l; c < (key >> 18); c += 4) __stcs(dst + c, src[c]);
         }
-        if (__any_sync(kFull, late)) late_emit<W>(ids + xoff, m, key, late ? a.out + at : nullptr);
+        if (__any_sync(kFull, late)) late_emit<W>(ids + xoff, m, key, late && placed ? a.out + at : nullptr);
         __syncwarp();                                                // image and staged IDs are free again
     }
 
-    if (a.n_buf == 0 && rank == 0 && threadIdx.x == 0) a.out_off[0] = total_out;
+    if (a.n_buf == 0 && rank == 0 && threadIdx.x == 0 && a.out_off) a.out_off[0] = total_out;
     // ---- stream headers, directory tails, E5 (RAW copies), out_offsets: a warp per stream, the streams dealt round the cluster
     for (uint32_t i = rank * kEncWorkers + warp; i < a.n_buf; i += kSmallCtas * kEncWorkers) {
         const unsigned long long s0 = stream_at(i), s1 = stream_at(i + 1);
         BFSC_CHECK(s0 + 32 <= s1 && s1 <= a.out_cap);
         const unsigned long long o0 = a.in_off[i], n = a.in_off[i + 1] - o0, tot = s1 - s0;
-        if (lane == 0) { a.out_off[i] = s0; if (i + 1 == a.n_buf) a.out_off[a.n_buf] = s1; }
+        if (lane == 0 && a.out_off) { a.out_off[i] = s0; if (i + 1 == a.n_buf) a.out_off[a.n_buf] = s1; }
         const bool raw_s = n * E < a.thr;
         unsigned char* s = a.out + s0;
+        if (a.dst) {
+            const unsigned long long dsti = a.dst[i];
+            const bool fits = dst_ok(dsti, tot);
+            if (lane == 0) {
+                a.out_sizes[i] = fits ? tot : 0ull;
+                if (!fits) set_status(a.status, (dsti == 0 || (dsti & 15)) ? BFSC_ERR_INVALID_ARG : BFSC_ERR_DST_TOO_SMALL);
+            }
+            if (!fits) continue;
+            s = reinterpret_cast<unsigned char*>(dsti);
+        }
         if (lane == 0) {
             const unsigned long long nb = s_first[i + 1] - s_first[i];
             uint4 h0, h1;
@@ -1568,7 +1593,7 @@ static bfsc_status launch_encode(const EncArgs& a_in, cudaStream_t s) {
         if (n_tiles < (unsigned long long)grid) grid = n_tiles ? (int)n_tiles : 1;
     }
     int small = 0;
-    if (!single && !scatter && a_in.n_buf <= kSmallMaxBuf && a_in.ws.blk_cap <= kSmallMaxBlocks) {
+    if (!single && a_in.n_buf <= kSmallMaxBuf && a_in.ws.blk_cap <= kSmallMaxBlocks) {
         small = enc_small_init<W>(dev.device);
         if (small == 0) return BFSC_ERR_CUDA;
     }

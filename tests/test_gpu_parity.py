@@ -1099,45 +1099,46 @@ def test_batch_scatter_errors(B, oracle_mod):
     destination is INVALID_ARG on the device; host-side argument errors; the RAW-fallback flag is UNSUPPORTED."""
     dev = torch.device("cuda")
     W = 32
-    counts = torch.tensor([1000, 128 * 64 * 3 + 5, 40, 0, 128 * 70])
-    ids, off = streams.batch_of_streams(counts, 16.0, seed=77, W=W)
-    n, n_buf = ids.numel(), counts.numel()
-    d_ids, d_off = ids.to(dev), off.to(dev)
-    ref, ref_off = oracle_mod.compress_batch(_np(ids, W), off.numpy().astype(np.uint64), 0)
-    sizes_ref = np.diff(ref_off.astype(np.int64))
-    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
-    status = torch.zeros(1, dtype=torch.int32, device=dev)
-    cap = int(sizes_ref[4])                                    # stream 4 fits exactly, stream 1 (three tiles) does not
-    assert sizes_ref[1] > cap > sizes_ref[0]
-    pitch = (cap + 15) // 16 * 16 + 64
-    recv = torch.full((n_buf * pitch,), 0xCD, dtype=torch.uint8, device=dev)
-    dst = recv.data_ptr() + pitch * torch.arange(n_buf, dtype=torch.int64, device=dev)
-    sizes = torch.full((n_buf,), -1, dtype=torch.int64, device=dev)
-    B.compress_batch_scatter(PFOR, d_ids, d_off, n_buf, W, 0, dst, cap, sizes, ws, status)
-    torch.cuda.synchronize()
-    assert int(status.item()) == B.ERR_DST_TOO_SMALL
-    got = recv.view(n_buf, pitch).cpu().numpy()
-    for i in range(n_buf):
-        if i == 1:
-            assert int(sizes[i]) == 0
-        else:
-            assert int(sizes[i]) == sizes_ref[i]
-            assert np.array_equal(got[i, :sizes_ref[i]], ref[int(ref_off[i]):int(ref_off[i + 1])]), f"stream {i}"
-            assert (got[i, sizes_ref[i]:] == 0xCD).all()
-        assert (got[i, cap:] == 0xCD).all(), f"slot {i}: wrote beyond its capacity"
-    # a null and a misaligned destination
-    cap2 = int(sizes_ref.max())
-    pitch2 = cap2 + 64
-    recv2 = torch.empty(n_buf * pitch2, dtype=torch.uint8, device=dev)
-    for bad_addr in (0, recv2.data_ptr() + 2 * pitch2 + 4):
-        recv2.fill_(0xCD); status.zero_(); sizes.fill_(-1)
-        dst2 = recv2.data_ptr() + pitch2 * torch.arange(n_buf, dtype=torch.int64, device=dev)
-        dst2[2] = bad_addr
-        B.compress_batch_scatter(PFOR, d_ids, d_off, n_buf, W, 0, dst2, cap2, sizes, ws, status)
+    # the one-cluster kernel (<= 2048 blocks), then the general path (plan -> tiles -> streams)
+    for counts in (torch.tensor([1000, 128 * 64 * 3 + 5, 40, 0, 128 * 70]), torch.tensor([1000, 128 * 64 * 40 + 5, 40, 0, 128 * 700])):
+        ids, off = streams.batch_of_streams(counts, 16.0, seed=77, W=W)
+        n, n_buf = ids.numel(), counts.numel()
+        d_ids, d_off = ids.to(dev), off.to(dev)
+        ref, ref_off = oracle_mod.compress_batch(_np(ids, W), off.numpy().astype(np.uint64), 0)
+        sizes_ref = np.diff(ref_off.astype(np.int64))
+        ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+        status = torch.zeros(1, dtype=torch.int32, device=dev)
+        cap = int(sizes_ref[4])                                    # stream 4 fits exactly, stream 1 (several tiles) does not
+        assert sizes_ref[1] > cap > sizes_ref[0]
+        pitch = (cap + 15) // 16 * 16 + 64
+        recv = torch.full((n_buf * pitch,), 0xCD, dtype=torch.uint8, device=dev)
+        dst = recv.data_ptr() + pitch * torch.arange(n_buf, dtype=torch.int64, device=dev)
+        sizes = torch.full((n_buf,), -1, dtype=torch.int64, device=dev)
+        B.compress_batch_scatter(PFOR, d_ids, d_off, n_buf, W, 0, dst, cap, sizes, ws, status)
         torch.cuda.synchronize()
-        assert int(status.item()) == B.ERR_INVALID_ARG
-        assert int(sizes[2]) == 0 and [int(sizes[i]) for i in (0, 1, 3, 4)] == [int(sizes_ref[i]) for i in (0, 1, 3, 4)]
-        assert bool((recv2.view(n_buf, pitch2)[2] == 0xCD).all())
+        assert int(status.item()) == B.ERR_DST_TOO_SMALL
+        got = recv.view(n_buf, pitch).cpu().numpy()
+        for i in range(n_buf):
+            if i == 1:
+                assert int(sizes[i]) == 0
+            else:
+                assert int(sizes[i]) == sizes_ref[i]
+                assert np.array_equal(got[i, :sizes_ref[i]], ref[int(ref_off[i]):int(ref_off[i + 1])]), f"stream {i}"
+                assert (got[i, sizes_ref[i]:] == 0xCD).all()
+            assert (got[i, cap:] == 0xCD).all(), f"slot {i}: wrote beyond its capacity"
+        # a null and a misaligned destination
+        cap2 = int(sizes_ref.max())
+        pitch2 = cap2 + 64
+        recv2 = torch.empty(n_buf * pitch2, dtype=torch.uint8, device=dev)
+        for bad_addr in (0, recv2.data_ptr() + 2 * pitch2 + 4):
+            recv2.fill_(0xCD); status.zero_(); sizes.fill_(-1)
+            dst2 = recv2.data_ptr() + pitch2 * torch.arange(n_buf, dtype=torch.int64, device=dev)
+            dst2[2] = bad_addr
+            B.compress_batch_scatter(PFOR, d_ids, d_off, n_buf, W, 0, dst2, cap2, sizes, ws, status)
+            torch.cuda.synchronize()
+            assert int(status.item()) == B.ERR_INVALID_ARG
+            assert int(sizes[2]) == 0 and [int(sizes[i]) for i in (0, 1, 3, 4)] == [int(sizes_ref[i]) for i in (0, 1, 3, 4)]
+            assert bool((recv2.view(n_buf, pitch2)[2] == 0xCD).all())
     # host-side rejections: nothing is enqueued
     status.zero_()
     for kwargs in (dict(dst=None), dict(sizes=None), dict(codec=PFOR | B.CODEC_FLAG_RAW_FALLBACK, code=B.ERR_UNSUPPORTED)):
