@@ -44,10 +44,11 @@ def peak_gbs():
 
 
 class Runner:
-    def __init__(self, dev, reps=5, codec=B.CODEC_PFOR, graph=False, cpu_timer=None):
+    def __init__(self, dev, reps=5, codec=B.CODEC_PFOR, graph=False, cpu_timer=None, scatter=False):
         """cpu_timer(ids: device tensor, off: device int64 offsets, W, thr, codec) -> (encode seconds, decode seconds)
         of a CPU implementation on the same buffers, or None (bench.py --config passes the oracle's)."""
         self.dev, self.reps, self.codec, self.graph, self.cpu_timer = dev, reps, codec, graph, cpu_timer
+        self.scatter = scatter                               # batch rows: the data path of exchange.SlotExchange (streams into / out of slots)
         self.totals = []                                     # one dict per report row marked as a total (--json)
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
         self.peak = peak_gbs()
@@ -151,6 +152,20 @@ class Runner:
             comp = int(nbytes.item())
             return {"n": n, "n_buf": 1, "raw": n * (W // 8), "comp": comp, "enc_ms": enc, "dec_ms": dec,
                     "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound} | cpu
+        if self.scatter:
+            # every stream into its own slot of a receive buffer (bfsc_compress_batch_scatter), decoded where it lies
+            slot = max([B.compress_bound(c, W) for c in set(counts)] + [32])
+            pitch = (slot + 255) // 256 * 256
+            recvs = [torch.empty(n_buf * pitch, dtype=torch.uint8, device=dev) for _ in range(copies)]
+            dsts = [r.data_ptr() + pitch * torch.arange(n_buf, dtype=torch.int64, device=dev) for r in recvs]
+            slot_off = pitch * torch.arange(n_buf + 1, dtype=torch.int64, device=dev)
+            sizes = torch.zeros(n_buf, dtype=torch.int64, device=dev)
+            enc, enc_iso = self._time([(lambda c=c: B.compress_batch_scatter(self.codec, pads[c], off, n_buf, W, thr, dsts[c], slot, sizes, ws, status)) for c in range(copies)])
+            dec, dec_iso = self._time([(lambda c=c: B.decompress_batch(recvs[c], slot_off, n_buf, W, backs[c], id_off, ws, status)) for c in range(copies)])
+            assert int(status.item()) == 0
+            assert torch.equal(backs[copies - 1][:n], ids) and torch.equal(id_off, off), "decode != input"
+            return {"n": n, "n_buf": n_buf, "raw": n * (W // 8), "comp": int(sizes.sum().item()), "enc_ms": enc, "dec_ms": dec,
+                    "enc_iso_ms": enc_iso, "dec_iso_ms": dec_iso, "host_bound": self.host_bound} | cpu
         enc, enc_iso = self._time([(lambda c=c: B.compress_batch_codec(self.codec, pads[c], off, n_buf, W, thr, outs[c], out_off, ws, status)) for c in range(copies)])
         dec, dec_iso = self._time([(lambda c=c: B.decompress_batch(outs[c], out_off, n_buf, W, backs[c], id_off, ws, status)) for c in range(copies)])
         assert int(status.item()) == 0
@@ -248,7 +263,10 @@ def run(a, cpu_timer=None):
     assert torch.cuda.is_available(), "needs a CUDA device (there is no CPU fallback)"
     dev = torch.device("cuda:0")
     B.lib()
-    R = Runner(dev, a.reps, B.CODEC_BP128 if a.codec == "bp128" else B.CODEC_PFOR, a.graph, cpu_timer)
+    R = Runner(dev, a.reps, B.CODEC_BP128 if a.codec == "bp128" else B.CODEC_PFOR, a.graph, cpu_timer, a.scatter)
+    if a.scatter:
+        print("batch rows: bfsc_compress_batch_scatter into a slotted receive buffer (one slot per stream, the layout of "
+              "exchange.SlotExchange) and bfsc_decompress_batch straight from the slots\n")
     if a.graph:
         print("timed runs replayed from CUDA graphs captured around the C-ABI calls (device-side time of the kernel chain)\n")
     print(f"encoder rule: {'BP128-D1 (mode 2, no exceptions)' if a.codec == 'bp128' else 'PFOR-D1 (mode 1)'}\n")
@@ -271,6 +289,7 @@ def add_arguments(ap):
     ap.add_argument("--codec", default="pfor", choices=["pfor", "bp128"], help="encoder rule (bfsc_codec)")
     ap.add_argument("--graph", action="store_true", help="replay the timed calls from captured CUDA graphs")
     ap.add_argument("--json", action="store_true", help="one JSON line with the totals after the table")
+    ap.add_argument("--scatter", action="store_true", help="batch rows through bfsc_compress_batch_scatter (streams into slots)")
 
 
 def main():
