@@ -231,6 +231,20 @@ bfsc_status bfsc_decompress_to_frontier(const void* d_in, size_t in_bytes, bfsc_
                                         uint32_t* d_frontier, uint32_t* d_visited, size_t n_bits, uint64_t* d_n_ids,
                                         void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream);
 
+/* The receive side of a whole exchange in one call (Algorithm 4 lines 10-13 over all received streams, PAPER.md
+ * L1369-1377): bfsc_decompress_to_frontier applied to the n_buf streams at d_in + d_in_offsets[i] (as in
+ * bfsc_decompress_batch: byte offsets, multiples of 16, a stream may be shorter than its span — the slots of a receive
+ * buffer). The result is the union: an ID that several streams carry, or that is visited already, enters the frontier
+ * once or not at all, whatever the order. d_visited == NULL: no filter, every ID is OR-ed into d_frontier (the batch form
+ * of bfsc_decompress_to_bitmap). *d_n_ids (device, written) = IDs decoded over all streams. Workspace:
+ * bfsc_workspace_bytes(upper bound of the IDs of all streams together, n_buf); more blocks than it was sized for:
+ * BFSC_ERR_INVALID_ARG in *d_status. At most 8192 streams (more: BFSC_ERR_UNSUPPORTED). Other errors as
+ * bfsc_decompress_to_bitmap. */
+bfsc_status bfsc_decompress_batch_to_frontier(const void* d_in, const uint64_t* d_in_offsets, size_t n_buf, bfsc_dtype t,
+                                              uint64_t id_base, uint32_t* d_frontier, uint32_t* d_visited, size_t n_bits,
+                                              uint64_t* d_n_ids, void* d_workspace, size_t workspace_bytes,
+                                              uint32_t* d_status, void* cuda_stream);
+
 /* End-to-end convenience calls with HOST buffers (pinned memory recommended): copy in,
  * run the device call above, copy the result out, synchronise the stream. d_scratch is a
  * caller-owned device buffer of at least bfsc_host_scratch_bytes(n_ids, t) bytes.

@@ -28,7 +28,7 @@ EXPORTS = [
     "bfsc_compress", "bfsc_decompress", "bfsc_compress_batch", "bfsc_decompress_batch",
     "bfsc_compress_codec", "bfsc_compress_batch_codec", "bfsc_compress_batch_scatter",
     "bfsc_bitmap_workspace_bytes", "bfsc_compress_bitmap", "bfsc_decompress_to_bitmap", "bfsc_compress_noalloc",
-    "bfsc_decompress_to_frontier",
+    "bfsc_decompress_to_frontier", "bfsc_decompress_batch_to_frontier",
     "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
 ]
 
@@ -65,6 +65,8 @@ def lib():
         L.bfsc_decompress_to_bitmap.argtypes = [vp, sz, i32, c.c_uint64, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_decompress_to_frontier.restype = i32
         L.bfsc_decompress_to_frontier.argtypes = [vp, sz, i32, c.c_uint64, vp, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_decompress_batch_to_frontier.restype = i32
+        L.bfsc_decompress_batch_to_frontier.argtypes = [vp, vp, sz, i32, c.c_uint64, vp, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_host_scratch_bytes.restype = sz
         L.bfsc_host_scratch_bytes.argtypes = [sz, i32]
         L.bfsc_compress.restype = i32
@@ -188,6 +190,14 @@ def decompress_to_frontier(d_in, in_bytes, W, id_base, d_frontier, d_visited, n_
     _check(lib().bfsc_decompress_to_frontier(_ptr(d_in), in_bytes, W, id_base, _ptr(d_frontier), _ptr(d_visited), n_bits,
                                              _ptr(d_n_ids), _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
                                              ctypes.c_void_p(_stream())), "bfsc_decompress_to_frontier")
+
+
+def decompress_batch_to_frontier(d_in, d_in_offsets, n_buf, W, id_base, d_frontier, d_visited, n_bits, d_n_ids, d_workspace,
+                                 d_status):
+    _check(lib().bfsc_decompress_batch_to_frontier(_ptr(d_in), _ptr(d_in_offsets), n_buf, W, id_base, _ptr(d_frontier),
+                                                   _ptr(d_visited), n_bits, _ptr(d_n_ids), _ptr(d_workspace),
+                                                   d_workspace.numel(), _ptr(d_status), ctypes.c_void_p(_stream())),
+           "bfsc_decompress_batch_to_frontier")
 
 
 def decompress(d_in, in_bytes, W, d_ids, d_n_ids, d_workspace, d_status):

@@ -362,7 +362,7 @@ struct BlockAt {                       // where the quad's block is
 constexpr uint32_t kSelfMaxStreams = 1024, kSelfMaxBlocks = 2048;
 template <int W, bool kBatch, bool kTma, bool kBits = false, bool kSelf = false>   // kBatch: a.in_off != nullptr; kBits: bits into a.sink instead of IDs into a.ids
 __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kCtasPerSm) k_dec_tiles(DecArgs a) {
-    static_assert(!kSelf || (kBatch && !kTma && !kBits), "kSelf: batch calls");
+    static_assert(!kSelf || (kBatch && !kTma), "kSelf: batch calls");
     constexpr uint32_t kSelfN = kSelf ? kSelfMaxStreams : 0;
     __shared__ unsigned long long s_idpre[kSelfN + 1];                     // kSelf: first ID of every stream (entry n_buf: total)
     __shared__ uint32_t s_first[kSelfN + 2], s_tot16[kSelfN + 1];          //        first block, total_bytes / 16
@@ -633,8 +633,12 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
             if constexpr (kSelf) { id0 = s_idpre[i]; n = s_idpre[i + 1] - id0; }
             else { id0 = a.ws.fixed_prefix[i]; n = a.ws.fixed_prefix[i + 1] - id0; }
             const T* xs = reinterpret_cast<const T*>(s + 32);
-            T* y = reinterpret_cast<T*>(a.ids) + id0;
-            for (unsigned long long t = threadIdx.x; t < n; t += blockDim.x) y[t] = xs[t];
+            if constexpr (kBits) {
+                for (unsigned long long t = threadIdx.x; t < n; t += blockDim.x) set_bits4<T>(a.sink, xs[t], (T)0, (T)0, (T)0, 1);
+            } else {
+                T* y = reinterpret_cast<T*>(a.ids) + id0;
+                for (unsigned long long t = threadIdx.x; t < n; t += blockDim.x) y[t] = xs[t];
+            }
         }
     }
 }
@@ -692,19 +696,25 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     const size_t want = (max_blocks + kDecBlocks - 1) / kDecBlocks;
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
+    const bool bits = a.sink.bm != nullptr;                                        // IDs -> bits of a frontier bitmap
     if (a.in_off && a.n_buf <= kSelfMaxStreams && max_blocks <= kSelfMaxBlocks) {
         // a small batch (both bounds known on the host: stream count, and blocks by the ID capacity / the workspace size):
         // one launch, no plan kernel
-        const int psm = dec_ctas_per_sm<W, true, false, false, true>(dev.device);
+        const int psm = bits ? dec_ctas_per_sm<W, true, false, true, true>(dev.device) : dec_ctas_per_sm<W, true, false, false, true>(dev.device);
         if (psm < 1) return BFSC_ERR_CUDA;
         const int g = want < (size_t)(dev.sms * psm) ? (want ? (int)want : 1) : dev.sms * psm;
-        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false, false, true>, g, DecCfg<W>::kThreads, kSmem, s, a));
+        if (bits) BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false, true, true>, g, DecCfg<W>::kThreads, kSmem, s, a));
+        else BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false, false, true>, g, DecCfg<W>::kThreads, kSmem, s, a));
     } else if (a.in_off && a.n_buf <= kFusedMaxStreams && a.ws.blk_cap < (1ull << 32)) {
         if (!dec_planblocks_init<W>(dev.device)) return BFSC_ERR_CUDA;
+        if (bits && dec_ctas_per_sm<W, true, false, true>(dev.device) < 1) return BFSC_ERR_CUDA;
         size_t pgrid = (a.ws.blk_cap + 1023) / 1024;
         if (pgrid > (size_t)kFusedPlanCtas) pgrid = kFusedPlanCtas;
         BFSC_LAUNCH(launch_dep(k_dec_planblocks<W>, pgrid ? (int)pgrid : 1, 1024, dec_planblocks_smem(a.n_buf), s, a));
-        BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
+        if (bits) BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false, true>, grid, DecCfg<W>::kThreads, kSmem, s, a));
+        else BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
+    } else if (a.in_off && bits) {
+        return BFSC_ERR_UNSUPPORTED;                                               // (more than kFusedMaxStreams streams into a bitmap)
     } else if (a.in_off) {
         const bool gather = a.n_buf >= kHeaderGatherMin && a.ws.blk_cap >= a.n_buf;
         if (gather) {
@@ -743,7 +753,8 @@ static bfsc_status decode_common(const void* d_in, const uint64_t* d_in_off, siz
     a.in = (const unsigned char*)d_in; a.in_off = (const unsigned long long*)d_in_off; a.in_single = in_single;
     a.n_buf = (uint32_t)n_buf; a.ids = d_ids; a.ids_cap = ids_cap; a.id_off = (unsigned long long*)d_id_off;
     a.n_ids_out = (unsigned long long*)d_n_ids; a.status = d_status; a.sink = sink;
-    const size_t max_blocks = (sink.bm ? (size_t)sink.n_bits : ids_cap) / kBlk + n_buf + 1;
+    size_t max_blocks = (sink.bm ? (size_t)sink.n_bits : ids_cap) / kBlk + n_buf + 1;
+    if (sink.bm && d_in_off) max_blocks = ~(size_t)0 >> 8;       // (streams of a batch may repeat IDs: bounded by the workspace only)
     return t == BFSC_U32 ? launch_decode<32>(a, max_blocks, (cudaStream_t)stream)
                          : launch_decode<64>(a, max_blocks, (cudaStream_t)stream);
 }
@@ -791,5 +802,17 @@ extern "C" bfsc_status bfsc_decompress_to_frontier(const void* d_in, size_t in_b
         ((uintptr_t)d_visited & 15) || n_bits > (1ull << 32))
         return BFSC_ERR_INVALID_ARG;
     return bfsc::decode_common(d_in, nullptr, in_bytes, 1, t, nullptr, ~(size_t)0, nullptr, d_n_ids, d_workspace,
+                               workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_frontier, id_base, n_bits, d_status, d_visited});
+}
+
+extern "C" bfsc_status bfsc_decompress_batch_to_frontier(const void* d_in, const uint64_t* d_in_offsets, size_t n_buf,
+                                                         bfsc_dtype t, uint64_t id_base, uint32_t* d_frontier,
+                                                         uint32_t* d_visited, size_t n_bits, uint64_t* d_n_ids,
+                                                         void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                                         void* cuda_stream) {
+    if (!d_in_offsets || !d_n_ids || !d_frontier || d_frontier == d_visited || ((uintptr_t)d_frontier & 15) ||
+        ((uintptr_t)d_visited & 15) || n_bits > (1ull << 32))
+        return BFSC_ERR_INVALID_ARG;
+    return bfsc::decode_common(d_in, d_in_offsets, 0, n_buf, t, nullptr, ~(size_t)0, nullptr, d_n_ids, d_workspace,
                                workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_frontier, id_base, n_bits, d_status, d_visited});
 }

@@ -102,6 +102,13 @@ class SlotExchange:
         self.codec.decompress_batch(self.slots.local, self.slot_off[self._par], self.P, self.W, ids_out, id_offsets,
                                     self.ws, self.status)
 
+    def receive_to_frontier(self, frontier, visited, n_bits, id_base, n_ids):
+        """Algorithm 4 lines 10-13 on the own slots in ONE call (`bfsc_decompress_batch_to_frontier`): every received
+        vertex that `visited` (bitmap of the rank's own vertices id_base .. id_base + n_bits) does not hold yet is set in
+        `visited` and in `frontier`; n_ids (device int64[1]) = IDs received. No ID list is ever written."""
+        self.codec.decompress_batch_to_frontier(self.slots.local, self.slot_off[self._par], self.P, self.W, id_base,
+                                                frontier, visited, n_bits, n_ids, self.ws, self.status)
+
     def exchange(self, ids, in_offsets, ids_out, id_offsets):
         """One level, enqueued on the current stream, nothing read back. Errors: `self.status` (device)."""
         self.send(ids, in_offsets)

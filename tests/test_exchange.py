@@ -176,6 +176,49 @@ def test_slot_exchange_four_ranks_on_one_device(B, oracle_mod, W):
                 assert int(ex[s].sent_bytes[d]) == len(want)
 
 
+@pytest.mark.gpu
+def test_slot_exchange_receive_to_frontier(B):
+    """The receive side fused with the frontier update: each rank ORs what it received into the bitmaps of its own vertex
+    range, filtered by its visited set. Expected bitmaps from set arithmetic on the lists the sources held."""
+    from paper_1704_00513_b200 import exchange
+    dev = torch.device("cuda")
+    W, P, max_ids, n_vertices = 32, 4, 40000, 1 << 22
+    chunk = n_vertices // P
+    nbytes = exchange.SlotExchange.receive_bytes(P, max_ids, W, B)
+    recv = [torch.zeros(nbytes, dtype=torch.uint8, device=dev) for _ in range(P)]
+    ptrs = [t.data_ptr() for t in recv]
+    ex = [exchange.SlotExchange(B, W, r, P, max_ids, _LocalSlots(recv[r], ptrs), raw_threshold_bytes=64) for r in range(P)]
+    g = torch.Generator().manual_seed(5)
+    visited = [(torch.rand(chunk, generator=g) < 0.3) for _ in range(P)]                  # per rank: its own vertices
+    frontier = [torch.zeros(chunk, dtype=torch.bool) for _ in range(P)]
+
+    def pack(bits):                                                                     # bool[chunk] -> int32 words, bit v % 32 of word v / 32
+        w = bits.view(-1, 32).to(torch.int64) << torch.arange(32, dtype=torch.int64)
+        return w.sum(1).to(torch.uint32).view(torch.int32).to(dev)
+
+    d_vis = [pack(v) for v in visited]
+    d_fr = [pack(f) for f in frontier]
+    n_ids = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(P)]
+    for level in (0, 1):
+        inputs = [level_buffers(level, r, P, W, n_vertices, dense=True) for r in range(P)]
+        for r in range(P):
+            ex[r].send(_resident(inputs[r][0], P * max_ids, dev), inputs[r][1].to(dev))
+        for r in range(P):
+            ex[r].receive_to_frontier(d_fr[r], d_vis[r], chunk, r * chunk, n_ids[r])
+        torch.cuda.synchronize()
+        for d in range(P):
+            assert int(ex[d].status.item()) == 0
+            got = torch.zeros(chunk, dtype=torch.bool)
+            for s in range(P):
+                got[inputs[s][2][d] - d * chunk] = True
+            new = got & ~visited[d]
+            frontier[d] |= new
+            visited[d] |= new
+            assert int(n_ids[d]) == sum(len(inputs[s][2][d]) for s in range(P))
+            assert torch.equal(d_fr[d].cpu(), pack(frontier[d]).cpu()), f"level {level}: frontier of rank {d}"
+            assert torch.equal(d_vis[d].cpu(), pack(visited[d]).cpu()), f"level {level}: visited set of rank {d}"
+
+
 @pytest.fixture(scope="module")
 def nccl_world1():
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29631", RANK="0", WORLD_SIZE="1")

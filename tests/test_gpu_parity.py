@@ -982,6 +982,83 @@ def test_decompress_to_frontier(B, oracle_mod, W):
     _frontier_case(B, oracle_mod, np.nonzero(bits)[0].astype(dt), W, 1 << 22, 0, seed=5)
 
 
+def _batch_frontier_case(B, oracle_mod, lists, W, n_bits, id_base, thr, pitch_pad, seed, with_visited=True, expect=0):
+    """lists: the ID arrays of the received streams. The streams (oracle bytes) lie in slots of a receive buffer, each
+    shorter than its span; expected bitmaps: the oracle's single-stream update applied stream after stream."""
+    dev = torch.device("cuda")
+    blobs = [oracle_mod.compress(x, thr) for x in lists]
+    pitch = (max(len(b) for b in blobs) + 15) // 16 * 16 + pitch_pad
+    recv = np.full(len(blobs) * pitch + 16, 0xCD, np.uint8)
+    for i, b in enumerate(blobs):
+        recv[i * pitch:i * pitch + len(b)] = b
+    words = max(4, ((n_bits + 31) // 32 + 3) // 4 * 4)
+    vis0 = streams.frontier_bitmap(words * 32, 0.4, seed=seed + 1)[:words].numpy().view(np.uint32).copy()
+    fr0 = streams.frontier_bitmap(words * 32, 0.1, seed=seed + 2)[:words].numpy().view(np.uint32).copy()
+    d_in = torch.from_numpy(recv).to(dev)
+    d_off = pitch * torch.arange(len(blobs) + 1, dtype=torch.int64, device=dev)
+    d_vis = torch.from_numpy(vis0.view(np.int32).copy()).to(dev)
+    d_fr = torch.from_numpy(fr0.view(np.int32).copy()).to(dev)
+    n_out = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    total = sum(len(x) for x in lists)
+    ws = torch.empty(B.workspace_bytes(max(total, 1), len(blobs), W), dtype=torch.uint8, device=dev)
+    B.decompress_batch_to_frontier(d_in, d_off, len(blobs), W, id_base, d_fr, d_vis if with_visited else None, n_bits, n_out,
+                                   ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == expect
+    if expect:
+        return
+    vis, fr = vis0.copy(), fr0.copy()
+    for b in blobs:
+        if with_visited:
+            oracle_mod.decompress_to_frontier(b, W, fr, vis, n_bits, id_base)
+        else:
+            oracle_mod.decompress_to_bitmap(b, W, fr, n_bits, id_base)
+    assert int(n_out.item()) == total
+    assert np.array_equal(d_fr.cpu().numpy().view(np.uint32), fr), "frontier bitmap differs from the oracle"
+    assert np.array_equal(d_vis.cpu().numpy().view(np.uint32), vis), "visited bitmap differs from the oracle"
+
+
+@pytest.mark.parametrize("W", [32, 64])
+def test_decompress_batch_to_frontier(B, oracle_mod, W):
+    """Algorithm 4 lines 10-13 over all received streams in one call: the union of the streams' IDs, filtered by the
+    visited set, whatever their order; streams that overlap (a vertex found by several ranks), empty and RAW streams,
+    the one-launch path (small levels) and the planned one, ID base offsets, IDs outside the bitmap."""
+    dt = np.uint32 if W == 32 else np.uint64
+    rng = np.random.default_rng(100 + W)
+
+    def draw(n_bits, n, id_base):
+        v = np.sort(rng.choice(n_bits, size=min(n, n_bits), replace=False)).astype(np.uint64)
+        return ((v + np.uint64(id_base)) & np.uint64(0xFFFFFFFFFFFFFFFF if W == 64 else 0xFFFFFFFF)).astype(dt)
+
+    # a small level: 8 streams over 2^16 vertices (one launch), overlapping, one empty, one below the RAW threshold
+    nb, base = 1 << 16, 1000
+    small = [draw(nb, n, base) for n in (3000, 0, 17, 5000, 128, 129, 1, 2500)]
+    _batch_frontier_case(B, oracle_mod, small, W, nb, base, 128, 64, seed=1)
+    _batch_frontier_case(B, oracle_mod, small, W, nb, base, 128, 0, seed=2, with_visited=False)
+    # a large level: 16 streams over 2^22 vertices (plan + tiles), heavy overlap
+    nb = 1 << 22
+    big = [draw(nb, n, 0) for n in (200000, 150000, 0, 1, 300000, 70000, 128 * 64, 90000, 5, 250000, 100000, 60000, 31, 0, 120000, 80000)]
+    _batch_frontier_case(B, oracle_mod, big, W, nb, 0, 1024, 256, seed=3)
+    # one stream carries an ID beyond the bitmap
+    bad = [x.copy() for x in small]
+    bad[3][-1] = base + (1 << 16) + 5
+    _batch_frontier_case(B, oracle_mod, bad, W, 1 << 16, base, 0, 64, seed=4, expect=B.ERR_DST_TOO_SMALL)
+    # a corrupt slot (no stream header) is rejected
+    dev = torch.device("cuda")
+    junk = torch.full((4096,), 0xCD, dtype=torch.uint8, device=dev)
+    off = torch.tensor([0, 2048, 4096], dtype=torch.int64, device=dev)
+    fr = torch.zeros(64, dtype=torch.int32, device=dev)
+    vis = torch.zeros(64, dtype=torch.int32, device=dev)
+    n_out = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    ws = torch.empty(B.workspace_bytes(1000, 2, W), dtype=torch.uint8, device=dev)
+    B.decompress_batch_to_frontier(junk, off, 2, W, 0, fr, vis, 2048, n_out, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_CORRUPT and int(n_out.item()) == 0
+    assert not bool(fr.any()) and not bool(vis.any())
+
+
 # ---- the one-launch cluster kernel of small batches (k_enc_small: <= 1024 buffers, <= 2048 blocks by the workspace size) ----
 @pytest.mark.parametrize("W", [32, 64])
 def test_small_batch_cluster_kernel_boundaries(B, oracle_mod, W):
