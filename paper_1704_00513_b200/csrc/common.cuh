@@ -138,20 +138,36 @@ __device__ __forceinline__ uint32_t exc_bytes(uint32_t n) {
 // Decoding into a frontier bitmap (FORMAT.md §9): bit (x - id_base) of bm for every decoded ID x. bm == nullptr: IDs go to
 // the ID array as usual.
 struct BitSink { uint32_t* bm; unsigned long long id_base, n_bits; uint32_t* status; uint32_t* visited; };
-// The bits `mask` of word w: plain OR into the bitmap, or (bfsc_decompress_to_frontier, Algorithm 4 lines 11-13) OR into
-// the visited bitmap first — what was not visited before goes into the frontier bitmap.
-__device__ __forceinline__ void sink_or(const BitSink& s, uint32_t w, uint32_t mask) {
-    BFSC_CHECK((unsigned long long)w < (s.n_bits + 31) / 32);
+// Up to four (word, mask) pairs into the sink: plain ORs into the bitmap, or (bfsc_decompress_to_frontier, Algorithm 4
+// lines 11-13) ORs into the visited bitmap first — what was not visited before goes into the frontier bitmap. The
+// atomic's return value says which of the bits were visited before (exactly once per vertex, whoever else updates the
+// same word); it costs a round trip to L2, so the (up to four) visited updates of a call go out TOGETHER and their
+// results are looked at afterwards (sparse levels: 28 -> 26 us per call on 8 x 4096 IDs over 2^16-2^20 vertices; what
+// remains is the rate at which one warp's scattered atomics are accepted, 32 addresses per instruction: with the same
+// IDs packed 4 to a word the call takes 11 us). Measured alternative to the returning atomic: a plain load
+// of the visited word + a non-returning atomic — no faster (the atomics of the same SM keep invalidating the L1 lines
+// the loads would hit: 59.6 against 54.1 us on the 2^25-bit frontier of bench.py).
+template <int N>
+__device__ __forceinline__ void sink_or_n(const BitSink& s, const uint32_t (&w)[N], const uint32_t (&mk)[N]) {
     if (s.visited != nullptr) {
-        // The atomic's return value says which of the bits were visited before (exactly once per vertex, whoever else
-        // updates the same word). It costs the warp a round trip to L2 per word. Measured alternative: a plain load of
-        // the visited word + a non-returning atomic — no faster (the atomics of the same SM keep invalidating the L1
-        // lines the loads would hit: 59.6 against 54.1 us on the 2^25-bit frontier of bench.py).
-        const uint32_t old = atomicOr(s.visited + w, mask);
-        mask &= ~old;
-        if (mask == 0u) return;
+        uint32_t old[N];
+#pragma unroll
+        for (int c = 0; c < N; c++) {
+            BFSC_CHECK(mk[c] == 0u || (unsigned long long)w[c] < (s.n_bits + 31) / 32);
+            old[c] = mk[c] ? atomicOr(s.visited + w[c], mk[c]) : 0xffffffffu;
+        }
+#pragma unroll
+        for (int c = 0; c < N; c++) {
+            const uint32_t fresh = mk[c] & ~old[c];
+            if (fresh) atomicOr(s.bm + w[c], fresh);
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < N; c++) {
+            BFSC_CHECK(mk[c] == 0u || (unsigned long long)w[c] < (s.n_bits + 31) / 32);
+            if (mk[c]) atomicOr(s.bm + w[c], mk[c]);
+        }
     }
-    atomicOr(s.bm + w, mask);
 }
 // Four consecutive decoded IDs (the first nvalid of them count). Neighbours that fall into the same 32-bit word go
 // out as ONE atomic OR (sorted dense frontiers: usually all four). An ID outside the bitmap: DST_TOO_SMALL, not set.
@@ -168,8 +184,8 @@ __device__ __forceinline__ void set_bits4(const BitSink& s, T v0, T v1, T v2, T 
                 const uint32_t b1 = 1u << ((uint32_t)r1 & 31u), b2 = 1u << ((uint32_t)r2 & 31u), b3 = 1u << ((uint32_t)r3 & 31u);
                 const uint32_t lo = (1u << (q0 & 31u)) | (d1 ? 0u : b1) | (d2 ? 0u : b2) | (d3 ? 0u : b3);
                 const uint32_t hi = (d1 ? b1 : 0u) | (d2 ? b2 : 0u) | (d3 ? b3 : 0u);
-                sink_or(s, w0, lo);
-                if (hi) sink_or(s, w0 + 1, hi);
+                const uint32_t w2[2] = {w0, w0 + 1u}, m2[2] = {lo, hi};
+                sink_or_n<2>(s, w2, m2);
                 return;
             }
         }
@@ -186,9 +202,7 @@ __device__ __forceinline__ void set_bits4(const BitSink& s, T v0, T v1, T v2, T 
 #pragma unroll
     for (int c = 1; c < 4; c++)
         if (w[c] == w[c - 1]) { mk[c] |= mk[c - 1]; mk[c - 1] = 0u; }
-#pragma unroll
-    for (int c = 0; c < 4; c++)
-        if (mk[c]) sink_or(s, w[c], mk[c]);
+    sink_or_n<4>(s, w, mk);
 }
 
 // Buffer of global block g: the last i with a[i] <= g (buffers without blocks are skipped), searched from a
