@@ -3,6 +3,7 @@
 // Launches per call: single stream: k_dec_tiles alone (it parses the stream header itself);
 // batch: [k_dec_headers ->] k_dec_plan -> k_dec_blocks -> k_dec_tiles, chained with programmatic dependent launch.
 #include <cstdlib>
+#include <atomic>
 #include <mutex>
 
 #include "block_decode.cuh"
@@ -22,6 +23,8 @@ struct DecArgs {
     uint32_t* status;
     BitSink sink;                       // bfsc_decompress_to_bitmap: where the IDs' bits go (ids == nullptr then)
     WsView ws;                          // blk_first, fixed_prefix (= id offsets)
+    unsigned long long plan_tag;        // k_dec_planchain: this call's tag (never 0 in its low 48 bits, unique per call in the process)
+    uint32_t plan_grid;                 //   its CTAs (0: another plan ran): k_dec_tiles clears their states behind it
 };
 
 __device__ __forceinline__ unsigned long long s_begin(const DecArgs& a, uint32_t i) {
@@ -322,6 +325,174 @@ __global__ void __launch_bounds__(1024) k_dec_planblocks(DecArgs a) {
     }
 }
 
+// ---- D0 for batches of MANY streams (kChainMinStreams .. kFusedMaxStreams): a single-pass CHAINED plan. The fused plan
+// above lets every CTA parse every header (no inter-CTA dependency, right for a handful of streams); with thousands of
+// streams that redundancy is the call's cost (4096 streams: 13.5 of 38.9 us). Here the streams are dealt out: a CTA takes
+// a ticket, parses the headers of slice `ticket` (<= 256 streams, one per thread), scans them, publishes the slice's
+// sums (blocks, IDs, rejected headers) and gets its prefix from the sums of the lower tickets — held by CTAs that
+// arrived earlier, so a CTA only ever waits for CTAs that are running or done (no residency assumption). Then it writes
+// the per-stream tables, d_id_offsets and the block-table entries of ITS OWN streams (a warp per stream, no search;
+// streams of more than kChainBigBlocks blocks by the whole CTA). The CTA with the last ticket knows the totals and
+// writes the verdict. States live in ws.tile_state (4 words per ticket: tag, blocks, IDs, rejected), the ticket counter
+// in ws.hdr; both are valid only with this call's TAG (host-side counter, unique per call), so whatever the workspace
+// held before reads as "not yet published"; k_dec_tiles clears them behind the plan so that a replay of a captured
+// call — same tag again — starts clean.
+constexpr uint32_t kChainMinStreams = 3072;                // measured, us per decompress call, chained / every-CTA-for-itself: 512 streams 18.0 / 13.3, 1024 19.9 / 16.4, 2048 24.7 / 23.2, 4096 35.9 / 38.9 (4096 short streams 23.6 / 26.7), 8192 34.6 / 48.6 — the chain pays seven dependent round trips (ticket, offsets, headers, publish, poll, payload, tables) where the other pays three
+constexpr int kChainThreads = 256;
+constexpr uint32_t kChainBigBlocks = 1024;
+__device__ __forceinline__ unsigned long long dec_ld_volatile(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void dec_st_volatile(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+template <int W>
+__global__ void __launch_bounds__(kChainThreads) k_dec_planchain(DecArgs a) {
+    constexpr unsigned long long E = W / 8;
+    __shared__ Scan2 sm[33];
+    __shared__ unsigned int s_ticket, s_nbig;
+    __shared__ Scan2 s_base;
+    __shared__ unsigned long long s_badbefore;
+    __shared__ unsigned long long s_inoff[kChainThreads], s_id0[kChainThreads];
+    __shared__ uint32_t s_nb[kChainThreads], s_tot16[kChainThreads], s_big[kChainThreads];
+    __shared__ unsigned long long s_blk0[kChainThreads];
+    pdl_wait();                                          // the call before this one is complete (workspace, inputs)
+    pdl_launch_dependents();
+    const unsigned long long tag48 = a.plan_tag & 0xffffffffffffull;
+    if (threadIdx.x == 0) {
+        // ticket word: (tag << 16 | tickets drawn); anything else = nobody has drawn yet. Whoever finds it without the
+        // tag tries ONCE to install (tag << 16 | 0): if that fails somebody else has, and from then on the word only
+        // moves through tagged values. Then one atomic add per CTA (a compare-and-swap loop of 148 contenders on one
+        // word takes 148 rounds: 80 us).
+        unsigned long long* tt = &a.ws.hdr->pad[0];
+        const unsigned long long seen = dec_ld_volatile(tt);
+        if ((seen >> 16) != tag48) atomicCAS(tt, seen, tag48 << 16);
+        s_ticket = (unsigned int)(atomicAdd(tt, 1ull) & 0xffffull);
+        s_nbig = 0;
+    }
+    __syncthreads();
+    const uint32_t ticket = s_ticket, grid = gridDim.x;
+    const uint32_t per = (a.n_buf + grid - 1) / grid;    // <= kChainThreads (the launch sees to it)
+    const uint32_t lo = min(ticket * per, a.n_buf), hi = min(lo + per, a.n_buf);
+    const uint32_t i = lo + threadIdx.x;
+    // this thread's stream: header parsed and validated (FORMAT.md §4), as in dec_plan_scan
+    Scan2 v{0, 0};
+    unsigned long long beg = 0, tot_bytes = 0, bad = 0;
+    if (i < hi) {
+        beg = a.in_off[i];
+        const unsigned long long end = a.in_off[i + 1];
+        const unsigned long long avail = end >= beg ? end - beg : 0;
+        bool ok = !(beg & 15) && avail >= 32;
+        if (ok) {
+            const uint4 h0 = __ldcg(reinterpret_cast<const uint4*>(a.in + beg));
+            const uint4 h1 = __ldcg(reinterpret_cast<const uint4*>(a.in + beg + 16));
+            const uint32_t mode = (h0.y >> 16) & 0xffu;
+            const unsigned long long n = (unsigned long long)h0.w << 32 | h0.z;
+            const unsigned long long total = (unsigned long long)h1.y << 32 | h1.x;
+            const unsigned long long nb = h1.z;
+            if (h0.x != 0x43534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != (uint32_t)W || mode > 2u || (h0.y >> 24) != 0u)
+                ok = false;
+            else if (total > avail || (total & 15) || total < 32) ok = false;
+            else if (mode == 0) { if (nb != 0 || n > (total - 32) / E) ok = false; }
+            else if (nb != (n + kBlk - 1) / kBlk || 32ull + ((4ull * (nb + 1) + 15ull) & ~15ull) > total) ok = false;
+            if (ok) { v.a = nb; v.b = n; tot_bytes = total; }
+        }
+        if (!ok) bad = 1;
+    }
+    const unsigned long long n_bad = __syncthreads_count(bad != 0);
+    Scan2 tot;
+    const Scan2 ex = block_scan_excl2(v, &tot, sm);
+    unsigned long long* states = a.ws.tile_state;
+    if (threadIdx.x == 0) {                              // publish: payload, fence, tag
+        unsigned long long* st = states + 4ull * ticket;
+        dec_st_volatile(st + 1, tot.a); dec_st_volatile(st + 2, tot.b); dec_st_volatile(st + 3, n_bad);
+        __threadfence();
+        dec_st_volatile(st, a.plan_tag);
+    }
+    if (threadIdx.x < 32) {
+        // prefix over the lower tickets: first every tag this lane needs (independent polls), ONE fence, then the
+        // payloads (independent loads) — a fence and two dependent round trips per state cost 8 us at 148 tickets
+        constexpr int kMaxPer = 32;                      // states per lane: tickets < 1024
+        Scan2 acc{0, 0};
+        unsigned long long badb = 0;
+        for (uint32_t j0 = threadIdx.x; j0 < ticket; j0 += 32 * kMaxPer) {
+            uint32_t pending = 0;
+#pragma unroll 1
+            for (int u = 0; u < kMaxPer; u++)
+                if (j0 + 32u * u < ticket) pending |= 1u << u;
+            while (pending) {
+                uint32_t still = 0;
+                for (int u = 0; u < kMaxPer; u++)
+                    if ((pending >> u & 1u) && dec_ld_volatile(states + 4ull * (j0 + 32u * u)) != a.plan_tag) still |= 1u << u;
+                pending = still;
+                if (pending) __nanosleep(64);
+            }
+        }
+        __threadfence();
+        for (uint32_t j = threadIdx.x; j < ticket; j += 32) {
+            const unsigned long long* st = states + 4ull * j;
+            acc.a += dec_ld_volatile(st + 1); acc.b += dec_ld_volatile(st + 2); badb += dec_ld_volatile(st + 3);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc.a += __shfl_xor_sync(kFull, acc.a, o); acc.b += __shfl_xor_sync(kFull, acc.b, o); badb += __shfl_xor_sync(kFull, badb, o);
+        }
+        if (threadIdx.x == 0) { s_base = acc; s_badbefore = badb; }
+    }
+    __syncthreads();
+    const Scan2 base = s_base;
+    if (ticket == grid - 1 && threadIdx.x == 0) {        // the last ticket: totals and the verdict
+        const unsigned long long blocks = base.a + tot.a, ids = base.b + tot.b;
+        const bool any_bad = s_badbefore + n_bad != 0;
+        const bool good = !any_bad && blocks <= a.ws.blk_cap && ids <= a.ids_cap && blocks < (1ull << 32);
+        a.ws.blk_first[a.n_buf] = blocks;
+        a.ws.fixed_prefix[a.n_buf] = ids;
+        a.ws.hdr->total_blocks = blocks;
+        a.ws.hdr->total_out = ids;
+        a.ws.hdr->ok = good ? 1u : 0u;
+        if (any_bad) set_status(a.status, BFSC_ERR_CORRUPT);
+        else if (ids > a.ids_cap) set_status(a.status, BFSC_ERR_DST_TOO_SMALL);
+        else if (!good) set_status(a.status, BFSC_ERR_INVALID_ARG);
+        if (a.n_ids_out) *a.n_ids_out = good ? ids : 0ull;
+        if (a.id_off) a.id_off[a.n_buf] = ids;           // (a rejected call: k_dec_tiles zeroes all of them)
+    }
+    // own streams: tables, d_id_offsets; block table by a warp per stream
+    const unsigned long long blk0 = base.a + ex.a, id0 = base.b + ex.b;
+    s_blk0[threadIdx.x] = blk0; s_id0[threadIdx.x] = id0; s_inoff[threadIdx.x] = beg;
+    s_nb[threadIdx.x] = (uint32_t)min(v.a, 0xffffffffull); s_tot16[threadIdx.x] = (uint32_t)(tot_bytes >> 4);
+    if (i < hi) {
+        a.ws.blk_first[i] = blk0; a.ws.fixed_prefix[i] = id0; a.ws.stream_start[i] = tot_bytes;
+        if (a.id_off) a.id_off[i] = id0;
+        if (v.a > kChainBigBlocks) s_big[atomicAdd(&s_nbig, 1u)] = threadIdx.x;
+    }
+    __syncthreads();
+    auto entry = [&](uint32_t t, unsigned long long k) {
+        const unsigned long long g = s_blk0[t] + k;
+        if (g >= a.ws.blk_cap) return;                   // (the call is rejected by the last ticket; nothing out of bounds)
+        const unsigned long long nb = s_nb[t];
+        // IDs of the stream: nb blocks, the last one ragged — from the header's n, kept as id0 of the next stream - id0
+        const unsigned long long n = (t + 1 < hi - lo ? s_id0[t + 1] : base.b + tot.b) - s_id0[t];
+        const unsigned long long sb = s_inoff[t], xi = s_id0[t] + kBlk * k;
+        uint4 e0, e1;
+        e0.x = (uint32_t)sb; e0.y = (uint32_t)(sb >> 32); e0.z = (uint32_t)xi; e0.w = (uint32_t)(xi >> 32);
+        e1.x = (uint32_t)k; e1.y = (uint32_t)min((unsigned long long)kBlk, n - kBlk * k);
+        e1.z = s_tot16[t]; e1.w = (uint32_t)nb;
+        a.ws.blk_tab[2 * g] = e0; a.ws.blk_tab[2 * g + 1] = e1;
+    };
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (uint32_t t = warp; t < hi - lo; t += kChainThreads / 32) {
+        const uint32_t nb = s_nb[t];
+        if (nb > kChainBigBlocks) continue;
+        for (uint32_t k = lane; k < nb; k += 32) entry(t, k);
+    }
+    for (uint32_t b = 0; b < s_nbig; b++) {              // long streams: the whole CTA
+        const uint32_t t = s_big[b];
+        for (unsigned long long k = threadIdx.x; k < s_nb[t]; k += kChainThreads) entry(t, k);
+    }
+}
+
 // ---- D1-D5 fused -------------------------------------------------------------------------
 // Warp = batch of 8 consecutive blocks, four lanes per block (quad_decode.cuh). Per batch:
 //   locate   per quad: stream, directory entries -> block address, span, valid IDs, output address
@@ -409,7 +580,16 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         if (!good) return;
         total_blocks = tot.a;
     } else if (batch) {
-        if (!a.ws.hdr->ok) return;
+        if (a.plan_grid != 0 && blockIdx.x == 0) {                         // k_dec_planchain's states and ticket: cleared behind it
+            for (uint32_t x = threadIdx.x; x < 4u * a.plan_grid; x += blockDim.x) a.ws.tile_state[x] = 0ull;
+            if (threadIdx.x == 0) a.ws.hdr->pad[0] = 0ull;
+        }
+        if (!a.ws.hdr->ok) {
+            if (a.plan_grid != 0 && a.id_off)                              // (the chained plan wrote them before the verdict was known)
+                for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i <= a.n_buf; i += (unsigned long long)gridDim.x * blockDim.x)
+                    a.id_off[i] = 0ull;
+            return;
+        }
         total_blocks = a.ws.hdr->total_blocks;
     } else {                                                               // D0 for one stream (FORMAT.md §1, §4)
         const bool first = blockIdx.x == 0 && threadIdx.x == 0;
@@ -674,8 +854,17 @@ static bool dec_planblocks_init(int device) {            // once per device: the
     return true;
 }
 
+static unsigned long long next_plan_tag() {              // unique per call in the process, low 48 bits never 0
+    static std::atomic<unsigned long long> counter{0x5bf5c0de0001ull};
+    unsigned long long t;
+    do { t = counter.fetch_add(1ull) + 1ull; } while ((t & 0xffffffffffffull) == 0);
+    return t;
+}
+
 template <int W>
-static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream_t s) {
+static bfsc_status launch_decode(const DecArgs& a_in, size_t max_blocks, cudaStream_t s) {
+    DecArgs a = a_in;
+    a.plan_tag = 0; a.plan_grid = 0;
     constexpr size_t kSmem = DecSmem<W>::kBytes;
     DeviceInfo dev;
     if (!current_device(&dev)) return BFSC_ERR_CUDA;
@@ -708,10 +897,20 @@ static bfsc_status launch_decode(const DecArgs& a, size_t max_blocks, cudaStream
     } else if (a.in_off && a.n_buf <= kFusedMaxStreams && a.ws.blk_cap < (1ull << 32)) {
         if (!dec_planblocks_init<W>(dev.device)) return BFSC_ERR_CUDA;
         if (bits && dec_ctas_per_sm<W, true, false, true>(dev.device) < 1) return BFSC_ERR_CUDA;
-        size_t pgrid = (a.ws.blk_cap + 1023) / 1024;
-        if (pgrid > (size_t)dev.sms) pgrid = (size_t)dev.sms;
-        if (pgrid > (size_t)kFusedPlanCtas) pgrid = kFusedPlanCtas;
-        BFSC_LAUNCH(launch_dep(k_dec_planblocks<W>, pgrid ? (int)pgrid : 1, 1024, dec_planblocks_smem(a.n_buf), s, a));
+        // many streams: the chained plan (streams dealt out over the CTAs, 4 state words per CTA in ws.tile_state);
+        // few: the plan every CTA runs for itself
+        size_t cgrid = (size_t)dev.sms;
+        if (cgrid > 2 * a.ws.tile_cap) cgrid = 2 * a.ws.tile_cap;
+        if (cgrid > 0xffffu) cgrid = 0xffffu;
+        if (a.n_buf >= kChainMinStreams && cgrid >= 1 && (a.n_buf + cgrid - 1) / cgrid <= (size_t)kChainThreads) {
+            a.plan_tag = next_plan_tag(); a.plan_grid = (uint32_t)cgrid;
+            BFSC_LAUNCH(launch_dep(k_dec_planchain<W>, (int)cgrid, kChainThreads, 0, s, a));
+        } else {
+            size_t pgrid = (a.ws.blk_cap + 1023) / 1024;
+            if (pgrid > (size_t)dev.sms) pgrid = (size_t)dev.sms;
+            if (pgrid > (size_t)kFusedPlanCtas) pgrid = kFusedPlanCtas;
+            BFSC_LAUNCH(launch_dep(k_dec_planblocks<W>, pgrid ? (int)pgrid : 1, 1024, dec_planblocks_smem(a.n_buf), s, a));
+        }
         if (bits) BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false, true>, grid, DecCfg<W>::kThreads, kSmem, s, a));
         else BFSC_LAUNCH(launch_dep(k_dec_tiles<W, true, false>, grid, DecCfg<W>::kThreads, kSmem, s, a));
     } else if (a.in_off && bits) {

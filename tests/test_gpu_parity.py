@@ -332,6 +332,90 @@ def test_batch_of_many_streams_rejects_corrupt_headers(B):
     assert int(status.item()) == B.ERR_CORRUPT
 
 
+@pytest.mark.parametrize("W", [32, 64])
+def test_chained_decode_plan(B, oracle_mod, W):
+    """Batches of >= 3072 streams are planned by k_dec_planchain (streams dealt out over the CTAs, prefixes from the
+    lower tickets' published sums). Covered here: a batch with empty, RAW and one long stream (over 1024 blocks: written
+    by the whole CTA); the same call replayed from a CUDA graph (same tag every replay: the tile kernel clears the states
+    behind the plan) with a different, shorter batch decoded through the same workspace in between; rejected headers
+    (status, nothing decoded, all ID offsets zero); the ID capacity exceeded; decode into frontier bitmaps."""
+    dev = torch.device("cuda")
+    g = torch.Generator().manual_seed(17 + W)
+    counts = torch.randint(0, 400, (3500,), generator=g)
+    counts[5] = 0
+    counts[1777] = 150000                                   # 1172 blocks
+    counts[3499] = 129
+    ids, off = streams.batch_of_streams(counts, 16.0, seed=13, W=W)
+    n, n_buf = ids.numel(), counts.numel()
+    ref, ref_off = oracle_mod.compress_batch(_np(ids, W), off.numpy().astype(np.uint64), 256)
+    d_in = torch.from_numpy(np.concatenate([ref, np.zeros(16, np.uint8)])).to(dev)
+    d_off = torch.from_numpy(ref_off.astype(np.int64)).to(dev)
+    ws = torch.empty(B.workspace_bytes(n, n_buf, W), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    back = torch.full((n + 4,), -1, dtype=ids.dtype, device=dev)
+    id_off = torch.zeros(n_buf + 1, dtype=torch.int64, device=dev)
+    B.decompress_batch(d_in, d_off, n_buf, W, back, id_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and torch.equal(back[:n].cpu(), ids) and torch.equal(id_off.cpu(), off)
+    assert bool((back[n:] == -1).all())
+    # a second, shorter batch of many streams (its own tag, the same workspace), also the one captured below
+    counts2 = torch.randint(1, 200, (3100,), generator=g)
+    ids2, off2 = streams.batch_of_streams(counts2, 4.0, seed=14, W=W)
+    ref2, ref2_off = oracle_mod.compress_batch(_np(ids2, W), off2.numpy().astype(np.uint64), 0)
+    d_in2 = torch.from_numpy(np.concatenate([ref2, np.zeros(16, np.uint8)])).to(dev)
+    d_off2 = torch.from_numpy(ref2_off.astype(np.int64)).to(dev)
+    back2 = torch.full((ids2.numel() + 4,), -1, dtype=ids.dtype, device=dev)
+    id_off2 = torch.zeros(counts2.numel() + 1, dtype=torch.int64, device=dev)
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        B.decompress_batch(d_in2, d_off2, counts2.numel(), W, back2, id_off2, ws, status)      # (warm-up outside the capture)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            B.decompress_batch(d_in2, d_off2, counts2.numel(), W, back2, id_off2, ws, status)
+    for rep in range(4):
+        back2.fill_(-1); id_off2.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0 and torch.equal(back2[:ids2.numel()].cpu(), ids2) and torch.equal(id_off2.cpu(), off2), rep
+        if rep == 1:                                        # another call through the same workspace between two replays
+            back.fill_(-1)
+            B.decompress_batch(d_in, d_off, n_buf, W, back, id_off, ws, status)
+            torch.cuda.synchronize()
+            assert int(status.item()) == 0 and torch.equal(back[:n].cpu(), ids)
+    # rejected headers in the first, a middle and the last slice; a stream off its 16-byte boundary
+    for which, (rel, val) in ((0, (0, 0x41)), (1777, (5, 64 if W == 32 else 32)), (3499, (4, 9)), (2000, (17, 0xFF))):
+        bad = d_in.clone()
+        bad[int(ref_off[which]) + rel] = val
+        status.zero_(); back.fill_(-1); id_off.fill_(7)
+        B.decompress_batch(bad, d_off, n_buf, W, back, id_off, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == B.ERR_CORRUPT, which
+        assert bool((back == -1).all()) and not bool(id_off.any()), which
+    status.zero_(); back.fill_(-1)
+    small = torch.full((n - 1,), -1, dtype=ids.dtype, device=dev)              # one ID short
+    B.decompress_batch(d_in, d_off, n_buf, W, small, id_off, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == B.ERR_DST_TOO_SMALL and bool((small == -1).all()) and not bool(id_off.any())
+    # the same streams into frontier bitmaps (the bitmap sink behind the same plan)
+    lo = int(_np(ids, W).min())
+    n_bits = int(_np(ids, W).max()) - lo + 1
+    if n_bits <= (1 << 27):
+        words = (n_bits + 127) // 128 * 4
+        d_fr = torch.zeros(words, dtype=torch.int32, device=dev)
+        d_vis = torch.zeros(words, dtype=torch.int32, device=dev)
+        n_dec = torch.zeros(1, dtype=torch.int64, device=dev)
+        status.zero_()
+        B.decompress_batch_to_frontier(d_in, d_off, n_buf, W, lo, d_fr, d_vis, n_bits, n_dec, ws, status)
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0 and int(n_dec.item()) == n
+        exp = np.zeros(words * 32, dtype=bool)
+        exp[(_np(ids, W).astype(np.uint64) - np.uint64(lo)).astype(np.int64)] = True
+        exp_words = np.packbits(exp.reshape(-1, 32), axis=1, bitorder="little").view(np.uint32).reshape(-1)
+        assert np.array_equal(d_fr.cpu().numpy().view(np.uint32), exp_words)
+        assert np.array_equal(d_vis.cpu().numpy().view(np.uint32), exp_words)
+
+
 def test_host_api_roundtrip(B, oracle_mod):
     dev = torch.device("cuda")
     for W in (32, 64):
