@@ -512,7 +512,7 @@ template <int W, bool kTma = false> struct DecCfg {
 
 template <int W, bool kTma = false> struct DecSmem {
     using T = typename IdT<W>::T;
-    static constexpr size_t kStageBytes = (size_t)DecCfg<W, kTma>::kStages * kDecStageChunks * 16;   // per warp
+    static constexpr size_t kStageBytes = (size_t)DecCfg<W, kTma>::kStages * DecStage<W, kTma>::kStageChunks * 16;   // per warp
     static constexpr size_t kTabBytes = (size_t)kDecBlocks * kBlk * sizeof(T);         // per warp
     static constexpr size_t kBytes = DecCfg<W, kTma>::kWarps * (kStageBytes + kTabBytes);
 };
@@ -548,6 +548,7 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
     T* tab_w = reinterpret_cast<T*>(dec_smem + kDecWarps * DecSmem<W, kTma>::kStageBytes + warp * DecSmem<W, kTma>::kTabBytes);
     for (int x = lane; x < kDecBlocks * kBlk; x += 32) tab_w[x] = 0;       // patch table: all zero between uses
     __syncwarp();
+    constexpr int kDecSpanMax = DecStage<W, kTma>::kSpanMax, kDecSlotChunks = DecStage<W, kTma>::kSlotChunks, kDecStageChunks = DecStage<W, kTma>::kStageChunks;
     uint4* slot = stage + kDecSlotChunks * q;
     T* tab = tab_w + kBlk * q;
     __shared__ unsigned long long s_mbar[kTma ? 2 * kDecWarps : 1];       // kTma: "the span in stage s of warp w has landed"
@@ -745,7 +746,7 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
             const bool big = cur.blk != nullptr && cur.span16 > (uint32_t)kDecSpanMax;
             const bool any_big = __any_sync(kFull, big);
             BFSC_CHECK(any_big || cur.blk == nullptr || cur.span16 <= (uint32_t)kDecSpanMax);
-            if (!any_big && cur.blk != nullptr) quad_stage_block(slot, cur.blk, cur.span16, l);
+            if (!any_big && cur.blk != nullptr) quad_stage_block<kDecSpanMax>(slot, cur.blk, cur.span16, l);
             const BlockAt<W> nxt = locate((bi + n_warps) * kDecBlocks + q);   // the next batch's directory reads overlap the copy
             if (!any_big) {
                 dec_cp_async_wait_all();

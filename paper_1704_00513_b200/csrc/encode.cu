@@ -274,6 +274,7 @@ __global__ void __launch_bounds__(1024) k_enc_planblocks(EncArgs a) {
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPre = 2ull << 62, kValMask = (1ull << 62) - 1;
 constexpr unsigned long long kNoTile = ~0ull, kSkip = ~0ull;
 constexpr uint32_t kLateBit = 1u << 31;                  // in a stored key: the block is assembled by late_emit, not in an image buffer
+constexpr uint32_t kDoneBit = 1u << 30;                  // in a stored key: the block is in the output already (packed straight from the registers)
 
 __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
     unsigned long long v;
@@ -797,8 +798,15 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             bar_arrive(kBarSizes + kp, kSizesThreads);
 
             const uint32_t b = 64u - ((key >> 7) & 127u), n_exc = key & 127u;
-            const bool late = !kBits && key != 0 && (wide || (key >> 14) > (uint32_t)Img::kCap);   // slow path, in global memory later
-            const bool fast = !wide && key != 0 && !late;
+            // u64 ID arrays: a block whose deltas fit 32 bits but whose image does not fit its slot (b > 17: gaps over 2^17)
+            // is packed from the registers STRAIGHT to its place in the output — this tile's offsets are awaited first
+            // (the scan warp needs only the sizes, posted above), which costs this warp its one tile of slack, not a
+            // re-read of the IDs with 64-bit arithmetic (late_emit: 2^24 IDs with gaps of 2^20 took 187 us, the same
+            // IDs with gaps of 16 take 49).
+            bool direct = false;
+            if constexpr (W == 64 && !kBits) direct = !wide && key != 0 && (key >> 14) > (uint32_t)Img::kCap;
+            const bool late = !kBits && key != 0 && !direct && (wide || (key >> 14) > (uint32_t)Img::kCap);   // slow path, in global memory later
+            const bool fast = !wide && key != 0 && !late && !direct;
             // The warp's 8 images lie back to back in the buffer, as they do in the output (consecutive blocks):
             // woff = exclusive scan of the fast blocks' sizes over the quads, in 16-byte chunks.
             {
@@ -811,8 +819,19 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             }
             unsigned char* img = ib + 16 * woff;
             BFSC_CHECK(!fast || 16u * woff + (key >> 14) <= (uint32_t)(Img::kBufChunks * 16));
-            if (!wide && __any_sync(kFull, fast && n_exc > 0))           // E4 into the image buffer: exceptions
-                col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, fast ? n_exc : 0u);
+            bool emit = fast;                                            // this quad packs now (into the image buffer, or directly)
+            if constexpr (W == 64 && !kBits) {
+                if (__any_sync(kFull, direct)) {
+                    mbar_wait(&mb_off[kp], (k / kNB) & 1);               // this tile's offsets are resolved
+                    if (direct) {
+                        const unsigned long long at = s_at[kp][j];
+                        emit = at != kSkip;                              // (kSkip: over the output capacity, status is set)
+                        img = a.out + at;
+                    }
+                }
+            }
+            if (!wide && __any_sync(kFull, emit && n_exc > 0))           // E4 into the image buffer: exceptions
+                col_exceptions_raw<W>(d, raw, img + 16 + 16 * b, b, emit ? n_exc : 0u);
             __syncwarp();                                                // the warp's staged IDs are consumed
             mbar_wait(&mb_post[(k + 1) & (kRing - 1)], ((k + 1) / kRing) & 1);   // tile k+1 is posted
             have_next = s_tile[(k + 1) & (kRing - 1)] != kNoTile;
@@ -821,7 +840,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             } else {
                 if (have_next) quad_prefetch<W>(slot, ids + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));   // same slots
             }
-            if (fast) {                                                  // payload + header
+            if (emit) {                                                  // payload + header
                 if (b > 0) col_pack32(d, b, reinterpret_cast<uint32_t*>(img) + 4 + l);
                 if (l == 0) {                                            // block header (FORMAT.md §2)
                     reinterpret_cast<unsigned long long*>(img)[0] = (unsigned long long)base;
@@ -829,6 +848,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                 }
             }
             if (late) key |= kLateBit;
+            if (direct) key |= kDoneBit;                                 // nothing of it waits in shared memory (and the warp's images are not one piece)
             __syncwarp();                                                // image complete
             n_wait++;
         }
@@ -850,7 +870,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             // images -> their final place. Usual case: the warp's blocks are consecutive in the output as well
             // (same stream, none late, all fit): ONE bulk store of the whole buffer by lane 0.
             const unsigned char* ib_e = ibuf + kpe * (Img::kBufChunks * 16);
-            const bool valid = key_e != 0, fast_e = valid && (key_e & kLateBit) == 0;
+            const bool valid = key_e != 0, fast_e = valid && (key_e & (kLateBit | kDoneBit)) == 0;
             const uint32_t z_e = fast_e ? key_e >> 18 : 0u;
             const unsigned long long at_n = __shfl_down_sync(kFull, at, 4);
             const bool valid_n = __shfl_down_sync(kFull, (int)valid, 4) != 0 && q < kQuadBlocks - 1;

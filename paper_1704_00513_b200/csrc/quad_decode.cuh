@@ -4,7 +4,7 @@
 // 64 (u32) / 128 (u64) contiguous bytes, so loads and stores are coalesced 128-bit accesses, and the
 // per-block scalar work (header, directory, validation) costs 1/8 of a warp instruction per block.
 //
-// Fast path only: blocks of at most kDecSpanMax 16-byte chunks (b <= 20 without exceptions),
+// Fast path only: blocks of at most DecStage<W>::kSpanMax 16-byte chunks (u32: b <= 20 without exceptions; u64: b <= 32),
 // staged in shared memory by cp.async. Larger blocks take the warp-per-block path of block_decode.cuh.
 #pragma once
 #include "common.cuh"
@@ -12,9 +12,15 @@
 namespace bfsc {
 
 constexpr int kDecBlocks = 8;                 // blocks per warp batch
-constexpr int kDecSpanMax = 21;               // largest staged block, in 16-byte chunks (336 B: b = 20)
-constexpr int kDecSlotChunks = 22;            // slot stride: one chunk of slack for the unpack's second read
-constexpr int kDecStageChunks = kDecBlocks * kDecSlotChunks;
+// Staging geometry. u32 (and the TMA variant): blocks of up to 21 chunks (336 B: b = 20) are staged, 16 warps x 2 CTAs fill
+// the SM's shared memory. u64 (8 warps x 2 CTAs: room to spare): up to 33 chunks (528 B: b = 32 without exceptions; NOT
+// more: a staged block is unpacked with 32-bit funnel shifts, and b = 33 starts at 34 chunks) — gaps over 2^20 between
+// sorted 64-bit IDs stay on the fast path (2^24 IDs: 77 -> 40 us).
+template <int W, bool kTma = false> struct DecStage {
+    static constexpr int kSpanMax = (W == 64 && !kTma) ? 33 : 21;   // largest staged block, in 16-byte chunks
+    static constexpr int kSlotChunks = kSpanMax + 1;               // slot stride: one chunk of slack for the unpack's second read
+    static constexpr int kStageChunks = kDecBlocks * kSlotChunks;
+};
 
 __device__ __forceinline__ void dec_cp_async16(void* smem_dst, const void* gmem_src) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
@@ -43,12 +49,13 @@ __device__ __forceinline__ void dec_mbar_wait(unsigned long long* b, uint32_t pa
     } while (!ok);
 }
 
-// D1: stage the quad's block (span16 <= kDecSpanMax chunks at blk) into its slot; lane l copies chunks l, l+4, ...
+// D1: stage the quad's block (span16 <= kSpanMax chunks at blk) into its slot; lane l copies chunks l, l+4, ...
+template <int kSpanMax>
 __device__ __forceinline__ void quad_stage_block(uint4* __restrict__ slot, const unsigned char* __restrict__ blk,
                                                  uint32_t span16, int l) {
     const uint4* src = reinterpret_cast<const uint4*>(blk);
 #pragma unroll
-    for (int i = 0; i < (kDecSpanMax + 3) / 4; i++) {
+    for (int i = 0; i < (kSpanMax + 3) / 4; i++) {
         const uint32_t c = 4 * i + l;
         if (c < span16) dec_cp_async16(slot + c, src + c);
     }
@@ -96,7 +103,7 @@ __device__ __forceinline__ void quad_decode_rows(const uint4* __restrict__ P, ui
                                                  typename IdT<W>::T base, typename IdT<W>::T* __restrict__ x, int m, int l,
                                                  const BitSink& sink = BitSink{nullptr, 0, 0, nullptr, nullptr}) {
     using T = typename IdT<W>::T;
-    const uint32_t mask = (1u << b) - 1u;
+    const uint32_t mask = b >= 32u ? 0xffffffffu : (1u << b) - 1u;       // (b <= 32 here: larger blocks are not staged)
     uint32_t bit = (uint32_t)l * b;
     T carry = base;
     const bool vec_ok = (m == kBlk) && ((reinterpret_cast<uintptr_t>(x) & 15) == 0);
