@@ -827,6 +827,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
                         const unsigned long long at = s_at[kp][j];
                         emit = at != kSkip;                              // (kSkip: over the output capacity, status is set)
                         img = a.out + at;
+                        BFSC_CHECK(!emit || at + (key >> 14) <= a.out_cap);
                     }
                 }
             }
