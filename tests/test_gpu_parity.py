@@ -416,6 +416,38 @@ def test_chained_decode_plan(B, oracle_mod, W):
         assert np.array_equal(d_vis.cpu().numpy().view(np.uint32), exp_words)
 
 
+def test_u64_wide_gap_blocks(B, oracle_mod):
+    """u64 blocks whose deltas fit 32 bits but whose image does not fit the encoder's 288-byte slot (17 < b <= 32: gaps of
+    2^17 .. 2^32 between sorted 64-bit IDs) are packed straight to the output once the tile's offsets are known, and the
+    decoder stages them up to b = 32. Single stream over many tiles (k_enc_tiles<64, 0>, tickets), a batch on the general
+    path (k_enc_tiles<64, 1>) with narrow and wide buffers side by side, exceptions on top (b + outliers), and the b = 32 /
+    b = 33 boundary of the decoder's staging; bytes against the oracle."""
+    rng = np.random.default_rng(64)
+    n = 128 * 64 * 700 + 77                                  # 700 tiles: every CTA draws tickets
+    for bits in (18, 21, 27, 32):
+        g = rng.integers(1 << (bits - 1), 1 << bits, size=n, dtype=np.uint64)
+        ids = np.cumsum(g).astype(np.uint64)
+        t = torch.from_numpy(ids.view(np.int64).copy())
+        run_single(B, oracle_mod, t, 64, 0)
+    # outliers that still fit 32 bits on top of 20-bit gaps: exceptions inside directly emitted blocks
+    g = rng.integers(1 << 19, 1 << 20, size=n, dtype=np.uint64)
+    idx = rng.integers(0, n, size=n // 100)
+    g[idx] = rng.integers(1 << 30, 1 << 32, size=idx.size, dtype=np.uint64)
+    run_single(B, oracle_mod, torch.from_numpy(np.cumsum(g).astype(np.uint64).view(np.int64).copy()), 64, 0)
+    # a batch on the general path: narrow, wide (b = 22), b = 32, b = 33 (wide deltas: the slow path) and ragged buffers
+    parts, counts = [], []
+    for k, (cnt, bits) in enumerate(((128 * 300 + 5, 4), (128 * 200 + 1, 22), (999, 22), (128 * 150, 32), (128 * 90 + 64, 33), (128 * 400, 19), (3, 25), (128 * 100 + 127, 8))):
+        gg = rng.integers(1 << (bits - 1), 1 << bits, size=cnt, dtype=np.uint64)
+        parts.append(np.cumsum(gg).astype(np.uint64) + np.uint64(k) * np.uint64(1 << 50))
+        counts.append(cnt)
+    ids = np.concatenate(parts)
+    off = torch.zeros(len(counts) + 1, dtype=torch.int64)
+    off[1:] = torch.cumsum(torch.tensor(counts), 0)
+    t = torch.from_numpy(ids.view(np.int64).copy())
+    for thr in (0, 1024):
+        run_batch(B, oracle_mod, t, off, 64, thr)
+
+
 def test_host_api_roundtrip(B, oracle_mod):
     dev = torch.device("cuda")
     for W in (32, 64):
