@@ -84,6 +84,12 @@ def lib():
         L.bfsc_ref_decompress_to_bitmap.argtypes = [vp, sz, i32, c.c_uint64, vp, sz, c.POINTER(sz)]
         L.bfsc_ref_decompress_to_frontier.restype = i32
         L.bfsc_ref_decompress_to_frontier.argtypes = [vp, sz, i32, c.c_uint64, vp, vp, sz, c.POINTER(sz)]
+        L.bfsc_ref_vbitmap_bound.restype = sz
+        L.bfsc_ref_vbitmap_bound.argtypes = [sz]
+        L.bfsc_ref_compress_vbitmap.restype = i32
+        L.bfsc_ref_compress_vbitmap.argtypes = [i32, vp, sz, vp, sz, c.POINTER(sz)]
+        L.bfsc_ref_decompress_vbitmap.restype = i32
+        L.bfsc_ref_decompress_vbitmap.argtypes = [vp, sz, vp, sz]
         _lib = L
     return _lib
 
@@ -259,3 +265,30 @@ def decompress_to_frontier(stream: np.ndarray, W: int, frontier: np.ndarray, vis
     if rc:
         raise OracleError(rc)
     return n.value
+
+
+def vbitmap_bound(n_bits: int) -> int:
+    return int(lib().bfsc_ref_vbitmap_bound(n_bits))
+
+
+def compress_vbitmap(bitmap: np.ndarray, n_bits: int, codec: int = CODEC_PFOR) -> np.ndarray:
+    """FORMAT.md §10: bitmap (uint32 words) -> container bytes."""
+    bitmap = np.ascontiguousarray(bitmap, dtype=np.uint32)
+    cap = vbitmap_bound(n_bits)
+    out = np.empty(cap, dtype=np.uint8)
+    nb = ctypes.c_size_t(0)
+    rc = lib().bfsc_ref_compress_vbitmap(codec, _p(bitmap), n_bits, _p(out), cap, ctypes.byref(nb))
+    if rc:
+        raise OracleError(rc)
+    return out[:nb.value].copy()
+
+
+def decompress_vbitmap(container: np.ndarray, n_bits: int) -> np.ndarray:
+    """-> the bitmap as uint32 words (ceil(n_bits / 32) of them)."""
+    container = np.ascontiguousarray(container, dtype=np.uint8)
+    bm = np.zeros(max((n_bits + 31) // 32, 1), dtype=np.uint32)
+    rc = lib().bfsc_ref_decompress_vbitmap(_p(container), len(container), _p(bm), n_bits)
+    if rc:
+        raise OracleError(rc)
+    return bm[:(n_bits + 31) // 32]
+

@@ -353,6 +353,84 @@ int bfsc_ref_decompress_to_bitmap(const uint8_t *in, size_t in_bytes, int W, uin
     return rc;
 }
 
+/* FORMAT.md §10: a (visited) bitmap as a container that lists its MINORITY bits — the set bits if there are at most as
+ * many of them as clear ones, else the clear bits — as one stream of §1 (u32 bit indices, threshold 0), or holds the
+ * bitmap itself (kind 0) when the stream would not be smaller. PAPER.md L2065, L2104-2113, L2166: the zone the thesis
+ * left uncompressed; the thesis gives no algorithm (reading 12). cap >= bfsc_ref_vbitmap_bound(n_bits). */
+size_t bfsc_ref_vbitmap_bound(size_t n_bits) {
+    size_t words = (n_bits + 31) / 32;
+    return 32 + (4 * words + 15) / 16 * 16;
+}
+
+int bfsc_ref_compress_vbitmap(int codec, const uint32_t *bitmap, size_t n_bits, uint8_t *out, size_t cap, size_t *out_bytes) {
+    if (!out || !out_bytes || (n_bits && !bitmap) || n_bits > ((size_t)1 << 32)) return BFSC_REF_ERR_INVALID_ARG;
+    size_t words = (n_bits + 31) / 32, raw = (4 * words + 15) / 16 * 16;
+    if (cap < 32 + raw) return BFSC_REF_ERR_DST_TOO_SMALL;
+    size_t k = 0;
+    for (size_t v = 0; v < n_bits; v++) k += (bitmap[v / 32] >> (v % 32)) & 1u;
+    int list_set = k <= n_bits - k;                                  /* the minority; a tie lists the set bits */
+    size_t n = list_set ? k : n_bits - k, j = 0;
+    uint32_t *ids = malloc((n ? n : 1) * sizeof(uint32_t));
+    size_t scap = bfsc_ref_compress_bound(n, 32);
+    uint8_t *stream = malloc(scap);
+    if (!ids || !stream) { free(ids); free(stream); return BFSC_REF_ERR_INVALID_ARG; }
+    for (size_t v = 0; v < n_bits; v++)
+        if ((int)((bitmap[v / 32] >> (v % 32)) & 1u) == list_set) ids[j++] = (uint32_t)v;
+    size_t sb = 0;
+    int rc = bfsc_ref_compress_codec(codec, ids, n, 32, 0, stream, scap, &sb);
+    free(ids);
+    if (rc) { free(stream); return rc; }
+    int kind = sb < raw ? (list_set ? 1 : 2) : 0;                    /* not smaller than the bitmap itself: kind 0 */
+    size_t payload = kind ? sb : raw;
+    memset(out, 0, 32 + payload);
+    out[0] = 'B'; out[1] = 'F'; out[2] = 'S'; out[3] = 'V';
+    out[4] = 1; out[5] = 32; out[6] = (uint8_t)kind; out[7] = 0;
+    st_le(out + 8, n_bits, 8);
+    st_le(out + 16, 32 + payload, 8);
+    st_le(out + 24, kind ? n : 0, 8);
+    if (kind) memcpy(out + 32, stream, sb);
+    else
+        for (size_t v = 0; v < n_bits; v++)                          /* bits >= n_bits stay 0 */
+            if ((bitmap[v / 32] >> (v % 32)) & 1u) out[32 + v / 8] |= (uint8_t)(1u << (v % 8));
+    free(stream);
+    *out_bytes = 32 + payload;
+    return BFSC_REF_OK;
+}
+
+/* The bitmap is overwritten (every word up to ceil(n_bits / 32); bits >= n_bits are 0). Nothing is changed on an error. */
+int bfsc_ref_decompress_vbitmap(const uint8_t *in, size_t in_bytes, uint32_t *bitmap, size_t n_bits) {
+    if (!in || (n_bits && !bitmap)) return BFSC_REF_ERR_INVALID_ARG;
+    if (in_bytes < 32) return BFSC_REF_ERR_CORRUPT;
+    if (in[0] != 'B' || in[1] != 'F' || in[2] != 'S' || in[3] != 'V') return BFSC_REF_ERR_CORRUPT;
+    if (in[4] != 1 || in[5] != 32 || in[6] > 2 || in[7] != 0) return BFSC_REF_ERR_CORRUPT;
+    uint64_t nbits = ld_le(in + 8, 8), total = ld_le(in + 16, 8), n_listed = ld_le(in + 24, 8);
+    int kind = in[6];
+    if (total > in_bytes || total % 16 || total < 32) return BFSC_REF_ERR_CORRUPT;
+    if (nbits != n_bits) return BFSC_REF_ERR_DST_TOO_SMALL;
+    size_t words = (n_bits + 31) / 32, raw = (4 * words + 15) / 16 * 16;
+    uint32_t *res = calloc(words ? words : 1, sizeof(uint32_t));
+    if (!res) return BFSC_REF_ERR_INVALID_ARG;
+    int rc = BFSC_REF_OK;
+    if (kind == 0) {
+        if (total != 32 + raw || n_listed != 0) rc = BFSC_REF_ERR_CORRUPT;
+        for (size_t v = 0; !rc && v < 8 * raw; v++) {
+            unsigned bit = (in[32 + v / 8] >> (v % 8)) & 1u;
+            if (v >= n_bits) { if (bit) rc = BFSC_REF_ERR_CORRUPT; }     /* the pad is zero */
+            else if (bit) res[v / 32] |= 1u << (v % 32);
+        }
+    } else {
+        size_t got = 0;
+        rc = bfsc_ref_decompress_to_bitmap(in + 32, (size_t)total - 32, 32, 0, res, n_bits, &got);
+        if (rc == BFSC_REF_ERR_DST_TOO_SMALL) rc = BFSC_REF_ERR_CORRUPT;   /* an ID >= n_bits inside the container */
+        if (!rc && got != n_listed) rc = BFSC_REF_ERR_CORRUPT;
+        if (!rc && kind == 2)
+            for (size_t v = 0; v < n_bits; v++) res[v / 32] ^= 1u << (v % 32);
+    }
+    if (!rc) memcpy(bitmap, res, words * sizeof(uint32_t));
+    free(res);
+    return rc;
+}
+
 /* Algorithm 4, lines 10-13, with the frontier t and the visited set of Pi as bitmaps:
  *   line 10  t <- decompress(t'')          the decoded IDs
  *   line 11  t <- t (.) not Pi             keep those not visited yet

@@ -111,6 +111,12 @@ int bfsc_ref_compress_bitmap(int codec, const uint32_t *bitmap, size_t n_bits, u
                              size_t raw_threshold_bytes, uint8_t *out, size_t out_capacity, size_t *out_bytes);
 int bfsc_ref_decompress_to_bitmap(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,
                                   uint32_t *bitmap, size_t n_bits, size_t *n_ids);
+/* FORMAT.md §10: a bitmap as a container that lists its minority bits (set or
+ * clear) as one u32 stream, or holds the bitmap itself when that is not smaller. cap >= bfsc_ref_vbitmap_bound(n_bits). */
+size_t bfsc_ref_vbitmap_bound(size_t n_bits);
+int bfsc_ref_compress_vbitmap(int codec, const uint32_t *bitmap, size_t n_bits, uint8_t *out, size_t out_capacity,
+                              size_t *out_bytes);
+int bfsc_ref_decompress_vbitmap(const uint8_t *in, size_t in_bytes, uint32_t *bitmap, size_t n_bits);
 /* Algorithm 4 lines 10-13 on bitmaps: for the decoded IDs S,
  * frontier |= S \ visited and visited |= S (FORMAT.md §9, last item). Nothing is changed on an error. */
 int bfsc_ref_decompress_to_frontier(const uint8_t *in, size_t in_bytes, int W, uint64_t id_base,

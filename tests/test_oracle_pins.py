@@ -391,3 +391,90 @@ def test_frontier_update_hand_example_and_set_algebra(oracle_mod):
                     oracle_mod.decompress_to_frontier(s, W, fr, vis, int(ids[-1]) - id_base, id_base=id_base)
                 assert ei.value.code == oracle_mod.ERR_DST_TOO_SMALL
                 assert np.array_equal(fr, fr0) and np.array_equal(vis, vis0)
+
+
+def _pack_bits(bits):
+    n = len(bits)
+    words = (n + 31) // 32
+    pad = np.zeros(words * 32, dtype=bool)
+    pad[:n] = bits
+    return np.packbits(pad.reshape(-1, 32), axis=1, bitorder="little").view(np.uint32).reshape(-1) if words else np.zeros(0, np.uint32)
+
+
+def test_vbitmap_container(oracle_mod):
+    """FORMAT.md §10: header typed by hand, the inner stream read back by the second
+    witness, the minority / tie / not-smaller rules from closed forms, complement symmetry, identity round trip, rejects."""
+    o = oracle_mod
+    # a hand example: 1000 bits, set {3, 500, 999}: the three set bits are listed (kind 1)
+    bits = np.zeros(1000, dtype=bool)
+    bits[[3, 500, 999]] = True
+    c = o.compress_vbitmap(_pack_bits(bits), 1000)
+    inner = o.compress(np.array([3, 500, 999], dtype=np.uint32), 0)
+    header = b"BFSV" + bytes([1, 32, 1, 0]) + (1000).to_bytes(8, "little") + (32 + len(inner)).to_bytes(8, "little") + (3).to_bytes(8, "little")
+    assert c.tobytes() == header + inner.tobytes()
+    assert witness.decode_stream(c[32:].tobytes(), 32) == [3, 500, 999]
+    # the complement: the same three positions are now the CLEAR bits: kind 2, same stream
+    c2 = o.compress_vbitmap(_pack_bits(~bits), 1000)
+    assert c2[6] == 2 and c2[32:].tobytes() == inner.tobytes() and c2[:6].tobytes() == c[:6].tobytes() and c2[8:].tobytes() == c[8:].tobytes()
+    assert np.array_equal(o.decompress_vbitmap(c2, 1000), _pack_bits(~bits))
+    # closed forms: an empty stream is 48 bytes (32-byte header + the 16-byte directory of zero blocks)
+    for n_bits in (4097, 1 << 16):
+        z = o.compress_vbitmap(_pack_bits(np.zeros(n_bits, bool)), n_bits)
+        f = o.compress_vbitmap(_pack_bits(np.ones(n_bits, bool)), n_bits)
+        assert (z[6], len(z), f[6], len(f)) == (1, 80, 2, 80)
+        assert int.from_bytes(z[24:32].tobytes(), "little") == 0
+    # half of the bits set, even as one run (gaps of 1: b = 1, 32 bytes per 128 IDs = 2 bits per ID = 1 bit per vertex,
+    # plus the directory): never smaller than the bitmap -> kind 0; the minority side decides from there on
+    tie = np.zeros(1 << 14, dtype=bool)
+    tie[:1 << 13] = True
+    assert o.compress_vbitmap(_pack_bits(tie), 1 << 14)[6] == 0
+    few = np.zeros(1 << 14, dtype=bool)
+    few[:1 << 10] = True                                          # 1024 of 16384 set: listed; all but 1024 set: the clear ones
+    assert o.compress_vbitmap(_pack_bits(few), 1 << 14)[6] == 1 and o.compress_vbitmap(_pack_bits(~few), 1 << 14)[6] == 2
+    # not smaller than the bitmap itself -> kind 0, payload = the bitmap's bytes, bits >= n_bits written as 0
+    rng = np.random.default_rng(3)
+    half = rng.random(5000) < 0.5
+    bm = _pack_bits(half)
+    dirty = bm.copy()
+    dirty[-1] |= np.uint32(0xFFFFFFFF) << np.uint32(5000 % 32)    # garbage beyond n_bits in the caller's last word
+    k0 = o.compress_vbitmap(dirty, 5000)
+    raw = (4 * len(bm) + 15) // 16 * 16
+    assert k0[6] == 0 and len(k0) == 32 + raw == o.vbitmap_bound(5000)
+    assert k0[32:32 + 4 * len(bm)].tobytes() == bm.tobytes() and not k0[32 + 4 * len(bm):].any()
+    assert k0.tobytes() == o.compress_vbitmap(bm, 5000).tobytes()
+    # tiny bitmaps: the 48-byte empty stream is never smaller than <= 48 bytes of bitmap
+    for n_bits in (0, 1, 31, 32, 33, 384):
+        t = o.compress_vbitmap(_pack_bits(np.zeros(n_bits, bool)), n_bits)
+        assert t[6] == 0 and len(t) == o.vbitmap_bound(n_bits)
+    assert o.compress_vbitmap(_pack_bits(np.zeros(385, bool)), 385)[6] == 1     # 64 bytes of bitmap: the empty stream wins
+    # identity and the size bound over densities, both rules
+    for n_bits in (1, 127, 128, 4096, 70001):
+        for dens in (0.0, 0.001, 0.05, 0.3, 0.5, 0.7, 0.95, 0.999, 1.0):
+            b = rng.random(n_bits) < dens
+            for codec in (o.CODEC_PFOR, o.CODEC_BP128):
+                cc = o.compress_vbitmap(_pack_bits(b), n_bits, codec)
+                assert len(cc) <= o.vbitmap_bound(n_bits) and len(cc) % 16 == 0
+                assert int.from_bytes(cc[16:24].tobytes(), "little") == len(cc)
+                assert np.array_equal(o.decompress_vbitmap(cc, n_bits), _pack_bits(b))
+                k = int(b.sum())
+                if cc[6]:
+                    assert cc[6] == (1 if k <= n_bits - k else 2) and int.from_bytes(cc[24:32].tobytes(), "little") == min(k, n_bits - k)
+    # rejects
+    def rc_of(buf, n_bits):
+        try:
+            o.decompress_vbitmap(buf, n_bits)
+            return 0
+        except o.OracleError as e:
+            return e.code
+    assert rc_of(c, 1000) == 0
+    for pos, val in ((0, ord("X")), (4, 2), (5, 64), (6, 3), (7, 1), (24, 4)):      # magic, version, width, kind, byte 7, n_listed
+        bad = c.copy()
+        bad[pos] = val
+        assert rc_of(bad, 1000) == 3, pos
+    assert rc_of(c, 1001) == 2 and rc_of(c[:-16], 1000) == 3
+    bad = k0.copy()
+    bad[32 + 5000 // 8] |= 1 << 7                                  # a pad bit of a kind-0 payload
+    assert rc_of(bad, 5000) == 3
+    far = o.compress_vbitmap(_pack_bits(bits), 1000).copy()        # claim fewer bits than the listed IDs need
+    far[8:16] = np.frombuffer((600).to_bytes(8, "little"), dtype=np.uint8)
+    assert rc_of(far, 600) == 3
