@@ -245,6 +245,26 @@ bfsc_status bfsc_decompress_batch_to_frontier(const void* d_in, const uint64_t* 
                                               uint64_t* d_n_ids, void* d_workspace, size_t workspace_bytes,
                                               uint32_t* d_status, void* cuda_stream);
 
+/* Visited bitmaps (FORMAT.md §10; the predecessor / visited zone the
+ * thesis left uncompressed, L2166: compressing the visited bitmap as future work). A bitmap of n_bits <= 2^32 bits (32-bit
+ * words, bit v = bit v % 32 of word v / 32; bits >= n_bits of the last word are ignored) becomes a container that lists
+ * its MINORITY bits — the set bits, or the clear bits of a mostly-visited bitmap — as one u32 stream of FORMAT.md §1, or
+ * holds the bitmap itself when that would not be smaller: never more than bfsc_vbitmap_bound(n_bits) = 32 + the bitmap's
+ * bytes rounded up to 16. Both calls: d_bitmap 4-byte aligned, d_out / d_in / d_workspace 16-byte aligned, workspace of
+ * bfsc_vbitmap_workspace_bytes(n_bits) bytes (it holds a copy of the bitmap), stream-ordered, nothing allocated.
+ * bfsc_compress_vbitmap: out_capacity >= bfsc_vbitmap_bound(n_bits) (else BFSC_ERR_DST_TOO_SMALL is returned);
+ *   *d_out_bytes (device, written) = the container's total_bytes. codec = the rule of the stream inside.
+ * bfsc_decompress_vbitmap: OVERWRITES d_bitmap[0 .. ceil(n_bits / 32)) (bits >= n_bits written as 0). n_bits must be the
+ *   container's (else BFSC_ERR_DST_TOO_SMALL in *d_status); a malformed container or stream inside: BFSC_ERR_CORRUPT in
+ *   *d_status; on either error d_bitmap is left as it was. */
+size_t bfsc_vbitmap_bound(size_t n_bits);
+size_t bfsc_vbitmap_workspace_bytes(size_t n_bits);
+bfsc_status bfsc_compress_vbitmap(bfsc_codec codec, const uint32_t* d_bitmap, size_t n_bits, void* d_out, size_t out_capacity,
+                                  uint64_t* d_out_bytes, void* d_workspace, size_t workspace_bytes, uint32_t* d_status,
+                                  void* cuda_stream);
+bfsc_status bfsc_decompress_vbitmap(const void* d_in, size_t in_bytes, uint32_t* d_bitmap, size_t n_bits,
+                                    void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream);
+
 /* End-to-end convenience calls with HOST buffers (pinned memory recommended): copy in,
  * run the device call above, copy the result out, synchronise the stream. d_scratch is a
  * caller-owned device buffer of at least bfsc_host_scratch_bytes(n_ids, t) bytes.

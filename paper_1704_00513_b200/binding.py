@@ -29,6 +29,7 @@ EXPORTS = [
     "bfsc_compress_codec", "bfsc_compress_batch_codec", "bfsc_compress_batch_scatter",
     "bfsc_bitmap_workspace_bytes", "bfsc_compress_bitmap", "bfsc_decompress_to_bitmap", "bfsc_compress_noalloc",
     "bfsc_decompress_to_frontier", "bfsc_decompress_batch_to_frontier",
+    "bfsc_vbitmap_bound", "bfsc_vbitmap_workspace_bytes", "bfsc_compress_vbitmap", "bfsc_decompress_vbitmap",
     "bfsc_host_scratch_bytes", "bfsc_compress_host", "bfsc_decompress_host", "bfsc_kernel_launches",
 ]
 
@@ -67,6 +68,14 @@ def lib():
         L.bfsc_decompress_to_frontier.argtypes = [vp, sz, i32, c.c_uint64, vp, vp, sz, vp, vp, sz, vp, vp]
         L.bfsc_decompress_batch_to_frontier.restype = i32
         L.bfsc_decompress_batch_to_frontier.argtypes = [vp, vp, sz, i32, c.c_uint64, vp, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_vbitmap_bound.restype = sz
+        L.bfsc_vbitmap_bound.argtypes = [sz]
+        L.bfsc_vbitmap_workspace_bytes.restype = sz
+        L.bfsc_vbitmap_workspace_bytes.argtypes = [sz]
+        L.bfsc_compress_vbitmap.restype = i32
+        L.bfsc_compress_vbitmap.argtypes = [i32, vp, sz, vp, sz, vp, vp, sz, vp, vp]
+        L.bfsc_decompress_vbitmap.restype = i32
+        L.bfsc_decompress_vbitmap.argtypes = [vp, sz, vp, sz, vp, sz, vp, vp]
         L.bfsc_host_scratch_bytes.restype = sz
         L.bfsc_host_scratch_bytes.argtypes = [sz, i32]
         L.bfsc_compress.restype = i32
@@ -198,6 +207,26 @@ def decompress_batch_to_frontier(d_in, d_in_offsets, n_buf, W, id_base, d_fronti
                                                    _ptr(d_visited), n_bits, _ptr(d_n_ids), _ptr(d_workspace),
                                                    d_workspace.numel(), _ptr(d_status), ctypes.c_void_p(_stream())),
            "bfsc_decompress_batch_to_frontier")
+
+
+def vbitmap_bound(n_bits: int) -> int:
+    return int(lib().bfsc_vbitmap_bound(n_bits))
+
+
+def vbitmap_workspace_bytes(n_bits: int) -> int:
+    return int(lib().bfsc_vbitmap_workspace_bytes(n_bits))
+
+
+def compress_vbitmap(codec, d_bitmap, n_bits, d_out, d_out_bytes, d_workspace, d_status):
+    _check(lib().bfsc_compress_vbitmap(codec, _ptr(d_bitmap), n_bits, _ptr(d_out), d_out.numel(), _ptr(d_out_bytes),
+                                       _ptr(d_workspace), d_workspace.numel(), _ptr(d_status),
+                                       ctypes.c_void_p(_stream())), "bfsc_compress_vbitmap")
+
+
+def decompress_vbitmap(d_in, in_bytes, d_bitmap, n_bits, d_workspace, d_status):
+    _check(lib().bfsc_decompress_vbitmap(_ptr(d_in), in_bytes, _ptr(d_bitmap), n_bits, _ptr(d_workspace),
+                                         d_workspace.numel(), _ptr(d_status), ctypes.c_void_p(_stream())),
+           "bfsc_decompress_vbitmap")
 
 
 def decompress(d_in, in_bytes, W, d_ids, d_n_ids, d_workspace, d_status):

@@ -36,6 +36,45 @@ __device__ __forceinline__ void bm_expand(T* __restrict__ raw, const uint32_t* _
     const uint32_t w_first = s >> 5, w_last = (e - 1u) >> 5;
     const uint32_t qmask = 0xfu << (4 * q);
     uint32_t rank = 0;
+    if (!landed) {
+        // A sparse batch (more than kLand chunks: under one ID in 32 bits on average): its words come from global memory,
+        // SIXTEEN per quad and trip (one 128-bit load per lane), and a trip without a set bit costs a vote, not a scan —
+        // one word per lane and trip made a block of a 0.2 % dense bitmap (2000 words) five hundred dependent trips long.
+        for (uint32_t w = w_first & ~3u; w <= w_last && w >= (w_first & ~3u); w += 16) {
+            const uint32_t w4 = w + 4u * (uint32_t)l;
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (w4 <= w_last && w4 >= w) v = *reinterpret_cast<const uint4*>(bitmap + w4);
+            uint32_t xs[4] = {v.x, v.y, v.z, v.w};
+            uint32_t c = 0;
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const uint32_t wi = w4 + (uint32_t)t;
+                if (wi < w_first || wi > w_last || wi < w) xs[t] = 0u;
+                if (wi == w_first) xs[t] &= 0xffffffffu << (s & 31u);
+                if (wi == w_last && (e & 31u)) xs[t] &= (1u << (e & 31u)) - 1u;
+                c += (uint32_t)__popc(xs[t]);
+            }
+            if (!__any_sync(qmask, c != 0u)) continue;
+            uint32_t inc = c, y;
+            y = __shfl_up_sync(qmask, inc, 1, 4); if (l >= 1) inc += y;
+            y = __shfl_up_sync(qmask, inc, 2, 4); if (l >= 2) inc += y;
+            T* out = raw + (rank + inc);                             // behind this lane's last ID: filled from the top down
+            rank += __shfl_sync(qmask, inc, 3, 4);
+#pragma unroll
+            for (int t = 3; t >= 0; t--) {
+                uint32_t x = xs[t];
+                const T id0 = (T)(id_base + 32ull * (w4 + (uint32_t)t));
+                while (x) {
+                    uint32_t b;
+                    asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(x));
+                    BFSC_CHECK(out - 1 >= raw && out - 1 < raw + kBlk);
+                    *--out = id0 + (T)b;
+                    x &= ~(1u << (b & 31u));
+                }
+            }
+        }
+        return;
+    }
     for (uint32_t w = w_first; w <= w_last && w >= w_first; w += 4) {
         const uint32_t wi = w + (uint32_t)l;
         uint32_t x = (wi <= w_last && wi >= w) ? words[wi] : 0u;

@@ -23,6 +23,7 @@ struct DecArgs {
     uint32_t* status;
     BitSink sink;                       // bfsc_decompress_to_bitmap: where the IDs' bits go (ids == nullptr then)
     WsView ws;                          // blk_first, fixed_prefix (= id offsets)
+    const unsigned int* skip;           // single-stream calls, or nullptr: *skip != 0 (device) = nothing to decode, return at once (FORMAT.md §10: kind 0)
     unsigned long long plan_tag;        // k_dec_planchain: this call's tag (never 0 in its low 48 bits, unique per call in the process)
     uint32_t plan_grid;                 //   its CTAs (0: another plan ran): k_dec_tiles clears their states behind it
 };
@@ -593,6 +594,7 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         }
         total_blocks = a.ws.hdr->total_blocks;
     } else {                                                               // D0 for one stream (FORMAT.md §1, §4)
+        if (a.skip != nullptr && *a.skip != 0u) return;
         const bool first = blockIdx.x == 0 && threadIdx.x == 0;
         bool ok = a.in_single >= 32;
         uint32_t mode = 0;
@@ -944,7 +946,7 @@ static bfsc_status launch_decode(const DecArgs& a_in, size_t max_blocks, cudaStr
 static bfsc_status decode_common(const void* d_in, const uint64_t* d_in_off, size_t in_single, size_t n_buf,
                                  bfsc_dtype t, void* d_ids, size_t ids_cap, uint64_t* d_id_off, uint64_t* d_n_ids,
                                  void* ws, size_t ws_bytes, uint32_t* d_status, void* stream,
-                                 BitSink sink = BitSink{nullptr, 0, 0, nullptr, nullptr}) {
+                                 BitSink sink = BitSink{nullptr, 0, 0, nullptr, nullptr}, const unsigned int* skip = nullptr) {
     if (t != BFSC_U32 && t != BFSC_U64) return BFSC_ERR_INVALID_ARG;
     if (!d_in || !ws || n_buf > 0x7fffffffu) return BFSC_ERR_INVALID_ARG;
     if (!d_ids && ids_cap && !sink.bm) return BFSC_ERR_INVALID_ARG;
@@ -953,7 +955,7 @@ static bfsc_status decode_common(const void* d_in, const uint64_t* d_in_off, siz
     if (!ws_carve(ws, ws_bytes, n_buf, &a.ws)) return BFSC_ERR_INVALID_ARG;
     a.in = (const unsigned char*)d_in; a.in_off = (const unsigned long long*)d_in_off; a.in_single = in_single;
     a.n_buf = (uint32_t)n_buf; a.ids = d_ids; a.ids_cap = ids_cap; a.id_off = (unsigned long long*)d_id_off;
-    a.n_ids_out = (unsigned long long*)d_n_ids; a.status = d_status; a.sink = sink;
+    a.n_ids_out = (unsigned long long*)d_n_ids; a.status = d_status; a.sink = sink; a.skip = skip;
     size_t max_blocks = (sink.bm ? (size_t)sink.n_bits : ids_cap) / kBlk + n_buf + 1;
     if (sink.bm && d_in_off) max_blocks = ~(size_t)0 >> 8;       // (streams of a batch may repeat IDs: bounded by the workspace only)
     return t == BFSC_U32 ? launch_decode<32>(a, max_blocks, (cudaStream_t)stream)
@@ -1016,4 +1018,98 @@ extern "C" bfsc_status bfsc_decompress_batch_to_frontier(const void* d_in, const
         return BFSC_ERR_INVALID_ARG;
     return bfsc::decode_common(d_in, d_in_offsets, 0, n_buf, t, nullptr, ~(size_t)0, nullptr, d_n_ids, d_workspace,
                                workspace_bytes, d_status, cuda_stream, bfsc::BitSink{d_frontier, id_base, n_bits, d_status, d_visited});
+}
+
+// ---- FORMAT.md §10: the (visited) bitmap container. begin (parse the header; kind 0: the payload is the bitmap; else the
+// scratch bitmap is cleared) -> the decode kernel into the scratch bitmap (skipped for kind 0 / a rejected container) ->
+// end (the scratch bitmap, or its complement, becomes the caller's; a rejected container leaves the caller's bitmap as
+// it was).
+namespace bfsc {
+struct VbScratch { unsigned long long count, stream_bytes, n_decoded, n_listed; unsigned int status, kind, skip, pad; };
+__global__ void __launch_bounds__(256) k_vb_begin(const unsigned char* __restrict__ in, unsigned long long in_bytes, unsigned long long n_bits,
+                                                  uint32_t* __restrict__ wb, uint32_t* __restrict__ bitmap, VbScratch* sc, uint32_t* status) {
+    const unsigned long long words = (n_bits + 31) / 32, raw_bytes = (4 * words + 15) & ~15ull;
+    uint32_t err = 0, kind = 0;
+    unsigned long long total = 0, n_listed = 0;
+    if (in_bytes < 32) err = BFSC_ERR_CORRUPT;
+    else {
+        const uint4 h0 = *reinterpret_cast<const uint4*>(in), h1 = *reinterpret_cast<const uint4*>(in + 16);
+        kind = (h0.y >> 16) & 0xffu;
+        const unsigned long long nb = (unsigned long long)h0.w << 32 | h0.z;
+        total = (unsigned long long)h1.y << 32 | h1.x;
+        n_listed = (unsigned long long)h1.w << 32 | h1.z;
+        if (h0.x != 0x56534642u || (h0.y & 0xffu) != 1u || ((h0.y >> 8) & 0xffu) != 32u || kind > 2u || (h0.y >> 24) != 0u) err = BFSC_ERR_CORRUPT;
+        else if (total > in_bytes || (total & 15) || total < 32) err = BFSC_ERR_CORRUPT;
+        else if (nb != n_bits) err = BFSC_ERR_DST_TOO_SMALL;
+        else if (kind == 0u) {
+            if (total != 32 + raw_bytes || n_listed != 0) err = BFSC_ERR_CORRUPT;
+            else                                                         // the pad behind bit n_bits - 1 is zero
+                for (unsigned long long w = n_bits / 32; w < raw_bytes / 4; w++) {
+                    uint32_t x = reinterpret_cast<const uint32_t*>(in + 32)[w];
+                    if (w == n_bits / 32 && (n_bits & 31)) x &= ~((1u << (uint32_t)(n_bits & 31)) - 1u);
+                    if (x) err = BFSC_ERR_CORRUPT;
+                }
+        } else {                                                         // the stream inside ends inside the container
+            if (total < 64) err = BFSC_ERR_CORRUPT;
+            else {
+                const uint4 s1 = *reinterpret_cast<const uint4*>(in + 48);
+                const unsigned long long inner = (unsigned long long)s1.y << 32 | s1.x;
+                if (inner + 32 > total) err = BFSC_ERR_CORRUPT;
+            }
+        }
+    }
+    const unsigned long long me = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x, stride = (unsigned long long)gridDim.x * blockDim.x;
+    if (me == 0) {
+        sc->kind = kind; sc->skip = (err != 0u || kind == 0u) ? 1u : 0u; sc->n_listed = n_listed; sc->status = 0; sc->n_decoded = 0;
+        sc->pad = err;
+        if (err) set_status(status, err);
+    }
+    if (err) return;
+    if (kind == 0u) { for (unsigned long long w = me; w < words; w += stride) bitmap[w] = reinterpret_cast<const uint32_t*>(in + 32)[w]; }
+    else for (unsigned long long w = me; w < words + 4; w += stride) wb[w] = 0u;
+}
+__global__ void __launch_bounds__(256) k_vb_end(const uint32_t* __restrict__ wb, uint32_t* __restrict__ bitmap, unsigned long long n_bits,
+                                                const VbScratch* sc, uint32_t* status) {
+    if (sc->skip) return;                                                // kind 0 (done) or rejected
+    if (sc->status != 0u || sc->n_decoded != sc->n_listed) {             // the stream inside: malformed, an ID >= n_bits, or not n_listed IDs
+        if (blockIdx.x == 0 && threadIdx.x == 0) set_status(status, sc->status == BFSC_ERR_CUDA ? BFSC_ERR_CUDA : BFSC_ERR_CORRUPT);
+        return;
+    }
+    const bool invert = sc->kind == 2u;
+    const unsigned long long words = (n_bits + 31) / 32;
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < words; w += (unsigned long long)gridDim.x * blockDim.x) {
+        uint32_t x = invert ? ~wb[w] : wb[w];
+        if (w == words - 1 && (n_bits & 31)) x &= (1u << (uint32_t)(n_bits & 31)) - 1u;
+        bitmap[w] = x;
+    }
+}
+}  // namespace bfsc
+
+extern "C" bfsc_status bfsc_decompress_vbitmap(const void* d_in, size_t in_bytes, uint32_t* d_bitmap, size_t n_bits,
+                                               void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
+    using namespace bfsc;
+    if (!d_in || !d_workspace || !d_status || (n_bits && !d_bitmap) || (unsigned long long)n_bits > (1ull << 32)) return BFSC_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in & 15) || ((uintptr_t)d_workspace & 15) || ((uintptr_t)d_bitmap & 3)) return BFSC_ERR_INVALID_ARG;
+    if (workspace_bytes < bfsc_vbitmap_workspace_bytes(n_bits)) return BFSC_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    DeviceInfo dev;
+    if (!current_device(&dev)) return BFSC_ERR_CUDA;
+    const size_t words = (n_bits + 31) / 32, wb_bytes = align_up(4 * words + 16, 256);
+    VbScratch* sc = reinterpret_cast<VbScratch*>(d_workspace);
+    uint32_t* wb = reinterpret_cast<uint32_t*>(static_cast<char*>(d_workspace) + 256);
+    void* ws_std = static_cast<char*>(d_workspace) + 256 + wb_bytes;
+    int grid = (int)((words + 255) / 256);
+    if (grid > dev.sms * 8) grid = dev.sms * 8;
+    if (grid < 1) grid = 1;
+    k_vb_begin<<<grid, 256, 0, s>>>(static_cast<const unsigned char*>(d_in), in_bytes, n_bits, wb, d_bitmap, sc, d_status);
+    __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED);
+    if (cudaGetLastError() != cudaSuccess) return BFSC_ERR_CUDA;
+    const bfsc_status rc = decode_common(static_cast<const unsigned char*>(d_in) + 32, nullptr, in_bytes >= 32 ? in_bytes - 32 : 0, 1, BFSC_U32,
+                                         nullptr, ~(size_t)0, nullptr, reinterpret_cast<uint64_t*>(&sc->n_decoded), ws_std,
+                                         workspace_bytes - 256 - wb_bytes, &sc->status, cuda_stream,
+                                         BitSink{wb, 0, n_bits, &sc->status, nullptr}, &sc->skip);
+    if (rc != BFSC_OK) return rc;
+    k_vb_end<<<grid, 256, 0, s>>>(wb, d_bitmap, n_bits, sc, d_status);
+    __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED);
+    return cudaGetLastError() == cudaSuccess ? BFSC_OK : BFSC_ERR_CUDA;
 }

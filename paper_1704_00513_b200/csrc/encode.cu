@@ -1790,6 +1790,101 @@ extern "C" bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_
     return t == BFSC_U32 ? launch_encode_bitmap<32>(a, (cudaStream_t)cuda_stream) : launch_encode_bitmap<64>(a, (cudaStream_t)cuda_stream);
 }
 
+// ---- FORMAT.md §10: a (visited) bitmap as a container that lists its MINORITY bits, or holds the bitmap itself.
+// count -> select (the bitmap or its complement, tail bits cleared, into the workspace) -> the bitmap encode chain above on
+// that copy, its stream straight behind the container header, capped at the size of the bitmap itself (a stream that does
+// not fit is not smaller either) -> finish (header; the raw bitmap over the stream if that did not pay).
+namespace bfsc {
+struct VbScratch { unsigned long long count, stream_bytes, n_decoded, n_listed; unsigned int status, kind, skip, pad; };
+static_assert(sizeof(VbScratch) <= 256, "VbScratch");
+
+__device__ __forceinline__ uint32_t vb_word(const uint32_t* __restrict__ bm, unsigned long long w, unsigned long long n_bits, bool invert) {
+    const unsigned long long bit0 = 32ull * w;
+    if (bit0 >= n_bits) return 0u;
+    uint32_t x = bm[w];
+    if (invert) x = ~x;
+    if (n_bits - bit0 < 32) x &= (1u << (uint32_t)(n_bits - bit0)) - 1u;
+    return x;
+}
+__global__ void __launch_bounds__(256) k_vb_count(const uint32_t* __restrict__ bm, unsigned long long n_bits, VbScratch* sc) {
+    const unsigned long long words = (n_bits + 31) / 32;
+    unsigned long long c = 0;
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < words; w += (unsigned long long)gridDim.x * blockDim.x)
+        c += (unsigned long long)__popc(vb_word(bm, w, n_bits, false));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(kFull, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(&sc->count, c);
+}
+__global__ void __launch_bounds__(256) k_vb_select(const uint32_t* __restrict__ bm, unsigned long long n_bits, uint32_t* __restrict__ wb,
+                                                   unsigned long long wb_words, const VbScratch* sc) {
+    const bool invert = sc->count > n_bits - sc->count;              // the clear bits are the minority
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < wb_words; w += (unsigned long long)gridDim.x * blockDim.x)
+        wb[w] = vb_word(bm, w, n_bits, invert);
+}
+__global__ void __launch_bounds__(256) k_vb_finish(const uint32_t* __restrict__ bm, unsigned long long n_bits, unsigned char* __restrict__ out,
+                                                   unsigned long long raw_bytes, const VbScratch* sc, unsigned long long* out_bytes) {
+    const unsigned long long k = sc->count, sb = sc->stream_bytes;
+    const bool invert = k > n_bits - k;
+    const uint32_t kind = (sc->status == 0u && sb != 0ull && sb < raw_bytes) ? (invert ? 2u : 1u) : 0u;
+    if (kind == 0u) {                                                // the bitmap itself (tail bits cleared, zero pad)
+        uint32_t* y = reinterpret_cast<uint32_t*>(out + 32);
+        for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < raw_bytes / 4; w += (unsigned long long)gridDim.x * blockDim.x)
+            y[w] = vb_word(bm, w, n_bits, false);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const unsigned long long total = 32ull + (kind ? sb : raw_bytes), n_listed = kind ? (invert ? n_bits - k : k) : 0ull;
+        uint4 h0, h1;
+        h0.x = 0x56534642u;                                          // "BFSV"
+        h0.y = 1u | (32u << 8) | (kind << 16);
+        h0.z = (uint32_t)n_bits; h0.w = (uint32_t)(n_bits >> 32);
+        h1.x = (uint32_t)total; h1.y = (uint32_t)(total >> 32);
+        h1.z = (uint32_t)n_listed; h1.w = (uint32_t)(n_listed >> 32);
+        reinterpret_cast<uint4*>(out)[0] = h0;
+        reinterpret_cast<uint4*>(out)[1] = h1;
+        *out_bytes = total;
+    }
+}
+}  // namespace bfsc
+
+extern "C" size_t bfsc_vbitmap_bound(size_t n_bits) { return 32 + bfsc::align_up(4 * ((n_bits + 31) / 32), 16); }
+extern "C" size_t bfsc_vbitmap_workspace_bytes(size_t n_bits) {
+    return 256 + bfsc::align_up(4 * ((n_bits + 31) / 32) + 16, 256) + bfsc_bitmap_workspace_bytes(n_bits, BFSC_U32);
+}
+
+extern "C" bfsc_status bfsc_compress_vbitmap(bfsc_codec codec, const uint32_t* d_bitmap, size_t n_bits, void* d_out,
+                                             size_t out_capacity, uint64_t* d_out_bytes, void* d_workspace,
+                                             size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
+    using namespace bfsc;
+    codec = (bfsc_codec)((uint32_t)codec & ~(uint32_t)BFSC_CODEC_FLAG_EXCLUSIVE);
+    if (codec != BFSC_CODEC_PFOR && codec != BFSC_CODEC_BP128) return BFSC_ERR_INVALID_ARG;
+    if (!d_out || !d_out_bytes || !d_workspace || (n_bits && !d_bitmap) || (unsigned long long)n_bits > (1ull << 32)) return BFSC_ERR_INVALID_ARG;
+    if (((uintptr_t)d_out & 15) || ((uintptr_t)d_workspace & 15) || ((uintptr_t)d_bitmap & 3)) return BFSC_ERR_INVALID_ARG;
+    if (workspace_bytes < bfsc_vbitmap_workspace_bytes(n_bits)) return BFSC_ERR_INVALID_ARG;
+    if (out_capacity < bfsc_vbitmap_bound(n_bits)) return BFSC_ERR_DST_TOO_SMALL;
+    (void)d_status;                                                  // (nothing can go wrong on the device that is not an argument error above)
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    DeviceInfo dev;
+    if (!current_device(&dev)) return BFSC_ERR_CUDA;
+    const size_t words = (n_bits + 31) / 32, raw_bytes = align_up(4 * words, 16), wb_bytes = align_up(4 * words + 16, 256);
+    VbScratch* sc = reinterpret_cast<VbScratch*>(d_workspace);
+    uint32_t* wb = reinterpret_cast<uint32_t*>(static_cast<char*>(d_workspace) + 256);
+    void* ws_bm = static_cast<char*>(d_workspace) + 256 + wb_bytes;
+    if (cudaMemsetAsync(sc, 0, 256, s) != cudaSuccess) return BFSC_ERR_CUDA;
+    int grid = (int)((words + 255) / 256);
+    if (grid > dev.sms * 8) grid = dev.sms * 8;
+    if (grid < 1) grid = 1;
+    k_vb_count<<<grid, 256, 0, s>>>(d_bitmap, n_bits, sc);
+    k_vb_select<<<grid, 256, 0, s>>>(d_bitmap, n_bits, wb, wb_bytes / 4, sc);      // (every word of the copy: the encode kernels read whole 16-byte chunks)
+    __atomic_fetch_add(&g_launches, 2ull, __ATOMIC_RELAXED);
+    if (cudaGetLastError() != cudaSuccess) return BFSC_ERR_CUDA;
+    const bfsc_status rc = bfsc_compress_bitmap(codec, wb, n_bits, 0, BFSC_U32, 0, static_cast<unsigned char*>(d_out) + 32, raw_bytes,
+                                                reinterpret_cast<uint64_t*>(&sc->stream_bytes), ws_bm, workspace_bytes - 256 - wb_bytes, &sc->status, cuda_stream);
+    if (rc != BFSC_OK) return rc;
+    k_vb_finish<<<grid, 256, 0, s>>>(d_bitmap, n_bits, static_cast<unsigned char*>(d_out), raw_bytes, sc, (unsigned long long*)d_out_bytes);
+    __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED);
+    return cudaGetLastError() == cudaSuccess ? BFSC_OK : BFSC_ERR_CUDA;
+}
+
 extern "C" bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
                                      void* d_out, size_t out_capacity, uint64_t* d_out_bytes, void* d_workspace,
                                      size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {

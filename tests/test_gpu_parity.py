@@ -1339,3 +1339,109 @@ def test_batch_scatter_errors(B, oracle_mod):
             B.compress_batch_scatter(kwargs.get("codec", PFOR), d_ids, d_off, n_buf, W, 0, kwargs.get("dst", dst), cap,
                                      kwargs.get("sizes", sizes), ws, status)
         assert e.value.code == kwargs.get("code", B.ERR_INVALID_ARG)
+
+
+# ---- FORMAT.md §10: visited-bitmap containers (bfsc_compress_vbitmap / bfsc_decompress_vbitmap) ----
+def _vb_case(B, oracle_mod, bm_words, n_bits, codec=PFOR, dirty_tail=False):
+    dev = torch.device("cuda")
+    words = (n_bits + 31) // 32
+    src = bm_words.copy()
+    if dirty_tail and n_bits % 32:
+        src[-1] |= np.uint32(0xFFFFFFFF) << np.uint32(n_bits % 32)     # garbage beyond n_bits in the caller's last word
+    d_bm = torch.from_numpy(src.view(np.int32).copy()).to(dev) if words else torch.zeros(1, dtype=torch.int32, device=dev)
+    cap = B.vbitmap_bound(n_bits)
+    out = torch.full((cap + 64,), 0xAB, dtype=torch.uint8, device=dev)
+    nb = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    ws = torch.empty(B.vbitmap_workspace_bytes(n_bits), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    B.compress_vbitmap(codec, d_bm, n_bits, out[:cap], nb, ws, status)
+    torch.cuda.synchronize()
+    ref = oracle_mod.compress_vbitmap(bm_words, n_bits, codec)
+    assert int(status.item()) == 0 and int(nb.item()) == len(ref), (n_bits, int(nb.item()), len(ref))
+    got = out[:len(ref)].cpu().numpy()
+    assert np.array_equal(got, ref), f"n_bits {n_bits}: container differs at byte {int(np.nonzero(got != ref)[0][0])} (kind {ref[6]})"
+    assert bool((out[cap:] == 0xAB).all()), "wrote beyond capacity"
+    back = torch.full((max(words, 1) + 2,), 0x55555555, dtype=torch.int32, device=dev)
+    B.decompress_vbitmap(out, len(ref), back, n_bits, ws, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    assert np.array_equal(back[:words].cpu().numpy().view(np.uint32), bm_words[:words]), f"n_bits {n_bits}: decoded bitmap differs (kind {ref[6]})"
+    assert bool((back[words:] == 0x55555555).all()), "wrote beyond the bitmap"
+    return ref
+
+
+@pytest.mark.parametrize("codec", CODECS)
+def test_vbitmap_container(B, oracle_mod, codec):
+    """Bytes against the oracle and identity round trip: sizes 0 … 2^22 + 17 bits, densities from empty to full (set bits
+    listed, clear bits listed, the bitmap itself), clustered bits, garbage beyond n_bits in the caller's last word."""
+    rng = np.random.default_rng(7 + codec)
+    kinds = set()
+    for n_bits in (0, 1, 31, 32, 33, 384, 385, 1000, 4097, 128 * 64 * 3 + 5, 1 << 20, (1 << 22) + 17):
+        for dens in (0.0, 1.0, 0.5, 0.001, 0.999, 0.05, 0.95, 0.12, 0.88):
+            bits = rng.random(n_bits) < dens
+            words = (n_bits + 31) // 32
+            pad = np.zeros(words * 32, dtype=bool)
+            pad[:n_bits] = bits
+            bm = np.packbits(pad.reshape(-1, 32), axis=1, bitorder="little").view(np.uint32).reshape(-1) if words else np.zeros(0, np.uint32)
+            kinds.add(int(_vb_case(B, oracle_mod, bm, n_bits, codec, dirty_tail=True)[6]))
+    assert kinds == {0, 1, 2}
+    # a late-BFS visited bitmap: 2^24 vertices, runs of unvisited ones
+    n_bits = 1 << 24
+    bm = streams.frontier_bitmap(n_bits, 0.02, seed=3, run=16).numpy().view(np.uint32)[:n_bits // 32]
+    ref = _vb_case(B, oracle_mod, ~bm, n_bits, codec)
+    assert ref[6] == 2 and len(ref) < n_bits // 8 // 3            # (2 % of the bits clear, in runs: under a third of the bitmap)
+
+
+def test_vbitmap_rejects(B, oracle_mod):
+    """The decoder's verdicts are the oracle's (FORMAT.md §10), and a rejected container leaves the caller's bitmap alone."""
+    dev = torch.device("cuda")
+    rng = np.random.default_rng(11)
+    n_bits = 5000
+    words = (n_bits + 31) // 32
+    ws = torch.empty(B.vbitmap_workspace_bytes(n_bits), dtype=torch.uint8, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+
+    def pack(b):
+        pad = np.zeros(words * 32, dtype=bool)
+        pad[:n_bits] = b
+        return np.packbits(pad.reshape(-1, 32), axis=1, bitorder="little").view(np.uint32).reshape(-1)
+
+    def verdict(buf, nb=n_bits):
+        d = torch.from_numpy(np.concatenate([buf, np.zeros(16, np.uint8)])).to(dev)
+        back = torch.full((words,), 0x77777777, dtype=torch.int32, device=dev)
+        status.zero_()
+        w2 = ws if nb == n_bits else torch.empty(B.vbitmap_workspace_bytes(nb), dtype=torch.uint8, device=dev)
+        B.decompress_vbitmap(d, len(buf), back, nb, w2, status)
+        torch.cuda.synchronize()
+        rc = int(status.item())
+        if rc:
+            assert bool((back == 0x77777777).all()), "a rejected container changed the bitmap"
+        try:
+            oracle_mod.decompress_vbitmap(buf, nb)
+            ref = 0
+        except oracle_mod.OracleError as e:
+            ref = e.code
+        assert rc == ref, (rc, ref)
+        return rc
+
+    sparse = oracle_mod.compress_vbitmap(pack(rng.random(n_bits) < 0.01), n_bits)        # kind 1
+    dense = oracle_mod.compress_vbitmap(pack(rng.random(n_bits) < 0.99), n_bits)         # kind 2
+    half = oracle_mod.compress_vbitmap(pack(rng.random(n_bits) < 0.5), n_bits)           # kind 0
+    assert (sparse[6], dense[6], half[6]) == (1, 2, 0)
+    for good in (sparse, dense, half):
+        assert verdict(good) == 0
+        for pos, val in ((0, 0x58), (4, 2), (5, 64), (6, 3), (7, 1), (16, (int(good[16]) + 16) & 0xff), (16, (int(good[16]) - 16) & 0xff), (24, (int(good[24]) + 1) & 0xff)):
+            bad = good.copy()
+            bad[pos] = val
+            assert verdict(bad) != 0, (int(good[6]), pos)
+        assert verdict(good[:-16]) == B.ERR_CORRUPT
+        assert verdict(good, n_bits + 1) == B.ERR_DST_TOO_SMALL
+    bad = half.copy()
+    bad[32 + n_bits // 8] |= 1 << 7                                        # a pad bit of the kind-0 payload
+    assert verdict(bad) == B.ERR_CORRUPT
+    bad = sparse.copy()
+    bad[32 + 40] ^= 0xFF                                                   # inside the stream: its first block header / directory
+    verdict(bad)                                                           # (whatever the oracle says)
+    far = sparse.copy()                                                    # the container claims fewer bits than its IDs need
+    far[8:16] = np.frombuffer((600).to_bytes(8, "little"), dtype=np.uint8)
+    assert verdict(far, 600) == B.ERR_CORRUPT
