@@ -5,7 +5,7 @@
 //   one buffer              k_enc_plan -> k_enc_tiles<W, 0> [-> k_enc_streams: no block at all] [-> k_enc_fallback: FORMAT.md §8]
 //   small batch             k_enc_small (one cluster; <= 1024 buffers, <= 2048 blocks by the workspace size)
 //   batch                   k_enc_planblocks (<= 8192 buffers; else k_enc_plan -> k_enc_blocks) -> k_enc_tiles<W, 1> -> k_enc_streams
-//   frontier bitmap         k_bm_count -> k_bm_plan -> k_bm_starts -> k_enc_tiles<W, 2> -> k_bm_finish
+//   frontier bitmap         k_bm_count -> k_bm_plan -> k_bm_list (sparse bitmaps: the ID list) -> k_bm_starts (dense ones: block starts) -> k_enc_tiles<W, 2> -> k_bm_finish
 #include <mutex>
 
 #include "bitmap_stage.cuh"
@@ -23,6 +23,8 @@ struct EncArgs {
     unsigned long long* super;          //   bitmap: set bits before every super-chunk of 32 chunks (n_super + 1 entries, behind the standard workspace and `chunk`)
     uint32_t* chunk;                    //   bitmap: set bits of every 1024-bit chunk (32 n_super entries, before `super`)
     unsigned long long n_chunks, n_super;
+    void* list;                         //   bitmap, sparse (at most one set bit in 32): the IDs written out by k_bm_list (behind `super`), staged by the
+                                        //   tile kernel like an ID array; denser bitmaps are expanded inside the tile kernel (bm_expand)
     uint32_t fallback;                  // BFSC_CODEC_FLAG_RAW_FALLBACK (FORMAT.md §8), single-buffer calls
     uint32_t n_buf;
     uint32_t codec;                     // encoder rule = mode byte: 1 PFOR-D1 (E2: size argmin), 2 BP128-D1 (b = maxw, no exceptions; FORMAT.md §7)
@@ -46,6 +48,8 @@ __device__ __forceinline__ unsigned long long buf_start(const EncArgs& a, uint32
 __device__ __forceinline__ unsigned long long buf_count(const EncArgs& a, uint32_t i) {
     return a.in_off ? a.in_off[i + 1] - a.in_off[i] : a.n_single;
 }
+// bitmap source: sparse (at most one set bit in 32 on average) = the IDs are listed by k_bm_list, not expanded in the tile kernel
+__device__ __forceinline__ bool bm_sparse(const EncArgs& a) { return a.ws.hdr->n_ids * 32ull <= a.n_bits; }
 
 
 constexpr int kEncWorkers = 8;                           // worker warps per CTA
@@ -742,9 +746,15 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     mbar_wait(&mb_post[0], 0);                                           // the CTA's first tile is posted (by the prep warp)
     bool have = s_tile[0] != kNoTile;
     uint4* land = area + Smem::kStageChunks + kNB * Img::kBufChunks;      // bitmap source: the words of the warp's 8 blocks
+    bool listed = false;                                                 // bitmap source, sparse: the IDs come from k_bm_list's list
+    const T* list = reinterpret_cast<const T*>(a.list);
     if constexpr (kBits) {
         static_assert(!kBits || Img::kCap >= 16 + 16 * 32 + 16, "a bitmap has no ID array for the slow path: every block must fit its image slot");
-        if (have) bm_prefetch<kLandChunks>(land, a.bitmap, s_start[0], warp, lane);
+        listed = bm_sparse(a);
+        if (have) {
+            if (listed) quad_prefetch<W>(slot, list + blk_xoff(0, j), blk_m(0, j));
+            else bm_prefetch<kLandChunks>(land, a.bitmap, s_start[0], warp, lane);
+        }
     } else {
         if (have && (kBatch || !a.exclusive)) quad_prefetch<W>(slot, ids + blk_xoff(0, j), blk_m(0, j));   // (exclusive single-buffer calls: see the top)
     }
@@ -763,7 +773,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             cp_async_wait_all();
             __syncwarp();
             if constexpr (kBits) {                                       // E1, first half: the block's set bits -> raw IDs in the slot
-                bm_expand<T, kLandChunks>(reinterpret_cast<T*>(slot), s_start[k & (kRing - 1)], warp, q, l, land, a.bitmap, a.id_base);
+                if (!listed) bm_expand<T, kLandChunks>(reinterpret_cast<T*>(slot), s_start[k & (kRing - 1)], warp, q, l, land, a.bitmap, a.id_base);
                 __syncwarp();
             }
             uint32_t d[32];
@@ -837,7 +847,10 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
             mbar_wait(&mb_post[(k + 1) & (kRing - 1)], ((k + 1) / kRing) & 1);   // tile k+1 is posted
             have_next = s_tile[(k + 1) & (kRing - 1)] != kNoTile;
             if constexpr (kBits) {
-                if (have_next) bm_prefetch<kLandChunks>(land, a.bitmap, s_start[(k + 1) & (kRing - 1)], warp, lane);
+                if (have_next) {
+                    if (listed) quad_prefetch<W>(slot, list + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));
+                    else bm_prefetch<kLandChunks>(land, a.bitmap, s_start[(k + 1) & (kRing - 1)], warp, lane);
+                }
             } else {
                 if (have_next) quad_prefetch<W>(slot, ids + blk_xoff((k + 1) & (kRing - 1), j), blk_m((k + 1) & (kRing - 1), j));   // same slots
             }
@@ -1421,6 +1434,43 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
 // The bitmap words (the caller's input, stable since this call's first kernel) are loaded and ranked BEFORE the wait for
 // the plan kernel, all kStartsPer loads in flight at once; after it only the two prefix tables are read.
 constexpr int kStartsPer = 4;
+// Sparse bitmaps (at most one set bit in 32 on average): the IDs are written out as a list by the WHOLE grid — a warp per
+// chunk, from the same chunk / super-chunk prefixes k_bm_starts uses — and the tile kernel stages its blocks from that
+// list as it does from an ID array. Inside the tile kernel a block's 128 set bits are found by ONE quad: a 0.2 % dense
+// bitmap of 2^25 bits is 524 blocks of 2000 words each, 200 us on 9 CTAs while 139 SMs idle.
+template <int W>
+__global__ void __launch_bounds__(256) k_bm_list(EncArgs a) {
+    using T = typename IdT<W>::T;
+    pdl_launch_dependents();
+    const int lane = threadIdx.x & 31;
+    const unsigned long long stride = (unsigned long long)gridDim.x * 8;
+    unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    pdl_wait();
+    if (a.ws.hdr->ok == 0 || !bm_sparse(a)) return;
+    T* list = reinterpret_cast<T*>(a.list);
+    for (; c < a.n_chunks; c += stride) {
+        uint32_t x = bm_word(a, c, lane);
+        const uint32_t k = (uint32_t)__popc(x);
+        uint32_t inc = k;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
+        if (__shfl_sync(kFull, inc, 31) == 0u) continue;             // an empty chunk
+        const unsigned long long sc = c / kSuperChunks;
+        const uint32_t cnt = a.chunk[sc * kSuperChunks + lane];
+        uint32_t ci = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, ci, o); if (lane >= o) ci += y; }
+        unsigned long long at = a.super[sc] + __shfl_sync(kFull, ci - cnt, (int)(c % kSuperChunks)) + (inc - k);
+        const unsigned long long id0 = a.id_base + c * kChunkBits + 32ull * lane;
+        while (x) {
+            const uint32_t b = (uint32_t)__ffs(x) - 1u;
+            x &= x - 1u;
+            BFSC_CHECK(at < a.ws.hdr->n_ids);
+            list[at++] = (T)(id0 + b);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
@@ -1439,7 +1489,7 @@ __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
             for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc[u], o); if (lane >= o) inc[u] += y; }
         }
         if (!waited) { pdl_wait(); waited = true; }
-        if (a.ws.hdr->ok == 0) return;
+        if (a.ws.hdr->ok == 0 || bm_sparse(a)) return;               // (sparse: the tile kernel stages from k_bm_list's list, no block starts)
         // set bits before each of the warp's chunks: its super-chunk's prefix + the counts of the chunks before it in
         // the super-chunk (the warp's chunks share one: one coalesced load of its 32 counts, scanned here)
         unsigned long long p0[kStartsPer];
@@ -1518,6 +1568,11 @@ __global__ void __launch_bounds__(256) k_bm_finish(EncArgs a) {
     const unsigned long long nb_all = (n + kBlk - 1) / kBlk;
     const int lane = threadIdx.x & 31;
     T* y = reinterpret_cast<T*>(a.out + 32);
+    if (bm_sparse(a)) {                                                      // the IDs are listed already (k_bm_list): the RAW body is that list
+        const T* list = reinterpret_cast<const T*>(a.list);
+        for (unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (unsigned long long)gridDim.x * blockDim.x)
+            y[j] = list[j];
+    } else
     for (unsigned long long g = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5); g < nb_all; g += (unsigned long long)gridDim.x * 8) {
         const uint32_t s = starts[g], e = starts[g + 1];
         if (e <= s) continue;
@@ -1695,6 +1750,7 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
     size_t tgrid = (size_t)((a.n_chunks + 8 * kStartsPer - 1) / (8 * kStartsPer));
     if (tgrid > (size_t)dev.sms * 8) tgrid = (size_t)dev.sms * 8;
     if (tgrid < 1) tgrid = 1;
+    BFSC_LAUNCH(launch_dep(k_bm_list<W>, (int)cgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_bm_starts, (int)tgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 2>, grid, kEncThreads, kSmem, s, a));
     if (a.thr > 0 || a.fallback)                                     // (else no stream can end up RAW, and the plan wrote the empty one)
@@ -1784,6 +1840,7 @@ extern "C" bfsc_status bfsc_compress_bitmap(bfsc_codec codec, const uint32_t* d_
     a.bitmap = d_bitmap; a.n_bits = n_bits; a.id_base = id_base;
     a.chunk = reinterpret_cast<uint32_t*>(static_cast<char*>(d_workspace) + std_bytes);       // 16-byte aligned: read as uint4
     a.super = reinterpret_cast<unsigned long long*>(a.chunk + n_super * kSuperChunks);
+    a.list = static_cast<char*>(d_workspace) + std_bytes + align_up(8 * (n_super + 1) + 4 * 32 * n_super + 16, 16);
     a.n_chunks = n_chunks; a.n_super = n_super;
     a.fallback = fallback; a.n_buf = 1; a.codec = (uint32_t)codec; a.thr = raw_threshold_bytes;
     a.out = (unsigned char*)d_out; a.out_cap = out_capacity; a.out_total = (unsigned long long*)d_out_bytes; a.status = d_status;
