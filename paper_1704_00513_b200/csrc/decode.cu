@@ -1028,6 +1028,8 @@ namespace bfsc {
 struct VbScratch { unsigned long long count, stream_bytes, n_decoded, n_listed; unsigned int status, kind, skip, pad; };
 __global__ void __launch_bounds__(256) k_vb_begin(const unsigned char* __restrict__ in, unsigned long long in_bytes, unsigned long long n_bits,
                                                   uint32_t* __restrict__ wb, uint32_t* __restrict__ bitmap, VbScratch* sc, uint32_t* status) {
+    pdl_wait();                                                          // the call before this one is complete (workspace, inputs)
+    pdl_launch_dependents();
     const unsigned long long words = (n_bits + 31) / 32, raw_bytes = (4 * words + 15) & ~15ull;
     uint32_t err = 0, kind = 0;
     unsigned long long total = 0, n_listed = 0;
@@ -1070,6 +1072,8 @@ __global__ void __launch_bounds__(256) k_vb_begin(const unsigned char* __restric
 }
 __global__ void __launch_bounds__(256) k_vb_end(const uint32_t* __restrict__ wb, uint32_t* __restrict__ bitmap, unsigned long long n_bits,
                                                 const VbScratch* sc, uint32_t* status) {
+    pdl_wait();
+    pdl_launch_dependents();
     if (sc->skip) return;                                                // kind 0 (done) or rejected
     if (sc->status != 0u || sc->n_decoded != sc->n_listed) {             // the stream inside: malformed, an ID >= n_bits, or not n_listed IDs
         if (blockIdx.x == 0 && threadIdx.x == 0) set_status(status, sc->status == BFSC_ERR_CUDA ? BFSC_ERR_CUDA : BFSC_ERR_CORRUPT);
@@ -1101,15 +1105,13 @@ extern "C" bfsc_status bfsc_decompress_vbitmap(const void* d_in, size_t in_bytes
     int grid = (int)((words + 255) / 256);
     if (grid > dev.sms * 8) grid = dev.sms * 8;
     if (grid < 1) grid = 1;
-    k_vb_begin<<<grid, 256, 0, s>>>(static_cast<const unsigned char*>(d_in), in_bytes, n_bits, wb, d_bitmap, sc, d_status);
-    __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED);
-    if (cudaGetLastError() != cudaSuccess) return BFSC_ERR_CUDA;
+    BFSC_LAUNCH(launch_dep_v(k_vb_begin, grid, 256, 0, s, static_cast<const unsigned char*>(d_in), (unsigned long long)in_bytes,
+                             (unsigned long long)n_bits, wb, d_bitmap, sc, d_status));
     const bfsc_status rc = decode_common(static_cast<const unsigned char*>(d_in) + 32, nullptr, in_bytes >= 32 ? in_bytes - 32 : 0, 1, BFSC_U32,
                                          nullptr, ~(size_t)0, nullptr, reinterpret_cast<uint64_t*>(&sc->n_decoded), ws_std,
                                          workspace_bytes - 256 - wb_bytes, &sc->status, cuda_stream,
                                          BitSink{wb, 0, n_bits, &sc->status, nullptr}, &sc->skip);
     if (rc != BFSC_OK) return rc;
-    k_vb_end<<<grid, 256, 0, s>>>(wb, d_bitmap, n_bits, sc, d_status);
-    __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED);
-    return cudaGetLastError() == cudaSuccess ? BFSC_OK : BFSC_ERR_CUDA;
+    BFSC_LAUNCH(launch_dep_v(k_vb_end, grid, 256, 0, s, (const uint32_t*)wb, d_bitmap, (unsigned long long)n_bits, (const VbScratch*)sc, d_status));
+    return BFSC_OK;
 }

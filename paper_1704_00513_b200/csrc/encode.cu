@@ -5,7 +5,7 @@
 //   one buffer              k_enc_plan -> k_enc_tiles<W, 0> [-> k_enc_streams: no block at all] [-> k_enc_fallback: FORMAT.md §8]
 //   small batch             k_enc_small (one cluster; <= 1024 buffers, <= 2048 blocks by the workspace size)
 //   batch                   k_enc_planblocks (<= 8192 buffers; else k_enc_plan -> k_enc_blocks) -> k_enc_tiles<W, 1> -> k_enc_streams
-//   frontier bitmap         k_bm_count -> k_bm_plan -> k_bm_list (sparse bitmaps: the ID list) -> k_bm_starts (dense ones: block starts) -> k_enc_tiles<W, 2> -> k_bm_finish
+//   frontier bitmap         k_bm_count -> k_bm_plan -> k_bm_starts (block starts; sparse bitmaps: the ID list instead) -> k_enc_tiles<W, 2> -> k_bm_finish
 #include <mutex>
 
 #include "bitmap_stage.cuh"
@@ -23,7 +23,7 @@ struct EncArgs {
     unsigned long long* super;          //   bitmap: set bits before every super-chunk of 32 chunks (n_super + 1 entries, behind the standard workspace and `chunk`)
     uint32_t* chunk;                    //   bitmap: set bits of every 1024-bit chunk (32 n_super entries, before `super`)
     unsigned long long n_chunks, n_super;
-    void* list;                         //   bitmap, sparse (at most one set bit in 32): the IDs written out by k_bm_list (behind `super`), staged by the
+    void* list;                         //   bitmap, sparse (at most one set bit in 32): the IDs written out by k_bm_starts (behind `super`), staged by the
                                         //   tile kernel like an ID array; denser bitmaps are expanded inside the tile kernel (bm_expand)
     uint32_t fallback;                  // BFSC_CODEC_FLAG_RAW_FALLBACK (FORMAT.md §8), single-buffer calls
     uint32_t n_buf;
@@ -48,7 +48,7 @@ __device__ __forceinline__ unsigned long long buf_start(const EncArgs& a, uint32
 __device__ __forceinline__ unsigned long long buf_count(const EncArgs& a, uint32_t i) {
     return a.in_off ? a.in_off[i + 1] - a.in_off[i] : a.n_single;
 }
-// bitmap source: sparse (at most one set bit in 32 on average) = the IDs are listed by k_bm_list, not expanded in the tile kernel
+// bitmap source: sparse (at most one set bit in 32 on average) = the IDs are listed by k_bm_starts, not expanded in the tile kernel
 __device__ __forceinline__ bool bm_sparse(const EncArgs& a) { return a.ws.hdr->n_ids * 32ull <= a.n_bits; }
 
 
@@ -746,7 +746,7 @@ __global__ void __launch_bounds__(kEncThreads, kEncCtasPerSm) k_enc_tiles(EncArg
     mbar_wait(&mb_post[0], 0);                                           // the CTA's first tile is posted (by the prep warp)
     bool have = s_tile[0] != kNoTile;
     uint4* land = area + Smem::kStageChunks + kNB * Img::kBufChunks;      // bitmap source: the words of the warp's 8 blocks
-    bool listed = false;                                                 // bitmap source, sparse: the IDs come from k_bm_list's list
+    bool listed = false;                                                 // bitmap source, sparse: the IDs come from k_bm_starts' list
     const T* list = reinterpret_cast<const T*>(a.list);
     if constexpr (kBits) {
         static_assert(!kBits || Img::kCap >= 16 + 16 * 32 + 16, "a bitmap has no ID array for the slow path: every block must fit its image slot");
@@ -1434,43 +1434,11 @@ __global__ void __launch_bounds__(1024) k_bm_plan(EncArgs a) {
 // The bitmap words (the caller's input, stable since this call's first kernel) are loaded and ranked BEFORE the wait for
 // the plan kernel, all kStartsPer loads in flight at once; after it only the two prefix tables are read.
 constexpr int kStartsPer = 4;
-// Sparse bitmaps (at most one set bit in 32 on average): the IDs are written out as a list by the WHOLE grid — a warp per
-// chunk, from the same chunk / super-chunk prefixes k_bm_starts uses — and the tile kernel stages its blocks from that
-// list as it does from an ID array. Inside the tile kernel a block's 128 set bits are found by ONE quad: a 0.2 % dense
-// bitmap of 2^25 bits is 524 blocks of 2000 words each, 200 us on 9 CTAs while 139 SMs idle.
+// Sparse bitmaps (at most one set bit in 32 on average, decided on the device from the popcount): no block starts — the IDs
+// are written out as a list by the WHOLE grid here, a warp per chunk from the same chunk / super-chunk prefixes, and the tile
+// kernel stages its blocks from that list as it does from an ID array. Inside the tile kernel a block's 128 set bits are
+// found by ONE quad: a 0.2 % dense bitmap of 2^25 bits is 524 blocks of 2000 words each, 250 us on 9 CTAs while 139 SMs idle.
 template <int W>
-__global__ void __launch_bounds__(256) k_bm_list(EncArgs a) {
-    using T = typename IdT<W>::T;
-    pdl_launch_dependents();
-    const int lane = threadIdx.x & 31;
-    const unsigned long long stride = (unsigned long long)gridDim.x * 8;
-    unsigned long long c = (unsigned long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-    pdl_wait();
-    if (a.ws.hdr->ok == 0 || !bm_sparse(a)) return;
-    T* list = reinterpret_cast<T*>(a.list);
-    for (; c < a.n_chunks; c += stride) {
-        uint32_t x = bm_word(a, c, lane);
-        const uint32_t k = (uint32_t)__popc(x);
-        uint32_t inc = k;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc, o); if (lane >= o) inc += y; }
-        if (__shfl_sync(kFull, inc, 31) == 0u) continue;             // an empty chunk
-        const unsigned long long sc = c / kSuperChunks;
-        const uint32_t cnt = a.chunk[sc * kSuperChunks + lane];
-        uint32_t ci = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, ci, o); if (lane >= o) ci += y; }
-        unsigned long long at = a.super[sc] + __shfl_sync(kFull, ci - cnt, (int)(c % kSuperChunks)) + (inc - k);
-        const unsigned long long id0 = a.id_base + c * kChunkBits + 32ull * lane;
-        while (x) {
-            const uint32_t b = (uint32_t)__ffs(x) - 1u;
-            x &= x - 1u;
-            BFSC_CHECK(at < a.ws.hdr->n_ids);
-            list[at++] = (T)(id0 + b);
-        }
-    }
-}
-
 __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
@@ -1489,7 +1457,8 @@ __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
             for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, inc[u], o); if (lane >= o) inc[u] += y; }
         }
         if (!waited) { pdl_wait(); waited = true; }
-        if (a.ws.hdr->ok == 0 || bm_sparse(a)) return;               // (sparse: the tile kernel stages from k_bm_list's list, no block starts)
+        if (a.ws.hdr->ok == 0) return;
+        const bool sparse = bm_sparse(a);
         // set bits before each of the warp's chunks: its super-chunk's prefix + the counts of the chunks before it in
         // the super-chunk (the warp's chunks share one: one coalesced load of its 32 counts, scanned here)
         unsigned long long p0[kStartsPer];
@@ -1502,6 +1471,23 @@ __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
             const unsigned long long sp = a.super[sc];
 #pragma unroll
             for (int u = 0; u < kStartsPer; u++) p0[u] = sp + __shfl_sync(kFull, ci - cnt, (int)((c0 + u) % kSuperChunks));
+        }
+        if (sparse) {                                                // the ID list instead of block starts
+            using T = typename IdT<W>::T;
+            T* list = reinterpret_cast<T*>(a.list);
+#pragma unroll
+            for (int u = 0; u < kStartsPer; u++) {
+                unsigned long long at = p0[u] + (inc[u] - k[u]);
+                const unsigned long long id0 = a.id_base + (c0 + u) * kChunkBits + 32ull * lane;
+                uint32_t xx = x[u];
+                while (xx) {
+                    const uint32_t b = (uint32_t)__ffs((int)xx) - 1u;
+                    xx &= xx - 1u;
+                    BFSC_CHECK(at < a.ws.hdr->n_ids);
+                    list[at++] = (T)(id0 + b);
+                }
+            }
+            continue;
         }
         uint32_t* starts = reinterpret_cast<uint32_t*>(a.ws.blk_tab);
 #pragma unroll
@@ -1524,7 +1510,7 @@ __global__ void __launch_bounds__(256) k_bm_starts(EncArgs a) {
         }
     }
     if (!waited) pdl_wait();
-    if (blockIdx.x == 0 && threadIdx.x == 0 && a.ws.hdr->ok != 0)
+    if (blockIdx.x == 0 && threadIdx.x == 0 && a.ws.hdr->ok != 0 && !bm_sparse(a))
         reinterpret_cast<uint32_t*>(a.ws.blk_tab)[(a.ws.hdr->n_ids + kBlk - 1) / kBlk] = (uint32_t)a.n_bits;
 }
 
@@ -1568,7 +1554,7 @@ __global__ void __launch_bounds__(256) k_bm_finish(EncArgs a) {
     const unsigned long long nb_all = (n + kBlk - 1) / kBlk;
     const int lane = threadIdx.x & 31;
     T* y = reinterpret_cast<T*>(a.out + 32);
-    if (bm_sparse(a)) {                                                      // the IDs are listed already (k_bm_list): the RAW body is that list
+    if (bm_sparse(a)) {                                                      // the IDs are listed already (k_bm_starts): the RAW body is that list
         const T* list = reinterpret_cast<const T*>(a.list);
         for (unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (unsigned long long)gridDim.x * blockDim.x)
             y[j] = list[j];
@@ -1750,8 +1736,7 @@ static bfsc_status launch_encode_bitmap(const EncArgs& a_in, cudaStream_t s) {
     size_t tgrid = (size_t)((a.n_chunks + 8 * kStartsPer - 1) / (8 * kStartsPer));
     if (tgrid > (size_t)dev.sms * 8) tgrid = (size_t)dev.sms * 8;
     if (tgrid < 1) tgrid = 1;
-    BFSC_LAUNCH(launch_dep(k_bm_list<W>, (int)cgrid, 256, 0, s, a));
-    BFSC_LAUNCH(launch_dep(k_bm_starts, (int)tgrid, 256, 0, s, a));
+    BFSC_LAUNCH(launch_dep(k_bm_starts<W>, (int)tgrid, 256, 0, s, a));
     BFSC_LAUNCH(launch_dep(k_enc_tiles<W, 2>, grid, kEncThreads, kSmem, s, a));
     if (a.thr > 0 || a.fallback)                                     // (else no stream can end up RAW, and the plan wrote the empty one)
         BFSC_LAUNCH(launch_dep(k_bm_finish<W>, (int)cgrid, 256, 0, s, a));
@@ -1863,23 +1848,42 @@ __device__ __forceinline__ uint32_t vb_word(const uint32_t* __restrict__ bm, uns
     if (n_bits - bit0 < 32) x &= (1u << (uint32_t)(n_bits - bit0)) - 1u;
     return x;
 }
-__global__ void __launch_bounds__(256) k_vb_count(const uint32_t* __restrict__ bm, unsigned long long n_bits, VbScratch* sc) {
+// (every kernel of the container is launched like the others of the library: programmatic dependent launch, no memset node)
+__global__ void __launch_bounds__(256) k_vb_count(const uint32_t* __restrict__ bm, unsigned long long n_bits, unsigned long long* __restrict__ partial) {
+    __shared__ unsigned long long s_c[8];
+    pdl_wait();                                                      // the call before this one is complete (workspace)
+    pdl_launch_dependents();
     const unsigned long long words = (n_bits + 31) / 32;
     unsigned long long c = 0;
     for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < words; w += (unsigned long long)gridDim.x * blockDim.x)
         c += (unsigned long long)__popc(vb_word(bm, w, n_bits, false));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(kFull, c, o);
-    if ((threadIdx.x & 31) == 0 && c) atomicAdd(&sc->count, c);
+    if ((threadIdx.x & 31) == 0) s_c[threadIdx.x >> 5] = c;
+    __syncthreads();
+    if (threadIdx.x == 0) partial[blockIdx.x] = s_c[0] + s_c[1] + s_c[2] + s_c[3] + s_c[4] + s_c[5] + s_c[6] + s_c[7];   // one sum per CTA
 }
 __global__ void __launch_bounds__(256) k_vb_select(const uint32_t* __restrict__ bm, unsigned long long n_bits, uint32_t* __restrict__ wb,
-                                                   unsigned long long wb_words, const VbScratch* sc) {
-    const bool invert = sc->count > n_bits - sc->count;              // the clear bits are the minority
+                                                   unsigned long long wb_words, VbScratch* sc, const unsigned long long* __restrict__ partial, int n_partial) {
+    __shared__ unsigned long long s_c[8];
+    pdl_wait();
+    pdl_launch_dependents();
+    unsigned long long c = 0;                                        // every CTA adds up the per-CTA popcounts for itself
+    for (int i = threadIdx.x; i < n_partial; i += blockDim.x) c += partial[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(kFull, c, o);
+    if ((threadIdx.x & 31) == 0) s_c[threadIdx.x >> 5] = c;
+    __syncthreads();
+    const unsigned long long count = s_c[0] + s_c[1] + s_c[2] + s_c[3] + s_c[4] + s_c[5] + s_c[6] + s_c[7];
+    if (blockIdx.x == 0 && threadIdx.x == 0) { sc->count = count; sc->stream_bytes = 0; sc->status = 0; }
+    const bool invert = count > n_bits - count;                      // the clear bits are the minority
     for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < wb_words; w += (unsigned long long)gridDim.x * blockDim.x)
         wb[w] = vb_word(bm, w, n_bits, invert);
 }
 __global__ void __launch_bounds__(256) k_vb_finish(const uint32_t* __restrict__ bm, unsigned long long n_bits, unsigned char* __restrict__ out,
                                                    unsigned long long raw_bytes, const VbScratch* sc, unsigned long long* out_bytes) {
+    pdl_wait();
+    pdl_launch_dependents();
     const unsigned long long k = sc->count, sb = sc->stream_bytes;
     const bool invert = k > n_bits - k;
     const uint32_t kind = (sc->status == 0u && sb != 0ull && sb < raw_bytes) ? (invert ? 2u : 1u) : 0u;
@@ -1926,20 +1930,21 @@ extern "C" bfsc_status bfsc_compress_vbitmap(bfsc_codec codec, const uint32_t* d
     VbScratch* sc = reinterpret_cast<VbScratch*>(d_workspace);
     uint32_t* wb = reinterpret_cast<uint32_t*>(static_cast<char*>(d_workspace) + 256);
     void* ws_bm = static_cast<char*>(d_workspace) + 256 + wb_bytes;
-    if (cudaMemsetAsync(sc, 0, 256, s) != cudaSuccess) return BFSC_ERR_CUDA;
     int grid = (int)((words + 255) / 256);
     if (grid > dev.sms * 8) grid = dev.sms * 8;
     if (grid < 1) grid = 1;
-    k_vb_count<<<grid, 256, 0, s>>>(d_bitmap, n_bits, sc);
-    k_vb_select<<<grid, 256, 0, s>>>(d_bitmap, n_bits, wb, wb_bytes / 4, sc);      // (every word of the copy: the encode kernels read whole 16-byte chunks)
-    __atomic_fetch_add(&g_launches, 2ull, __ATOMIC_RELAXED);
-    if (cudaGetLastError() != cudaSuccess) return BFSC_ERR_CUDA;
+    // per-CTA popcounts: at the start of the bitmap-encode workspace, which nothing uses before k_vb_select has read them
+    unsigned long long* partial = reinterpret_cast<unsigned long long*>(ws_bm);
+    if ((size_t)grid * 8 > workspace_bytes - 256 - wb_bytes) return BFSC_ERR_INVALID_ARG;
+    BFSC_LAUNCH(launch_dep_v(k_vb_count, grid, 256, 0, s, d_bitmap, (unsigned long long)n_bits, partial));
+    BFSC_LAUNCH(launch_dep_v(k_vb_select, grid, 256, 0, s, d_bitmap, (unsigned long long)n_bits, wb, (unsigned long long)(wb_bytes / 4), sc,
+                           (const unsigned long long*)partial, grid));      // (every word of the copy: the encode kernels read whole 16-byte chunks)
     const bfsc_status rc = bfsc_compress_bitmap(codec, wb, n_bits, 0, BFSC_U32, 0, static_cast<unsigned char*>(d_out) + 32, raw_bytes,
                                                 reinterpret_cast<uint64_t*>(&sc->stream_bytes), ws_bm, workspace_bytes - 256 - wb_bytes, &sc->status, cuda_stream);
     if (rc != BFSC_OK) return rc;
-    k_vb_finish<<<grid, 256, 0, s>>>(d_bitmap, n_bits, static_cast<unsigned char*>(d_out), raw_bytes, sc, (unsigned long long*)d_out_bytes);
-    __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED);
-    return cudaGetLastError() == cudaSuccess ? BFSC_OK : BFSC_ERR_CUDA;
+    BFSC_LAUNCH(launch_dep_v(k_vb_finish, grid, 256, 0, s, d_bitmap, (unsigned long long)n_bits, static_cast<unsigned char*>(d_out),
+                           (unsigned long long)raw_bytes, (const VbScratch*)sc, (unsigned long long*)d_out_bytes));
+    return BFSC_OK;
 }
 
 extern "C" bfsc_status bfsc_compress(const void* d_ids, size_t n_ids, bfsc_dtype t, size_t raw_threshold_bytes,
