@@ -544,6 +544,22 @@ def run_ours(args, rank, local_rank, world):
                   "note": "algorithmic bytes = bitmap + stream (the ID list is never materialised); the decode ORs into a bitmap that "
                           "already holds the bits after the first pass (same work: one atomic OR per touched word group)"}
         del bms, bm_back, bm, ws_bm, ws_d
+        # a late-BFS VISITED bitmap through the container of FORMAT.md §10 (bfsc_compress_vbitmap / bfsc_decompress_vbitmap): 2^25
+        # vertices, 98 % visited, the unvisited ones in runs of 16 — the clear bits are listed
+        vb_bits = 1 << 25
+        vb_bm = ~streams.frontier_bitmap(vb_bits, 0.02, seed=3, run=16).to(dev)
+        vb_in = [vb_bm.clone() for _ in range(kC)]
+        vb_cap = B.vbitmap_bound(vb_bits)
+        vb_out = [torch.empty(vb_cap, dtype=torch.uint8, device=dev) for _ in range(kC)]
+        vb_back = [torch.zeros_like(vb_bm) for _ in range(kC)]
+        vb_ws = torch.empty(B.vbitmap_workspace_bytes(vb_bits), dtype=torch.uint8, device=dev)
+        vb_nb = torch.zeros(1, dtype=torch.int64, device=dev)
+        vb_enc = float(np.median([run_bm(lambda c: B.compress_vbitmap(B.CODEC_PFOR, vb_in[c], vb_bits, vb_out[c], vb_nb, vb_ws, status)) for _ in range(3)]))
+        vb_dec = float(np.median([run_bm(lambda c: B.decompress_vbitmap(vb_out[c], vb_cap, vb_back[c], vb_bits, vb_ws, status)) for _ in range(3)]))
+        assert int(status.item()) == 0 and torch.equal(vb_back[kC - 1], vb_bm), "visited bitmap: decode != input"
+        bitmap["visited"] = {"workload": f"{vb_bits} vertices, 98 % visited, unvisited in runs of 16", "bitmap_bytes": vb_bits // 8,
+                             "container_bytes": int(vb_nb.item()), "kind": int(vb_out[0][6].item()), "encode_ms": vb_enc, "decode_ms": vb_dec}
+        del vb_in, vb_out, vb_back, vb_ws
 
     # ---- end to end through the host-buffer C-ABI calls (pinned host memory) ----
     e2e = None
