@@ -66,7 +66,7 @@ __host__ inline size_t ws_bytes_for(size_t n_ids_total, size_t n_buf) {
 
 // bfsc_compress_bitmap: behind the standard workspace of one stream of n_bits IDs — the set bits before every super-chunk of
 // 32 x 1024 bits (u64, + the total) and, inside its super-chunk, before every chunk (u32)
-__host__ inline size_t bitmap_list_ids(size_t n_bits) { return n_bits / 32 + 128; }      // IDs the sparse path's list holds (used up to one set bit in 32)
+__host__ inline size_t bitmap_list_ids(size_t n_bits) { return n_bits / 16 + 128; }      // IDs the sparse path's list holds (used up to one set bit in 16)
 __host__ inline size_t bitmap_extra_ws_bytes(size_t n_bits) {
     const size_t n_super = (n_bits + 32767) / 32768;
     return align_up(8 * (n_super + 1) + 4 * 32 * n_super + 16, 16) + 8 * bitmap_list_ids(n_bits);   // (the list: 8 bytes per ID, either width)
