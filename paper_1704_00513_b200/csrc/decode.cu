@@ -1092,7 +1092,7 @@ __global__ void __launch_bounds__(256) k_vb_end(const uint32_t* __restrict__ wb,
 extern "C" bfsc_status bfsc_decompress_vbitmap(const void* d_in, size_t in_bytes, uint32_t* d_bitmap, size_t n_bits,
                                                void* d_workspace, size_t workspace_bytes, uint32_t* d_status, void* cuda_stream) {
     using namespace bfsc;
-    if (!d_in || !d_workspace || !d_status || (n_bits && !d_bitmap) || (unsigned long long)n_bits > (1ull << 32)) return BFSC_ERR_INVALID_ARG;
+    if (!d_in || !d_workspace || (n_bits && !d_bitmap) || (unsigned long long)n_bits > (1ull << 32)) return BFSC_ERR_INVALID_ARG;
     if (((uintptr_t)d_in & 15) || ((uintptr_t)d_workspace & 15) || ((uintptr_t)d_bitmap & 3)) return BFSC_ERR_INVALID_ARG;
     if (workspace_bytes < bfsc_vbitmap_workspace_bytes(n_bits)) return BFSC_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
