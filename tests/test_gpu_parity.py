@@ -397,6 +397,21 @@ def test_chained_decode_plan(B, oracle_mod, W):
     B.decompress_batch(d_in, d_off, n_buf, W, small, id_off, ws, status)
     torch.cuda.synchronize()
     assert int(status.item()) == B.ERR_DST_TOO_SMALL and bool((small == -1).all()) and not bool(id_off.any())
+    # two such calls at the same time on two streams (own workspaces and outputs; the plans' CTAs interleave on the device)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    ws_b = torch.empty_like(ws)
+    back_b = torch.full_like(back, -1)
+    id_off_b = torch.zeros_like(id_off)
+    status.zero_()
+    torch.cuda.synchronize()
+    for rep in range(20):
+        with torch.cuda.stream(s1):
+            B.decompress_batch(d_in, d_off, n_buf, W, back, id_off, ws, status)
+        with torch.cuda.stream(s2):
+            B.decompress_batch(d_in, d_off, n_buf, W, back_b, id_off_b, ws_b, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and torch.equal(back[:n].cpu(), ids) and torch.equal(back_b[:n].cpu(), ids)
+    assert torch.equal(id_off.cpu(), off) and torch.equal(id_off_b.cpu(), off)
     # the same streams into frontier bitmaps (the bitmap sink behind the same plan)
     lo = int(_np(ids, W).min())
     n_bits = int(_np(ids, W).max()) - lo + 1
