@@ -947,22 +947,28 @@ __global__ void __launch_bounds__(256) k_enc_streams(EncArgs a) {
     // byte offset of stream i = fixed_prefix[i] + 16 * (scan value at its first block q). The block belongs to
     // stream i itself when the stream has blocks (q_next > q: no search, one load less in the chain), else to
     // the next stream that has some.
-    auto stream_at = [&](uint32_t i, unsigned long long q, unsigned long long q_next) -> unsigned long long {
+    // ss_i / fp_i: stream_start[i] and fixed_prefix[i], requested by the caller together with the block counts (a stream
+    // with blocks — the usual case — then needs no further load: one round trip per buffer instead of three)
+    auto stream_at = [&](uint32_t i, unsigned long long q, unsigned long long q_next, unsigned long long ss_i, unsigned long long fp_i) -> unsigned long long {
         unsigned long long bb = grand16;
         if (q < total_blocks) {
-            const uint32_t j = q_next > q ? i
-                               : (a.in_off ? find_buf_from(a.ws.blk_first, a.n_buf, q, group_hint(a.ws.tile_state, q)) : 0u);
-            bb = (a.ws.stream_start[j] - 1 - a.ws.fixed_prefix[j]) >> 4;
+            if (q_next > q) bb = (ss_i - 1 - fp_i) >> 4;
+            else {
+                const uint32_t j = a.in_off ? find_buf_from(a.ws.blk_first, a.n_buf, q, group_hint(a.ws.tile_state, q)) : 0u;
+                bb = (a.ws.stream_start[j] - 1 - a.ws.fixed_prefix[j]) >> 4;
+            }
         }
-        return a.ws.fixed_prefix[i] + 16ull * bb;
+        return fp_i + 16ull * bb;
     };
     const int lane = threadIdx.x & 31, warps = blockDim.x >> 5;
     for (uint32_t i = blockIdx.x * warps + (threadIdx.x >> 5); i < a.n_buf; i += gridDim.x * warps) {   // warp = buffer
         const unsigned long long f0 = a.ws.blk_first[i], f1 = a.ws.blk_first[i + 1];
         const unsigned long long f2 = (i + 1 < a.n_buf) ? a.ws.blk_first[i + 2] : f1;
+        const unsigned long long ss0 = a.ws.stream_start[i], ss1 = a.ws.stream_start[i + 1];
+        const unsigned long long fp0 = a.ws.fixed_prefix[i], fp1 = a.ws.fixed_prefix[i + 1];
         if (!ok) { if (lane == 0) { if (a.out_off) a.out_off[i] = 0; if (a.out_sizes) a.out_sizes[i] = 0; } continue; }
-        const unsigned long long s0 = stream_at(i, f0, f1);
-        const unsigned long long s1 = (i + 1 < a.n_buf) ? stream_at(i + 1, f1, f2) : a.ws.hdr->total_out;
+        const unsigned long long s0 = stream_at(i, f0, f1, ss0, fp0);
+        const unsigned long long s1 = (i + 1 < a.n_buf) ? stream_at(i + 1, f1, f2, ss1, fp1) : a.ws.hdr->total_out;
         const unsigned long long n = buf_count(a, i), total = s1 - s0;
         const bool raw = n * E < a.thr;
         unsigned char* s = a.out + s0;
