@@ -532,6 +532,7 @@ struct BlockAt {                       // where the quad's block is
 // kSelf (small batches: up to kSelfMaxStreams streams, kSelfMaxBlocks blocks): the whole call in ONE launch — every CTA
 // runs D0 for itself (dec_plan_scan, tables in shared memory) instead of reading what a plan kernel left in the workspace.
 constexpr uint32_t kSelfMaxStreams = 1024, kSelfMaxBlocks = 2048;
+constexpr uint32_t kSelfFewStreams = 64, kSelfFewBlocks = 32768;   // a few long streams: kSelf up to so many blocks (no plan launch, no block table: 8 x 2^18 u32 IDs 10.3 -> 7.2 us per call; from ~10^5 blocks on the block table's single lookup per block wins: 64 x 220 K u64 IDs 37.3 / 40.7)
 template <int W, bool kBatch, bool kTma, bool kBits = false, bool kSelf = false>   // kBatch: a.in_off != nullptr; kBits: bits into a.sink instead of IDs into a.ids
 __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kCtasPerSm) k_dec_tiles(DecArgs a) {
     static_assert(!kSelf || (kBatch && !kTma), "kSelf: batch calls");
@@ -636,6 +637,7 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         lo16_1 = (32ull + ((4ull * (nb + 1) + 15ull) & ~15ull)) >> 4;
     }
 
+    uint32_t self_hint = 0;                                                // kSelf: the stream of this lane's last block
     auto locate = [&](unsigned long long g) -> BlockAt<W> {
         BlockAt<W> r; r.blk = nullptr; r.x = nullptr; r.span16 = 0; r.m = 0;
         if (g >= total_blocks) return r;
@@ -644,11 +646,16 @@ __global__ void __launch_bounds__(DecCfg<W, kTma>::kThreads, DecCfg<W, kTma>::kC
         int m;
         unsigned long long xi;
         if constexpr (kSelf) {                                             // the CTA's own tables
-            uint32_t lo = 0, hi = a.n_buf;                                 // the last i with s_first[i] <= g
+            // the last i with s_first[i] <= g, searched from the stream of this lane's previous block (a warp's batches
+            // ascend): gallop, then bisect — a level of a few long streams finds its stream with two reads
+            uint32_t lo = s_first[self_hint] <= (uint32_t)g ? self_hint : 0u, step = 1;
+            while (lo + step < a.n_buf && s_first[lo + step] <= (uint32_t)g) { lo += step; step <<= 1; }
+            uint32_t hi = min(lo + step, a.n_buf);
             while (hi - lo > 1) {
                 const uint32_t mid = (lo + hi) >> 1;
                 if (s_first[mid] <= (uint32_t)g) lo = mid; else hi = mid;
             }
+            self_hint = lo;
             s = a.in + a.in_off[lo];
             k = g - s_first[lo]; id0 = s_idpre[lo]; n = s_idpre[lo + 1] - id0; total16 = s_tot16[lo];
             m = (int)min((unsigned long long)kBlk, n - kBlk * k);
@@ -889,7 +896,7 @@ static bfsc_status launch_decode(const DecArgs& a_in, size_t max_blocks, cudaStr
     int grid = want < (size_t)max_grid ? (int)want : max_grid;
     if (grid < 1) grid = 1;
     const bool bits = a.sink.bm != nullptr;                                        // IDs -> bits of a frontier bitmap
-    if (a.in_off && a.n_buf <= kSelfMaxStreams && max_blocks <= kSelfMaxBlocks) {
+    if (a.in_off && a.n_buf <= kSelfMaxStreams && (max_blocks <= kSelfMaxBlocks || (a.n_buf <= kSelfFewStreams && max_blocks <= kSelfFewBlocks))) {
         // a small batch (both bounds known on the host: stream count, and blocks by the ID capacity / the workspace size):
         // one launch, no plan kernel
         const int psm = bits ? dec_ctas_per_sm<W, true, false, true, true>(dev.device) : dec_ctas_per_sm<W, true, false, false, true>(dev.device);
