@@ -1,7 +1,12 @@
 // decode.cu — bfsc_decompress / bfsc_decompress_batch (steps D0-D5).
 //
-// Launches per call: single stream: k_dec_tiles alone (it parses the stream header itself);
-// batch: [k_dec_headers ->] k_dec_plan -> k_dec_blocks -> k_dec_tiles, chained with programmatic dependent launch.
+// Launches per call, chained with programmatic dependent launch:
+//   single stream                                   k_dec_tiles alone (it parses the stream header itself)
+//   batch, small or of a few long streams           k_dec_tiles<..., kSelf> alone (every CTA plans for itself)
+//   batch of up to 8192 streams                     k_dec_planblocks (from 3072 streams: k_dec_planchain) -> k_dec_tiles
+//   larger batches                                  [k_dec_headers ->] k_dec_plan -> k_dec_blocks -> k_dec_tiles
+//   into bitmaps (FORMAT.md §9)                     the same kernels with the bitmap sink (single stream and batches up to 8192 streams)
+//   visited bitmap (FORMAT.md §10)                  k_vb_begin -> k_dec_tiles (bitmap sink, skipped for kind 0) -> k_vb_end
 #include <cstdlib>
 #include <atomic>
 #include <mutex>

@@ -6,6 +6,8 @@
 //   small batch             k_enc_small (one cluster; <= 1024 buffers, <= 2048 blocks by the workspace size)
 //   batch                   k_enc_planblocks (<= 8192 buffers; else k_enc_plan -> k_enc_blocks) -> k_enc_tiles<W, 1> -> k_enc_streams
 //   frontier bitmap         k_bm_count -> k_bm_plan -> k_bm_starts (block starts; sparse bitmaps: the ID list instead) -> k_enc_tiles<W, 2> -> k_bm_finish
+//   batch, scattered        as `batch` / `small batch` with k_enc_tiles<W, 3>: every stream to its own destination address (bfsc_compress_batch_scatter)
+//   visited bitmap          k_vb_count -> k_vb_select -> the frontier-bitmap chain on the selected copy -> k_vb_finish (FORMAT.md §10)
 #include <mutex>
 
 #include "bitmap_stage.cuh"
